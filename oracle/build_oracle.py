@@ -1,0 +1,22 @@
+"""Build the CPU oracle (test infrastructure) into oracle/libsfd_oracle.so with g++.
+
+Called by __graft_entry__.build(), tests/conftest.py and bench.py's cpu_baseline leg.
+Building the checker is not using it: nothing under paper_2304_06340_b200/ links or loads it.
+"""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "sfd_oracle.cpp")
+LIB = os.path.join(HERE, "libsfd_oracle.so")
+CMD = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", SRC, "-o", LIB]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
+        subprocess.run(CMD, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))

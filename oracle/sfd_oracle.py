@@ -1,0 +1,134 @@
+"""numpy/ctypes face of the CPU oracle (oracle/sfd_oracle.cpp).  TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import
+this module.  It never imports paper_2304_06340_b200 and the CUDA path never imports it.
+Every function is a marshalling shim: all arithmetic is in sfd_oracle.cpp.
+"""
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+import build_oracle  # noqa: E402
+
+_lib = C.CDLL(build_oracle.build())
+
+_dp = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_ip = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+_i64 = C.c_int64
+
+_lib.orc_mesh_sizes.argtypes = [C.c_int, C.POINTER(_i64), C.POINTER(_i64)]
+_lib.orc_mesh_icosphere.argtypes = [C.c_int, _dp, _ip]
+_lib.orc_subdivide.argtypes = [_dp, _i64, _ip, _i64, _dp, _ip]
+_lib.orc_subdivide.restype = _i64
+_lib.orc_rule.argtypes = [C.c_int, _dp, _dp]
+_lib.orc_nodes.argtypes = [_dp, _i64, _ip, _i64, C.c_int, _dp, _dp]
+_lib.orc_gauss_legendre.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
+_lib.orc_freq_nodes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _dp, _dp]
+_lib.orc_direct_sum.argtypes = [_dp, _dp, _i64, _dp, _i64, _dp]
+_lib.orc_sigma_hat.argtypes = [C.c_double]
+_lib.orc_sigma_hat.restype = C.c_double
+_lib.orc_reduce.argtypes = [_dp, _dp, _dp, _i64, C.c_double]
+_lib.orc_reduce.restype = C.c_double
+_lib.orc_weak_distance.argtypes = [_dp, _i64, _ip, _i64, C.c_int, C.c_double, C.c_double, C.c_int,
+                                   C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+_lib.orc_num_threads.restype = C.c_int
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise ValueError(f"oracle {what} failed with status {rc}")
+
+
+def mesh_sizes(level):
+    nv, nf = _i64(), _i64()
+    _lib.orc_mesh_sizes(level, C.byref(nv), C.byref(nf))
+    return nv.value, nf.value
+
+
+def mesh_icosphere(level):
+    nv, nf = mesh_sizes(level)
+    V = np.empty((nv, 3), np.float64)
+    F = np.empty((nf, 3), np.int32)
+    _chk(_lib.orc_mesh_icosphere(level, V, F), "mesh_icosphere")
+    return V, F
+
+
+def subdivide(V, F):
+    V = np.ascontiguousarray(V, np.float64)
+    F = np.ascontiguousarray(F, np.int32)
+    nv, nf = len(V), len(F)
+    Vo = np.empty((nv + 3 * nf // 2, 3), np.float64)
+    Fo = np.empty((4 * nf, 3), np.int32)
+    e = _lib.orc_subdivide(V, nv, F, nf, Vo, Fo)
+    assert e == 3 * nf // 2, "not a closed manifold mesh"
+    return Vo, Fo
+
+
+def rule(q):
+    lam = np.empty((q, 3), np.float64)
+    om = np.empty(q, np.float64)
+    if _lib.orc_rule(q, lam, om) != q:
+        raise ValueError(f"unknown rule {q}")
+    return lam, om
+
+
+def nodes(V, F, q):
+    V = np.ascontiguousarray(V, np.float64)
+    F = np.ascontiguousarray(F, np.int32)
+    x = np.empty((len(F) * q, 3), np.float64)
+    w = np.empty(len(F) * q, np.float64)
+    _chk(_lib.orc_nodes(V, len(V), F, len(F), q, x, w), "nodes")
+    return x, w
+
+
+def gauss_legendre(n, a=-1.0, b=1.0):
+    x = np.empty(n, np.float64)
+    w = np.empty(n, np.float64)
+    _chk(_lib.orc_gauss_legendre(n, a, b, x, w), "gauss_legendre")
+    return x, w
+
+
+def freq_nodes(n_r, n_th, n_ph, R):
+    K = n_r * n_th * n_ph
+    xi = np.empty((K, 3), np.float64)
+    W = np.empty(K, np.float64)
+    _chk(_lib.orc_freq_nodes(n_r, n_th, n_ph, R, xi, W), "freq_nodes")
+    return xi, W
+
+
+def direct_sum(x, w, xi):
+    """nuhat_k = sum_j w_j exp(-i xi_k . x_j) as complex128[K]."""
+    x = np.ascontiguousarray(x, np.float64).reshape(-1, 3)
+    w = np.ascontiguousarray(w, np.float64).reshape(-1)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    out = np.empty((len(xi), 2), np.float64)
+    _chk(_lib.orc_direct_sum(x, w, len(w), xi, len(xi), out), "direct_sum")
+    return out.view(np.complex128).reshape(-1)
+
+
+def sigma_hat(r):
+    return _lib.orc_sigma_hat(float(r))
+
+
+def reduce(nuhat, xi, W, s):
+    """I = (2 pi)^-3 sum_k W_k |nuhat_k - sigmahat|^2 (1+|xi_k|^2)^-s."""
+    nu = np.ascontiguousarray(nuhat, np.complex128).view(np.float64).reshape(-1, 2)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    W = np.ascontiguousarray(W, np.float64).reshape(-1)
+    return _lib.orc_reduce(nu, xi, W, len(W), float(s))
+
+
+def weak_distance(V, F, q, s, R, n_r, n_th, n_ph):
+    V = np.ascontiguousarray(V, np.float64)
+    F = np.ascontiguousarray(F, np.int32)
+    d, i = C.c_double(), C.c_double()
+    _chk(_lib.orc_weak_distance(V, len(V), F, len(F), q, s, R, n_r, n_th, n_ph, C.byref(d), C.byref(i)),
+         "weak_distance")
+    return d.value, i.value
+
+
+def num_threads():
+    return _lib.orc_num_threads()
