@@ -1,0 +1,140 @@
+/* sfd.h -- C ABI of the surface-Fourier-distance library (hand-written CUDA for sm_100a, one GPU).
+ *
+ * The hot path of Koga, "Computing weak distance between the 2-sphere and its nonsmooth
+ * approximations" (arXiv 2304.06340).  "P:n" = /root/reference/PAPER.md line n.  The variant is the
+ * one BASELINE.json fixes: Fourier kernel e^{-i xi.x}, Sobolev weight
+ * (1+|xi|^2)^{-s} with s > 1/2, ball-shaped frequency quadrature, symmetric triangle rules.
+ *
+ * Conventions for every function
+ *   - extern "C"; returns an int status: SFD_OK (0) or a negative sfd_status; never throws/aborts.
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  All buffers are owned by
+ *     the caller; the library keeps no pointer after the call returns except for work already
+ *     enqueued on `stream`.  Outputs are fully overwritten, never accumulated into.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
+ *     calls only enqueue work unless the description says "synchronises".
+ *   - Every call that needs scratch memory has a *_workspace query; d_work must be 256-byte aligned.
+ *   - Arrays are C-contiguous fp64 / int32: points double[n][3], complex values double[n][2] = (re,im).
+ *   - NULL pointer where one is required -> SFD_ERR_NULL; out-of-range scalar -> SFD_ERR_INVALID_ARG;
+ *     n == 0 (no faces / sources / targets) is valid and yields empty or zero output.
+ *   - sfd_last_error() returns a thread-local, human-readable description of the last failure.
+ *   - Process-global state: a small cache of cuFFT plans keyed by grid shape (sfd_release_cache()).
+ */
+#ifndef SFD_H_
+#define SFD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SFD_OK = 0,
+  SFD_ERR_NULL = -1,
+  SFD_ERR_INVALID_ARG = -2,
+  SFD_ERR_BUFFER_TOO_SMALL = -3,
+  SFD_ERR_WORKSPACE_TOO_SMALL = -4,
+  SFD_ERR_CUDA = -5,
+  SFD_ERR_CUFFT = -6,
+  SFD_ERR_UNSUPPORTED = -7
+} sfd_status;
+
+/* Symmetric triangle quadrature rules ("more symmetric rules are available on triangles");
+ * the value is the number of nodes q per face. */
+typedef enum { SFD_RULE_SYM6_DEG4 = 6, SFD_RULE_SYM12_DEG6 = 12 } sfd_rule;
+
+/* Ball-shaped frequency quadrature: n_r-point Gauss-Legendre in r on [0,R] x n_theta-point
+ * Gauss-Legendre in mu = cos(theta) on [-1,1] x n_phi-point periodic trapezoid in phi.
+ * K = n_r*n_theta*n_phi nodes, index k = (a*n_theta + b)*n_phi + c (phi fastest, mu ascending),
+ * xi_k = r_a (sqrt(1-mu_b^2) cos phi_c, sqrt(1-mu_b^2) sin phi_c, mu_b), phi_c = 2 pi c / n_phi,
+ * W_k = w^r_a r_a^2 w^mu_b 2 pi / n_phi. */
+typedef struct { int32_t n_r, n_theta, n_phi; } sfd_freq_quadrature;
+
+typedef void* sfd_stream; /* cudaStream_t */
+
+const char* sfd_last_error(void);
+/* Library version string and the CUDA arch it was compiled for ("sm_100a"). */
+const char* sfd_version(void);
+/* Drops cached cuFFT plans.  Synchronises the device. */
+int sfd_release_cache(void);
+
+/* ---- A1/A2: icosahedral discretization T_level ------------------------------------
+ * T_0 = icosahedron inscribed in S^2; each step adds the midpoint of every edge, projected onto
+ * S^2, and splits each face into four.  nV = 10*4^level + 2, nF = 20*4^level.
+ * Vertex/face numbering is the convention of DESIGN.md reading R4 (integer output is unique).
+ * level in [0,10], else SFD_ERR_INVALID_ARG.  Any of nV, nF, work_bytes may be NULL. */
+int sfd_mesh_icosphere_sizes(int level, int64_t* nV, int64_t* nF, size_t* work_bytes);
+int sfd_mesh_icosphere(int level, double* d_vertices /*[nV][3]*/, int32_t* d_faces /*[nF][3]*/,
+                       void* d_work, size_t work_bytes, sfd_stream stream);
+
+/* ---- A3: triangle-quadrature atoms (eqs. 3.1-3.2) -----------------------------------
+ * Converts the rule {(u_i,q_i)} on the standard simplex into {(L(u_i), q_i*gamma_A)} on each face:
+ * x[f*q+i] = sum_m lambda_{i,m} p_m(f),  w[f*q+i] = omega_i * area(f).  Degenerate faces give zero
+ * weights.  A face index outside [0,nV) makes the face contribute NaN nodes (not checked on host). */
+int sfd_nodes(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
+              double* d_x /*[nF*q][3]*/, double* d_w /*[nF*q]*/, sfd_stream stream);
+/* The rule itself (host): barycentric points h_lambda[q][3] and weights h_omega[q] summing to 1. */
+int sfd_rule_table(int rule, double* h_lambda, double* h_omega);
+
+/* ---- frequency quadrature (struct above) ------------------------------------------------
+ * Host version: deterministic, no GPU needed.  Device version: uploads the three 1-D tables and
+ * expands them with a kernel (d_xi [K][3], d_W [K]); n_r, n_theta, n_phi >= 1 and R > 0. */
+int sfd_freq_nodes(const sfd_freq_quadrature* q, double R, double* h_xi /*[K][3]*/, double* h_W /*[K]*/);
+int sfd_freq_nodes_workspace(const sfd_freq_quadrature* q, size_t* bytes);
+int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi /*[K][3]*/, double* d_W /*[K] or NULL*/,
+                          void* d_work, size_t work_bytes, sfd_stream stream);
+
+/* ---- A4/A5: Fourier transform of the atomic measure nu = sum_j w_j delta_{x_j} -----------------
+ * nuhat_k = sum_{j<J} w_j exp(-i xi_k . x_j)   (eq. 2.8 applied to the atoms of P:152).
+ *   eps == 0        : fp64 direct summation, error <= 1e-12 * sum|w_j| for |xi.x| <~ 2e3.
+ *   0 < eps < 1     : 3-D type-3 nonuniform FFT at tolerance eps (>= 1e-14), error
+ *                     <= 10 * eps * sum|w_j|.  Synchronises `stream` once (grid sizing).
+ * Workspace: query with the same (J, K, eps) and bounding half-widths X[d] >= max_j|x_jd - centre_d|,
+ * S[d] >= max_k|xi_kd - centre_d| (ignored for eps == 0, may then be NULL).  If the data's actual
+ * extents need more than work_bytes, the call fails with SFD_ERR_WORKSPACE_TOO_SMALL and writes
+ * nothing. */
+int sfd_surface_ft_workspace(int64_t J, int64_t K, const double X[3], const double S[3], double eps, size_t* bytes);
+int sfd_surface_ft(const double* d_x /*[J][3]*/, const double* d_w /*[J]*/, int64_t J,
+                   const double* d_xi /*[K][3]*/, int64_t K, double eps, double* d_nuhat /*[K][2]*/,
+                   void* d_work, size_t work_bytes, sfd_stream stream);
+
+/* ---- A6: fused target-side reduction (eq. 2.7 with P:55 eq. 2.5; eq. 2.14) ----------
+ * I = (2 pi)^-3 sum_k W_k |nuhat_k - sigmahat(xi_k)|^2 (1+|xi_k|^2)^-s,  sigmahat = 4 pi sin|xi|/|xi|
+ * (the unit sphere's transform).  Deterministic compensated fp64 sum.  s > 0.5, else
+ * SFD_ERR_INVALID_ARG.  Writes I to *h_I; synchronises `stream`.  Workspace: sfd_reduce_workspace. */
+int sfd_reduce_workspace(int64_t K, size_t* bytes);
+int sfd_reduce(const double* d_nuhat /*[K][2]*/, const double* d_xi /*[K][3]*/, const double* d_W /*[K]*/,
+               int64_t K, double s, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+
+/* ---- whole path: mesh -> atoms -> nuhat on the ball quadrature -> sqrt(I) -----------------------
+ * Distance in H^{-s} between the mesh's surface measure and the unit sphere's.  Runs A3,
+ * the frequency quadrature, A4 (eps == 0) or A5 (eps > 0) and A6 on `stream`; synchronises; writes
+ * sqrt(I) to *h_distance and I to *h_I (either may be NULL).  R > 0, s > 0.5.
+ * The workspace is sized for meshes whose bounding box has half-width <= x_extent on every axis (1.0 for an
+ * icosphere; only used when eps > 0); a wider mesh fails with SFD_ERR_WORKSPACE_TOO_SMALL. */
+int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps,
+                                double x_extent, size_t* bytes);
+int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
+                      double s, double R, const sfd_freq_quadrature* q, double eps, void* d_work,
+                      size_t work_bytes, sfd_stream stream, double* h_distance, double* h_I);
+
+/* ---- host-buffer entry points (end-to-end: allocate, copy in, run, copy out, free) -------------
+ * Same operations with HOST pointers; device memory comes from the stream-ordered CUDA pool of the
+ * current device.  Synchronise. */
+int sfd_surface_ft_host(const double* h_x, const double* h_w, int64_t J, const double* h_xi, int64_t K,
+                        double eps, double* h_nuhat);
+int sfd_weak_distance_host(const double* h_vertices, int64_t nV, const int32_t* h_faces, int64_t nF, int rule,
+                           double s, double R, const sfd_freq_quadrature* q, double eps,
+                           double* h_distance, double* h_I);
+
+/* ---- per-stage device timings of the last sfd_surface_ft / sfd_weak_distance call on this thread
+ * (only recorded after sfd_set_profiling(1); adds event records and a sync).  Names are static
+ * strings; returns the number of stages written (<= max). */
+int sfd_set_profiling(int on);
+int sfd_last_stage_times(const char** names, float* ms, int max);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFD_H_ */

@@ -1,0 +1,255 @@
+"""ctypes face of libsfd.so (include/sfd.h).  Argument marshalling only: torch supplies device memory and the
+current CUDA stream; every step of the path runs in the library's kernels.  There is no fallback: if the
+library is not built (`python -m paper_2304_06340_b200.build`) importing this module raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libsfd.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2304_06340_b200.build` "
+                      "(nvcc, sm_100a). There is no CPU fallback.")
+_lib = C.CDLL(LIB_PATH)
+
+SFD_OK = 0
+STATUS = {0: "SFD_OK", -1: "SFD_ERR_NULL", -2: "SFD_ERR_INVALID_ARG", -3: "SFD_ERR_BUFFER_TOO_SMALL",
+          -4: "SFD_ERR_WORKSPACE_TOO_SMALL", -5: "SFD_ERR_CUDA", -6: "SFD_ERR_CUFFT", -7: "SFD_ERR_UNSUPPORTED"}
+SFD_RULE_SYM6_DEG4, SFD_RULE_SYM12_DEG6 = 6, 12
+
+
+class sfd_freq_quadrature(C.Structure):
+    _fields_ = [("n_r", C.c_int32), ("n_theta", C.c_int32), ("n_phi", C.c_int32)]
+
+
+class SfdError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+_vp, _i64, _sz, _dbl = C.c_void_p, C.c_int64, C.c_size_t, C.c_double
+_P = C.POINTER
+_SIGS = {
+    "sfd_last_error": (C.c_char_p, []),
+    "sfd_version": (C.c_char_p, []),
+    "sfd_release_cache": (C.c_int, []),
+    "sfd_mesh_icosphere_sizes": (C.c_int, [C.c_int, _P(_i64), _P(_i64), _P(_sz)]),
+    "sfd_mesh_icosphere": (C.c_int, [C.c_int, _vp, _vp, _vp, _sz, _vp]),
+    "sfd_nodes": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _vp, _vp, _vp]),
+    "sfd_rule_table": (C.c_int, [C.c_int, _vp, _vp]),
+    "sfd_freq_nodes": (C.c_int, [_P(sfd_freq_quadrature), _dbl, _vp, _vp]),
+    "sfd_freq_nodes_workspace": (C.c_int, [_P(sfd_freq_quadrature), _P(_sz)]),
+    "sfd_freq_nodes_device": (C.c_int, [_P(sfd_freq_quadrature), _dbl, _vp, _vp, _vp, _sz, _vp]),
+    "sfd_surface_ft_workspace": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(_sz)]),
+    "sfd_surface_ft": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp, _vp, _sz, _vp]),
+    "sfd_reduce_workspace": (C.c_int, [_i64, _P(_sz)]),
+    "sfd_reduce": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
+    "sfd_weak_distance_workspace": (C.c_int, [_i64, C.c_int, _P(sfd_freq_quadrature), _dbl, _dbl, _dbl, _P(_sz)]),
+    "sfd_weak_distance": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl, _vp,
+                                    _sz, _vp, _P(_dbl), _P(_dbl)]),
+    "sfd_surface_ft_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp]),
+    "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
+                                         _P(_dbl), _P(_dbl)]),
+    "sfd_set_profiling": (C.c_int, [C.c_int]),
+    "sfd_last_stage_times": (C.c_int, [_P(C.c_char_p), _P(C.c_float), C.c_int]),
+}
+for _name, (_res, _args) in _SIGS.items():
+    _f = getattr(_lib, _name)
+    _f.restype, _f.argtypes = _res, _args
+EXPORTS = tuple(_SIGS)
+
+
+def _chk(rc):
+    if rc != SFD_OK:
+        raise SfdError(rc, _lib.sfd_last_error().decode())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _dev_f64(t, cols=None):
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), "need a contiguous CUDA float64 tensor"
+    if cols is not None:
+        assert t.dim() == 2 and t.shape[1] == cols
+    return t
+
+
+def _work(nbytes, device):
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def _quad(q):
+    return q if isinstance(q, sfd_freq_quadrature) else sfd_freq_quadrature(*[int(v) for v in q])
+
+
+def sfd_version():
+    return _lib.sfd_version().decode()
+
+
+def sfd_release_cache():
+    _chk(_lib.sfd_release_cache())
+
+
+def sfd_mesh_icosphere_sizes(level):
+    nv, nf, wb = _i64(), _i64(), _sz()
+    _chk(_lib.sfd_mesh_icosphere_sizes(int(level), C.byref(nv), C.byref(nf), C.byref(wb)))
+    return nv.value, nf.value, wb.value
+
+
+def sfd_mesh_icosphere(level, device="cuda"):
+    """T_level: vertices float64[nV,3], faces int32[nF,3] on `device`."""
+    nv, nf, wb = sfd_mesh_icosphere_sizes(level)
+    V = torch.empty((nv, 3), dtype=torch.float64, device=device)
+    F = torch.empty((nf, 3), dtype=torch.int32, device=device)
+    work = _work(wb, device)
+    _chk(_lib.sfd_mesh_icosphere(int(level), _ptr(V), _ptr(F), _ptr(work), work.numel(), _stream()))
+    return V, F
+
+
+def sfd_rule_table(rule):
+    lam = np.empty((rule, 3), np.float64)
+    om = np.empty(rule, np.float64)
+    _chk(_lib.sfd_rule_table(int(rule), lam.ctypes.data_as(_vp), om.ctypes.data_as(_vp)))
+    return lam, om
+
+
+def sfd_nodes(V, F, rule):
+    """Atoms (x_j, w_j) of the triangle rule on every face: x float64[nF*q,3], w float64[nF*q]."""
+    _dev_f64(V, 3)
+    assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous() and F.shape[1] == 3
+    J = F.shape[0] * int(rule)
+    x = torch.empty((J, 3), dtype=torch.float64, device=V.device)
+    w = torch.empty((J,), dtype=torch.float64, device=V.device)
+    _chk(_lib.sfd_nodes(_ptr(V), V.shape[0], _ptr(F), F.shape[0], int(rule), _ptr(x), _ptr(w), _stream()))
+    return x, w
+
+
+def sfd_freq_nodes(q, R):
+    """Host version of the ball quadrature: numpy xi[K,3], W[K]."""
+    q = _quad(q)
+    K = q.n_r * q.n_theta * q.n_phi
+    xi = np.empty((max(K, 0), 3), np.float64)
+    W = np.empty(max(K, 0), np.float64)
+    _chk(_lib.sfd_freq_nodes(C.byref(q), float(R), xi.ctypes.data_as(_vp), W.ctypes.data_as(_vp)))
+    return xi, W
+
+
+def sfd_freq_nodes_device(q, R, device="cuda"):
+    q = _quad(q)
+    wb = _sz()
+    _chk(_lib.sfd_freq_nodes_workspace(C.byref(q), C.byref(wb)))
+    K = q.n_r * q.n_theta * q.n_phi
+    xi = torch.empty((K, 3), dtype=torch.float64, device=device)
+    W = torch.empty((K,), dtype=torch.float64, device=device)
+    work = _work(wb.value, device)
+    _chk(_lib.sfd_freq_nodes_device(C.byref(q), float(R), _ptr(xi), _ptr(W), _ptr(work), work.numel(), _stream()))
+    return xi, W
+
+
+def sfd_surface_ft_workspace(J, K, X, S, eps):
+    wb = _sz()
+    Xa = (_dbl * 3)(*[float(v) for v in X]) if X is not None else None
+    Sa = (_dbl * 3)(*[float(v) for v in S]) if S is not None else None
+    _chk(_lib.sfd_surface_ft_workspace(int(J), int(K), Xa, Sa, float(eps), C.byref(wb)))
+    return wb.value
+
+
+def _half_widths(t):
+    if t.shape[0] == 0:
+        return [0.0, 0.0, 0.0]
+    return [float(v) * (1 + 1e-12) + 1e-300 for v in (0.5 * (t.amax(0) - t.amin(0))).tolist()]
+
+
+def sfd_surface_ft(x, w, xi, eps=0.0, work=None, out=None):
+    """nuhat_k = sum_j w_j exp(-i xi_k . x_j): complex128[K].  eps = 0 -> fp64 direct sum; eps > 0 -> type-3 NUFFT."""
+    _dev_f64(x, 3), _dev_f64(w), _dev_f64(xi, 3)
+    J, K = x.shape[0], xi.shape[0]
+    assert w.shape[0] == J
+    if work is None:
+        if eps > 0 and J > 0 and K > 0:
+            wb = sfd_surface_ft_workspace(J, K, _half_widths(x), _half_widths(xi), eps)
+        else:
+            wb = sfd_surface_ft_workspace(J, K, None, None, 0.0)
+        work = _work(wb, x.device)
+    nu = out if out is not None else torch.empty((K, 2), dtype=torch.float64, device=x.device)
+    _chk(_lib.sfd_surface_ft(_ptr(x), _ptr(w), J, _ptr(xi), K, float(eps), _ptr(nu), _ptr(work), work.numel(),
+                             _stream()))
+    return torch.view_as_complex(nu) if K > 0 else torch.empty(0, dtype=torch.complex128, device=x.device)
+
+
+def sfd_reduce(nuhat, xi, W, s):
+    """I = (2 pi)^-3 sum_k W_k |nuhat_k - sigmahat(xi_k)|^2 (1+|xi_k|^2)^-s (host float)."""
+    nu = torch.view_as_real(nuhat) if nuhat.is_complex() else nuhat
+    _dev_f64(nu, 2), _dev_f64(xi, 3), _dev_f64(W)
+    K = xi.shape[0]
+    wb = _sz()
+    _chk(_lib.sfd_reduce_workspace(K, C.byref(wb)))
+    work = _work(wb.value, xi.device)
+    I = _dbl()
+    _chk(_lib.sfd_reduce(_ptr(nu), _ptr(xi), _ptr(W), K, float(s), _ptr(work), work.numel(), _stream(), C.byref(I)))
+    return I.value
+
+
+def sfd_weak_distance_workspace(nF, rule, q, R, eps, x_extent=1.0):
+    q = _quad(q)
+    wb = _sz()
+    _chk(_lib.sfd_weak_distance_workspace(int(nF), int(rule), C.byref(q), float(R), float(eps), float(x_extent),
+                                          C.byref(wb)))
+    return wb.value
+
+
+def sfd_weak_distance(V, F, rule, s, R, q, eps=0.0, work=None, x_extent=None):
+    """(sqrt(I), I): the H^{-s} distance between the mesh's surface measure and the unit sphere's."""
+    _dev_f64(V, 3)
+    assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous()
+    q = _quad(q)
+    if work is None:
+        if x_extent is None:
+            x_extent = max(_half_widths(V)) if eps > 0 else 1.0
+        work = _work(sfd_weak_distance_workspace(F.shape[0], rule, q, R, eps, x_extent), V.device)
+    d, I = _dbl(), _dbl()
+    _chk(_lib.sfd_weak_distance(_ptr(V), V.shape[0], _ptr(F), F.shape[0], int(rule), float(s), float(R), C.byref(q),
+                                float(eps), _ptr(work), work.numel(), _stream(), C.byref(d), C.byref(I)))
+    return d.value, I.value
+
+
+def sfd_surface_ft_host(x, w, xi, eps=0.0):
+    """End-to-end call on HOST numpy buffers (copies in, runs, copies out)."""
+    x = np.ascontiguousarray(x, np.float64).reshape(-1, 3)
+    w = np.ascontiguousarray(w, np.float64).reshape(-1)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    nu = np.empty((len(xi), 2), np.float64)
+    _chk(_lib.sfd_surface_ft_host(x.ctypes.data_as(_vp), w.ctypes.data_as(_vp), len(w), xi.ctypes.data_as(_vp),
+                                  len(xi), float(eps), nu.ctypes.data_as(_vp)))
+    return nu.view(np.complex128).reshape(-1)
+
+
+def sfd_weak_distance_host(V, F, rule, s, R, q, eps=0.0):
+    V = np.ascontiguousarray(V, np.float64).reshape(-1, 3)
+    F = np.ascontiguousarray(F, np.int32).reshape(-1, 3)
+    q = _quad(q)
+    d, I = _dbl(), _dbl()
+    _chk(_lib.sfd_weak_distance_host(V.ctypes.data_as(_vp), len(V), F.ctypes.data_as(_vp), len(F), int(rule), float(s),
+                                     float(R), C.byref(q), float(eps), C.byref(d), C.byref(I)))
+    return d.value, I.value
+
+
+def sfd_set_profiling(on):
+    _chk(_lib.sfd_set_profiling(1 if on else 0))
+
+
+def sfd_last_stage_times():
+    names = (C.c_char_p * 32)()
+    ms = (C.c_float * 32)()
+    n = _lib.sfd_last_stage_times(names, ms, 32)
+    return [(names[i].decode(), float(ms[i])) for i in range(n)]

@@ -1,0 +1,407 @@
+// api.cu -- the C ABI of libsfd.so (include/sfd.h): argument checks, workspace carving, stage timing.  Every
+// step of the path runs in the kernels of mesh.cu / nodes.cu / direct.cu / nufft3.cu / reduce.cu; there is no CPU
+// fallback: without a CUDA device every compute call returns SFD_ERR_CUDA.
+#include <cmath>
+#include <cstring>
+
+#include "internal.cuh"
+
+namespace sfd {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int num_sms() {
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+      sms = n;
+    else
+      return 148;  // B200; not cached so that a later successful query wins
+  }
+  return sms;
+}
+
+// ---- stage timing ---------------------------------------------------------------------------------
+namespace {
+constexpr int kMaxStages = 32;
+struct Prof {
+  bool on = false, active = false;
+  int n = 0;
+  cudaEvent_t ev[kMaxStages + 1] = {};
+  const char* name[kMaxStages] = {};
+  float ms[kMaxStages] = {};
+  int n_done = 0;
+};
+thread_local Prof g_prof;
+}  // namespace
+
+void prof_begin(cudaStream_t st) {
+  Prof& p = g_prof;
+  if (!p.on) return;
+  p.n = 0;
+  p.active = true;
+  if (!p.ev[0]) cudaEventCreate(&p.ev[0]);
+  cudaEventRecord(p.ev[0], st);
+}
+void prof_mark(const char* name, cudaStream_t st) {
+  Prof& p = g_prof;
+  if (!p.on || !p.active || p.n >= kMaxStages) return;
+  p.name[p.n] = name;
+  ++p.n;
+  if (!p.ev[p.n]) cudaEventCreate(&p.ev[p.n]);
+  cudaEventRecord(p.ev[p.n], st);
+}
+void prof_end(cudaStream_t st) {
+  Prof& p = g_prof;
+  if (!p.on || !p.active) return;
+  p.active = false;
+  cudaStreamSynchronize(st);
+  for (int i = 0; i < p.n; ++i) cudaEventElapsedTime(&p.ms[i], p.ev[i], p.ev[i + 1]);
+  p.n_done = p.n;
+}
+
+namespace {
+inline cudaStream_t as_stream(sfd_stream s) { return static_cast<cudaStream_t>(s); }
+
+int check_quadrature(const sfd_freq_quadrature* q, double R) {
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  SFD_REQUIRE(q->n_r >= 1 && q->n_theta >= 1 && q->n_phi >= 1, SFD_ERR_INVALID_ARG,
+              "frequency quadrature sizes must be >= 1 (got %d,%d,%d)", q->n_r, q->n_theta, q->n_phi);
+  SFD_REQUIRE(R > 0.0 && std::isfinite(R), SFD_ERR_INVALID_ARG, "R must be positive and finite");
+  return SFD_OK;
+}
+int check_eps(double eps) {
+  SFD_REQUIRE(eps == 0.0 || (eps >= 1e-14 && eps < 1.0), SFD_ERR_INVALID_ARG,
+              "eps must be 0 (direct sum) or in [1e-14, 1), got %g", eps);
+  return SFD_OK;
+}
+}  // namespace
+}  // namespace sfd
+
+using namespace sfd;
+
+extern "C" {
+
+const char* sfd_last_error(void) { return g_err; }
+const char* sfd_version(void) { return "sfd 0.1 (sm_100a)"; }
+
+int sfd_release_cache(void) {
+  cudaDeviceSynchronize();
+  return nufft3_release_cache();
+}
+
+int sfd_set_profiling(int on) {
+  g_prof.on = on != 0;
+  g_prof.n_done = 0;
+  return SFD_OK;
+}
+int sfd_last_stage_times(const char** names, float* ms, int max) {
+  int n = g_prof.n_done < max ? g_prof.n_done : max;
+  for (int i = 0; i < n; ++i) {
+    if (names) names[i] = g_prof.name[i];
+    if (ms) ms[i] = g_prof.ms[i];
+  }
+  return n;
+}
+
+// ---- A1/A2 ----------------------------------------------------------------------------------------
+int sfd_mesh_icosphere_sizes(int level, int64_t* nV, int64_t* nF, size_t* work_bytes) {
+  return mesh_sizes(level, nV, nF, work_bytes);
+}
+int sfd_mesh_icosphere(int level, double* d_vertices, int32_t* d_faces, void* d_work, size_t work_bytes,
+                       sfd_stream stream) {
+  return mesh_icosphere(level, d_vertices, d_faces, d_work, work_bytes, as_stream(stream));
+}
+
+// ---- A3 -------------------------------------------------------------------------------------------
+int sfd_nodes(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double* d_x,
+              double* d_w, sfd_stream stream) {
+  return nodes(d_vertices, nV, d_faces, nF, rule, d_x, d_w, as_stream(stream));
+}
+int sfd_rule_table(int rule, double* h_lambda, double* h_omega) {
+  SFD_REQUIRE(h_lambda && h_omega, SFD_ERR_NULL, "sfd_rule_table: NULL output");
+  return rule_table_host(rule, h_lambda, h_omega);
+}
+
+// ---- frequency quadrature -------------------------------------------------------------------------
+int sfd_freq_nodes(const sfd_freq_quadrature* q, double R, double* h_xi, double* h_W) {
+  SFD_TRY(check_quadrature(q, R));
+  SFD_REQUIRE(h_xi && h_W, SFD_ERR_NULL, "sfd_freq_nodes: NULL output");
+  FreqTables t;
+  SFD_TRY(freq_tables(q, R, t));
+  for (int a = 0; a < q->n_r; ++a)
+    for (int b = 0; b < q->n_theta; ++b)
+      for (int c = 0; c < q->n_phi; ++c) {
+        const int64_t k = ((int64_t)a * q->n_theta + b) * q->n_phi + c;
+        // same roundings as freq_expand_kernel (each product rounds once)
+        volatile double sc = t.st[b] * t.cph[c], ss = t.st[b] * t.sph[c];
+        h_xi[3 * k + 0] = t.r[a] * sc;
+        h_xi[3 * k + 1] = t.r[a] * ss;
+        h_xi[3 * k + 2] = t.r[a] * t.mu[b];
+        volatile double m1 = t.wr[a] * t.r[a];
+        volatile double m2 = m1 * t.r[a];
+        volatile double m3 = m2 * t.wmu[b];
+        h_W[k] = m3 * t.wph;
+      }
+  return SFD_OK;
+}
+int sfd_freq_nodes_workspace(const sfd_freq_quadrature* q, size_t* bytes) {
+  SFD_REQUIRE(q && bytes, SFD_ERR_NULL, "sfd_freq_nodes_workspace: NULL argument");
+  SFD_TRY(check_quadrature(q, 1.0));
+  *bytes = freq_tables_bytes(q);
+  return SFD_OK;
+}
+int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi, double* d_W, void* d_work,
+                          size_t work_bytes, sfd_stream stream) {
+  SFD_TRY(check_quadrature(q, R));
+  SFD_REQUIRE(d_xi, SFD_ERR_NULL, "sfd_freq_nodes_device: NULL output");
+  FreqTables t;
+  SFD_TRY(freq_tables(q, R, t));
+  return freq_expand(q, t, d_xi, d_W, d_work, work_bytes, as_stream(stream));
+}
+
+// ---- A4/A5 ----------------------------------------------------------------------------------------
+int sfd_surface_ft_workspace(int64_t J, int64_t K, const double X[3], const double S[3], double eps, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_surface_ft_workspace: bytes is NULL");
+  SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
+  SFD_TRY(check_eps(eps));
+  if (eps == 0.0) {
+    *bytes = (J == 0 || K == 0) ? 0 : direct_plan(J, K).work_bytes;
+    return SFD_OK;
+  }
+  SFD_REQUIRE(X && S, SFD_ERR_NULL, "sfd_surface_ft_workspace: X and S are required when eps > 0");
+  Nufft3Sizes sz;
+  SFD_TRY(nufft3_sizes(J, K, X, S, eps, &sz));
+  *bytes = sz.work_bytes;
+  return SFD_OK;
+}
+
+int sfd_surface_ft(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
+                   double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+  SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
+  SFD_TRY(check_eps(eps));
+  if (K == 0) return SFD_OK;
+  SFD_REQUIRE(d_xi && d_nuhat, SFD_ERR_NULL, "sfd_surface_ft: NULL target buffer");
+  SFD_REQUIRE(J == 0 || (d_x && d_w), SFD_ERR_NULL, "sfd_surface_ft: NULL source buffer");
+  cudaStream_t st = as_stream(stream);
+  const bool own_prof = !g_prof.active;
+  if (own_prof) prof_begin(st);
+  int rc;
+  if (eps == 0.0 || J == 0) {
+    rc = direct_sum(d_x, d_w, J, d_xi, K, d_nuhat, d_work, work_bytes, st);
+    prof_mark("direct_sum", st);
+  } else {
+    rc = nufft3(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, st);
+  }
+  if (own_prof) prof_end(st);
+  return rc;
+}
+
+// ---- A6 -------------------------------------------------------------------------------------------
+int sfd_reduce_workspace(int64_t K, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_reduce_workspace: bytes is NULL");
+  SFD_REQUIRE(K >= 0, SFD_ERR_INVALID_ARG, "K must be >= 0");
+  *bytes = reduce_workspace(K);
+  return SFD_OK;
+}
+
+int sfd_reduce(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
+               size_t work_bytes, sfd_stream stream, double* h_I) {
+  SFD_REQUIRE(h_I, SFD_ERR_NULL, "sfd_reduce: h_I is NULL");
+  cudaStream_t st = as_stream(stream);
+  double* d_res = nullptr;
+  SFD_TRY(reduce_enqueue(d_nuhat, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res));
+  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  return SFD_OK;
+}
+
+// ---- whole path -----------------------------------------------------------------------------------
+namespace {
+struct DistLayout {
+  int64_t J, K;
+  size_t x, w, xi, W, nu, tab, red, ft, total;
+  size_t ft_bytes, tab_bytes, red_bytes;
+};
+int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps, double x_extent,
+                DistLayout* L) {
+  SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
+  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  SFD_TRY(check_quadrature(q, R));
+  SFD_TRY(check_eps(eps));
+  L->J = nF * rule;
+  L->K = (int64_t)q->n_r * q->n_theta * q->n_phi;
+  const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {R, R, R};
+  if (eps > 0.0) SFD_REQUIRE(x_extent > 0.0 && std::isfinite(x_extent), SFD_ERR_INVALID_ARG, "x_extent must be > 0");
+  SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, eps, &L->ft_bytes));
+  L->tab_bytes = freq_tables_bytes(q);
+  L->red_bytes = reduce_workspace(L->K);
+  size_t o = 0;
+  auto put = [&](size_t bytes) {
+    const size_t at = o;
+    o += align_up(bytes);
+    return at;
+  };
+  L->x = put((size_t)L->J * 24);
+  L->w = put((size_t)L->J * 8);
+  L->xi = put((size_t)L->K * 24);
+  L->W = put((size_t)L->K * 8);
+  L->nu = put((size_t)L->K * 16);
+  L->tab = put(L->tab_bytes);
+  L->red = put(L->red_bytes);
+  L->ft = put(L->ft_bytes);
+  L->total = o;
+  return SFD_OK;
+}
+}  // namespace
+
+int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps,
+                                double x_extent, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_weak_distance_workspace: bytes is NULL");
+  DistLayout L;
+  SFD_TRY(dist_layout(nF, rule, q, R, eps, x_extent, &L));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
+                      double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes,
+                      sfd_stream stream, double* h_distance, double* h_I) {
+  SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
+  SFD_REQUIRE(nF == 0 || (d_vertices && d_faces), SFD_ERR_NULL, "sfd_weak_distance: NULL mesh buffer");
+  DistLayout L;
+  // the workspace may have been sized with any x_extent: recompute the fixed part, give the rest to the transform
+  SFD_TRY(dist_layout(nF, rule, q, R, 0.0, 1.0, &L));
+  SFD_TRY(check_eps(eps));
+  SFD_REQUIRE(d_work && work_bytes >= L.ft, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "sfd_weak_distance needs at least %zu workspace bytes, got %zu", L.total, work_bytes);
+  cudaStream_t st = as_stream(stream);
+  char* base = static_cast<char*>(d_work);
+  double* x = reinterpret_cast<double*>(base + L.x);
+  double* w = reinterpret_cast<double*>(base + L.w);
+  double* xi = reinterpret_cast<double*>(base + L.xi);
+  double* W = reinterpret_cast<double*>(base + L.W);
+  double* nu = reinterpret_cast<double*>(base + L.nu);
+  prof_begin(st);
+  int rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
+  prof_mark("nodes", st);
+  FreqTables t;
+  if (rc == SFD_OK) rc = freq_tables(q, R, t);
+  if (rc == SFD_OK) rc = freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st);
+  prof_mark("freq_nodes", st);
+  if (rc == SFD_OK) rc = sfd_surface_ft(x, w, L.J, xi, L.K, eps, nu, base + L.ft, work_bytes - L.ft, stream);
+  double* d_res = nullptr;
+  if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, L.K, s, base + L.red, L.red_bytes, st, &d_res);
+  prof_mark("reduce", st);
+  double I = 0.0;
+  if (rc == SFD_OK) {
+    cudaError_t e = cudaMemcpyAsync(&I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+      set_error("sfd_weak_distance: %s", cudaGetErrorString(e));
+      rc = SFD_ERR_CUDA;
+    }
+  }
+  prof_end(st);
+  if (rc != SFD_OK) return rc;
+  if (h_I) *h_I = I;
+  if (h_distance) *h_distance = std::sqrt(I);
+  return SFD_OK;
+}
+
+// ---- host-buffer entry points -----------------------------------------------------------------------
+namespace {
+struct HostCall {
+  cudaStream_t st = nullptr;
+  void* bufs[8] = {};
+  int n = 0;
+  int open() {
+    SFD_CUDA_TRY(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    return SFD_OK;
+  }
+  int alloc(void** p, size_t bytes) {
+    *p = nullptr;
+    SFD_CUDA_TRY(cudaMallocAsync(p, bytes ? bytes : 256, st));
+    bufs[n++] = *p;
+    return SFD_OK;
+  }
+  ~HostCall() {
+    if (!st) return;
+    for (int i = 0; i < n; ++i) cudaFreeAsync(bufs[i], st);
+    cudaStreamSynchronize(st);
+    cudaStreamDestroy(st);
+  }
+};
+void half_widths(const double* p, int64_t n, double out[3]) {
+  for (int c = 0; c < 3; ++c) {
+    double lo = 0.0, hi = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+      const double v = p[3 * i + c];
+      if (i == 0 || v < lo) lo = v;
+      if (i == 0 || v > hi) hi = v;
+    }
+    out[c] = 0.5 * (hi - lo) * (1.0 + 1e-12) + 1e-300;
+  }
+}
+}  // namespace
+
+int sfd_surface_ft_host(const double* h_x, const double* h_w, int64_t J, const double* h_xi, int64_t K, double eps,
+                        double* h_nuhat) {
+  SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
+  SFD_TRY(check_eps(eps));
+  if (K == 0) return SFD_OK;
+  SFD_REQUIRE(h_xi && h_nuhat && (J == 0 || (h_x && h_w)), SFD_ERR_NULL, "sfd_surface_ft_host: NULL buffer");
+  size_t wb = 0;
+  double X[3], S[3];
+  half_widths(h_x, J, X);
+  half_widths(h_xi, K, S);
+  SFD_TRY(sfd_surface_ft_workspace(J, K, X, S, J == 0 ? 0.0 : eps, &wb));
+  HostCall hc;
+  SFD_TRY(hc.open());
+  void *dx, *dw, *dxi, *dnu, *dwork;
+  SFD_TRY(hc.alloc(&dx, (size_t)J * 24));
+  SFD_TRY(hc.alloc(&dw, (size_t)J * 8));
+  SFD_TRY(hc.alloc(&dxi, (size_t)K * 24));
+  SFD_TRY(hc.alloc(&dnu, (size_t)K * 16));
+  SFD_TRY(hc.alloc(&dwork, wb));
+  if (J > 0) {
+    SFD_CUDA_TRY(cudaMemcpyAsync(dx, h_x, (size_t)J * 24, cudaMemcpyHostToDevice, hc.st));
+    SFD_CUDA_TRY(cudaMemcpyAsync(dw, h_w, (size_t)J * 8, cudaMemcpyHostToDevice, hc.st));
+  }
+  SFD_CUDA_TRY(cudaMemcpyAsync(dxi, h_xi, (size_t)K * 24, cudaMemcpyHostToDevice, hc.st));
+  SFD_TRY(sfd_surface_ft((double*)dx, (double*)dw, J, (double*)dxi, K, eps, (double*)dnu, dwork, wb, hc.st));
+  SFD_CUDA_TRY(cudaMemcpyAsync(h_nuhat, dnu, (size_t)K * 16, cudaMemcpyDeviceToHost, hc.st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(hc.st));
+  return SFD_OK;
+}
+
+int sfd_weak_distance_host(const double* h_vertices, int64_t nV, const int32_t* h_faces, int64_t nF, int rule, double s,
+                           double R, const sfd_freq_quadrature* q, double eps, double* h_distance, double* h_I) {
+  SFD_REQUIRE(nV >= 0 && nF >= 0, SFD_ERR_INVALID_ARG, "negative mesh size");
+  SFD_REQUIRE(nF == 0 || (h_vertices && h_faces), SFD_ERR_NULL, "sfd_weak_distance_host: NULL mesh buffer");
+  double X[3];
+  half_widths(h_vertices, nV, X);
+  const double ext = std::fmax(X[0], std::fmax(X[1], X[2]));
+  size_t wb = 0;
+  SFD_TRY(sfd_weak_distance_workspace(nF, rule, q, R, eps, ext, &wb));
+  HostCall hc;
+  SFD_TRY(hc.open());
+  void *dV, *dF, *dwork;
+  SFD_TRY(hc.alloc(&dV, (size_t)nV * 24));
+  SFD_TRY(hc.alloc(&dF, (size_t)nF * 12));
+  SFD_TRY(hc.alloc(&dwork, wb));
+  if (nV > 0) SFD_CUDA_TRY(cudaMemcpyAsync(dV, h_vertices, (size_t)nV * 24, cudaMemcpyHostToDevice, hc.st));
+  if (nF > 0) SFD_CUDA_TRY(cudaMemcpyAsync(dF, h_faces, (size_t)nF * 12, cudaMemcpyHostToDevice, hc.st));
+  return sfd_weak_distance((double*)dV, nV, (int32_t*)dF, nF, rule, s, R, q, eps, dwork, wb, hc.st, h_distance, h_I);
+}
+
+}  // extern "C"

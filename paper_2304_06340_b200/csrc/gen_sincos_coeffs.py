@@ -1,0 +1,72 @@
+"""Derives the polynomial coefficients of sincos_fp64 (csrc/common.cuh) and checks them.
+
+    sin r = r + r z P(z),      P of degree 5 in z = r^2,  |r| <= pi/4 (+ a little slack)
+    cos r = 1 - z/2 + z^2 Q(z), Q of degree 5
+
+P and Q interpolate (sin(sqrt z)/sqrt z - 1)/z and (cos(sqrt z) - 1 + z/2)/z^2 at the Chebyshev
+nodes of [0, zmax] (near-minimax), in 60-digit arithmetic.  Run: python gen_sincos_coeffs.py
+The printed constants are pasted into common.cuh; the script then evaluates the fp64 Horner forms
+on 200k points against mpmath and prints the worst absolute error.
+"""
+import mpmath as mp
+import numpy as np
+
+mp.mp.dps = 60
+RMAX = mp.pi / 4 * mp.mpf("1.02")
+ZMAX = RMAX ** 2
+DEG = 5
+
+
+def f_sin(z):
+    if z == 0:
+        return -mp.mpf(1) / 6
+    r = mp.sqrt(z)
+    return (mp.sin(r) / r - 1) / z
+
+
+def f_cos(z):
+    if z == 0:
+        return mp.mpf(1) / 24
+    r = mp.sqrt(z)
+    return (mp.cos(r) - 1 + z / 2) / (z * z)
+
+
+def cheb_interp(f, deg):
+    n = deg + 1
+    zs = [ZMAX / 2 * (1 + mp.cos(mp.pi * (2 * i + 1) / (2 * n))) for i in range(n)]
+    A = mp.matrix(n, n)
+    b = mp.matrix(n, 1)
+    for i, z in enumerate(zs):
+        for j in range(n):
+            A[i, j] = z ** j
+        b[i] = f(z)
+    return list(mp.lu_solve(A, b))
+
+
+def main():
+    P = cheb_interp(f_sin, DEG)
+    Q = cheb_interp(f_cos, DEG)
+    print("// sin: S1..S6 (ascending powers of z)")
+    for c in P:
+        print("  %s," % mp.nstr(c, 21))
+    print("// cos: C1..C6 (ascending powers of z)")
+    for c in Q:
+        print("  %s," % mp.nstr(c, 21))
+    Pd = [float(c) for c in P]
+    Qd = [float(c) for c in Q]
+    r = np.linspace(-float(mp.pi / 4), float(mp.pi / 4), 200001)
+    z = r * r
+    ps = np.full_like(r, Pd[5])
+    pc = np.full_like(r, Qd[5])
+    for k in range(4, -1, -1):
+        ps = ps * z + Pd[k]
+        pc = pc * z + Qd[k]
+    s = r + (r * z) * ps
+    c = 1.0 + z * (z * pc - 0.5)
+    es = max(abs(mp.mpf(float(a)) - mp.sin(mp.mpf(float(b)))) for a, b in zip(s[::97], r[::97]))
+    ec = max(abs(mp.mpf(float(a)) - mp.cos(mp.mpf(float(b)))) for a, b in zip(c[::97], r[::97]))
+    print("max |sin err| = %s, max |cos err| = %s (fp64 Horner without FMA, sampled)" % (mp.nstr(es, 3), mp.nstr(ec, 3)))
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,57 @@
+// internal.cuh -- launcher interfaces between the translation units of libsfd.so (the CUDA path).
+// Every function returns an sfd_status and only enqueues work on `st` unless it says otherwise.
+#pragma once
+#include <vector>
+
+#include "common.cuh"
+#include "direct.cuh"
+
+namespace sfd {
+
+// ---- mesh.cu: A1/A2 icosahedral discretization --------------------------------------
+int mesh_sizes(int level, int64_t* nV, int64_t* nF, size_t* work_bytes);
+int mesh_icosphere(int level, double* d_V, int32_t* d_F, void* d_work, size_t work_bytes, cudaStream_t st);
+
+// ---- nodes.cu: A3 atoms and the ball-shaped frequency quadrature --------------
+struct FreqTables {
+  std::vector<double> r, wr;         // Gauss-Legendre on [0,R]
+  std::vector<double> mu, st, wmu;   // Gauss-Legendre in mu = cos(theta); st = sqrt(1-mu^2)
+  std::vector<double> cph, sph;      // cos/sin of phi_c = 2 pi c / n_phi
+  double wph;                        // 2 pi / n_phi
+};
+int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t);
+size_t freq_tables_bytes(const sfd_freq_quadrature* q);
+int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
+                size_t work_bytes, cudaStream_t st);
+int rule_table_host(int rule, double* lam, double* om);
+int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rule, double* d_x, double* d_w,
+          cudaStream_t st);
+
+// ---- scan.cu: exclusive prefix sum of int32 counts (used by the mesh ranks and the bin sorts) -----
+size_t scan_workspace(int64_t n);
+// out[i] = sum_{i'<i} in[i'] (in-place allowed); total (sum of all) is written to d_total if non-NULL.
+int exclusive_scan_i32(const int32_t* d_in, int32_t* d_out, int64_t n, int32_t* d_total, void* d_work,
+                       size_t work_bytes, cudaStream_t st);
+
+// ---- reduce.cu: A6 fused target-side reduction (eq. 2.7, eq. 2.14) --------------------
+size_t reduce_workspace(int64_t K);
+// Enqueues the reduction; the result (I, already scaled by (2 pi)^-3) lands in d_result[0] (device double,
+// inside the workspace: reduce_result_ptr).
+int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
+                   size_t work_bytes, cudaStream_t st, double** d_result);
+
+// ---- nufft3.cu: A5 three-dimensional type-3 nonuniform FFT -------------------------------
+struct Nufft3Sizes {
+  int w;               // kernel width in fine-grid cells
+  double beta;         // ES kernel parameter: phi(z) = exp(beta (sqrt(1-z^2) - 1))
+  int64_t nf[3];       // fine (spreading) grid
+  int64_t n2[3];       // inner type-2 grid (sigma2 * nf)
+  int64_t nout[3];     // kept part of the inner grid per axis (pruned FFT output)
+  size_t work_bytes;   // total workspace
+};
+int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out);
+int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
+           double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st);
+int nufft3_release_cache();
+
+}  // namespace sfd

@@ -1,0 +1,241 @@
+// nodes.cu -- A3: triangle-quadrature atoms (eqs. 3.1-3.2) and the ball-shaped frequency quadrature
+// of the CUDA path.  HBM-bound, one pass: 12 B + 72 B (cached) read and 32*q B written per face.
+#include <cmath>
+#include <vector>
+
+#include "internal.cuh"
+
+namespace sfd {
+namespace {
+
+// Symmetric rules in barycentric coordinates (weights sum to 1).  Orbit parameters solve the moment
+// equations of degree 4 (6 points) and 6 (12 points); tests/test_binding_cpu.py re-checks exactness through
+// sfd_rule_table.  Point order: DESIGN.md reading R6.
+struct RuleTable {
+  double lam[12][3];
+  double om[12];
+};
+__constant__ RuleTable c_rule[2];
+
+void orbit3(double a, double w, double lam[][3], double* om) {
+  const double b = 1.0 - 2.0 * a;
+  const double p[3][3] = {{a, a, b}, {a, b, a}, {b, a, a}};
+  for (int i = 0; i < 3; ++i) {
+    for (int c = 0; c < 3; ++c) lam[i][c] = p[i][c];
+    om[i] = w;
+  }
+}
+
+void fill_rule(int q, RuleTable& t) {
+  for (auto& r : t.lam) r[0] = r[1] = r[2] = 0.0;
+  for (auto& o : t.om) o = 0.0;
+  if (q == 6) {
+    orbit3(0.445948490915964886318329, 0.223381589678011465695007, t.lam, t.om);
+    orbit3(0.091576213509770743459571, 0.109951743655321867638326, t.lam + 3, t.om + 3);
+  } else {
+    orbit3(0.063089014491502228340332, 0.050844906370206816920937, t.lam, t.om);
+    orbit3(0.249286745170910421291639, 0.116786275726379366025290, t.lam + 3, t.om + 3);
+    const double a = 0.053145049844816947353250, b = 0.310352451033784405416608, c = 1.0 - a - b;
+    const double w = 0.082851075618373575193553;
+    const double p[6][3] = {{a, b, c}, {b, a, c}, {a, c, b}, {c, a, b}, {b, c, a}, {c, b, a}};
+    for (int i = 0; i < 6; ++i) {
+      for (int k = 0; k < 3; ++k) t.lam[6 + i][k] = p[i][k];
+      t.om[6 + i] = w;
+    }
+  }
+}
+
+// One thread per atom j = f*q + i.  Each operation rounds once (no FMA contraction), so that the atoms are
+// the same doubles on every build.
+template <int Q>
+__global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V, const int32_t* __restrict__ F,
+                                                    int64_t nF, int64_t nV, double* __restrict__ x,
+                                                    double* __restrict__ w) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nF * Q) return;
+  const int64_t f = j / Q;
+  const int i = (int)(j - f * Q);
+  const RuleTable& R = c_rule[Q == 6 ? 0 : 1];
+  const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
+  const double nan = __longlong_as_double(0x7ff8000000000000LL);
+  if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
+    x[3 * j] = x[3 * j + 1] = x[3 * j + 2] = nan;
+    w[j] = nan;
+    return;
+  }
+  double p0[3], p1[3], p2[3], e1[3], e2[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    p0[c] = V[3 * (int64_t)i0 + c];
+    p1[c] = V[3 * (int64_t)i1 + c];
+    p2[c] = V[3 * (int64_t)i2 + c];
+    e1[c] = __dsub_rn(p1[c], p0[c]);
+    e2[c] = __dsub_rn(p2[c], p0[c]);
+  }
+  const double cx = __dsub_rn(__dmul_rn(e1[1], e2[2]), __dmul_rn(e1[2], e2[1]));
+  const double cy = __dsub_rn(__dmul_rn(e1[2], e2[0]), __dmul_rn(e1[0], e2[2]));
+  const double cz = __dsub_rn(__dmul_rn(e1[0], e2[1]), __dmul_rn(e1[1], e2[0]));
+  const double n2 = __dadd_rn(__dadd_rn(__dmul_rn(cx, cx), __dmul_rn(cy, cy)), __dmul_rn(cz, cz));
+  const double area = __dmul_rn(0.5, __dsqrt_rn(n2));
+  const double l0 = R.lam[i][0], l1 = R.lam[i][1], l2 = R.lam[i][2];
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+    x[3 * j + c] = __dadd_rn(__dadd_rn(__dmul_rn(l0, p0[c]), __dmul_rn(l1, p1[c])), __dmul_rn(l2, p2[c]));
+  w[j] = __dmul_rn(R.om[i], area);
+}
+
+// Gauss-Legendre nodes/weights on [-1,1], ascending, by Newton iteration on P_n evaluated with the
+// Bonnet recurrence in long double; the derivative comes from (1-t^2) P_n' = n (P_{n-1} - t P_n).
+void legendre_rule(int n, std::vector<long double>& t, std::vector<long double>& wt) {
+  const long double pi = 3.141592653589793238462643383279502884L;
+  t.assign(n, 0.0L);
+  wt.assign(n, 0.0L);
+  for (int m = 0; m < (n + 1) / 2; ++m) {
+    long double u = cosl(pi * (4 * m + 3) / (4 * n + 2));  // m-th largest root, Tricomi-like start
+    long double pn = 0, pm = 0;
+    for (int it = 0; it < 64; ++it) {
+      pm = 1.0L;
+      pn = u;
+      for (int k = 1; k < n; ++k) {
+        const long double nx = ((2 * k + 1) * u * pn - k * pm) / (k + 1);
+        pm = pn;
+        pn = nx;
+      }
+      const long double d = n * (pm - u * pn) / (1.0L - u * u);
+      const long double step = pn / d;
+      u -= step;
+      if (fabsl(step) <= 4e-20L * (1.0L + fabsl(u))) break;
+    }
+    pm = 1.0L;
+    pn = u;
+    for (int k = 1; k < n; ++k) {
+      const long double nx = ((2 * k + 1) * u * pn - k * pm) / (k + 1);
+      pm = pn;
+      pn = nx;
+    }
+    const long double d = n * (pm - u * pn) / (1.0L - u * u);
+    const long double wgt = 2.0L / ((1.0L - u * u) * d * d);
+    t[n - 1 - m] = u;
+    t[m] = -u;
+    wt[n - 1 - m] = wgt;
+    wt[m] = wgt;
+  }
+  if (n & 1) t[n / 2] = 0.0L;
+}
+
+__global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restrict__ tab, int n_r, int n_th, int n_ph,
+                                                          double wph, double* __restrict__ xi, double* __restrict__ W) {
+  const int64_t K = (int64_t)n_r * n_th * n_ph;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= K) return;
+  const int c = (int)(k % n_ph);
+  const int64_t ab = k / n_ph;
+  const int b = (int)(ab % n_th);
+  const int a = (int)(ab / n_th);
+  const double* r = tab;
+  const double* wr = r + n_r;
+  const double* mu = wr + n_r;
+  const double* st = mu + n_th;
+  const double* wmu = st + n_th;
+  const double* cph = wmu + n_th;
+  const double* sph = cph + n_ph;
+  const double ra = r[a];
+  xi[3 * k + 0] = __dmul_rn(ra, __dmul_rn(st[b], cph[c]));
+  xi[3 * k + 1] = __dmul_rn(ra, __dmul_rn(st[b], sph[c]));
+  xi[3 * k + 2] = __dmul_rn(ra, mu[b]);
+  if (W) W[k] = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(wr[a], ra), ra), wmu[b]), wph);
+}
+
+}  // namespace
+
+int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t) {
+  SFD_REQUIRE(q, SFD_ERR_NULL, "freq quadrature is NULL");
+  SFD_REQUIRE(q->n_r >= 1 && q->n_theta >= 1 && q->n_phi >= 1, SFD_ERR_INVALID_ARG,
+              "freq quadrature sizes must be >= 1 (got %d,%d,%d)", q->n_r, q->n_theta, q->n_phi);
+  SFD_REQUIRE(R > 0.0 && std::isfinite(R), SFD_ERR_INVALID_ARG, "R must be positive and finite");
+  const double pi = 3.14159265358979323846;
+  std::vector<long double> u, wu;
+  legendre_rule(q->n_r, u, wu);
+  t.r.resize(q->n_r);
+  t.wr.resize(q->n_r);
+  const long double half = (long double)R / 2;
+  for (int a = 0; a < q->n_r; ++a) {
+    t.r[a] = (double)(half + half * u[a]);
+    t.wr[a] = (double)(half * wu[a]);
+  }
+  legendre_rule(q->n_theta, u, wu);
+  t.mu.resize(q->n_theta);
+  t.st.resize(q->n_theta);
+  t.wmu.resize(q->n_theta);
+  for (int b = 0; b < q->n_theta; ++b) {
+    t.mu[b] = (double)u[b];
+    t.wmu[b] = (double)wu[b];
+    t.st[b] = std::sqrt(1.0 - t.mu[b] * t.mu[b]);
+  }
+  t.cph.resize(q->n_phi);
+  t.sph.resize(q->n_phi);
+  for (int c = 0; c < q->n_phi; ++c) {
+    const double ph = 2.0 * pi * c / q->n_phi;
+    t.cph[c] = std::cos(ph);
+    t.sph[c] = std::sin(ph);
+  }
+  t.wph = 2.0 * pi / q->n_phi;
+  return SFD_OK;
+}
+
+size_t freq_tables_bytes(const sfd_freq_quadrature* q) {
+  return align_up(sizeof(double) * (2 * (size_t)q->n_r + 3 * (size_t)q->n_theta + 2 * (size_t)q->n_phi));
+}
+
+int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
+                size_t work_bytes, cudaStream_t st) {
+  SFD_REQUIRE(work_bytes >= freq_tables_bytes(q) && d_work, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "frequency quadrature needs %zu workspace bytes, got %zu", freq_tables_bytes(q), work_bytes);
+  std::vector<double> h;
+  h.reserve(2 * t.r.size() + 3 * t.mu.size() + 2 * t.cph.size());
+  for (const auto* v : {&t.r, &t.wr, &t.mu, &t.st, &t.wmu, &t.cph, &t.sph}) h.insert(h.end(), v->begin(), v->end());
+  // pageable source: the runtime stages the copy before returning, so `h` may die at scope exit
+  SFD_CUDA_TRY(cudaMemcpyAsync(d_work, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+  const int64_t K = (int64_t)q->n_r * q->n_theta * q->n_phi;
+  freq_expand_kernel<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(static_cast<const double*>(d_work), q->n_r,
+                                                                   q->n_theta, q->n_phi, t.wph, d_xi, d_W);
+  return launch_check("freq_expand_kernel");
+}
+
+int rule_table_host(int rule, double* lam, double* om) {
+  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  RuleTable t;
+  fill_rule(rule, t);
+  for (int i = 0; i < rule; ++i) {
+    for (int c = 0; c < 3; ++c) lam[3 * i + c] = t.lam[i][c];
+    om[i] = t.om[i];
+  }
+  return SFD_OK;
+}
+
+int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rule, double* d_x, double* d_w,
+          cudaStream_t st) {
+  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  SFD_REQUIRE(nF >= 0 && nV >= 0, SFD_ERR_INVALID_ARG, "negative mesh size");
+  if (nF == 0) return SFD_OK;
+  SFD_REQUIRE(d_V && d_F && d_x && d_w, SFD_ERR_NULL, "sfd_nodes: NULL buffer");
+  static thread_local int uploaded_dev = -1;
+  int dev = 0;
+  SFD_CUDA_TRY(cudaGetDevice(&dev));
+  if (uploaded_dev != dev) {
+    RuleTable t[2];
+    fill_rule(6, t[0]);
+    fill_rule(12, t[1]);
+    SFD_CUDA_TRY(cudaMemcpyToSymbol(c_rule, t, sizeof(t)));
+    uploaded_dev = dev;
+  }
+  const int64_t J = nF * rule;
+  const unsigned blocks = (unsigned)((J + 255) / 256);
+  if (rule == 6)
+    nodes_kernel<6><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+  else
+    nodes_kernel<12><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+  return launch_check("nodes_kernel");
+}
+
+}  // namespace sfd

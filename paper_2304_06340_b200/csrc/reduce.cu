@@ -1,0 +1,138 @@
+// reduce.cu -- A6: fused target-side kernel.  For every frequency node: r = |xi_k|, sigmahat = 4 pi sin r / r (the
+// unit sphere's transform, eq. 2.14 in the e^{-i xi.x} convention), Sobolev weight (1+r^2)^{-s} (eq. 2.7),
+// quadrature weight W_k, then I = (2 pi)^-3 sum_k W_k |nuhat_k - sigmahat|^2 (1+r^2)^{-s} (Plancherel, eq. 2.5).
+// The paper leaves this step out of its timings ("can be ideally accelerated by GPUs").
+//
+// HBM-bound, 48 B per target, one pass.  The sum is carried as a (sum, compensation) fp64 pair (TwoSum) from the
+// per-thread accumulators through warp shuffles, the block tree and a fixed-order final pass over the per-CTA
+// partials: deterministic for a given K.
+#include "internal.cuh"
+
+namespace sfd {
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kMaxBlocks = 148 * 8;
+
+struct Comp {
+  double s, c;
+};
+
+__device__ __forceinline__ void two_sum_add(Comp& a, double v) {
+  const double t = __dadd_rn(a.s, v);
+  const double bp = __dsub_rn(t, a.s);
+  const double e = __dadd_rn(__dsub_rn(a.s, __dsub_rn(t, bp)), __dsub_rn(v, bp));
+  a.s = t;
+  a.c = __dadd_rn(a.c, e);
+}
+__device__ __forceinline__ void comp_merge(Comp& a, const Comp& b) {
+  two_sum_add(a, b.s);
+  a.c = __dadd_rn(a.c, b.c);
+}
+__device__ __forceinline__ Comp comp_shfl_down(const Comp& a, int d) {
+  Comp b;
+  b.s = __shfl_down_sync(0xffffffffu, a.s, d);
+  b.c = __shfl_down_sync(0xffffffffu, a.c, d);
+  return b;
+}
+
+__device__ __forceinline__ Comp block_reduce(Comp v) {
+  __shared__ Comp part[kThreads / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    const Comp o = comp_shfl_down(v, d);
+    comp_merge(v, o);
+  }
+  if (lane == 0) part[wid] = v;
+  __syncthreads();
+  if (wid == 0) {
+    v = lane < kThreads / 32 ? part[lane] : Comp{0.0, 0.0};
+#pragma unroll
+    for (int d = 4; d > 0; d >>= 1) {
+      const Comp o = comp_shfl_down(v, d);
+      comp_merge(v, o);
+    }
+  }
+  return v;  // valid in thread 0
+}
+
+__device__ __forceinline__ double sigma_hat(double r) {
+  const double four_pi = 12.566370614359172;
+  if (r < 1e-4) {
+    const double r2 = r * r;
+    return four_pi * (1.0 - r2 / 6.0 + r2 * r2 / 120.0);
+  }
+  return four_pi * sin(r) / r;
+}
+
+__device__ __forceinline__ double sobolev_weight(double q, double s, int s_kind) {
+  if (s_kind == 1) return 1.0 / q;
+  if (s_kind == 2) return 1.0 / (q * q);
+  return pow(q, -s);
+}
+
+__global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* __restrict__ nuhat, const double* __restrict__ xi,
+                                                               const double* __restrict__ W, int64_t K, double s, int s_kind,
+                                                               Comp* __restrict__ partial) {
+  Comp acc{0.0, 0.0};
+  const int64_t stride = (int64_t)gridDim.x * kThreads;
+  for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += stride) {
+    const double a = xi[3 * k], b = xi[3 * k + 1], c = xi[3 * k + 2];
+    const double2 nu = nuhat[k];
+    const double r2 = a * a + b * b + c * c;
+    const double r = sqrt(r2);
+    const double dre = nu.x - sigma_hat(r);
+    const double term = W[k] * (dre * dre + nu.y * nu.y) * sobolev_weight(1.0 + r2, s, s_kind);
+    two_sum_add(acc, term);
+  }
+  const Comp tot = block_reduce(acc);
+  if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(kThreads) reduce_final_kernel(const Comp* __restrict__ partial, int n, double* __restrict__ result) {
+  Comp acc{0.0, 0.0};
+  for (int i = threadIdx.x; i < n; i += kThreads) comp_merge(acc, partial[i]);
+  const Comp tot = block_reduce(acc);
+  if (threadIdx.x == 0) {
+    const double two_pi = 6.283185307179586;
+    result[0] = (tot.s + tot.c) / (two_pi * two_pi * two_pi);
+  }
+}
+
+int reduce_blocks(int64_t K) {
+  const int64_t want = (K + kThreads - 1) / kThreads;
+  return (int)(want < 1 ? 1 : (want > kMaxBlocks ? kMaxBlocks : want));
+}
+
+}  // namespace
+
+size_t reduce_workspace(int64_t K) {
+  (void)K;
+  return 256 + align_up(sizeof(Comp) * kMaxBlocks);
+}
+
+int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
+                   size_t work_bytes, cudaStream_t st, double** d_result) {
+  SFD_REQUIRE(K >= 0, SFD_ERR_INVALID_ARG, "K must be >= 0");
+  SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
+  SFD_REQUIRE(d_work && work_bytes >= reduce_workspace(K), SFD_ERR_WORKSPACE_TOO_SMALL,
+              "reduction needs %zu workspace bytes, got %zu", reduce_workspace(K), work_bytes);
+  SFD_REQUIRE(K == 0 || (d_nuhat && d_xi && d_W), SFD_ERR_NULL, "sfd_reduce: NULL input buffer");
+  double* result = static_cast<double*>(d_work);
+  Comp* partial = reinterpret_cast<Comp*>(static_cast<char*>(d_work) + 256);
+  *d_result = result;
+  if (K == 0) {
+    SFD_CUDA_TRY(cudaMemsetAsync(result, 0, sizeof(double), st));
+    return SFD_OK;
+  }
+  const int blocks = reduce_blocks(K);
+  const int s_kind = s == 1.0 ? 1 : (s == 2.0 ? 2 : 0);
+  reduce_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(d_nuhat), d_xi, d_W, K, s, s_kind,
+                                                   partial);
+  SFD_TRY(launch_check("reduce_terms_kernel"));
+  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, result);
+  return launch_check("reduce_final_kernel");
+}
+
+}  // namespace sfd

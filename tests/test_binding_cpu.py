@@ -1,0 +1,102 @@
+"""CPU-side checks of the CUDA path's host logic (-m "not gpu"): the C-ABI library loads and exports every
+symbol include/sfd.h declares, argument checking, size queries, the rule table and the host frequency
+quadrature.  No compute call needs a GPU here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def sfd():
+    from paper_2304_06340_b200 import build
+    build.build()
+    import paper_2304_06340_b200 as P
+    return P
+
+
+def test_exports_match_header(sfd):
+    hdr = open(os.path.join(ROOT, "include", "sfd.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sfd_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 20
+    lib = C.CDLL(sfd.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in sfd.h but not exported"
+    assert declared == set(sfd.EXPORTS), declared ^ set(sfd.EXPORTS)
+
+
+def test_mesh_sizes_P228(sfd):
+    for line in open(os.path.join(ROOT, "tests", "golden", "mesh_counts.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        lvl, nv, nf = [int(t) for t in line.split()[:3]]
+        got = sfd.sfd_mesh_icosphere_sizes(lvl)
+        assert got[:2] == (nv, nf)
+    with pytest.raises(sfd.SfdError) as e:
+        sfd.sfd_mesh_icosphere_sizes(11)
+    assert e.value.status == -2
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_mesh_icosphere_sizes(-1)
+
+
+@pytest.mark.parametrize("q,deg", [(6, 4), (12, 6)])
+def test_rule_exactness(sfd, q, deg):
+    """Integral of u^a v^b over the standard simplex is a! b!/(a+b+2)!; weights sum to 1 (times area 1/2)."""
+    from math import factorial
+    lam, om = sfd.sfd_rule_table(q)
+    assert abs(om.sum() - 1) < 1e-15 and (om > 0).all() and (lam > 0).all()
+    assert np.abs(lam.sum(1) - 1).max() < 1e-15
+    for a in range(deg + 1):
+        for b in range(deg + 1 - a):
+            got = 0.5 * np.sum(om * lam[:, 1] ** a * lam[:, 2] ** b)
+            assert abs(got - factorial(a) * factorial(b) / factorial(a + b + 2)) < 2e-16 * 8
+    # first inexact degree
+    a, b = deg + 1, 0
+    got = 0.5 * np.sum(om * lam[:, 1] ** a)
+    assert abs(got - factorial(a) / factorial(a + 2)) > 1e-8
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_rule_table(7)
+
+
+def test_freq_nodes_match_oracle(sfd, orc):
+    for (nr, nt, nph, R) in [(32, 16, 32, 32.0), (5, 3, 4, 2.5), (1, 1, 1, 1.0), (128, 64, 8, 128.0)]:
+        xi, W = sfd.sfd_freq_nodes((nr, nt, nph), R)
+        xo, Wo = orc.freq_nodes(nr, nt, nph, R)
+        assert np.abs(xi - xo).max() <= 4e-16 * R
+        assert np.abs(W - Wo).max() <= 1e-14 * np.abs(Wo).max()
+        # volume of the ball: sum W = 4/3 pi R^3 (GL exact for r^2)
+        assert abs(W.sum() - 4 / 3 * np.pi * R ** 3) < 1e-12 * R ** 3
+
+
+def test_argument_errors(sfd):
+    with pytest.raises(sfd.SfdError) as e:
+        sfd.sfd_freq_nodes((0, 4, 4), 1.0)
+    assert e.value.status == -2
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_freq_nodes((4, 4, 4), -1.0)
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_surface_ft_workspace(-1, 4, None, None, 0.0)
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_surface_ft_workspace(4, 4, None, None, 2.0)      # eps >= 1
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_surface_ft_workspace(4, 4, None, None, 1e-16)    # eps too small
+    with pytest.raises(sfd.SfdError) as e:
+        sfd.sfd_surface_ft_workspace(4, 4, None, None, 1e-6)     # X, S required
+    assert e.value.status == -1
+    assert sfd.sfd_surface_ft_workspace(0, 0, None, None, 0.0) == 0
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_weak_distance_workspace(80, 5, (4, 4, 4), 1.0, 0.0)  # unknown rule
+    assert "rule" in sfd.binding._lib.sfd_last_error().decode()
+
+
+def test_workspace_queries_scale(sfd):
+    a = sfd.sfd_surface_ft_workspace(1000, 1000, [1, 1, 1], [32, 32, 32], 1e-6)
+    b = sfd.sfd_surface_ft_workspace(1000, 1000, [1, 1, 1], [64, 64, 64], 1e-6)
+    assert b > a > 0
+    w0 = sfd.sfd_weak_distance_workspace(80, 6, (32, 16, 32), 32.0, 0.0)
+    assert w0 >= 480 * 32 + 16384 * 48

@@ -1,0 +1,202 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs (-m gpu).
+
+Bars (BASELINE.json north_star): integer mesh output bit-exact; direct-sum nuhat max|d| <= 1e-12 * sum|w|;
+I to relative 1e-8.  Vertices / atoms / frequency nodes are compared to a few ulp (they are the same operations
+rounded once each, so they are in fact expected to be bit-identical; the tolerance only guards libm differences).
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sfd():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2304_06340_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+# ---- A1/A2 ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("level", [0, 1, 2, 3, 4, 5, 6, 7])
+def test_mesh_bit_exact(sfd, orc, torch, level):
+    V, F = sfd.sfd_mesh_icosphere(level)
+    Vo, Fo = orc.mesh_icosphere(level)
+    assert np.array_equal(F.cpu().numpy(), Fo), "integer mesh output must be bit-exact"
+    assert np.array_equal(V.cpu().numpy(), Vo), "vertex arithmetic is IEEE add/mul/sqrt/div: bit-identical"
+
+
+def test_mesh_level8_invariants(sfd, torch):
+    """Level 8 (1.31 M faces): properties that hold at any size (Euler, valence, every directed edge once)."""
+    V, F = sfd.sfd_mesh_icosphere(8)
+    nV, nF = V.shape[0], F.shape[0]
+    assert (nV, nF) == (10 * 4 ** 8 + 2, 20 * 4 ** 8)
+    Fl = F.long()
+    assert int(Fl.min()) == 0 and int(Fl.max()) == nV - 1
+    e = torch.cat([Fl[:, [0, 1]], Fl[:, [1, 2]], Fl[:, [2, 0]]])
+    key = e[:, 0] * nV + e[:, 1]
+    assert torch.unique(key).numel() == 3 * nF            # every directed edge exactly once
+    rkey = e[:, 1] * nV + e[:, 0]
+    assert torch.equal(torch.sort(key).values, torch.sort(rkey).values)  # and its reverse: closed, oriented
+    val = torch.bincount(Fl.reshape(-1), minlength=nV)
+    assert int((val == 5).sum()) == 12 and int((val == 6).sum()) == nV - 12
+    assert float((V.norm(dim=1) - 1).abs().max()) < 4e-16
+    assert nV - 3 * nF // 2 + nF == 2
+
+
+# ---- A3 ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("level,rule", [(0, 6), (1, 6), (3, 12), (5, 6), (5, 12)])
+def test_nodes(sfd, orc, torch, level, rule):
+    Vo, Fo = orc.mesh_icosphere(level)
+    xo, wo = orc.nodes(Vo, Fo, rule)
+    x, w = sfd.sfd_nodes(dev(torch, Vo), dev(torch, Fo), rule)
+    assert np.abs(x.cpu().numpy() - xo).max() <= 2e-16
+    assert np.abs(w.cpu().numpy() - wo).max() <= 2e-16 * wo.max()
+
+
+def test_nodes_degenerate_and_empty(sfd, torch):
+    V = dev(torch, np.array([[0, 0, 0], [1, 0, 0], [2, 0, 0], [0, 1, 0]], np.float64))
+    F = dev(torch, np.array([[0, 1, 2], [0, 1, 3]], np.int32))   # first face has zero area
+    x, w = sfd.sfd_nodes(V, F, 6)
+    w = w.cpu().numpy()
+    assert np.all(w[:6] == 0) and abs(w[6:].sum() - 0.5) < 1e-15
+    x0, w0 = sfd.sfd_nodes(V, F[:0].contiguous(), 12)
+    assert x0.shape == (0, 3) and w0.shape == (0,)
+
+
+def test_freq_nodes_device(sfd, orc, torch):
+    for (nr, nt, nph, R) in [(32, 16, 32, 32.0), (7, 5, 3, 4.0)]:
+        xi, W = sfd.sfd_freq_nodes_device((nr, nt, nph), R)
+        xo, Wo = orc.freq_nodes(nr, nt, nph, R)
+        assert np.abs(xi.cpu().numpy() - xo).max() <= 4e-16 * R
+        assert np.abs(W.cpu().numpy() - Wo).max() <= 1e-14 * Wo.max()
+
+
+# ---- A4 direct sum ----------------------------------------------------------------------------------
+def _direct_case(sfd, orc, torch, x, w, xi, tol=1e-12):
+    nu = sfd.sfd_surface_ft(dev(torch, x), dev(torch, w), dev(torch, xi), 0.0).cpu().numpy()
+    ref = orc.direct_sum(x, w, xi)
+    err = np.abs(nu - ref).max() if len(ref) else 0.0
+    assert err <= tol * np.abs(w).sum(), (err, np.abs(w).sum())
+    return nu, ref
+
+
+def test_direct_config1_full(sfd, orc, torch):
+    c = workloads.CONFIGS[1]
+    V, F = orc.mesh_icosphere(c["level"])
+    x, w = orc.nodes(V, F, c["rule"])
+    xi, W = orc.freq_nodes(c["n_r"], c["n_theta"], c["n_phi"], c["R"])
+    nu, ref = _direct_case(sfd, orc, torch, x, w, xi)
+    # spot values of SURVEY 8(c) pin 5 fix the target ordering
+    assert abs(nu[0] - 11.6625241207662) < 1e-9 and abs(nu[-1] - (-1.0556323496997)) < 1e-9
+    assert np.abs(nu.imag).max() < 1e-13
+
+
+@pytest.mark.parametrize("J,K", [(1, 1), (7, 33), (33, 7), (1000, 1000), (513, 2049), (3000, 131), (512, 128 * 4 + 1)])
+def test_direct_random_clouds(sfd, orc, torch, J, K):
+    """Off-centre sources and targets, signed weights: exercises Im != 0, ragged tiles and the source split."""
+    x, w, xi = workloads.random_cloud(J, K)
+    _direct_case(sfd, orc, torch, x, w, xi)
+
+
+def test_direct_large_phase(sfd, orc, torch):
+    """|xi.x| up to ~1.8e3 (config-5 scale, R = 1024): the range reduction must hold 1e-12 * sum|w|."""
+    x, w, xi = workloads.random_cloud(600, 700, seed=7, x_offset=(0, 0, 0), xi_radius=1024.0, xi_offset=(0, 0, 0))
+    _direct_case(sfd, orc, torch, x, np.abs(w), xi)
+
+
+def test_direct_empty(sfd, torch):
+    x, w, xi = workloads.random_cloud(5, 9)
+    nu = sfd.sfd_surface_ft(dev(torch, x[:0]), dev(torch, w[:0]), dev(torch, xi), 0.0)
+    assert nu.shape == (9,) and float(nu.abs().max()) == 0.0
+    nu = sfd.sfd_surface_ft(dev(torch, x), dev(torch, w), dev(torch, xi[:0]), 0.0)
+    assert nu.shape == (0,)
+
+
+def test_direct_config2_sampled(sfd, orc, torch):
+    """Config 2 at full size in the launch configuration bench.py times; the oracle checks a seeded sample."""
+    c = workloads.CONFIGS[2]
+    V, F = orc.mesh_icosphere(c["level"])
+    x, w = orc.nodes(V, F, c["rule"])
+    xi, W = orc.freq_nodes(c["n_r"], c["n_theta"], c["n_phi"], c["R"])
+    nu = sfd.sfd_surface_ft(dev(torch, x), dev(torch, w), dev(torch, xi), 0.0).cpu().numpy()
+    idx = workloads.target_subset(len(xi), 2048, seed=0)
+    ref = orc.direct_sum(x, w, xi[idx])
+    assert np.abs(nu[idx] - ref).max() <= 1e-12 * w.sum()
+    assert abs(nu[0].real - w.sum()) < 1e-2 and np.abs(nu.imag).max() < 1e-12  # central symmetry (pin 4 note)
+
+
+# ---- A6 reduction -----------------------------------------------------------------------------------
+@pytest.mark.parametrize("s", [1.0, 2.0, 0.75, 3.5])
+def test_reduce_fed_oracle_nuhat(sfd, orc, torch, s):
+    c = workloads.CONFIGS[1]
+    V, F = orc.mesh_icosphere(c["level"])
+    x, w = orc.nodes(V, F, c["rule"])
+    xi, W = orc.freq_nodes(c["n_r"], c["n_theta"], c["n_phi"], c["R"])
+    nu = orc.direct_sum(x, w, xi)
+    I_ref = orc.reduce(nu, xi, W, s)
+    I = sfd.sfd_reduce(dev(torch, nu.view(np.float64).reshape(-1, 2)), dev(torch, xi), dev(torch, W), s)
+    assert abs(I - I_ref) <= 1e-8 * I_ref
+    assert abs(I - I_ref) <= 1e-12 * I_ref  # what the arithmetic actually delivers
+
+
+def test_reduce_small_r_and_complex(sfd, orc, torch):
+    """r < 1e-4 series branch of sigmahat, r = 0, non-zero imaginary parts, ragged K."""
+    rng = np.random.default_rng(3)
+    K = 1237
+    xi = rng.normal(size=(K, 3)) * np.logspace(-8, 1, K)[:, None]
+    xi[0] = 0.0
+    W = rng.random(K)
+    nu = rng.normal(size=K) + 1j * rng.normal(size=K)
+    I_ref = orc.reduce(nu, xi, W, 1.5)
+    I = sfd.sfd_reduce(dev(torch, nu.view(np.float64).reshape(-1, 2)), dev(torch, xi), dev(torch, W), 1.5)
+    assert abs(I - I_ref) <= 1e-12 * I_ref
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_reduce(dev(torch, nu.view(np.float64).reshape(-1, 2)), dev(torch, xi), dev(torch, W), 0.5)
+    assert sfd.sfd_reduce(dev(torch, np.zeros((0, 2))), dev(torch, np.zeros((0, 3))), dev(torch, np.zeros(0)), 2.0) == 0.0
+
+
+# ---- whole path -------------------------------------------------------------------------------------
+def test_weak_distance_config1(sfd, orc, torch):
+    c = workloads.CONFIGS[1]
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    V, F = sfd.sfd_mesh_icosphere(c["level"])
+    d, I = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 0.0)
+    Vo, Fo = orc.mesh_icosphere(c["level"])
+    d_ref, I_ref = orc.weak_distance(Vo, Fo, c["rule"], 2.0, c["R"], *q)
+    assert abs(I - I_ref) <= 1e-8 * I_ref and abs(d - d_ref) <= 1e-8 * d_ref
+    assert abs(d - 9.336109377069e-2) < 1e-9   # SURVEY 8(c) pin 5, config 1 in full
+    # host-buffer entry point gives the same number
+    d2, I2 = sfd.sfd_weak_distance_host(Vo, Fo, c["rule"], 2.0, c["R"], q, 0.0)
+    assert abs(I2 - I) <= 1e-13 * I
+
+
+def test_weak_distance_jittered_mesh(sfd, orc, torch):
+    """Config-4-style radial jitter (an input, workloads.jitter_vertices) on a small mesh: Im(nuhat) != 0."""
+    Vo, Fo = orc.mesh_icosphere(2)
+    Vj = workloads.jitter_vertices(Vo, Fo, 0.1, 0)
+    q = (24, 12, 16)
+    for s in (1.0, 2.0):
+        d_ref, I_ref = orc.weak_distance(Vj, Fo, 6, s, 16.0, *q)
+        d, I = sfd.sfd_weak_distance(dev(torch, Vj), dev(torch, Fo), 6, s, 16.0, q, 0.0)
+        assert abs(I - I_ref) <= 1e-8 * I_ref
+
+
+def test_surface_ft_host_entry(sfd, orc):
+    x, w, xi = workloads.random_cloud(300, 500)
+    nu = sfd.sfd_surface_ft_host(x, w, xi, 0.0)
+    ref = orc.direct_sum(x, w, xi)
+    assert np.abs(nu - ref).max() <= 1e-12 * np.abs(w).sum()
