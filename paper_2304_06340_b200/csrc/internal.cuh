@@ -20,6 +20,8 @@ struct FreqTables {
   double wph;                        // 2 pi / n_phi
 };
 int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t);
+// n-point Gauss-Legendre rule on [-1,1] (ascending), long double Newton iteration (host)
+void gauss_legendre_host(int n, std::vector<long double>& t, std::vector<long double>& wt);
 size_t freq_tables_bytes(const sfd_freq_quadrature* q);
 int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
                 size_t work_bytes, cudaStream_t st);

@@ -148,6 +148,8 @@ __global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restri
 
 }  // namespace
 
+void gauss_legendre_host(int n, std::vector<long double>& t, std::vector<long double>& wt) { legendre_rule(n, t, wt); }
+
 int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t) {
   SFD_REQUIRE(q, SFD_ERR_NULL, "freq quadrature is NULL");
   SFD_REQUIRE(q->n_r >= 1 && q->n_theta >= 1 && q->n_phi >= 1, SFD_ERR_INVALID_ARG,

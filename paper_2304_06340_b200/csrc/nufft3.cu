@@ -1,13 +1,344 @@
-// placeholder, replaced by the type-3 NUFFT
+// nufft3.cu -- A5: 3-D type-3 nonuniform FFT, nuhat_k = sum_j w_j exp(-i xi_k . x_j) to tolerance eps, for
+// nonuniform sources AND nonuniform targets ("in general it is required to compute contributions from
+// nonuniform sources to nonuniform targets, which can be accelerated by the Type-3 NUFFT [18]").  The paper
+// itself runs the type-1 special case on a lattice (eq. 3.6, eq. 3.7) through a library; this is a
+// from-scratch implementation of the general case in fp64.  DESIGN.md "type-3 NUFFT" derives the formulas.
+//
+//   xi.x = (xi-D).(x-C) + D.x + (xi-D).C            C, D = centres of sources / targets
+//   1. c'_j = w_j e^{-i D.x_j};  u_j = (x_j-C) sigma S/pi + nf/2   (rescaling: analogue of P:188 eq. 3.7)
+//   2. bin-sort sources ("sort"), spread onto the fine grid nf^3 (spread.cu)
+//   3. deconvolve by the kernel's transform on the integer modes and zero-pad into the inner grid n2 = 2 nf
+//   4. uniform FFT of size n2^3 (cuFFT: "fastest GPU version ... provided by CUDA Toolkit")
+//   5. bin-sort targets, interpolate at u2_k = (xi_k-D) n2/(2 sigma S) + n2/2 (interp.cu)
+//   6. divide by the kernel's transform at the non-integer frequencies, multiply by e^{-i (xi_k-D).C}
+#include <cufft.h>
+
+#include <cmath>
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <vector>
+
 #include "internal.cuh"
+#include "nufft3.cuh"
+
 namespace sfd {
-int nufft3_sizes(int64_t, int64_t, const double*, const double*, double, Nufft3Sizes*) {
-  set_error("type-3 NUFFT not built yet");
-  return SFD_ERR_UNSUPPORTED;
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr int kSrcCap = 1024;   // sources per spread work item
+constexpr int kTgtCap = 2048;   // targets per interp work item
+constexpr int kMaxBin = 16;
+// fixed head of the workspace: [0,96) bounds of x and xi; [128,144) n_items_s, n_items_t, queue counters;
+// [1024, ...) scratch of the bounds reduction
+constexpr size_t kMiscBytes = 32768;
+
+// smallest even n' >= n of the form 2^a 3^b 5^c (sizes cuFFT handles with its fastest radices)
+int64_t next_smooth_even(int64_t n) {
+  if (n < 2) n = 2;
+  if (n & 1) ++n;
+  for (;; n += 2) {
+    int64_t m = n;
+    while (m % 2 == 0) m /= 2;
+    while (m % 3 == 0) m /= 3;
+    while (m % 5 == 0) m /= 5;
+    if (m == 1) return n;
+  }
 }
-int nufft3(const double*, const double*, int64_t, const double*, int64_t, double, double*, void*, size_t, cudaStream_t) {
-  set_error("type-3 NUFFT not built yet");
-  return SFD_ERR_UNSUPPORTED;
+
+// Kernel width and shape for tolerance eps at upsampling 2 (parameter choice of the ES-kernel papers, refs [2,3]
+// of P:185; reading R10): w = ceil(log10(1/eps)) + 1, beta = 2.30 w.
+void kernel_params(double eps, int* w, double* beta) {
+  int ww = (int)std::ceil(std::log10(1.0 / eps) - 1e-9) + 1;
+  if (ww < 2) ww = 2;
+  if (ww > kMaxW) ww = kMaxW;
+  *w = ww;
+  *beta = 2.30 * ww;
 }
-int nufft3_release_cache() { return SFD_OK; }
+
+struct Layout {
+  size_t src, skey, shist, soff, scur, sitems, tgt, tkey, thist, toff, tcur, titems, fine, inner, fftwork, dec, scan,
+      misc, total;
+  int64_t ns_bins, nt_bins, ns_items, nt_items;
+  size_t inner_bytes;
+};
+
+// Geometry from half-widths X (sources) and S (targets); centres are filled in by the caller.
+int make_params(const double X_in[3], const double S_in[3], double eps, bool real_c, N3Params* p) {
+  kernel_params(eps, &p->w, &p->beta);
+  p->real_c = real_c ? 1 : 0;
+  for (int d = 0; d < 3; ++d) {
+    double X = X_in[d], S = S_in[d];
+    SFD_REQUIRE(std::isfinite(X) && std::isfinite(S) && X >= 0 && S >= 0, SFD_ERR_INVALID_ARG,
+                "type-3 NUFFT: extents must be finite and >= 0");
+    if (S < 1e-150) S = 1.0;
+    if (X * S < 1.0) X = 1.0 / S;
+    const double need = 2.0 * kSigma * X * S / kPi + p->w + 1;
+    SFD_REQUIRE(need < 8192.0, SFD_ERR_UNSUPPORTED, "type-3 NUFFT: fine grid of %.0f points per axis is too large", need);
+    const int64_t nf = next_smooth_even((int64_t)std::ceil(need));
+    p->nf[d] = (int)nf;
+    p->n2[d] = (int)(2 * nf);
+    p->sx[d] = kSigma * S / kPi;
+    p->st[d] = (double)p->n2[d] / (2.0 * kSigma * S);
+    p->kap[d] = p->w * kPi / (2.0 * kSigma * S);
+  }
+  p->bs = std::min(kMaxBin, spread_max_bin(p->w, real_c));
+  p->bt = std::min(kMaxBin, interp_max_bin(p->w));
+  for (int d = 0; d < 3; ++d) {
+    p->nbs[d] = (p->nf[d] + p->bs - 1) / p->bs;
+    p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
+    p->nbt[d] = (p->n2[d] / 2) / p->bt + 1;
+  }
+  return SFD_OK;
+}
+
+int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
+  L->ns_bins = (int64_t)p.nbs[0] * p.nbs[1] * p.nbs[2];
+  L->nt_bins = (int64_t)p.nbt[0] * p.nbt[1] * p.nbt[2];
+  L->ns_items = L->ns_bins + J / kSrcCap + 1;
+  L->nt_items = L->nt_bins + K / kTgtCap + 1;
+  SFD_REQUIRE(L->ns_bins < 0x7fffffffLL && L->nt_bins < 0x7fffffffLL && J < 0x7fffffffLL && K < 0x7fffffffLL,
+              SFD_ERR_UNSUPPORTED, "type-3 NUFFT: problem too large for 32-bit bin bookkeeping");
+  size_t o = 0;
+  auto put = [&](size_t bytes) {
+    const size_t at = o;
+    o += align_up(bytes);
+    return at;
+  };
+  L->misc = put(kMiscBytes);
+  L->src = put((size_t)J * sizeof(SrcRec));
+  L->skey = put((size_t)J * 4);
+  L->shist = put((size_t)(L->ns_bins + 1) * 4);
+  L->soff = put((size_t)(L->ns_bins + 1) * 4);
+  L->scur = put((size_t)(L->ns_bins + 1) * 4);
+  L->sitems = put((size_t)L->ns_items * 4 * 3);
+  L->tgt = put((size_t)K * sizeof(TgtRec));
+  L->tkey = put((size_t)K * 4);
+  L->thist = put((size_t)(L->nt_bins + 1) * 4);
+  L->toff = put((size_t)(L->nt_bins + 1) * 4);
+  L->tcur = put((size_t)(L->nt_bins + 1) * 4);
+  L->titems = put((size_t)L->nt_items * 4 * 3);
+  L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2]) * 8);
+  L->scan = put(scan_workspace(std::max(L->ns_bins, L->nt_bins) + 1));
+  L->fine = put((size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16));
+  L->inner_bytes = (size_t)p.n2[0] * p.n2[1] * p.n2[2] * 16;
+  L->inner = put(L->inner_bytes);
+  L->fftwork = put(L->inner_bytes);   // cuFFT work area (checked against the plan's real need)
+  L->total = o;
+  return SFD_OK;
+}
+
+}  // namespace
+}  // namespace sfd
+
+// ================================================================================================================
+namespace sfd {
+namespace {
+
+// (w/2) phihat(kappa) = (w/2) * 2 int_0^1 phi(z) cos(kappa z) dz; with z = sin(theta) the integrand
+// exp(beta (cos(theta) - 1)) cos(kappa sin(theta)) cos(theta) is analytic on [0, pi/2] and n = 2w+6 Gauss-Legendre
+// nodes give ~1e-14 relative accuracy for every kappa <= w pi / 4 that the two deconvolutions use.
+void make_quad(const N3Params& p, QuadTable* q) {
+  const int n = std::min(kMaxQuad, 2 * p.w + 6);
+  std::vector<long double> t, wt;
+  gauss_legendre_host(n, t, wt);
+  q->n = n;
+  const long double quarter_pi = 0.785398163397448309615660845819875721L;
+  for (int i = 0; i < n; ++i) {
+    const long double th = (t[i] + 1.0L) * quarter_pi;
+    const long double om = wt[i] * quarter_pi;
+    q->z[i] = (double)sinl(th);
+    q->f[i] = (double)((long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)));
+  }
+  for (int i = n; i < kMaxQuad; ++i) q->z[i] = q->f[i] = 0.0;
+}
+
+// ---- cuFFT plan cache (process-global, guarded; sfd_release_cache() empties it) --------------------------------
+struct PlanEntry {
+  cufftHandle h;
+  size_t work;
+};
+std::mutex g_plan_mu;
+std::map<std::tuple<int, int, int, int>, PlanEntry> g_plans;
+
+int get_plan(int dev, const int n2[3], PlanEntry* out) {
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  const auto key = std::make_tuple(dev, n2[0], n2[1], n2[2]);
+  auto it = g_plans.find(key);
+  if (it != g_plans.end()) {
+    *out = it->second;
+    return SFD_OK;
+  }
+  PlanEntry e{};
+  cufftResult r = cufftCreate(&e.h);
+  SFD_REQUIRE(r == CUFFT_SUCCESS, SFD_ERR_CUFFT, "cufftCreate failed (%d)", (int)r);
+  r = cufftSetAutoAllocation(e.h, 0);
+  if (r == CUFFT_SUCCESS) r = cufftMakePlan3d(e.h, n2[0], n2[1], n2[2], CUFFT_Z2Z, &e.work);
+  if (r != CUFFT_SUCCESS) {
+    cufftDestroy(e.h);
+    set_error("cufftMakePlan3d(%d,%d,%d) failed (%d)", n2[0], n2[1], n2[2], (int)r);
+    return SFD_ERR_CUFFT;
+  }
+  g_plans[key] = e;
+  *out = e;
+  return SFD_OK;
+}
+
+}  // namespace
+
+int nufft3_release_cache() {
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  for (auto& kv : g_plans) cufftDestroy(kv.second.h);
+  g_plans.clear();
+  return SFD_OK;
+}
+
+int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out) {
+  SFD_REQUIRE(X && S && out, SFD_ERR_NULL, "nufft3_sizes: NULL argument");
+  // the call recomputes the extents from the data; the query leaves room for their rounding
+  double Xi[3], Si[3];
+  for (int d = 0; d < 3; ++d) {
+    Xi[d] = X[d] * (1.0 + 1e-6);
+    Si[d] = S[d] * (1.0 + 1e-6);
+  }
+  size_t total = 0;
+  N3Params p{};
+  for (int real_c = 0; real_c < 2; ++real_c) {   // whether the strengths stay real is only known from the data
+    SFD_TRY(make_params(Xi, Si, eps, real_c != 0, &p));
+    Layout L;
+    SFD_TRY(make_layout(p, J, K, &L));
+    total = std::max(total, L.total);
+  }
+  out->w = p.w;
+  out->beta = p.beta;
+  for (int d = 0; d < 3; ++d) {
+    out->nf[d] = p.nf[d];
+    out->n2[d] = p.n2[d];
+    out->nout[d] = p.n2[d] / 2 + p.w + 2;
+  }
+  out->work_bytes = total;
+  return SFD_OK;
+}
+
+}  // namespace sfd
+
+// ================================================================================================================
+namespace sfd {
+
+int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps, double* d_nuhat,
+           void* d_work, size_t work_bytes, cudaStream_t st) {
+  if (K == 0) return SFD_OK;
+  SFD_REQUIRE(J > 0, SFD_ERR_INVALID_ARG, "nufft3: J must be > 0 (the caller handles J == 0)");
+  SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "type-3 NUFFT needs a workspace (sfd_surface_ft_workspace), got %zu bytes", work_bytes);
+  char* base = static_cast<char*>(d_work);
+  double* d_bounds = reinterpret_cast<double*>(base);
+  int32_t* d_ctl = reinterpret_cast<int32_t*>(base + 128);
+  double* d_scratch = reinterpret_cast<double*>(base + 1024);
+
+  // A5-1: extents of sources and targets (the one host synchronisation of the transform)
+  SFD_TRY(bounds_minmax(d_x, J, d_bounds, d_scratch, st));
+  SFD_TRY(bounds_minmax(d_xi, K, d_bounds + 6, d_scratch, st));
+  double hb[12];
+  SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, sizeof(hb), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  prof_mark("bounds", st);
+
+  N3Params p{};
+  double X[3], S[3];
+  bool real_c = true;
+  for (int d = 0; d < 3; ++d) {
+    SFD_REQUIRE(std::isfinite(hb[d]) && std::isfinite(hb[3 + d]) && std::isfinite(hb[6 + d]) && std::isfinite(hb[9 + d]),
+                SFD_ERR_INVALID_ARG, "type-3 NUFFT: non-finite source or target coordinate");
+    p.C[d] = 0.5 * (hb[d] + hb[3 + d]);
+    X[d] = (0.5 * (hb[3 + d] - hb[d])) * (1.0 + 1e-12) + 1e-300;
+    p.D[d] = 0.5 * (hb[6 + d] + hb[9 + d]);
+    S[d] = (0.5 * (hb[9 + d] - hb[6 + d])) * (1.0 + 1e-12) + 1e-300;
+    // targets centred at the origin up to rounding (the ball quadrature): snap D to 0 so that c'_j = w_j is real
+    const double reach = std::fmax(std::fabs(hb[6 + d]), std::fabs(hb[9 + d]));
+    if (std::fabs(p.D[d]) <= 1e-9 * reach) {
+      p.D[d] = 0.0;
+      S[d] = reach * (1.0 + 1e-12) + 1e-300;
+    } else {
+      real_c = false;
+    }
+  }
+  SFD_TRY(make_params(X, S, eps, real_c, &p));
+  Layout L;
+  SFD_TRY(make_layout(p, J, K, &L));
+  SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "type-3 NUFFT (w=%d, fine grid %dx%dx%d) needs %zu workspace bytes, got %zu", p.w, p.nf[0], p.nf[1], p.nf[2],
+              L.total, work_bytes);
+  QuadTable quad;
+  make_quad(p, &quad);
+  int dev = 0;
+  SFD_CUDA_TRY(cudaGetDevice(&dev));
+  PlanEntry plan;
+  SFD_TRY(get_plan(dev, p.n2, &plan));
+  SFD_REQUIRE(plan.work <= L.inner_bytes, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "cuFFT wants a %zu-byte work area for %dx%dx%d, more than the %zu reserved", plan.work, p.n2[0], p.n2[1],
+              p.n2[2], L.inner_bytes);
+
+  SrcRec* src = reinterpret_cast<SrcRec*>(base + L.src);
+  TgtRec* tgt = reinterpret_cast<TgtRec*>(base + L.tgt);
+  int32_t* skey = reinterpret_cast<int32_t*>(base + L.skey);
+  int32_t* shist = reinterpret_cast<int32_t*>(base + L.shist);
+  int32_t* soff = reinterpret_cast<int32_t*>(base + L.soff);
+  int32_t* scur = reinterpret_cast<int32_t*>(base + L.scur);
+  int32_t* sitems = reinterpret_cast<int32_t*>(base + L.sitems);
+  int32_t* tkey = reinterpret_cast<int32_t*>(base + L.tkey);
+  int32_t* thist = reinterpret_cast<int32_t*>(base + L.thist);
+  int32_t* toff = reinterpret_cast<int32_t*>(base + L.toff);
+  int32_t* tcur = reinterpret_cast<int32_t*>(base + L.tcur);
+  int32_t* titems = reinterpret_cast<int32_t*>(base + L.titems);
+  double* dec = reinterpret_cast<double*>(base + L.dec);
+  double* fine = reinterpret_cast<double*>(base + L.fine);
+  double* inner = reinterpret_cast<double*>(base + L.inner);
+  void* scan_w = base + L.scan;
+  const size_t scan_b = L.fine - L.scan;
+  const size_t fine_bytes = L.inner - L.fine;
+
+  // A5-2/A5-3: rescale, pre-phase and bin-sort the sources
+  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
+  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_bins, nullptr, scan_w, scan_b, st));
+  SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
+  SFD_TRY(make_items(shist, soff, L.ns_bins, kSrcCap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
+  prof_mark("src_sort", st);
+
+  // A5-4: spread
+  SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
+  SFD_TRY(spread(p, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
+  prof_mark("spread", st);
+
+  // A5-5: deconvolve + zero-pad;  A5-6: uniform FFT (cuFFT, timed on its own)
+  SFD_TRY(deconv_tables(p, quad, dec, st));
+  SFD_TRY(deconv_pad(p, fine, dec, inner, st));
+  prof_mark("deconv_pad", st);
+  cufftResult r = cufftSetStream(plan.h, st);
+  if (r == CUFFT_SUCCESS) r = cufftSetWorkArea(plan.h, base + L.fftwork);
+  if (r == CUFFT_SUCCESS)
+    r = cufftExecZ2Z(plan.h, reinterpret_cast<cufftDoubleComplex*>(inner), reinterpret_cast<cufftDoubleComplex*>(inner),
+                     CUFFT_FORWARD);
+  SFD_REQUIRE(r == CUFFT_SUCCESS, SFD_ERR_CUFFT, "cuFFT Z2Z %dx%dx%d failed (%d)", p.n2[0], p.n2[1], p.n2[2], (int)r);
+  prof_mark("cufft", st);
+
+  // A5-7: rescale and bin-sort the targets
+  SFD_CUDA_TRY(cudaMemsetAsync(thist, 0, (size_t)(L.nt_bins + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(tcur, 0, (size_t)(L.nt_bins + 1) * 4, st));
+  SFD_TRY(target_keys(p, d_xi, K, tkey, thist, st));
+  SFD_TRY(exclusive_scan_i32(thist, toff, L.nt_bins, nullptr, scan_w, scan_b, st));
+  SFD_TRY(target_scatter(p, d_xi, K, tkey, toff, tcur, tgt, st));
+  SFD_TRY(make_items(thist, toff, L.nt_bins, kTgtCap, tcur, titems, L.nt_items, d_ctl + 1, scan_w, scan_b, st));
+  prof_mark("tgt_sort", st);
+
+  // A5-8: interpolate;  A5-9: post-deconvolve + post-phase
+  SFD_TRY(interp(p, inner, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
+  prof_mark("interp", st);
+  SFD_TRY(post_deconv(p, quad, d_xi, K, d_nuhat, st));
+  prof_mark("post", st);
+  return SFD_OK;
+}
+
 }  // namespace sfd

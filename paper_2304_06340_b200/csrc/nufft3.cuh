@@ -1,0 +1,82 @@
+// nufft3.cuh -- internal interfaces of the 3-D type-3 nonuniform FFT (A5; "contributions from nonuniform
+// sources to nonuniform targets, which can be accelerated by the Type-3 NUFFT [18]").
+// derives every formula used here.  Shared by nufft3.cu (plan, glue kernels), spread.cu and interp.cu.
+#pragma once
+#include "common.cuh"
+
+namespace sfd {
+
+constexpr int kMaxW = 16;        // widest kernel (eps = 1e-14 -> w = 15)
+constexpr int kMaxQuad = 48;     // Gauss-Legendre nodes for the kernel's Fourier transform
+constexpr double kSigma = 2.0;   // upsampling factor of both the spreading and the inner type-2 step
+
+// Everything the kernels need to know about one transform (passed by value).
+struct N3Params {
+  int w;              // kernel width in cells
+  double beta;        // ES kernel: phi(z) = exp(beta (sqrt(1-z^2) - 1)), |z| <= 1   (P:185 refs [2,3])
+  int nf[3];          // fine (spreading) grid, index i = l + nf/2 for mode l in [-nf/2, nf/2)
+  int n2[3];          // inner type-2 grid (2 nf), index m <-> t = m h2 - pi
+  double C[3], D[3];  // centres of the sources / of the targets
+  double sx[3];       // source  -> fine-grid coordinate: u  = (x - C) sx + nf/2,   sx = sigma S / pi
+  double st[3];       // target  -> inner-grid coordinate: u2 = (xi - D) st + n2/2, st = n2 / (2 sigma S)
+  double kap[3];      // target  -> argument of phihat:    kappa = (xi - D) kap,    kap = w pi / (2 sigma S)
+  int real_c;         // 1 when D == 0: the strengths c'_j = w_j stay real and so does the fine grid
+  int bs, nbs[3];     // source bins: bs^3 cells, nbs[d] = ceil(nf[d] / bs)
+  int bt, nbt[3], t0[3];  // target bins over the band [t0, t0 + nbt*bt) of the inner grid that holds every target
+};
+
+struct __align__(8) SrcRec { double u[3]; double re, im; };   // sorted source: grid coordinate + strength (40 B)
+struct __align__(8) TgtRec { double u[3]; int64_t k; };       // sorted target: grid coordinate + original index
+
+// quadrature table for phihat(kappa) = 2 int_0^1 phi(z) cos(kappa z) dz  (uploaded per transform)
+struct QuadTable {
+  int n;
+  double z[kMaxQuad];   // GL nodes on [0,1]
+  double f[kMaxQuad];   // (w/2) * 2 * weight * phi(z): sum_q f_q cos(kappa z_q) = (w/2) phihat(kappa)
+};
+
+__device__ __forceinline__ double es_kernel(double z, double beta) {
+  const double t = fmax(0.0, __fma_rn(-z, z, 1.0));
+  return exp(beta * (sqrt(t) - 1.0));
+}
+
+// ---- spread.cu (A5-4) ------------------------------------------------------------------------------------
+// Work item i: sources [item_start[i], item_start[i]+item_count[i]) of bin item_bin[i].  *n_items on the device.
+// grid is real double[nf0][nf1][nf2] (real_c) or complex double[nf0][nf1][nf2][2]; must be zero on entry.
+int spread_max_bin(int w, bool real_c);   // largest bin edge whose padded subgrid fits shared memory
+int interp_max_bin(int w);
+size_t spread_smem_bytes(const N3Params& p);
+int spread(const N3Params& p, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
+           const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st);
+
+// ---- interp.cu (A5-8) ------------------------------------------------------------------------------------
+// v = complex double[n2_0][n2_1][n2_2][2]; writes G[k] (complex) for every sorted target.
+size_t interp_smem_bytes(const N3Params& p);
+int interp(const N3Params& p, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
+           const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
+           double* d_G, cudaStream_t st);
+
+// ---- nufft3_glue.cu: the HBM-bound one-pass kernels around spread / FFT / interp ---------------------------
+constexpr int kBoundsBlocks = 296;
+// (min[3], max[3]) of n points into d_out6; d_scratch holds kBoundsBlocks*6 doubles.
+int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scratch, cudaStream_t st);
+// A5-2/A5-3: bin key of every source + histogram; then scatter into bin order with grid coordinates and c'_j.
+int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st);
+int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
+                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st);
+// A5-7: same for the targets.
+int target_keys(const N3Params& p, const double* d_xi, int64_t K, int32_t* d_key, int32_t* d_hist, cudaStream_t st);
+int target_scatter(const N3Params& p, const double* d_xi, int64_t K, const int32_t* d_key, const int32_t* d_off,
+                   int32_t* d_cursor, TgtRec* d_out, cudaStream_t st);
+// Work items: every occupied bin is cut into slices of <= cap points.  d_items = int32[3][max_items] (bin, start,
+// count); *d_n_items = number of items.  d_tmp holds nbins+1 int32.
+int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int cap, int32_t* d_tmp, int32_t* d_items,
+               int64_t max_items, int32_t* d_n_items, void* d_scan, size_t scan_bytes, cudaStream_t st);
+// A5-5: dec[d][i] = (-1)^l / ((w/2) phihat(l w pi / n2_d)), l = i - nf_d/2; then b~ = g * dec x dec x dec zero-padded
+// into the inner grid at index l mod n2.
+int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st);
+int deconv_pad(const N3Params& p, const double* d_fine, const double* d_dec, double* d_inner, cudaStream_t st);
+// A5-9: nuhat_k = G_k e^{-i (xi_k-D).C} / prod_d (w/2) phihat((xi_kd-D_d) kap_d), in place on d_nuhat.
+int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st);
+
+}  // namespace sfd

@@ -1,0 +1,291 @@
+// nufft3_glue.cu -- the one-pass, HBM-bound kernels of the type-3 NUFFT around spread / FFT / interp:
+// bounds (A5-1), source rescaling + pre-phase + bin sort (A5-2, A5-3; "sort"), deconvolution + zero padding
+// (A5-5), target rescaling + bin sort (A5-7), post-deconvolution + post-phase (A5-9).  Formulas: DESIGN.md
+// "type-3 NUFFT"; layouts: nufft3.cuh.
+#include <algorithm>
+
+#include "internal.cuh"
+#include "nufft3.cuh"
+
+namespace sfd {
+namespace {
+
+constexpr int kT = 256;
+
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, d));
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, d));
+  return v;
+}
+
+// ---- A5-1 bounds ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kT) bounds_partial_kernel(const double* __restrict__ pts, int64_t n, double* __restrict__ part) {
+  __shared__ double sm[kT / 32][6];
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double lo[3] = {inf, inf, inf}, hi[3] = {-inf, -inf, -inf};
+  for (int64_t i = (int64_t)blockIdx.x * kT + threadIdx.x; i < n; i += (int64_t)gridDim.x * kT) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double v = pts[3 * i + c];
+      lo[c] = fmin(lo[c], v);
+      hi[c] = fmax(hi[c], v);
+    }
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    lo[c] = warp_min(lo[c]);
+    hi[c] = warp_max(hi[c]);
+  }
+  if (lane == 0)
+    for (int c = 0; c < 3; ++c) {
+      sm[wid][c] = lo[c];
+      sm[wid][3 + c] = hi[c];
+    }
+  __syncthreads();
+  if (threadIdx.x < 6) {
+    double v = sm[0][threadIdx.x];
+    for (int i = 1; i < kT / 32; ++i) v = threadIdx.x < 3 ? fmin(v, sm[i][threadIdx.x]) : fmax(v, sm[i][threadIdx.x]);
+    part[blockIdx.x * 6 + threadIdx.x] = v;
+  }
+}
+__global__ void bounds_final_kernel(const double* __restrict__ part, int nblocks, double* __restrict__ out6) {
+  const int c = threadIdx.x;
+  if (c >= 6) return;
+  double v = part[c];
+  for (int i = 1; i < nblocks; ++i) v = c < 3 ? fmin(v, part[i * 6 + c]) : fmax(v, part[i * 6 + c]);
+  out6[c] = v;
+}
+
+// ---- bin keys ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+// Fine-grid coordinate of a source (A5-2).  Analytically u lies in [(w+1)/2, nf-(w+1)/2]; the clamp only guards
+// the rounding of the caller's extents, so that the w-cell footprint can never leave the grid.
+__device__ __forceinline__ double src_coord(const N3Params& p, double x, int d) {
+  const double u = __fma_rn(x - p.C[d], p.sx[d], 0.5 * p.nf[d]);
+  const double lo = 0.5 * p.w + 1e-9;
+  return fmin(fmax(u, lo), p.nf[d] - lo);
+}
+// Inner-grid coordinate of a target (A5-7): analytically in [n2/4, 3 n2/4].
+__device__ __forceinline__ double tgt_coord(const N3Params& p, double xi, int d) {
+  const double u = __fma_rn(xi - p.D[d], p.st[d], 0.5 * p.n2[d]);
+  return fmin(fmax(u, (double)p.t0[d]), (double)(p.t0[d] + p.n2[d] / 2));
+}
+
+__global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, const double* __restrict__ x, int64_t J,
+                                                        int32_t* __restrict__ key, int32_t* __restrict__ hist) {
+  const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (j >= J) return;
+  int b[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const double u = src_coord(p, x[3 * j + d], d);
+    b[d] = clampi((int)floor(u / p.bs), 0, p.nbs[d] - 1);
+  }
+  const int k = (b[0] * p.nbs[1] + b[1]) * p.nbs[2] + b[2];
+  key[j] = k;
+  atomicAdd(&hist[k], 1);
+}
+
+__global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const double* __restrict__ x, const double* __restrict__ w,
+                                                           int64_t J, const int32_t* __restrict__ key,
+                                                           const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
+                                                           SrcRec* __restrict__ out) {
+  const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (j >= J) return;
+  const int k = key[j];
+  const int pos = off[k] + atomicAdd(&cursor[k], 1);
+  SrcRec r;
+  const double x0 = x[3 * j], x1 = x[3 * j + 1], x2 = x[3 * j + 2];
+  r.u[0] = src_coord(p, x0, 0);
+  r.u[1] = src_coord(p, x1, 1);
+  r.u[2] = src_coord(p, x2, 2);
+  const double wj = w[j];
+  if (p.real_c) {
+    r.re = wj;
+    r.im = 0.0;
+  } else {
+    double s, c;
+    sincos_fp64(__fma_rn(p.D[0], x0, __fma_rn(p.D[1], x1, p.D[2] * x2)), s, c);
+    r.re = wj * c;
+    r.im = -wj * s;
+  }
+  out[pos] = r;
+}
+
+__global__ void __launch_bounds__(kT) target_keys_kernel(N3Params p, const double* __restrict__ xi, int64_t K,
+                                                        int32_t* __restrict__ key, int32_t* __restrict__ hist) {
+  const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (k >= K) return;
+  int b[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const double u = tgt_coord(p, xi[3 * k + d], d);
+    b[d] = clampi((int)floor((u - p.t0[d]) / p.bt), 0, p.nbt[d] - 1);
+  }
+  const int kk = (b[0] * p.nbt[1] + b[1]) * p.nbt[2] + b[2];
+  key[k] = kk;
+  atomicAdd(&hist[kk], 1);
+}
+
+__global__ void __launch_bounds__(kT) target_scatter_kernel(N3Params p, const double* __restrict__ xi, int64_t K,
+                                                           const int32_t* __restrict__ key, const int32_t* __restrict__ off,
+                                                           int32_t* __restrict__ cursor, TgtRec* __restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (k >= K) return;
+  const int kk = key[k];
+  const int pos = off[kk] + atomicAdd(&cursor[kk], 1);
+  TgtRec r;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) r.u[d] = tgt_coord(p, xi[3 * k + d], d);
+  r.k = k;
+  out[pos] = r;
+}
+
+// ---- work items ----------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kT) item_counts_kernel(const int32_t* __restrict__ hist, int64_t nbins, int cap,
+                                                        int32_t* __restrict__ nit) {
+  const int64_t b = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (b < nbins) nit[b] = (hist[b] + cap - 1) / cap;
+}
+__global__ void __launch_bounds__(kT) item_fill_kernel(const int32_t* __restrict__ hist, const int32_t* __restrict__ off,
+                                                      const int32_t* __restrict__ pos, int64_t nbins, int cap,
+                                                      int64_t max_items, int32_t* __restrict__ items) {
+  const int64_t b = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (b >= nbins) return;
+  const int n = hist[b];
+  int at = pos[b];
+  for (int s = 0; s < n; s += cap, ++at) {
+    items[at] = (int32_t)b;
+    items[max_items + at] = off[b] + s;
+    items[2 * max_items + at] = min(cap, n - s);
+  }
+}
+
+// ---- A5-5 deconvolution + zero padding -----------------------------------------------------------------------
+// (w/2) phihat(kappa) = sum_q f_q cos(kappa z_q)   (QuadTable: GL in theta after z = sin theta)
+__device__ __forceinline__ double half_w_phihat(const QuadTable& q, double kappa) {
+  double acc = 0.0;
+  for (int i = 0; i < q.n; ++i) acc = __fma_rn(q.f[i], cos(kappa * q.z[i]), acc);
+  return acc;
+}
+
+__global__ void __launch_bounds__(kT) deconv_tables_kernel(N3Params p, QuadTable q, double* __restrict__ dec) {
+  const int i = blockIdx.x * kT + threadIdx.x;
+  const int n0 = p.nf[0], n1 = p.nf[1], n2 = p.nf[2];
+  if (i >= n0 + n1 + n2) return;
+  const int d = i < n0 ? 0 : (i < n0 + n1 ? 1 : 2);
+  const int ii = i - (d == 0 ? 0 : (d == 1 ? n0 : n0 + n1));
+  const int l = ii - p.nf[d] / 2;
+  const double kappa = (double)l * p.w * 3.14159265358979323846 / (double)p.n2[d];
+  const double v = 1.0 / half_w_phihat(q, kappa);
+  dec[i] = (l & 1) ? -v : v;   // (-1)^l: shifts the inner grid by half a period, t_m = m h2 - pi
+}
+
+template <bool REAL>
+__global__ void __launch_bounds__(kT) deconv_pad_kernel(N3Params p, const double* __restrict__ fine,
+                                                       const double* __restrict__ dec, double2* __restrict__ inner) {
+  const int pz = blockIdx.x * kT + threadIdx.x;
+  const int py = blockIdx.y, px = blockIdx.z;
+  if (pz >= p.n2[2]) return;
+  const int lx = px < p.n2[0] / 2 ? px : px - p.n2[0];
+  const int ly = py < p.n2[1] / 2 ? py : py - p.n2[1];
+  const int lz = pz < p.n2[2] / 2 ? pz : pz - p.n2[2];
+  const int ix = lx + p.nf[0] / 2, iy = ly + p.nf[1] / 2, iz = lz + p.nf[2] / 2;
+  double2 out = make_double2(0.0, 0.0);
+  if (ix >= 0 && ix < p.nf[0] && iy >= 0 && iy < p.nf[1] && iz >= 0 && iz < p.nf[2]) {
+    const double f = dec[ix] * dec[p.nf[0] + iy] * dec[p.nf[0] + p.nf[1] + iz];
+    const size_t g = ((size_t)ix * p.nf[1] + iy) * p.nf[2] + iz;
+    if (REAL) {
+      out.x = fine[g] * f;
+    } else {
+      const double2 v = reinterpret_cast<const double2*>(fine)[g];
+      out.x = v.x * f;
+      out.y = v.y * f;
+    }
+  }
+  inner[((size_t)px * p.n2[1] + py) * p.n2[2] + pz] = out;
+}
+
+// ---- A5-9 post-deconvolution + post-phase --------------------------------------------------------------------
+__global__ void __launch_bounds__(kT) post_deconv_kernel(N3Params p, QuadTable q, const double* __restrict__ xi, int64_t K,
+                                                        double2* __restrict__ nuhat) {
+  const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (k >= K) return;
+  const double a0 = xi[3 * k] - p.D[0], a1 = xi[3 * k + 1] - p.D[1], a2 = xi[3 * k + 2] - p.D[2];
+  const double den = half_w_phihat(q, a0 * p.kap[0]) * half_w_phihat(q, a1 * p.kap[1]) * half_w_phihat(q, a2 * p.kap[2]);
+  double s, c;
+  sincos_fp64(__fma_rn(a0, p.C[0], __fma_rn(a1, p.C[1], a2 * p.C[2])), s, c);
+  const double2 g = nuhat[k];
+  const double inv = 1.0 / den;
+  // G * (c - i s) / den
+  nuhat[k] = make_double2((g.x * c + g.y * s) * inv, (g.y * c - g.x * s) * inv);
+}
+
+}  // namespace
+
+static inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kT - 1) / kT); }
+
+int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scratch, cudaStream_t st) {
+  const int nb = (int)std::min<int64_t>(kBoundsBlocks, std::max<int64_t>(1, (n + kT - 1) / kT));
+  bounds_partial_kernel<<<nb, kT, 0, st>>>(d_pts, n, d_scratch);
+  SFD_TRY(launch_check("bounds_partial_kernel"));
+  bounds_final_kernel<<<1, 32, 0, st>>>(d_scratch, nb, d_out6);
+  return launch_check("bounds_final_kernel");
+}
+
+int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st) {
+  source_keys_kernel<<<blocks_for(J), kT, 0, st>>>(p, d_x, J, d_key, d_hist);
+  return launch_check("source_keys_kernel");
+}
+int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
+                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st) {
+  source_scatter_kernel<<<blocks_for(J), kT, 0, st>>>(p, d_x, d_w, J, d_key, d_off, d_cursor, d_out);
+  return launch_check("source_scatter_kernel");
+}
+int target_keys(const N3Params& p, const double* d_xi, int64_t K, int32_t* d_key, int32_t* d_hist, cudaStream_t st) {
+  target_keys_kernel<<<blocks_for(K), kT, 0, st>>>(p, d_xi, K, d_key, d_hist);
+  return launch_check("target_keys_kernel");
+}
+int target_scatter(const N3Params& p, const double* d_xi, int64_t K, const int32_t* d_key, const int32_t* d_off,
+                   int32_t* d_cursor, TgtRec* d_out, cudaStream_t st) {
+  target_scatter_kernel<<<blocks_for(K), kT, 0, st>>>(p, d_xi, K, d_key, d_off, d_cursor, d_out);
+  return launch_check("target_scatter_kernel");
+}
+
+int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int cap, int32_t* d_tmp, int32_t* d_items,
+               int64_t max_items, int32_t* d_n_items, void* d_scan, size_t scan_bytes, cudaStream_t st) {
+  item_counts_kernel<<<blocks_for(nbins), kT, 0, st>>>(d_hist, nbins, cap, d_tmp);
+  SFD_TRY(launch_check("item_counts_kernel"));
+  SFD_TRY(exclusive_scan_i32(d_tmp, d_tmp, nbins, d_n_items, d_scan, scan_bytes, st));
+  item_fill_kernel<<<blocks_for(nbins), kT, 0, st>>>(d_hist, d_off, d_tmp, nbins, cap, max_items, d_items);
+  return launch_check("item_fill_kernel");
+}
+
+
+int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st) {
+  deconv_tables_kernel<<<blocks_for(p.nf[0] + p.nf[1] + p.nf[2]), kT, 0, st>>>(p, q, d_dec);
+  return launch_check("deconv_tables_kernel");
+}
+
+int deconv_pad(const N3Params& p, const double* d_fine, const double* d_dec, double* d_inner, cudaStream_t st) {
+  dim3 grid(blocks_for(p.n2[2]), (unsigned)p.n2[1], (unsigned)p.n2[0]);
+  if (p.real_c)
+    deconv_pad_kernel<true><<<grid, kT, 0, st>>>(p, d_fine, d_dec, reinterpret_cast<double2*>(d_inner));
+  else
+    deconv_pad_kernel<false><<<grid, kT, 0, st>>>(p, d_fine, d_dec, reinterpret_cast<double2*>(d_inner));
+  return launch_check("deconv_pad_kernel");
+}
+
+int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st) {
+  post_deconv_kernel<<<blocks_for(K), kT, 0, st>>>(p, q, d_xi, K, reinterpret_cast<double2*>(d_nuhat));
+  return launch_check("post_deconv_kernel");
+}
+
+}  // namespace sfd

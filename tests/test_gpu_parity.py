@@ -200,3 +200,30 @@ def test_surface_ft_host_entry(sfd, orc):
     nu = sfd.sfd_surface_ft_host(x, w, xi, 0.0)
     ref = orc.direct_sum(x, w, xi)
     assert np.abs(nu - ref).max() <= 1e-12 * np.abs(w).sum()
+
+
+# ---- A5 type-3 NUFFT --------------------------------------------------------------------------------
+def _nufft_case(sfd, orc, torch, x, w, xi, eps, factor=10.0):
+    nu = sfd.sfd_surface_ft(dev(torch, x), dev(torch, w), dev(torch, xi), eps).cpu().numpy()
+    ref = orc.direct_sum(x, w, xi)
+    err = np.abs(nu - ref).max() / np.abs(w).sum()
+    assert err <= factor * eps, (err, eps)
+    return err
+
+
+@pytest.mark.parametrize("eps", [1e-3, 1e-6, 1e-9, 1e-12])
+def test_nufft_config1(sfd, orc, torch, eps):
+    """Config-1 geometry (centred sources and targets: the real-strength path)."""
+    c = workloads.CONFIGS[1]
+    V, F = orc.mesh_icosphere(c["level"])
+    x, w = orc.nodes(V, F, c["rule"])
+    xi, W = orc.freq_nodes(c["n_r"], c["n_theta"], c["n_phi"], c["R"])
+    _nufft_case(sfd, orc, torch, x, w, xi, eps)
+
+
+@pytest.mark.parametrize("J,K", [(1, 1), (7, 33), (33, 7), (1000, 1000), (3000, 4097)])
+@pytest.mark.parametrize("eps", [1e-6, 1e-9, 1e-12])
+def test_nufft_random_clouds(sfd, orc, torch, J, K, eps):
+    """Off-centre sources (C != 0), off-centre targets (D != 0, complex strengths), signed weights."""
+    x, w, xi = workloads.random_cloud(J, K)
+    _nufft_case(sfd, orc, torch, x, w, xi, eps)
