@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of arXiv 2304.06340 on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl reference]
+
+A *step* is one pass of the whole hot path (every row of SURVEY.md 8(a)) on BASELINE.json's config 2 (the
+configuration the metric is quoted on; icosphere level 4, 6-pt rule, 30,720 sources, 128x64x128 = 1,048,576 ball
+quadrature nodes on [0,128]):
+
+    sfd_mesh_icosphere(level)                               A1/A2
+    for s in config.s:  sfd_weak_distance(eps = 0)          A3 + frequency nodes + A4 direct sum + A6
+    for s in config.s:  sfd_weak_distance(eps = 1e-9)       A3 + frequency nodes + A5 type-3 NUFFT + A6
+
+`value` = source.frequency pairs per second = (number of nuhat evaluations in the step) * J * K / step time, with the
+inputs resident in HBM.  `e2e` = the same through the host-buffer C-ABI calls (sfd_weak_distance_host: mesh copied
+from pinned host memory, distance copied back, inside the timed region).  `roofline` describes the dominant kernel
+(direct_sum_kernel, FP64-ALU bound); `roofline_nufft` lists the HBM-judged type-3 stages.  `cpu_baseline` times the
+oracle (oracle/, as it stands) on a bounded sample of the same workload on this box's host cores.
+Multi-GPU (torchrun): every rank evaluates its own independent mesh-vs-sphere distance (weak scaling, no data-path
+collective).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads  # noqa: E402
+
+METRIC = "source*frequency pairs/s (fp64 nuhat)"
+UNIT = "pairs/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (2 = the headline)")
+    ap.add_argument("--impl", default="sfd", choices=["sfd", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def workload(cfg_id):
+    c = workloads.CONFIGS[cfg_id]
+    level = c["level"] if isinstance(c["level"], int) else max(c["level"])
+    F = 20 * 4 ** level
+    J = F * c["rule"]
+    K = c["n_r"] * c["n_theta"] * c["n_phi"]
+    return c, level, J, K
+
+
+def config_dict(cfg_id, n_gpus):
+    c, level, J, K = workload(cfg_id)
+    return {"workload": f"BASELINE.json config {cfg_id}: icosphere level {level}, {c['rule']}-pt rule, J={J} sources; "
+                        f"ball quadrature {c['n_r']}x{c['n_theta']}x{c['n_phi']} on [0,{c['R']:g}], K={K} targets",
+            "level": level, "rule": c["rule"], "J": J, "K": K, "R": c["R"],
+            "n_r": c["n_r"], "n_theta": c["n_theta"], "n_phi": c["n_phi"], "s": list(c["s"]), "eps": list(c["eps"]),
+            "parallelism": f"{n_gpus} independent distance evaluations (one per GPU), no collective",
+            "l2": "L2 flushed (512 MiB memset) between timed steps; NUFFT grids (0.75 GB) also exceed L2"}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle, as it stands, on a bounded sample of the workload
+def oracle_sample(cfg_id, seconds, steps=1, warmup=0):
+    """Times oracle.direct_sum (+ nodes, reduce) on K_sub seeded targets x all J sources.  Returns
+    (pairs_per_s, ms_per_step, cores, sample description, K_sub)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import sfd_oracle as O
+    c, level, J, K = workload(cfg_id)
+    V, F = O.mesh_icosphere(level)
+    if c["jitter"]:
+        V = workloads.jitter_vertices(V, F, *c["jitter"])
+    x, w = O.nodes(V, F, c["rule"])
+    xi, W = O.freq_nodes(c["n_r"], c["n_theta"], c["n_phi"], c["R"])
+    cores = O.num_threads()
+    # calibrate on 64 targets, then size the sample for ~`seconds` of CPU work
+    idx = workloads.target_subset(K, 64, seed=1)
+    t0 = time.perf_counter()
+    O.direct_sum(x, w, xi[idx])
+    rate = 64 * J / (time.perf_counter() - t0)
+    k_sub = int(min(K, max(64, seconds * rate / J)))
+    idx = workloads.target_subset(K, k_sub, seed=0)
+    xs, Ws = np.ascontiguousarray(xi[idx]), np.ascontiguousarray(W[idx])
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        Vs, Fs = O.mesh_icosphere(level)
+        xo, wo = O.nodes(Vs if not c["jitter"] else V, Fs, c["rule"])
+        nu = O.direct_sum(xo, wo, xs)
+        for s in c["s"]:
+            O.reduce(nu, xs, Ws, s)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    sample = (f"oracle mesh+nodes+direct_sum+reduce on {k_sub} of {K} targets (SplitMix64 seed 0) x all {J} sources, "
+              f"{k_sub * J:.3e} pairs per step")
+    return k_sub * J / t, t * 1e3, cores, sample, k_sub
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    v, ms, cores, sample, _ = oracle_sample(args.config, per_step, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_dict(args.config, args.gpus),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU, sampled every 100 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [f.strip() for f in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "samples": len(rows),
+                "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
+
+
+def run_sfd(args):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the sfd arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2304_06340_b200 as P
+
+    c, level, J, K = workload(args.config)
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    R, rule = c["R"], c["rule"]
+    eps_list = [e for e in c["eps"]]
+    if args.config == 2:
+        eps_list = [0.0, 1e-9]
+    n_eval = len(eps_list) * len(c["s"])          # nuhat evaluations per step
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream()
+
+    # device-resident buffers, sized once (allocation is outside the timed region, like the paper's P:238)
+    nV, nF, mesh_wb = P.sfd_mesh_icosphere_sizes(level)
+    V = torch.empty((nV, 3), dtype=torch.float64, device=dev)
+    F = torch.empty((nF, 3), dtype=torch.int32, device=dev)
+    mesh_work = torch.empty(max(mesh_wb, 256), dtype=torch.uint8, device=dev)
+    ext = 1.0 + (0.0 if not c["jitter"] else 0.01)
+    wb = max(P.sfd_weak_distance_workspace(nF, rule, q, R, e, ext) for e in eps_list)
+    work = torch.empty(wb, dtype=torch.uint8, device=dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    Vj = None
+    if c["jitter"]:   # config 4: the jitter is an input (workloads.jitter_vertices), applied to the device mesh
+        V0, F0 = P.sfd_mesh_icosphere(level)
+        Vj = torch.as_tensor(workloads.jitter_vertices(V0.cpu().numpy(), F0.cpu().numpy(), *c["jitter"]), device=dev)
+
+    import ctypes as C
+    lib = P.binding._lib
+
+    def step(results=None):
+        rc = lib.sfd_mesh_icosphere(level, V.data_ptr(), F.data_ptr(), mesh_work.data_ptr(), mesh_work.numel(),
+                                    C.c_void_p(stream.cuda_stream))
+        assert rc == 0, P.binding._lib.sfd_last_error()
+        Vin = Vj if Vj is not None else V
+        for eps in eps_list:
+            for s in c["s"]:
+                d, I = P.sfd_weak_distance(Vin, F, rule, s, R, q, eps, work=work)
+                if results is not None:
+                    results[(eps, s)] = (d, I)
+                    for name, ms in P.sfd_last_stage_times():
+                        stage_ms.setdefault((eps, name), []).append(ms)
+
+    stage_ms = {}
+    sampler = ClockSampler(local)          # started before the warm-up so that it is sampling by the timed region
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    P.sfd_set_profiling(True)
+    results = {}
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = P.sfd_launch_count()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.zero_()                      # evict L2 between timed steps (outside the event pair)
+        ev[i][0].record(stream)
+        step(results)
+        ev[i][1].record(stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop(t0, t1)
+    launches = (P.sfd_launch_count() - l0) // args.steps
+    P.sfd_set_profiling(False)
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    return dict(P=P, torch=torch, dist=dist, world=world, rank=rank, dev=dev, c=c, level=level, J=J, K=K, q=q,
+                eps_list=eps_list, n_eval=n_eval, total_ms=total_ms, results=results, stage_ms=stage_ms,
+                clocks=clocks, launches=launches, V=V, F=F, Vj=Vj, nV=nV, nF=nF, ext=ext)
+
+
+# FP64-pipe instructions per source.target pair of direct_sum_kernel (checked against the SASS of
+# the inner loop): phase 1 DMUL + 2 DFMA; sincos 16 DFMA + 2 DMUL + 1 DADD; accumulate 2 DFMA.
+DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 20, 4
+FLOPS_PER_PAIR = 2 * DFMA_PER_PAIR + DMUL_DADD_PER_PAIR
+FP64_LANES_PER_SM = 64          # DFMA / clk / SM on B200 (nominal 37-40 TFLOP/s at 1.965 GHz x 148 SMs)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    r = run_sfd(args)
+    P, torch, dist = r["P"], r["torch"], r["dist"]
+    c, J, K, q = r["c"], r["J"], r["K"], r["q"]
+    world, rank = r["world"], r["rank"]
+
+    # ---- e2e: the same step through the host-buffer entry point (pinned host mesh in, distance out) ----------
+    Vh = (r["Vj"] if r["Vj"] is not None else r["V"]).cpu().pin_memory()
+    Fh = r["F"].cpu().pin_memory()
+    Vn, Fn = Vh.numpy(), Fh.numpy()
+
+    def e2e_step():
+        for eps in r["eps_list"]:
+            for s in c["s"]:
+                P.sfd_weak_distance_host(Vn, Fn, c["rule"], s, c["R"], q, eps)
+
+    for _ in range(2):
+        e2e_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3)   # host-blocking calls: take the wall clock
+
+    t = torch.tensor([r["total_ms"], e2e_ms], dtype=torch.float64, device=r["dev"])
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    n_eval = r["n_eval"]
+    pairs_per_step = n_eval * J * K * world
+    ms_per_step = total_ms / args.steps
+    value = pairs_per_step / (ms_per_step * 1e-3)
+    e2e_value = pairs_per_step / (e2e_ms / args.steps * 1e-3)
+    n_dist = len(r["eps_list"]) * len(c["s"])
+
+    # ---- per-stage device times (CUDA events recorded by the library on the launching stream) -------------------
+    stages = {}
+    for (eps, name), v in r["stage_ms"].items():
+        stages.setdefault("direct" if eps == 0.0 else f"nufft_{eps:g}", {})[name] = float(np.mean(v))
+    ms_dist = {k: sum(v.values()) for k, v in stages.items()}
+
+    # ---- roofline of the dominant kernel ----------------------------------------------------------------------
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    hbm_peak, hbm_src = (peaks["hbm_gbs"], "MEASURED_PEAKS.json") if "hbm_gbs" in peaks else (6650.0, "fallback")
+    fp64_tf, _ = P.sfd_probe_fp64(8192)
+    sm_mhz = r["clocks"].get("sm_mhz") or 1965.0
+    roofline, extra = None, []
+    if "direct" in stages:
+        dms = stages["direct"]["direct_sum"]
+        ach = FLOPS_PER_PAIR * J * K / (dms * 1e-3) * 1e-12
+        roofline = {"kernel": "direct_sum_kernel", "bound": "alu", "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s",
+                    "frac": ach / fp64_tf, "traffic": None,
+                    "peak_source": "measured live by sfd_probe_fp64 (dependency-free DFMA loop on all SMs)",
+                    "peak_derived": 2 * FP64_LANES_PER_SM * 148 * sm_mhz * 1e6 * 1e-12,
+                    "pipe_frac": (DFMA_PER_PAIR + DMUL_DADD_PER_PAIR) * J * K / (dms * 1e-3) /
+                                 (fp64_tf * 1e12 / 2),
+                    "ms_per_launch": dms, "pairs_per_s": J * K / (dms * 1e-3),
+                    "flops_per_pair": FLOPS_PER_PAIR}
+    for eps in r["eps_list"]:
+        if eps == 0.0:
+            continue
+        st = stages[f"nufft_{eps:g}"]
+        w, nf, n2 = P.sfd_surface_ft_plan(J, K, [r["ext"]] * 3, [c["R"]] * 3, eps)
+        cell = 8      # ball-centred targets: real strengths, real fine grid
+        fine = nf[0] * nf[1] * nf[2] * cell
+        band = 1
+        for d in range(3):
+            band *= n2[d] // 2 + w + 1
+        sp_bytes = 2 * fine + 40 * J            # zero-fill + one accumulation pass of the grid + sorted sources
+        ip_bytes = 16 * band + (32 + 16) * K    # the band of the inner grid that holds targets, records in, G out
+        for name, nbytes in (("spread", sp_bytes), ("interp", ip_bytes)):
+            ach = nbytes / (st[name] * 1e-3) * 1e-9
+            extra.append({"kernel": f"{name}_kernel", "eps": eps, "w": w, "nf": nf[0], "n2": n2[0], "bound": "hbm",
+                          "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                          "ms_per_launch": st[name], "algorithmic_bytes": nbytes, "peak_source": hbm_src})
+        if roofline is None:
+            roofline = dict(extra[-1], traffic=None)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(args.config, world),
+            "clocks": r["clocks"],
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                    "h2d_bytes_per_step": n_dist * (Vn.nbytes + Fn.nbytes), "d2h_bytes_per_step": n_dist * 16,
+                    "api": "sfd_weak_distance_host"},
+            "gpu_launches": r["launches"],
+            "roofline": roofline, "roofline_nufft": extra,
+            "ms_per_distance": ms_dist, "stage_ms": stages,
+            "equivalent_pairs_per_s": {k: J * K / (v * 1e-3) for k, v in ms_dist.items()},
+            "distance": {f"eps={e:g},s={s:g}": d for (e, s), (d, _) in r["results"].items()}}
+    if not args.no_cpu_baseline and world == 1:
+        v, ms, cores, sample, _ = oracle_sample(args.config, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                "ms": ms}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

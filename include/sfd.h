@@ -95,6 +95,10 @@ int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi /
  * extents need more than work_bytes, the call fails with SFD_ERR_WORKSPACE_TOO_SMALL and writes
  * nothing. */
 int sfd_surface_ft_workspace(int64_t J, int64_t K, const double X[3], const double S[3], double eps, size_t* bytes);
+/* What the type-3 transform would use for these extents: kernel width w (cells), fine (spreading) grid nf[3] and
+ * inner FFT grid n2[3].  Host only; any output may be NULL. */
+int sfd_surface_ft_plan(int64_t J, int64_t K, const double X[3], const double S[3], double eps, int32_t* w,
+                        int64_t nf[3], int64_t n2[3]);
 int sfd_surface_ft(const double* d_x /*[J][3]*/, const double* d_w /*[J]*/, int64_t J,
                    const double* d_xi /*[K][3]*/, int64_t K, double eps, double* d_nuhat /*[K][2]*/,
                    void* d_work, size_t work_bytes, sfd_stream stream);
@@ -133,6 +137,15 @@ int sfd_weak_distance_host(const double* h_vertices, int64_t nV, const int32_t* 
  * strings; returns the number of stages written (<= max). */
 int sfd_set_profiling(int on);
 int sfd_last_stage_times(const char** names, float* ms, int max);
+
+/* Number of kernels of this library launched so far by the process (cuFFT's own kernels are not counted). */
+long long sfd_launch_count(void);
+
+/* ---- roofline denominator of A4 ------------------------------------------------------------------
+ * Runs a dependency-free DFMA loop (8 independent chains per thread, `iters` x 64 FMAs per chain-step,
+ * one persistent CTA set covering every SM) and reports the achieved FP64 throughput in TFLOP/s
+ * (FMA = 2 flops) and the kernel time in ms.  Synchronises `stream`.  iters in [1, 1<<20]. */
+int sfd_probe_fp64(int iters, sfd_stream stream, double* h_tflops, double* h_ms);
 
 #ifdef __cplusplus
 }

@@ -46,6 +46,7 @@ _SIGS = {
     "sfd_freq_nodes_workspace": (C.c_int, [_P(sfd_freq_quadrature), _P(_sz)]),
     "sfd_freq_nodes_device": (C.c_int, [_P(sfd_freq_quadrature), _dbl, _vp, _vp, _vp, _sz, _vp]),
     "sfd_surface_ft_workspace": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(_sz)]),
+    "sfd_surface_ft_plan": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(C.c_int32), _P(_i64), _P(_i64)]),
     "sfd_surface_ft": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp, _vp, _sz, _vp]),
     "sfd_reduce_workspace": (C.c_int, [_i64, _P(_sz)]),
     "sfd_reduce": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
@@ -55,6 +56,8 @@ _SIGS = {
     "sfd_surface_ft_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp]),
     "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
                                          _P(_dbl), _P(_dbl)]),
+    "sfd_launch_count": (C.c_longlong, []),
+    "sfd_probe_fp64": (C.c_int, [C.c_int, _vp, _P(_dbl), _P(_dbl)]),
     "sfd_set_profiling": (C.c_int, [C.c_int]),
     "sfd_last_stage_times": (C.c_int, [_P(C.c_char_p), _P(C.c_float), C.c_int]),
 }
@@ -164,6 +167,14 @@ def sfd_surface_ft_workspace(J, K, X, S, eps):
     return wb.value
 
 
+def sfd_surface_ft_plan(J, K, X, S, eps):
+    """(w, nf[3], n2[3]) of the type-3 transform for sources / targets of half-widths X / S."""
+    w, nf, n2 = C.c_int32(), (_i64 * 3)(), (_i64 * 3)()
+    Xa, Sa = (_dbl * 3)(*[float(v) for v in X]), (_dbl * 3)(*[float(v) for v in S])
+    _chk(_lib.sfd_surface_ft_plan(int(J), int(K), Xa, Sa, float(eps), C.byref(w), nf, n2))
+    return w.value, list(nf), list(n2)
+
+
 def _half_widths(t):
     if t.shape[0] == 0:
         return [0.0, 0.0, 0.0]
@@ -253,3 +264,14 @@ def sfd_last_stage_times():
     ms = (C.c_float * 32)()
     n = _lib.sfd_last_stage_times(names, ms, 32)
     return [(names[i].decode(), float(ms[i])) for i in range(n)]
+
+
+def sfd_launch_count():
+    return int(_lib.sfd_launch_count())
+
+
+def sfd_probe_fp64(iters=4096):
+    """(TFLOP/s, ms) of a dependency-free DFMA loop on every SM: the measured FP64 peak."""
+    tf, ms = _dbl(), _dbl()
+    _chk(_lib.sfd_probe_fp64(int(iters), _stream(), C.byref(tf), C.byref(ms)))
+    return tf.value, ms.value

@@ -9,6 +9,7 @@
 namespace sfd {
 
 static thread_local char g_err[512] = "";
+long long g_launches = 0;
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -99,6 +100,12 @@ int sfd_release_cache(void) {
   return nufft3_release_cache();
 }
 
+long long sfd_launch_count(void) { return g_launches; }
+
+int sfd_probe_fp64(int iters, sfd_stream stream, double* h_tflops, double* h_ms) {
+  return probe_fp64(iters, as_stream(stream), h_tflops, h_ms);
+}
+
 int sfd_set_profiling(int on) {
   g_prof.on = on != 0;
   g_prof.n_done = 0;
@@ -182,6 +189,22 @@ int sfd_surface_ft_workspace(int64_t J, int64_t K, const double X[3], const doub
   Nufft3Sizes sz;
   SFD_TRY(nufft3_sizes(J, K, X, S, eps, &sz));
   *bytes = sz.work_bytes;
+  return SFD_OK;
+}
+
+int sfd_surface_ft_plan(int64_t J, int64_t K, const double X[3], const double S[3], double eps, int32_t* w,
+                        int64_t nf[3], int64_t n2[3]) {
+  SFD_REQUIRE(X && S, SFD_ERR_NULL, "sfd_surface_ft_plan: X and S are required");
+  SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
+  SFD_TRY(check_eps(eps));
+  SFD_REQUIRE(eps > 0.0, SFD_ERR_INVALID_ARG, "sfd_surface_ft_plan: eps must be > 0 (the direct sum has no plan)");
+  Nufft3Sizes sz;
+  SFD_TRY(nufft3_sizes(J, K, X, S, eps, &sz));
+  if (w) *w = sz.w;
+  for (int d = 0; d < 3; ++d) {
+    if (nf) nf[d] = sz.nf[d];
+    if (n2) n2[d] = sz.n2[d];
+  }
   return SFD_OK;
 }
 

@@ -37,7 +37,11 @@ void set_error(const char* fmt, ...);
     }                                \
   } while (0)
 
+// number of kernels of this library launched so far in the process (sfd_launch_count)
+extern long long g_launches;
+
 inline int launch_check(const char* what) {
+  ++g_launches;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     set_error("launch of %s failed: %s", what, cudaGetErrorString(e));

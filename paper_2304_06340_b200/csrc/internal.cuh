@@ -42,6 +42,9 @@ size_t reduce_workspace(int64_t K);
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
                    size_t work_bytes, cudaStream_t st, double** d_result);
 
+// ---- probe.cu: measured FP64 FMA peak of the device (the direct sum's roofline denominator) ----------
+int probe_fp64(int iters, cudaStream_t st, double* h_tflops, double* h_ms);
+
 // ---- nufft3.cu: A5 three-dimensional type-3 nonuniform FFT -------------------------------
 struct Nufft3Sizes {
   int w;               // kernel width in fine-grid cells
