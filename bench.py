@@ -246,8 +246,9 @@ def run_sfd(args):
 
 
 # FP64-pipe instructions per source.target pair of direct_sum_kernel (checked against the SASS of
-# the inner loop): phase 1 DMUL + 2 DFMA; sincos 16 DFMA + 2 DMUL + 1 DADD; accumulate 2 DFMA.
-DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 20, 4
+# the inner loop: 120 DFMA + 24 DMUL + 24 DADD per 8 pairs): phase 1 DMUL + 2 DFMA; quarter-turn reduction 3 DADD;
+# z 1 DMUL; sin 5 DFMA + 1 DMUL; cos 6 DFMA; accumulate 2 DFMA.
+DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 15, 6
 FLOPS_PER_PAIR = 2 * DFMA_PER_PAIR + DMUL_DADD_PER_PAIR
 FP64_LANES_PER_SM = 64          # DFMA / clk / SM on B200 (nominal 37-40 TFLOP/s at 1.965 GHz x 148 SMs)
 

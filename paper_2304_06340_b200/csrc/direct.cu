@@ -45,6 +45,43 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                : "memory");
 }
 
+// sin and cos of (pi/2) tq for the inner loop: the targets are pre-scaled by 2/pi once per thread, so the phase
+// arrives in quarter turns and the range reduction is three exact additions (n = rint(tq) by the 1.5*2^52 trick,
+// f = tq - n in [-1/2, 1/2] exactly); sin(pi/2 f) = f S(f^2), cos(pi/2 f) = C(f^2) with 6 / 7 coefficients
+// (gen_sincos_coeffs.py qturn: max error 3.8e-15 / 1.8e-16, far below the 1e-12 sum|w| bar and below the rounding of
+// the phase itself, ~|tq| 2^-52).  14 FP64-pipe instructions + the quadrant fix-up on the integer pipe.
+// Coefficients live in the constant bank and are used as direct c[3][..] operands: measured 2 % faster than
+// immediates, which ptxas re-materialises into uniform registers inside the loop (every non-FP64 instruction costs
+// an issue cycle next to a 2-cycle DFMA; profiles/r1b_direct_sum.md).
+__constant__ double c_sc[14] = {
+    -3.55553766329449158383e-6, 1.60428782872071630554e-4, -4.68175249674726216909e-3, 7.96926261482708977477e-2,
+    -6.45964097504106775201e-1, 1.57079632679488904148,                                  // S5..S0
+    4.65418527335501644036e-7, -2.52000581168362530624e-5, 9.19259930116159750314e-4, -2.08634807325982068569e-2,
+    2.53669507899741166079e-1, -1.23370055013614900029, 0.999999999999999945803,         // C6..C0
+    6755399441055744.0};                                                                 // 1.5 * 2^52
+__device__ __forceinline__ void sincos_qturn(double tq, double& s, double& c) {
+  const double nm = __dadd_rn(tq, c_sc[13]);
+  const int q = __double2loint(nm);
+  const double n = __dsub_rn(nm, c_sc[13]);
+  const double f = __dsub_rn(tq, n);
+  const double z = f * f;
+  double ps = c_sc[0];
+#pragma unroll
+  for (int i = 1; i <= 5; ++i) ps = __fma_rn(ps, z, c_sc[i]);
+  const double sr = f * ps;
+  double pc = c_sc[6];
+#pragma unroll
+  for (int i = 7; i <= 11; ++i) pc = __fma_rn(pc, z, c_sc[i]);
+  const double cr = __fma_rn(pc, z, c_sc[12]);
+  // quadrant: q&1 swaps, sign of sin flips for q&2, sign of cos flips for (q+1)&2
+  const double so = (q & 1) ? cr : sr;
+  const double co = (q & 1) ? sr : cr;
+  const int shi = __double2hiint(so) ^ ((q & 2) << 30);
+  const int chi = __double2hiint(co) ^ (((q + 1) & 2) << 30);
+  s = __hiloint2double(shi, __double2loint(so));
+  c = __hiloint2double(chi, __double2loint(co));
+}
+
 struct __align__(16) Stage {
   double x[kTile * 3];
   double w[kTile];
@@ -66,9 +103,10 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
 #pragma unroll
   for (int t = 0; t < T; ++t) {
     const int64_t k = min(k0 + t * kThreads + tid, K - 1);
-    a0[t] = xi[3 * k];
-    a1[t] = xi[3 * k + 1];
-    a2[t] = xi[3 * k + 2];
+    const double kTwoOverPi = 6.36619772367581382433e-01;
+    a0[t] = xi[3 * k] * kTwoOverPi;   // phases in quarter turns (sincos_qturn)
+    a1[t] = xi[3 * k + 1] * kTwoOverPi;
+    a2[t] = xi[3 * k + 2] * kTwoOverPi;
     re[t] = 0.0;
     im[t] = 0.0;
   }
@@ -112,7 +150,7 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
       for (int u = 0; u < T; ++u) {
         const double th = __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
         double sn, cs;
-        sincos_fp64(th, sn, cs);
+        sincos_qturn(th, sn, cs);
         re[u] = __fma_rn(wj, cs, re[u]);
         im[u] = __fma_rn(wj, sn, im[u]);
       }
@@ -136,18 +174,55 @@ __global__ void combine_splits_kernel(const double* __restrict__ part, int nspli
   out[i] = acc;
 }
 
+// Resident CTAs per SM of direct_sum_kernel<T> (registers bind: 6 / 10 / 16 with the current build); queried from
+// the runtime once, with those numbers as the fallback when there is no device (workspace queries on a CPU box).
+int ctas_per_sm(int T) {
+  static int cache[5] = {0, 0, 0, 0, 0};
+  if (cache[T] == 0) {
+    int n = 0;
+    cudaError_t e = cudaErrorUnknown;
+    if (T == 4) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<4>, kThreads, 0);
+    if (T == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<2>, kThreads, 0);
+    if (T == 1) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<1>, kThreads, 0);
+    if (e != cudaSuccess || n <= 0) {
+      cudaGetLastError();
+      return T == 4 ? 6 : (T == 2 ? 10 : 16);
+    }
+    cache[T] = n;
+  }
+  return cache[T];
+}
+
 }  // namespace
 
 DirectPlan direct_plan(int64_t J, int64_t K) {
   DirectPlan p;
   const int64_t sms = num_sms();
-  p.T = K >= sms * kThreads * 4 * 6 ? 4 : (K >= sms * kThreads * 2 * 4 ? 2 : 1);
+  p.T = K >= sms * kThreads * 4 * 2 ? 4 : (K >= sms * kThreads * 2 * 2 ? 2 : 1);
   p.blocks_k = (K + (int64_t)kThreads * p.T - 1) / ((int64_t)kThreads * p.T);
-  // few target tiles (small K): split the sources over gridDim.y so that every SM has work
+  // The CTAs are equal pieces of work and the SMs hold `slots` of them at a time: blocks_k * nsplit CTAs run in
+  // ceil(blocks_k * nsplit / slots) waves, the last one partly empty.  Split the sources over gridDim.y so that
+  // (a) every slot has work when K is small and (b) the last wave is nearly full (config 2: 2048 CTAs on 888 slots
+  // are 2.31 waves, 77 % efficient; split in 3 they are 6.92 waves, 98.8 %).
+  const int64_t slots = sms * ctas_per_sm(p.T);
   const int64_t tiles = std::max<int64_t>(1, (J + kTile - 1) / kTile);
-  const int64_t want = (4 * sms + p.blocks_k - 1) / std::max<int64_t>(1, p.blocks_k);
-  const int64_t nsplit = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(want, tiles), 64));
-  const int64_t tiles_per = (tiles + nsplit - 1) / nsplit;
+  const int64_t max_split = std::min<int64_t>(tiles, 32);
+  int64_t best = 1;
+  double best_eff = 0.0;
+  for (int64_t n = 1; n <= max_split; ++n) {
+    const int64_t tiles_per = (tiles + n - 1) / n;
+    const int64_t n_eff = (tiles + tiles_per - 1) / tiles_per;   // splits that actually get sources
+    if (n_eff != n) continue;
+    const double waves = (double)(p.blocks_k * n) / (double)slots;
+    // uneven source split: the longest split sets the pace
+    const double eff = waves / std::ceil(waves) * ((double)tiles / (double)(tiles_per * n));
+    if (eff > best_eff + 0.02) {   // a further split must pay for its extra partial-sum traffic
+      best_eff = eff;
+      best = n;
+    }
+    if (best_eff >= 0.97) break;
+  }
+  const int64_t tiles_per = (tiles + best - 1) / best;
   p.j_per_split = tiles_per * kTile;
   p.nsplit = (int)std::max<int64_t>(1, (J + p.j_per_split - 1) / p.j_per_split);
   p.work_bytes = p.nsplit > 1 ? align_up((size_t)p.nsplit * (size_t)K * 16) : 0;

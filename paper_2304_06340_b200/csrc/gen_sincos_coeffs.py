@@ -68,5 +68,62 @@ def main():
     print("max |sin err| = %s, max |cos err| = %s (fp64 Horner without FMA, sampled)" % (mp.nstr(es, 3), mp.nstr(ec, 3)))
 
 
+
+
+# ---------------------------------------------------------------------------------------------
+# Quarter-turn form used by the direct sum's inner loop (csrc/direct.cu, sincos_qturn):
+#     sin(pi/2 f) = f S(f^2),  cos(pi/2 f) = C(f^2),  |f| <= 1/2,
+# S with 6 and C with 7 coefficients (Chebyshev-node interpolants on [0, (0.505)^2]).
+# Run: python gen_sincos_coeffs.py qturn
+def qturn():
+    H = mp.pi / 2
+    zmax = (mp.mpf("0.505")) ** 2
+
+    def f_s(z):
+        if z == 0:
+            return H
+        f = mp.sqrt(z)
+        return mp.sin(H * f) / f
+
+    def f_c(z):
+        return mp.cos(H * mp.sqrt(z))
+
+    def interp(f, n):
+        zs = [zmax / 2 * (1 + mp.cos(mp.pi * (2 * i + 1) / (2 * n))) for i in range(n)]
+        A = mp.matrix(n, n)
+        b = mp.matrix(n, 1)
+        for i, z in enumerate(zs):
+            for j in range(n):
+                A[i, j] = z ** j
+            b[i] = f(z)
+        return list(mp.lu_solve(A, b))
+
+    S = interp(f_s, 6)
+    Cc = interp(f_c, 7)
+    print("// S0..S5 (ascending powers of z = f^2)")
+    for c in S:
+        print("  %s," % mp.nstr(c, 21))
+    print("// C0..C6")
+    for c in Cc:
+        print("  %s," % mp.nstr(c, 21))
+    Sd, Cd = [float(c) for c in S], [float(c) for c in Cc]
+    f = np.linspace(-0.5, 0.5, 200001)
+    z = f * f
+    ps = np.full_like(f, Sd[-1])
+    for k in range(len(Sd) - 2, -1, -1):
+        ps = ps * z + Sd[k]
+    pc = np.full_like(f, Cd[-1])
+    for k in range(len(Cd) - 2, -1, -1):
+        pc = pc * z + Cd[k]
+    s = f * ps
+    es = max(abs(mp.mpf(float(a)) - mp.sin(H * mp.mpf(float(b)))) for a, b in zip(s[::97], f[::97]))
+    ec = max(abs(mp.mpf(float(a)) - mp.cos(H * mp.mpf(float(b)))) for a, b in zip(pc[::97], f[::97]))
+    print("qturn: max |sin err| = %s, max |cos err| = %s" % (mp.nstr(es, 3), mp.nstr(ec, 3)))
+
+
 if __name__ == "__main__":
-    main()
+    import sys
+    if "qturn" in sys.argv:
+        qturn()
+    else:
+        main()
