@@ -2,40 +2,59 @@
 // its adjoint").  G_k = sum over the w^3 cells m around t_k of v[m] psi2(m h2 - t_k), the gather twin of the
 // spreading step: same kernel, no write conflicts.
 //
-// One persistent CTA per SM pulls work items (an occupied target bin or a slice of one) from a device-side queue,
-// stages the bin's padded subgrid (bt+w)^3 of the inner grid in shared memory as complex128 (16 B LDG/STS) and
-// lets each of its 16 warps gather one target at a time: the 32 lanes cover the w x w cells of an x-plane, walk
-// the w planes accumulating v * kx in registers, weight by ky kz at the end and finish with a warp-shuffle sum.
+// Roofline: every target reads w^3 complex128 cells = 16 w^3 bytes of shared memory and does 2 w^3 DFMAs; at
+// 128 B/clk/SM of shared-memory bandwidth against 64 DFMA/clk/SM the gather is shared-memory-bandwidth bound by 4x
+// (w = 10: 125 clk per target and SM), far above its HBM traffic (the band of the inner grid, read once per bin).
+// The kernel is built to sit on that bound:
+//   * one persistent CTA per SM pulls work items (a target bin, or a slice of <= kTgtCap targets of one) from a
+//     device-side queue and stages the bin's padded subgrid (bt+w cells per axis) in shared memory as complex128;
+//   * the z extent of a bin is 8 or 16 cells, so the row pitch Pz = bt_z + w is congruent to w modulo 8 and the
+//     flattened (y,z) cell index c = y w + z lands in bank group c mod 8: any 8 consecutive lanes of an LDS.128 hit 8
+//     distinct 16-byte bank groups -- no bank conflicts for any w;
+//   * each of the 16 warps gathers one target at a time: the 32 lanes cover the w x w cells of an x-plane
+//     (ceil(w^2/32) cells per lane, fixed for the whole kernel), walk the w planes accumulating v * kx in registers,
+//     weight by ky kz at the end and finish with a warp-shuffle sum;
+//   * the 3w kernel values of a target are piecewise polynomials (nufft3.cuh footprint()) whose coefficients live
+//     in registers: lane i (mod 16) owns interval i, lanes 0-15 evaluate x then z, lanes 16-31 evaluate y;
+//   * w is a template parameter: plane loop, cell map and polynomial degree are compile-time.
 #include "nufft3.cuh"
 
 namespace sfd {
 namespace {
 
 constexpr int kWarps = 16;
-constexpr int kMaxCellsPerLane = (kMaxW * kMaxW + 31) / 32;
-constexpr int kMaxP = 23;  // 23^3 * 16 B = 195 KB
+constexpr int kSmemCells = 13700;   // complex128 cells of the subgrid: 219,200 B (+ 6 KB of kernel tables)
 
+template <int W>
 __global__ void __launch_bounds__(32 * kWarps, 1)
-interp_kernel(N3Params p, const double2* __restrict__ v, const TgtRec* __restrict__ tgt,
+interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __restrict__ v, const TgtRec* __restrict__ tgt,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
               const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
               int32_t* __restrict__ counter, double2* __restrict__ G) {
+  constexpr int DEG = W + 3;
+  constexpr int NCL = (W * W + 31) / 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double (*ktab)[3][kMaxW] = reinterpret_cast<double (*)[3][kMaxW]>(smem_raw);
-  double2* sub = reinterpret_cast<double2*>(smem_raw + sizeof(double) * kWarps * 3 * kMaxW);
+  double (*ktab)[3][16] = reinterpret_cast<double (*)[3][16]>(smem_raw);
+  double2* sub = reinterpret_cast<double2*>(smem_raw + sizeof(double) * kWarps * 3 * 16);
   __shared__ int s_item;
 
-  const int w = p.w, P = p.bt + w, fw = w / 2;
-  const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-  const int ncell = P * P * P;
+  const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, li = lane & 15;
+  const int Px = p.bt[0] + W, Py = p.bt[1] + W, Pz = p.bt[2] + W;
+  const int plane = Py * Pz;
 
-  int cy[kMaxCellsPerLane], cz[kMaxCellsPerLane];
-  const int ncl = (w * w + 31) / 32;
+  // the polynomial of interval li, in registers
+  double pc[DEG + 1];
 #pragma unroll
-  for (int i = 0; i < kMaxCellsPerLane; ++i) {
-    const int c = lane + 32 * i;
-    cy[i] = c < w * w ? c / w : -1;
-    cz[i] = c < w * w ? c % w : 0;
+  for (int q = 0; q <= DEG; ++q) pc[q] = li < W ? ptab[q * kPolyStride + li] : 0.0;
+
+  // the lane's cells of a W x W plane: c = lane + 32 i -> (cy, cz); offset inside the plane cy Pz + cz
+  int off[NCL], cy[NCL], cz[NCL];
+#pragma unroll
+  for (int i = 0; i < NCL; ++i) {
+    const int c = min(lane + 32 * i, W * W - 1);
+    cy[i] = c / W;
+    cz[i] = c - cy[i] * W;
+    off[i] = cy[i] * Pz + cz[i];
   }
 
   const int total = *n_items;
@@ -48,41 +67,56 @@ interp_kernel(N3Params p, const double2* __restrict__ v, const TgtRec* __restric
     const int bin = item_bin[item];
     const int start = item_start[item], count = item_count[item];
     const int bz = bin % p.nbt[2], by = (bin / p.nbt[2]) % p.nbt[1], bx = bin / (p.nbt[2] * p.nbt[1]);
-    const int o[3] = {p.t0[0] + bx * p.bt - fw, p.t0[1] + by * p.bt - fw, p.t0[2] + bz * p.bt - fw};
+    const int ox = p.t0[0] + bx * p.bt[0] - W / 2, oy = p.t0[1] + by * p.bt[1] - W / 2, oz = p.t0[2] + bz * p.bt[2] - W / 2;
 
-    for (int i = tid; i < ncell; i += 32 * kWarps) {
-      const int iz = i % P, iy = (i / P) % P, ix = i / (P * P);
-      const int gx = o[0] + ix, gy = o[1] + iy, gz = o[2] + iz;
-      double2 val = make_double2(0.0, 0.0);
-      if (gx >= 0 && gy >= 0 && gz >= 0 && gx < p.n2[0] && gy < p.n2[1] && gz < p.n2[2])
-        val = v[((size_t)gx * p.n2[1] + gy) * p.n2[2] + gz];
-      sub[i] = val;
+    // stage the subgrid: one (x,y) row of Pz <= 32 cells per warp pass, 16 B per lane, coalesced along z
+    for (int row = wq; row < Px * Py; row += kWarps) {
+      const int ix = row / Py, iy = row - ix * Py;
+      const int gx = ox + ix, gy = oy + iy, gz = oz + lane;
+      if (lane < Pz) {
+        double2 val = make_double2(0.0, 0.0);
+        if (gx >= 0 && gy >= 0 && gz >= 0 && gx < p.n2[0] && gy < p.n2[1] && gz < p.n2[2])
+          val = v[((size_t)gx * p.n2[1] + gy) * p.n2[2] + gz];
+        sub[row * Pz + lane] = val;
+      }
     }
     __syncthreads();
 
+    TgtRec r = tgt[start + min(wq, count - 1)];
     for (int t = wq; t < count; t += kWarps) {
-      const TgtRec r = tgt[start + t];
-      int i0[3];
+      const TgtRec cur = r;
+      if (t + kWarps < count) r = tgt[start + t + kWarps];   // prefetch the warp's next target
+      // kernel values: lanes 0-15 do x then z, lanes 16-31 do y
+      int i0x, i0y, i0z;
+      double sx, sy, sz;
+      footprint(cur.u[0], W, i0x, sx);
+      footprint(cur.u[1], W, i0y, sy);
+      footprint(cur.u[2], W, i0z, sz);
+      const double s1 = lane < 16 ? sx : sy;
+      double k1 = pc[DEG], k2 = pc[DEG];
 #pragma unroll
-      for (int d = 0; d < 3; ++d) i0[d] = (int)ceil(r.u[d] - 0.5 * w);
-      __syncwarp();
-      for (int e = lane; e < 3 * w; e += 32) {
-        const int d = e / w, i = e - d * w;
-        const double ud = d == 0 ? r.u[0] : (d == 1 ? r.u[1] : r.u[2]);
-        const int id = d == 0 ? i0[0] : (d == 1 ? i0[1] : i0[2]);
-        ktab[wq][d][i] = es_kernel(((double)(id + i) - ud) * (2.0 / w), p.beta);
+      for (int q = DEG - 1; q >= 0; --q) {
+        k1 = __fma_rn(k1, s1, pc[q]);
+        k2 = __fma_rn(k2, sz, pc[q]);
+      }
+      __syncwarp();   // the previous target's reads of ktab are done
+      if (li < W) {
+        ktab[wq][lane < 16 ? 0 : 1][li] = k1;
+        if (lane < 16) ktab[wq][2][li] = k2;
       }
       __syncwarp();
-      double are[kMaxCellsPerLane], aim[kMaxCellsPerLane];
+
+      double are[NCL], aim[NCL];
 #pragma unroll
-      for (int i = 0; i < kMaxCellsPerLane; ++i) are[i] = aim[i] = 0.0;
-      const int base = ((i0[0] - o[0]) * P + (i0[1] - o[1])) * P + (i0[2] - o[2]);
-      for (int a = 0; a < w; ++a) {
+      for (int i = 0; i < NCL; ++i) are[i] = aim[i] = 0.0;
+      const double2* base = sub + ((i0x - ox) * Py + (i0y - oy)) * Pz + (i0z - oz);
+#pragma unroll
+      for (int a = 0; a < W; ++a) {
         const double kx = ktab[wq][0][a];
 #pragma unroll
-        for (int i = 0; i < kMaxCellsPerLane; ++i) {
-          if (i < ncl && cy[i] >= 0) {
-            const double2 c = sub[base + (a * P + cy[i]) * P + cz[i]];
+        for (int i = 0; i < NCL; ++i) {
+          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
+            const double2 c = base[a * plane + off[i]];
             are[i] = __fma_rn(c.x, kx, are[i]);
             aim[i] = __fma_rn(c.y, kx, aim[i]);
           }
@@ -90,8 +124,8 @@ interp_kernel(N3Params p, const double2* __restrict__ v, const TgtRec* __restric
       }
       double re = 0.0, im = 0.0;
 #pragma unroll
-      for (int i = 0; i < kMaxCellsPerLane; ++i) {
-        if (i < ncl && cy[i] >= 0) {
+      for (int i = 0; i < NCL; ++i) {
+        if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
           const double kyz = ktab[wq][1][cy[i]] * ktab[wq][2][cz[i]];
           re = __fma_rn(are[i], kyz, re);
           im = __fma_rn(aim[i], kyz, im);
@@ -102,35 +136,69 @@ interp_kernel(N3Params p, const double2* __restrict__ v, const TgtRec* __restric
         re += __shfl_xor_sync(0xffffffffu, re, d);
         im += __shfl_xor_sync(0xffffffffu, im, d);
       }
-      if (lane == 0) G[r.k] = make_double2(re, im);
+      if (lane == 0) G[cur.k] = make_double2(re, im);
     }
   }
 }
 
-}  // namespace
-
-int interp_max_bin(int w) { return kMaxP - w; }
-
-size_t interp_smem_bytes(const N3Params& p) {
-  const size_t P = p.bt + p.w;
-  return sizeof(double) * kWarps * 3 * kMaxW + P * P * P * 16;
+template <int W>
+int launch(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
+           const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
+           double* d_G, size_t smem, cudaStream_t st) {
+  static bool attr = false;
+  if (!attr) {
+    SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
+    attr = true;
+  }
+  interp_kernel<W><<<num_sms(), 32 * kWarps, smem, st>>>(p, d_ptab, reinterpret_cast<const double2*>(d_v), d_tgt,
+                                                        d_item_bin, d_item_start, d_item_count, d_n_items, d_counter,
+                                                        reinterpret_cast<double2*>(d_G));
+  return launch_check("interp_kernel");
 }
 
-int interp(const N3Params& p, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
+}  // namespace
+
+// Target-bin shape: z extent 8 or 16 (conflict-free pitch), x and y as large as the shared-memory budget allows;
+// the shape with the best owned-cells / staged-cells ratio wins.
+void interp_bins(int w, int bt[3]) {
+  double best = -1.0;
+  for (int bz = 8; bz <= 16; bz += 8) {
+    const int pz = bz + w;
+    int m = 1;
+    while ((m + 1) * (m + 1) * pz <= kSmemCells) ++m;
+    const int b = m - w;
+    if (b < 1) continue;
+    const double ratio = (double)b * b * bz / ((double)m * m * pz);
+    if (ratio > best) {
+      best = ratio;
+      bt[0] = bt[1] = b;
+      bt[2] = bz;
+    }
+  }
+}
+
+size_t interp_smem_bytes(const N3Params& p) {
+  return sizeof(double) * kWarps * 3 * 16 +
+         (size_t)(p.bt[0] + p.w) * (p.bt[1] + p.w) * (p.bt[2] + p.w) * 16;
+}
+
+int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_G, cudaStream_t st) {
   const size_t smem = interp_smem_bytes(p);
-  SFD_REQUIRE(smem <= 227 * 1024 - 1024, SFD_ERR_INVALID_ARG, "interp subgrid does not fit shared memory (%zu B)", smem);
+  SFD_REQUIRE(smem <= 227 * 1024 - 1024 && p.bt[2] + p.w <= 32, SFD_ERR_INVALID_ARG,
+              "interp subgrid does not fit shared memory (%zu B)", smem);
   SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
-  static bool attr = false;
-  if (!attr) {
-    SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
-    attr = true;
+#define SFD_INTERP_CASE(W_) \
+  case W_: return launch<W_>(p, d_ptab, d_v, d_tgt, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_G, smem, st);
+  switch (p.w) {
+    SFD_INTERP_CASE(2) SFD_INTERP_CASE(3) SFD_INTERP_CASE(4) SFD_INTERP_CASE(5) SFD_INTERP_CASE(6)
+    SFD_INTERP_CASE(7) SFD_INTERP_CASE(8) SFD_INTERP_CASE(9) SFD_INTERP_CASE(10) SFD_INTERP_CASE(11)
+    SFD_INTERP_CASE(12) SFD_INTERP_CASE(13) SFD_INTERP_CASE(14) SFD_INTERP_CASE(15) SFD_INTERP_CASE(16)
   }
-  interp_kernel<<<num_sms(), 32 * kWarps, smem, st>>>(p, reinterpret_cast<const double2*>(d_v), d_tgt, d_item_bin,
-                                                     d_item_start, d_item_count, d_n_items, d_counter,
-                                                     reinterpret_cast<double2*>(d_G));
-  return launch_check("interp_kernel");
+#undef SFD_INTERP_CASE
+  set_error("interp: unsupported kernel width %d", p.w);
+  return SFD_ERR_UNSUPPORTED;
 }
 
 }  // namespace sfd

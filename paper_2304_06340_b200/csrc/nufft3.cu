@@ -27,7 +27,7 @@ namespace {
 
 constexpr double kPi = 3.14159265358979323846;
 constexpr int kSrcCap = 1024;   // sources per spread work item
-constexpr int kTgtCap = 2048;   // targets per interp work item
+constexpr int kTgtCap = 512;    // targets per interp work item
 constexpr int kMaxBin = 16;
 // fixed head of the workspace: [0,96) bounds of x and xi; [128,144) n_items_s, n_items_t, queue counters;
 // [1024, ...) scratch of the bounds reduction
@@ -58,7 +58,7 @@ void kernel_params(double eps, int* w, double* beta) {
 
 struct Layout {
   size_t src, skey, shist, soff, scur, sitems, tgt, tkey, thist, toff, tcur, titems, fine, inner, fftwork, dec, scan,
-      misc, total;
+      misc, ptab, total;
   int64_t ns_bins, nt_bins, ns_items, nt_items;
   size_t inner_bytes;
 };
@@ -82,12 +82,13 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
     p->st[d] = (double)p->n2[d] / (2.0 * kSigma * S);
     p->kap[d] = p->w * kPi / (2.0 * kSigma * S);
   }
+  p->deg = p->w + 3;
   p->bs = std::min(kMaxBin, spread_max_bin(p->w, real_c));
-  p->bt = std::min(kMaxBin, interp_max_bin(p->w));
+  interp_bins(p->w, p->bt);
   for (int d = 0; d < 3; ++d) {
     p->nbs[d] = (p->nf[d] + p->bs - 1) / p->bs;
     p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
-    p->nbt[d] = (p->n2[d] / 2) / p->bt + 1;
+    p->nbt[d] = (p->n2[d] / 2) / p->bt[d] + 1;
   }
   return SFD_OK;
 }
@@ -106,6 +107,7 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
     return at;
   };
   L->misc = put(kMiscBytes);
+  L->ptab = put((size_t)(kMaxDeg + 1) * kPolyStride * 8);
   L->src = put((size_t)J * sizeof(SrcRec));
   L->skey = put((size_t)J * 4);
   L->shist = put((size_t)(L->ns_bins + 1) * 4);
@@ -151,6 +153,42 @@ void make_quad(const N3Params& p, QuadTable* q) {
     q->f[i] = (double)((long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)));
   }
   for (int i = n; i < kMaxQuad; ++i) q->z[i] = q->f[i] = 0.0;
+}
+
+// Piecewise-polynomial kernel table (nufft3.cuh footprint()): on interval i the function s -> phi((t + i - w/2) 2/w),
+// t = (s+1)/2, is interpolated at the deg+1 Chebyshev nodes of [-1,1] (discrete Chebyshev transform in long double)
+// and converted to monomial coefficients by the T_j recurrence (|coefficients| <= 1: Horner in fp64 is accurate to
+// ~1e-15).  tab[q * kPolyStride + i] = coefficient of s^q.
+void make_poly(const N3Params& p, double* tab) {
+  const int n = p.deg + 1;
+  const long double pi = 3.14159265358979323846264338327950288L;
+  std::vector<long double> x(n), fx(n), co(n);
+  std::vector<std::vector<long double>> T(n, std::vector<long double>(n, 0.0L));
+  T[0][0] = 1.0L;
+  if (n > 1) T[1][1] = 1.0L;
+  for (int j = 2; j < n; ++j) {
+    for (int q = 1; q < n; ++q) T[j][q] = 2.0L * T[j - 1][q - 1];
+    for (int q = 0; q < n; ++q) T[j][q] -= T[j - 2][q];
+  }
+  for (int k = 0; k < n; ++k) x[k] = cosl(pi * (2 * k + 1) / (2.0L * n));
+  for (int i = 0; i < (kMaxDeg + 1) * kPolyStride; ++i) tab[i] = 0.0;
+  for (int i = 0; i < p.w; ++i) {
+    for (int k = 0; k < n; ++k) {
+      const long double z = ((x[k] + 1.0L) / 2.0L + i - p.w / 2.0L) * 2.0L / p.w;
+      const long double a = 1.0L - z * z;
+      fx[k] = expl((long double)p.beta * (sqrtl(a > 0 ? a : 0.0L) - 1.0L));
+    }
+    for (int j = 0; j < n; ++j) {
+      long double acc = 0.0L;
+      for (int k = 0; k < n; ++k) acc += fx[k] * cosl(j * pi * (2 * k + 1) / (2.0L * n));
+      co[j] = acc * (j == 0 ? 1.0L : 2.0L) / n;
+    }
+    for (int q = 0; q < n; ++q) {
+      long double m = 0.0L;
+      for (int j = q; j < n; ++j) m += co[j] * T[j][q];
+      tab[q * kPolyStride + i] = (double)m;
+    }
+  }
 }
 
 // ---- cuFFT plan cache (process-global, guarded; sfd_release_cache() empties it) --------------------------------
@@ -271,6 +309,10 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
               L.total, work_bytes);
   QuadTable quad;
   make_quad(p, &quad);
+  double h_ptab[(kMaxDeg + 1) * kPolyStride];
+  make_poly(p, h_ptab);
+  double* ptab = reinterpret_cast<double*>(base + L.ptab);
+  SFD_CUDA_TRY(cudaMemcpyAsync(ptab, h_ptab, sizeof(h_ptab), cudaMemcpyHostToDevice, st));
   int dev = 0;
   SFD_CUDA_TRY(cudaGetDevice(&dev));
   PlanEntry plan;
@@ -309,7 +351,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
 
   // A5-4: spread
   SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
-  SFD_TRY(spread(p, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
+  SFD_TRY(spread(p, ptab, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
   prof_mark("spread", st);
 
   // A5-5: deconvolve + zero-pad;  A5-6: uniform FFT (cuFFT, timed on its own)
@@ -334,7 +376,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   prof_mark("tgt_sort", st);
 
   // A5-8: interpolate;  A5-9: post-deconvolve + post-phase
-  SFD_TRY(interp(p, inner, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
+  SFD_TRY(interp(p, ptab, inner, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
   prof_mark("interp", st);
   SFD_TRY(post_deconv(p, quad, d_xi, K, d_nuhat, st));
   prof_mark("post", st);

@@ -22,8 +22,13 @@ struct N3Params {
   double kap[3];      // target  -> argument of phihat:    kappa = (xi - D) kap,    kap = w pi / (2 sigma S)
   int real_c;         // 1 when D == 0: the strengths c'_j = w_j stay real and so does the fine grid
   int bs, nbs[3];     // source bins: bs^3 cells, nbs[d] = ceil(nf[d] / bs)
-  int bt, nbt[3], t0[3];  // target bins over the band [t0, t0 + nbt*bt) of the inner grid that holds every target
+  int bt[3], nbt[3], t0[3];  // target bins (bt[0] x bt[1] x bt[2] cells) over the band [t0, t0 + nbt*bt) of the
+                             // inner grid that holds every target; bt[2] is 8 or 16 (bank-conflict-free pitch)
+  int deg;                   // degree of the piecewise-polynomial kernel evaluation (w + 3)
 };
+
+constexpr int kMaxDeg = kMaxW + 3;
+constexpr int kPolyStride = 16;   // ptab[q * kPolyStride + i]: coefficient of s^q on interval i (i < w)
 
 struct __align__(8) SrcRec { double u[3]; double re, im; };   // sorted source: grid coordinate + strength (40 B)
 struct __align__(8) TgtRec { double u[3]; int64_t k; };       // sorted target: grid coordinate + original index
@@ -40,19 +45,32 @@ __device__ __forceinline__ double es_kernel(double z, double beta) {
   return exp(beta * (sqrt(t) - 1.0));
 }
 
+// Piecewise-polynomial evaluation of the kernel (the "Horner" evaluation of the ES-kernel papers [2,3]): for a point
+// at grid coordinate u the footprint starts at i0 = ceil(u - w/2); with t = i0 - (u - w/2) in [0,1) and s = 2t - 1 the
+// value on cell i0 + i is phi((t + i - w/2) 2/w) = P_i(s), a polynomial of degree p.deg per interval i whose
+// coefficients (Chebyshev-node interpolants, host long double; nufft3.cu make_poly) sit in ptab.  Interior intervals
+// are accurate to ~1e-15; the two edge intervals, where phi has a square-root singularity and is ~e^-beta, to
+// ~0.05 eps.
+__device__ __forceinline__ void footprint(double u, int w, int& i0, double& s) {
+  const double lo = u - 0.5 * w;
+  const double c = ceil(lo);
+  i0 = (int)c;
+  s = __fma_rn(2.0, c - lo, -1.0);
+}
+
 // ---- spread.cu (A5-4) ------------------------------------------------------------------------------------
 // Work item i: sources [item_start[i], item_start[i]+item_count[i]) of bin item_bin[i].  *n_items on the device.
 // grid is real double[nf0][nf1][nf2] (real_c) or complex double[nf0][nf1][nf2][2]; must be zero on entry.
 int spread_max_bin(int w, bool real_c);   // largest bin edge whose padded subgrid fits shared memory
-int interp_max_bin(int w);
 size_t spread_smem_bytes(const N3Params& p);
-int spread(const N3Params& p, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
+int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
            const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st);
 
 // ---- interp.cu (A5-8) ------------------------------------------------------------------------------------
 // v = complex double[n2_0][n2_1][n2_2][2]; writes G[k] (complex) for every sorted target.
 size_t interp_smem_bytes(const N3Params& p);
-int interp(const N3Params& p, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
+void interp_bins(int w, int bt[3]);   // target-bin shape for kernel width w
+int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_G, cudaStream_t st);
 

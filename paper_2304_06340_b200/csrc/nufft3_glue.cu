@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(kT) target_keys_kernel(N3Params p, const doubl
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     const double u = tgt_coord(p, xi[3 * k + d], d);
-    b[d] = clampi((int)floor((u - p.t0[d]) / p.bt), 0, p.nbt[d] - 1);
+    b[d] = clampi((int)floor((u - p.t0[d]) / p.bt[d]), 0, p.nbt[d] - 1);
   }
   const int kk = (b[0] * p.nbt[1] + b[1]) * p.nbt[2] + b[2];
   key[k] = kk;

@@ -29,13 +29,16 @@ constexpr int kCplxMaxP = 23;   // 23^3 * 16 B = 195 KB
 
 template <bool REAL>
 __global__ void __launch_bounds__(32 * kMaxW, 1)
-spread_kernel(N3Params p, const SrcRec* __restrict__ src, const int32_t* __restrict__ item_bin,
+spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restrict__ src,
+              const int32_t* __restrict__ item_bin,
               const int32_t* __restrict__ item_start, const int32_t* __restrict__ item_count,
               const int32_t* __restrict__ n_items, int32_t* __restrict__ counter, double* __restrict__ grid) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ChunkTables& tab = *reinterpret_cast<ChunkTables*>(smem_raw);
   double* sub = reinterpret_cast<double*>(smem_raw + sizeof(ChunkTables));
   __shared__ int s_item;
+  __shared__ double s_poly[(kMaxDeg + 1) * kPolyStride];   // piecewise-polynomial kernel table (footprint())
+  for (int i = threadIdx.x; i < (kMaxDeg + 1) * kPolyStride; i += blockDim.x) s_poly[i] = ptab[i];
 
   const int w = p.w, P = p.bs + w, fw = w / 2;
   const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, nthreads = blockDim.x;
@@ -70,12 +73,25 @@ spread_kernel(N3Params p, const SrcRec* __restrict__ src, const int32_t* __restr
       __syncthreads();  // zero-fill / previous sweep finished
       if (lane < nch) {
         const SrcRec r = src[start + c0 + lane];
+        // warp wq evaluates interval wq of the three 1-D kernels for 32 sources at once (coefficients: broadcast)
+        int i0[3];
+        double sv[3];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-          const int i0 = (int)ceil(r.u[d] - 0.5 * w);
-          const double z = ((double)(i0 + wq) - r.u[d]) * (2.0 / w);
-          tab.k[d][lane][wq] = es_kernel(z, p.beta);
-          if (wq == 0) tab.i0[lane][d] = i0 - o[d];
+        for (int d = 0; d < 3; ++d) footprint(r.u[d], w, i0[d], sv[d]);
+        double k0 = s_poly[p.deg * kPolyStride + wq], k1 = k0, k2 = k0;
+        for (int q = p.deg - 1; q >= 0; --q) {
+          const double c = s_poly[q * kPolyStride + wq];
+          k0 = __fma_rn(k0, sv[0], c);
+          k1 = __fma_rn(k1, sv[1], c);
+          k2 = __fma_rn(k2, sv[2], c);
+        }
+        tab.k[0][lane][wq] = k0;
+        tab.k[1][lane][wq] = k1;
+        tab.k[2][lane][wq] = k2;
+        if (wq == 0) {
+          tab.i0[lane][0] = i0[0] - o[0];
+          tab.i0[lane][1] = i0[1] - o[1];
+          tab.i0[lane][2] = i0[2] - o[2];
         }
         if (wq == 0) {
           tab.c[lane][0] = r.re;
@@ -138,29 +154,29 @@ size_t spread_smem_bytes(const N3Params& p) {
   return sizeof(ChunkTables) + P * P * P * (p.real_c ? 8 : 16);
 }
 
-int spread(const N3Params& p, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
+int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
            const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st) {
   const size_t smem = spread_smem_bytes(p);
-  SFD_REQUIRE(smem <= 227 * 1024, SFD_ERR_INVALID_ARG, "spread subgrid does not fit shared memory (%zu B)", smem);
+  SFD_REQUIRE(smem <= 227 * 1024 - 4096, SFD_ERR_INVALID_ARG, "spread subgrid does not fit shared memory (%zu B)", smem);
   SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
   const int threads = 32 * p.w;
   const int blocks = num_sms();
   if (p.real_c) {
     static bool attr = false;
     if (!attr) {
-      SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096));
       attr = true;
     }
-    spread_kernel<true><<<blocks, threads, smem, st>>>(p, d_src, d_item_bin, d_item_start, d_item_count, d_n_items,
-                                                      d_counter, d_grid);
+    spread_kernel<true><<<blocks, threads, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
+                                                      d_n_items, d_counter, d_grid);
   } else {
     static bool attr = false;
     if (!attr) {
-      SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096));
       attr = true;
     }
-    spread_kernel<false><<<blocks, threads, smem, st>>>(p, d_src, d_item_bin, d_item_start, d_item_count, d_n_items,
-                                                       d_counter, d_grid);
+    spread_kernel<false><<<blocks, threads, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
+                                                       d_n_items, d_counter, d_grid);
   }
   return launch_check("spread_kernel");
 }
