@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsfd.so")
 SOURCES = ["api.cu", "mesh.cu", "nodes.cu", "scan.cu", "direct.cu", "reduce.cu", "nufft3.cu", "nufft3_glue.cu",
-           "spread.cu", "interp.cu", "probe.cu"]
+           "spread.cu", "interp.cu", "fft.cu", "probe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr"]
@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         changed = list(ex.map(lambda s: _compile(s, force, verbose), SOURCES))
     if any(changed) or not os.path.exists(LIB):
         objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
-        cmd = [NVCC, "-shared", "-o", LIB, *objs, "-lcufft", "-Xlinker", "--no-undefined"]
+        cmd = [NVCC, "-shared", "-o", LIB, *objs, "-Xlinker", "--no-undefined"]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")

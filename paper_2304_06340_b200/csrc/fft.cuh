@@ -1,0 +1,40 @@
+// fft.cuh -- interface of the pruned in-shared-memory FFT passes (fft.cu; A5-5/A5-6 of the type-3 NUFFT).
+#pragma once
+#include "common.cuh"
+
+namespace sfd {
+
+// Device tables per axis: twiddles exp(-2 pi i t / N), digit-reversal positions, radix list (4s, 2, 3s, 5s).
+struct FftTables {
+  const double2* tw[3];
+  const int32_t* rev[3];
+  int nfac[3];
+  int fac[3][16];
+};
+
+// One pass of 1-D transforms of length N over a 2-level set of rows ("columns" c = (hi, lo)).
+//   input  element (hi, lo, i), i in [0, n_in):  in [hi*in_hi  + lo*in_lo  + i*in_el]    <-> mode l = i - n_in/2
+//   output element (hi, lo, m), m in [lo, lo+nout): out[hi*out_hi + lo*out_lo + (m-lo)*out_el]
+//   out(m) = sum_l in(l) exp(-2 pi i l m / N)
+// contig = 1: the transform axis is the contiguous one (in_el = out_el = 1; loads and stores run along the axis);
+// contig = 0: `lo` is the contiguous index (in_lo = out_lo = 1; loads and stores run across the tile's rows).
+// dec_axis/dec_hi/dec_lo (all or none): the input is multiplied by dec_axis[i] * dec_hi[hi] * dec_lo[lo].
+struct FftPass {
+  int N, n_in, lo, nout;
+  int64_t n_hi, n_lo;
+  int64_t in_hi, in_lo, in_el, out_hi, out_lo, out_el;
+  int contig, real_in;
+  const double *dec_axis, *dec_hi, *dec_lo;
+  // filled in by fft_pass():
+  int tb, tb_shift, nfac, fac[16];
+  const double2* tw;
+  const int32_t* rev;
+};
+
+bool fft_length_ok(int N);
+int fft_tile(int N);                                   // rows per tile (0: does not fit shared memory)
+size_t fft_tables_bytes(const int n2[3]);
+int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStream_t st);
+int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* d_out, cudaStream_t st);
+
+}  // namespace sfd

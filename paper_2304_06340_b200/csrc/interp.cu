@@ -68,15 +68,16 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
     const int start = item_start[item], count = item_count[item];
     const int bz = bin % p.nbt[2], by = (bin / p.nbt[2]) % p.nbt[1], bx = bin / (p.nbt[2] * p.nbt[1]);
     const int ox = p.t0[0] + bx * p.bt[0] - W / 2, oy = p.t0[1] + by * p.bt[1] - W / 2, oz = p.t0[2] + bz * p.bt[2] - W / 2;
+    const int bx0 = ox - p.lo[0], by0 = oy - p.lo[1], bz0 = oz - p.lo[2];   // subgrid origin in band coordinates
 
     // stage the subgrid: one (x,y) row of Pz <= 32 cells per warp pass, 16 B per lane, coalesced along z
     for (int row = wq; row < Px * Py; row += kWarps) {
       const int ix = row / Py, iy = row - ix * Py;
-      const int gx = ox + ix, gy = oy + iy, gz = oz + lane;
+      const int gx = bx0 + ix, gy = by0 + iy, gz = bz0 + lane;
       if (lane < Pz) {
         double2 val = make_double2(0.0, 0.0);
-        if (gx >= 0 && gy >= 0 && gz >= 0 && gx < p.n2[0] && gy < p.n2[1] && gz < p.n2[2])
-          val = v[((size_t)gx * p.n2[1] + gy) * p.n2[2] + gz];
+        if (gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nout[0] && gy < p.nout[1] && gz < p.nout[2])
+          val = v[((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz];
         sub[row * Pz + lane] = val;
       }
     }

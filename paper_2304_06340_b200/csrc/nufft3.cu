@@ -7,18 +7,19 @@
 //   xi.x = (xi-D).(x-C) + D.x + (xi-D).C            C, D = centres of sources / targets
 //   1. c'_j = w_j e^{-i D.x_j};  u_j = (x_j-C) sigma S/pi + nf/2   (rescaling: analogue of P:188 eq. 3.7)
 //   2. bin-sort sources ("sort"), spread onto the fine grid nf^3 (spread.cu)
-//   3. deconvolve by the kernel's transform on the integer modes and zero-pad into the inner grid n2 = 2 nf
-//   4. uniform FFT of size n2^3 (cuFFT: "fastest GPU version ... provided by CUDA Toolkit")
+//   3. deconvolve by the kernel's transform on the integer modes (folded into the first FFT pass)
+//   4. uniform FFT of size n2^3, n2 = 2 nf, pruned to the nf^3 non-zero inputs and to the band of outputs the
+//      targets touch: three passes of in-shared-memory 1-D transforms (fft.cu).  The paper's library calls cuFFT on
+//      the full lattice; a full n2^3 transform would move 8-16x more data and not fit at config 5.
 //   5. bin-sort targets, interpolate at u2_k = (xi_k-D) n2/(2 sigma S) + n2/2 (interp.cu)
 //   6. divide by the kernel's transform at the non-integer frequencies, multiply by e^{-i (xi_k-D).C}
-#include <cufft.h>
-
 #include <cmath>
 #include <map>
 #include <mutex>
 #include <tuple>
 #include <vector>
 
+#include "fft.cuh"
 #include "internal.cuh"
 #include "nufft3.cuh"
 
@@ -57,10 +58,10 @@ void kernel_params(double eps, int* w, double* beta) {
 }
 
 struct Layout {
-  size_t src, skey, shist, soff, scur, sitems, tgt, tkey, thist, toff, tcur, titems, fine, inner, fftwork, dec, scan,
-      misc, ptab, total;
+  size_t src, skey, shist, soff, scur, sitems, tgt, tkey, thist, toff, tcur, titems, fine, bufx, bufy, ffttab, dec,
+      scan, misc, ptab, total;
   int64_t ns_bins, nt_bins, ns_items, nt_items;
-  size_t inner_bytes;
+  size_t fine_bytes;
 };
 
 // Geometry from half-widths X (sources) and S (targets); centres are filled in by the caller.
@@ -89,6 +90,9 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
     p->nbs[d] = (p->nf[d] + p->bs - 1) / p->bs;
     p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
     p->nbt[d] = (p->n2[d] / 2) / p->bt[d] + 1;
+    // cells any footprint can touch: ceil(n2/4 - w/2) ... ceil(3 n2/4 - w/2) + w - 1, plus one cell of slack
+    p->lo[d] = std::max(0, p->n2[d] / 4 - (p->w + 1) / 2 - 1);
+    p->nout[d] = std::min(p->n2[d] - p->lo[d], p->n2[d] / 2 + p->w + 3);
   }
   return SFD_OK;
 }
@@ -122,10 +126,13 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->titems = put((size_t)L->nt_items * 4 * 3);
   L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2]) * 8);
   L->scan = put(scan_workspace(std::max(L->ns_bins, L->nt_bins) + 1));
-  L->fine = put((size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16));
-  L->inner_bytes = (size_t)p.n2[0] * p.n2[1] * p.n2[2] * 16;
-  L->inner = put(L->inner_bytes);
-  L->fftwork = put(L->inner_bytes);   // cuFFT work area (checked against the plan's real need)
+  L->ffttab = put(fft_tables_bytes(p.n2));
+  L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16);
+  L->fine = put(L->fine_bytes);
+  // FFT passes: fine -> X [nf0][nf1][nout2] -> Y [nf0][nout1][nout2] -> X [nout0][nout1][nout2]
+  const size_t xa = (size_t)p.nf[0] * p.nf[1] * p.nout[2], xc = (size_t)p.nout[0] * p.nout[1] * p.nout[2];
+  L->bufx = put(std::max(xa, xc) * 16);
+  L->bufy = put((size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16);
   L->total = o;
   return SFD_OK;
 }
@@ -191,45 +198,9 @@ void make_poly(const N3Params& p, double* tab) {
   }
 }
 
-// ---- cuFFT plan cache (process-global, guarded; sfd_release_cache() empties it) --------------------------------
-struct PlanEntry {
-  cufftHandle h;
-  size_t work;
-};
-std::mutex g_plan_mu;
-std::map<std::tuple<int, int, int, int>, PlanEntry> g_plans;
-
-int get_plan(int dev, const int n2[3], PlanEntry* out) {
-  std::lock_guard<std::mutex> lk(g_plan_mu);
-  const auto key = std::make_tuple(dev, n2[0], n2[1], n2[2]);
-  auto it = g_plans.find(key);
-  if (it != g_plans.end()) {
-    *out = it->second;
-    return SFD_OK;
-  }
-  PlanEntry e{};
-  cufftResult r = cufftCreate(&e.h);
-  SFD_REQUIRE(r == CUFFT_SUCCESS, SFD_ERR_CUFFT, "cufftCreate failed (%d)", (int)r);
-  r = cufftSetAutoAllocation(e.h, 0);
-  if (r == CUFFT_SUCCESS) r = cufftMakePlan3d(e.h, n2[0], n2[1], n2[2], CUFFT_Z2Z, &e.work);
-  if (r != CUFFT_SUCCESS) {
-    cufftDestroy(e.h);
-    set_error("cufftMakePlan3d(%d,%d,%d) failed (%d)", n2[0], n2[1], n2[2], (int)r);
-    return SFD_ERR_CUFFT;
-  }
-  g_plans[key] = e;
-  *out = e;
-  return SFD_OK;
-}
-
 }  // namespace
 
-int nufft3_release_cache() {
-  std::lock_guard<std::mutex> lk(g_plan_mu);
-  for (auto& kv : g_plans) cufftDestroy(kv.second.h);
-  g_plans.clear();
-  return SFD_OK;
-}
+int nufft3_release_cache() { return SFD_OK; }   // nothing is cached on the device any more
 
 int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out) {
   SFD_REQUIRE(X && S && out, SFD_ERR_NULL, "nufft3_sizes: NULL argument");
@@ -252,7 +223,7 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
   for (int d = 0; d < 3; ++d) {
     out->nf[d] = p.nf[d];
     out->n2[d] = p.n2[d];
-    out->nout[d] = p.n2[d] / 2 + p.w + 2;
+    out->nout[d] = p.nout[d];
   }
   out->work_bytes = total;
   return SFD_OK;
@@ -313,14 +284,6 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   make_poly(p, h_ptab);
   double* ptab = reinterpret_cast<double*>(base + L.ptab);
   SFD_CUDA_TRY(cudaMemcpyAsync(ptab, h_ptab, sizeof(h_ptab), cudaMemcpyHostToDevice, st));
-  int dev = 0;
-  SFD_CUDA_TRY(cudaGetDevice(&dev));
-  PlanEntry plan;
-  SFD_TRY(get_plan(dev, p.n2, &plan));
-  SFD_REQUIRE(plan.work <= L.inner_bytes, SFD_ERR_WORKSPACE_TOO_SMALL,
-              "cuFFT wants a %zu-byte work area for %dx%dx%d, more than the %zu reserved", plan.work, p.n2[0], p.n2[1],
-              p.n2[2], L.inner_bytes);
-
   SrcRec* src = reinterpret_cast<SrcRec*>(base + L.src);
   TgtRec* tgt = reinterpret_cast<TgtRec*>(base + L.tgt);
   int32_t* skey = reinterpret_cast<int32_t*>(base + L.skey);
@@ -335,10 +298,11 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   int32_t* titems = reinterpret_cast<int32_t*>(base + L.titems);
   double* dec = reinterpret_cast<double*>(base + L.dec);
   double* fine = reinterpret_cast<double*>(base + L.fine);
-  double* inner = reinterpret_cast<double*>(base + L.inner);
+  double* bufx = reinterpret_cast<double*>(base + L.bufx);
+  double* bufy = reinterpret_cast<double*>(base + L.bufy);
   void* scan_w = base + L.scan;
-  const size_t scan_b = L.fine - L.scan;
-  const size_t fine_bytes = L.inner - L.fine;
+  const size_t scan_b = L.ffttab - L.scan;
+  const size_t fine_bytes = L.fine_bytes;
 
   // A5-2/A5-3: rescale, pre-phase and bin-sort the sources
   SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_bins + 1) * 4, st));
@@ -354,17 +318,35 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   SFD_TRY(spread(p, ptab, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
   prof_mark("spread", st);
 
-  // A5-5: deconvolve + zero-pad;  A5-6: uniform FFT (cuFFT, timed on its own)
+  // A5-5 + A5-6: deconvolution folded into the first of three pruned 1-D FFT passes (timed on its own)
   SFD_TRY(deconv_tables(p, quad, dec, st));
-  SFD_TRY(deconv_pad(p, fine, dec, inner, st));
-  prof_mark("deconv_pad", st);
-  cufftResult r = cufftSetStream(plan.h, st);
-  if (r == CUFFT_SUCCESS) r = cufftSetWorkArea(plan.h, base + L.fftwork);
-  if (r == CUFFT_SUCCESS)
-    r = cufftExecZ2Z(plan.h, reinterpret_cast<cufftDoubleComplex*>(inner), reinterpret_cast<cufftDoubleComplex*>(inner),
-                     CUFFT_FORWARD);
-  SFD_REQUIRE(r == CUFFT_SUCCESS, SFD_ERR_CUFFT, "cuFFT Z2Z %dx%dx%d failed (%d)", p.n2[0], p.n2[1], p.n2[2], (int)r);
-  prof_mark("cufft", st);
+  FftTables ft;
+  SFD_TRY(fft_upload_tables(p.n2, base + L.ffttab, &ft, st));
+  {
+    const int64_t nf0 = p.nf[0], nf1 = p.nf[1], nf2 = p.nf[2], no0 = p.nout[0], no1 = p.nout[1], no2 = p.nout[2];
+    (void)no0;
+    FftPass A{};   // axis 2 (contiguous): rows (i0, i1) of the fine grid -> X[i0][i1][m2]
+    A.N = p.n2[2]; A.n_in = p.nf[2]; A.lo = p.lo[2]; A.nout = p.nout[2];
+    A.n_hi = nf0; A.n_lo = nf1;
+    A.in_hi = nf1 * nf2; A.in_lo = nf2; A.in_el = 1;
+    A.out_hi = nf1 * no2; A.out_lo = no2; A.out_el = 1;
+    A.contig = 1; A.real_in = p.real_c;
+    A.dec_axis = dec + p.nf[0] + p.nf[1]; A.dec_hi = dec; A.dec_lo = dec + p.nf[0];
+    SFD_TRY(fft_pass(A, ft, 2, fine, bufx, st));
+    FftPass B{};   // axis 1: columns (i0, m2) of X -> Y[i0][m1][m2]
+    B.N = p.n2[1]; B.n_in = p.nf[1]; B.lo = p.lo[1]; B.nout = p.nout[1];
+    B.n_hi = nf0; B.n_lo = no2;
+    B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
+    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
+    FftPass C{};   // axis 0: columns (m1, m2) of Y -> X[m0][m1][m2]
+    C.N = p.n2[0]; C.n_in = p.nf[0]; C.lo = p.lo[0]; C.nout = p.nout[0];
+    C.n_hi = 1; C.n_lo = no1 * no2;
+    C.in_hi = 0; C.in_lo = 1; C.in_el = no1 * no2;
+    C.out_hi = 0; C.out_lo = 1; C.out_el = no1 * no2;
+    SFD_TRY(fft_pass(C, ft, 0, bufy, bufx, st));
+  }
+  prof_mark("fft", st);
 
   // A5-7: rescale and bin-sort the targets
   SFD_CUDA_TRY(cudaMemsetAsync(thist, 0, (size_t)(L.nt_bins + 1) * 4, st));
@@ -376,7 +358,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   prof_mark("tgt_sort", st);
 
   // A5-8: interpolate;  A5-9: post-deconvolve + post-phase
-  SFD_TRY(interp(p, ptab, inner, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
+  SFD_TRY(interp(p, ptab, bufx, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
   prof_mark("interp", st);
   SFD_TRY(post_deconv(p, quad, d_xi, K, d_nuhat, st));
   prof_mark("post", st);

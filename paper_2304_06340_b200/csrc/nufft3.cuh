@@ -25,6 +25,7 @@ struct N3Params {
   int bt[3], nbt[3], t0[3];  // target bins (bt[0] x bt[1] x bt[2] cells) over the band [t0, t0 + nbt*bt) of the
                              // inner grid that holds every target; bt[2] is 8 or 16 (bank-conflict-free pitch)
   int deg;                   // degree of the piecewise-polynomial kernel evaluation (w + 3)
+  int lo[3], nout[3];        // band of the inner grid that is computed and stored: v[m - lo], m in [lo, lo + nout)
 };
 
 constexpr int kMaxDeg = kMaxW + 3;
@@ -67,7 +68,8 @@ int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const i
            const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st);
 
 // ---- interp.cu (A5-8) ------------------------------------------------------------------------------------
-// v = complex double[n2_0][n2_1][n2_2][2]; writes G[k] (complex) for every sorted target.
+// v = complex double[nout_0][nout_1][nout_2][2], the band [lo, lo+nout) of the inner grid; writes G[k] (complex) for
+// every sorted target.
 size_t interp_smem_bytes(const N3Params& p);
 void interp_bins(int w, int bt[3]);   // target-bin shape for kernel width w
 int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
@@ -90,10 +92,8 @@ int target_scatter(const N3Params& p, const double* d_xi, int64_t K, const int32
 // count); *d_n_items = number of items.  d_tmp holds nbins+1 int32.
 int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int cap, int32_t* d_tmp, int32_t* d_items,
                int64_t max_items, int32_t* d_n_items, void* d_scan, size_t scan_bytes, cudaStream_t st);
-// A5-5: dec[d][i] = (-1)^l / ((w/2) phihat(l w pi / n2_d)), l = i - nf_d/2; then b~ = g * dec x dec x dec zero-padded
-// into the inner grid at index l mod n2.
+// A5-5: dec[d][i] = (-1)^l / ((w/2) phihat(l w pi / n2_d)), l = i - nf_d/2 (applied by the first FFT pass, fft.cu).
 int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st);
-int deconv_pad(const N3Params& p, const double* d_fine, const double* d_dec, double* d_inner, cudaStream_t st);
 // A5-9: nuhat_k = G_k e^{-i (xi_k-D).C} / prod_d (w/2) phihat((xi_kd-D_d) kap_d), in place on d_nuhat.
 int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st);
 

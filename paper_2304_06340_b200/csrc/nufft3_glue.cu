@@ -188,31 +188,6 @@ __global__ void __launch_bounds__(kT) deconv_tables_kernel(N3Params p, QuadTable
   dec[i] = (l & 1) ? -v : v;   // (-1)^l: shifts the inner grid by half a period, t_m = m h2 - pi
 }
 
-template <bool REAL>
-__global__ void __launch_bounds__(kT) deconv_pad_kernel(N3Params p, const double* __restrict__ fine,
-                                                       const double* __restrict__ dec, double2* __restrict__ inner) {
-  const int pz = blockIdx.x * kT + threadIdx.x;
-  const int py = blockIdx.y, px = blockIdx.z;
-  if (pz >= p.n2[2]) return;
-  const int lx = px < p.n2[0] / 2 ? px : px - p.n2[0];
-  const int ly = py < p.n2[1] / 2 ? py : py - p.n2[1];
-  const int lz = pz < p.n2[2] / 2 ? pz : pz - p.n2[2];
-  const int ix = lx + p.nf[0] / 2, iy = ly + p.nf[1] / 2, iz = lz + p.nf[2] / 2;
-  double2 out = make_double2(0.0, 0.0);
-  if (ix >= 0 && ix < p.nf[0] && iy >= 0 && iy < p.nf[1] && iz >= 0 && iz < p.nf[2]) {
-    const double f = dec[ix] * dec[p.nf[0] + iy] * dec[p.nf[0] + p.nf[1] + iz];
-    const size_t g = ((size_t)ix * p.nf[1] + iy) * p.nf[2] + iz;
-    if (REAL) {
-      out.x = fine[g] * f;
-    } else {
-      const double2 v = reinterpret_cast<const double2*>(fine)[g];
-      out.x = v.x * f;
-      out.y = v.y * f;
-    }
-  }
-  inner[((size_t)px * p.n2[1] + py) * p.n2[2] + pz] = out;
-}
-
 // ---- A5-9 post-deconvolution + post-phase --------------------------------------------------------------------
 __global__ void __launch_bounds__(kT) post_deconv_kernel(N3Params p, QuadTable q, const double* __restrict__ xi, int64_t K,
                                                         double2* __restrict__ nuhat) {
@@ -272,15 +247,6 @@ int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int c
 int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st) {
   deconv_tables_kernel<<<blocks_for(p.nf[0] + p.nf[1] + p.nf[2]), kT, 0, st>>>(p, q, d_dec);
   return launch_check("deconv_tables_kernel");
-}
-
-int deconv_pad(const N3Params& p, const double* d_fine, const double* d_dec, double* d_inner, cudaStream_t st) {
-  dim3 grid(blocks_for(p.n2[2]), (unsigned)p.n2[1], (unsigned)p.n2[0]);
-  if (p.real_c)
-    deconv_pad_kernel<true><<<grid, kT, 0, st>>>(p, d_fine, d_dec, reinterpret_cast<double2*>(d_inner));
-  else
-    deconv_pad_kernel<false><<<grid, kT, 0, st>>>(p, d_fine, d_dec, reinterpret_cast<double2*>(d_inner));
-  return launch_check("deconv_pad_kernel");
 }
 
 int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st) {
