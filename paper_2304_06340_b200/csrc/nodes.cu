@@ -1,6 +1,9 @@
 // nodes.cu -- A3: triangle-quadrature atoms (eqs. 3.1-3.2) and the ball-shaped frequency quadrature
 // of the CUDA path.  HBM-bound, one pass: 12 B + 72 B (cached) read and 32*q B written per face.
 #include <cmath>
+#include <map>
+#include <mutex>
+#include <tuple>
 #include <vector>
 
 #include "internal.cuh"
@@ -155,6 +158,19 @@ int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t) {
   SFD_REQUIRE(q->n_r >= 1 && q->n_theta >= 1 && q->n_phi >= 1, SFD_ERR_INVALID_ARG,
               "freq quadrature sizes must be >= 1 (got %d,%d,%d)", q->n_r, q->n_theta, q->n_phi);
   SFD_REQUIRE(R > 0.0 && std::isfinite(R), SFD_ERR_INVALID_ARG, "R must be positive and finite");
+  // the Newton iterations cost ~1 ms of host time at 256 x 128 nodes: keep the last few rules (host-side cache,
+  // thread-safe; the rules are a pure function of the key)
+  static std::mutex mu;
+  static std::map<std::tuple<int, int, int, double>, FreqTables> cache;
+  const auto key = std::make_tuple(q->n_r, q->n_theta, q->n_phi, R);
+  {
+    std::lock_guard<std::mutex> lk(mu);
+    auto it = cache.find(key);
+    if (it != cache.end()) {
+      t = it->second;
+      return SFD_OK;
+    }
+  }
   const double pi = 3.14159265358979323846;
   std::vector<long double> u, wu;
   legendre_rule(q->n_r, u, wu);
@@ -182,6 +198,11 @@ int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t) {
     t.sph[c] = std::sin(ph);
   }
   t.wph = 2.0 * pi / q->n_phi;
+  {
+    std::lock_guard<std::mutex> lk(mu);
+    if (cache.size() >= 16) cache.clear();
+    cache[key] = t;
+  }
   return SFD_OK;
 }
 

@@ -14,6 +14,7 @@
 //   5. bin-sort targets, interpolate at u2_k = (xi_k-D) n2/(2 sigma S) + n2/2 (interp.cu)
 //   6. divide by the kernel's transform at the non-integer frequencies, multiply by e^{-i (xi_k-D).C}
 #include <cmath>
+#include <cstring>
 #include <map>
 #include <mutex>
 #include <tuple>
@@ -145,21 +146,36 @@ namespace sfd {
 namespace {
 
 // (w/2) phihat(kappa) = (w/2) * 2 int_0^1 phi(z) cos(kappa z) dz; with z = sin(theta) the integrand
-// exp(beta (cos(theta) - 1)) cos(kappa sin(theta)) cos(theta) is analytic on [0, pi/2] and n = 2w+6 Gauss-Legendre
-// nodes give ~1e-14 relative accuracy for every kappa <= w pi / 4 that the two deconvolutions use.
-void make_quad(const N3Params& p, QuadTable* q) {
-  const int n = std::min(kMaxQuad, 2 * p.w + 6);
-  std::vector<long double> t, wt;
-  gauss_legendre_host(n, t, wt);
-  q->n = n;
-  const long double quarter_pi = 0.785398163397448309615660845819875721L;
-  for (int i = 0; i < n; ++i) {
-    const long double th = (t[i] + 1.0L) * quarter_pi;
-    const long double om = wt[i] * quarter_pi;
-    q->z[i] = (double)sinl(th);
-    q->f[i] = (double)((long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)));
+// exp(beta (cos(theta) - 1)) cos(kappa sin(theta)) cos(theta) is analytic on [0, pi/2] and 64 Gauss-Legendre nodes
+// in long double give it to ~1e-18.  Sampled at the Chebyshev nodes of y = 2 (kappa/kmax)^2 - 1 and turned into the
+// Chebyshev coefficients that the device evaluates (nufft3.cuh ChebTable).
+void make_cheb(const N3Params& p, ChebTable* t) {
+  const int nq = 64;
+  std::vector<long double> gt, gw;
+  gauss_legendre_host(nq, gt, gw);
+  const long double pi = 3.14159265358979323846264338327950288L;
+  const long double kmax = (long double)p.w * pi / 4.0L * (1.0L + 1e-9L);
+  auto F = [&](long double kappa) {
+    long double acc = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const long double th = (gt[i] + 1.0L) * pi / 4.0L;
+      const long double om = gw[i] * pi / 4.0L;
+      acc += (long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)) * cosl(kappa * sinl(th));
+    }
+    return acc;
+  };
+  const int n = kChebN;
+  std::vector<long double> fv(n);
+  for (int k = 0; k < n; ++k) {
+    const long double y = cosl(pi * (2 * k + 1) / (2.0L * n));
+    fv[k] = F(kmax * sqrtl((y + 1.0L) / 2.0L));
   }
-  for (int i = n; i < kMaxQuad; ++i) q->z[i] = q->f[i] = 0.0;
+  for (int j = 0; j < n; ++j) {
+    long double acc = 0.0L;
+    for (int k = 0; k < n; ++k) acc += fv[k] * cosl(j * pi * (2 * k + 1) / (2.0L * n));
+    t->c[j] = (double)(acc * (j == 0 ? 1.0L : 2.0L) / n);
+  }
+  t->inv_kmax2_x2 = (double)(2.0L / (kmax * kmax));
 }
 
 // Piecewise-polynomial kernel table (nufft3.cuh footprint()): on interval i the function s -> phi((t + i - w/2) 2/w),
@@ -278,10 +294,29 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
               "type-3 NUFFT (w=%d, fine grid %dx%dx%d) needs %zu workspace bytes, got %zu", p.w, p.nf[0], p.nf[1], p.nf[2],
               L.total, work_bytes);
-  QuadTable quad;
-  make_quad(p, &quad);
+  // host-side tables are pure functions of (w, beta): computed once per width (long-double work, ~ms), then reused
+  struct WidthTables {
+    bool ready = false;
+    double beta = 0.0;
+    ChebTable cheb;
+    double poly[(kMaxDeg + 1) * kPolyStride];
+  };
+  static WidthTables wt_cache[kMaxW + 1];
+  static std::mutex wt_mu;
+  ChebTable quad;
   double h_ptab[(kMaxDeg + 1) * kPolyStride];
-  make_poly(p, h_ptab);
+  {
+    std::lock_guard<std::mutex> lk(wt_mu);
+    WidthTables& wt = wt_cache[p.w];
+    if (!wt.ready || wt.beta != p.beta) {
+      make_cheb(p, &wt.cheb);
+      make_poly(p, wt.poly);
+      wt.beta = p.beta;
+      wt.ready = true;
+    }
+    quad = wt.cheb;
+    std::memcpy(h_ptab, wt.poly, sizeof(h_ptab));
+  }
   double* ptab = reinterpret_cast<double*>(base + L.ptab);
   SFD_CUDA_TRY(cudaMemcpyAsync(ptab, h_ptab, sizeof(h_ptab), cudaMemcpyHostToDevice, st));
   SrcRec* src = reinterpret_cast<SrcRec*>(base + L.src);

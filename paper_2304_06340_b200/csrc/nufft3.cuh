@@ -7,7 +7,6 @@
 namespace sfd {
 
 constexpr int kMaxW = 16;        // widest kernel (eps = 1e-14 -> w = 15)
-constexpr int kMaxQuad = 48;     // Gauss-Legendre nodes for the kernel's Fourier transform
 constexpr double kSigma = 2.0;   // upsampling factor of both the spreading and the inner type-2 step
 
 // Everything the kernels need to know about one transform (passed by value).
@@ -34,12 +33,28 @@ constexpr int kPolyStride = 16;   // ptab[q * kPolyStride + i]: coefficient of s
 struct __align__(8) SrcRec { double u[3]; double re, im; };   // sorted source: grid coordinate + strength (40 B)
 struct __align__(8) TgtRec { double u[3]; int64_t k; };       // sorted target: grid coordinate + original index
 
-// quadrature table for phihat(kappa) = 2 int_0^1 phi(z) cos(kappa z) dz  (uploaded per transform)
-struct QuadTable {
-  int n;
-  double z[kMaxQuad];   // GL nodes on [0,1]
-  double f[kMaxQuad];   // (w/2) * 2 * weight * phi(z): sum_q f_q cos(kappa z_q) = (w/2) phihat(kappa)
+// (w/2) phihat(kappa) = (w/2) 2 int_0^1 phi(z) cos(kappa z) dz, the kernel's Fourier transform that both
+// deconvolutions divide by, as a Chebyshev series in y = 2 (kappa/kmax)^2 - 1 on |kappa| <= kmax = w pi / 4 (the whole
+// range either deconvolution reaches at sigma = 2).  phihat is even and entire and only falls to ~0.1-0.6 of its peak
+// there, so 17 coefficients reproduce it to ~1e-14 relative; coefficients come from a long-double Gauss-Legendre
+// quadrature on the host (nufft3.cu make_cheb).  Evaluated by Clenshaw's recurrence: 17 FMAs instead of 2w+6 cosines.
+constexpr int kChebN = 17;
+struct ChebTable {
+  double inv_kmax2_x2;   // 2 / kmax^2
+  double c[kChebN];
 };
+__device__ __forceinline__ double half_w_phihat(const ChebTable& t, double kappa) {
+  const double y = __fma_rn(kappa * kappa, t.inv_kmax2_x2, -1.0);
+  const double y2 = y + y;
+  double b1 = 0.0, b2 = 0.0;
+#pragma unroll
+  for (int k = kChebN - 1; k >= 1; --k) {
+    const double b0 = __fma_rn(y2, b1, t.c[k] - b2);
+    b2 = b1;
+    b1 = b0;
+  }
+  return __fma_rn(y, b1, t.c[0] - b2);
+}
 
 __device__ __forceinline__ double es_kernel(double z, double beta) {
   const double t = fmax(0.0, __fma_rn(-z, z, 1.0));
@@ -93,8 +108,8 @@ int target_scatter(const N3Params& p, const double* d_xi, int64_t K, const int32
 int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int cap, int32_t* d_tmp, int32_t* d_items,
                int64_t max_items, int32_t* d_n_items, void* d_scan, size_t scan_bytes, cudaStream_t st);
 // A5-5: dec[d][i] = (-1)^l / ((w/2) phihat(l w pi / n2_d)), l = i - nf_d/2 (applied by the first FFT pass, fft.cu).
-int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st);
+int deconv_tables(const N3Params& p, const ChebTable& q, double* d_dec, cudaStream_t st);
 // A5-9: nuhat_k = G_k e^{-i (xi_k-D).C} / prod_d (w/2) phihat((xi_kd-D_d) kap_d), in place on d_nuhat.
-int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st);
+int post_deconv(const N3Params& p, const ChebTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st);
 
 }  // namespace sfd

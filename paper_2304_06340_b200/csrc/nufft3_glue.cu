@@ -62,6 +62,22 @@ __global__ void bounds_final_kernel(const double* __restrict__ part, int nblocks
   out6[c] = v;
 }
 
+// Warp-aggregated counter update: lanes of a warp that hold the same key share one atomicAdd (consecutive points
+// fall into the same bin -- 256 points of a phi-ring near the origin, the 6 atoms of a face -- so per-lane atomics
+// serialise on a handful of counters).  Returns the lane's slot: value of counter[key] before the add + its rank.
+__device__ __forceinline__ int warp_agg_inc(int32_t* counter, int key, bool active) {
+  const unsigned live = __ballot_sync(0xffffffffu, active);
+  if (!active) return 0;
+  const unsigned peers = __match_any_sync(live, key);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  const int rank = __popc(peers & ((1u << lane) - 1u));
+  int base = 0;
+  if (lane == leader) base = atomicAdd(&counter[key], __popc(peers));
+  base = __shfl_sync(peers, base, leader);
+  return base + rank;
+}
+
 // ---- bin keys ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
@@ -81,16 +97,19 @@ __device__ __forceinline__ double tgt_coord(const N3Params& p, double xi, int d)
 __global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, const double* __restrict__ x, int64_t J,
                                                         int32_t* __restrict__ key, int32_t* __restrict__ hist) {
   const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
-  if (j >= J) return;
-  int b[3];
+  const bool active = j < J;
+  int k = 0;
+  if (active) {
+    int b[3];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    const double u = src_coord(p, x[3 * j + d], d);
-    b[d] = clampi((int)floor(u / p.bs), 0, p.nbs[d] - 1);
+    for (int d = 0; d < 3; ++d) {
+      const double u = src_coord(p, x[3 * j + d], d);
+      b[d] = clampi((int)floor(u / p.bs), 0, p.nbs[d] - 1);
+    }
+    k = (b[0] * p.nbs[1] + b[1]) * p.nbs[2] + b[2];
+    key[j] = k;
   }
-  const int k = (b[0] * p.nbs[1] + b[1]) * p.nbs[2] + b[2];
-  key[j] = k;
-  atomicAdd(&hist[k], 1);
+  warp_agg_inc(hist, k, active);
 }
 
 __global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const double* __restrict__ x, const double* __restrict__ w,
@@ -98,9 +117,11 @@ __global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const do
                                                            const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
                                                            SrcRec* __restrict__ out) {
   const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
-  if (j >= J) return;
-  const int k = key[j];
-  const int pos = off[k] + atomicAdd(&cursor[k], 1);
+  const bool active = j < J;
+  const int k = active ? key[j] : 0;
+  const int slot = warp_agg_inc(cursor, k, active);
+  if (!active) return;
+  const int pos = off[k] + slot;
   SrcRec r;
   const double x0 = x[3 * j], x1 = x[3 * j + 1], x2 = x[3 * j + 2];
   r.u[0] = src_coord(p, x0, 0);
@@ -122,25 +143,30 @@ __global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const do
 __global__ void __launch_bounds__(kT) target_keys_kernel(N3Params p, const double* __restrict__ xi, int64_t K,
                                                         int32_t* __restrict__ key, int32_t* __restrict__ hist) {
   const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
-  if (k >= K) return;
-  int b[3];
+  const bool active = k < K;
+  int kk = 0;
+  if (active) {
+    int b[3];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    const double u = tgt_coord(p, xi[3 * k + d], d);
-    b[d] = clampi((int)floor((u - p.t0[d]) / p.bt[d]), 0, p.nbt[d] - 1);
+    for (int d = 0; d < 3; ++d) {
+      const double u = tgt_coord(p, xi[3 * k + d], d);
+      b[d] = clampi((int)floor((u - p.t0[d]) / p.bt[d]), 0, p.nbt[d] - 1);
+    }
+    kk = (b[0] * p.nbt[1] + b[1]) * p.nbt[2] + b[2];
+    key[k] = kk;
   }
-  const int kk = (b[0] * p.nbt[1] + b[1]) * p.nbt[2] + b[2];
-  key[k] = kk;
-  atomicAdd(&hist[kk], 1);
+  warp_agg_inc(hist, kk, active);
 }
 
 __global__ void __launch_bounds__(kT) target_scatter_kernel(N3Params p, const double* __restrict__ xi, int64_t K,
                                                            const int32_t* __restrict__ key, const int32_t* __restrict__ off,
                                                            int32_t* __restrict__ cursor, TgtRec* __restrict__ out) {
   const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
-  if (k >= K) return;
-  const int kk = key[k];
-  const int pos = off[kk] + atomicAdd(&cursor[kk], 1);
+  const bool active = k < K;
+  const int kk = active ? key[k] : 0;
+  const int slot = warp_agg_inc(cursor, kk, active);
+  if (!active) return;
+  const int pos = off[kk] + slot;
   TgtRec r;
 #pragma unroll
   for (int d = 0; d < 3; ++d) r.u[d] = tgt_coord(p, xi[3 * k + d], d);
@@ -169,14 +195,7 @@ __global__ void __launch_bounds__(kT) item_fill_kernel(const int32_t* __restrict
 }
 
 // ---- A5-5 deconvolution + zero padding -----------------------------------------------------------------------
-// (w/2) phihat(kappa) = sum_q f_q cos(kappa z_q)   (QuadTable: GL in theta after z = sin theta)
-__device__ __forceinline__ double half_w_phihat(const QuadTable& q, double kappa) {
-  double acc = 0.0;
-  for (int i = 0; i < q.n; ++i) acc = __fma_rn(q.f[i], cos(kappa * q.z[i]), acc);
-  return acc;
-}
-
-__global__ void __launch_bounds__(kT) deconv_tables_kernel(N3Params p, QuadTable q, double* __restrict__ dec) {
+__global__ void __launch_bounds__(kT) deconv_tables_kernel(N3Params p, ChebTable q, double* __restrict__ dec) {
   const int i = blockIdx.x * kT + threadIdx.x;
   const int n0 = p.nf[0], n1 = p.nf[1], n2 = p.nf[2];
   if (i >= n0 + n1 + n2) return;
@@ -189,7 +208,7 @@ __global__ void __launch_bounds__(kT) deconv_tables_kernel(N3Params p, QuadTable
 }
 
 // ---- A5-9 post-deconvolution + post-phase --------------------------------------------------------------------
-__global__ void __launch_bounds__(kT) post_deconv_kernel(N3Params p, QuadTable q, const double* __restrict__ xi, int64_t K,
+__global__ void __launch_bounds__(kT) post_deconv_kernel(N3Params p, ChebTable q, const double* __restrict__ xi, int64_t K,
                                                         double2* __restrict__ nuhat) {
   const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
   if (k >= K) return;
@@ -244,12 +263,12 @@ int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int c
 }
 
 
-int deconv_tables(const N3Params& p, const QuadTable& q, double* d_dec, cudaStream_t st) {
+int deconv_tables(const N3Params& p, const ChebTable& q, double* d_dec, cudaStream_t st) {
   deconv_tables_kernel<<<blocks_for(p.nf[0] + p.nf[1] + p.nf[2]), kT, 0, st>>>(p, q, d_dec);
   return launch_check("deconv_tables_kernel");
 }
 
-int post_deconv(const N3Params& p, const QuadTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st) {
+int post_deconv(const N3Params& p, const ChebTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st) {
   post_deconv_kernel<<<blocks_for(K), kT, 0, st>>>(p, q, d_xi, K, reinterpret_cast<double2*>(d_nuhat));
   return launch_check("post_deconv_kernel");
 }
