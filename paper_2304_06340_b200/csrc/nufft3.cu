@@ -30,7 +30,6 @@ namespace {
 constexpr double kPi = 3.14159265358979323846;
 constexpr int kSrcCap = 1024;   // sources per spread work item
 constexpr int kTgtCap = 512;    // targets per interp work item
-constexpr int kMaxBin = 16;
 // fixed head of the workspace: [0,96) bounds of x and xi; [128,144) n_items_s, n_items_t, queue counters;
 // [1024, ...) scratch of the bounds reduction
 constexpr size_t kMiscBytes = 32768;
@@ -85,10 +84,10 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
     p->kap[d] = p->w * kPi / (2.0 * kSigma * S);
   }
   p->deg = p->w + 3;
-  p->bs = std::min(kMaxBin, spread_max_bin(p->w, real_c));
+  spread_bins(p->w, real_c, p->bs);
   interp_bins(p->w, p->bt);
   for (int d = 0; d < 3; ++d) {
-    p->nbs[d] = (p->nf[d] + p->bs - 1) / p->bs;
+    p->nbs[d] = (p->nf[d] + p->bs[d] - 1) / p->bs[d];
     p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
     p->nbt[d] = (p->n2[d] / 2) / p->bt[d] + 1;
     // cells any footprint can touch: ceil(n2/4 - w/2) ... ceil(3 n2/4 - w/2) + w - 1, plus one cell of slack

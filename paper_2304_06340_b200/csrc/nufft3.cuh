@@ -20,7 +20,7 @@ struct N3Params {
   double st[3];       // target  -> inner-grid coordinate: u2 = (xi - D) st + n2/2, st = n2 / (2 sigma S)
   double kap[3];      // target  -> argument of phihat:    kappa = (xi - D) kap,    kap = w pi / (2 sigma S)
   int real_c;         // 1 when D == 0: the strengths c'_j = w_j stay real and so does the fine grid
-  int bs, nbs[3];     // source bins: bs^3 cells, nbs[d] = ceil(nf[d] / bs)
+  int bs[3], nbs[3];  // source bins: bs[0] x bs[1] x bs[2] cells (bs[2] = 8 or 16), nbs[d] = ceil(nf[d] / bs[d])
   int bt[3], nbt[3], t0[3];  // target bins (bt[0] x bt[1] x bt[2] cells) over the band [t0, t0 + nbt*bt) of the
                              // inner grid that holds every target; bt[2] is 8 or 16 (bank-conflict-free pitch)
   int deg;                   // degree of the piecewise-polynomial kernel evaluation (w + 3)
@@ -77,7 +77,7 @@ __device__ __forceinline__ void footprint(double u, int w, int& i0, double& s) {
 // ---- spread.cu (A5-4) ------------------------------------------------------------------------------------
 // Work item i: sources [item_start[i], item_start[i]+item_count[i]) of bin item_bin[i].  *n_items on the device.
 // grid is real double[nf0][nf1][nf2] (real_c) or complex double[nf0][nf1][nf2][2]; must be zero on entry.
-int spread_max_bin(int w, bool real_c);   // largest bin edge whose padded subgrid fits shared memory
+void spread_bins(int w, bool real_c, int bs[3]);   // source-bin shape for kernel width w
 size_t spread_smem_bytes(const N3Params& p);
 int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
            const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st);

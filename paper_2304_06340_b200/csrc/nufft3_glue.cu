@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, const doubl
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       const double u = src_coord(p, x[3 * j + d], d);
-      b[d] = clampi((int)floor(u / p.bs), 0, p.nbs[d] - 1);
+      b[d] = clampi((int)floor(u / p.bs[d]), 0, p.nbs[d] - 1);
     }
     k = (b[0] * p.nbs[1] + b[1]) * p.nbs[2] + b[2];
     key[j] = k;
