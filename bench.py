@@ -262,6 +262,7 @@ def main():
     c, J, K, q = r["c"], r["J"], r["K"], r["q"]
     world, rank = r["world"], r["rank"]
 
+    torch.cuda.empty_cache()   # the host-buffer calls allocate from the CUDA pool: hand torch's cached blocks back
     # ---- e2e: the same step through the host-buffer entry point (pinned host mesh in, distance out) ----------
     Vh = (r["Vj"] if r["Vj"] is not None else r["V"]).cpu().pin_memory()
     Fh = r["F"].cpu().pin_memory()

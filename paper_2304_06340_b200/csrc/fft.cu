@@ -24,7 +24,7 @@
 namespace sfd {
 namespace {
 
-constexpr int kFftThreads = 256;
+constexpr int kFftThreads = 512;
 
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, const 
                                                               double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* a = reinterpret_cast<double2*>(smem_raw);
-  const int N = P.N, tb = P.tb, tbp = tb | 1, tid = threadIdx.x;
+  const int N = P.N, tb = P.tb, tbp = P.tbp, tid = threadIdx.x;
   const int64_t tiles_per_hi = (P.n_lo + tb - 1) / tb;
   const int64_t hi = blockIdx.x / tiles_per_hi;
   const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * tb;
@@ -88,7 +88,8 @@ __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, const 
     const int nbf = N / r;
     for (int idx = tid; idx < (nbf << tsh); idx += kFftThreads) {
       const int bf = idx >> tsh, col = idx & (tb - 1);
-      const int b = bf / Ls, j = bf - b * Ls;
+      const int b = Ls == 1 ? bf : (int)__umulhi((unsigned)bf, P.magic[s]);   // bf / Ls (exact: bf < 2^16)
+      const int j = bf - b * Ls;
       double2* x = a + (b * L + j) * tbp + col;
       const int st = Ls * tbp;
       const int tj = j * tstep;
@@ -207,20 +208,25 @@ size_t fft_tables_bytes(const int n2[3]) {
   return b;
 }
 
-int fft_tile(int N) {
-  // two CTAs per SM when possible (load/compute overlap), else one; tb is a power of two
-  for (int tb = 8; tb >= 1; tb >>= 1)
-    if ((size_t)N * (tb | 1) * 16 <= (size_t)110 * 1024) return tb;
-  for (int tb = 8; tb >= 1; tb >>= 1)
-    if ((size_t)N * (tb | 1) * 16 <= (size_t)224 * 1024) return tb;
-  return 0;
+// Rows per tile (a power of two) and row pitch.  Two CTAs per SM whenever at least 4 rows fit in half the shared
+// memory (one CTA's loads and stores overlap the other's butterflies), else one CTA per SM.  Only the transposing
+// load of the contiguous-axis pass needs the odd pitch.
+int fft_tile(int N, int contig, int* tbp) {
+  auto pitch = [&](int tb) { return contig ? (tb | 1) : tb; };
+  int pick = 0;
+  for (int tb = 8; tb >= 4 && !pick; tb >>= 1)
+    if ((size_t)N * pitch(tb) * 16 <= (size_t)112 * 1024) pick = tb;
+  for (int tb = 8; tb >= 1 && !pick; tb >>= 1)
+    if ((size_t)N * pitch(tb) * 16 <= (size_t)224 * 1024) pick = tb;
+  if (tbp) *tbp = pick ? pitch(pick) : 0;
+  return pick;
 }
 
 int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStream_t st) {
   char* base = static_cast<char*>(d_tables);
   size_t o = 0;
   for (int d = 0; d < 3; ++d) {
-    SFD_REQUIRE(fft_length_ok(n2[d]) && fft_tile(n2[d]) > 0, SFD_ERR_UNSUPPORTED, "FFT length %d is not supported", n2[d]);
+    SFD_REQUIRE(fft_length_ok(n2[d]) && fft_tile(n2[d], 1, nullptr) > 0, SFD_ERR_UNSUPPORTED, "FFT length %d is not supported", n2[d]);
     const HostTables& t = tables_for(n2[d]);
     out->tw[d] = reinterpret_cast<double2*>(base + o);
     SFD_CUDA_TRY(cudaMemcpyAsync(base + o, t.tw.data(), (size_t)n2[d] * 16, cudaMemcpyHostToDevice, st));
@@ -239,13 +245,21 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   P.rev = T.rev[axis];
   P.nfac = T.nfac[axis];
   for (int s = 0; s < P.nfac; ++s) P.fac[s] = T.fac[axis][s];
-  P.tb = fft_tile(P.N);
+  P.tb = fft_tile(P.N, P.contig, &P.tbp);
   P.tb_shift = 0;
   while ((1 << P.tb_shift) < P.tb) ++P.tb_shift;
+  {
+    int L = P.N;
+    for (int s = 0; s < P.nfac; ++s) {
+      const int Ls = L / P.fac[s];
+      P.magic[s] = Ls > 1 ? (unsigned)(0x100000000ULL / (unsigned long long)Ls + 1ULL) : 0u;
+      L = Ls;
+    }
+  }
   const int64_t tiles = P.n_hi * ((P.n_lo + P.tb - 1) / P.tb);
   if (tiles == 0) return SFD_OK;
   SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
-  const size_t smem = (size_t)P.N * (P.tb | 1) * 16;
+  const size_t smem = (size_t)P.N * P.tbp * 16;
   static bool attr[2] = {false, false};
   if (!attr[P.real_in]) {
     if (P.real_in)

@@ -26,13 +26,14 @@ struct FftPass {
   int contig, real_in;
   const double *dec_axis, *dec_hi, *dec_lo;
   // filled in by fft_pass():
-  int tb, tb_shift, nfac, fac[16];
+  int tb, tbp, tb_shift, nfac, fac[16];
+  unsigned magic[16];   // floor(2^32 / Ls) + 1 per stage: bf / Ls = umulhi(bf, magic)
   const double2* tw;
   const int32_t* rev;
 };
 
 bool fft_length_ok(int N);
-int fft_tile(int N);                                   // rows per tile (0: does not fit shared memory)
+int fft_tile(int N, int contig, int* tbp);             // rows per tile (0: does not fit shared memory) and pitch
 size_t fft_tables_bytes(const int n2[3]);
 int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStream_t st);
 int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* d_out, cudaStream_t st);
