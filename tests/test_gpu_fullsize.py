@@ -1,0 +1,128 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (-m gpu).
+
+The CPU oracle cannot afford J x K at configs 2-5 (3e10 ... 5e14 pairs): it checks a seeded sample of targets one by
+one (reading R14), the GPU direct sum -- itself oracle-checked in test_gpu_parity.py and here on the
+sample -- checks a larger sample, and properties that hold at any size (Hermitian symmetry of nuhat for real weights,
+nuhat(0) = area, quadratic rate) cover the rest.  Bars: direct 1e-12 sum|w|; NUFFT 10 eps sum|w|; I per R13.
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sfd():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2304_06340_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+def _workload(sfd, torch, cfg_id, level=None):
+    c = workloads.CONFIGS[cfg_id]
+    level = c["level"] if level is None else level
+    V, F = sfd.sfd_mesh_icosphere(level)
+    if c["jitter"]:
+        Vj = workloads.jitter_vertices(V.cpu().numpy(), F.cpu().numpy(), *c["jitter"])
+        V = torch.as_tensor(Vj, device="cuda")
+    x, w = sfd.sfd_nodes(V, F, c["rule"])
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    xi, W = sfd.sfd_freq_nodes_device(q, c["R"])
+    return c, V, F, x, w, xi, W, q
+
+
+def _check_nufft(sfd, orc, torch, x, w, xi, eps, n_gpu=4096, n_cpu=96):
+    K = xi.shape[0]
+    sw = float(w.abs().sum())
+    nu = sfd.sfd_surface_ft(x, w, xi, eps)
+    idx = torch.as_tensor(workloads.target_subset(K, n_gpu, seed=0), device="cuda")
+    ref = sfd.sfd_surface_ft(x, w, xi[idx].contiguous(), 0.0)
+    err = float((nu[idx] - ref).abs().max()) / sw
+    assert err <= 10 * eps, (err, eps)
+    # the GPU direct sum on the same sample against the oracle (one target at a time on the CPU)
+    sub = idx[:n_cpu]
+    oref = orc.direct_sum(x.cpu().numpy(), w.cpu().numpy(), xi[sub].cpu().numpy())
+    derr = np.abs(ref[:n_cpu].cpu().numpy() - oref).max() / sw
+    assert derr <= 1e-12, derr
+    return nu, err
+
+
+def _i_bound(W, xi, s, eps, sw):
+    """R13: E^2 = (2 pi)^-3 sum_k W_k (10 eps sum|w|)^2 (1+r^2)^-s."""
+    r2 = (xi * xi).sum(1)
+    return float((W * (1 + r2) ** (-s)).sum()) * (10 * eps * sw) ** 2 / (2 * np.pi) ** 3
+
+
+def test_config2_full(sfd, orc, torch):
+    """Config 2: NUFFT (eps 1e-9) against the direct sum at ALL 1,048,576 targets; I by both paths, s = 1, 2."""
+    c, V, F, x, w, xi, W, q = _workload(sfd, torch, 2)
+    sw = float(w.sum())
+    nu_d = sfd.sfd_surface_ft(x, w, xi, 0.0)
+    nu_n = sfd.sfd_surface_ft(x, w, xi, 1e-9)
+    assert float((nu_d - nu_n).abs().max()) <= 10 * 1e-9 * sw
+    # any-size properties: nuhat(xi) for real weights is Hermitian; the quadrature is symmetric under xi -> -xi
+    # (mu_b -> mu_{n-1-b}, phi_c -> phi_{c+n/2}); central symmetry of the icosphere makes nuhat real
+    assert float(nu_d.imag.abs().max()) <= 1e-12 * sw
+    nr, nt, nph = q
+    g = nu_d.real.reshape(nr, nt, nph)
+    mirror = torch.roll(torch.flip(g, dims=[1]), shifts=nph // 2, dims=2)
+    assert float((g - mirror).abs().max()) <= 1e-11 * sw
+    for s in c["s"]:
+        d0, I0 = sfd.sfd_weak_distance(V, F, c["rule"], s, c["R"], q, 0.0)
+        d1, I1 = sfd.sfd_weak_distance(V, F, c["rule"], s, c["R"], q, 1e-9)
+        I_red = sfd.sfd_reduce(nu_d, xi, W, s)
+        assert abs(I0 - I_red) <= 1e-12 * I0
+        E2 = _i_bound(W, xi, s, 1e-9, sw)
+        assert abs(I1 - I0) <= 2 * np.sqrt(I0 * E2) + E2, (I1, I0, E2)
+    # SURVEY 8(c) pin 5 digits for level 4 on this grid (a cross-check computed independently of both sides)
+    d_s2, _ = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 0.0)
+    assert abs(d_s2 - 1.5501793453e-3) <= 1e-9
+
+
+@pytest.mark.parametrize("eps", [1e-6, 1e-12])
+def test_config3_sampled(sfd, orc, torch, eps):
+    """Config 3 (level 6, 12-pt rule, 983,040 sources; 8,388,608 targets)."""
+    c, V, F, x, w, xi, W, q = _workload(sfd, torch, 3)
+    _check_nufft(sfd, orc, torch, x, w, xi, eps)
+
+
+def test_config4_sampled(sfd, orc, torch):
+    """Config 4 (level 7 with radial jitter: Im nuhat != 0; 1,966,080 sources; 28,311,552 targets), eps 1e-9."""
+    c, V, F, x, w, xi, W, q = _workload(sfd, torch, 4)
+    nu, err = _check_nufft(sfd, orc, torch, x, w, xi, 1e-9, n_gpu=2048, n_cpu=48)
+    assert float(nu.imag.abs().max()) > 1e-6   # the jitter breaks the central symmetry
+    d, I = sfd.sfd_weak_distance(V, F, c["rule"], 1.0, c["R"], q, 1e-9)
+    I_red = sfd.sfd_reduce(nu, xi, W, 1.0)
+    assert abs(I - I_red) <= 1e-9 * I
+
+
+def test_config5_sweep_levels(sfd, orc, torch):
+    """Config 5: the fixed 512x256x512 = 67,108,864-target grid on [0,1024] (n2 = 2700, pruned FFT), eps 1e-10, levels
+    2..5 of the sweep: sampled parity at level 3 and the rate in h for s = 2 (P:5; R15).  On this grid the
+    radial rule is marginal (512 nodes for a phase 2R = 2048, SURVEY 8(c) pin 3), which biases sqrt(I) upwards at high
+    frequency: the observed slopes are 1.88-1.91 instead of the 1.99-2.00 of the well-resolved R = 32 / 128 grids
+    (tests/test_oracle_pins.py asserts [1.9, 2.1] there).  Asserted here: [1.8, 2.1]."""
+    c = workloads.CONFIGS[5]
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    dist = {}
+    for level in (2, 3, 4, 5):
+        V, F = sfd.sfd_mesh_icosphere(level)
+        dist[level] = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 1e-10)[0]
+        if level == 3:
+            x, w = sfd.sfd_nodes(V, F, c["rule"])
+            xi, W = sfd.sfd_freq_nodes_device(q, c["R"])
+            _check_nufft(sfd, orc, torch, x, w, xi, 1e-10, n_gpu=4096, n_cpu=256)
+            del xi, W
+        torch.cuda.empty_cache()
+    for level in (3, 4, 5):
+        slope = np.log2(dist[level - 1] / dist[level])
+        assert 1.8 <= slope <= 2.1, (level, slope, dist)
