@@ -337,18 +337,26 @@ def main():
         w, nf, n2 = P.sfd_surface_ft_plan(J, K, [r["ext"]] * 3, [c["R"]] * 3, eps)
         cell = 8      # ball-centred targets: real strengths, real fine grid
         fine = nf[0] * nf[1] * nf[2] * cell
-        band = 1
-        for d in range(3):
-            band *= n2[d] // 2 + w + 1
+        no = [min(n2[d], n2[d] // 2 + w + 3) for d in range(3)]
+        band = no[0] * no[1] * no[2]
+        pa, pb = nf[0] * nf[1] * no[2], nf[0] * no[1] * no[2]
         sp_bytes = 2 * fine + 40 * J            # zero-fill + one accumulation pass of the grid + sorted sources
-        ip_bytes = 16 * band + (32 + 16) * K    # the band of the inner grid that holds targets, records in, G out
-        for name, nbytes in (("spread", sp_bytes), ("interp", ip_bytes)):
+        ip_bytes = 16 * band + (32 + 16) * K    # the band of the inner grid, target records in, G out
+        ft_bytes = fine + 16 * (2 * pa + 2 * pb + band)   # three passes: read non-zero rows, write the band
+        smem_peak = 128.0 * 148 * sm_mhz * 1e6 * 1e-9     # GB/s of shared memory, 128 B/clk/SM
+        for name, kern, nbytes in (("spread", "spread_kernel", sp_bytes), ("fft", "fft_pass_kernel x3", ft_bytes),
+                                   ("interp", "interp_kernel", ip_bytes)):
             ach = nbytes / (st[name] * 1e-3) * 1e-9
-            extra.append({"kernel": f"{name}_kernel", "eps": eps, "w": w, "nf": nf[0], "n2": n2[0], "bound": "hbm",
-                          "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                          "ms_per_launch": st[name], "algorithmic_bytes": nbytes, "peak_source": hbm_src})
+            e = {"kernel": kern, "eps": eps, "w": w, "nf": nf[0], "n2": n2[0], "bound": "hbm",
+                 "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                 "ms_per_launch": st[name], "algorithmic_bytes": nbytes, "peak_source": hbm_src}
+            if name == "interp":   # the roof that actually binds the gather: 16 w^3 B of shared memory per target
+                sm_ach = 16.0 * w ** 3 * K / (st[name] * 1e-3) * 1e-9
+                e.update({"binding_roof": "shared memory", "smem_achieved_gbs": sm_ach, "smem_peak_gbs": smem_peak,
+                          "smem_frac": sm_ach / smem_peak})
+            extra.append(e)
         if roofline is None:
-            roofline = dict(extra[-1], traffic=None)
+            roofline = dict(max(extra, key=lambda e: e["ms_per_launch"]), traffic=None)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

@@ -85,6 +85,13 @@ int sfd_freq_nodes_workspace(const sfd_freq_quadrature* q, size_t* bytes);
 int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi /*[K][3]*/, double* d_W /*[K] or NULL*/,
                           void* d_work, size_t work_bytes, sfd_stream stream);
 
+/* The nodes of the radial shells a in [a_begin, a_end) only: (a_end - a_begin) * n_theta * n_phi nodes, in the same
+ * order as the full rule (node k of the full rule is node k - a_begin*n_theta*n_phi here).  The ball rule is a sum
+ * over shells, so disjoint ranges partition the quadrature: this is how the targets are sharded over GPUs (DESIGN.md
+ * "Multi-GPU"; partial sums I of sfd_reduce add up).  Same workspace as sfd_freq_nodes_device. */
+int sfd_freq_nodes_device_range(const sfd_freq_quadrature* q, double R, int32_t a_begin, int32_t a_end,
+                                double* d_xi, double* d_W, void* d_work, size_t work_bytes, sfd_stream stream);
+
 /* ---- A4/A5: Fourier transform of the atomic measure nu = sum_j w_j delta_{x_j} -----------------
  * nuhat_k = sum_{j<J} w_j exp(-i xi_k . x_j)   (eq. 2.8 applied to the atoms of P:152).
  *   eps == 0        : fp64 direct summation, error <= 1e-12 * sum|w_j| for |xi.x| <~ 2e3.

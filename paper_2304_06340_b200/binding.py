@@ -45,6 +45,8 @@ _SIGS = {
     "sfd_freq_nodes": (C.c_int, [_P(sfd_freq_quadrature), _dbl, _vp, _vp]),
     "sfd_freq_nodes_workspace": (C.c_int, [_P(sfd_freq_quadrature), _P(_sz)]),
     "sfd_freq_nodes_device": (C.c_int, [_P(sfd_freq_quadrature), _dbl, _vp, _vp, _vp, _sz, _vp]),
+    "sfd_freq_nodes_device_range": (C.c_int, [_P(sfd_freq_quadrature), _dbl, C.c_int32, C.c_int32, _vp, _vp, _vp, _sz,
+                                              _vp]),
     "sfd_surface_ft_workspace": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(_sz)]),
     "sfd_surface_ft_plan": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(C.c_int32), _P(_i64), _P(_i64)]),
     "sfd_surface_ft": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp, _vp, _sz, _vp]),
@@ -156,6 +158,20 @@ def sfd_freq_nodes_device(q, R, device="cuda"):
     W = torch.empty((K,), dtype=torch.float64, device=device)
     work = _work(wb.value, device)
     _chk(_lib.sfd_freq_nodes_device(C.byref(q), float(R), _ptr(xi), _ptr(W), _ptr(work), work.numel(), _stream()))
+    return xi, W
+
+
+def sfd_freq_nodes_device_range(q, R, a_begin, a_end, device="cuda"):
+    """Nodes of the radial shells [a_begin, a_end) of the ball quadrature (a shard of the targets)."""
+    q = _quad(q)
+    wb = _sz()
+    _chk(_lib.sfd_freq_nodes_workspace(C.byref(q), C.byref(wb)))
+    K = (int(a_end) - int(a_begin)) * q.n_theta * q.n_phi
+    xi = torch.empty((K, 3), dtype=torch.float64, device=device)
+    W = torch.empty((K,), dtype=torch.float64, device=device)
+    work = _work(wb.value, device)
+    _chk(_lib.sfd_freq_nodes_device_range(C.byref(q), float(R), int(a_begin), int(a_end), _ptr(xi), _ptr(W),
+                                          _ptr(work), work.numel(), _stream()))
     return xi, W
 
 

@@ -176,6 +176,18 @@ int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi, 
   return freq_expand(q, t, d_xi, d_W, d_work, work_bytes, as_stream(stream));
 }
 
+int sfd_freq_nodes_device_range(const sfd_freq_quadrature* q, double R, int32_t a_begin, int32_t a_end, double* d_xi,
+                                double* d_W, void* d_work, size_t work_bytes, sfd_stream stream) {
+  SFD_TRY(check_quadrature(q, R));
+  SFD_REQUIRE(a_begin >= 0 && a_begin <= a_end && a_end <= q->n_r, SFD_ERR_INVALID_ARG,
+              "radial range [%d,%d) outside [0,%d)", a_begin, a_end, q->n_r);
+  if (a_begin == a_end) return SFD_OK;
+  SFD_REQUIRE(d_xi, SFD_ERR_NULL, "sfd_freq_nodes_device_range: NULL output");
+  FreqTables t;
+  SFD_TRY(freq_tables(q, R, t));
+  return freq_expand(q, t, d_xi, d_W, d_work, work_bytes, as_stream(stream), a_begin, a_end);
+}
+
 // ---- A4/A5 ----------------------------------------------------------------------------------------
 int sfd_surface_ft_workspace(int64_t J, int64_t K, const double X[3], const double S[3], double eps, size_t* bytes) {
   SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_surface_ft_workspace: bytes is NULL");

@@ -23,8 +23,9 @@ int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t);
 // n-point Gauss-Legendre rule on [-1,1] (ascending), long double Newton iteration (host)
 void gauss_legendre_host(int n, std::vector<long double>& t, std::vector<long double>& wt);
 size_t freq_tables_bytes(const sfd_freq_quadrature* q);
+// radial shells [a0, a1) only (a1 < 0: all of them)
 int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
-                size_t work_bytes, cudaStream_t st);
+                size_t work_bytes, cudaStream_t st, int a0 = 0, int a1 = -1);
 int rule_table_host(int rule, double* lam, double* om);
 int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rule, double* d_x, double* d_w,
           cudaStream_t st);

@@ -126,15 +126,17 @@ void legendre_rule(int n, std::vector<long double>& t, std::vector<long double>&
   if (n & 1) t[n / 2] = 0.0L;
 }
 
+// Nodes of the radial shells [a0, a1) (a0 = 0, a1 = n_r: the whole rule); output index k - a0 n_th n_ph.
 __global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restrict__ tab, int n_r, int n_th, int n_ph,
-                                                          double wph, double* __restrict__ xi, double* __restrict__ W) {
-  const int64_t K = (int64_t)n_r * n_th * n_ph;
+                                                          int a0, int a1, double wph, double* __restrict__ xi,
+                                                          double* __restrict__ W) {
+  const int64_t K = (int64_t)(a1 - a0) * n_th * n_ph;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= K) return;
   const int c = (int)(k % n_ph);
   const int64_t ab = k / n_ph;
   const int b = (int)(ab % n_th);
-  const int a = (int)(ab / n_th);
+  const int a = a0 + (int)(ab / n_th);
   const double* r = tab;
   const double* wr = r + n_r;
   const double* mu = wr + n_r;
@@ -211,7 +213,10 @@ size_t freq_tables_bytes(const sfd_freq_quadrature* q) {
 }
 
 int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
-                size_t work_bytes, cudaStream_t st) {
+                size_t work_bytes, cudaStream_t st, int a0, int a1) {
+  if (a1 < 0) a1 = q->n_r;
+  SFD_REQUIRE(0 <= a0 && a0 <= a1 && a1 <= q->n_r, SFD_ERR_INVALID_ARG, "radial range [%d,%d) outside [0,%d)", a0, a1,
+              q->n_r);
   SFD_REQUIRE(work_bytes >= freq_tables_bytes(q) && d_work, SFD_ERR_WORKSPACE_TOO_SMALL,
               "frequency quadrature needs %zu workspace bytes, got %zu", freq_tables_bytes(q), work_bytes);
   std::vector<double> h;
@@ -219,9 +224,10 @@ int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi,
   for (const auto* v : {&t.r, &t.wr, &t.mu, &t.st, &t.wmu, &t.cph, &t.sph}) h.insert(h.end(), v->begin(), v->end());
   // pageable source: the runtime stages the copy before returning, so `h` may die at scope exit
   SFD_CUDA_TRY(cudaMemcpyAsync(d_work, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-  const int64_t K = (int64_t)q->n_r * q->n_theta * q->n_phi;
+  const int64_t K = (int64_t)(a1 - a0) * q->n_theta * q->n_phi;
+  if (K == 0) return SFD_OK;
   freq_expand_kernel<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(static_cast<const double*>(d_work), q->n_r,
-                                                                   q->n_theta, q->n_phi, t.wph, d_xi, d_W);
+                                                                   q->n_theta, q->n_phi, a0, a1, t.wph, d_xi, d_W);
   return launch_check("freq_expand_kernel");
 }
 

@@ -227,3 +227,26 @@ def test_nufft_random_clouds(sfd, orc, torch, J, K, eps):
     """Off-centre sources (C != 0), off-centre targets (D != 0, complex strengths), signed weights."""
     x, w, xi = workloads.random_cloud(J, K)
     _nufft_case(sfd, orc, torch, x, w, xi, eps)
+
+
+# ---- multi-GPU path on one GPU: the ranks' shards evaluated one after the other ----------------------
+@pytest.mark.parametrize("eps,world", [(0.0, 3), (1e-9, 4)])
+def test_target_shards_add_up(sfd, orc, torch, eps, world):
+    """The partial sums of disjoint radial shards (what each rank of sharding.weak_distance_sharded computes) add up
+    to the unsharded I; the shard nodes are the full rule's nodes."""
+    from paper_2304_06340_b200 import sharding
+    c = workloads.CONFIGS[1]
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    V, F = sfd.sfd_mesh_icosphere(c["level"])
+    d_full, I_full = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, eps)
+    xi_full, W_full = sfd.sfd_freq_nodes_device(q, c["R"])
+    n = q[1] * q[2]
+    I_sum = 0.0
+    for rank in range(world):
+        a0, a1 = sharding.shard_of(q[0], rank, world, eps)
+        xi, W = sfd.sfd_freq_nodes_device_range(q, c["R"], a0, a1)
+        assert torch.equal(xi, xi_full[a0 * n:a1 * n]) and torch.equal(W, W_full[a0 * n:a1 * n])
+        d, I = sharding.weak_distance_sharded(V, F, c["rule"], 2.0, c["R"], q, eps, rank=rank, world_size=world)
+        I_sum += I          # no process group: each call returns its own partial sum
+    tol = 1e-12 if eps == 0.0 else 1e-7   # every shard's type-3 transform has its own grids (errors <= 10 eps sum|w|)
+    assert abs(I_sum - I_full) <= tol * I_full
