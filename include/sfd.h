@@ -17,7 +17,9 @@
  *   - NULL pointer where one is required -> SFD_ERR_NULL; out-of-range scalar -> SFD_ERR_INVALID_ARG;
  *     n == 0 (no faces / sources / targets) is valid and yields empty or zero output.
  *   - sfd_last_error() returns a thread-local, human-readable description of the last failure.
- *   - Process-global state: a small cache of cuFFT plans keyed by grid shape (sfd_release_cache()).
+ *   - Process-global state: host-side caches of quadrature / kernel / FFT tables (pure functions of their keys), and
+ *     the device's stream-ordered memory pool, in which the host-buffer entry points keep their workspaces between
+ *     calls (sfd_release_cache() trims it).
  */
 #ifndef SFD_H_
 #define SFD_H_
@@ -56,7 +58,7 @@ typedef void* sfd_stream; /* cudaStream_t */
 const char* sfd_last_error(void);
 /* Library version string and the CUDA arch it was compiled for ("sm_100a"). */
 const char* sfd_version(void);
-/* Drops cached cuFFT plans.  Synchronises the device. */
+/* Returns the memory kept in the device's stream-ordered pool to the driver.  Synchronises the device. */
 int sfd_release_cache(void);
 
 /* ---- A1/A2: icosahedral discretization T_level ------------------------------------

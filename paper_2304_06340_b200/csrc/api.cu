@@ -97,6 +97,10 @@ const char* sfd_version(void) { return "sfd 0.1 (sm_100a)"; }
 
 int sfd_release_cache(void) {
   cudaDeviceSynchronize();
+  int dev = 0;
+  cudaMemPool_t pool;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess)
+    cudaMemPoolTrimTo(pool, 0);   // workspaces kept by the host-buffer entry points
   return nufft3_release_cache();
 }
 
@@ -360,6 +364,18 @@ struct HostCall {
   void* bufs[8] = {};
   int n = 0;
   int open() {
+    // keep freed workspaces in the device's stream-ordered pool between calls (the default threshold of 0 hands
+    // them back to the driver at every synchronisation, which costs tens of ms per call at GB sizes)
+    static thread_local int pooled_dev = -1;
+    int dev = 0;
+    SFD_CUDA_TRY(cudaGetDevice(&dev));
+    if (pooled_dev != dev) {
+      cudaMemPool_t pool;
+      SFD_CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
+      unsigned long long keep = ~0ULL;
+      SFD_CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+      pooled_dev = dev;
+    }
     SFD_CUDA_TRY(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
     return SFD_OK;
   }

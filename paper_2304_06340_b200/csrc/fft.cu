@@ -24,7 +24,6 @@
 namespace sfd {
 namespace {
 
-constexpr int kFftThreads = 512;
 
 __device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
@@ -34,10 +33,115 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
 __device__ __forceinline__ double2 mul_mi(double2 a) { return make_double2(a.y, -a.x); }   // a * (-i)
 __device__ __forceinline__ double2 mul_pi(double2 a) { return make_double2(-a.y, a.x); }   // a * (+i)
 
-// One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128, tbp = tb | 1.
-template <bool REAL_IN>
-__global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, const void* __restrict__ in_raw,
-                                                              double2* __restrict__ out) {
+// ---- radix-R butterflies on register arrays: x <- DFT_R(x), forward sign, natural output order -------------------
+template <int R>
+__device__ __forceinline__ void bfly(double2 (&x)[R]);
+template <>
+__device__ __forceinline__ void bfly<1>(double2 (&)[1]) {}
+template <>
+__device__ __forceinline__ void bfly<2>(double2 (&x)[2]) {
+  const double2 a = x[0], b = x[1];
+  x[0] = cadd(a, b);
+  x[1] = csub(a, b);
+}
+template <>
+__device__ __forceinline__ void bfly<3>(double2 (&x)[3]) {
+  const double2 x0 = x[0], x1 = x[1], x2 = x[2];
+  const double2 t1 = cadd(x1, x2);
+  const double2 t2 = make_double2(x0.x - 0.5 * t1.x, x0.y - 0.5 * t1.y);
+  const double h = 0.86602540378443864676;
+  const double2 t3 = make_double2(h * (x1.x - x2.x), h * (x1.y - x2.y));
+  x[0] = cadd(x0, t1);
+  x[1] = cadd(t2, mul_mi(t3));
+  x[2] = cadd(t2, mul_pi(t3));
+}
+template <>
+__device__ __forceinline__ void bfly<4>(double2 (&x)[4]) {
+  const double2 t0 = cadd(x[0], x[2]), t1 = csub(x[0], x[2]), t2 = cadd(x[1], x[3]), t3 = csub(x[1], x[3]);
+  x[0] = cadd(t0, t2);
+  x[1] = cadd(t1, mul_mi(t3));
+  x[2] = csub(t0, t2);
+  x[3] = cadd(t1, mul_pi(t3));
+}
+template <>
+__device__ __forceinline__ void bfly<5>(double2 (&x)[5]) {
+  const double2 x0 = x[0], x1 = x[1], x2 = x[2], x3 = x[3], x4 = x[4];
+  const double c1 = 0.30901699437494742410, c2 = -0.80901699437494742410;
+  const double s1 = 0.95105651629515357212, s2 = 0.58778525229247312917;
+  const double2 t1 = cadd(x1, x4), t2 = cadd(x2, x3), t3 = csub(x1, x4), t4 = csub(x2, x3);
+  const double2 a1 = make_double2(x0.x + c1 * t1.x + c2 * t2.x, x0.y + c1 * t1.y + c2 * t2.y);
+  const double2 a2 = make_double2(x0.x + c2 * t1.x + c1 * t2.x, x0.y + c2 * t1.y + c1 * t2.y);
+  const double2 b1 = make_double2(s1 * t3.x + s2 * t4.x, s1 * t3.y + s2 * t4.y);
+  const double2 b2 = make_double2(s2 * t3.x - s1 * t4.x, s2 * t3.y - s1 * t4.y);
+  x[0] = make_double2(x0.x + t1.x + t2.x, x0.y + t1.y + t2.y);
+  x[1] = cadd(a1, mul_mi(b1));
+  x[2] = cadd(a2, mul_mi(b2));
+  x[3] = cadd(a2, mul_pi(b2));
+  x[4] = cadd(a1, mul_pi(b1));
+}
+
+// Two consecutive decimation-in-frequency stages (radices R1 then R2; R2 = 1: a single stage) fused in registers:
+// a thread owns the R1 R2 elements b L + j' + q1 L/R1 + q2 L/(R1 R2) of one row, which stage s (radix R1 over q1, twiddle
+// w_L^{(j' + q2 Lq) p1}) and stage s+1 (radix R2 over q2 inside block (b, p1), twiddle w_{L/R1}^{j' p2}) map onto
+// themselves: one shared-memory round trip instead of two.
+template <int R1, int R2>
+__device__ __forceinline__ void fused_stages(double2* __restrict__ a, const double2* __restrict__ tw, int N, int L,
+                                             unsigned magic, int tb, int tbp, int tsh, int tid, int nthreads) {
+  constexpr int R = R1 * R2;
+  const int Lq = L / R;              // j' range
+  const int L1 = L / R1;             // stride of q1
+  const int tstep = N / L;           // twiddle index step of stage s; stage s+1 uses tstep * R1
+  const int ngroups = N / R;
+  for (int idx = tid; idx < (ngroups << tsh); idx += nthreads) {
+    const int g = idx >> tsh, col = idx & (tb - 1);
+    const int b = Lq == 1 ? g : (int)__umulhi((unsigned)g, magic);   // g / Lq
+    const int jp = g - b * Lq;
+    double2* base = a + (b * L + jp) * tbp + col;
+    double2 v[R1][R2];
+#pragma unroll
+    for (int q1 = 0; q1 < R1; ++q1)
+#pragma unroll
+      for (int q2 = 0; q2 < R2; ++q2) v[q1][q2] = base[(q1 * L1 + q2 * Lq) * tbp];
+    // stage s
+#pragma unroll
+    for (int q2 = 0; q2 < R2; ++q2) {
+      double2 x[R1];
+#pragma unroll
+      for (int q1 = 0; q1 < R1; ++q1) x[q1] = v[q1][q2];
+      bfly<R1>(x);
+      const int tj = (jp + q2 * Lq) * tstep;
+      v[0][q2] = x[0];
+#pragma unroll
+      for (int p1 = 1; p1 < R1; ++p1) v[p1][q2] = cmul(x[p1], tw[p1 * tj]);
+    }
+    // stage s+1
+    if (R2 > 1) {
+      const int tj2 = jp * tstep * R1;
+#pragma unroll
+      for (int p1 = 0; p1 < R1; ++p1) {
+        double2 x[R2];
+#pragma unroll
+        for (int q2 = 0; q2 < R2; ++q2) x[q2] = v[p1][q2];
+        bfly<R2>(x);
+        v[p1][0] = x[0];
+#pragma unroll
+        for (int p2 = 1; p2 < R2; ++p2) v[p1][p2] = cmul(x[p2], tw[p2 * tj2]);
+      }
+    }
+#pragma unroll
+    for (int p1 = 0; p1 < R1; ++p1)
+#pragma unroll
+      for (int p2 = 0; p2 < R2; ++p2) base[(p1 * L1 + p2 * Lq) * tbp] = v[p1][p2];
+  }
+}
+
+// One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
+// 1024 with one (long transforms): 32 warps per SM either way -- the stages are latency-bound (shared-memory and
+// twiddle loads feeding short FP64 chains), so occupancy is what buys throughput (profiles/r1c_nufft.md).
+template <bool REAL_IN, int THREADS>
+__global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 1 : 2)
+fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
+  constexpr int kFftThreads = THREADS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* a = reinterpret_cast<double2*>(smem_raw);
   const int N = P.N, tb = P.tb, tbp = P.tbp, tid = threadIdx.x;
@@ -48,89 +152,74 @@ __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, const 
   const int tsh = P.tb_shift;
   const double2* __restrict__ tw = P.tw;
 
-  // ---- load: position j of the padded row holds mode l = j (j < N/2) or j - N; input index i = l + n_in/2
+  // ---- load: input i <-> mode l = i - n_in/2 goes to position l mod N of the padded row; the rest is zero.
+  // Four independent loads per thread are in flight before the first store (the pass is latency-bound otherwise).
   const int half_in = P.n_in / 2;
   const double fhi = P.dec_hi ? P.dec_hi[hi] : 1.0;
-  for (int idx = tid; idx < N * tb; idx += kFftThreads) {
+  const int n_pad = N - P.n_in;   // zero positions: [n_in - half_in, N - half_in)
+  for (int idx = tid; idx < n_pad * tb; idx += kFftThreads) {
     int j, col;
     if (P.contig) {
-      col = idx / N;
-      j = idx - col * N;
+      col = idx / n_pad;
+      j = idx - col * n_pad;
     } else {
       j = idx >> tsh;
       col = idx & (tb - 1);
     }
-    const int l = j < N / 2 ? j : j - N;
-    const int i = l + half_in;
-    double2 val = make_double2(0.0, 0.0);
-    if (col < ncol && i >= 0 && i < P.n_in) {
-      const int64_t g = hi * P.in_hi + (lo0 + col) * P.in_lo + (int64_t)i * P.in_el;
-      if (REAL_IN)
-        val.x = static_cast<const double*>(in_raw)[g];
-      else
-        val = static_cast<const double2*>(in_raw)[g];
-      if (P.dec_axis) {
-        const double f = P.dec_axis[i] * fhi * P.dec_lo[lo0 + col];
-        val.x *= f;
-        val.y *= f;
+    a[(P.n_in - half_in + j) * tbp + col] = make_double2(0.0, 0.0);
+  }
+  const int n_ld = P.n_in * tb;
+  for (int idx0 = tid; idx0 < n_ld; idx0 += 4 * kFftThreads) {
+    double2 val[4];
+    int pos[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int idx = idx0 + u * kFftThreads;
+      val[u] = make_double2(0.0, 0.0);
+      pos[u] = -1;
+      if (idx < n_ld) {
+        int i, col;
+        if (P.contig) {
+          col = idx / P.n_in;
+          i = idx - col * P.n_in;
+        } else {
+          i = idx >> tsh;
+          col = idx & (tb - 1);
+        }
+        const int l = i - half_in;
+        pos[u] = (l < 0 ? l + N : l) * tbp + col;
+        if (col < ncol) {
+          const int64_t g = hi * P.in_hi + (lo0 + col) * P.in_lo + (int64_t)i * P.in_el;
+          if (REAL_IN)
+            val[u].x = static_cast<const double*>(in_raw)[g];
+          else
+            val[u] = static_cast<const double2*>(in_raw)[g];
+          if (P.dec_axis) {
+            const double f = P.dec_axis[i] * fhi * P.dec_lo[lo0 + col];
+            val[u].x *= f;
+            val[u].y *= f;
+          }
+        }
       }
     }
-    a[j * tbp + col] = val;
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (pos[u] >= 0) a[pos[u]] = val[u];
   }
   __syncthreads();
 
   // ---- in-place decimation-in-frequency stages
   int L = N;
-  for (int s = 0; s < P.nfac; ++s) {
-    const int r = P.fac[s];
-    const int Ls = L / r;
-    const int tstep = N / L;
-    const int nbf = N / r;
-    for (int idx = tid; idx < (nbf << tsh); idx += kFftThreads) {
-      const int bf = idx >> tsh, col = idx & (tb - 1);
-      const int b = Ls == 1 ? bf : (int)__umulhi((unsigned)bf, P.magic[s]);   // bf / Ls (exact: bf < 2^16)
-      const int j = bf - b * Ls;
-      double2* x = a + (b * L + j) * tbp + col;
-      const int st = Ls * tbp;
-      const int tj = j * tstep;
-      if (r == 4) {
-        const double2 x0 = x[0], x1 = x[st], x2 = x[2 * st], x3 = x[3 * st];
-        const double2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = csub(x1, x3);
-        x[0] = cadd(t0, t2);
-        x[st] = cmul(cadd(t1, mul_mi(t3)), tw[tj]);
-        x[2 * st] = cmul(csub(t0, t2), tw[2 * tj]);
-        x[3 * st] = cmul(cadd(t1, mul_pi(t3)), tw[3 * tj]);
-      } else if (r == 2) {
-        const double2 x0 = x[0], x1 = x[st];
-        x[0] = cadd(x0, x1);
-        x[st] = cmul(csub(x0, x1), tw[tj]);
-      } else if (r == 3) {
-        const double2 x0 = x[0], x1 = x[st], x2 = x[2 * st];
-        const double2 t1 = cadd(x1, x2);
-        const double2 t2 = make_double2(x0.x - 0.5 * t1.x, x0.y - 0.5 * t1.y);
-        const double h = 0.86602540378443864676;
-        const double2 t3 = make_double2(h * (x1.x - x2.x), h * (x1.y - x2.y));
-        x[0] = cadd(x0, t1);
-        x[st] = cmul(cadd(t2, mul_mi(t3)), tw[tj]);
-        x[2 * st] = cmul(cadd(t2, mul_pi(t3)), tw[2 * tj]);
-      } else {  // r == 5
-        const double2 x0 = x[0], x1 = x[st], x2 = x[2 * st], x3 = x[3 * st], x4 = x[4 * st];
-        const double c1 = 0.30901699437494742410, c2 = -0.80901699437494742410;
-        const double s1 = 0.95105651629515357212, s2 = 0.58778525229247312917;
-        const double2 t1 = cadd(x1, x4), t2 = cadd(x2, x3), t3 = csub(x1, x4), t4 = csub(x2, x3);
-        const double2 a1 = make_double2(x0.x + c1 * t1.x + c2 * t2.x, x0.y + c1 * t1.y + c2 * t2.y);
-        const double2 a2 = make_double2(x0.x + c2 * t1.x + c1 * t2.x, x0.y + c2 * t1.y + c1 * t2.y);
-        const double2 b1 = make_double2(s1 * t3.x + s2 * t4.x, s1 * t3.y + s2 * t4.y);
-        const double2 b2 = make_double2(s2 * t3.x - s1 * t4.x, s2 * t3.y - s1 * t4.y);
-        x[0] = make_double2(x0.x + t1.x + t2.x, x0.y + t1.y + t2.y);
-        x[st] = cmul(cadd(a1, mul_mi(b1)), tw[tj]);
-        x[2 * st] = cmul(cadd(a2, mul_mi(b2)), tw[2 * tj]);
-        x[3 * st] = cmul(cadd(a2, mul_pi(b2)), tw[3 * tj]);
-        x[4 * st] = cmul(cadd(a1, mul_pi(b1)), tw[4 * tj]);
-      }
+  for (int s = 0; s < P.npair; ++s) {
+    const int code = P.pair[s];
+    const unsigned mg = P.magic[s];
+#define SFD_FFT_PAIR(R1_, R2_) \
+  case R1_ * 8 + R2_: fused_stages<R1_, R2_>(a, tw, N, L, mg, tb, tbp, tsh, tid, kFftThreads); L /= R1_ * R2_; break;
+    switch (code) {
+      SFD_FFT_PAIR(4, 1) SFD_FFT_PAIR(2, 1) SFD_FFT_PAIR(3, 1) SFD_FFT_PAIR(5, 1)
     }
+#undef SFD_FFT_PAIR
     __syncthreads();
-    L = Ls;
   }
 
   // ---- store the band m in [lo, lo + nout) through the digit-reversal table
@@ -249,29 +338,34 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   P.tb_shift = 0;
   while ((1 << P.tb_shift) < P.tb) ++P.tb_shift;
   {
+    // stage list (fused_stages<R, 1> = one radix-R stage; the pair mechanism is kept for experiments)
     int L = P.N;
-    for (int s = 0; s < P.nfac; ++s) {
-      const int Ls = L / P.fac[s];
-      P.magic[s] = Ls > 1 ? (unsigned)(0x100000000ULL / (unsigned long long)Ls + 1ULL) : 0u;
-      L = Ls;
+    P.npair = 0;
+    for (int s = 0; s < P.nfac;) {
+      const int r1 = P.fac[s];
+      const int r2 = 1;   // fusing two stages in registers was measured: no gain, and it halves the occupancy
+      const int Lq = L / (r1 * r2);
+      P.pair[P.npair] = r1 * 8 + r2;
+      P.magic[P.npair] = Lq > 1 ? (unsigned)(0x100000000ULL / (unsigned long long)Lq + 1ULL) : 0u;
+      ++P.npair;
+      L = Lq;
+      s += r2 > 1 ? 2 : 1;
     }
   }
   const int64_t tiles = P.n_hi * ((P.n_lo + P.tb - 1) / P.tb);
   if (tiles == 0) return SFD_OK;
   SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
   const size_t smem = (size_t)P.N * P.tbp * 16;
-  static bool attr[2] = {false, false};
-  if (!attr[P.real_in]) {
-    if (P.real_in)
-      SFD_CUDA_TRY(cudaFuncSetAttribute(fft_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-    else
-      SFD_CUDA_TRY(cudaFuncSetAttribute(fft_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
-    attr[P.real_in] = true;
-  }
+  const bool two = smem <= (size_t)112 * 1024;   // two CTAs of 512 threads per SM, else one of 1024
+  auto go = [&](auto kern, int threads) -> int {
+    SFD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
+    kern<<<(unsigned)tiles, threads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
+    return SFD_OK;
+  };
   if (P.real_in)
-    fft_pass_kernel<true><<<(unsigned)tiles, kFftThreads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
+    SFD_TRY(two ? go(fft_pass_kernel<true, 512>, 512) : go(fft_pass_kernel<true, 1024>, 1024));
   else
-    fft_pass_kernel<false><<<(unsigned)tiles, kFftThreads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
+    SFD_TRY(two ? go(fft_pass_kernel<false, 512>, 512) : go(fft_pass_kernel<false, 1024>, 1024));
   return launch_check("fft_pass_kernel");
 }
 

@@ -27,7 +27,8 @@ struct FftPass {
   const double *dec_axis, *dec_hi, *dec_lo;
   // filled in by fft_pass():
   int tb, tbp, tb_shift, nfac, fac[16];
-  unsigned magic[16];   // floor(2^32 / Ls) + 1 per stage: bf / Ls = umulhi(bf, magic)
+  int npair, pair[16];  // fused stage pairs: code = R1 * 8 + R2 (R2 = 1: single stage)
+  unsigned magic[16];   // floor(2^32 / Lq) + 1 per pair: g / Lq = umulhi(g, magic)
   const double2* tw;
   const int32_t* rev;
 };

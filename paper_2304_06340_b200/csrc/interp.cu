@@ -70,20 +70,25 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
     const int ox = p.t0[0] + bx * p.bt[0] - W / 2, oy = p.t0[1] + by * p.bt[1] - W / 2, oz = p.t0[2] + bz * p.bt[2] - W / 2;
     const int bx0 = ox - p.lo[0], by0 = oy - p.lo[1], bz0 = oz - p.lo[2];   // subgrid origin in band coordinates
 
-    // stage the subgrid: one (x,y) row of Pz <= 32 cells per warp pass, 16 B per lane, coalesced along z
+    // stage the subgrid with 16-byte asynchronous copies (LDGSTS; zero-filled outside the band): every warp issues
+    // all of its rows back to back and waits once, so the staging runs at L2 bandwidth instead of one round trip per
+    // row.  One (x,y) row of Pz <= 32 cells per warp pass, coalesced along z.
     for (int row = wq; row < Px * Py; row += kWarps) {
       const int ix = row / Py, iy = row - ix * Py;
       const int gx = bx0 + ix, gy = by0 + iy, gz = bz0 + lane;
       if (lane < Pz) {
-        double2 val = make_double2(0.0, 0.0);
-        if (gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nout[0] && gy < p.nout[1] && gz < p.nout[2])
-          val = v[((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz];
-        sub[row * Pz + lane] = val;
+        const bool inside = gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nout[0] && gy < p.nout[1] && gz < p.nout[2];
+        const double2* srcp = inside ? v + (((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz) : v;
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(sub + row * Pz + lane);
+        const int nbytes = inside ? 16 : 0;   // src-size 0: the 16 destination bytes are zero-filled
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(srcp), "r"(nbytes) : "memory");
       }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    TgtRec r = tgt[start + min(wq, count - 1)];
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    TgtRec r = tgt[start + min(wq, count - 1)];
     for (int t = wq; t < count; t += kWarps) {
       const TgtRec cur = r;
       if (t + kWarps < count) r = tgt[start + t + kWarps];   // prefetch the warp's next target
