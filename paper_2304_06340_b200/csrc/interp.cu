@@ -23,7 +23,10 @@ namespace sfd {
 namespace {
 
 constexpr int kWarps = 16;
-constexpr int kSmemCells = 13700;   // complex128 cells of the subgrid: 219,200 B (+ 6 KB of kernel tables)
+constexpr int kMaxTpw = 2;           // targets a warp works on at a time (2 where the accumulators fit the registers)
+constexpr int tpw_for(int W) { return W <= 10 ? 2 : 1; }
+constexpr int kTabBytes = sizeof(double) * kWarps * kMaxTpw * 3 * 16;   // per-warp kernel values: 12 KB
+constexpr int kSmemCells = 13600;   // complex128 cells of the subgrid: 217,600 B
 
 template <int W>
 __global__ void __launch_bounds__(32 * kWarps, 1)
@@ -33,9 +36,10 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
               int32_t* __restrict__ counter, double2* __restrict__ G) {
   constexpr int DEG = W + 3;
   constexpr int NCL = (W * W + 31) / 32;
+  constexpr int TPW = tpw_for(W);
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double (*ktab)[3][16] = reinterpret_cast<double (*)[3][16]>(smem_raw);
-  double2* sub = reinterpret_cast<double2*>(smem_raw + sizeof(double) * kWarps * 3 * 16);
+  double (*ktab)[kMaxTpw][3][16] = reinterpret_cast<double (*)[kMaxTpw][3][16]>(smem_raw);
+  double2* sub = reinterpret_cast<double2*>(smem_raw + kTabBytes);
   __shared__ int s_item;
 
   const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, li = lane & 15;
@@ -85,64 +89,103 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
-    TgtRec r = tgt[start + min(wq, count - 1)];
+    TgtRec r[TPW];
+#pragma unroll
+    for (int u = 0; u < TPW; ++u) r[u] = tgt[start + min(wq + u * kWarps, count - 1)];
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    for (int t = wq; t < count; t += kWarps) {
-      const TgtRec cur = r;
-      if (t + kWarps < count) r = tgt[start + t + kWarps];   // prefetch the warp's next target
+    for (int t = wq; t < count; t += kWarps * TPW) {
+      // TPW targets per warp and iteration: their dependency chains (polynomials, gathers, shuffles) are independent
+      // and interleave, which hides the latencies that 16 warps per SM cannot
+      TgtRec cur[TPW];
+      bool live[TPW];
+#pragma unroll
+      for (int u = 0; u < TPW; ++u) {
+        cur[u] = r[u];
+        live[u] = t + u * kWarps < count;
+        const int nx = t + (TPW + u) * kWarps;
+        if (nx < count) r[u] = tgt[start + nx];   // prefetch the warp's next targets
+      }
       // kernel values: lanes 0-15 do x then z, lanes 16-31 do y
-      int i0x, i0y, i0z;
-      double sx, sy, sz;
-      footprint(cur.u[0], W, i0x, sx);
-      footprint(cur.u[1], W, i0y, sy);
-      footprint(cur.u[2], W, i0z, sz);
-      const double s1 = lane < 16 ? sx : sy;
-      double k1 = pc[DEG], k2 = pc[DEG];
+      int i0x[TPW], i0y[TPW], i0z[TPW];
+      double k1[TPW], k2[TPW], s1[TPW], sz[TPW];
+#pragma unroll
+      for (int u = 0; u < TPW; ++u) {
+        double sx, sy;
+        footprint(cur[u].u[0], W, i0x[u], sx);
+        footprint(cur[u].u[1], W, i0y[u], sy);
+        footprint(cur[u].u[2], W, i0z[u], sz[u]);
+        s1[u] = lane < 16 ? sx : sy;
+        k1[u] = k2[u] = pc[DEG];
+      }
 #pragma unroll
       for (int q = DEG - 1; q >= 0; --q) {
-        k1 = __fma_rn(k1, s1, pc[q]);
-        k2 = __fma_rn(k2, sz, pc[q]);
+#pragma unroll
+        for (int u = 0; u < TPW; ++u) {
+          k1[u] = __fma_rn(k1[u], s1[u], pc[q]);
+          k2[u] = __fma_rn(k2[u], sz[u], pc[q]);
+        }
       }
-      __syncwarp();   // the previous target's reads of ktab are done
+      __syncwarp();   // the previous targets' reads of ktab are done
       if (li < W) {
-        ktab[wq][lane < 16 ? 0 : 1][li] = k1;
-        if (lane < 16) ktab[wq][2][li] = k2;
+#pragma unroll
+        for (int u = 0; u < TPW; ++u) {
+          ktab[wq][u][lane < 16 ? 0 : 1][li] = k1[u];
+          if (lane < 16) ktab[wq][u][2][li] = k2[u];
+        }
       }
       __syncwarp();
 
-      double are[NCL], aim[NCL];
+      double are[TPW][NCL], aim[TPW][NCL];
+      const double2* base[TPW];
 #pragma unroll
-      for (int i = 0; i < NCL; ++i) are[i] = aim[i] = 0.0;
-      const double2* base = sub + ((i0x - ox) * Py + (i0y - oy)) * Pz + (i0z - oz);
+      for (int u = 0; u < TPW; ++u) {
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) are[u][i] = aim[u][i] = 0.0;
+        base[u] = sub + ((i0x[u] - ox) * Py + (i0y[u] - oy)) * Pz + (i0z[u] - oz);
+      }
 #pragma unroll
       for (int a = 0; a < W; ++a) {
-        const double kx = ktab[wq][0][a];
 #pragma unroll
-        for (int i = 0; i < NCL; ++i) {
-          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
-            const double2 c = base[a * plane + off[i]];
-            are[i] = __fma_rn(c.x, kx, are[i]);
-            aim[i] = __fma_rn(c.y, kx, aim[i]);
+        for (int u = 0; u < TPW; ++u) {
+          const double kx = ktab[wq][u][0][a];
+#pragma unroll
+          for (int i = 0; i < NCL; ++i) {
+            if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
+              const double2 c = base[u][a * plane + off[i]];
+              are[u][i] = __fma_rn(c.x, kx, are[u][i]);
+              aim[u][i] = __fma_rn(c.y, kx, aim[u][i]);
+            }
           }
         }
       }
-      double re = 0.0, im = 0.0;
+      double re[TPW], im[TPW];
 #pragma unroll
-      for (int i = 0; i < NCL; ++i) {
-        if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
-          const double kyz = ktab[wq][1][cy[i]] * ktab[wq][2][cz[i]];
-          re = __fma_rn(are[i], kyz, re);
-          im = __fma_rn(aim[i], kyz, im);
+      for (int u = 0; u < TPW; ++u) {
+        re[u] = im[u] = 0.0;
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) {
+          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
+            const double kyz = ktab[wq][u][1][cy[i]] * ktab[wq][u][2][cz[i]];
+            re[u] = __fma_rn(are[u][i], kyz, re[u]);
+            im[u] = __fma_rn(aim[u][i], kyz, im[u]);
+          }
         }
       }
 #pragma unroll
       for (int d = 16; d > 0; d >>= 1) {
-        re += __shfl_xor_sync(0xffffffffu, re, d);
-        im += __shfl_xor_sync(0xffffffffu, im, d);
+#pragma unroll
+        for (int u = 0; u < TPW; ++u) {
+          re[u] += __shfl_xor_sync(0xffffffffu, re[u], d);
+          im[u] += __shfl_xor_sync(0xffffffffu, im[u], d);
+        }
       }
-      if (lane == 0) G[cur.k] = make_double2(re, im);
+      if (lane == 0) {
+#pragma unroll
+        for (int u = 0; u < TPW; ++u)
+          if (live[u]) G[cur[u].k] = make_double2(re[u], im[u]);
+      }
     }
   }
 }
@@ -184,8 +227,7 @@ void interp_bins(int w, int bt[3]) {
 }
 
 size_t interp_smem_bytes(const N3Params& p) {
-  return sizeof(double) * kWarps * 3 * 16 +
-         (size_t)(p.bt[0] + p.w) * (p.bt[1] + p.w) * (p.bt[2] + p.w) * 16;
+  return kTabBytes + (size_t)(p.bt[0] + p.w) * (p.bt[1] + p.w) * (p.bt[2] + p.w) * 16;
 }
 
 int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
