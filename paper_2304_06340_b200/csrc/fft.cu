@@ -15,6 +15,7 @@
 // consecutive rows, so every shared-memory access is a contiguous run (row pitch tb+1: the transposing load of pass
 // A is conflict-free too) -- and the band is written out through the digit-reversal table.  HBM traffic per pass is
 // one read of the input rows and one write of the band: ~16x less than padded library transforms at config 3.
+#include <algorithm>
 #include <map>
 #include <mutex>
 #include <vector>
@@ -80,66 +81,43 @@ __device__ __forceinline__ void bfly<5>(double2 (&x)[5]) {
   x[4] = cadd(a1, mul_pi(b1));
 }
 
-// Two consecutive decimation-in-frequency stages (radices R1 then R2; R2 = 1: a single stage) fused in registers:
-// a thread owns the R1 R2 elements b L + j' + q1 L/R1 + q2 L/(R1 R2) of one row, which stage s (radix R1 over q1, twiddle
-// w_L^{(j' + q2 Lq) p1}) and stage s+1 (radix R2 over q2 inside block (b, p1), twiddle w_{L/R1}^{j' p2}) map onto
-// themselves: one shared-memory round trip instead of two.
-template <int R1, int R2>
-__device__ __forceinline__ void fused_stages(double2* __restrict__ a, const double2* __restrict__ tw, int N, int L,
-                                             unsigned magic, int tb, int tbp, int tsh, int tid, int nthreads) {
-  constexpr int R = R1 * R2;
-  const int Lq = L / R;              // j' range
-  const int L1 = L / R1;             // stride of q1
-  const int tstep = N / L;           // twiddle index step of stage s; stage s+1 uses tstep * R1
-  const int ngroups = N / R;
-  for (int idx = tid; idx < (ngroups << tsh); idx += nthreads) {
-    const int g = idx >> tsh, col = idx & (tb - 1);
-    const int b = Lq == 1 ? g : (int)__umulhi((unsigned)g, magic);   // g / Lq
-    const int jp = g - b * Lq;
-    double2* base = a + (b * L + jp) * tbp + col;
-    double2 v[R1][R2];
+// One decimation-in-frequency stage of radix R.  A thread owns butterfly bf of CG consecutive rows of the tile: the
+// index arithmetic and the R-1 twiddle loads are paid once per thread and amortised over CG butterflies, whose
+// chains are independent (instruction-level parallelism on top of the warps).  Lanes run over (bf, column group) with
+// the group fastest; with the odd row pitch tbp every 8 lanes of an LDS/STS.128 fall into distinct bank groups.
+template <int R, int CG>
+__device__ __forceinline__ void dif_stage(double2* __restrict__ a, const double2* __restrict__ tw, int N, int L,
+                                          unsigned magic, int cgsh, int tbp, int tid, int nthreads) {
+  const int Ls = L / R;
+  const int tstep = N / L;
+  const int nitems = (N / R) << cgsh;
+  const int st = Ls * tbp;
+  for (int idx = tid; idx < nitems; idx += nthreads) {
+    const int bf = idx >> cgsh, cg = idx & ((1 << cgsh) - 1);
+    const int b = Ls == 1 ? bf : (int)__umulhi((unsigned)bf, magic);   // bf / Ls (exact: bf * Ls < 2^32)
+    const int j = bf - b * Ls;
+    double2* base = a + (b * L + j) * tbp + cg * CG;
+    double2 w[R];
 #pragma unroll
-    for (int q1 = 0; q1 < R1; ++q1)
+    for (int p = 1; p < R; ++p) w[p] = tw[p * j * tstep];
 #pragma unroll
-      for (int q2 = 0; q2 < R2; ++q2) v[q1][q2] = base[(q1 * L1 + q2 * Lq) * tbp];
-    // stage s
+    for (int c = 0; c < CG; ++c) {
+      double2 x[R];
 #pragma unroll
-    for (int q2 = 0; q2 < R2; ++q2) {
-      double2 x[R1];
+      for (int q = 0; q < R; ++q) x[q] = base[q * st + c];
+      bfly<R>(x);
+      base[c] = x[0];
 #pragma unroll
-      for (int q1 = 0; q1 < R1; ++q1) x[q1] = v[q1][q2];
-      bfly<R1>(x);
-      const int tj = (jp + q2 * Lq) * tstep;
-      v[0][q2] = x[0];
-#pragma unroll
-      for (int p1 = 1; p1 < R1; ++p1) v[p1][q2] = cmul(x[p1], tw[p1 * tj]);
+      for (int p = 1; p < R; ++p) base[p * st + c] = cmul(x[p], w[p]);
     }
-    // stage s+1
-    if (R2 > 1) {
-      const int tj2 = jp * tstep * R1;
-#pragma unroll
-      for (int p1 = 0; p1 < R1; ++p1) {
-        double2 x[R2];
-#pragma unroll
-        for (int q2 = 0; q2 < R2; ++q2) x[q2] = v[p1][q2];
-        bfly<R2>(x);
-        v[p1][0] = x[0];
-#pragma unroll
-        for (int p2 = 1; p2 < R2; ++p2) v[p1][p2] = cmul(x[p2], tw[p2 * tj2]);
-      }
-    }
-#pragma unroll
-    for (int p1 = 0; p1 < R1; ++p1)
-#pragma unroll
-      for (int p2 = 0; p2 < R2; ++p2) base[(p1 * L1 + p2 * Lq) * tbp] = v[p1][p2];
   }
 }
 
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
 // 1024 with one (long transforms): 32 warps per SM either way -- the stages are latency-bound (shared-memory and
 // twiddle loads feeding short FP64 chains), so occupancy is what buys throughput (profiles/r1c_nufft.md).
-template <bool REAL_IN, int THREADS>
-__global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 1 : 2)
+template <bool REAL_IN, int THREADS, int CG>
+__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
 fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
   constexpr int kFftThreads = THREADS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -213,12 +191,12 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   for (int s = 0; s < P.npair; ++s) {
     const int code = P.pair[s];
     const unsigned mg = P.magic[s];
-#define SFD_FFT_PAIR(R1_, R2_) \
-  case R1_ * 8 + R2_: fused_stages<R1_, R2_>(a, tw, N, L, mg, tb, tbp, tsh, tid, kFftThreads); L /= R1_ * R2_; break;
+#define SFD_FFT_STAGE(R_) \
+  case R_ * 8 + 1: dif_stage<R_, CG>(a, tw, N, L, mg, P.cg_shift, tbp, tid, kFftThreads); L /= R_; break;
     switch (code) {
-      SFD_FFT_PAIR(4, 1) SFD_FFT_PAIR(2, 1) SFD_FFT_PAIR(3, 1) SFD_FFT_PAIR(5, 1)
+      SFD_FFT_STAGE(4) SFD_FFT_STAGE(2) SFD_FFT_STAGE(3) SFD_FFT_STAGE(5)
     }
-#undef SFD_FFT_PAIR
+#undef SFD_FFT_STAGE
     __syncthreads();
   }
 
@@ -297,17 +275,18 @@ size_t fft_tables_bytes(const int n2[3]) {
   return b;
 }
 
-// Rows per tile (a power of two) and row pitch.  Two CTAs per SM whenever at least 4 rows fit in half the shared
-// memory (one CTA's loads and stores overlap the other's butterflies), else one CTA per SM.  Only the transposing
-// load of the contiguous-axis pass needs the odd pitch.
+// Rows per tile (a power of two) and row pitch.  Prefer tiles that let two CTAs share an SM (one CTA's loads and
+// stores overlap the other's butterflies).  The pitch is odd (conflict-free transposing load of the contiguous-axis
+// pass, conflict-free column-group lanes) except for long transforms in the strided passes, where 4 unpadded rows
+// are what still fits twice (their lanes run over consecutive rows: contiguous either way).
 int fft_tile(int N, int contig, int* tbp) {
-  auto pitch = [&](int tb) { return contig ? (tb | 1) : tb; };
-  int pick = 0;
-  for (int tb = 8; tb >= 4 && !pick; tb >>= 1)
-    if ((size_t)N * pitch(tb) * 16 <= (size_t)112 * 1024) pick = tb;
-  for (int tb = 8; tb >= 1 && !pick; tb >>= 1)
-    if ((size_t)N * pitch(tb) * 16 <= (size_t)224 * 1024) pick = tb;
-  if (tbp) *tbp = pick ? pitch(pick) : 0;
+  int pick = 0, pitch = 0;
+  auto fits = [&](int tb, int pt, size_t cap) { return (size_t)N * pt * 16 <= cap; };
+  if (fits(8, 9, (size_t)112 * 1024)) pick = 8, pitch = 9;                       // column groups of 2, 2-4 CTAs per SM
+  if (!pick && fits(4, contig ? 5 : 4, (size_t)112 * 1024)) pick = 4, pitch = contig ? 5 : 4;   // two CTAs per SM
+  for (int tb = 8; tb >= 1 && !pick; tb >>= 1)                                   // one CTA per SM
+    if (fits(tb, contig ? (tb | 1) : tb, (size_t)224 * 1024)) pick = tb, pitch = contig ? (tb | 1) : tb;
+  if (tbp) *tbp = pitch;
   return pick;
 }
 
@@ -356,16 +335,26 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   if (tiles == 0) return SFD_OK;
   SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
   const size_t smem = (size_t)P.N * P.tbp * 16;
-  const bool two = smem <= (size_t)112 * 1024;   // two CTAs of 512 threads per SM, else one of 1024
-  auto go = [&](auto kern, int threads) -> int {
+  // column group CG = 2 rows per thread; threads per CTA sized to the butterflies of a stage (N/5 .. N/2 per row) and
+  // to the CTAs that fit an SM: 32 warps per SM in every case
+  // (measured: the column groups pay off for the short transforms that fit 2-4 CTAs per SM, not for the long ones)
+  const int cg = (P.tb == 8 && smem <= (size_t)112 * 1024) ? 2 : 1;
+  P.cg_shift = 0;
+  while ((cg << P.cg_shift) < P.tb) ++P.cg_shift;
+  const int per_sm = (int)std::min<size_t>(4, (size_t)(226 * 1024) / (smem + 1024));
+  const int threads = per_sm >= 4 ? 256 : (per_sm >= 2 ? 512 : 1024);
+  auto go = [&](auto kern) -> int {
     SFD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
     kern<<<(unsigned)tiles, threads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
     return SFD_OK;
   };
+#define SFD_FFT_GO(REAL_, T_)                                     \
+  (cg == 2 ? go(fft_pass_kernel<REAL_, T_, 2>) : go(fft_pass_kernel<REAL_, T_, 1>))
   if (P.real_in)
-    SFD_TRY(two ? go(fft_pass_kernel<true, 512>, 512) : go(fft_pass_kernel<true, 1024>, 1024));
+    SFD_TRY(threads == 256 ? SFD_FFT_GO(true, 256) : (threads == 512 ? SFD_FFT_GO(true, 512) : SFD_FFT_GO(true, 1024)));
   else
-    SFD_TRY(two ? go(fft_pass_kernel<false, 512>, 512) : go(fft_pass_kernel<false, 1024>, 1024));
+    SFD_TRY(threads == 256 ? SFD_FFT_GO(false, 256) : (threads == 512 ? SFD_FFT_GO(false, 512) : SFD_FFT_GO(false, 1024)));
+#undef SFD_FFT_GO
   return launch_check("fft_pass_kernel");
 }
 

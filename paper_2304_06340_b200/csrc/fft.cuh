@@ -26,7 +26,7 @@ struct FftPass {
   int contig, real_in;
   const double *dec_axis, *dec_hi, *dec_lo;
   // filled in by fft_pass():
-  int tb, tbp, tb_shift, nfac, fac[16];
+  int tb, tbp, tb_shift, cg_shift, nfac, fac[16];   // cg_shift: log2(column groups per tile)
   int npair, pair[16];  // fused stage pairs: code = R1 * 8 + R2 (R2 = 1: single stage)
   unsigned magic[16];   // floor(2^32 / Lq) + 1 per pair: g / Lq = umulhi(g, magic)
   const double2* tw;

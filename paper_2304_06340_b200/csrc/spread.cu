@@ -7,9 +7,12 @@
 //   * one persistent CTA per SM pulls work items (an occupied bin, or a slice of <= kSrcCap sources of a heavy bin)
 //     from a device-side queue; the bin's padded subgrid lives in up to ~200 KB of shared memory in fp64 (real when
 //     the strengths are real, i.e. ball-centred targets; complex otherwise);
-//   * no atomics in shared memory: cell (ix, iy, .) of the subgrid is owned by warp (ix mod W, iy mod NSPLIT) -- an
-//     absolute assignment, the same for every source -- so the W planes of a source go to W different warp groups,
-//     each plane's rows to NSPLIT warps, and no two warps ever touch the same cell;
+//   * no atomics in shared memory: x-plane ix of the subgrid is owned by warp ix mod W -- an absolute assignment, the
+//     same for every source -- so the W planes of a footprint go to the W warps of the CTA and no two warps ever
+//     touch the same cell; inside a warp the 32 lanes cover the W x W cells of the plane;
+//   * per chunk of 32 sources the per-source set-up (owned plane, its address, strength x x-kernel) is computed with
+//     one source per lane and broadcast by shuffles in the sweep, which keeps the sweep at ~10 instructions per
+//     source and 32 cells;
 //   * the z extent of a bin is 16 (real) or 8/16 (complex) cells, which makes the row pitch congruent to W modulo
 //     the number of bank groups: the lanes' cells c = y W + z of a plane fall into distinct banks for every W;
 //   * kernel values are piecewise polynomials (nufft3.cuh footprint()): for a chunk of 32 sources (one per lane) warp
@@ -27,13 +30,6 @@ namespace {
 constexpr int kChunk = 32;               // sources whose 3W kernel values are tabulated at a time (one per lane)
 constexpr int kSmemBytes = 200 * 1024;   // subgrid budget
 
-constexpr int nsplit_for(int W) {
-  int n = (20 + W / 2) / W;
-  if (n < 1) n = 1;
-  if (n > W) n = W;
-  return n;
-}
-
 struct ChunkTables {
   double k[3][kChunk][16];   // kernel values per dimension
   double c[kChunk][2];       // strengths
@@ -41,38 +37,33 @@ struct ChunkTables {
 };
 
 template <int W, bool REAL>
-__global__ void __launch_bounds__(32 * W * nsplit_for(W), 1)
+__global__ void __launch_bounds__(32 * W, 1)
 spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restrict__ src,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
               const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
               int32_t* __restrict__ counter, double* __restrict__ grid) {
-  constexpr int NSPLIT = nsplit_for(W);
-  constexpr int NWARPS = W * NSPLIT;
-  constexpr int RS = (W + NSPLIT - 1) / NSPLIT;     // rows of a footprint plane that one warp can own (at most)
-  constexpr int NCL = (RS * W + 31) / 32;
+  constexpr int NCL = (W * W + 31) / 32;
   constexpr int DEG = W + 3;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ChunkTables& tab = *reinterpret_cast<ChunkTables*>(smem_raw);
   double* sub = reinterpret_cast<double*>(smem_raw + sizeof(ChunkTables));
   __shared__ int s_item;
 
-  const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5;
-  const int a_own = wq % W, slab = wq / W;
+  const int tid = threadIdx.x, lane = tid & 31, a_own = tid >> 5;   // warp a_own owns the x-planes ix = a_own mod W
   const int Px = p.bs[0] + W, Py = p.bs[1] + W, Pz = p.bs[2] + W;
 
   double pc[DEG + 1];
 #pragma unroll
   for (int q = 0; q <= DEG; ++q) pc[q] = ptab[q * kPolyStride + a_own];
 
-  // the lane's cells: c = lane + 32 i -> (m, cz); the warp's m-th row of a footprint is cy = r0 + NSPLIT m, where
-  // r0 = (slab - i0y) mod NSPLIT depends on the source
-  int cm[NCL], cz[NCL], off[NCL];
+  // the lane's cells of a W x W plane: c = lane + 32 i -> (cy, cz)
+  int cy[NCL], cz[NCL], off[NCL];
 #pragma unroll
   for (int i = 0; i < NCL; ++i) {
-    const int c = min(lane + 32 * i, RS * W - 1);
-    cm[i] = NSPLIT * (c / W);
+    const int c = min(lane + 32 * i, W * W - 1);
+    cy[i] = c / W;
     cz[i] = c % W;
-    off[i] = cm[i] * Pz + cz[i];
+    off[i] = cy[i] * Pz + cz[i];
   }
 
   const int total = *n_items;
@@ -88,7 +79,7 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
     const int ox = bx * p.bs[0] - W / 2, oy = by * p.bs[1] - W / 2, oz = bz * p.bs[2] - W / 2;
 
     const int ncell = Px * Py * Pz;
-    for (int i = tid; i < ncell * (REAL ? 1 : 2); i += 32 * NWARPS) sub[i] = 0.0;
+    for (int i = tid; i < ncell * (REAL ? 1 : 2); i += 32 * W) sub[i] = 0.0;
 
     SrcRec rn = src[start + min(lane, count - 1)];
     for (int c0 = 0; c0 < count; c0 += kChunk) {
@@ -96,61 +87,63 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
       const SrcRec r = rn;
       if (c0 + kChunk < count) rn = src[start + min(c0 + kChunk + lane, count - 1)];   // prefetch the next chunk
       __syncthreads();  // zero-fill / previous sweep finished: the tables may be overwritten
-      // warp group a_own evaluates interval a_own for 32 sources at once; slab s takes the dimensions d = s mod NSPLIT
-      if (lane < nch && slab < 3) {
+      // lane = source of the chunk; warp a_own evaluates interval a_own of the three 1-D kernels for 32 sources at once
+      int i0[3];
+      {
+        double sv[3];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-          if (d % NSPLIT == slab) {
-            int i0;
-            double s;
-            footprint(r.u[d], W, i0, s);
-            double kv = pc[DEG];
+        for (int d = 0; d < 3; ++d) footprint(r.u[d], W, i0[d], sv[d]);
+        double k0 = pc[DEG], k1 = pc[DEG], k2 = pc[DEG];
 #pragma unroll
-            for (int q = DEG - 1; q >= 0; --q) kv = __fma_rn(kv, s, pc[q]);
-            tab.k[d][lane][a_own] = kv;
-            if (a_own == 0) tab.i0[lane][d] = i0 - (d == 0 ? ox : (d == 1 ? oy : oz));
-          }
+        for (int q = DEG - 1; q >= 0; --q) {
+          k0 = __fma_rn(k0, sv[0], pc[q]);
+          k1 = __fma_rn(k1, sv[1], pc[q]);
+          k2 = __fma_rn(k2, sv[2], pc[q]);
         }
-        if (wq == 0) {
-          tab.c[lane][0] = r.re;
-          tab.c[lane][1] = r.im;
+        i0[0] -= ox;
+        i0[1] -= oy;
+        i0[2] -= oz;
+        if (lane < nch) {
+          tab.k[0][lane][a_own] = k0;
+          tab.k[1][lane][a_own] = k1;
+          tab.k[2][lane][a_own] = k2;
         }
       }
       __syncthreads();
-      {
-        for (int s = 0; s < nch; ++s) {
-          const int ix0 = tab.i0[s][0], iy0 = tab.i0[s][1];
-          int a = (a_own - ix0) % W;   // the plane of this footprint that this warp group owns
-          if (a < 0) a += W;
-          int r0 = (slab - iy0) % NSPLIT;   // its first row of that plane
-          if (r0 < 0) r0 += NSPLIT;
-          const double kx = tab.k[0][s][a];
-          const double cre = tab.c[s][0] * kx;
-          const double cim = REAL ? 0.0 : tab.c[s][1] * kx;
-          const int base = ((ix0 + a) * Py + iy0 + r0) * Pz + tab.i0[s][2];
+      // per-source quantities of this warp, one source per lane: the plane of the footprint that the warp owns, the
+      // address of that plane's first cell and the strength times the x-kernel; broadcast by shuffles in the sweep
+      int a = (a_own - i0[0]) % W;
+      if (a < 0) a += W;
+      const int base_l = ((i0[0] + a) * Py + i0[1]) * Pz + i0[2];
+      const double kx = lane < nch ? tab.k[0][lane][a] : 0.0;
+      const double cre_l = r.re * kx;
+      const double cim_l = REAL ? 0.0 : r.im * kx;
+      for (int s = 0; s < nch; ++s) {
+        const int base = __shfl_sync(0xffffffffu, base_l, s);
+        const double cre = __shfl_sync(0xffffffffu, cre_l, s);
+        const double cim = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, s);
 #pragma unroll
-          for (int i = 0; i < NCL; ++i) {
-            if (lane + 32 * i < RS * W && r0 + cm[i] < W) {
-              const double kyz = tab.k[1][s][r0 + cm[i]] * tab.k[2][s][cz[i]];
-              const int idx = base + off[i];
-              if (REAL) {
-                sub[idx] = __fma_rn(cre, kyz, sub[idx]);
-              } else {
-                double2 v = reinterpret_cast<double2*>(sub)[idx];
-                v.x = __fma_rn(cre, kyz, v.x);
-                v.y = __fma_rn(cim, kyz, v.y);
-                reinterpret_cast<double2*>(sub)[idx] = v;
-              }
+        for (int i = 0; i < NCL; ++i) {
+          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
+            const double kyz = tab.k[1][s][cy[i]] * tab.k[2][s][cz[i]];
+            const int idx = base + off[i];
+            if (REAL) {
+              sub[idx] = __fma_rn(cre, kyz, sub[idx]);
+            } else {
+              double2 v = reinterpret_cast<double2*>(sub)[idx];
+              v.x = __fma_rn(cre, kyz, v.x);
+              v.y = __fma_rn(cim, kyz, v.y);
+              reinterpret_cast<double2*>(sub)[idx] = v;
             }
           }
-          __syncwarp();
         }
+        __syncwarp();
       }
     }
     __syncthreads();
     // write-back: neighbouring bins overlap in their paddings -> fp64 reductions into the global fine grid.
     // One (x,y) row of Pz <= 32 cells per warp pass, coalesced along z.
-    for (int row = wq; row < Px * Py; row += NWARPS) {
+    for (int row = a_own; row < Px * Py; row += W) {
       const int ix = row / Py, iy = row - ix * Py;
       const int gx = ox + ix, gy = oy + iy, gz = oz + lane;
       if (lane < Pz && gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nf[0] && gy < p.nf[1] && gz < p.nf[2]) {
@@ -177,7 +170,7 @@ int launch(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const i
     SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048));
     attr = true;
   }
-  spread_kernel<W, REAL><<<num_sms(), 32 * W * nsplit_for(W), smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start,
+  spread_kernel<W, REAL><<<num_sms(), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start,
                                                                          d_item_count, d_n_items, d_counter, d_grid);
   return launch_check("spread_kernel");
 }
