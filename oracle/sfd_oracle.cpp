@@ -117,7 +117,29 @@ int64_t subdivide(const double* V, int64_t nV, const int32_t* F, int64_t nF, dou
 // degree-6 members).  Orbit parameters: the solutions of the moment equations, re-derived to
 // 1e-15 by tests/test_oracle_pins.py::test_rule_exactness (never trusted as digits).
 // ---------------------------------------------------------------------------------------------
+void gauss_legendre_unit(int n, long double* x, long double* w);
+
 int rule_table(int rule, double lam[][3], double* om) {
+  if (rule == 64) {
+    // The paper's own rule: "the 8-point Gauss-Legendre rule is applied twice to the right-hand side of
+    // (3.1) as an iterated integral", 64 nodes per triangle (P:173 N_P = 64 N_S).  Reading (R16): the
+    // iterated integral over Q_0^2 = {u1, u2 >= 0, u1 + u2 <= 1} (eq. 2.17) is int_0^1 du1 int_0^{1-u1} du2;
+    // the inner interval is mapped to [0,1] by u2 = (1 - u1) t.  With (a_i, g_i) the 8-point rule on [0,1]:
+    // u = (a_i, (1 - a_i) a_j), q_ij = g_i g_j (1 - a_i); sum q = 1/2 = |Q_0^2| and om = 2 q sums to 1.
+    // L(u) = p0 + u1 (p1 - p0) + u2 (p2 - p0) (eq. 2.18) = barycentric (1 - u1 - u2, u1, u2).  Point i*8+j.
+    long double t[8], g[8];
+    gauss_legendre_unit(8, t, g);
+    for (int i = 0; i < 8; ++i)
+      for (int j = 0; j < 8; ++j) {
+        const long double ai = (t[i] + 1.0L) / 2.0L, aj = (t[j] + 1.0L) / 2.0L;
+        const long double u1 = ai, u2 = (1.0L - ai) * aj;
+        lam[8 * i + j][0] = (double)(1.0L - u1 - u2);
+        lam[8 * i + j][1] = (double)u1;
+        lam[8 * i + j][2] = (double)u2;
+        om[8 * i + j] = (double)(2.0L * (g[i] / 2.0L) * (g[j] / 2.0L) * (1.0L - ai));
+      }
+    return 64;
+  }
   if (rule == 6) {
     const double a[2] = {0.4459484909159648863183293, 0.09157621350977074345957146};
     const double w[2] = {0.2233815896780114656950070, 0.1099517436553218676383263};
@@ -228,7 +250,7 @@ int64_t orc_subdivide(const double* V, int64_t nV, const int32_t* F, int64_t nF,
 
 // Rule table: lam double[q][3] barycentric, om double[q] (sum 1).  Returns q or -1.
 int orc_rule(int rule, double* lam, double* om) {
-  double l[12][3], o[12];
+  double l[64][3], o[64];
   const int q = rule_table(rule, l, o);
   if (q < 0) return -1;
   std::memcpy(lam, l, sizeof(double) * 3 * q);
@@ -241,7 +263,7 @@ int orc_rule(int rule, double* lam, double* om) {
 // x double[nF*q][3], w double[nF*q], index j = f*q + i.
 int orc_nodes(const double* V, int64_t nV, const int32_t* F, int64_t nF, int rule, double* x,
               double* w) {
-  double lam[12][3], om[12];
+  double lam[64][3], om[64];
   const int q = rule_table(rule, lam, om);
   if (q < 0) return -2;
   for (int64_t f = 0; f < nF; ++f) {
@@ -355,10 +377,51 @@ double orc_reduce(const double* nuhat, const double* xi, const double* W, int64_
                          3.14159265358979323846264338327950288L));
 }
 
+// The paper's own frequency quadrature (eqs. 3.3-3.4): the cube D = [-xi_max, xi_max]^3 sampled on the
+// lattice xi_ijk = (i h, j h, k h), h = 2 xi_max / M, i,j,k = -M/2..M/2 (M even), with the three-dimensional
+// trapezoidal rule: weight w_ijk h^3, w = 1 inside, 1/2 on faces, 1/4 on edges, 1/8 at corners.  The paper's
+// transform is e^{-2 pi i xi.x} (eq. 2.1); this code base evaluates e^{-i xi'.x}, so the nodes are returned as
+// xi' = 2 pi xi (R1) while the weights stay in the paper's units (d xi).  Node index
+// k = (a (M+1) + b)(M+1) + c with a,b,c = i + M/2 etc.  xi double[K][3], W double[K], K = (M+1)^3.
+int orc_lattice_nodes(int M, double xi_max, double* xi, double* W) {
+  if (M < 2 || (M & 1) || !(xi_max > 0)) return -2;
+  const double h = 2.0 * xi_max / M;
+  const int n = M + 1;
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b)
+      for (int c = 0; c < n; ++c) {
+        const int64_t k = ((int64_t)a * n + b) * n + c;
+        const int idx[3] = {a - M / 2, b - M / 2, c - M / 2};
+        double wt = h * h * h;
+        for (int d = 0; d < 3; ++d) {
+          xi[3 * k + d] = 2.0 * kPi * (idx[d] * h);
+          if (idx[d] == -M / 2 || idx[d] == M / 2) wt *= 0.5;
+        }
+        W[k] = wt;
+      }
+  return 0;
+}
+
+// General form of the reduction: I = pref * sum_k W_k |nuhat_k - sigmahat(|xi_k|)|^2 (1 + (scale |xi_k|)^2)^{-s}.
+// scale = 1, pref = (2 pi)^-3: orc_reduce.  The paper's norm (eq. 2.7, exponent s_paper < -1/2) on nodes given
+// as xi' = 2 pi xi: scale = 1/(2 pi), s = -s_paper, pref = 1 (weights already in d xi).
+double orc_reduce_ex(const double* nuhat, const double* xi, const double* W, int64_t K, double s, double scale,
+                     double pref) {
+  long double acc = 0;
+  for (int64_t k = 0; k < K; ++k) {
+    const double r2 = xi[3 * k] * xi[3 * k] + xi[3 * k + 1] * xi[3 * k + 1] + xi[3 * k + 2] * xi[3 * k + 2];
+    const double r = std::sqrt(r2);
+    const double dre = nuhat[2 * k] - orc_sigma_hat(r);
+    const double dim = nuhat[2 * k + 1];
+    acc += (long double)(W[k] * (dre * dre + dim * dim) * std::pow(1.0 + (scale * scale) * r2, -s));
+  }
+  return (double)(acc * (long double)pref);
+}
+
 // sqrt(I) for a mesh against the unit sphere; also returns I.
 int orc_weak_distance(const double* V, int64_t nV, const int32_t* F, int64_t nF, int rule, double s,
                       double R, int n_r, int n_th, int n_ph, double* dist, double* I) {
-  double lam[12][3], om[12];
+  double lam[64][3], om[64];
   const int q = rule_table(rule, lam, om);
   if (q < 0) return -2;
   const int64_t J = nF * q, K = (int64_t)n_r * n_th * n_ph;

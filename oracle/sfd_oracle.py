@@ -32,6 +32,9 @@ _lib.orc_sigma_hat.argtypes = [C.c_double]
 _lib.orc_sigma_hat.restype = C.c_double
 _lib.orc_reduce.argtypes = [_dp, _dp, _dp, _i64, C.c_double]
 _lib.orc_reduce.restype = C.c_double
+_lib.orc_lattice_nodes.argtypes = [C.c_int, C.c_double, _dp, _dp]
+_lib.orc_reduce_ex.argtypes = [_dp, _dp, _dp, _i64, C.c_double, C.c_double, C.c_double]
+_lib.orc_reduce_ex.restype = C.c_double
 _lib.orc_weak_distance.argtypes = [_dp, _i64, _ip, _i64, C.c_int, C.c_double, C.c_double, C.c_int,
                                    C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.orc_num_threads.restype = C.c_int
@@ -119,6 +122,23 @@ def reduce(nuhat, xi, W, s):
     xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
     W = np.ascontiguousarray(W, np.float64).reshape(-1)
     return _lib.orc_reduce(nu, xi, W, len(W), float(s))
+
+
+def lattice_nodes(M, xi_max):
+    """The paper's cube lattice: xi' = 2 pi xi_ijk as float64[(M+1)^3, 3], trapezoid weights w_ijk h^3."""
+    K = (M + 1) ** 3
+    xi = np.empty((K, 3), np.float64)
+    W = np.empty(K, np.float64)
+    _chk(_lib.orc_lattice_nodes(M, xi_max, xi, W), "lattice_nodes")
+    return xi, W
+
+
+def reduce_ex(nuhat, xi, W, s, scale, pref):
+    """pref * sum_k W_k |nuhat_k - sigmahat|^2 (1 + (scale |xi_k|)^2)^-s."""
+    nu = np.ascontiguousarray(nuhat, np.complex128).view(np.float64).reshape(-1, 2)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    W = np.ascontiguousarray(W, np.float64).reshape(-1)
+    return _lib.orc_reduce_ex(nu, xi, W, len(W), float(s), float(scale), float(pref))
 
 
 def weak_distance(V, F, q, s, R, n_r, n_th, n_ph):
