@@ -44,7 +44,10 @@ typedef enum {
 
 /* Symmetric triangle quadrature rules ("more symmetric rules are available on triangles");
  * the value is the number of nodes q per face. */
-typedef enum { SFD_RULE_SYM6_DEG4 = 6, SFD_RULE_SYM12_DEG6 = 12 } sfd_rule;
+typedef enum { SFD_RULE_SYM6_DEG4 = 6, SFD_RULE_SYM12_DEG6 = 12,
+               /* the paper's own rule: 8-point Gauss-Legendre applied twice as an iterated integral,
+                * 64 nodes per face, exact for polynomials of total degree <= 14 */
+               SFD_RULE_GL8X8 = 64 } sfd_rule;
 
 /* Ball-shaped frequency quadrature: n_r-point Gauss-Legendre in r on [0,R] x n_theta-point
  * Gauss-Legendre in mu = cos(theta) on [-1,1] x n_phi-point periodic trapezoid in phi.
@@ -131,6 +134,30 @@ int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature*
 int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
                       double s, double R, const sfd_freq_quadrature* q, double eps, void* d_work,
                       size_t work_bytes, sfd_stream stream, double* h_distance, double* h_I);
+
+/* ---- the paper's own variant: cube lattice, trapezoidal rule, its norm convention ----
+ * Lattice of P:156-166 eqs. 3.3-3.4: xi_ijk = (i,j,k) h, h = 2 xi_max / M, i,j,k = -M/2..M/2 (M even, 2..2046), with
+ * trapezoid weights w_ijk h^3 (1 inside, 1/2 faces, 1/4 edges, 1/8 corners).  K = (M+1)^3, node index
+ * ((i+M/2)(M+1) + (j+M/2))(M+1) + (k+M/2).  The paper's transform is e^{-2 pi i xi.x} (eq. 2.1); this library
+ * evaluates e^{-i xi'.x}, so the nodes are written as xi' = 2 pi xi and can be passed to sfd_surface_ft as they are;
+ * the weights stay in the paper's units (d xi). */
+int sfd_lattice_nodes(int32_t M, double xi_max, double* h_xi /*[K][3]*/, double* h_W /*[K]*/);
+int sfd_lattice_nodes_device(int32_t M, double xi_max, double* d_xi /*[K][3]*/, double* d_W /*[K] or NULL*/,
+                             sfd_stream stream);
+/* General form of A6: I = prefactor * sum_k W_k |nuhat_k - sigmahat(|xi_k|)|^2 (1 + (xi_scale |xi_k|)^2)^-s.
+ * sfd_reduce is xi_scale = 1, prefactor = (2 pi)^-3; the paper's norm (eq. 2.7, exponent s_paper < -1/2) on
+ * lattice nodes xi' = 2 pi xi is xi_scale = 1/(2 pi), s = -s_paper, prefactor = 1.  s > 0.5.  Synchronises. */
+int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, double xi_scale,
+                  double prefactor, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+/* ||mu - sigma||_{H_s(R^3)} of P:65 eq. 2.7 for the mesh's surface measure mu against the unit sphere's, by the
+ * paper's quadrature: atoms (rule 64 = the paper's) -> transform on the lattice (eps == 0: direct sum; eps > 0:
+ * type-3 NUFFT, which takes lattice targets like any others) -> trapezoidal rule.  s_paper < -1/2.
+ * Writes the norm to *h_norm and its square to *h_I.  Synchronises. */
+int sfd_weak_distance_lattice_workspace(int64_t nF, int rule, int32_t M, double xi_max, double eps, double x_extent,
+                                        size_t* bytes);
+int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
+                              double s_paper, double xi_max, int32_t M, double eps, void* d_work, size_t work_bytes,
+                              sfd_stream stream, double* h_norm, double* h_I);
 
 /* ---- host-buffer entry points (end-to-end: allocate, copy in, run, copy out, free) -------------
  * Same operations with HOST pointers; device memory comes from the stream-ordered CUDA pool of the

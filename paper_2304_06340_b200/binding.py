@@ -55,6 +55,12 @@ _SIGS = {
     "sfd_weak_distance_workspace": (C.c_int, [_i64, C.c_int, _P(sfd_freq_quadrature), _dbl, _dbl, _dbl, _P(_sz)]),
     "sfd_weak_distance": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl, _vp,
                                     _sz, _vp, _P(_dbl), _P(_dbl)]),
+    "sfd_lattice_nodes": (C.c_int, [C.c_int32, _dbl, _vp, _vp]),
+    "sfd_lattice_nodes_device": (C.c_int, [C.c_int32, _dbl, _vp, _vp, _vp]),
+    "sfd_reduce_ex": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _dbl, _vp, _sz, _vp, _P(_dbl)]),
+    "sfd_weak_distance_lattice_workspace": (C.c_int, [_i64, C.c_int, C.c_int32, _dbl, _dbl, _dbl, _P(_sz)]),
+    "sfd_weak_distance_lattice": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, C.c_int32, _dbl, _vp, _sz, _vp,
+                                            _P(_dbl), _P(_dbl)]),
     "sfd_surface_ft_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp]),
     "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
                                          _P(_dbl), _P(_dbl)]),
@@ -291,3 +297,60 @@ def sfd_probe_fp64(iters=4096):
     tf, ms = _dbl(), _dbl()
     _chk(_lib.sfd_probe_fp64(int(iters), _stream(), C.byref(tf), C.byref(ms)))
     return tf.value, ms.value
+
+
+# ---- the paper's own variant: cube lattice, trapezoidal rule, its norm convention ---------------------------------
+SFD_RULE_GL8X8 = 64
+
+
+def sfd_lattice_nodes(M, xi_max):
+    """Host version of the paper's lattice: numpy xi' = 2 pi xi [K,3], trapezoid weights W[K]."""
+    K = max(int(M) + 1, 1) ** 3
+    xi = np.empty((K, 3), np.float64)
+    W = np.empty(K, np.float64)
+    _chk(_lib.sfd_lattice_nodes(int(M), float(xi_max), xi.ctypes.data_as(_vp), W.ctypes.data_as(_vp)))
+    return xi, W
+
+
+def sfd_lattice_nodes_device(M, xi_max, device="cuda"):
+    K = (int(M) + 1) ** 3
+    xi = torch.empty((K, 3), dtype=torch.float64, device=device)
+    W = torch.empty((K,), dtype=torch.float64, device=device)
+    _chk(_lib.sfd_lattice_nodes_device(int(M), float(xi_max), _ptr(xi), _ptr(W), _stream()))
+    return xi, W
+
+
+def sfd_reduce_ex(nuhat, xi, W, s, xi_scale, prefactor):
+    """prefactor * sum_k W_k |nuhat_k - sigmahat|^2 (1 + (xi_scale |xi_k|)^2)^-s (host float)."""
+    nu = torch.view_as_real(nuhat) if nuhat.is_complex() else nuhat
+    _dev_f64(nu, 2), _dev_f64(xi, 3), _dev_f64(W)
+    K = xi.shape[0]
+    wb = _sz()
+    _chk(_lib.sfd_reduce_workspace(K, C.byref(wb)))
+    work = _work(wb.value, xi.device)
+    I = _dbl()
+    _chk(_lib.sfd_reduce_ex(_ptr(nu), _ptr(xi), _ptr(W), K, float(s), float(xi_scale), float(prefactor), _ptr(work),
+                            work.numel(), _stream(), C.byref(I)))
+    return I.value
+
+
+def sfd_weak_distance_lattice_workspace(nF, rule, M, xi_max, eps, x_extent=1.0):
+    wb = _sz()
+    _chk(_lib.sfd_weak_distance_lattice_workspace(int(nF), int(rule), int(M), float(xi_max), float(eps),
+                                                  float(x_extent), C.byref(wb)))
+    return wb.value
+
+
+def sfd_weak_distance_lattice(V, F, rule, s_paper, xi_max, M, eps=0.0, work=None, x_extent=None):
+    """(||mu - sigma||_{H_s}, its square) in the paper's convention (eq. 2.7, s_paper < -1/2) on its lattice."""
+    _dev_f64(V, 3)
+    assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous()
+    if work is None:
+        if x_extent is None:
+            x_extent = max(_half_widths(V)) if eps > 0 else 1.0
+        work = _work(sfd_weak_distance_lattice_workspace(F.shape[0], rule, M, xi_max, eps, x_extent), V.device)
+    d, I = _dbl(), _dbl()
+    _chk(_lib.sfd_weak_distance_lattice(_ptr(V), V.shape[0], _ptr(F), F.shape[0], int(rule), float(s_paper),
+                                        float(xi_max), int(M), float(eps), _ptr(work), work.numel(), _stream(),
+                                        C.byref(d), C.byref(I)))
+    return d.value, I.value

@@ -274,7 +274,7 @@ struct DistLayout {
 int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps, double x_extent,
                 DistLayout* L) {
   SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
-  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
   SFD_TRY(check_quadrature(q, R));
   SFD_TRY(check_eps(eps));
   L->J = nF * rule;
@@ -354,6 +354,136 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
   if (rc != SFD_OK) return rc;
   if (h_I) *h_I = I;
   if (h_distance) *h_distance = std::sqrt(I);
+  return SFD_OK;
+}
+
+// ---- the paper's own variant: cube lattice + trapezoidal rule + its norm convention (S:8(f) NEXT-1/2) -----------
+int sfd_lattice_nodes(int32_t M, double xi_max, double* h_xi, double* h_W) {
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 2046, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..2046 (got %d)", M);
+  SFD_REQUIRE(xi_max > 0.0 && std::isfinite(xi_max), SFD_ERR_INVALID_ARG, "xi_max must be positive and finite");
+  SFD_REQUIRE(h_xi && h_W, SFD_ERR_NULL, "sfd_lattice_nodes: NULL output");
+  const int n = M + 1;
+  const double two_pi = 6.283185307179586476925286766559;
+  volatile double h = 2.0 * xi_max / M;
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b)
+      for (int c = 0; c < n; ++c) {
+        const int64_t k = ((int64_t)a * n + b) * n + c;
+        const int idx[3] = {a - M / 2, b - M / 2, c - M / 2};
+        volatile double wt = h * h;   // same roundings as lattice_kernel
+        wt = wt * h;
+        for (int d = 0; d < 3; ++d) {
+          volatile double t = (double)idx[d] * h;
+          h_xi[3 * k + d] = two_pi * t;
+          if (idx[d] == -M / 2 || idx[d] == M / 2) wt = wt * 0.5;
+        }
+        h_W[k] = wt;
+      }
+  return SFD_OK;
+}
+int sfd_lattice_nodes_device(int32_t M, double xi_max, double* d_xi, double* d_W, sfd_stream stream) {
+  return lattice_expand(M, xi_max, d_xi, d_W, as_stream(stream));
+}
+
+int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, double xi_scale,
+                  double prefactor, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I) {
+  SFD_REQUIRE(h_I, SFD_ERR_NULL, "sfd_reduce_ex: h_I is NULL");
+  SFD_REQUIRE(xi_scale > 0.0 && std::isfinite(xi_scale) && prefactor > 0.0 && std::isfinite(prefactor),
+              SFD_ERR_INVALID_ARG, "sfd_reduce_ex: xi_scale and prefactor must be positive and finite");
+  cudaStream_t st = as_stream(stream);
+  double* d_res = nullptr;
+  SFD_TRY(reduce_enqueue(d_nuhat, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res, xi_scale, prefactor));
+  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  return SFD_OK;
+}
+
+namespace {
+int lattice_layout(int64_t nF, int rule, int M, double xi_max, double eps, double x_extent, DistLayout* L) {
+  SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
+  SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 2046, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..2046 (got %d)", M);
+  SFD_REQUIRE(xi_max > 0.0 && std::isfinite(xi_max), SFD_ERR_INVALID_ARG, "xi_max must be positive and finite");
+  SFD_TRY(check_eps(eps));
+  L->J = nF * rule;
+  L->K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  const double Sx = 6.283185307179586476925286766559 * xi_max;
+  const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {Sx, Sx, Sx};
+  if (eps > 0.0) SFD_REQUIRE(x_extent > 0.0 && std::isfinite(x_extent), SFD_ERR_INVALID_ARG, "x_extent must be > 0");
+  SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, eps, &L->ft_bytes));
+  L->tab_bytes = 0;
+  L->red_bytes = reduce_workspace(L->K);
+  size_t o = 0;
+  auto put = [&](size_t bytes) {
+    const size_t at = o;
+    o += align_up(bytes);
+    return at;
+  };
+  L->x = put((size_t)L->J * 24);
+  L->w = put((size_t)L->J * 8);
+  L->xi = put((size_t)L->K * 24);
+  L->W = put((size_t)L->K * 8);
+  L->nu = put((size_t)L->K * 16);
+  L->tab = put(256);
+  L->red = put(L->red_bytes);
+  L->ft = put(L->ft_bytes);
+  L->total = o;
+  return SFD_OK;
+}
+}  // namespace
+
+int sfd_weak_distance_lattice_workspace(int64_t nF, int rule, int32_t M, double xi_max, double eps, double x_extent,
+                                        size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_weak_distance_lattice_workspace: bytes is NULL");
+  DistLayout L;
+  SFD_TRY(lattice_layout(nF, rule, M, xi_max, eps, x_extent, &L));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
+                              double s_paper, double xi_max, int32_t M, double eps, void* d_work, size_t work_bytes,
+                              sfd_stream stream, double* h_norm, double* h_I) {
+  SFD_REQUIRE(s_paper < -0.5 && s_paper > -1e6, SFD_ERR_INVALID_ARG,
+              "the paper's Sobolev exponent s must be below -1/2 (P:113), got %g", s_paper);
+  SFD_REQUIRE(nF == 0 || (d_vertices && d_faces), SFD_ERR_NULL, "sfd_weak_distance_lattice: NULL mesh buffer");
+  DistLayout L;
+  SFD_TRY(lattice_layout(nF, rule, M, xi_max, 0.0, 1.0, &L));
+  SFD_TRY(check_eps(eps));
+  SFD_REQUIRE(d_work && work_bytes >= L.ft, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "sfd_weak_distance_lattice needs at least %zu workspace bytes, got %zu", L.total, work_bytes);
+  cudaStream_t st = as_stream(stream);
+  char* base = static_cast<char*>(d_work);
+  double* x = reinterpret_cast<double*>(base + L.x);
+  double* w = reinterpret_cast<double*>(base + L.w);
+  double* xi = reinterpret_cast<double*>(base + L.xi);
+  double* W = reinterpret_cast<double*>(base + L.W);
+  double* nu = reinterpret_cast<double*>(base + L.nu);
+  prof_begin(st);
+  int rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
+  prof_mark("nodes", st);
+  if (rc == SFD_OK) rc = lattice_expand(M, xi_max, xi, W, st);
+  prof_mark("freq_nodes", st);
+  if (rc == SFD_OK) rc = sfd_surface_ft(x, w, L.J, xi, L.K, eps, nu, base + L.ft, work_bytes - L.ft, stream);
+  double* d_res = nullptr;
+  // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
+  if (rc == SFD_OK)
+    rc = reduce_enqueue(nu, xi, W, L.K, -s_paper, base + L.red, L.red_bytes, st, &d_res,
+                        1.0 / 6.283185307179586476925286766559, 1.0);
+  prof_mark("reduce", st);
+  double I = 0.0;
+  if (rc == SFD_OK) {
+    cudaError_t e = cudaMemcpyAsync(&I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+      set_error("sfd_weak_distance_lattice: %s", cudaGetErrorString(e));
+      rc = SFD_ERR_CUDA;
+    }
+  }
+  prof_end(st);
+  if (rc != SFD_OK) return rc;
+  if (h_I) *h_I = I;
+  if (h_norm) *h_norm = std::sqrt(I);
   return SFD_OK;
 }
 

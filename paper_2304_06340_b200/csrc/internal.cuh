@@ -40,8 +40,11 @@ int exclusive_scan_i32(const int32_t* d_in, int32_t* d_out, int64_t n, int32_t* 
 size_t reduce_workspace(int64_t K);
 // Enqueues the reduction; the result (I, already scaled by (2 pi)^-3) lands in d_result[0] (device double,
 // inside the workspace: reduce_result_ptr).
+// General form: I = pref * sum_k W_k |nuhat_k - sigmahat(|xi_k|)|^2 (1 + (scale |xi_k|)^2)^-s; pref < 0 means (2 pi)^-3.
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
-                   size_t work_bytes, cudaStream_t st, double** d_result);
+                   size_t work_bytes, cudaStream_t st, double** d_result, double scale = 1.0, double pref = -1.0);
+// nodes.cu: the paper's cube lattice: xi' = 2 pi xi_ijk, W = w_ijk h^3
+int lattice_expand(int M, double xi_max, double* d_xi, double* d_W, cudaStream_t st);
 
 // ---- probe.cu: measured FP64 FMA peak of the device (the direct sum's roofline denominator) ----------
 int probe_fp64(int iters, cudaStream_t st, double* h_tflops, double* h_ms);

@@ -15,10 +15,12 @@ namespace {
 // equations of degree 4 (6 points) and 6 (12 points); tests/test_binding_cpu.py re-checks exactness through
 // sfd_rule_table.  Point order: DESIGN.md reading R6.
 struct RuleTable {
-  double lam[12][3];
-  double om[12];
+  double lam[64][3];
+  double om[64];
 };
-__constant__ RuleTable c_rule[2];
+__constant__ RuleTable c_rule[3];   // 6-, 12- and 64-point rules
+
+void legendre_rule(int n, std::vector<long double>& t, std::vector<long double>& wt);
 
 void orbit3(double a, double w, double lam[][3], double* om) {
   const double b = 1.0 - 2.0 * a;
@@ -32,7 +34,23 @@ void orbit3(double a, double w, double lam[][3], double* om) {
 void fill_rule(int q, RuleTable& t) {
   for (auto& r : t.lam) r[0] = r[1] = r[2] = 0.0;
   for (auto& o : t.om) o = 0.0;
-  if (q == 6) {
+  if (q == 64) {
+    // The paper's own rule (N_P = 64 N_S): "the 8-point Gauss-Legendre rule is applied twice to the
+    // right-hand side of (3.1) as an iterated integral" (reading R16): int_0^1 du1 int_0^{1-u1} du2, i.e.
+    // u1 = a_i, u2 = (1 - a_i) a_j with a, g the 8-point rule on [0,1]; q_ij = g_i g_j (1 - a_i) sums to 1/2, so the
+    // weights relative to the triangle's area are 2 q_ij.  Point i*8+j; barycentric (1-u1-u2, u1, u2).
+    std::vector<long double> u, g;
+    legendre_rule(8, u, g);
+    for (int i = 0; i < 8; ++i)
+      for (int j = 0; j < 8; ++j) {
+        const long double ai = (1.0L + u[i]) / 2, aj = (1.0L + u[j]) / 2, gi = g[i] / 2, gj = g[j] / 2;
+        const long double u1 = ai, u2 = (1.0L - ai) * aj;
+        t.lam[8 * i + j][0] = (double)(1.0L - u1 - u2);
+        t.lam[8 * i + j][1] = (double)u1;
+        t.lam[8 * i + j][2] = (double)u2;
+        t.om[8 * i + j] = (double)(2.0L * gi * gj * (1.0L - ai));
+      }
+  } else if (q == 6) {
     orbit3(0.445948490915964886318329, 0.223381589678011465695007, t.lam, t.om);
     orbit3(0.091576213509770743459571, 0.109951743655321867638326, t.lam + 3, t.om + 3);
   } else {
@@ -58,7 +76,7 @@ __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V
   if (j >= nF * Q) return;
   const int64_t f = j / Q;
   const int i = (int)(j - f * Q);
-  const RuleTable& R = c_rule[Q == 6 ? 0 : 1];
+  const RuleTable& R = c_rule[Q == 6 ? 0 : (Q == 12 ? 1 : 2)];
   const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
   const double nan = __longlong_as_double(0x7ff8000000000000LL);
   if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
@@ -87,8 +105,11 @@ __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V
   w[j] = __dmul_rn(R.om[i], area);
 }
 
+}  // namespace
+
 // Gauss-Legendre nodes/weights on [-1,1], ascending, by Newton iteration on P_n evaluated with the
 // Bonnet recurrence in long double; the derivative comes from (1-t^2) P_n' = n (P_{n-1} - t P_n).
+namespace {
 void legendre_rule(int n, std::vector<long double>& t, std::vector<long double>& wt) {
   const long double pi = 3.141592653589793238462643383279502884L;
   t.assign(n, 0.0L);
@@ -154,6 +175,38 @@ __global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restri
 }  // namespace
 
 void gauss_legendre_host(int n, std::vector<long double>& t, std::vector<long double>& wt) { legendre_rule(n, t, wt); }
+
+namespace {
+// The paper's frequency quadrature (eqs. 3.3-3.4): lattice xi_ijk = (i,j,k) h, h = 2 xi_max / M,
+// i,j,k = -M/2..M/2, trapezoid weights w_ijk h^3 (1, 1/2, 1/4, 1/8).  Nodes are written as xi' = 2 pi xi (reading R1).
+__global__ void __launch_bounds__(256) lattice_kernel(int M, double h, double* __restrict__ xi, double* __restrict__ W) {
+  const int n = M + 1;
+  const int64_t K = (int64_t)n * n * n;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= K) return;
+  const int c = (int)(k % n);
+  const int64_t ab = k / n;
+  const int b = (int)(ab % n), a = (int)(ab / n);
+  const int idx[3] = {a - M / 2, b - M / 2, c - M / 2};
+  const double two_pi = 6.283185307179586476925286766559;
+  double wt = __dmul_rn(__dmul_rn(h, h), h);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    xi[3 * k + d] = __dmul_rn(two_pi, __dmul_rn((double)idx[d], h));
+    if (idx[d] == -M / 2 || idx[d] == M / 2) wt = __dmul_rn(wt, 0.5);
+  }
+  if (W) W[k] = wt;
+}
+}  // namespace
+
+int lattice_expand(int M, double xi_max, double* d_xi, double* d_W, cudaStream_t st) {
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 2046, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..2046 (got %d)", M);
+  SFD_REQUIRE(xi_max > 0.0 && std::isfinite(xi_max), SFD_ERR_INVALID_ARG, "xi_max must be positive and finite");
+  SFD_REQUIRE(d_xi, SFD_ERR_NULL, "lattice nodes: NULL output");
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  lattice_kernel<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(M, 2.0 * xi_max / M, d_xi, d_W);
+  return launch_check("lattice_kernel");
+}
 
 int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t) {
   SFD_REQUIRE(q, SFD_ERR_NULL, "freq quadrature is NULL");
@@ -232,7 +285,7 @@ int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi,
 }
 
 int rule_table_host(int rule, double* lam, double* om) {
-  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
   RuleTable t;
   fill_rule(rule, t);
   for (int i = 0; i < rule; ++i) {
@@ -244,7 +297,7 @@ int rule_table_host(int rule, double* lam, double* om) {
 
 int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rule, double* d_x, double* d_w,
           cudaStream_t st) {
-  SFD_REQUIRE(rule == 6 || rule == 12, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6 or 12)", rule);
+  SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
   SFD_REQUIRE(nF >= 0 && nV >= 0, SFD_ERR_INVALID_ARG, "negative mesh size");
   if (nF == 0) return SFD_OK;
   SFD_REQUIRE(d_V && d_F && d_x && d_w, SFD_ERR_NULL, "sfd_nodes: NULL buffer");
@@ -252,9 +305,10 @@ int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rul
   int dev = 0;
   SFD_CUDA_TRY(cudaGetDevice(&dev));
   if (uploaded_dev != dev) {
-    RuleTable t[2];
+    static RuleTable t[3];
     fill_rule(6, t[0]);
     fill_rule(12, t[1]);
+    fill_rule(64, t[2]);
     SFD_CUDA_TRY(cudaMemcpyToSymbol(c_rule, t, sizeof(t)));
     uploaded_dev = dev;
   }
@@ -262,6 +316,8 @@ int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rul
   const unsigned blocks = (unsigned)((J + 255) / 256);
   if (rule == 6)
     nodes_kernel<6><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+  else if (rule == 64)
+    nodes_kernel<64><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
   else
     nodes_kernel<12><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
   return launch_check("nodes_kernel");

@@ -100,7 +100,7 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
 int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->ns_bins = (int64_t)p.nbs[0] * p.nbs[1] * p.nbs[2];
   L->nt_bins = (int64_t)p.nbt[0] * p.nbt[1] * p.nbt[2];
-  L->ns_items = L->ns_bins + J / kSrcCap + 1;
+  L->ns_items = L->ns_bins + J / kSrcCap + 1;   // upper bound for any cap >= kSrcCap
   L->nt_items = L->nt_bins + K / kTgtCap + 1;
   SFD_REQUIRE(L->ns_bins < 0x7fffffffLL && L->nt_bins < 0x7fffffffLL && J < 0x7fffffffLL && K < 0x7fffffffLL,
               SFD_ERR_UNSUPPORTED, "type-3 NUFFT: problem too large for 32-bit bin bookkeeping");
@@ -344,7 +344,11 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
   SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_bins, nullptr, scan_w, scan_b, st));
   SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
-  SFD_TRY(make_items(shist, soff, L.ns_bins, kSrcCap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
+  // items of <= cap sources: 1024 normally; when the sources crowd into few bins (the paper's lattice variant maps
+  // 2e7 atoms onto ~60^3 cells, "highly clustered") larger slices keep the number of subgrid write-backs --
+  // global fp64 reductions onto the same few cells -- proportional to the SM count instead of to J
+  const int src_cap = (int)std::max<int64_t>(kSrcCap, J / ((int64_t)num_sms() * 8));
+  SFD_TRY(make_items(shist, soff, L.ns_bins, src_cap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
   prof_mark("src_sort", st);
 
   // A5-4: spread

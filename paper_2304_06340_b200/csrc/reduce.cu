@@ -74,7 +74,7 @@ __device__ __forceinline__ double sobolev_weight(double q, double s, int s_kind)
 
 __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* __restrict__ nuhat, const double* __restrict__ xi,
                                                                const double* __restrict__ W, int64_t K, double s, int s_kind,
-                                                               Comp* __restrict__ partial) {
+                                                               double scale2, Comp* __restrict__ partial) {
   Comp acc{0.0, 0.0};
   const int64_t stride = (int64_t)gridDim.x * kThreads;
   for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += stride) {
@@ -83,20 +83,20 @@ __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* _
     const double r2 = a * a + b * b + c * c;
     const double r = sqrt(r2);
     const double dre = nu.x - sigma_hat(r);
-    const double term = W[k] * (dre * dre + nu.y * nu.y) * sobolev_weight(1.0 + r2, s, s_kind);
+    const double term = W[k] * (dre * dre + nu.y * nu.y) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
     two_sum_add(acc, term);
   }
   const Comp tot = block_reduce(acc);
   if (threadIdx.x == 0) partial[blockIdx.x] = tot;
 }
 
-__global__ void __launch_bounds__(kThreads) reduce_final_kernel(const Comp* __restrict__ partial, int n, double* __restrict__ result) {
+__global__ void __launch_bounds__(kThreads) reduce_final_kernel(const Comp* __restrict__ partial, int n, double pref,
+                                                               double* __restrict__ result) {
   Comp acc{0.0, 0.0};
   for (int i = threadIdx.x; i < n; i += kThreads) comp_merge(acc, partial[i]);
   const Comp tot = block_reduce(acc);
   if (threadIdx.x == 0) {
-    const double two_pi = 6.283185307179586;
-    result[0] = (tot.s + tot.c) / (two_pi * two_pi * two_pi);
+    result[0] = (tot.s + tot.c) * pref;
   }
 }
 
@@ -113,7 +113,8 @@ size_t reduce_workspace(int64_t K) {
 }
 
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
-                   size_t work_bytes, cudaStream_t st, double** d_result) {
+                   size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref) {
+  if (pref < 0.0) pref = 1.0 / (6.283185307179586 * 6.283185307179586 * 6.283185307179586);   // (2 pi)^-3
   SFD_REQUIRE(K >= 0, SFD_ERR_INVALID_ARG, "K must be >= 0");
   SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
   SFD_REQUIRE(d_work && work_bytes >= reduce_workspace(K), SFD_ERR_WORKSPACE_TOO_SMALL,
@@ -129,9 +130,9 @@ int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W,
   const int blocks = reduce_blocks(K);
   const int s_kind = s == 1.0 ? 1 : (s == 2.0 ? 2 : 0);
   reduce_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(d_nuhat), d_xi, d_W, K, s, s_kind,
-                                                   partial);
+                                                   scale * scale, partial);
   SFD_TRY(launch_check("reduce_terms_kernel"));
-  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, result);
+  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);
   return launch_check("reduce_final_kernel");
 }
 
