@@ -113,11 +113,66 @@ __device__ __forceinline__ void dif_stage(double2* __restrict__ a, const double2
   }
 }
 
+// Two consecutive decimation-in-frequency stages (radices R1 then R2; R2 = 1: a single stage) fused in registers:
+// a thread owns the R1 R2 elements b L + j' + q1 L/R1 + q2 L/(R1 R2) of one row, which stage s (radix R1 over q1, twiddle
+// w_L^{(j' + q2 Lq) p1}) and stage s+1 (radix R2 over q2 inside block (b, p1), twiddle w_{L/R1}^{j' p2}) map onto
+// themselves: one shared-memory round trip instead of two.
+template <int R1, int R2>
+__device__ __forceinline__ void fused_stages(double2* __restrict__ a, const double2* __restrict__ tw, int N, int L,
+                                             unsigned magic, int tb, int tbp, int tsh, int tid, int nthreads) {
+  constexpr int R = R1 * R2;
+  const int Lq = L / R;              // j' range
+  const int L1 = L / R1;             // stride of q1
+  const int tstep = N / L;           // twiddle index step of stage s; stage s+1 uses tstep * R1
+  const int ngroups = N / R;
+  for (int idx = tid; idx < (ngroups << tsh); idx += nthreads) {
+    const int g = idx >> tsh, col = idx & (tb - 1);
+    const int b = Lq == 1 ? g : (int)__umulhi((unsigned)g, magic);   // g / Lq
+    const int jp = g - b * Lq;
+    double2* base = a + (b * L + jp) * tbp + col;
+    double2 v[R1][R2];
+#pragma unroll
+    for (int q1 = 0; q1 < R1; ++q1)
+#pragma unroll
+      for (int q2 = 0; q2 < R2; ++q2) v[q1][q2] = base[(q1 * L1 + q2 * Lq) * tbp];
+    // stage s
+#pragma unroll
+    for (int q2 = 0; q2 < R2; ++q2) {
+      double2 x[R1];
+#pragma unroll
+      for (int q1 = 0; q1 < R1; ++q1) x[q1] = v[q1][q2];
+      bfly<R1>(x);
+      const int tj = (jp + q2 * Lq) * tstep;
+      v[0][q2] = x[0];
+#pragma unroll
+      for (int p1 = 1; p1 < R1; ++p1) v[p1][q2] = cmul(x[p1], tw[p1 * tj]);
+    }
+    // stage s+1
+    if (R2 > 1) {
+      const int tj2 = jp * tstep * R1;
+#pragma unroll
+      for (int p1 = 0; p1 < R1; ++p1) {
+        double2 x[R2];
+#pragma unroll
+        for (int q2 = 0; q2 < R2; ++q2) x[q2] = v[p1][q2];
+        bfly<R2>(x);
+        v[p1][0] = x[0];
+#pragma unroll
+        for (int p2 = 1; p2 < R2; ++p2) v[p1][p2] = cmul(x[p2], tw[p2 * tj2]);
+      }
+    }
+#pragma unroll
+    for (int p1 = 0; p1 < R1; ++p1)
+#pragma unroll
+      for (int p2 = 0; p2 < R2; ++p2) base[(p1 * L1 + p2 * Lq) * tbp] = v[p1][p2];
+  }
+}
+
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
 // 1024 with one (long transforms): 32 warps per SM either way -- the stages are latency-bound (shared-memory and
 // twiddle loads feeding short FP64 chains), so occupancy is what buys throughput (profiles/r1c_nufft.md).
-template <bool REAL_IN, int THREADS, int CG>
-__global__ void __launch_bounds__(THREADS, 1024 / THREADS)
+template <bool REAL_IN, int THREADS, int CG, bool FUSED>
+__global__ void __launch_bounds__(THREADS, (FUSED ? 512 : 1024) / THREADS)
 fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
   constexpr int kFftThreads = THREADS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -193,9 +248,19 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
     const unsigned mg = P.magic[s];
 #define SFD_FFT_STAGE(R_) \
   case R_ * 8 + 1: dif_stage<R_, CG>(a, tw, N, L, mg, P.cg_shift, tbp, tid, kFftThreads); L /= R_; break;
-    switch (code) {
-      SFD_FFT_STAGE(4) SFD_FFT_STAGE(2) SFD_FFT_STAGE(3) SFD_FFT_STAGE(5)
+#define SFD_FFT_PAIR(R1_, R2_) \
+  case R1_ * 8 + R2_: fused_stages<R1_, R2_>(a, tw, N, L, mg, tb, tbp, tsh, tid, kFftThreads); L /= R1_ * R2_; break;
+    if (FUSED) {
+      switch (code) {
+        SFD_FFT_PAIR(4, 4) SFD_FFT_PAIR(4, 2) SFD_FFT_PAIR(4, 3) SFD_FFT_PAIR(2, 3) SFD_FFT_PAIR(2, 5) SFD_FFT_PAIR(3, 3)
+        SFD_FFT_PAIR(3, 5) SFD_FFT_PAIR(2, 2) SFD_FFT_PAIR(4, 1) SFD_FFT_PAIR(2, 1) SFD_FFT_PAIR(3, 1) SFD_FFT_PAIR(5, 1)
+      }
+    } else {
+      switch (code) {
+        SFD_FFT_STAGE(4) SFD_FFT_STAGE(2) SFD_FFT_STAGE(3) SFD_FFT_STAGE(5)
+      }
     }
+#undef SFD_FFT_PAIR
 #undef SFD_FFT_STAGE
     __syncthreads();
   }
@@ -222,7 +287,9 @@ struct HostTables {
   std::vector<double> tw;     // N complex: exp(-2 pi i t / N)
   std::vector<int32_t> rev;   // position of output frequency k after the DIF stages
   int nfac;
-  int fac[16];
+  int fac[16];      // single radices in execution order
+  int npair;
+  int pair[16];     // the same sequence grouped into fused pairs: code R1 * 8 + R2 (R2 = 1: single)
 };
 std::mutex g_mu;
 std::map<int, HostTables> g_tables;
@@ -232,12 +299,32 @@ const HostTables& tables_for(int N) {
   auto it = g_tables.find(N);
   if (it != g_tables.end()) return it->second;
   HostTables t;
-  t.nfac = 0;
+  // radices 4s, 2, 3s, 5s, then ordered so that consecutive stages pair up into register-resident radix-(R1 R2)
+  // butterflies with R1 R2 <= 16: take the first remaining factor and the largest other one that fits
+  // (2700 -> (4,3)(3,5)(3,5); 1440 -> (4,4)(2,5)(3,3); 720 -> (4,4)(3,5)(3); 360 -> (4,3)(2,5)(3))
+  std::vector<int> rest;
   int n = N;
-  while (n % 4 == 0) { t.fac[t.nfac++] = 4; n /= 4; }
-  while (n % 2 == 0) { t.fac[t.nfac++] = 2; n /= 2; }
-  while (n % 3 == 0) { t.fac[t.nfac++] = 3; n /= 3; }
-  while (n % 5 == 0) { t.fac[t.nfac++] = 5; n /= 5; }
+  while (n % 4 == 0) { rest.push_back(4); n /= 4; }
+  while (n % 2 == 0) { rest.push_back(2); n /= 2; }
+  while (n % 3 == 0) { rest.push_back(3); n /= 3; }
+  while (n % 5 == 0) { rest.push_back(5); n /= 5; }
+  t.nfac = 0;
+  t.npair = 0;
+  while (!rest.empty()) {
+    const int r1 = rest.front();
+    rest.erase(rest.begin());
+    int best = -1;
+    for (size_t i = 0; i < rest.size(); ++i)
+      if (r1 * rest[i] <= 16 && (best < 0 || rest[i] > rest[best])) best = (int)i;
+    int r2 = 1;
+    if (best >= 0) {
+      r2 = rest[best];
+      rest.erase(rest.begin() + best);
+    }
+    t.fac[t.nfac++] = r1;
+    if (r2 > 1) t.fac[t.nfac++] = r2;
+    t.pair[t.npair++] = r1 * 8 + r2;
+  }
   t.tw.resize(2 * (size_t)N);
   const long double two_pi = 6.283185307179586476925286766559005768L;
   for (int k = 0; k < N; ++k) {
@@ -304,6 +391,8 @@ int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStrea
     o += align_up((size_t)n2[d] * 4);
     out->nfac[d] = t.nfac;
     for (int s = 0; s < t.nfac; ++s) out->fac[d][s] = t.fac[s];
+    out->npair[d] = t.npair;
+    for (int s = 0; s < t.npair; ++s) out->pair[d][s] = t.pair[s];
   }
   return SFD_OK;
 }
@@ -316,20 +405,24 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   P.tb = fft_tile(P.N, P.contig, &P.tbp);
   P.tb_shift = 0;
   while ((1 << P.tb_shift) < P.tb) ++P.tb_shift;
+  // Long transforms (one CTA per SM either way) run two stages per shared-memory round trip in registers (128
+  // registers, 16 warps): measured 13-19 % faster at N = 1440 / 2700; the short ones are faster with single stages
+  // at 32 warps and column groups (profiles/r1c_after_rewrites.md).
+  const bool fused = (size_t)P.N * 9 * 16 > (size_t)112 * 1024;
   {
-    // stage list (fused_stages<R, 1> = one radix-R stage; the pair mechanism is kept for experiments)
     int L = P.N;
     P.npair = 0;
-    for (int s = 0; s < P.nfac;) {
-      const int r1 = P.fac[s];
-      const int r2 = 1;   // fusing two stages in registers was measured: no gain, and it halves the occupancy
+    auto push = [&](int r1, int r2) {
       const int Lq = L / (r1 * r2);
       P.pair[P.npair] = r1 * 8 + r2;
       P.magic[P.npair] = Lq > 1 ? (unsigned)(0x100000000ULL / (unsigned long long)Lq + 1ULL) : 0u;
       ++P.npair;
       L = Lq;
-      s += r2 > 1 ? 2 : 1;
-    }
+    };
+    if (fused)
+      for (int s = 0; s < T.npair[axis]; ++s) push(T.pair[axis][s] / 8, T.pair[axis][s] % 8);
+    else
+      for (int s = 0; s < P.nfac; ++s) push(P.fac[s], 1);
   }
   const int64_t tiles = P.n_hi * ((P.n_lo + P.tb - 1) / P.tb);
   if (tiles == 0) return SFD_OK;
@@ -338,19 +431,25 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   // column group CG = 2 rows per thread; threads per CTA sized to the butterflies of a stage (N/5 .. N/2 per row) and
   // to the CTAs that fit an SM: 32 warps per SM in every case
   // (measured: the column groups pay off for the short transforms that fit 2-4 CTAs per SM, not for the long ones)
-  const int cg = (P.tb == 8 && smem <= (size_t)112 * 1024) ? 2 : 1;
+  const int cg = (!fused && P.tb == 8 && smem <= (size_t)112 * 1024) ? 2 : 1;
   P.cg_shift = 0;
   while ((cg << P.cg_shift) < P.tb) ++P.cg_shift;
   const int per_sm = (int)std::min<size_t>(4, (size_t)(226 * 1024) / (smem + 1024));
-  const int threads = per_sm >= 4 ? 256 : (per_sm >= 2 ? 512 : 1024);
+  int threads = per_sm >= 4 ? 256 : (per_sm >= 2 ? 512 : 1024);
+  if (fused) threads = per_sm >= 2 ? 256 : 512;   // 128 registers per thread: 16 warps per SM
   auto go = [&](auto kern) -> int {
     SFD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024));
     kern<<<(unsigned)tiles, threads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
     return SFD_OK;
   };
 #define SFD_FFT_GO(REAL_, T_)                                     \
-  (cg == 2 ? go(fft_pass_kernel<REAL_, T_, 2>) : go(fft_pass_kernel<REAL_, T_, 1>))
-  if (P.real_in)
+  (cg == 2 ? go(fft_pass_kernel<REAL_, T_, 2, false>) : go(fft_pass_kernel<REAL_, T_, 1, false>))
+  if (fused) {
+    if (P.real_in)
+      SFD_TRY(threads == 256 ? go(fft_pass_kernel<true, 256, 1, true>) : go(fft_pass_kernel<true, 512, 1, true>));
+    else
+      SFD_TRY(threads == 256 ? go(fft_pass_kernel<false, 256, 1, true>) : go(fft_pass_kernel<false, 512, 1, true>));
+  } else if (P.real_in)
     SFD_TRY(threads == 256 ? SFD_FFT_GO(true, 256) : (threads == 512 ? SFD_FFT_GO(true, 512) : SFD_FFT_GO(true, 1024)));
   else
     SFD_TRY(threads == 256 ? SFD_FFT_GO(false, 256) : (threads == 512 ? SFD_FFT_GO(false, 512) : SFD_FFT_GO(false, 1024)));

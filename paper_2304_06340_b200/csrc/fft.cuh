@@ -10,6 +10,8 @@ struct FftTables {
   const int32_t* rev[3];
   int nfac[3];
   int fac[3][16];
+  int npair[3];
+  int pair[3][16];   // fused stage pairs, code R1 * 8 + R2
 };
 
 // One pass of 1-D transforms of length N over a 2-level set of rows ("columns" c = (hi, lo)).
