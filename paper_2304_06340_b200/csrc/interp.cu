@@ -77,10 +77,17 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
     // stage the subgrid with 16-byte asynchronous copies (LDGSTS; zero-filled outside the band): every warp issues
     // all of its rows back to back and waits once, so the staging runs at L2 bandwidth instead of one round trip per
     // row.  One (x,y) row of Pz <= 32 cells per warp pass, coalesced along z.
+    const int cx2 = p.n2[0], cy2 = p.n2[1], czc = p.n2[2] / 2;   // reflection m -> n2 - m about the centre n2/2
     for (int row = wq; row < Px * Py; row += kWarps) {
       const int ix = row / Py, iy = row - ix * Py;
-      const int gx = bx0 + ix, gy = by0 + iy, gz = bz0 + lane;
       if (lane < Pz) {
+        int mx = ox + ix, my = oy + iy, mz = oz + lane;          // absolute inner-grid indices of the cell
+        if (p.zh && mz < czc) {                                   // lower half: the conjugate of the mirror cell (sign applied in the gather)
+          mx = cx2 - mx;
+          my = cy2 - my;
+          mz = 2 * czc - mz;
+        }
+        const int gx = mx - p.lo[0], gy = my - p.lo[1], gz = mz - p.lo[2];
         const bool inside = gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nout[0] && gy < p.nout[1] && gz < p.nout[2];
         const double2* srcp = inside ? v + (((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz) : v;
         const unsigned dst = (unsigned)__cvta_generic_to_shared(sub + row * Pz + lane);
@@ -169,7 +176,8 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
           if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
             const double kyz = ktab[wq][u][1][cy[i]] * ktab[wq][u][2][cz[i]];
             re[u] = __fma_rn(are[u][i], kyz, re[u]);
-            im[u] = __fma_rn(aim[u][i], kyz, im[u]);
+            // cells below the centre plane hold the mirror cell un-conjugated: flip the sign of their imaginary part
+            im[u] = __fma_rn(aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
           }
         }
       }

@@ -91,8 +91,17 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
     p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
     p->nbt[d] = (p->n2[d] / 2) / p->bt[d] + 1;
     // cells any footprint can touch: ceil(n2/4 - w/2) ... ceil(3 n2/4 - w/2) + w - 1, plus one cell of slack
+    // (+1 for odd w: the band is then symmetric about n2/2, which the Hermitian reflection needs)
     p->lo[d] = std::max(0, p->n2[d] / 4 - (p->w + 1) / 2 - 1);
-    p->nout[d] = std::min(p->n2[d] - p->lo[d], p->n2[d] / 2 + p->w + 3);
+    p->nout[d] = std::min(p->n2[d] - p->lo[d], p->n2[d] / 2 + p->w + 3 + (p->w & 1));
+  }
+  // real strengths: keep only the upper half of the band along z (the last FFT-pass axis to be produced first)
+  p->zh = 0;
+  if (real_c && p->lo[2] > 0 && p->lo[0] > 0 && p->lo[1] > 0) {
+    const int c2 = p->n2[2] / 2, hi2 = p->lo[2] + p->nout[2] - 1;
+    p->zh = 1;
+    p->lo[2] = c2;
+    p->nout[2] = hi2 - c2 + 1;
   }
   return SFD_OK;
 }

@@ -25,6 +25,9 @@ struct N3Params {
                              // inner grid that holds every target; bt[2] is 8 or 16 (bank-conflict-free pitch)
   int deg;                   // degree of the piecewise-polynomial kernel evaluation (w + 3)
   int lo[3], nout[3];        // band of the inner grid that is computed and stored: v[m - lo], m in [lo, lo + nout)
+  int zh;                    // 1: real strengths => v is Hermitian about the centre m = n2/2 (v[c+k] = conj v[c-k]) and
+                             // only the half m_2 >= n2_2/2 of the band is computed and stored (lo[2] = n2_2/2); the
+                             // interpolation reads the other half by reflection (all three indices) and conjugation
 };
 
 constexpr int kMaxDeg = kMaxW + 3;
