@@ -178,10 +178,15 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double2* a = reinterpret_cast<double2*>(smem_raw);
   const int N = P.N, tb = P.tb, tbp = P.tbp, tid = threadIdx.x;
-  const int64_t tiles_per_hi = (P.n_lo + tb - 1) / tb;
+  // PACK (real input only): a column of the tile carries two real rows, 2c as the real and 2c+1 as the imaginary
+  // part; their transforms are separated at the store, A[m] = (Z[m] + conj Z[-m])/2, B[m] = (Z[m] - conj Z[-m])/(2i)
+  constexpr int PACK = REAL_IN ? 2 : 1;
+  const int64_t rows_per_tile = (int64_t)tb * PACK;
+  const int64_t tiles_per_hi = (P.n_lo + rows_per_tile - 1) / rows_per_tile;
   const int64_t hi = blockIdx.x / tiles_per_hi;
-  const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * tb;
-  const int ncol = (int)min((int64_t)tb, P.n_lo - lo0);
+  const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * rows_per_tile;
+  const int nrow = (int)min(rows_per_tile, P.n_lo - lo0);   // rows of this tile
+  const int ncol = (nrow + PACK - 1) / PACK;
   const int tsh = P.tb_shift;
   const double2* __restrict__ tw = P.tw;
 
@@ -222,15 +227,21 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         const int l = i - half_in;
         pos[u] = (l < 0 ? l + N : l) * tbp + col;
         if (col < ncol) {
-          const int64_t g = hi * P.in_hi + (lo0 + col) * P.in_lo + (int64_t)i * P.in_el;
-          if (REAL_IN)
-            val[u].x = static_cast<const double*>(in_raw)[g];
-          else
+          if (REAL_IN) {
+            const int64_t r0 = lo0 + 2 * col;
+            const int64_t g = hi * P.in_hi + r0 * P.in_lo + (int64_t)i * P.in_el;
+            const double fa = P.dec_axis ? P.dec_axis[i] * fhi : 1.0;
+            val[u].x = static_cast<const double*>(in_raw)[g] * (P.dec_axis ? fa * P.dec_lo[r0] : 1.0);
+            if (2 * col + 1 < nrow)
+              val[u].y = static_cast<const double*>(in_raw)[g + P.in_lo] * (P.dec_axis ? fa * P.dec_lo[r0 + 1] : 1.0);
+          } else {
+            const int64_t g = hi * P.in_hi + (lo0 + col) * P.in_lo + (int64_t)i * P.in_el;
             val[u] = static_cast<const double2*>(in_raw)[g];
-          if (P.dec_axis) {
-            const double f = P.dec_axis[i] * fhi * P.dec_lo[lo0 + col];
-            val[u].x *= f;
-            val[u].y *= f;
+            if (P.dec_axis) {
+              const double f = P.dec_axis[i] * fhi * P.dec_lo[lo0 + col];
+              val[u].x *= f;
+              val[u].y *= f;
+            }
           }
         }
       }
@@ -278,7 +289,14 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
     if (col >= ncol) continue;
     int m = P.lo + mm;
     m = m < 0 ? m + N : (m >= N ? m - N : m);
-    out[hi * P.out_hi + (lo0 + col) * P.out_lo + (int64_t)mm * P.out_el] = a[P.rev[m] * tbp + col];
+    if (REAL_IN) {
+      const double2 z = a[P.rev[m] * tbp + col], zc = a[P.rev[m == 0 ? 0 : N - m] * tbp + col];
+      const int64_t o = hi * P.out_hi + (lo0 + 2 * col) * P.out_lo + (int64_t)mm * P.out_el;
+      out[o] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
+      if (2 * col + 1 < nrow) out[o + P.out_lo] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
+    } else {
+      out[hi * P.out_hi + (lo0 + col) * P.out_lo + (int64_t)mm * P.out_el] = a[P.rev[m] * tbp + col];
+    }
   }
 }
 
@@ -424,7 +442,8 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
     else
       for (int s = 0; s < P.nfac; ++s) push(P.fac[s], 1);
   }
-  const int64_t tiles = P.n_hi * ((P.n_lo + P.tb - 1) / P.tb);
+  const int64_t rows_per_tile = (int64_t)P.tb * (P.real_in ? 2 : 1);   // real rows are packed in pairs
+  const int64_t tiles = P.n_hi * ((P.n_lo + rows_per_tile - 1) / rows_per_tile);
   if (tiles == 0) return SFD_OK;
   SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
   const size_t smem = (size_t)P.N * P.tbp * 16;
