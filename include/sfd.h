@@ -159,6 +159,13 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
                               double s_paper, double xi_max, int32_t M, double eps, void* d_work, size_t work_bytes,
                               sfd_stream stream, double* h_norm, double* h_I);
 
+/* ---- two meshes against each other ------------------------------------------------------------------
+ * I = (2 pi)^-3 sum_k W_k |nuhat_a,k - nuhat_b,k|^2 (1+|xi_k|^2)^-s: the squared H^{-s} distance between two atomic
+ * measures whose transforms on the same nodes are given (two calls of sfd_surface_ft).  Same workspace, determinism
+ * and error behaviour as sfd_reduce.  Synchronises. */
+int sfd_reduce_pair(const double* d_nuhat_a, const double* d_nuhat_b, const double* d_xi, const double* d_W, int64_t K,
+                    double s, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+
 /* ---- host-buffer entry points (end-to-end: allocate, copy in, run, copy out, free) -------------
  * Same operations with HOST pointers; device memory comes from the stream-ordered CUDA pool of the
  * current device.  Synchronise. */

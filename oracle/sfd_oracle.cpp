@@ -418,6 +418,18 @@ double orc_reduce_ex(const double* nuhat, const double* xi, const double* W, int
   return (double)(acc * (long double)pref);
 }
 
+// Two atomic measures against each other: I = (2 pi)^-3 sum_k W_k |a_k - b_k|^2 (1+|xi_k|^2)^{-s}.
+double orc_reduce_pair(const double* a, const double* b, const double* xi, const double* W, int64_t K, double s) {
+  long double acc = 0;
+  for (int64_t k = 0; k < K; ++k) {
+    const double r2 = xi[3 * k] * xi[3 * k] + xi[3 * k + 1] * xi[3 * k + 1] + xi[3 * k + 2] * xi[3 * k + 2];
+    const double dre = a[2 * k] - b[2 * k], dim = a[2 * k + 1] - b[2 * k + 1];
+    acc += (long double)(W[k] * (dre * dre + dim * dim) * std::pow(1.0 + r2, -s));
+  }
+  return (double)(acc / (8.0L * 3.14159265358979323846264338327950288L * 3.14159265358979323846264338327950288L *
+                         3.14159265358979323846264338327950288L));
+}
+
 // sqrt(I) for a mesh against the unit sphere; also returns I.
 int orc_weak_distance(const double* V, int64_t nV, const int32_t* F, int64_t nF, int rule, double s,
                       double R, int n_r, int n_th, int n_ph, double* dist, double* I) {

@@ -35,6 +35,8 @@ _lib.orc_reduce.restype = C.c_double
 _lib.orc_lattice_nodes.argtypes = [C.c_int, C.c_double, _dp, _dp]
 _lib.orc_reduce_ex.argtypes = [_dp, _dp, _dp, _i64, C.c_double, C.c_double, C.c_double]
 _lib.orc_reduce_ex.restype = C.c_double
+_lib.orc_reduce_pair.argtypes = [_dp, _dp, _dp, _dp, _i64, C.c_double]
+_lib.orc_reduce_pair.restype = C.c_double
 _lib.orc_weak_distance.argtypes = [_dp, _i64, _ip, _i64, C.c_int, C.c_double, C.c_double, C.c_int,
                                    C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.orc_num_threads.restype = C.c_int
@@ -139,6 +141,15 @@ def reduce_ex(nuhat, xi, W, s, scale, pref):
     xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
     W = np.ascontiguousarray(W, np.float64).reshape(-1)
     return _lib.orc_reduce_ex(nu, xi, W, len(W), float(s), float(scale), float(pref))
+
+
+def reduce_pair(a, b, xi, W, s):
+    """(2 pi)^-3 sum_k W_k |a_k - b_k|^2 (1+|xi_k|^2)^-s for two transforms on the same nodes."""
+    a = np.ascontiguousarray(a, np.complex128).view(np.float64).reshape(-1, 2)
+    b = np.ascontiguousarray(b, np.complex128).view(np.float64).reshape(-1, 2)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    W = np.ascontiguousarray(W, np.float64).reshape(-1)
+    return _lib.orc_reduce_pair(a, b, xi, W, len(W), float(s))
 
 
 def weak_distance(V, F, q, s, R, n_r, n_th, n_ph):

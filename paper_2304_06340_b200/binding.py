@@ -61,6 +61,7 @@ _SIGS = {
     "sfd_weak_distance_lattice_workspace": (C.c_int, [_i64, C.c_int, C.c_int32, _dbl, _dbl, _dbl, _P(_sz)]),
     "sfd_weak_distance_lattice": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, C.c_int32, _dbl, _vp, _sz, _vp,
                                             _P(_dbl), _P(_dbl)]),
+    "sfd_reduce_pair": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
     "sfd_surface_ft_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp]),
     "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
                                          _P(_dbl), _P(_dbl)]),
@@ -354,3 +355,31 @@ def sfd_weak_distance_lattice(V, F, rule, s_paper, xi_max, M, eps=0.0, work=None
                                         float(xi_max), int(M), float(eps), _ptr(work), work.numel(), _stream(),
                                         C.byref(d), C.byref(I)))
     return d.value, I.value
+
+
+# ---- two meshes against each other ----------------------------------------------------------------
+def sfd_reduce_pair(nuhat_a, nuhat_b, xi, W, s):
+    """(2 pi)^-3 sum_k W_k |nuhat_a - nuhat_b|^2 (1+|xi_k|^2)^-s (host float)."""
+    na = torch.view_as_real(nuhat_a) if nuhat_a.is_complex() else nuhat_a
+    nb = torch.view_as_real(nuhat_b) if nuhat_b.is_complex() else nuhat_b
+    _dev_f64(na, 2), _dev_f64(nb, 2), _dev_f64(xi, 3), _dev_f64(W)
+    K = xi.shape[0]
+    assert na.shape[0] == K and nb.shape[0] == K
+    wb = _sz()
+    _chk(_lib.sfd_reduce_workspace(K, C.byref(wb)))
+    work = _work(wb.value, xi.device)
+    I = _dbl()
+    _chk(_lib.sfd_reduce_pair(_ptr(na), _ptr(nb), _ptr(xi), _ptr(W), K, float(s), _ptr(work), work.numel(), _stream(),
+                              C.byref(I)))
+    return I.value
+
+
+def sfd_mesh_distance(Va, Fa, Vb, Fb, rule, s, R, q, eps=0.0):
+    """(sqrt(I), I): H^{-s} distance between the surface measures of two meshes on the ball quadrature (q, R)."""
+    xa, wa = sfd_nodes(Va, Fa, rule)
+    xb, wb_ = sfd_nodes(Vb, Fb, rule)
+    xi, W = sfd_freq_nodes_device(q, R, Va.device)
+    na = sfd_surface_ft(xa, wa, xi, eps)
+    nb = sfd_surface_ft(xb, wb_, xi, eps)
+    I = sfd_reduce_pair(na, nb, xi, W, s)
+    return float(np.sqrt(I)), I

@@ -487,6 +487,20 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   return SFD_OK;
 }
 
+// ---- mesh against mesh ("discretized surfaces are compared to each other by recomputing the Fourier
+// transform from their own data representations") ---------------------------------------------------------------
+int sfd_reduce_pair(const double* d_nuhat_a, const double* d_nuhat_b, const double* d_xi, const double* d_W, int64_t K,
+                    double s, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I) {
+  SFD_REQUIRE(h_I, SFD_ERR_NULL, "sfd_reduce_pair: h_I is NULL");
+  SFD_REQUIRE(K == 0 || d_nuhat_b, SFD_ERR_NULL, "sfd_reduce_pair: NULL second operand");
+  cudaStream_t st = as_stream(stream);
+  double* d_res = nullptr;
+  SFD_TRY(reduce_enqueue(d_nuhat_a, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res, 1.0, -1.0, d_nuhat_b));
+  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  return SFD_OK;
+}
+
 // ---- host-buffer entry points -----------------------------------------------------------------------
 namespace {
 struct HostCall {

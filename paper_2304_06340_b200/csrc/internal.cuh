@@ -42,7 +42,8 @@ size_t reduce_workspace(int64_t K);
 // inside the workspace: reduce_result_ptr).
 // General form: I = pref * sum_k W_k |nuhat_k - sigmahat(|xi_k|)|^2 (1 + (scale |xi_k|)^2)^-s; pref < 0 means (2 pi)^-3.
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
-                   size_t work_bytes, cudaStream_t st, double** d_result, double scale = 1.0, double pref = -1.0);
+                   size_t work_bytes, cudaStream_t st, double** d_result, double scale = 1.0, double pref = -1.0,
+                   const double* d_nuhat2 = nullptr);   // d_nuhat2: second operand instead of sigmahat
 // nodes.cu: the paper's cube lattice: xi' = 2 pi xi_ijk, W = w_ijk h^3
 int lattice_expand(int M, double xi_max, double* d_xi, double* d_W, cudaStream_t st);
 

@@ -72,7 +72,9 @@ __device__ __forceinline__ double sobolev_weight(double q, double s, int s_kind)
   return pow(q, -s);
 }
 
-__global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* __restrict__ nuhat, const double* __restrict__ xi,
+// nuhat2 == nullptr: difference against the unit sphere's closed form; else against a second transform (mesh vs mesh)
+__global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* __restrict__ nuhat,
+                                                               const double2* __restrict__ nuhat2, const double* __restrict__ xi,
                                                                const double* __restrict__ W, int64_t K, double s, int s_kind,
                                                                double scale2, Comp* __restrict__ partial) {
   Comp acc{0.0, 0.0};
@@ -82,8 +84,16 @@ __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* _
     const double2 nu = nuhat[k];
     const double r2 = a * a + b * b + c * c;
     const double r = sqrt(r2);
-    const double dre = nu.x - sigma_hat(r);
-    const double term = W[k] * (dre * dre + nu.y * nu.y) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
+    double dre, dim;
+    if (nuhat2) {
+      const double2 nb = nuhat2[k];
+      dre = nu.x - nb.x;
+      dim = nu.y - nb.y;
+    } else {
+      dre = nu.x - sigma_hat(r);
+      dim = nu.y;
+    }
+    const double term = W[k] * (dre * dre + dim * dim) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
     two_sum_add(acc, term);
   }
   const Comp tot = block_reduce(acc);
@@ -113,7 +123,8 @@ size_t reduce_workspace(int64_t K) {
 }
 
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
-                   size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref) {
+                   size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref,
+                   const double* d_nuhat2) {
   if (pref < 0.0) pref = 1.0 / (6.283185307179586 * 6.283185307179586 * 6.283185307179586);   // (2 pi)^-3
   SFD_REQUIRE(K >= 0, SFD_ERR_INVALID_ARG, "K must be >= 0");
   SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
@@ -129,7 +140,8 @@ int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W,
   }
   const int blocks = reduce_blocks(K);
   const int s_kind = s == 1.0 ? 1 : (s == 2.0 ? 2 : 0);
-  reduce_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(d_nuhat), d_xi, d_W, K, s, s_kind,
+  reduce_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(d_nuhat),
+                                                   reinterpret_cast<const double2*>(d_nuhat2), d_xi, d_W, K, s, s_kind,
                                                    scale * scale, partial);
   SFD_TRY(launch_check("reduce_terms_kernel"));
   reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);

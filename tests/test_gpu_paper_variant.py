@@ -93,3 +93,22 @@ def test_paper_fig3b_convergence(sfd, orc, torch):
     V, F = sfd.sfd_mesh_icosphere(3)
     d0, _ = sfd.sfd_weak_distance_lattice(V, F, 64, -10.0, 5.0, 128, 0.0)
     assert abs(d0 / nrm - rel[3]) <= 1e-6 * rel[3]
+
+
+def test_mesh_vs_mesh(sfd, orc, torch):
+    """sfd_reduce_pair / sfd_mesh_distance against the oracle; NUFFT path within its bound."""
+    V1, F1 = orc.mesh_icosphere(2)
+    V2, F2 = orc.mesh_icosphere(3)
+    q, R = (16, 8, 12), 12.0
+    xi, W = orc.freq_nodes(*q, R)
+    n1 = orc.direct_sum(*orc.nodes(V1, F1, 6), xi)
+    n2 = orc.direct_sum(*orc.nodes(V2, F2, 6), xi)
+    for s in (1.0, 2.0):
+        I_ref = orc.reduce_pair(n1, n2, xi, W, s)
+        I = sfd.sfd_reduce_pair(dev(torch, n1.view(np.float64).reshape(-1, 2)), dev(torch, n2.view(np.float64).reshape(-1, 2)),
+                                dev(torch, xi), dev(torch, W), s)
+        assert abs(I - I_ref) <= 1e-12 * I_ref
+        d, I2 = sfd.sfd_mesh_distance(dev(torch, V1), dev(torch, F1), dev(torch, V2), dev(torch, F2), 6, s, R, q, 0.0)
+        assert abs(I2 - I_ref) <= 1e-8 * I_ref
+        d3, I3 = sfd.sfd_mesh_distance(dev(torch, V1), dev(torch, F1), dev(torch, V2), dev(torch, F2), 6, s, R, q, 1e-12)
+        assert abs(I3 - I_ref) <= 1e-6 * I_ref

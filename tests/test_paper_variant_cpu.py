@@ -107,3 +107,26 @@ def test_library_rule64_and_lattice_host(orc):
             P.sfd_lattice_nodes(bad, 5.0)
     with pytest.raises(P.SfdError):
         P.sfd_lattice_nodes(8, -1.0)
+
+
+def test_reduce_pair_pins(orc):
+    """Mesh against mesh: the pair reduction against (i) the sphere reduction when the second operand
+    is sigmahat sampled on the nodes, (ii) the closed form for a translated copy, |1 - e^{-i xi.c}|^2 = 4 sin^2(xi.c/2),
+    (iii) the triangle inequality through the sphere."""
+    V1, F1 = orc.mesh_icosphere(1)
+    V2, F2 = orc.mesh_icosphere(2)
+    xi, W = orc.freq_nodes(12, 6, 8, 10.0)
+    n1 = orc.direct_sum(*orc.nodes(V1, F1, 6), xi)
+    n2 = orc.direct_sum(*orc.nodes(V2, F2, 6), xi)
+    sig = np.array([orc.sigma_hat(float(np.linalg.norm(v))) for v in xi], complex)
+    for s in (1.0, 2.0):
+        I1 = orc.reduce(n1, xi, W, s)
+        assert abs(orc.reduce_pair(n1, sig, xi, W, s) - I1) <= 1e-14 * I1
+        assert orc.reduce_pair(n1, n1, xi, W, s) == 0.0
+        d12 = np.sqrt(orc.reduce_pair(n1, n2, xi, W, s))
+        d1, d2 = np.sqrt(I1), np.sqrt(orc.reduce(n2, xi, W, s))
+        assert abs(d1 - d2) <= d12 <= d1 + d2 and abs(d12 - np.sqrt(orc.reduce_pair(n2, n1, xi, W, s))) < 1e-15
+    c = np.array([0.3, -0.2, 0.1])
+    nt = orc.direct_sum(orc.nodes(V1, F1, 6)[0] + c, orc.nodes(V1, F1, 6)[1], xi)
+    expect = (W * np.abs(n1) ** 2 * 4 * np.sin(xi @ c / 2) ** 2 * (1 + (xi ** 2).sum(1)) ** -2.0).sum() / (2 * np.pi) ** 3
+    assert abs(orc.reduce_pair(n1, nt, xi, W, 2.0) - expect) <= 1e-12 * expect
