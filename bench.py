@@ -385,7 +385,8 @@ def main():
         w, nf, n2 = P.sfd_surface_ft_plan(J, K, [r["ext"]] * 3, [c["R"]] * 3, eps)
         cell = 8      # ball-centred targets: real strengths, real fine grid
         fine = nf[0] * nf[1] * nf[2] * cell
-        no = [min(n2[d], n2[d] // 2 + w + 3) for d in range(3)]
+        no = [min(n2[d], n2[d] // 2 + w + 3 + (w & 1)) for d in range(3)]
+        no[2] = no[2] - (n2[2] // 2 - (n2[2] // 4 - (w + 1) // 2 - 1))   # real strengths: only the upper z half is stored
         band = no[0] * no[1] * no[2]
         pa, pb = nf[0] * nf[1] * no[2], nf[0] * no[1] * no[2]
         sp_bytes = 2 * fine + 40 * J            # zero-fill + one accumulation pass of the grid + sorted sources
