@@ -171,7 +171,7 @@ __device__ __forceinline__ void fused_stages(double2* __restrict__ a, const doub
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
 // 1024 with one (long transforms): 32 warps per SM either way -- the stages are latency-bound (shared-memory and
 // twiddle loads feeding short FP64 chains), so occupancy is what buys throughput (profiles/r1c_nufft.md).
-template <bool REAL_IN, int THREADS, int CG, bool FUSED>
+template <bool REAL_IN, bool CONTIG, int THREADS, int CG, bool FUSED>
 __global__ void __launch_bounds__(THREADS, (FUSED ? 512 : 1024) / THREADS)
 fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
   constexpr int kFftThreads = THREADS;
@@ -191,64 +191,98 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   const double2* __restrict__ tw = P.tw;
 
   // ---- load: input i <-> mode l = i - n_in/2 goes to position l mod N of the padded row; the rest is zero.
-  // Four independent loads per thread are in flight before the first store (the pass is latency-bound otherwise).
+  // Addressing is kept out of the inner loops (the first version spent 70 % of its instructions on 64-bit index
+  // arithmetic here and in the store): threads form a (ty, col) grid with col fastest in the strided passes, a
+  // (warp = column, lane = element) grid in the contiguous one; pointers advance by constant strides; four
+  // independent loads per thread are in flight before the first store.
   const int half_in = P.n_in / 2;
   const double fhi = P.dec_hi ? P.dec_hi[hi] : 1.0;
-  const int n_pad = N - P.n_in;   // zero positions: [n_in - half_in, N - half_in)
-  for (int idx = tid; idx < n_pad * tb; idx += kFftThreads) {
-    int j, col;
-    if (P.contig) {
-      col = idx / n_pad;
-      j = idx - col * n_pad;
-    } else {
-      j = idx >> tsh;
-      col = idx & (tb - 1);
-    }
-    a[(P.n_in - half_in + j) * tbp + col] = make_double2(0.0, 0.0);
-  }
-  const int n_ld = P.n_in * tb;
-  for (int idx0 = tid; idx0 < n_ld; idx0 += 4 * kFftThreads) {
-    double2 val[4];
-    int pos[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int idx = idx0 + u * kFftThreads;
-      val[u] = make_double2(0.0, 0.0);
-      pos[u] = -1;
-      if (idx < n_ld) {
-        int i, col;
-        if (P.contig) {
-          col = idx / P.n_in;
-          i = idx - col * P.n_in;
-        } else {
-          i = idx >> tsh;
-          col = idx & (tb - 1);
+  const int n_pad = N - P.n_in;          // zero positions: [n_in - half_in, N - half_in)
+  const int pad0 = P.n_in - half_in;
+  if (CONTIG) {
+    const int lane = tid & 31, wrp = tid >> 5, nw = kFftThreads / 32;
+    for (int col = wrp; col < tb; col += nw) {
+      for (int j = lane; j < n_pad; j += 32) a[(pad0 + j) * tbp + col] = make_double2(0.0, 0.0);
+      if (col >= ncol) {
+        for (int i = lane; i < P.n_in; i += 32) {
+          const int l = i - half_in;
+          a[(l < 0 ? l + N : l) * tbp + col] = make_double2(0.0, 0.0);
         }
-        const int l = i - half_in;
-        pos[u] = (l < 0 ? l + N : l) * tbp + col;
-        if (col < ncol) {
-          if (REAL_IN) {
-            const int64_t r0 = lo0 + 2 * col;
-            const int64_t g = hi * P.in_hi + r0 * P.in_lo + (int64_t)i * P.in_el;
-            const double fa = P.dec_axis ? P.dec_axis[i] * fhi : 1.0;
-            val[u].x = static_cast<const double*>(in_raw)[g] * (P.dec_axis ? fa * P.dec_lo[r0] : 1.0);
-            if (2 * col + 1 < nrow)
-              val[u].y = static_cast<const double*>(in_raw)[g + P.in_lo] * (P.dec_axis ? fa * P.dec_lo[r0 + 1] : 1.0);
-          } else {
-            const int64_t g = hi * P.in_hi + (lo0 + col) * P.in_lo + (int64_t)i * P.in_el;
-            val[u] = static_cast<const double2*>(in_raw)[g];
-            if (P.dec_axis) {
-              const double f = P.dec_axis[i] * fhi * P.dec_lo[lo0 + col];
-              val[u].x *= f;
-              val[u].y *= f;
+        continue;
+      }
+      if (REAL_IN) {
+        const int64_t r0 = lo0 + 2 * col;
+        const bool two = 2 * col + 1 < nrow;
+        const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
+        const double* src1 = src0 + (two ? P.in_lo : 0);
+        const double f0 = P.dec_axis ? fhi * P.dec_lo[r0] : 1.0;
+        const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
+        for (int i0 = lane; i0 < P.n_in; i0 += 128) {
+          double va[4], vb[4], fa[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = i0 + 32 * u;
+            const bool ok = i < P.n_in;
+            va[u] = ok ? src0[i] : 0.0;
+            vb[u] = ok ? src1[i] : 0.0;
+            fa[u] = (ok && P.dec_axis) ? P.dec_axis[i] : 1.0;
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = i0 + 32 * u;
+            if (i < P.n_in) {
+              const int l = i - half_in;
+              a[(l < 0 ? l + N : l) * tbp + col] = make_double2(va[u] * (fa[u] * f0), vb[u] * (fa[u] * f1));
+            }
+          }
+        }
+      } else {
+        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + col) * P.in_lo;
+        const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + col] : 1.0;
+        for (int i0 = lane; i0 < P.n_in; i0 += 128) {
+          double2 v[4];
+          double fa[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = i0 + 32 * u;
+            const bool ok = i < P.n_in;
+            v[u] = ok ? src[i] : make_double2(0.0, 0.0);
+            fa[u] = (ok && P.dec_axis) ? P.dec_axis[i] * f0 : 1.0;
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = i0 + 32 * u;
+            if (i < P.n_in) {
+              const int l = i - half_in;
+              a[(l < 0 ? l + N : l) * tbp + col] = make_double2(v[u].x * fa[u], v[u].y * fa[u]);
             }
           }
         }
       }
     }
+  } else {
+    // strided passes (complex input, no deconvolution factors): in_lo = 1, rows in_el apart
+    const int col = tid & (tb - 1), ty = tid >> tsh, nty = kFftThreads >> tsh;
+    for (int j = ty; j < n_pad; j += nty) a[(pad0 + j) * tbp + col] = make_double2(0.0, 0.0);
+    const bool live = col < ncol;
+    const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + col + (int64_t)ty * P.in_el;
+    const int64_t step = (int64_t)nty * P.in_el;
+    for (int i0 = ty; i0 < P.n_in; i0 += 4 * nty) {
+      double2 v[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (pos[u] >= 0) a[pos[u]] = val[u];
+      for (int u = 0; u < 4; ++u) {
+        v[u] = (live && i0 + u * nty < P.n_in) ? src[u * step] : make_double2(0.0, 0.0);
+      }
+      src += 4 * step;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + u * nty;
+        if (i < P.n_in) {
+          const int l = i - half_in;
+          a[(l < 0 ? l + N : l) * tbp + col] = v[u];
+        }
+      }
+    }
   }
   __syncthreads();
 
@@ -277,25 +311,40 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   }
 
   // ---- store the band m in [lo, lo + nout) through the digit-reversal table
-  for (int idx = tid; idx < P.nout * tb; idx += kFftThreads) {
-    int mm, col;
-    if (P.contig) {
-      col = idx / P.nout;
-      mm = idx - col * P.nout;
-    } else {
-      mm = idx >> tsh;
-      col = idx & (tb - 1);
+  if (CONTIG) {
+    const int lane = tid & 31, wrp = tid >> 5, nw = kFftThreads / 32;
+    for (int col = wrp; col < ncol; col += nw) {
+      if (REAL_IN) {
+        const bool two = 2 * col + 1 < nrow;
+        double2* o0 = out + hi * P.out_hi + (lo0 + 2 * col) * P.out_lo;
+        double2* o1 = o0 + P.out_lo;
+        for (int mm = lane; mm < P.nout; mm += 32) {
+          int m = P.lo + mm;
+          m = m < 0 ? m + N : (m >= N ? m - N : m);
+          const double2 z = a[P.rev[m] * tbp + col], zc = a[P.rev[m == 0 ? 0 : N - m] * tbp + col];
+          o0[mm] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
+          if (two) o1[mm] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
+        }
+      } else {
+        double2* o0 = out + hi * P.out_hi + (lo0 + col) * P.out_lo;
+        for (int mm = lane; mm < P.nout; mm += 32) {
+          int m = P.lo + mm;
+          m = m < 0 ? m + N : (m >= N ? m - N : m);
+          o0[mm] = a[P.rev[m] * tbp + col];
+        }
+      }
     }
-    if (col >= ncol) continue;
-    int m = P.lo + mm;
-    m = m < 0 ? m + N : (m >= N ? m - N : m);
-    if (REAL_IN) {
-      const double2 z = a[P.rev[m] * tbp + col], zc = a[P.rev[m == 0 ? 0 : N - m] * tbp + col];
-      const int64_t o = hi * P.out_hi + (lo0 + 2 * col) * P.out_lo + (int64_t)mm * P.out_el;
-      out[o] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
-      if (2 * col + 1 < nrow) out[o + P.out_lo] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
-    } else {
-      out[hi * P.out_hi + (lo0 + col) * P.out_lo + (int64_t)mm * P.out_el] = a[P.rev[m] * tbp + col];
+  } else {
+    const int col = tid & (tb - 1), ty = tid >> tsh, nty = kFftThreads >> tsh;
+    if (col < ncol) {
+      double2* o = out + hi * P.out_hi + lo0 + col + (int64_t)ty * P.out_el;
+      const int64_t step = (int64_t)nty * P.out_el;
+      for (int mm = ty; mm < P.nout; mm += nty) {
+        int m = P.lo + mm;
+        m = m < 0 ? m + N : (m >= N ? m - N : m);
+        *o = a[P.rev[m] * tbp + col];
+        o += step;
+      }
     }
   }
 }
@@ -461,18 +510,27 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
     kern<<<(unsigned)tiles, threads, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
     return SFD_OK;
   };
-#define SFD_FFT_GO(REAL_, T_)                                     \
-  (cg == 2 ? go(fft_pass_kernel<REAL_, T_, 2, false>) : go(fft_pass_kernel<REAL_, T_, 1, false>))
-  if (fused) {
-    if (P.real_in)
-      SFD_TRY(threads == 256 ? go(fft_pass_kernel<true, 256, 1, true>) : go(fft_pass_kernel<true, 512, 1, true>));
-    else
-      SFD_TRY(threads == 256 ? go(fft_pass_kernel<false, 256, 1, true>) : go(fft_pass_kernel<false, 512, 1, true>));
-  } else if (P.real_in)
-    SFD_TRY(threads == 256 ? SFD_FFT_GO(true, 256) : (threads == 512 ? SFD_FFT_GO(true, 512) : SFD_FFT_GO(true, 1024)));
+  // kernel variants: (real, contiguous) = pass A with real strengths; (complex, contiguous) = pass A otherwise;
+  // (complex, strided) = passes B and C
+#define SFD_FFT_T(REAL_, CONTIG_)                                                                               \
+  (fused ? (threads == 256 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, true>)                                   \
+                           : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, true>))                                  \
+         : (threads == 256 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 2, false>)                       \
+                                      : go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, false>))                      \
+            : threads == 512 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 512, 2, false>)                     \
+                                        : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, false>))                    \
+                             : go(fft_pass_kernel<REAL_, CONTIG_, 1024, 1, false>)))
+  SFD_REQUIRE(P.contig || (!P.real_in && !P.dec_axis && P.in_lo == 1 && P.out_lo == 1), SFD_ERR_INVALID_ARG,
+              "strided FFT passes take complex input with unit row stride and no deconvolution factors");
+  SFD_REQUIRE(!P.contig || (P.in_el == 1 && P.out_el == 1), SFD_ERR_INVALID_ARG,
+              "the contiguous FFT pass needs unit element stride");
+  if (P.contig && P.real_in)
+    SFD_TRY(SFD_FFT_T(true, true));
+  else if (P.contig)
+    SFD_TRY(SFD_FFT_T(false, true));
   else
-    SFD_TRY(threads == 256 ? SFD_FFT_GO(false, 256) : (threads == 512 ? SFD_FFT_GO(false, 512) : SFD_FFT_GO(false, 1024)));
-#undef SFD_FFT_GO
+    SFD_TRY(SFD_FFT_T(false, false));
+#undef SFD_FFT_T
   return launch_check("fft_pass_kernel");
 }
 
