@@ -436,10 +436,15 @@ size_t fft_tables_bytes(const int n2[3]) {
 int fft_tile(int N, int contig, int* tbp) {
   int pick = 0, pitch = 0;
   auto fits = [&](int tb, int pt, size_t cap) { return (size_t)N * pt * 16 <= cap; };
-  if (fits(8, 9, (size_t)112 * 1024)) pick = 8, pitch = 9;                       // column groups of 2, 2-4 CTAs per SM
-  if (!pick && fits(4, contig ? 5 : 4, (size_t)112 * 1024)) pick = 4, pitch = contig ? 5 : 4;   // two CTAs per SM
-  for (int tb = 8; tb >= 1 && !pick; tb >>= 1)                                   // one CTA per SM
-    if (fits(tb, contig ? (tb | 1) : tb, (size_t)224 * 1024)) pick = tb, pitch = contig ? (tb | 1) : tb;
+  const size_t half = (size_t)112 * 1024, full = (size_t)224 * 1024;
+  if (fits(8, 9, half)) pick = 8, pitch = 9;                       // column groups of 2, 2-4 CTAs per SM
+  // long transforms: two CTAs per SM matter more than the conflict-free transposing load (even pitch)
+  if (!pick && fits(4, contig ? 5 : 4, half)) pick = 4, pitch = contig ? 5 : 4;
+  if (!pick && fits(4, 4, half)) pick = 4, pitch = 4;
+  if (!pick && fits(2, contig ? 3 : 2, half)) pick = 2, pitch = contig ? 3 : 2;
+  if (!pick && fits(2, 2, half)) pick = 2, pitch = 2;
+  for (int tb = 8; tb >= 1 && !pick; tb >>= 1)                     // one CTA per SM
+    if (fits(tb, contig ? (tb | 1) : tb, full)) pick = tb, pitch = contig ? (tb | 1) : tb;
   if (tbp) *tbp = pitch;
   return pick;
 }

@@ -28,6 +28,24 @@ constexpr int tpw_for(int W) { return W <= 10 ? 2 : 1; }
 constexpr int kTabBytes = sizeof(double) * kWarps * kMaxTpw * 3 * 16;   // per-warp kernel values: 12 KB
 constexpr int kSmemCells = 13600;   // complex128 cells of the subgrid: 217,600 B
 
+// Target-bin shape for kernel width w, as compile-time functions (host and device use the same numbers): z extent 8
+// or 16 (conflict-free pitch), x and y as large as the shared-memory budget allows; the shape with the best
+// owned-cells / staged-cells ratio wins.  With the shape fixed per W every subgrid stride is an immediate.
+constexpr int bin_xy(int w, int bz) {
+  int m = 1;
+  while ((m + 1) * (m + 1) * (bz + w) <= kSmemCells) ++m;
+  return m - w;
+}
+constexpr int bin_z(int w) {
+  const int b8 = bin_xy(w, 8), b16 = bin_xy(w, 16);
+  if (b8 < 1) return 16;
+  if (b16 < 1) return 8;
+  // ratio b^2 bz / ((b+w)^2 (bz+w)), compared by cross-multiplication in 64-bit
+  const long long l8 = (long long)b8 * b8 * 8 * (b16 + w) * (b16 + w) * (16 + w);
+  const long long l16 = (long long)b16 * b16 * 16 * (b8 + w) * (b8 + w) * (8 + w);
+  return l16 > l8 ? 16 : 8;
+}
+
 template <int W>
 __global__ void __launch_bounds__(32 * kWarps, 1)
 interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __restrict__ v, const TgtRec* __restrict__ tgt,
@@ -43,8 +61,9 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
   __shared__ int s_item;
 
   const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, li = lane & 15;
-  const int Px = p.bt[0] + W, Py = p.bt[1] + W, Pz = p.bt[2] + W;
-  const int plane = Py * Pz;
+  constexpr int BZ = bin_z(W), BXY = bin_xy(W, BZ);
+  constexpr int Px = BXY + W, Py = BXY + W, Pz = BZ + W;
+  constexpr int plane = Py * Pz;
 
   // the polynomial of interval li, in registers
   double pc[DEG + 1];
@@ -52,10 +71,13 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
   for (int q = 0; q <= DEG; ++q) pc[q] = li < W ? ptab[q * kPolyStride + li] : 0.0;
 
   // the lane's cells of a W x W plane: c = lane + 32 i -> (cy, cz); offset inside the plane cy Pz + cz
+  // (lanes beyond the last cell of the last round read cell 0 and get weight 0: no predicate in the plane loop)
   int off[NCL], cy[NCL], cz[NCL];
+  bool on[NCL];
 #pragma unroll
   for (int i = 0; i < NCL; ++i) {
-    const int c = min(lane + 32 * i, W * W - 1);
+    on[i] = lane + 32 * i < W * W;
+    const int c = on[i] ? lane + 32 * i : 0;
     cy[i] = c / W;
     cz[i] = c - cy[i] * W;
     off[i] = cy[i] * Pz + cz[i];
@@ -145,12 +167,15 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
       __syncwarp();
 
       double are[TPW][NCL], aim[TPW][NCL];
-      const double2* base[TPW];
+      const double2* cell[TPW][NCL];   // the lane's cells in plane 0 of the footprint; plane a is an immediate offset
 #pragma unroll
       for (int u = 0; u < TPW; ++u) {
+        const double2* base = sub + ((i0x[u] - ox) * Py + (i0y[u] - oy)) * Pz + (i0z[u] - oz);
 #pragma unroll
-        for (int i = 0; i < NCL; ++i) are[u][i] = aim[u][i] = 0.0;
-        base[u] = sub + ((i0x[u] - ox) * Py + (i0y[u] - oy)) * Pz + (i0z[u] - oz);
+        for (int i = 0; i < NCL; ++i) {
+          are[u][i] = aim[u][i] = 0.0;
+          cell[u][i] = base + off[i];
+        }
       }
 #pragma unroll
       for (int a = 0; a < W; ++a) {
@@ -159,11 +184,9 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
           const double kx = ktab[wq][u][0][a];
 #pragma unroll
           for (int i = 0; i < NCL; ++i) {
-            if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
-              const double2 c = base[u][a * plane + off[i]];
-              are[u][i] = __fma_rn(c.x, kx, are[u][i]);
-              aim[u][i] = __fma_rn(c.y, kx, aim[u][i]);
-            }
+            const double2 c = cell[u][i][a * plane];
+            are[u][i] = __fma_rn(c.x, kx, are[u][i]);
+            aim[u][i] = __fma_rn(c.y, kx, aim[u][i]);
           }
         }
       }
@@ -173,12 +196,10 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
         re[u] = im[u] = 0.0;
 #pragma unroll
         for (int i = 0; i < NCL; ++i) {
-          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
-            const double kyz = ktab[wq][u][1][cy[i]] * ktab[wq][u][2][cz[i]];
-            re[u] = __fma_rn(are[u][i], kyz, re[u]);
-            // cells below the centre plane hold the mirror cell un-conjugated: flip the sign of their imaginary part
-            im[u] = __fma_rn(aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
-          }
+          const double kyz = on[i] ? ktab[wq][u][1][cy[i]] * ktab[wq][u][2][cz[i]] : 0.0;
+          re[u] = __fma_rn(are[u][i], kyz, re[u]);
+          // cells below the centre plane hold the mirror cell un-conjugated: flip the sign of their imaginary part
+          im[u] = __fma_rn(aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
         }
       }
 #pragma unroll
@@ -215,23 +236,9 @@ int launch(const N3Params& p, const double* d_ptab, const double* d_v, const Tgt
 
 }  // namespace
 
-// Target-bin shape: z extent 8 or 16 (conflict-free pitch), x and y as large as the shared-memory budget allows;
-// the shape with the best owned-cells / staged-cells ratio wins.
 void interp_bins(int w, int bt[3]) {
-  double best = -1.0;
-  for (int bz = 8; bz <= 16; bz += 8) {
-    const int pz = bz + w;
-    int m = 1;
-    while ((m + 1) * (m + 1) * pz <= kSmemCells) ++m;
-    const int b = m - w;
-    if (b < 1) continue;
-    const double ratio = (double)b * b * bz / ((double)m * m * pz);
-    if (ratio > best) {
-      best = ratio;
-      bt[0] = bt[1] = b;
-      bt[2] = bz;
-    }
-  }
+  bt[2] = bin_z(w);
+  bt[0] = bt[1] = bin_xy(w, bt[2]);
 }
 
 size_t interp_smem_bytes(const N3Params& p) {
