@@ -202,18 +202,27 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
           im[u] = __fma_rn(aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
         }
       }
+      if (TPW == 2) {
+        // two targets: the first exchange hands target 0 to lanes 0-15 and target 1 to lanes 16-31, the remaining
+        // four rounds reduce both at once -- 10 fp64 shuffles for two targets instead of 20
+        const bool up = (lane & 16) != 0;
+        const double sre = up ? re[0] : re[TPW - 1], sim = up ? im[0] : im[TPW - 1];
+        double rr = (up ? re[TPW - 1] : re[0]) + __shfl_xor_sync(0xffffffffu, sre, 16);
+        double ri = (up ? im[TPW - 1] : im[0]) + __shfl_xor_sync(0xffffffffu, sim, 16);
 #pragma unroll
-      for (int d = 16; d > 0; d >>= 1) {
-#pragma unroll
-        for (int u = 0; u < TPW; ++u) {
-          re[u] += __shfl_xor_sync(0xffffffffu, re[u], d);
-          im[u] += __shfl_xor_sync(0xffffffffu, im[u], d);
+        for (int d = 8; d > 0; d >>= 1) {
+          rr += __shfl_xor_sync(0xffffffffu, rr, d);
+          ri += __shfl_xor_sync(0xffffffffu, ri, d);
         }
-      }
-      if (lane == 0) {
+        if (lane == 0 && live[0]) G[cur[0].k] = make_double2(rr, ri);
+        if (lane == 16 && live[TPW - 1]) G[cur[TPW - 1].k] = make_double2(rr, ri);
+      } else {
 #pragma unroll
-        for (int u = 0; u < TPW; ++u)
-          if (live[u]) G[cur[u].k] = make_double2(re[u], im[u]);
+        for (int d = 16; d > 0; d >>= 1) {
+          re[0] += __shfl_xor_sync(0xffffffffu, re[0], d);
+          im[0] += __shfl_xor_sync(0xffffffffu, im[0], d);
+        }
+        if (lane == 0 && live[0]) G[cur[0].k] = make_double2(re[0], im[0]);
       }
     }
   }
