@@ -101,3 +101,29 @@ def test_workspace_queries_scale(sfd):
     assert b > a > 0
     w0 = sfd.sfd_weak_distance_workspace(80, 6, (32, 16, 32), 32.0, 0.0)
     assert w0 >= 480 * 32 + 16384 * 48
+
+
+def test_plan_and_workspace_queries(sfd):
+    """sfd_surface_ft_plan / *_workspace are host-only: sizes of BASELINE.json's configs and argument checks."""
+    w, nf, n2 = sfd.sfd_surface_ft_plan(30720, 1 << 20, [1, 1, 1], [128, 128, 128], 1e-9)
+    assert w == 10 and nf == [180] * 3 and n2 == [360] * 3            # SURVEY 8(a) type-3 size table, config 2
+    w, nf, n2 = sfd.sfd_surface_ft_plan(983040, 1 << 23, [1, 1, 1], [256, 256, 256], 1e-12)
+    assert w == 13 and nf == [360] * 3 and n2 == [720] * 3            # config 3
+    w, nf, n2 = sfd.sfd_surface_ft_plan(7864320, 1 << 26, [1, 1, 1], [1024, 1024, 1024], 1e-10)
+    assert w == 11 and nf == [1350] * 3 and n2 == [2700] * 3          # config 5, level 8
+    # the pruned transform fits one B200 at config 5 (the padded 2700^3 grid alone would be 315 GB); the query is
+    # sized for complex strengths (127 GB), the ball-centred case that runs uses about half of it
+    wb = sfd.sfd_weak_distance_workspace(20 * 4 ** 8, 6, (512, 256, 512), 1024.0, 1e-10)
+    assert wb < 140e9
+    assert sfd.sfd_surface_ft_workspace(100, 100, None, None, 0.0) >= 0
+    for bad_eps in (-1.0, 1.0, 1e-15):
+        with pytest.raises(sfd.SfdError):
+            sfd.sfd_surface_ft_workspace(10, 10, [1, 1, 1], [1, 1, 1], bad_eps)
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_surface_ft_plan(10, 10, [1, 1, 1], [1, 1, 1], 0.0)    # the direct sum has no plan
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_weak_distance_workspace(10, 7, (4, 4, 4), 1.0, 0.0)   # unknown rule
+    with pytest.raises(sfd.SfdError):
+        sfd.sfd_weak_distance_lattice_workspace(10, 64, 7, 5.0, 0.0)  # odd M
+    assert sfd.sfd_weak_distance_lattice_workspace(20 * 4 ** 7, 64, 128, 5.0, 1e-7) > 20 * 4 ** 7 * 64 * 32
+    assert sfd.sfd_launch_count() >= 0

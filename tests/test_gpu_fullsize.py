@@ -126,3 +126,14 @@ def test_config5_sweep_levels(sfd, orc, torch):
     for level in (3, 4, 5):
         slope = np.log2(dist[level - 1] / dist[level])
         assert 1.8 <= slope <= 2.1, (level, slope, dist)
+    # the top of the sweep: level 8 (7,864,320 atoms) on the same grid, three levels further down the same line
+    V, F = sfd.sfd_mesh_icosphere(8)
+    d8 = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 1e-10)[0]
+    slope = np.log2(dist[5] / d8) / 3
+    assert 1.8 <= slope <= 2.2, (slope, dist, d8)   # 2.13: the coarse levels are biased upwards on this grid (above)
+    # cross-grid check: at level 8 the mesh's spectrum is resolved by this grid too (R h = 4.8), so the value must sit
+    # on the quadratic line through the well-resolved config-3 grid: d_8 = d_6 / 16 to ~1 %
+    c3 = workloads.CONFIGS[3]
+    V6, F6 = sfd.sfd_mesh_icosphere(6)
+    d6 = sfd.sfd_weak_distance(V6, F6, 6, 2.0, c3["R"], (c3["n_r"], c3["n_theta"], c3["n_phi"]), 1e-10)[0]
+    assert abs(16 * d8 / d6 - 1) < 0.02, (d8, d6)
