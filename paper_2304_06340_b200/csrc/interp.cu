@@ -24,7 +24,7 @@ namespace {
 
 constexpr int kWarps = 16;
 constexpr int kMaxTpw = 2;           // targets a warp works on at a time (2 where the accumulators fit the registers)
-constexpr int tpw_for(int W) { return W <= 10 ? 2 : 1; }
+constexpr int tpw_for(int W) { return W <= 10 ? 2 : 1; }   // (w = 11..13 measured slower with 2: spills)
 constexpr int kTabBytes = sizeof(double) * kWarps * kMaxTpw * 3 * 16;   // per-warp kernel values: 12 KB
 constexpr int kSmemCells = 13600;   // complex128 cells of the subgrid: 217,600 B
 
