@@ -249,9 +249,9 @@ def run_sfd(args):
 
 
 # FP64-pipe instructions per source.target pair of direct_sum_kernel (checked against the SASS of
-# the inner loop: 120 DFMA + 24 DMUL + 24 DADD per 8 pairs): phase 1 DMUL + 2 DFMA; quarter-turn reduction 3 DADD;
-# z 1 DMUL; sin 5 DFMA + 1 DMUL; cos 6 DFMA; accumulate 2 DFMA.
-DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 15, 6
+# the inner loop): phase 1 DMUL + 2 DFMA; reduction to 1/256 turn 3 DADD; f^2 1 DMUL; sin 2 DFMA + 1 DMUL; cos 2 DFMA;
+# rotation by the table entry and accumulation 2 DMUL + 4 DFMA  ->  10 DFMA + 5 DMUL + 3 DADD = 18.
+DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 10, 8
 FLOPS_PER_PAIR = 2 * DFMA_PER_PAIR + DMUL_DADD_PER_PAIR
 FP64_LANES_PER_SM = 64          # DFMA / clk / SM on B200 (nominal 37-40 TFLOP/s at 1.965 GHz x 148 SMs)
 

@@ -1,5 +1,6 @@
 // direct.cu -- A4: fp64 direct summation nuhat_k = sum_j w_j exp(-i xi_k . x_j)  (eq. 2.8
-// applied to the atoms of P:152).  FP64-pipe bound: per pair 3 FMA (phase) + 20 (sincos) + 2 (accumulate).
+// applied to the atoms of P:152).  FP64-pipe bound: 18 FP64 instructions per pair (phase 3, reduction 3, table +
+// short polynomials 6, rotate and accumulate 6).
 //
 // Layout: one CTA = 128 threads x T targets held in registers (xi and the two accumulators); the sources
 // stream through shared memory in tiles of kTile atoms, double-buffered with 1-D bulk TMA copies
@@ -15,7 +16,7 @@ namespace sfd {
 namespace {
 
 constexpr int kThreads = 128;
-constexpr int kTile = 512;  // atoms per stage: 512*32 B = 16 KB; two stages
+constexpr int kTile = 256;  // atoms per stage: 256*32 B = 8 KB; two stages (+ the 32 KB table: 48 KB per CTA, 4 CTAs per SM)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -45,42 +46,23 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                : "memory");
 }
 
-// sin and cos of (pi/2) tq for the inner loop: the targets are pre-scaled by 2/pi once per thread, so the phase
-// arrives in quarter turns and the range reduction is three exact additions (n = rint(tq) by the 1.5*2^52 trick,
-// f = tq - n in [-1/2, 1/2] exactly); sin(pi/2 f) = f S(f^2), cos(pi/2 f) = C(f^2) with 6 / 7 coefficients
-// (gen_sincos_coeffs.py qturn: max error 3.8e-15 / 1.8e-16, far below the 1e-12 sum|w| bar and below the rounding of
-// the phase itself, ~|tq| 2^-52).  14 FP64-pipe instructions + the quadrant fix-up on the integer pipe.
-// Coefficients live in the constant bank and are used as direct c[3][..] operands: measured 2 % faster than
-// immediates, which ptxas re-materialises into uniform registers inside the loop (every non-FP64 instruction costs
-// an issue cycle next to a 2-cycle DFMA; profiles/r1b_direct_sum.md).
-__constant__ double c_sc[14] = {
-    -3.55553766329449158383e-6, 1.60428782872071630554e-4, -4.68175249674726216909e-3, 7.96926261482708977477e-2,
-    -6.45964097504106775201e-1, 1.57079632679488904148,                                  // S5..S0
-    4.65418527335501644036e-7, -2.52000581168362530624e-5, 9.19259930116159750314e-4, -2.08634807325982068569e-2,
-    2.53669507899741166079e-1, -1.23370055013614900029, 0.999999999999999945803,         // C6..C0
-    6755399441055744.0};                                                                 // 1.5 * 2^52
-__device__ __forceinline__ void sincos_qturn(double tq, double& s, double& c) {
-  const double nm = __dadd_rn(tq, c_sc[13]);
-  const int q = __double2loint(nm);
-  const double n = __dsub_rn(nm, c_sc[13]);
-  const double f = __dsub_rn(tq, n);
-  const double z = f * f;
-  double ps = c_sc[0];
-#pragma unroll
-  for (int i = 1; i <= 5; ++i) ps = __fma_rn(ps, z, c_sc[i]);
-  const double sr = f * ps;
-  double pc = c_sc[6];
-#pragma unroll
-  for (int i = 7; i <= 11; ++i) pc = __fma_rn(pc, z, c_sc[i]);
-  const double cr = __fma_rn(pc, z, c_sc[12]);
-  // quadrant: q&1 swaps, sign of sin flips for q&2, sign of cos flips for (q+1)&2
-  const double so = (q & 1) ? cr : sr;
-  const double co = (q & 1) ? sr : cr;
-  const int shi = __double2hiint(so) ^ ((q & 2) << 30);
-  const int chi = __double2hiint(co) ^ (((q + 1) & 2) << 30);
-  s = __hiloint2double(shi, __double2loint(so));
-  c = __hiloint2double(chi, __double2loint(co));
-}
+// exp(-i theta) for the inner loop, table + short polynomials.  The targets are pre-scaled by kTab/(2 pi) once per
+// thread, so the phase arrives in units of 1/kTab of a turn: tq = n + f with n = rint(tq) (the 1.5*2^52 trick: three
+// exact additions) and |f| <= 1/2, i.e. a residual angle of at most pi/256.  The table holds (cos, sin)(2 pi k / kTab)
+// for the whole turn, so there is no quadrant logic at all; sin and cos of the residual need 3 coefficients each
+// (gen_sincos_coeffs.py table: max error 1.2e-18 and 2.3e-16); one complex rotation joins the two.  18 FP64-pipe
+// instructions per pair (phase 3, reduction 3, f^2 1, sin 3, cos 2, rotate + accumulate 6) against 21 plus a 10-instruction
+// integer fix-up for the polynomial-only version: measured 1.31x faster (profiles/r1e_direct_sum_table.md), because
+// every non-FP64 instruction costs an issue cycle next to a 2-cycle DFMA.
+// The table is replicated kRep = 8 times in shared memory, entry (k, lane & 7) at index k*8 + (lane & 7): the 8 lanes
+// of each LDS.128 phase then read 8 different 16-byte bank groups whatever their k -- conflict-free by construction.
+constexpr int kTab = 256;
+constexpr int kRep = 8;
+__constant__ double c_sc[8] = {
+    7.4219134520576935249e-11, -2.4641574764100320108e-6, 0.024543692606170259123,   // S2..S0: sin(a f) = f S(f^2)
+    1.5119764735229900432e-8, -0.00030119642336197489329, 0.9999999999999998425,      // C2..C0: cos(a f) = C(f^2)
+    6755399441055744.0,                                                               // 1.5 * 2^52
+    40.743665431525205956834243423364};                                               // kTab / (2 pi)
 
 struct __align__(16) Stage {
   double x[kTile * 3];
@@ -91,9 +73,18 @@ template <int T>
 __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __restrict__ x, const double* __restrict__ w,
                                                              int64_t J, const double* __restrict__ xi, int64_t K,
                                                              double* __restrict__ out, int64_t j_per_split, int use_tma) {
-  __shared__ Stage stage[2];
-  __shared__ __align__(8) uint64_t bar[2];
+  extern __shared__ __align__(16) unsigned char smem_raw[];   // 48.1 KB: beyond the static limit
+  Stage* stage = reinterpret_cast<Stage*>(smem_raw);
+  double2* tab = reinterpret_cast<double2*>(smem_raw + 2 * sizeof(Stage));
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * sizeof(Stage) + sizeof(double2) * kTab * kRep);
   const int tid = threadIdx.x;
+  // (cos, sin)(2 pi k / kTab), replicated: entry (k, r) at k*kRep + r
+  for (int i = tid; i < kTab * kRep; i += kThreads) {
+    double sv, cv;
+    sincospi((double)(i / kRep) * (2.0 / kTab), &sv, &cv);
+    tab[i] = make_double2(cv, sv);
+  }
+  const double2* tl = tab + (tid & (kRep - 1));
   const int64_t k0 = (int64_t)blockIdx.x * (kThreads * T);
   const int64_t jb = (int64_t)blockIdx.y * j_per_split;
   const int64_t je = min(J, jb + j_per_split);
@@ -103,10 +94,9 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
 #pragma unroll
   for (int t = 0; t < T; ++t) {
     const int64_t k = min(k0 + t * kThreads + tid, K - 1);
-    const double kTwoOverPi = 6.36619772367581382433e-01;
-    a0[t] = xi[3 * k] * kTwoOverPi;   // phases in quarter turns (sincos_qturn)
-    a1[t] = xi[3 * k + 1] * kTwoOverPi;
-    a2[t] = xi[3 * k + 2] * kTwoOverPi;
+    a0[t] = xi[3 * k] * c_sc[7];   // phases in units of 1/kTab of a turn
+    a1[t] = xi[3 * k + 1] * c_sc[7];
+    a2[t] = xi[3 * k + 2] * c_sc[7];
     re[t] = 0.0;
     im[t] = 0.0;
   }
@@ -148,11 +138,21 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
       const double x0 = s.x[3 * j], x1 = s.x[3 * j + 1], x2 = s.x[3 * j + 2], wj = s.w[j];
 #pragma unroll
       for (int u = 0; u < T; ++u) {
-        const double th = __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
-        double sn, cs;
-        sincos_qturn(th, sn, cs);
-        re[u] = __fma_rn(wj, cs, re[u]);
-        im[u] = __fma_rn(wj, sn, im[u]);
+        const double tq = __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
+        const double nm = __dadd_rn(tq, c_sc[6]);
+        const int q = __double2loint(nm);
+        const double nn = __dsub_rn(nm, c_sc[6]);
+        const double f = __dsub_rn(tq, nn);
+        const double z = f * f;
+        const double sr = f * __fma_rn(__fma_rn(c_sc[0], z, c_sc[1]), z, c_sc[2]);
+        const double cr = __fma_rn(__fma_rn(c_sc[3], z, c_sc[4]), z, c_sc[5]);
+        const double2 e = tl[(q & (kTab - 1)) * kRep];
+        // w e^{+i theta} = w (e.x + i e.y)(cr + i sr); the sign of the imaginary part is flipped at the store
+        const double wc = wj * cr, ws = wj * sr;
+        re[u] = __fma_rn(e.x, wc, re[u]);
+        re[u] = __fma_rn(-e.y, ws, re[u]);
+        im[u] = __fma_rn(e.y, wc, im[u]);
+        im[u] = __fma_rn(e.x, ws, im[u]);
       }
     }
     __syncthreads();  // everyone is done with this stage before it is refilled
@@ -174,19 +174,24 @@ __global__ void combine_splits_kernel(const double* __restrict__ part, int nspli
   out[i] = acc;
 }
 
-// Resident CTAs per SM of direct_sum_kernel<T> (registers bind: 6 / 10 / 16 with the current build); queried from
-// the runtime once, with those numbers as the fallback when there is no device (workspace queries on a CPU box).
+constexpr size_t kSmemBytes = 2 * sizeof(Stage) + sizeof(double2) * kTab * kRep + 16;   // stages, table, 2 mbarriers
+
+// Resident CTAs per SM of direct_sum_kernel<T> (shared memory binds: 4 with the current build); queried from the
+// runtime once, with that number as the fallback when there is no device (workspace queries on a CPU box).
 int ctas_per_sm(int T) {
   static int cache[5] = {0, 0, 0, 0, 0};
   if (cache[T] == 0) {
     int n = 0;
     cudaError_t e = cudaErrorUnknown;
-    if (T == 4) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<4>, kThreads, 0);
-    if (T == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<2>, kThreads, 0);
-    if (T == 1) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<1>, kThreads, 0);
+    cudaFuncSetAttribute(direct_sum_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    cudaFuncSetAttribute(direct_sum_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    cudaFuncSetAttribute(direct_sum_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (T == 4) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<4>, kThreads, kSmemBytes);
+    if (T == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<2>, kThreads, kSmemBytes);
+    if (T == 1) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<1>, kThreads, kSmemBytes);
     if (e != cudaSuccess || n <= 0) {
       cudaGetLastError();
-      return T == 4 ? 6 : (T == 2 ? 10 : 16);
+      return 4;
     }
     cache[T] = n;
   }
@@ -237,6 +242,17 @@ int direct_sum(const double* d_x, const double* d_w, int64_t J, const double* d_
     return SFD_OK;
   }
   const DirectPlan p = direct_plan(J, K);
+  {  // > 48 KB of dynamic shared memory needs the opt-in (per device; cheap to repeat)
+    static thread_local int attr_dev = -1;
+    int dev = 0;
+    SFD_CUDA_TRY(cudaGetDevice(&dev));
+    if (attr_dev != dev) {
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      attr_dev = dev;
+    }
+  }
   SFD_REQUIRE(work_bytes >= p.work_bytes && (p.work_bytes == 0 || d_work), SFD_ERR_WORKSPACE_TOO_SMALL,
               "direct sum needs %zu workspace bytes, got %zu", p.work_bytes, work_bytes);
   SFD_REQUIRE(p.blocks_k <= 0x7fffffffLL, SFD_ERR_INVALID_ARG, "K too large");
@@ -244,9 +260,9 @@ int direct_sum(const double* d_x, const double* d_w, int64_t J, const double* d_
   double* out = p.nsplit > 1 ? static_cast<double*>(d_work) : d_nuhat;
   dim3 grid((unsigned)p.blocks_k, (unsigned)p.nsplit);
   switch (p.T) {
-    case 4: direct_sum_kernel<4><<<grid, kThreads, 0, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
-    case 2: direct_sum_kernel<2><<<grid, kThreads, 0, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
-    default: direct_sum_kernel<1><<<grid, kThreads, 0, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
+    case 4: direct_sum_kernel<4><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
+    case 2: direct_sum_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
+    default: direct_sum_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
   }
   SFD_TRY(launch_check("direct_sum_kernel"));
   if (p.nsplit > 1) {

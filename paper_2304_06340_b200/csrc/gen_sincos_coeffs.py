@@ -121,9 +121,53 @@ def qturn():
     print("qturn: max |sin err| = %s, max |cos err| = %s" % (mp.nstr(es, 3), mp.nstr(ec, 3)))
 
 
+# ---------------------------------------------------------------------------------------------
+# Table form used by the direct sum's inner loop (csrc/direct.cu): the phase is reduced to |f| <= 1/2 in units of
+# 1/256 turn (a = 2 pi / 256), the table supplies the multiple of a, and the residual needs
+#     sin(a f) = f S(f^2),  cos(a f) = C(f^2)   with 3 coefficients each.
+# Run: python gen_sincos_coeffs.py table
+def table(ntab=256, ns=3, nc=3):
+    a = 2 * mp.pi / ntab
+    zmax = mp.mpf("0.2551")
+
+    def f_s(z):
+        return a if z == 0 else mp.sin(a * mp.sqrt(z)) / mp.sqrt(z)
+
+    def f_c(z):
+        return mp.cos(a * mp.sqrt(z))
+
+    def interp(f, n):
+        zs = [zmax / 2 * (1 + mp.cos(mp.pi * (2 * i + 1) / (2 * n))) for i in range(n)]
+        A = mp.matrix(n, n)
+        b = mp.matrix(n, 1)
+        for i, z in enumerate(zs):
+            for j in range(n):
+                A[i, j] = z ** j
+            b[i] = f(z)
+        return list(mp.lu_solve(A, b))
+
+    S, Cc = interp(f_s, ns), interp(f_c, nc)
+    print("// S%d..S0:" % (ns - 1), ", ".join(mp.nstr(c, 20) for c in S[::-1]))
+    print("// C%d..C0:" % (nc - 1), ", ".join(mp.nstr(c, 20) for c in Cc[::-1]))
+    print("// ntab / (2 pi) =", mp.nstr(ntab / (2 * mp.pi), 32))
+    f = np.linspace(-0.5, 0.5, 20001)
+    z = f * f
+    ps = np.full_like(f, float(S[-1]))
+    for k in range(ns - 2, -1, -1):
+        ps = ps * z + float(S[k])
+    pc = np.full_like(f, float(Cc[-1]))
+    for k in range(nc - 2, -1, -1):
+        pc = pc * z + float(Cc[k])
+    es = max(abs(mp.mpf(float(x)) - mp.sin(a * mp.mpf(float(y)))) for x, y in zip((f * ps)[::97], f[::97]))
+    ec = max(abs(mp.mpf(float(x)) - mp.cos(a * mp.mpf(float(y)))) for x, y in zip(pc[::97], f[::97]))
+    print("table %d: max |sin err| = %s, max |cos err| = %s" % (ntab, mp.nstr(es, 3), mp.nstr(ec, 3)))
+
+
 if __name__ == "__main__":
     import sys
-    if "qturn" in sys.argv:
+    if "table" in sys.argv:
+        table()
+    elif "qturn" in sys.argv:
         qturn()
     else:
         main()
