@@ -200,11 +200,17 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   const int n_pad = N - P.n_in;          // zero positions: [n_in - half_in, N - half_in)
   const int pad0 = P.n_in - half_in;
   if (CONTIG) {
+    // warp grid (column, segment): with fewer columns than warps every column is shared by nseg warps, each taking
+    // every nseg-th group of 32 elements, so all warps load whatever the tile height is
     const int lane = tid & 31, wrp = tid >> 5, nw = kFftThreads / 32;
-    for (int col = wrp; col < tb; col += nw) {
-      for (int j = lane; j < n_pad; j += 32) a[(pad0 + j) * tbp + col] = make_double2(0.0, 0.0);
+    const int nseg = nw >= tb ? nw / tb : 1;
+    const int cstep = nw >= tb ? tb : nw;            // columns advance by this per outer iteration
+    const int seg = nw >= tb ? wrp / tb : 0;
+    const int lstep = 32 * nseg;                     // element stride of one warp inside a row
+    for (int col = nw >= tb ? wrp % tb : wrp; col < tb && seg < nseg; col += cstep) {
+      for (int j = lane + 32 * seg; j < n_pad; j += lstep) a[(pad0 + j) * tbp + col] = make_double2(0.0, 0.0);
       if (col >= ncol) {
-        for (int i = lane; i < P.n_in; i += 32) {
+        for (int i = lane + 32 * seg; i < P.n_in; i += lstep) {
           const int l = i - half_in;
           a[(l < 0 ? l + N : l) * tbp + col] = make_double2(0.0, 0.0);
         }
@@ -217,11 +223,11 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         const double* src1 = src0 + (two ? P.in_lo : 0);
         const double f0 = P.dec_axis ? fhi * P.dec_lo[r0] : 1.0;
         const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
-        for (int i0 = lane; i0 < P.n_in; i0 += 128) {
+        for (int i0 = lane + 32 * seg; i0 < P.n_in; i0 += 4 * lstep) {
           double va[4], vb[4], fa[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int i = i0 + 32 * u;
+            const int i = i0 + lstep * u;
             const bool ok = i < P.n_in;
             va[u] = ok ? src0[i] : 0.0;
             vb[u] = ok ? src1[i] : 0.0;
@@ -229,7 +235,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int i = i0 + 32 * u;
+            const int i = i0 + lstep * u;
             if (i < P.n_in) {
               const int l = i - half_in;
               a[(l < 0 ? l + N : l) * tbp + col] = make_double2(va[u] * (fa[u] * f0), vb[u] * (fa[u] * f1));
@@ -239,19 +245,19 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
       } else {
         const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + col) * P.in_lo;
         const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + col] : 1.0;
-        for (int i0 = lane; i0 < P.n_in; i0 += 128) {
+        for (int i0 = lane + 32 * seg; i0 < P.n_in; i0 += 4 * lstep) {
           double2 v[4];
           double fa[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int i = i0 + 32 * u;
+            const int i = i0 + lstep * u;
             const bool ok = i < P.n_in;
             v[u] = ok ? src[i] : make_double2(0.0, 0.0);
             fa[u] = (ok && P.dec_axis) ? P.dec_axis[i] * f0 : 1.0;
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int i = i0 + 32 * u;
+            const int i = i0 + lstep * u;
             if (i < P.n_in) {
               const int l = i - half_in;
               a[(l < 0 ? l + N : l) * tbp + col] = make_double2(v[u].x * fa[u], v[u].y * fa[u]);
@@ -313,12 +319,16 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   // ---- store the band m in [lo, lo + nout) through the digit-reversal table
   if (CONTIG) {
     const int lane = tid & 31, wrp = tid >> 5, nw = kFftThreads / 32;
-    for (int col = wrp; col < ncol; col += nw) {
+    const int nseg = nw >= tb ? nw / tb : 1;
+    const int cstep = nw >= tb ? tb : nw;
+    const int seg = nw >= tb ? wrp / tb : 0;
+    const int lstep = 32 * nseg;
+    for (int col = nw >= tb ? wrp % tb : wrp; col < ncol && seg < nseg; col += cstep) {
       if (REAL_IN) {
         const bool two = 2 * col + 1 < nrow;
         double2* o0 = out + hi * P.out_hi + (lo0 + 2 * col) * P.out_lo;
         double2* o1 = o0 + P.out_lo;
-        for (int mm = lane; mm < P.nout; mm += 32) {
+        for (int mm = lane + 32 * seg; mm < P.nout; mm += lstep) {
           int m = P.lo + mm;
           m = m < 0 ? m + N : (m >= N ? m - N : m);
           const double2 z = a[P.rev[m] * tbp + col], zc = a[P.rev[m == 0 ? 0 : N - m] * tbp + col];
@@ -327,7 +337,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         }
       } else {
         double2* o0 = out + hi * P.out_hi + (lo0 + col) * P.out_lo;
-        for (int mm = lane; mm < P.nout; mm += 32) {
+        for (int mm = lane + 32 * seg; mm < P.nout; mm += lstep) {
           int m = P.lo + mm;
           m = m < 0 ? m + N : (m >= N ? m - N : m);
           o0[mm] = a[P.rev[m] * tbp + col];
