@@ -198,6 +198,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   const int half_in = P.n_in / 2;
   const double fhi = P.dec_hi ? P.dec_hi[hi] : 1.0;
   const int n_pad = N - P.n_in;          // zero positions: [n_in - half_in, N - half_in)
+  bool nz = false;                       // did this thread load anything non-zero?
   const int pad0 = P.n_in - half_in;
   if (CONTIG) {
     // warp grid (column, segment): with fewer columns than warps every column is shared by nseg warps, each taking
@@ -239,6 +240,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
             if (i < P.n_in) {
               const int l = i - half_in;
               a[(l < 0 ? l + N : l) * tbp + col] = make_double2(va[u] * (fa[u] * f0), vb[u] * (fa[u] * f1));
+              nz |= (va[u] != 0.0) | (vb[u] != 0.0);
             }
           }
         }
@@ -261,6 +263,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
             if (i < P.n_in) {
               const int l = i - half_in;
               a[(l < 0 ? l + N : l) * tbp + col] = make_double2(v[u].x * fa[u], v[u].y * fa[u]);
+              nz |= (v[u].x != 0.0) | (v[u].y != 0.0);
             }
           }
         }
@@ -286,15 +289,18 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         if (i < P.n_in) {
           const int l = i - half_in;
           a[(l < 0 ? l + N : l) * tbp + col] = v[u];
+          nz |= (v[u].x != 0.0) | (v[u].y != 0.0);
         }
       }
     }
   }
-  __syncthreads();
+  // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) and the
+  // outer planes of the second are entirely zero, and so is their transform: skip the stages, store zeros.
+  const bool all_zero = __syncthreads_or(nz) == 0;
 
   // ---- in-place decimation-in-frequency stages
   int L = N;
-  for (int s = 0; s < P.npair; ++s) {
+  for (int s = 0; s < (all_zero ? 0 : P.npair); ++s) {
     const int code = P.pair[s];
     const unsigned mg = P.magic[s];
 #define SFD_FFT_STAGE(R_) \
