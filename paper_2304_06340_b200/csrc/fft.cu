@@ -273,26 +273,21 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
     // strided passes (complex input, no deconvolution factors): in_lo = 1, rows in_el apart
     const int col = tid & (tb - 1), ty = tid >> tsh, nty = kFftThreads >> tsh;
     for (int j = ty; j < n_pad; j += nty) a[(pad0 + j) * tbp + col] = make_double2(0.0, 0.0);
+    // 16-byte asynchronous copies (LDGSTS) straight into the padded rows: every thread issues all of its elements
+    // back to back and waits once -- the pass is bound by memory latency, so what counts is bytes in flight
     const bool live = col < ncol;
-    const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + col + (int64_t)ty * P.in_el;
+    const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0) + (int64_t)ty * P.in_el;
     const int64_t step = (int64_t)nty * P.in_el;
-    for (int i0 = ty; i0 < P.n_in; i0 += 4 * nty) {
-      double2 v[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        v[u] = (live && i0 + u * nty < P.n_in) ? src[u * step] : make_double2(0.0, 0.0);
-      }
-      src += 4 * step;
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int i = i0 + u * nty;
-        if (i < P.n_in) {
-          const int l = i - half_in;
-          a[(l < 0 ? l + N : l) * tbp + col] = v[u];
-          nz |= (v[u].x != 0.0) | (v[u].y != 0.0);
-        }
-      }
+    for (int i = ty; i < P.n_in; i += nty) {
+      const int l = i - half_in;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(a + (l < 0 ? l + N : l) * tbp + col);
+      const int nbytes = live ? 16 : 0;   // src-size 0: zero-fill (columns beyond the edge of the array)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(nbytes) : "memory");
+      src += step;
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    nz = true;   // (no zero-tile detection in the strided passes)
   }
   // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) and the
   // outer planes of the second are entirely zero, and so is their transform: skip the stages, store zeros.
