@@ -250,3 +250,15 @@ def test_target_shards_add_up(sfd, orc, torch, eps, world):
         I_sum += I          # no process group: each call returns its own partial sum
     tol = 1e-12 if eps == 0.0 else 1e-7   # every shard's type-3 transform has its own grids (errors <= 10 eps sum|w|)
     assert abs(I_sum - I_full) <= tol * I_full
+
+
+@pytest.mark.parametrize("eps", [1e-1, 1e-2, 1e-4, 1e-5, 1e-7, 1e-8, 1e-10, 1e-11, 1e-13, 1e-14])
+def test_nufft_every_kernel_width(sfd, orc, torch, eps):
+    """Every instantiated kernel width (w = 2 ... 15; 1e-3/-6/-9/-12 are covered above): real-strength path (ball
+    quadrature, Hermitian half band) and complex path (off-centre cloud)."""
+    V, F = orc.mesh_icosphere(2)
+    x, w = orc.nodes(V, F, 6)
+    xi, W = orc.freq_nodes(12, 8, 10, 20.0)
+    _nufft_case(sfd, orc, torch, x, w, xi, eps)
+    x, w, xi = workloads.random_cloud(400, 300)
+    _nufft_case(sfd, orc, torch, x, w, xi, eps)
