@@ -58,8 +58,10 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
 
   // the lane's cells of a W x W plane: c = lane + 32 i -> (cy, cz)
   int cy[NCL], cz[NCL], off[NCL];
+  bool on[NCL];
 #pragma unroll
   for (int i = 0; i < NCL; ++i) {
+    on[i] = lane + 32 * i < W * W;
     const int c = min(lane + 32 * i, W * W - 1);
     cy[i] = c / W;
     cz[i] = c % W;
@@ -118,21 +120,36 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
       const double kx = lane < nch ? tab.k[0][lane][a] : 0.0;
       const double cre_l = r.re * kx;
       const double cim_l = REAL ? 0.0 : r.im * kx;
+      // sweep over the chunk's sources, software-pipelined: the broadcasts and the ky kz products of source s+1 are
+      // fetched while source s does its read-modify-write (the sweep is latency-bound otherwise)
+      int base_n = __shfl_sync(0xffffffffu, base_l, 0);
+      double cre_n = __shfl_sync(0xffffffffu, cre_l, 0);
+      double cim_n = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, 0);
+      double kyz_n[NCL];
+#pragma unroll
+      for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? tab.k[1][0][cy[i]] * tab.k[2][0][cz[i]] : 0.0;
       for (int s = 0; s < nch; ++s) {
-        const int base = __shfl_sync(0xffffffffu, base_l, s);
-        const double cre = __shfl_sync(0xffffffffu, cre_l, s);
-        const double cim = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, s);
+        const int base = base_n;
+        const double cre = cre_n, cim = cim_n;
+        double kyz[NCL];
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) kyz[i] = kyz_n[i];
+        const int sn = min(s + 1, nch - 1);
+        base_n = __shfl_sync(0xffffffffu, base_l, sn);
+        cre_n = __shfl_sync(0xffffffffu, cre_l, sn);
+        if (!REAL) cim_n = __shfl_sync(0xffffffffu, cim_l, sn);
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? tab.k[1][sn][cy[i]] * tab.k[2][sn][cz[i]] : 0.0;
 #pragma unroll
         for (int i = 0; i < NCL; ++i) {
-          if (32 * i + 31 < W * W || lane + 32 * i < W * W) {
-            const double kyz = tab.k[1][s][cy[i]] * tab.k[2][s][cz[i]];
+          if (on[i]) {
             const int idx = base + off[i];
             if (REAL) {
-              sub[idx] = __fma_rn(cre, kyz, sub[idx]);
+              sub[idx] = __fma_rn(cre, kyz[i], sub[idx]);
             } else {
               double2 v = reinterpret_cast<double2*>(sub)[idx];
-              v.x = __fma_rn(cre, kyz, v.x);
-              v.y = __fma_rn(cim, kyz, v.y);
+              v.x = __fma_rn(cre, kyz[i], v.x);
+              v.y = __fma_rn(cim, kyz[i], v.y);
               reinterpret_cast<double2*>(sub)[idx] = v;
             }
           }
