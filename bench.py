@@ -371,7 +371,10 @@ def main():
         dms = stages["direct"]["direct_sum"]
         ach = FLOPS_PER_PAIR * J * K / (dms * 1e-3) * 1e-12
         roofline = {"kernel": "direct_sum_kernel", "bound": "alu", "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s",
-                    "frac": ach / fp64_tf, "traffic": None,
+                    "frac": ach / fp64_tf,
+                    # DRAM bytes per launch from the ncu --set full capture of this kernel on this workload
+                    # (profiles/r1e_direct_sum_table.md: 26.2 MB read + 0.54 MB written; config 2 only)
+                    "traffic": 26743808 if args.config == 2 else None,
                     "peak_source": "measured live by sfd_probe_fp64 (dependency-free DFMA loop on all SMs)",
                     "peak_derived": 2 * FP64_LANES_PER_SM * 148 * sm_mhz * 1e6 * 1e-12,
                     "pipe_frac": (DFMA_PER_PAIR + DMUL_DADD_PER_PAIR) * J * K / (dms * 1e-3) /
