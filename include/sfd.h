@@ -38,7 +38,7 @@ typedef enum {
   SFD_ERR_BUFFER_TOO_SMALL = -3,
   SFD_ERR_WORKSPACE_TOO_SMALL = -4,
   SFD_ERR_CUDA = -5,
-  SFD_ERR_CUFFT = -6,
+  SFD_ERR_CUFFT = -6, /* kept for ABI stability: unused since the inner FFT is the library's own (fft.cu) */
   SFD_ERR_UNSUPPORTED = -7
 } sfd_status;
 
@@ -181,7 +181,7 @@ int sfd_weak_distance_host(const double* h_vertices, int64_t nV, const int32_t* 
 int sfd_set_profiling(int on);
 int sfd_last_stage_times(const char** names, float* ms, int max);
 
-/* Number of kernels of this library launched so far by the process (cuFFT's own kernels are not counted). */
+/* Number of kernels of this library launched so far by the process. */
 long long sfd_launch_count(void);
 
 /* ---- roofline denominator of A4 ------------------------------------------------------------------

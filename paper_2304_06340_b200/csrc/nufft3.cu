@@ -34,7 +34,7 @@ constexpr int kTgtCap = 512;    // targets per interp work item
 // [1024, ...) scratch of the bounds reduction
 constexpr size_t kMiscBytes = 32768;
 
-// smallest even n' >= n of the form 2^a 3^b 5^c (sizes cuFFT handles with its fastest radices)
+// smallest even n' >= n of the form 2^a 3^b 5^c (the radices of fft.cu: 4, 2, 3, 5)
 int64_t next_smooth_even(int64_t n) {
   if (n < 2) n = 2;
   if (n & 1) ++n;
