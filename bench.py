@@ -407,8 +407,18 @@ def main():
                 e.update({"binding_roof": "shared memory", "smem_achieved_gbs": sm_ach, "smem_peak_gbs": smem_peak,
                           "smem_frac": sm_ach / smem_peak})
             extra.append(e)
+        # the one-pass HBM-bound stages around the transform (A3, frequency nodes, A5-9, A6), algorithmic bytes per unit
+        for name, kern, nbytes in (("nodes", "nodes_kernel", 32 * J + 12 * (J // c["rule"])),
+                                   ("freq_nodes", "freq_expand_kernel", 32 * K),
+                                   ("post", "post_deconv_kernel", (24 + 32) * K),
+                                   ("reduce", "reduce_terms_kernel", 48 * K)):
+            if name in st and st[name] > 0:
+                ach = nbytes / (st[name] * 1e-3) * 1e-9
+                extra.append({"kernel": kern, "eps": eps, "bound": "hbm", "achieved": ach, "peak": hbm_peak,
+                              "unit": "GB/s", "frac": ach / hbm_peak, "ms_per_launch": st[name],
+                              "algorithmic_bytes": nbytes, "peak_source": hbm_src})
         if roofline is None:
-            roofline = dict(max(extra, key=lambda e: e["ms_per_launch"]), traffic=None)
+            roofline = dict(max(extra[-7:], key=lambda e: e["ms_per_launch"]), traffic=None)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
