@@ -149,9 +149,20 @@ int sfd_lattice_nodes_device(int32_t M, double xi_max, double* d_xi /*[K][3]*/, 
  * lattice nodes xi' = 2 pi xi is xi_scale = 1/(2 pi), s = -s_paper, prefactor = 1.  s > 0.5.  Synchronises. */
 int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, double xi_scale,
                   double prefactor, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+/* nuhat on the lattice of sfd_lattice_nodes (same node order) -- the transform the paper itself runs (eq. 3.6:
+ * type-1 NUFFT, nonuniform sources -> integer modes, after the rescaling x -> h x of P:188 eq. 3.7).  eps > 0: type-1
+ * NUFFT (sort, spread, pruned FFT whose output band IS the lattice, deconvolution; no interpolation step); when the
+ * lattice is too coarse for the sources' extent (2 pi h max|x - centre| close to pi: the periodic images would
+ * overlap) or eps == 0, the lattice nodes are expanded in the workspace and the call runs sfd_surface_ft on them
+ * (type-3 / direct sum).  X[3] in the workspace query: upper bounds of the half-extents of the sources per axis.
+ * Device pointers; d_nuhat complex128 [K = (M+1)^3]; enqueues on `stream` after one synchronisation (the extents).
+ * Errors as sfd_surface_ft. */
+int sfd_surface_ft_lattice_workspace(int64_t J, int32_t M, double xi_max, const double X[3], double eps, size_t* bytes);
+int sfd_surface_ft_lattice(const double* d_x, const double* d_w, int64_t J, int32_t M, double xi_max, double eps,
+                           double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream);
 /* ||mu - sigma||_{H_s(R^3)} of P:65 eq. 2.7 for the mesh's surface measure mu against the unit sphere's, by the
- * paper's quadrature: atoms (rule 64 = the paper's) -> transform on the lattice (eps == 0: direct sum; eps > 0:
- * type-3 NUFFT, which takes lattice targets like any others) -> trapezoidal rule.  s_paper < -1/2.
+ * paper's quadrature: atoms (rule 64 = the paper's) -> transform on the lattice (sfd_surface_ft_lattice: eps == 0
+ * direct sum, eps > 0 type-1 NUFFT) -> trapezoidal rule.  s_paper < -1/2.
  * Writes the norm to *h_norm and its square to *h_I.  Synchronises. */
 int sfd_weak_distance_lattice_workspace(int64_t nF, int rule, int32_t M, double xi_max, double eps, double x_extent,
                                         size_t* bytes);

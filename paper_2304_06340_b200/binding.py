@@ -58,6 +58,8 @@ _SIGS = {
     "sfd_lattice_nodes": (C.c_int, [C.c_int32, _dbl, _vp, _vp]),
     "sfd_lattice_nodes_device": (C.c_int, [C.c_int32, _dbl, _vp, _vp, _vp]),
     "sfd_reduce_ex": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _dbl, _vp, _sz, _vp, _P(_dbl)]),
+    "sfd_surface_ft_lattice_workspace": (C.c_int, [_i64, C.c_int32, _dbl, _P(_dbl), _dbl, _P(_sz)]),
+    "sfd_surface_ft_lattice": (C.c_int, [_vp, _vp, _i64, C.c_int32, _dbl, _dbl, _vp, _vp, _sz, _vp]),
     "sfd_weak_distance_lattice_workspace": (C.c_int, [_i64, C.c_int, C.c_int32, _dbl, _dbl, _dbl, _P(_sz)]),
     "sfd_weak_distance_lattice": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, C.c_int32, _dbl, _vp, _sz, _vp,
                                             _P(_dbl), _P(_dbl)]),
@@ -333,6 +335,28 @@ def sfd_reduce_ex(nuhat, xi, W, s, xi_scale, prefactor):
     _chk(_lib.sfd_reduce_ex(_ptr(nu), _ptr(xi), _ptr(W), K, float(s), float(xi_scale), float(prefactor), _ptr(work),
                             work.numel(), _stream(), C.byref(I)))
     return I.value
+
+
+def sfd_surface_ft_lattice_workspace(J, M, xi_max, X, eps):
+    wb = _sz()
+    Xa = (_dbl * 3)(*[float(v) for v in X])
+    _chk(_lib.sfd_surface_ft_lattice_workspace(int(J), int(M), float(xi_max), Xa, float(eps), C.byref(wb)))
+    return wb.value
+
+
+def sfd_surface_ft_lattice(x, w, M, xi_max, eps, work=None):
+    """nuhat on the lattice of sfd_lattice_nodes (same order): complex128[(M+1)^3].  eps > 0: the paper's type-1
+    NUFFT (eq. 3.6); eps = 0 (or a lattice too coarse for the sources): sfd_surface_ft on the expanded nodes."""
+    _dev_f64(x, 3), _dev_f64(w)
+    J = x.shape[0]
+    assert w.shape[0] == J
+    if work is None:
+        work = _work(sfd_surface_ft_lattice_workspace(J, M, xi_max, _half_widths(x), eps), x.device)
+    K = (int(M) + 1) ** 3
+    nu = torch.empty((K, 2), dtype=torch.float64, device=x.device)
+    _chk(_lib.sfd_surface_ft_lattice(_ptr(x), _ptr(w), J, int(M), float(xi_max), float(eps), _ptr(nu), _ptr(work),
+                                     work.numel(), _stream()))
+    return torch.view_as_complex(nu)
 
 
 def sfd_weak_distance_lattice_workspace(nF, rule, M, xi_max, eps, x_extent=1.0):

@@ -399,6 +399,86 @@ int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, 
 }
 
 namespace {
+int check_lattice(int M, double xi_max) {
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 2046, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..2046 (got %d)", M);
+  SFD_REQUIRE(xi_max > 0.0 && std::isfinite(xi_max), SFD_ERR_INVALID_ARG, "xi_max must be positive and finite");
+  return SFD_OK;
+}
+
+// Workspace of the transform on the lattice when the expanded nodes are supplied by the caller.
+int lattice_ft_bytes(int64_t J, int M, double xi_max, const double X[3], double eps, size_t* bytes) {
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  const double Sx = 6.283185307179586476925286766559 * xi_max;
+  const double S[3] = {Sx, Sx, Sx};
+  size_t t3 = 0, t1 = 0;
+  bool ok = false;
+  if (eps > 0.0 && J > 0) SFD_TRY(nufft1_lattice_sizes(J, M, 2.0 * xi_max / M, X, eps, &ok, &t1));
+  if (ok) {
+    *bytes = t1;
+    return SFD_OK;
+  }
+  SFD_TRY(sfd_surface_ft_workspace(J, K, X, S, eps, &t3));
+  *bytes = t3;
+  return SFD_OK;
+}
+
+// nuhat on the lattice; d_xi = the expanded nodes (lattice_expand), used only by the type-3 / direct path.
+int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi_max, double eps, const double* d_xi,
+               double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  if (eps > 0.0 && J > 0) {
+    cudaStream_t st = as_stream(stream);
+    const bool own_prof = !g_prof.active;
+    if (own_prof) prof_begin(st);
+    bool ok = false;
+    const int rc = nufft1_lattice(d_x, d_w, J, M, 2.0 * xi_max / M, eps, d_nuhat, d_work, work_bytes, st, &ok);
+    if (own_prof) prof_end(st);
+    if (rc != SFD_OK || ok) return rc;
+  }
+  return sfd_surface_ft(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, stream);
+}
+}  // namespace
+
+int sfd_surface_ft_lattice_workspace(int64_t J, int32_t M, double xi_max, const double X[3], double eps, size_t* bytes) {
+  SFD_REQUIRE(bytes && X, SFD_ERR_NULL, "sfd_surface_ft_lattice_workspace: NULL argument");
+  SFD_REQUIRE(J >= 0, SFD_ERR_INVALID_ARG, "J must be >= 0");
+  SFD_TRY(check_lattice(M, xi_max));
+  SFD_TRY(check_eps(eps));
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  size_t b = 0;
+  SFD_TRY(lattice_ft_bytes(J, M, xi_max, X, eps, &b));
+  *bytes = align_up((size_t)K * 24) + b;   // room for the expanded nodes of the fallback
+  return SFD_OK;
+}
+
+int sfd_surface_ft_lattice(const double* d_x, const double* d_w, int64_t J, int32_t M, double xi_max, double eps,
+                           double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+  SFD_REQUIRE(J >= 0, SFD_ERR_INVALID_ARG, "J must be >= 0");
+  SFD_TRY(check_lattice(M, xi_max));
+  SFD_TRY(check_eps(eps));
+  SFD_REQUIRE(d_nuhat, SFD_ERR_NULL, "sfd_surface_ft_lattice: NULL output");
+  SFD_REQUIRE(J == 0 || (d_x && d_w), SFD_ERR_NULL, "sfd_surface_ft_lattice: NULL source buffer");
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  const size_t xi_bytes = align_up((size_t)K * 24);
+  SFD_REQUIRE(d_work && work_bytes >= xi_bytes, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "sfd_surface_ft_lattice needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
+  cudaStream_t st = as_stream(stream);
+  char* base = static_cast<char*>(d_work);
+  if (eps > 0.0 && J > 0) {
+    const bool own_prof = !g_prof.active;
+    if (own_prof) prof_begin(st);
+    bool ok = false;
+    const int rc = nufft1_lattice(d_x, d_w, J, M, 2.0 * xi_max / M, eps, d_nuhat, base + xi_bytes, work_bytes - xi_bytes,
+                                  st, &ok);
+    if (own_prof) prof_end(st);
+    if (rc != SFD_OK || ok) return rc;
+  }
+  double* xi = reinterpret_cast<double*>(base);
+  SFD_TRY(lattice_expand(M, xi_max, xi, nullptr, st));
+  return sfd_surface_ft(d_x, d_w, J, xi, K, eps, d_nuhat, base + xi_bytes, work_bytes - xi_bytes, stream);
+}
+
+namespace {
 int lattice_layout(int64_t nF, int rule, int M, double xi_max, double eps, double x_extent, DistLayout* L) {
   SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
   SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
@@ -407,10 +487,9 @@ int lattice_layout(int64_t nF, int rule, int M, double xi_max, double eps, doubl
   SFD_TRY(check_eps(eps));
   L->J = nF * rule;
   L->K = (int64_t)(M + 1) * (M + 1) * (M + 1);
-  const double Sx = 6.283185307179586476925286766559 * xi_max;
-  const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {Sx, Sx, Sx};
+  const double X[3] = {x_extent, x_extent, x_extent};
   if (eps > 0.0) SFD_REQUIRE(x_extent > 0.0 && std::isfinite(x_extent), SFD_ERR_INVALID_ARG, "x_extent must be > 0");
-  SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, eps, &L->ft_bytes));
+  SFD_TRY(lattice_ft_bytes(L->J, M, xi_max, X, eps, &L->ft_bytes));
   L->tab_bytes = 0;
   L->red_bytes = reduce_workspace(L->K);
   size_t o = 0;
@@ -464,7 +543,7 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   prof_mark("nodes", st);
   if (rc == SFD_OK) rc = lattice_expand(M, xi_max, xi, W, st);
   prof_mark("freq_nodes", st);
-  if (rc == SFD_OK) rc = sfd_surface_ft(x, w, L.J, xi, L.K, eps, nu, base + L.ft, work_bytes - L.ft, stream);
+  if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream);
   double* d_res = nullptr;
   // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
   if (rc == SFD_OK)

@@ -133,7 +133,7 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->toff = put((size_t)(L->nt_bins + 1) * 4);
   L->tcur = put((size_t)(L->nt_bins + 1) * 4);
   L->titems = put((size_t)L->nt_items * 4 * 3);
-  L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2]) * 8);
+  L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2] + p.nout[0] + p.nout[1] + p.nout[2]) * 8);
   L->scan = put(scan_workspace(std::max(L->ns_bins, L->nt_bins) + 1));
   L->ffttab = put(fft_tables_bytes(p.n2));
   L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16);
@@ -222,6 +222,28 @@ void make_poly(const N3Params& p, double* tab) {
   }
 }
 
+// host-side tables are pure functions of (w, beta): computed once per width (long-double work, ~ms), then reused
+void width_tables(const N3Params& p, ChebTable* quad, double* h_ptab) {
+  struct WidthTables {
+    bool ready = false;
+    double beta = 0.0;
+    ChebTable cheb;
+    double poly[(kMaxDeg + 1) * kPolyStride];
+  };
+  static WidthTables wt_cache[kMaxW + 1];
+  static std::mutex wt_mu;
+  std::lock_guard<std::mutex> lk(wt_mu);
+  WidthTables& wt = wt_cache[p.w];
+  if (!wt.ready || wt.beta != p.beta) {
+    make_cheb(p, &wt.cheb);
+    make_poly(p, wt.poly);
+    wt.beta = p.beta;
+    wt.ready = true;
+  }
+  *quad = wt.cheb;
+  std::memcpy(h_ptab, wt.poly, sizeof(wt.poly));
+}
+
 }  // namespace
 
 int nufft3_release_cache() { return SFD_OK; }   // nothing is cached on the device any more
@@ -302,29 +324,9 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
               "type-3 NUFFT (w=%d, fine grid %dx%dx%d) needs %zu workspace bytes, got %zu", p.w, p.nf[0], p.nf[1], p.nf[2],
               L.total, work_bytes);
-  // host-side tables are pure functions of (w, beta): computed once per width (long-double work, ~ms), then reused
-  struct WidthTables {
-    bool ready = false;
-    double beta = 0.0;
-    ChebTable cheb;
-    double poly[(kMaxDeg + 1) * kPolyStride];
-  };
-  static WidthTables wt_cache[kMaxW + 1];
-  static std::mutex wt_mu;
   ChebTable quad;
   double h_ptab[(kMaxDeg + 1) * kPolyStride];
-  {
-    std::lock_guard<std::mutex> lk(wt_mu);
-    WidthTables& wt = wt_cache[p.w];
-    if (!wt.ready || wt.beta != p.beta) {
-      make_cheb(p, &wt.cheb);
-      make_poly(p, wt.poly);
-      wt.beta = p.beta;
-      wt.ready = true;
-    }
-    quad = wt.cheb;
-    std::memcpy(h_ptab, wt.poly, sizeof(h_ptab));
-  }
+  width_tables(p, &quad, h_ptab);
   double* ptab = reinterpret_cast<double*>(base + L.ptab);
   SFD_CUDA_TRY(cudaMemcpyAsync(ptab, h_ptab, sizeof(h_ptab), cudaMemcpyHostToDevice, st));
   SrcRec* src = reinterpret_cast<SrcRec*>(base + L.src);
@@ -408,6 +410,174 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   SFD_TRY(interp(p, ptab, bufx, tgt, titems, titems + L.nt_items, titems + 2 * L.nt_items, d_ctl + 1, d_ctl + 3, d_nuhat, st));
   prof_mark("interp", st);
   SFD_TRY(post_deconv(p, quad, d_xi, K, d_nuhat, st));
+  prof_mark("post", st);
+  return SFD_OK;
+}
+
+}  // namespace sfd
+
+// ================================================================================================================
+// Type-1 NUFFT on the paper's lattice (eq. 3.6, eq. 3.7): nuhat(xi_m) = sum_j w_j e^{-i xi_m . x_j} at
+// xi_m = 2 pi h m, m in [-M/2, M/2]^3 (nodes.cu lattice_kernel).  With x' = 2 pi h (x - C) in [-pi, pi) -- the
+// rescaling x -> h x of eq. 3.7 -- the sum is a Fourier series on integer modes: spread onto a grid of N >= 2(M+1)
+// points per period, FFT, keep the band |m| <= M/2, divide by the kernel's transform.  Everything is shared with the
+// type-3 transform: the same sort, spread.cu and fft.cu with other geometry (the spread grid is only the n_in^3
+// cells around the origin that the rescaled sources reach, the "highly clustered" case of P:236; the FFT is pruned
+// to those inputs and to the band; real strengths keep the half m_2 >= 0).  No interpolation step.
+namespace sfd {
+namespace {
+
+// *ok = false: the lattice is too coarse for the extent of the sources (2 pi h X >= pi up to the kernel's
+// footprint: the periodic images would overlap) or the transform is too long for fft.cu -- use the type-3 path.
+int make_params_lattice(const double X_in[3], const double C[3], int M, double h, double eps, N3Params* p, bool* ok) {
+  kernel_params(eps, &p->w, &p->beta);
+  p->real_c = 1;
+  p->zh = 1;
+  p->deg = p->w + 3;
+  *ok = false;
+  const double hx = 2.0 * kPi * h;   // lattice step in the e^{-i xi.x} convention
+  const int64_t N = next_smooth_even((int64_t)std::ceil(kSigma * (M + 1)));
+  int tbp = 0;
+  if (!fft_length_ok((int)N) || fft_tile((int)N, 0, &tbp) == 0 || fft_tile((int)N, 1, &tbp) == 0) return SFD_OK;
+  for (int d = 0; d < 3; ++d) {
+    SFD_REQUIRE(std::isfinite(X_in[d]) && X_in[d] >= 0, SFD_ERR_INVALID_ARG, "type-1 NUFFT: extents must be finite and >= 0");
+    p->n2[d] = (int)N;
+    p->sx[d] = hx * (double)N / (2.0 * kPi);
+    const int64_t nin = 2 * (int64_t)std::ceil(X_in[d] * p->sx[d] + 0.5 * (p->w + 1)) + 2;
+    if (nin > N) return SFD_OK;
+    p->nf[d] = (int)nin;
+    p->C[d] = C[d];
+    p->D[d] = 0.0;
+    p->st[d] = 0.0;
+    p->kap[d] = p->w * kPi / ((double)N * hx);
+    p->lo[d] = -(M / 2);
+    p->nout[d] = M + 1;
+    p->bt[d] = 1;
+    p->nbt[d] = 1;
+    p->t0[d] = 0;
+  }
+  p->lo[2] = 0;
+  p->nout[2] = M / 2 + 1;
+  spread_bins(p->w, true, p->bs);
+  for (int d = 0; d < 3; ++d) p->nbs[d] = (p->nf[d] + p->bs[d] - 1) / p->bs[d];
+  *ok = true;
+  return SFD_OK;
+}
+
+}  // namespace
+
+int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double eps, bool* applicable, size_t* bytes) {
+  SFD_REQUIRE(X && applicable && bytes, SFD_ERR_NULL, "nufft1_lattice_sizes: NULL argument");
+  double Xi[3];
+  const double C0[3] = {0.0, 0.0, 0.0};
+  for (int d = 0; d < 3; ++d) Xi[d] = X[d] * (1.0 + 1e-6);
+  N3Params p{};
+  SFD_TRY(make_params_lattice(Xi, C0, M, h, eps, &p, applicable));
+  *bytes = 0;
+  if (!*applicable) return SFD_OK;
+  Layout L;
+  SFD_TRY(make_layout(p, J, 0, &L));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
+                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable) {
+  SFD_REQUIRE(J > 0 && applicable, SFD_ERR_INVALID_ARG, "nufft1_lattice: J must be > 0");
+  SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "type-1 NUFFT needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
+  char* base = static_cast<char*>(d_work);
+  double* d_bounds = reinterpret_cast<double*>(base);
+  int32_t* d_ctl = reinterpret_cast<int32_t*>(base + 128);
+  double* d_scratch = reinterpret_cast<double*>(base + 1024);
+
+  SFD_TRY(bounds_minmax(d_x, J, d_bounds, d_scratch, st));
+  double hb[6];
+  SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, sizeof(hb), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  prof_mark("bounds", st);
+  double X[3], C[3];
+  for (int d = 0; d < 3; ++d) {
+    SFD_REQUIRE(std::isfinite(hb[d]) && std::isfinite(hb[3 + d]), SFD_ERR_INVALID_ARG,
+                "type-1 NUFFT: non-finite source coordinate");
+    C[d] = 0.5 * (hb[d] + hb[3 + d]);
+    X[d] = (0.5 * (hb[3 + d] - hb[d])) * (1.0 + 1e-12) + 1e-300;
+    // sources centred at the origin up to rounding (a closed surface around it): snap C to 0, no post-phase
+    const double reach = std::fmax(std::fabs(hb[d]), std::fabs(hb[3 + d]));
+    if (std::fabs(C[d]) <= 1e-9 * reach) {
+      C[d] = 0.0;
+      X[d] = reach * (1.0 + 1e-12) + 1e-300;
+    }
+  }
+  N3Params p{};
+  SFD_TRY(make_params_lattice(X, C, M, h, eps, &p, applicable));
+  if (!*applicable) return SFD_OK;
+  Layout L;
+  SFD_TRY(make_layout(p, J, 0, &L));
+  SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
+              "type-1 NUFFT (w=%d, spread grid %dx%dx%d, FFT length %d) needs %zu workspace bytes, got %zu", p.w, p.nf[0],
+              p.nf[1], p.nf[2], p.n2[0], L.total, work_bytes);
+  ChebTable quad;
+  double h_ptab[(kMaxDeg + 1) * kPolyStride];
+  width_tables(p, &quad, h_ptab);
+  double* ptab = reinterpret_cast<double*>(base + L.ptab);
+  SFD_CUDA_TRY(cudaMemcpyAsync(ptab, h_ptab, sizeof(h_ptab), cudaMemcpyHostToDevice, st));
+  SrcRec* src = reinterpret_cast<SrcRec*>(base + L.src);
+  int32_t* skey = reinterpret_cast<int32_t*>(base + L.skey);
+  int32_t* shist = reinterpret_cast<int32_t*>(base + L.shist);
+  int32_t* soff = reinterpret_cast<int32_t*>(base + L.soff);
+  int32_t* scur = reinterpret_cast<int32_t*>(base + L.scur);
+  int32_t* sitems = reinterpret_cast<int32_t*>(base + L.sitems);
+  double* dec = reinterpret_cast<double*>(base + L.dec);
+  double* fine = reinterpret_cast<double*>(base + L.fine);
+  double* bufx = reinterpret_cast<double*>(base + L.bufx);
+  double* bufy = reinterpret_cast<double*>(base + L.bufy);
+  void* scan_w = base + L.scan;
+  const size_t scan_b = L.ffttab - L.scan;
+
+  // rescale (eq. 3.7) and bin-sort the sources, as in the type-3 transform
+  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
+  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_bins, nullptr, scan_w, scan_b, st));
+  SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
+  const int src_cap = (int)std::max<int64_t>(kSrcCap, J / ((int64_t)num_sms() * 8));
+  SFD_TRY(make_items(shist, soff, L.ns_bins, src_cap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
+  prof_mark("src_sort", st);
+
+  SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, L.fine_bytes, st));
+  SFD_TRY(spread(p, ptab, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
+  prof_mark("spread", st);
+
+  // three pruned FFT passes: position l = i - n_in/2 <-> x' = 2 pi l / N, output = the lattice modes
+  SFD_TRY(lattice_tables(p, quad, M, dec, st));
+  FftTables ft;
+  SFD_TRY(fft_upload_tables(p.n2, base + L.ffttab, &ft, st));
+  {
+    const int64_t nf0 = p.nf[0], nf1 = p.nf[1], nf2 = p.nf[2], no1 = p.nout[1], no2 = p.nout[2];
+    FftPass A{};
+    A.N = p.n2[2]; A.n_in = p.nf[2]; A.lo = p.lo[2]; A.nout = p.nout[2];
+    A.n_hi = nf0; A.n_lo = nf1;
+    A.in_hi = nf1 * nf2; A.in_lo = nf2; A.in_el = 1;
+    A.out_hi = nf1 * no2; A.out_lo = no2; A.out_el = 1;
+    A.contig = 1; A.real_in = 1;
+    SFD_TRY(fft_pass(A, ft, 2, fine, bufx, st));
+    FftPass B{};
+    B.N = p.n2[1]; B.n_in = p.nf[1]; B.lo = p.lo[1]; B.nout = p.nout[1];
+    B.n_hi = nf0; B.n_lo = no2;
+    B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
+    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
+    FftPass C3{};
+    C3.N = p.n2[0]; C3.n_in = p.nf[0]; C3.lo = p.lo[0]; C3.nout = p.nout[0];
+    C3.n_hi = 1; C3.n_lo = no1 * no2;
+    C3.in_hi = 0; C3.in_lo = 1; C3.in_el = no1 * no2;
+    C3.out_hi = 0; C3.out_lo = 1; C3.out_el = no1 * no2;
+    SFD_TRY(fft_pass(C3, ft, 0, bufy, bufx, st));
+  }
+  prof_mark("fft", st);
+
+  SFD_TRY(lattice_post(p, M, h, dec, bufx, d_nuhat, st));
   prof_mark("post", st);
   return SFD_OK;
 }

@@ -114,5 +114,11 @@ int make_items(const int32_t* d_hist, const int32_t* d_off, int64_t nbins, int c
 int deconv_tables(const N3Params& p, const ChebTable& q, double* d_dec, cudaStream_t st);
 // A5-9: nuhat_k = G_k e^{-i (xi_k-D).C} / prod_d (w/2) phihat((xi_kd-D_d) kap_d), in place on d_nuhat.
 int post_deconv(const N3Params& p, const ChebTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st);
+// Type-1 tail (eq. 3.6): dec[d][m] = 1 / ((w/2) phihat(m w pi / n2_d)), m in [0, M/2]; then the FFT band
+// v[M+1][M+1][M/2+1] (modes m0, m1, m2 >= 0) is unfolded by Hermitian symmetry into lattice order (nodes.cu
+// lattice_kernel), deconvolved and multiplied by e^{-i xi.C}.
+int lattice_tables(const N3Params& p, const ChebTable& q, int M, double* d_dec, cudaStream_t st);
+int lattice_post(const N3Params& p, int M, double h, const double* d_dec, const double* d_v, double* d_nuhat,
+                 cudaStream_t st);
 
 }  // namespace sfd

@@ -222,6 +222,47 @@ __global__ void __launch_bounds__(kT) post_deconv_kernel(N3Params p, ChebTable q
   nuhat[k] = make_double2((g.x * c + g.y * s) * inv, (g.y * c - g.x * s) * inv);
 }
 
+// ---- type-1 tail (eq. 3.6): lattice modes out of the FFT band ---------------------------------------------
+// dec[d * (M/2+1) + m] = 1 / ((w/2) phihat(m w pi / N_d)), m = |mode| (phihat is even)
+__global__ void __launch_bounds__(kT) lattice_tables_kernel(N3Params p, ChebTable q, int M, double* __restrict__ dec) {
+  const int i = blockIdx.x * kT + threadIdx.x;
+  const int nh = M / 2 + 1;
+  if (i >= 3 * nh) return;
+  const int d = i / nh, m = i - d * nh;
+  dec[i] = 1.0 / half_w_phihat(q, (double)m * p.w * 3.14159265358979323846 / (double)p.n2[d]);
+}
+
+// v = complex[M+1][M+1][M/2+1], modes (m0, m1, m2 >= 0); the other half by v(-m) = conj v(m) (real strengths).
+// nuhat[k], k = ((a (M+1)) + b)(M+1) + c as in lattice_kernel (nodes.cu), m = (a, b, c) - M/2:
+//   nuhat = v(m) e^{-i xi.C} prod_d dec_d[|m_d|],  xi_d = 2 pi (m_d h)
+__global__ void __launch_bounds__(kT) lattice_post_kernel(N3Params p, int M, double h, const double* __restrict__ dec,
+                                                         const double2* __restrict__ v, double2* __restrict__ nuhat) {
+  const int n = M + 1, nh = M / 2 + 1;
+  const int64_t K = (int64_t)n * n * n;
+  const int64_t k = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (k >= K) return;
+  const int c = (int)(k % n);
+  const int64_t ab = k / n;
+  const int b = (int)(ab % n), a = (int)(ab / n);
+  const int m0 = a - M / 2, m1 = b - M / 2, m2 = c - M / 2;
+  const bool refl = m2 < 0;
+  const int ia = refl ? M - a : a, ib = refl ? M - b : b, ic = refl ? -m2 : m2;
+  double2 g = v[((int64_t)ia * n + ib) * nh + ic];
+  if (refl) g.y = -g.y;
+  const double f = dec[abs(m0)] * dec[nh + abs(m1)] * dec[2 * nh + ic];
+  g.x *= f;
+  g.y *= f;
+  if (p.C[0] != 0.0 || p.C[1] != 0.0 || p.C[2] != 0.0) {
+    const double two_pi = 6.283185307179586476925286766559;
+    const double x0 = __dmul_rn(two_pi, __dmul_rn((double)m0, h)), x1 = __dmul_rn(two_pi, __dmul_rn((double)m1, h)),
+                 x2 = __dmul_rn(two_pi, __dmul_rn((double)m2, h));
+    double sn, cs;
+    sincos_fp64(__fma_rn(x0, p.C[0], __fma_rn(x1, p.C[1], x2 * p.C[2])), sn, cs);
+    g = make_double2(g.x * cs + g.y * sn, g.y * cs - g.x * sn);
+  }
+  nuhat[k] = g;
+}
+
 }  // namespace
 
 static inline unsigned blocks_for(int64_t n) { return (unsigned)((n + kT - 1) / kT); }
@@ -271,6 +312,19 @@ int deconv_tables(const N3Params& p, const ChebTable& q, double* d_dec, cudaStre
 int post_deconv(const N3Params& p, const ChebTable& q, const double* d_xi, int64_t K, double* d_nuhat, cudaStream_t st) {
   post_deconv_kernel<<<blocks_for(K), kT, 0, st>>>(p, q, d_xi, K, reinterpret_cast<double2*>(d_nuhat));
   return launch_check("post_deconv_kernel");
+}
+
+int lattice_tables(const N3Params& p, const ChebTable& q, int M, double* d_dec, cudaStream_t st) {
+  lattice_tables_kernel<<<blocks_for(3 * (M / 2 + 1)), kT, 0, st>>>(p, q, M, d_dec);
+  return launch_check("lattice_tables_kernel");
+}
+
+int lattice_post(const N3Params& p, int M, double h, const double* d_dec, const double* d_v, double* d_nuhat,
+                 cudaStream_t st) {
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  lattice_post_kernel<<<blocks_for(K), kT, 0, st>>>(p, M, h, d_dec, reinterpret_cast<const double2*>(d_v),
+                                                    reinterpret_cast<double2*>(d_nuhat));
+  return launch_check("lattice_post_kernel");
 }
 
 }  // namespace sfd

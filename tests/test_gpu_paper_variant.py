@@ -58,6 +58,60 @@ def test_reduce_ex(sfd, orc, torch):
         assert abs(got - ref) <= 1e-12 * ref
 
 
+def _cloud(rng, J, centre, half):
+    x = (rng.random((J, 3)) * 2 - 1) * np.asarray(half) + np.asarray(centre)
+    w = rng.normal(size=J)
+    return x, w
+
+
+@pytest.mark.parametrize("M,xi_max,centre,half,eps", [
+    (16, 2.0, (0, 0, 0), (1, 1, 1), 1e-9),          # M/2 even
+    (18, 1.5, (0, 0, 0), (1, 0.7, 0.4), 1e-6),      # M/2 odd, anisotropic extent
+    (30, 2.5, (0.3, -0.2, 0.1), (0.8, 0.8, 0.8), 1e-12),   # off-centre sources: post-phase e^{-i xi.C}
+    (64, 3.0, (0, 0, 0), (1, 1, 1), 1e-4),
+    (6, 2.0, (0, 0, 0), (1, 1, 1), 1e-9),           # lattice too coarse for the extent (2 pi h X > pi): type-3 fallback
+    (16, 2.0, (0, 0, 0), (1, 1, 1), 0.0),           # direct sum on the expanded nodes
+])
+def test_surface_ft_lattice_vs_oracle(sfd, orc, torch, M, xi_max, centre, half, eps):
+    """sfd_surface_ft_lattice (the paper's type-1 NUFFT, eq. 3.6 / P:188 eq. 3.7) against the oracle's direct
+    sum on the oracle's lattice nodes, element by element: 10 eps sum|w|."""
+    rng = np.random.default_rng(M * 7 + 1)
+    x, w = _cloud(rng, 4001, centre, half)
+    xi, _ = orc.lattice_nodes(M, xi_max)
+    ref = orc.direct_sum(x, w, xi)
+    got = sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), M, xi_max, eps).cpu().numpy()
+    assert got.shape == ref.shape
+    tol = (10 * eps if eps > 0 else 1e-12) * np.abs(w).sum()
+    assert np.abs(got - ref).max() <= tol, (np.abs(got - ref).max() / np.abs(w).sum(), eps)
+
+
+@pytest.mark.parametrize("w_", range(2, 16))
+def test_surface_ft_lattice_every_kernel_width(sfd, orc, torch, w_):
+    eps = 10.0 ** (-(w_ - 1))
+    rng = np.random.default_rng(w_)
+    x, w = _cloud(rng, 1500, (0, 0, 0), (1, 1, 1))
+    xi, _ = orc.lattice_nodes(20, 2.0)
+    ref = orc.direct_sum(x, w, xi)
+    got = sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), 20, 2.0, eps).cpu().numpy()
+    assert np.abs(got - ref).max() <= 10 * max(eps, 1e-14) * np.abs(w).sum()
+
+
+def test_surface_ft_lattice_is_the_type1_path(sfd, torch):
+    """The stage list of the last call shows which transform ran: no interpolation stage on the type-1 path."""
+    rng = np.random.default_rng(5)
+    x, w = _cloud(rng, 3000, (0, 0, 0), (1, 1, 1))
+    sfd.sfd_set_profiling(1)
+    try:
+        sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), 32, 3.0, 1e-9)
+        names = [n for n, _ in sfd.sfd_last_stage_times()]
+        assert "spread" in names and "fft" in names and "interp" not in names, names
+        sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), 6, 2.0, 1e-9)
+        names = [n for n, _ in sfd.sfd_last_stage_times()]
+        assert "interp" in names, names
+    finally:
+        sfd.sfd_set_profiling(0)
+
+
 def test_weak_distance_lattice_vs_oracle(sfd, orc, torch):
     """Whole path of the paper's variant on a small case: level 1, 64-point rule, M = 16, xi_max = 2, s = -5 and -10."""
     Vo, Fo = orc.mesh_icosphere(1)
