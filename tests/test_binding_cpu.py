@@ -127,3 +127,26 @@ def test_plan_and_workspace_queries(sfd):
         sfd.sfd_weak_distance_lattice_workspace(10, 64, 7, 5.0, 0.0)  # odd M
     assert sfd.sfd_weak_distance_lattice_workspace(20 * 4 ** 7, 64, 128, 5.0, 1e-7) > 20 * 4 ** 7 * 64 * 32
     assert sfd.sfd_launch_count() >= 0
+
+
+def test_lattice_transform_workspace_query(sfd):
+    """sfd_surface_ft_lattice_workspace (host-only): the type-1 plan needs the lattice's nuhat band, not a type-3 grid;
+    a lattice too coarse for the sources' extent is sized for the type-3 fallback; argument checks."""
+    K = 417 ** 3
+    t1 = sfd.sfd_surface_ft_lattice_workspace(1310720, 416, 5.0, [1, 1, 1], 1e-7)
+    t3 = sfd.sfd_surface_ft_workspace(1310720, K, [1, 1, 1], [10 * np.pi] * 3, 1e-7)
+    # expanded nodes of the fallback (24 K) + the half band 16 (M+1)^2 (M/2+1) + the n_in-plane intermediates + sorted
+    # sources: well below the type-3 need
+    band = 16 * 417 * 417 * 209
+    assert 24 * K + band < t1 < 24 * K + 1.5 * band
+    assert t1 < t3
+    # growing extent -> larger spread grid -> more workspace, until the type-1 plan stops applying (2 pi h X ~ pi)
+    a = sfd.sfd_surface_ft_lattice_workspace(1000, 64, 4.0, [0.5] * 3, 1e-9)
+    b = sfd.sfd_surface_ft_lattice_workspace(1000, 64, 4.0, [1.0] * 3, 1e-9)
+    assert a < b
+    coarse = sfd.sfd_surface_ft_lattice_workspace(1000, 6, 2.0, [1, 1, 1], 1e-9)
+    assert coarse >= sfd.sfd_surface_ft_workspace(1000, 343, [1, 1, 1], [4 * np.pi] * 3, 1e-9)
+    for bad in ((7, 5.0, 1e-7), (0, 5.0, 1e-7), (16, -1.0, 1e-7), (16, 5.0, 2.0)):
+        with pytest.raises(sfd.SfdError):
+            sfd.sfd_surface_ft_lattice_workspace(10, bad[0], bad[1], [1, 1, 1], bad[2])
+
