@@ -58,9 +58,9 @@ void kernel_params(double eps, int* w, double* beta) {
 }
 
 struct Layout {
-  size_t src, skey, shist, soff, scur, sitems, tgt, tkey, thist, toff, tcur, titems, fine, bufx, bufy, ffttab, dec,
+  size_t src, skey, shist, soff, scur, sbhist, sboff, sitems, tgt, tkey, thist, toff, tcur, titems, fine, bufx, bufy, ffttab, dec,
       scan, misc, ptab, total;
-  int64_t ns_bins, nt_bins, ns_items, nt_items;
+  int64_t ns_bins, ns_keys, nt_bins, ns_items, nt_items;
   size_t fine_bytes;
 };
 
@@ -106,10 +106,21 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
   return SFD_OK;
 }
 
+// Order the sources of a bin by footprint (N3Params::fine) when there are enough of them per cell for runs of equal
+// footprints to form -- the clustered case of the paper's lattice variant -- and the key table stays small.
+// sizing = true (workspace queries): whenever the table is small enough, so that the query bounds either choice.
+void choose_sort(N3Params* p, int64_t J, bool sizing = false) {
+  const int64_t nkeys = (int64_t)p->nbs[0] * p->nbs[1] * p->nbs[2] * source_subkeys(*p);
+  p->fine = (nkeys <= (int64_t(1) << 22) && (sizing || J * 16 >= nkeys)) ? 1 : 0;
+  // tens of sources per occupied cell (the sources lie on a surface: a few per cent of the cells): one warp per run
+  if (p->fine && (sizing || J >= nkeys) && spread_runs_ok(p->w, p->real_c != 0)) p->fine = 2;
+}
+
 int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->ns_bins = (int64_t)p.nbs[0] * p.nbs[1] * p.nbs[2];
   L->nt_bins = (int64_t)p.nbt[0] * p.nbt[1] * p.nbt[2];
   L->ns_items = L->ns_bins + J / kSrcCap + 1;   // upper bound for any cap >= kSrcCap
+  if (p.fine == 2) L->ns_items = std::max(L->ns_items, L->ns_bins * source_subkeys(p) + J / spread_runs_cap() + 1);
   L->nt_items = L->nt_bins + K / kTgtCap + 1;
   SFD_REQUIRE(L->ns_bins < 0x7fffffffLL && L->nt_bins < 0x7fffffffLL && J < 0x7fffffffLL && K < 0x7fffffffLL,
               SFD_ERR_UNSUPPORTED, "type-3 NUFFT: problem too large for 32-bit bin bookkeeping");
@@ -121,11 +132,14 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   };
   L->misc = put(kMiscBytes);
   L->ptab = put((size_t)(kMaxDeg + 1) * kPolyStride * 8);
+  L->ns_keys = p.fine ? L->ns_bins * source_subkeys(p) : L->ns_bins;
   L->src = put((size_t)J * sizeof(SrcRec));
   L->skey = put((size_t)J * 4);
-  L->shist = put((size_t)(L->ns_bins + 1) * 4);
-  L->soff = put((size_t)(L->ns_bins + 1) * 4);
-  L->scur = put((size_t)(L->ns_bins + 1) * 4);
+  L->shist = put((size_t)(L->ns_keys + 1) * 4);
+  L->soff = put((size_t)(L->ns_keys + 1) * 4);
+  L->scur = put((size_t)(L->ns_keys + 1) * 4);
+  L->sbhist = put(p.fine ? (size_t)(L->ns_bins + 1) * 4 : 0);
+  L->sboff = put(p.fine ? (size_t)(L->ns_bins + 1) * 4 : 0);
   L->sitems = put((size_t)L->ns_items * 4 * 3);
   L->tgt = put((size_t)K * sizeof(TgtRec));
   L->tkey = put((size_t)K * 4);
@@ -134,7 +148,7 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->tcur = put((size_t)(L->nt_bins + 1) * 4);
   L->titems = put((size_t)L->nt_items * 4 * 3);
   L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2] + p.nout[0] + p.nout[1] + p.nout[2]) * 8);
-  L->scan = put(scan_workspace(std::max(L->ns_bins, L->nt_bins) + 1));
+  L->scan = put(scan_workspace(std::max(L->ns_keys, L->nt_bins) + 1));
   L->ffttab = put(fft_tables_bytes(p.n2));
   L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16);
   L->fine = put(L->fine_bytes);
@@ -244,6 +258,31 @@ void width_tables(const N3Params& p, ChebTable* quad, double* h_ptab) {
   std::memcpy(h_ptab, wt.poly, sizeof(wt.poly));
 }
 
+// Work items of the spreader and the spread itself (shared by the type-3 and the type-1 transform).
+int items_and_spread(const N3Params& p, int64_t J, int64_t ns_bins, int64_t ns_keys, int64_t ns_items, int32_t* hist,
+                     int32_t* off, int32_t* tmp, int32_t* sitems, int32_t* d_ctl, void* scan_w, size_t scan_b,
+                     const double* ptab, const SrcRec* src, double* fine, size_t fine_bytes, cudaStream_t st) {
+  if (p.fine == 2) {
+    // one item per run of equal footprints (hist / off are the per-footprint tables), cut at spread_runs_cap()
+    SFD_TRY(make_items(hist, off, ns_keys, spread_runs_cap(), tmp, sitems, ns_items, d_ctl + 0, scan_w, scan_b, st));
+    prof_mark("src_sort", st);
+    SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
+    SFD_TRY(spread_runs(p, ptab, src, sitems, sitems + ns_items, sitems + 2 * ns_items, d_ctl + 0, d_ctl + 2, fine, st));
+    prof_mark("spread", st);
+    return SFD_OK;
+  }
+  // items of <= cap sources: 1024 normally; when the sources crowd into few bins (the paper's lattice variant maps
+  // 2e7 atoms onto ~60^3 cells, "highly clustered", P:236) larger slices keep the number of subgrid write-backs --
+  // global fp64 reductions onto the same few cells -- proportional to the SM count instead of to J
+  const int src_cap = (int)std::max<int64_t>(kSrcCap, J / ((int64_t)num_sms() * 8));
+  SFD_TRY(make_items(hist, off, ns_bins, src_cap, tmp, sitems, ns_items, d_ctl + 0, scan_w, scan_b, st));
+  prof_mark("src_sort", st);
+  SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
+  SFD_TRY(spread(p, ptab, src, sitems, sitems + ns_items, sitems + 2 * ns_items, d_ctl + 0, d_ctl + 2, fine, st));
+  prof_mark("spread", st);
+  return SFD_OK;
+}
+
 }  // namespace
 
 int nufft3_release_cache() { return SFD_OK; }   // nothing is cached on the device any more
@@ -260,6 +299,7 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
   N3Params p{};
   for (int real_c = 0; real_c < 2; ++real_c) {   // whether the strengths stay real is only known from the data
     SFD_TRY(make_params(Xi, Si, eps, real_c != 0, &p));
+    choose_sort(&p, J, true);
     Layout L;
     SFD_TRY(make_layout(p, J, K, &L));
     total = std::max(total, L.total);
@@ -319,6 +359,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     }
   }
   SFD_TRY(make_params(X, S, eps, real_c, &p));
+  choose_sort(&p, J);
   Layout L;
   SFD_TRY(make_layout(p, J, K, &L));
   SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
@@ -350,22 +391,21 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   const size_t fine_bytes = L.fine_bytes;
 
   // A5-2/A5-3: rescale, pre-phase and bin-sort the sources
-  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_bins + 1) * 4, st));
-  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_keys + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_keys + 1) * 4, st));
   SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
-  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_bins, nullptr, scan_w, scan_b, st));
+  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_keys, nullptr, scan_w, scan_b, st));
   SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
-  // items of <= cap sources: 1024 normally; when the sources crowd into few bins (the paper's lattice variant maps
-  // 2e7 atoms onto ~60^3 cells, "highly clustered", P:236) larger slices keep the number of subgrid write-backs --
-  // global fp64 reductions onto the same few cells -- proportional to the SM count instead of to J
-  const int src_cap = (int)std::max<int64_t>(kSrcCap, J / ((int64_t)num_sms() * 8));
-  SFD_TRY(make_items(shist, soff, L.ns_bins, src_cap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
-  prof_mark("src_sort", st);
-
-  // A5-4: spread
-  SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
-  SFD_TRY(spread(p, ptab, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
-  prof_mark("spread", st);
+  if (p.fine == 1) {   // per-bin ranges out of the per-footprint ones
+    int32_t* bh = reinterpret_cast<int32_t*>(base + L.sbhist);
+    int32_t* bo = reinterpret_cast<int32_t*>(base + L.sboff);
+    SFD_TRY(source_bin_ranges(p, soff, L.ns_bins, J, bh, bo, st));
+    shist = bh;
+    soff = bo;
+  }
+  // A5-4: work items and spread
+  SFD_TRY(items_and_spread(p, J, L.ns_bins, L.ns_keys, L.ns_items, shist, soff, scur, sitems, d_ctl, scan_w, scan_b, ptab,
+                           src, fine, fine_bytes, st));
 
   // A5-5 + A5-6: deconvolution folded into the first of three pruned 1-D FFT passes (timed on its own)
   SFD_TRY(deconv_tables(p, quad, dec, st));
@@ -475,6 +515,7 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
   SFD_TRY(make_params_lattice(Xi, C0, M, h, eps, &p, applicable));
   *bytes = 0;
   if (!*applicable) return SFD_OK;
+  choose_sort(&p, J, true);
   Layout L;
   SFD_TRY(make_layout(p, J, 0, &L));
   *bytes = L.total;
@@ -512,6 +553,7 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   N3Params p{};
   SFD_TRY(make_params_lattice(X, C, M, h, eps, &p, applicable));
   if (!*applicable) return SFD_OK;
+  choose_sort(&p, J);
   Layout L;
   SFD_TRY(make_layout(p, J, 0, &L));
   SFD_REQUIRE(work_bytes >= L.total, SFD_ERR_WORKSPACE_TOO_SMALL,
@@ -536,18 +578,20 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   const size_t scan_b = L.ffttab - L.scan;
 
   // rescale (eq. 3.7) and bin-sort the sources, as in the type-3 transform
-  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_bins + 1) * 4, st));
-  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_bins + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_keys + 1) * 4, st));
+  SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_keys + 1) * 4, st));
   SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
-  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_bins, nullptr, scan_w, scan_b, st));
+  SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_keys, nullptr, scan_w, scan_b, st));
   SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
-  const int src_cap = (int)std::max<int64_t>(kSrcCap, J / ((int64_t)num_sms() * 8));
-  SFD_TRY(make_items(shist, soff, L.ns_bins, src_cap, scur, sitems, L.ns_items, d_ctl + 0, scan_w, scan_b, st));
-  prof_mark("src_sort", st);
-
-  SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, L.fine_bytes, st));
-  SFD_TRY(spread(p, ptab, src, sitems, sitems + L.ns_items, sitems + 2 * L.ns_items, d_ctl + 0, d_ctl + 2, fine, st));
-  prof_mark("spread", st);
+  if (p.fine == 1) {   // per-bin ranges out of the per-footprint ones
+    int32_t* bh = reinterpret_cast<int32_t*>(base + L.sbhist);
+    int32_t* bo = reinterpret_cast<int32_t*>(base + L.sboff);
+    SFD_TRY(source_bin_ranges(p, soff, L.ns_bins, J, bh, bo, st));
+    shist = bh;
+    soff = bo;
+  }
+  SFD_TRY(items_and_spread(p, J, L.ns_bins, L.ns_keys, L.ns_items, shist, soff, scur, sitems, d_ctl, scan_w, scan_b, ptab,
+                           src, fine, L.fine_bytes, st));
 
   // three pruned FFT passes: position l = i - n_in/2 <-> x' = 2 pi l / N, output = the lattice modes
   SFD_TRY(lattice_tables(p, quad, M, dec, st));

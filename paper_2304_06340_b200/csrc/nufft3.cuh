@@ -24,6 +24,10 @@ struct N3Params {
   int bt[3], nbt[3], t0[3];  // target bins (bt[0] x bt[1] x bt[2] cells) over the band [t0, t0 + nbt*bt) of the
                              // inner grid that holds every target; bt[2] is 8 or 16 (bank-conflict-free pitch)
   int deg;                   // degree of the piecewise-polynomial kernel evaluation (w + 3)
+  int fine;                  // 1: inside a bin the sources are also ordered by the first cell of their footprint
+                             // ((bs+1)^3 sub-keys per bin), so that sources with the same footprint are consecutive
+                             // and the spreader accumulates them in registers (many sources per cell: P:236)
+                             // 2: so many per cell that one warp spreads a whole run (spread.cu spread_runs_kernel)
   int lo[3], nout[3];        // band of the inner grid that is computed and stored: v[m - lo], m in [lo, lo + nout)
   int zh;                    // 1: real strengths => v is Hermitian about the centre m = n2/2 (v[c+k] = conj v[c-k]) and
                              // only the half m_2 >= n2_2/2 of the band is computed and stored (lo[2] = n2_2/2); the
@@ -85,6 +89,14 @@ size_t spread_smem_bytes(const N3Params& p);
 int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
            const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter, double* d_grid, cudaStream_t st);
 
+// Clustered sources (N3Params::fine == 2): items are (key, start, count) slices of <= spread_runs_cap() sources with
+// the same footprint (make_items over the per-footprint histogram); one warp per item, register accumulation.
+int spread_runs_cap();
+bool spread_runs_ok(int w, bool real_c);
+int spread_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_key,
+                const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
+                double* d_grid, cudaStream_t st);
+
 // ---- interp.cu (A5-8) ------------------------------------------------------------------------------------
 // v = complex double[nout_0][nout_1][nout_2][2], the band [lo, lo+nout) of the inner grid; writes G[k] (complex) for
 // every sorted target.
@@ -100,6 +112,11 @@ constexpr int kBoundsBlocks = 296;
 int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scratch, cudaStream_t st);
 // A5-2/A5-3: bin key of every source + histogram; then scatter into bin order with grid coordinates and c'_j.
 int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st);
+// p.fine: keys are bin * cpb + sub-key, cpb = (bs0+1)(bs1+1)(bs2+1); after the scan of the fine histogram this
+// extracts the per-bin offsets and counts that make_items wants: d_boff[b] = d_off[b cpb], d_bhist[b] = their differences.
+inline int64_t source_subkeys(const N3Params& p) { return (int64_t)(p.bs[0] + 1) * (p.bs[1] + 1) * (p.bs[2] + 1); }
+int source_bin_ranges(const N3Params& p, const int32_t* d_off, int64_t nbins, int64_t J, int32_t* d_bhist,
+                      int32_t* d_boff, cudaStream_t st);
 int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
                    const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st);
 // A5-7: same for the targets.

@@ -100,16 +100,31 @@ __global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, const doubl
   const bool active = j < J;
   int k = 0;
   if (active) {
-    int b[3];
+    int b[3], c[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       const double u = src_coord(p, x[3 * j + d], d);
       b[d] = clampi((int)floor(u / p.bs[d]), 0, p.nbs[d] - 1);
+      // first cell of the footprint relative to the bin's padded subgrid: in [0, bs] (the footprint fits the subgrid)
+      int i0;
+      double s;
+      footprint(u, p.w, i0, s);
+      c[d] = clampi(i0 - (b[d] * p.bs[d] - p.w / 2), 0, p.bs[d]);
     }
     k = (b[0] * p.nbs[1] + b[1]) * p.nbs[2] + b[2];
+    if (p.fine) k = (k * (p.bs[0] + 1) + c[0]) * (p.bs[1] + 1) * (p.bs[2] + 1) + c[1] * (p.bs[2] + 1) + c[2];
     key[j] = k;
   }
   warp_agg_inc(hist, k, active);
+}
+
+__global__ void __launch_bounds__(kT) bin_ranges_kernel(const int32_t* __restrict__ off, int64_t nbins, int64_t cpb, int64_t J,
+                                                       int32_t* __restrict__ bhist, int32_t* __restrict__ boff) {
+  const int64_t b = (int64_t)blockIdx.x * kT + threadIdx.x;
+  if (b > nbins) return;
+  const int32_t lo = b < nbins ? off[b * cpb] : (int32_t)J;
+  boff[b] = lo;
+  if (b < nbins) bhist[b] = (b + 1 < nbins ? off[(b + 1) * cpb] : (int32_t)J) - lo;
 }
 
 __global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const double* __restrict__ x, const double* __restrict__ w,
@@ -278,6 +293,11 @@ int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scra
 int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st) {
   source_keys_kernel<<<blocks_for(J), kT, 0, st>>>(p, d_x, J, d_key, d_hist);
   return launch_check("source_keys_kernel");
+}
+int source_bin_ranges(const N3Params& p, const int32_t* d_off, int64_t nbins, int64_t J, int32_t* d_bhist,
+                      int32_t* d_boff, cudaStream_t st) {
+  bin_ranges_kernel<<<blocks_for(nbins + 1), kT, 0, st>>>(d_off, nbins, source_subkeys(p), J, d_bhist, d_boff);
+  return launch_check("bin_ranges_kernel");
 }
 int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
                    const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st) {

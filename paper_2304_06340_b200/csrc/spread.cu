@@ -18,6 +18,9 @@
 //   * kernel values are piecewise polynomials (nufft3.cuh footprint()): for a chunk of 32 sources (one per lane) warp
 //     group a evaluates interval a with the coefficients in registers; the next chunk's records are prefetched
 //     while the current one is accumulated;
+//   * consecutive sources whose footprints cover the same cells of the warp's plane are summed in registers and
+//     added to the subgrid once: with many sources per cell (the paper's lattice variant maps 2e7 atoms onto a
+//     54^3 grid) and the sort by footprint (N3Params::fine) this removes almost all shared-memory traffic;
 //   * only the final write-back of the subgrid uses fp64 global reductions (RED.ADD.F64), because neighbouring
 //     bins' paddings overlap; all-zero cells are skipped (the sources lie on a 2-D shell).
 #include <algorithm>
@@ -36,7 +39,7 @@ struct ChunkTables {
   int i0[kChunk][3];         // first cell of the footprint, relative to the subgrid origin
 };
 
-template <int W, bool REAL>
+template <int W, bool REAL, bool RUNS>
 __global__ void __launch_bounds__(32 * W, 1)
 spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restrict__ src,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
@@ -83,6 +86,33 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
     const int ncell = Px * Py * Pz;
     for (int i = tid; i < ncell * (REAL ? 1 : 2); i += 32 * W) sub[i] = 0.0;
 
+    // RUNS (N3Params::fine == 1, the sort is by footprint): consecutive sources with the same footprint cells in this
+    // warp's plane form a run, which is accumulated in registers and added to the subgrid once.
+    int run_base = -1;
+    double acc_re[NCL], acc_im[NCL];
+#pragma unroll
+    for (int i = 0; i < NCL; ++i) acc_re[i] = acc_im[i] = 0.0;
+    auto flush = [&]() {
+      if (run_base >= 0) {
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) {
+          if (on[i]) {
+            const int idx = run_base + off[i];
+            if (REAL) {
+              sub[idx] += acc_re[i];
+            } else {
+              double2 v = reinterpret_cast<double2*>(sub)[idx];
+              v.x += acc_re[i];
+              v.y += acc_im[i];
+              reinterpret_cast<double2*>(sub)[idx] = v;
+            }
+          }
+          acc_re[i] = acc_im[i] = 0.0;
+        }
+        __syncwarp();   // the next run's cells may be ones other lanes have just written
+      }
+    };
+
     SrcRec rn = src[start + min(lane, count - 1)];
     for (int c0 = 0; c0 < count; c0 += kChunk) {
       const int nch = min(kChunk, count - c0);
@@ -121,7 +151,7 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
       const double cre_l = r.re * kx;
       const double cim_l = REAL ? 0.0 : r.im * kx;
       // sweep over the chunk's sources, software-pipelined: the broadcasts and the ky kz products of source s+1 are
-      // fetched while source s does its read-modify-write (the sweep is latency-bound otherwise)
+      // fetched while source s is accumulated
       int base_n = __shfl_sync(0xffffffffu, base_l, 0);
       double cre_n = __shfl_sync(0xffffffffu, cre_l, 0);
       double cim_n = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, 0);
@@ -140,23 +170,36 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
         if (!REAL) cim_n = __shfl_sync(0xffffffffu, cim_l, sn);
 #pragma unroll
         for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? tab.k[1][sn][cy[i]] * tab.k[2][sn][cz[i]] : 0.0;
+        if (RUNS) {
+          if (base != run_base) {   // warp-uniform
+            flush();
+            run_base = base;
+          }
 #pragma unroll
-        for (int i = 0; i < NCL; ++i) {
-          if (on[i]) {
-            const int idx = base + off[i];
-            if (REAL) {
-              sub[idx] = __fma_rn(cre, kyz[i], sub[idx]);
-            } else {
-              double2 v = reinterpret_cast<double2*>(sub)[idx];
-              v.x = __fma_rn(cre, kyz[i], v.x);
-              v.y = __fma_rn(cim, kyz[i], v.y);
-              reinterpret_cast<double2*>(sub)[idx] = v;
+          for (int i = 0; i < NCL; ++i) {
+            acc_re[i] = __fma_rn(cre, kyz[i], acc_re[i]);
+            if (!REAL) acc_im[i] = __fma_rn(cim, kyz[i], acc_im[i]);
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < NCL; ++i) {
+            if (on[i]) {
+              const int idx = base + off[i];
+              if (REAL) {
+                sub[idx] = __fma_rn(cre, kyz[i], sub[idx]);
+              } else {
+                double2 v = reinterpret_cast<double2*>(sub)[idx];
+                v.x = __fma_rn(cre, kyz[i], v.x);
+                v.y = __fma_rn(cim, kyz[i], v.y);
+                reinterpret_cast<double2*>(sub)[idx] = v;
+              }
             }
           }
+          __syncwarp();
         }
-        __syncwarp();
       }
     }
+    if (RUNS) flush();
     __syncthreads();
     // write-back: neighbouring bins overlap in their paddings -> fp64 reductions into the global fine grid.
     // One (x,y) row of Pz <= 32 cells per warp pass, coalesced along z.
@@ -178,21 +221,161 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
   }
 }
 
-template <int W, bool REAL>
+template <int W, bool REAL, bool RUNS>
 int launch(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_grid, size_t smem, cudaStream_t st) {
   static bool attr = false;
   if (!attr) {
-    SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048));
+    SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL, RUNS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048));
     attr = true;
   }
-  spread_kernel<W, REAL><<<num_sms(), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start,
-                                                                         d_item_count, d_n_items, d_counter, d_grid);
+  spread_kernel<W, REAL, RUNS><<<num_sms(), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
+                                                                d_n_items, d_counter, d_grid);
   return launch_check("spread_kernel");
 }
 
+
+// ---- many sources per cell ("highly clustered"): one warp per run of equal footprints --------------------
+// With the sources ordered by footprint (N3Params::fine == 2) a work item is a slice of <= kRunCap consecutive
+// sources that all start at the same cell i0.  One warp takes the whole item: the lanes evaluate the 3 W kernel
+// values of 32 sources at once (one source per lane, Horner), the sweep then adds c kx[a] * (ky kz)[cell] into
+// W x NCL register accumulators per lane -- 16 DFMA per source at W = 8, no shared-memory read-modify-write and no
+// redundancy between warps -- and the W^3 sums go to the global grid by fp64 reductions once per item.  Warps are
+// independent (dynamic queue), so many of them hide each other's latencies.  Real strengths, W <= 10.
+constexpr int kRunWarps = 16;
+constexpr int kRunCap = 512;
+
+template <int W>
+__global__ void __launch_bounds__(32 * kRunWarps, 1)
+spread_runs_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restrict__ src,
+                   const int32_t* __restrict__ item_key, const int32_t* __restrict__ item_start,
+                   const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
+                   int32_t* __restrict__ counter, double* __restrict__ grid) {
+  constexpr int NCL = (W * W + 31) / 32;
+  constexpr int DEG = W + 3;
+  constexpr int PITCH = 33;                      // kv[d][a][lane]: conflict-free for reads across a at a fixed lane
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* s_pc = reinterpret_cast<double*>(smem_raw);   // polynomial coefficients, [q][a]
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  for (int i = tid; i < (DEG + 1) * W; i += 32 * kRunWarps) s_pc[i] = ptab[(i / W) * kPolyStride + (i % W)];
+  __syncthreads();
+  double* kv = s_pc + (DEG + 1) * W + wrp * (3 * W * PITCH);
+
+  int cy[NCL], cz[NCL];
+  bool on[NCL];
+#pragma unroll
+  for (int i = 0; i < NCL; ++i) {
+    on[i] = lane + 32 * i < W * W;
+    const int c = min(lane + 32 * i, W * W - 1);
+    cy[i] = c / W;
+    cz[i] = c % W;
+  }
+  const int sub1 = p.bs[1] + 1, sub2 = p.bs[2] + 1, sub0 = p.bs[0] + 1;
+  const int total = *n_items;
+  for (;;) {
+    int item = 0;
+    if (lane == 0) item = atomicAdd(counter, 1);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= total) break;
+    const int key = item_key[item], start = item_start[item], count = item_count[item];
+    // key = ((bin * sub0 + c0) * sub1 + c1) * sub2 + c2 (nufft3_glue.cu source_keys_kernel)
+    const int c2 = key % sub2, c1 = (key / sub2) % sub1, c0 = (key / (sub2 * sub1)) % sub0, bin = key / (sub2 * sub1 * sub0);
+    const int bz = bin % p.nbs[2], by = (bin / p.nbs[2]) % p.nbs[1], bx = bin / (p.nbs[2] * p.nbs[1]);
+    const int i0x = bx * p.bs[0] - W / 2 + c0, i0y = by * p.bs[1] - W / 2 + c1, i0z = bz * p.bs[2] - W / 2 + c2;
+
+    double acc[W][NCL];
+#pragma unroll
+    for (int a = 0; a < W; ++a)
+#pragma unroll
+      for (int i = 0; i < NCL; ++i) acc[a][i] = 0.0;
+
+    for (int c0s = 0; c0s < count; c0s += 32) {
+      const int nch = min(32, count - c0s);
+      const SrcRec r = src[start + min(c0s + lane, count - 1)];
+      double sv[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        int i0;
+        footprint(r.u[d], W, i0, sv[d]);
+      }
+      __syncwarp();   // the previous chunk's sweep has finished reading kv
+#pragma unroll
+      for (int a = 0; a < W; ++a) {
+        double k0 = s_pc[DEG * W + a], k1 = k0, k2 = k0;
+#pragma unroll
+        for (int q = DEG - 1; q >= 0; --q) {
+          const double cq = s_pc[q * W + a];
+          k0 = __fma_rn(k0, sv[0], cq);
+          k1 = __fma_rn(k1, sv[1], cq);
+          k2 = __fma_rn(k2, sv[2], cq);
+        }
+        kv[(0 * W + a) * PITCH + lane] = lane < nch ? k0 * r.re : 0.0;
+        kv[(1 * W + a) * PITCH + lane] = k1;
+        kv[(2 * W + a) * PITCH + lane] = k2;
+      }
+      __syncwarp();
+#pragma unroll 2
+      for (int s2 = 0; s2 < nch; ++s2) {
+        double kyz[NCL];
+#pragma unroll
+        for (int i = 0; i < NCL; ++i) kyz[i] = kv[(W + cy[i]) * PITCH + s2] * kv[(2 * W + cz[i]) * PITCH + s2];
+#pragma unroll
+        for (int a = 0; a < W; ++a) {
+          const double ck = kv[a * PITCH + s2];
+#pragma unroll
+          for (int i = 0; i < NCL; ++i) acc[a][i] = __fma_rn(ck, kyz[i], acc[a][i]);
+        }
+      }
+    }
+    // W^3 sums of the item -> global grid (footprints of different items overlap: fp64 reductions)
+#pragma unroll
+    for (int a = 0; a < W; ++a) {
+#pragma unroll
+      for (int i = 0; i < NCL; ++i) {
+        if (on[i] && acc[a][i] != 0.0) {
+          const size_t g = ((size_t)(i0x + a) * p.nf[1] + (i0y + cy[i])) * p.nf[2] + (i0z + cz[i]);
+          atomicAdd(&grid[g], acc[a][i]);
+        }
+      }
+    }
+  }
+}
+
+template <int W>
+int launch_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_key,
+                const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
+                double* d_grid, cudaStream_t st) {
+  constexpr size_t smem = ((size_t)(W + 4) * W + (size_t)kRunWarps * 3 * W * 33) * sizeof(double);
+  static bool attr = false;
+  if (!attr) {
+    SFD_CUDA_TRY(cudaFuncSetAttribute(spread_runs_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr = true;
+  }
+  spread_runs_kernel<W><<<num_sms(), 32 * kRunWarps, smem, st>>>(p, d_ptab, d_src, d_item_key, d_item_start, d_item_count,
+                                                              d_n_items, d_counter, d_grid);
+  return launch_check("spread_runs_kernel");
+}
+
 }  // namespace
+
+int spread_runs_cap() { return kRunCap; }
+bool spread_runs_ok(int w, bool real_c) { return real_c && w >= 2 && w <= 10; }
+
+int spread_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_key,
+                const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
+                double* d_grid, cudaStream_t st) {
+  SFD_REQUIRE(spread_runs_ok(p.w, p.real_c != 0), SFD_ERR_INVALID_ARG, "spread_runs: unsupported width %d", p.w);
+  SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
+#define SFD_RUNS_CASE(W_) \
+  case W_: return launch_runs<W_>(p, d_ptab, d_src, d_item_key, d_item_start, d_item_count, d_n_items, d_counter, d_grid, st);
+  switch (p.w) {
+    SFD_RUNS_CASE(2) SFD_RUNS_CASE(3) SFD_RUNS_CASE(4) SFD_RUNS_CASE(5) SFD_RUNS_CASE(6)
+    SFD_RUNS_CASE(7) SFD_RUNS_CASE(8) SFD_RUNS_CASE(9) SFD_RUNS_CASE(10)
+  }
+#undef SFD_RUNS_CASE
+  return SFD_ERR_UNSUPPORTED;
+}
 
 // Source-bin shape: z extent 16 (real grid: 16 eight-byte bank groups) or 8/16 (complex), x and y as large as the
 // shared-memory budget allows (at most 24: the sources lie on a shell, and smaller bins balance better).
@@ -226,18 +409,18 @@ int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const i
   SFD_REQUIRE(smem <= 227 * 1024 - 2048 && p.bs[2] + p.w <= 32, SFD_ERR_INVALID_ARG,
               "spread subgrid does not fit shared memory (%zu B)", smem);
   SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
-#define SFD_SPREAD_CASE(W_)                                                                                          \
-  case W_:                                                                                                           \
-    return p.real_c ? launch<W_, true>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count, d_n_items,          \
-                                       d_counter, d_grid, smem, st)                                                  \
-                    : launch<W_, false>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count, d_n_items,         \
-                                        d_counter, d_grid, smem, st);
+#define SFD_SPREAD_ARGS p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_grid, smem, st
+#define SFD_SPREAD_CASE(W_)                                                                        \
+  case W_:                                                                                         \
+    if (p.fine == 1) return p.real_c ? launch<W_, true, true>(SFD_SPREAD_ARGS) : launch<W_, false, true>(SFD_SPREAD_ARGS); \
+    return p.real_c ? launch<W_, true, false>(SFD_SPREAD_ARGS) : launch<W_, false, false>(SFD_SPREAD_ARGS);
   switch (p.w) {
     SFD_SPREAD_CASE(2) SFD_SPREAD_CASE(3) SFD_SPREAD_CASE(4) SFD_SPREAD_CASE(5) SFD_SPREAD_CASE(6)
     SFD_SPREAD_CASE(7) SFD_SPREAD_CASE(8) SFD_SPREAD_CASE(9) SFD_SPREAD_CASE(10) SFD_SPREAD_CASE(11)
     SFD_SPREAD_CASE(12) SFD_SPREAD_CASE(13) SFD_SPREAD_CASE(14) SFD_SPREAD_CASE(15) SFD_SPREAD_CASE(16)
   }
 #undef SFD_SPREAD_CASE
+#undef SFD_SPREAD_ARGS
   set_error("spread: unsupported kernel width %d", p.w);
   return SFD_ERR_UNSUPPORTED;
 }

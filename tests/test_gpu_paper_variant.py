@@ -96,6 +96,37 @@ def test_surface_ft_lattice_every_kernel_width(sfd, orc, torch, w_):
     assert np.abs(got - ref).max() <= 10 * max(eps, 1e-14) * np.abs(w).sum()
 
 
+@pytest.mark.parametrize("eps", [1e-6, 1e-9, 1e-12])
+def test_clustered_sources_lattice(sfd, orc, torch, eps):
+    """Many sources per grid cell ("highly clustered"): the sort by footprint and the spreaders that sum runs of
+    equal footprints in registers (one warp per run for w <= 10, the plane-owner kernel above) -- 300 k atoms on the
+    sphere against a 17^3 lattice, element by element against the oracle."""
+    rng = np.random.default_rng(int(-np.log10(eps)))
+    J = 300_000
+    x = rng.normal(size=(J, 3))
+    x /= np.linalg.norm(x, axis=1, keepdims=True)
+    w = rng.random(J) * 4 * np.pi / J
+    xi, _ = orc.lattice_nodes(16, 2.0)
+    ref = orc.direct_sum(x, w, xi)
+    got = sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), 16, 2.0, eps).cpu().numpy()
+    assert np.abs(got - ref).max() <= 10 * eps * np.abs(w).sum()
+
+
+@pytest.mark.parametrize("centre,eps", [((0, 0, 0), 1e-9), ((0, 0, 0), 1e-12), ((3.0, -2.0, 1.0), 1e-9)])
+def test_clustered_sources_type3(sfd, orc, torch, centre, eps):
+    """The same regime through the type-3 transform: real strengths (ball-centred targets) and complex ones."""
+    rng = np.random.default_rng(17)
+    J, K = 250_000, 2000
+    x = (rng.random((J, 3)) * 2 - 1) * np.array([1.0, 0.8, 0.6])
+    w = rng.normal(size=J)
+    xi = (rng.random((K, 3)) * 2 - 1) * 8.0 + np.asarray(centre)
+    xi[0] = np.asarray(centre) + 8.0      # symmetric extent about the centre
+    xi[1] = np.asarray(centre) - 8.0
+    ref = orc.direct_sum(x, w, xi)
+    got = sfd.sfd_surface_ft(dev(torch, x), dev(torch, w), dev(torch, xi), eps).cpu().numpy()
+    assert np.abs(got - ref).max() <= 10 * eps * np.abs(w).sum()
+
+
 def test_surface_ft_lattice_is_the_type1_path(sfd, torch):
     """The stage list of the last call shows which transform ran: no interpolation stage on the type-1 path."""
     rng = np.random.default_rng(5)
