@@ -149,6 +149,11 @@ int sfd_lattice_nodes_device(int32_t M, double xi_max, double* d_xi /*[K][3]*/, 
  * lattice nodes xi' = 2 pi xi is xi_scale = 1/(2 pi), s = -s_paper, prefactor = 1.  s > 0.5.  Synchronises. */
 int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, double xi_scale,
                   double prefactor, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+/* sfd_reduce_ex on the lattice of sfd_lattice_nodes without reading it: nodes and trapezoid weights are recomputed from
+ * the index with the same roundings, so the result equals sfd_reduce_ex on the expanded lattice bit for bit; 16 B of
+ * traffic per node instead of 48.  d_nuhat complex128 [(M+1)^3] in lattice order; M even, 2..1624.  Synchronises. */
+int sfd_reduce_lattice(const double* d_nuhat, int32_t M, double xi_max, double s, double xi_scale, double prefactor,
+                       void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
 /* nuhat on the lattice of sfd_lattice_nodes (same node order) -- the transform the paper itself runs (eq. 3.6:
  * type-1 NUFFT, nonuniform sources -> integer modes, after the rescaling x -> h x of P:188 eq. 3.7).  eps > 0: type-1
  * NUFFT (sort, spread, pruned FFT whose output band IS the lattice, deconvolution; no interpolation step); when the

@@ -58,6 +58,7 @@ _SIGS = {
     "sfd_lattice_nodes": (C.c_int, [C.c_int32, _dbl, _vp, _vp]),
     "sfd_lattice_nodes_device": (C.c_int, [C.c_int32, _dbl, _vp, _vp, _vp]),
     "sfd_reduce_ex": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _dbl, _vp, _sz, _vp, _P(_dbl)]),
+    "sfd_reduce_lattice": (C.c_int, [_vp, C.c_int32, _dbl, _dbl, _dbl, _dbl, _vp, _sz, _vp, _P(_dbl)]),
     "sfd_surface_ft_lattice_workspace": (C.c_int, [_i64, C.c_int32, _dbl, _P(_dbl), _dbl, _P(_sz)]),
     "sfd_surface_ft_lattice": (C.c_int, [_vp, _vp, _i64, C.c_int32, _dbl, _dbl, _vp, _vp, _sz, _vp]),
     "sfd_weak_distance_lattice_workspace": (C.c_int, [_i64, C.c_int, C.c_int32, _dbl, _dbl, _dbl, _P(_sz)]),
@@ -334,6 +335,21 @@ def sfd_reduce_ex(nuhat, xi, W, s, xi_scale, prefactor):
     I = _dbl()
     _chk(_lib.sfd_reduce_ex(_ptr(nu), _ptr(xi), _ptr(W), K, float(s), float(xi_scale), float(prefactor), _ptr(work),
                             work.numel(), _stream(), C.byref(I)))
+    return I.value
+
+
+def sfd_reduce_lattice(nuhat, M, xi_max, s, xi_scale, prefactor):
+    """sfd_reduce_ex on the lattice of sfd_lattice_nodes, nodes and weights recomputed from the index (not read)."""
+    K = (int(M) + 1) ** 3
+    nu = torch.view_as_real(nuhat) if nuhat.is_complex() else nuhat
+    _dev_f64(nu, 2)
+    assert nu.shape[0] == K
+    wb = _sz()
+    _chk(_lib.sfd_reduce_workspace(K, C.byref(wb)))
+    work = _work(wb.value, nu.device)
+    I = _dbl()
+    _chk(_lib.sfd_reduce_lattice(_ptr(nu), int(M), float(xi_max), float(s), float(xi_scale), float(prefactor),
+                                 _ptr(work), work.numel(), _stream(), C.byref(I)))
     return I.value
 
 

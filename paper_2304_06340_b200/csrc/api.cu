@@ -422,12 +422,13 @@ int lattice_ft_bytes(int64_t J, int M, double xi_max, const double X[3], double 
   return SFD_OK;
 }
 
-// nuhat on the lattice; d_xi = the expanded nodes (lattice_expand), used only by the type-3 / direct path.
-int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi_max, double eps, const double* d_xi,
+// nuhat on the lattice; d_xi_buf = room for the expanded nodes (24 K bytes), filled and used only by the type-3 /
+// direct path.
+int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi_max, double eps, double* d_xi_buf,
                double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
   const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  cudaStream_t st = as_stream(stream);
   if (eps > 0.0 && J > 0) {
-    cudaStream_t st = as_stream(stream);
     const bool own_prof = !g_prof.active;
     if (own_prof) prof_begin(st);
     bool ok = false;
@@ -435,7 +436,8 @@ int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi
     if (own_prof) prof_end(st);
     if (rc != SFD_OK || ok) return rc;
   }
-  return sfd_surface_ft(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, stream);
+  SFD_TRY(lattice_expand(M, xi_max, d_xi_buf, nullptr, st));
+  return sfd_surface_ft(d_x, d_w, J, d_xi_buf, K, eps, d_nuhat, d_work, work_bytes, stream);
 }
 }  // namespace
 
@@ -462,20 +464,23 @@ int sfd_surface_ft_lattice(const double* d_x, const double* d_w, int64_t J, int3
   const size_t xi_bytes = align_up((size_t)K * 24);
   SFD_REQUIRE(d_work && work_bytes >= xi_bytes, SFD_ERR_WORKSPACE_TOO_SMALL,
               "sfd_surface_ft_lattice needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
-  cudaStream_t st = as_stream(stream);
   char* base = static_cast<char*>(d_work);
-  if (eps > 0.0 && J > 0) {
-    const bool own_prof = !g_prof.active;
-    if (own_prof) prof_begin(st);
-    bool ok = false;
-    const int rc = nufft1_lattice(d_x, d_w, J, M, 2.0 * xi_max / M, eps, d_nuhat, base + xi_bytes, work_bytes - xi_bytes,
-                                  st, &ok);
-    if (own_prof) prof_end(st);
-    if (rc != SFD_OK || ok) return rc;
-  }
-  double* xi = reinterpret_cast<double*>(base);
-  SFD_TRY(lattice_expand(M, xi_max, xi, nullptr, st));
-  return sfd_surface_ft(d_x, d_w, J, xi, K, eps, d_nuhat, base + xi_bytes, work_bytes - xi_bytes, stream);
+  return lattice_ft(d_x, d_w, J, M, xi_max, eps, reinterpret_cast<double*>(base), d_nuhat, base + xi_bytes,
+                    work_bytes - xi_bytes, stream);
+}
+
+int sfd_reduce_lattice(const double* d_nuhat, int32_t M, double xi_max, double s, double xi_scale, double prefactor,
+                       void* d_work, size_t work_bytes, sfd_stream stream, double* h_I) {
+  SFD_REQUIRE(h_I, SFD_ERR_NULL, "sfd_reduce_lattice: h_I is NULL");
+  SFD_TRY(check_lattice(M, xi_max));
+  SFD_REQUIRE(xi_scale > 0.0 && std::isfinite(xi_scale) && prefactor > 0.0 && std::isfinite(prefactor),
+              SFD_ERR_INVALID_ARG, "sfd_reduce_lattice: xi_scale and prefactor must be positive and finite");
+  cudaStream_t st = as_stream(stream);
+  double* d_res = nullptr;
+  SFD_TRY(reduce_lattice_enqueue(d_nuhat, M, xi_max, s, d_work, work_bytes, st, &d_res, xi_scale, prefactor));
+  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  return SFD_OK;
 }
 
 namespace {
@@ -536,19 +541,18 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   double* x = reinterpret_cast<double*>(base + L.x);
   double* w = reinterpret_cast<double*>(base + L.w);
   double* xi = reinterpret_cast<double*>(base + L.xi);
-  double* W = reinterpret_cast<double*>(base + L.W);
   double* nu = reinterpret_cast<double*>(base + L.nu);
   prof_begin(st);
   int rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
   prof_mark("nodes", st);
-  if (rc == SFD_OK) rc = lattice_expand(M, xi_max, xi, W, st);
-  prof_mark("freq_nodes", st);
+  // the lattice nodes are expanded only if the transform falls back to type-3 / direct (lattice_ft); the reduction
+  // recomputes them from the index
   if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream);
   double* d_res = nullptr;
   // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
   if (rc == SFD_OK)
-    rc = reduce_enqueue(nu, xi, W, L.K, -s_paper, base + L.red, L.red_bytes, st, &d_res,
-                        1.0 / 6.283185307179586476925286766559, 1.0);
+    rc = reduce_lattice_enqueue(nu, M, xi_max, -s_paper, base + L.red, L.red_bytes, st, &d_res,
+                                1.0 / 6.283185307179586476925286766559, 1.0);
   prof_mark("reduce", st);
   double I = 0.0;
   if (rc == SFD_OK) {

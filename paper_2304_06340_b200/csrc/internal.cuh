@@ -44,6 +44,9 @@ size_t reduce_workspace(int64_t K);
 int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
                    size_t work_bytes, cudaStream_t st, double** d_result, double scale = 1.0, double pref = -1.0,
                    const double* d_nuhat2 = nullptr);   // d_nuhat2: second operand instead of sigmahat
+// The same on the paper's lattice (nodes and trapezoid weights recomputed from the index, not read): 16 B per node.
+int reduce_lattice_enqueue(const double* d_nuhat, int M, double xi_max, double s, void* d_work, size_t work_bytes,
+                           cudaStream_t st, double** d_result, double scale, double pref);
 // nodes.cu: the paper's cube lattice: xi' = 2 pi xi_ijk, W = w_ijk h^3
 int lattice_expand(int M, double xi_max, double* d_xi, double* d_W, cudaStream_t st);
 

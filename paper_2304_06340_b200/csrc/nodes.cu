@@ -67,42 +67,56 @@ void fill_rule(int q, RuleTable& t) {
 }
 
 // One thread per atom j = f*q + i.  Each operation rounds once (no FMA contraction), so that the atoms are
-// the same doubles on every build.
+// the same doubles on every build.  The coordinates go through shared memory so that the block's 3 x 256 doubles
+// are stored contiguously (a thread's own three are 24 B apart from its neighbour's).
 template <int Q>
 __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V, const int32_t* __restrict__ F,
                                                     int64_t nF, int64_t nV, double* __restrict__ x,
                                                     double* __restrict__ w) {
-  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= nF * Q) return;
-  const int64_t f = j / Q;
-  const int i = (int)(j - f * Q);
-  const RuleTable& R = c_rule[Q == 6 ? 0 : (Q == 12 ? 1 : 2)];
-  const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
-  const double nan = __longlong_as_double(0x7ff8000000000000LL);
-  if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
-    x[3 * j] = x[3 * j + 1] = x[3 * j + 2] = nan;
-    w[j] = nan;
-    return;
+  __shared__ double sx[3 * 256];
+  // the rule, one array per column: a warp's 32 atoms read 32 different rows, which the constant cache would serialise
+  __shared__ double s_rule[4][Q];
+  {
+    const RuleTable& R = c_rule[Q == 6 ? 0 : (Q == 12 ? 1 : 2)];
+    for (int t = threadIdx.x; t < 4 * Q; t += 256) s_rule[t / Q][t % Q] = t / Q < 3 ? R.lam[t % Q][t / Q] : R.om[t % Q];
   }
-  double p0[3], p1[3], p2[3], e1[3], e2[3];
+  __syncthreads();
+  const int64_t j0 = (int64_t)blockIdx.x * 256;
+  const int64_t j = j0 + threadIdx.x;
+  const int64_t J = nF * Q;
+  if (j < J) {
+    const int64_t f = j / Q;
+    const int i = (int)(j - f * Q);
+    const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
+      sx[3 * threadIdx.x] = sx[3 * threadIdx.x + 1] = sx[3 * threadIdx.x + 2] = nan;
+      w[j] = nan;
+    } else {
+      double p0[3], p1[3], p2[3], e1[3], e2[3];
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    p0[c] = V[3 * (int64_t)i0 + c];
-    p1[c] = V[3 * (int64_t)i1 + c];
-    p2[c] = V[3 * (int64_t)i2 + c];
-    e1[c] = __dsub_rn(p1[c], p0[c]);
-    e2[c] = __dsub_rn(p2[c], p0[c]);
+      for (int c = 0; c < 3; ++c) {
+        p0[c] = V[3 * (int64_t)i0 + c];
+        p1[c] = V[3 * (int64_t)i1 + c];
+        p2[c] = V[3 * (int64_t)i2 + c];
+        e1[c] = __dsub_rn(p1[c], p0[c]);
+        e2[c] = __dsub_rn(p2[c], p0[c]);
+      }
+      const double cx = __dsub_rn(__dmul_rn(e1[1], e2[2]), __dmul_rn(e1[2], e2[1]));
+      const double cy = __dsub_rn(__dmul_rn(e1[2], e2[0]), __dmul_rn(e1[0], e2[2]));
+      const double cz = __dsub_rn(__dmul_rn(e1[0], e2[1]), __dmul_rn(e1[1], e2[0]));
+      const double n2 = __dadd_rn(__dadd_rn(__dmul_rn(cx, cx), __dmul_rn(cy, cy)), __dmul_rn(cz, cz));
+      const double area = __dmul_rn(0.5, __dsqrt_rn(n2));
+      const double l0 = s_rule[0][i], l1 = s_rule[1][i], l2 = s_rule[2][i];
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+        sx[3 * threadIdx.x + c] = __dadd_rn(__dadd_rn(__dmul_rn(l0, p0[c]), __dmul_rn(l1, p1[c])), __dmul_rn(l2, p2[c]));
+      w[j] = __dmul_rn(s_rule[3][i], area);
+    }
   }
-  const double cx = __dsub_rn(__dmul_rn(e1[1], e2[2]), __dmul_rn(e1[2], e2[1]));
-  const double cy = __dsub_rn(__dmul_rn(e1[2], e2[0]), __dmul_rn(e1[0], e2[2]));
-  const double cz = __dsub_rn(__dmul_rn(e1[0], e2[1]), __dmul_rn(e1[1], e2[0]));
-  const double n2 = __dadd_rn(__dadd_rn(__dmul_rn(cx, cx), __dmul_rn(cy, cy)), __dmul_rn(cz, cz));
-  const double area = __dmul_rn(0.5, __dsqrt_rn(n2));
-  const double l0 = R.lam[i][0], l1 = R.lam[i][1], l2 = R.lam[i][2];
-#pragma unroll
-  for (int c = 0; c < 3; ++c)
-    x[3 * j + c] = __dadd_rn(__dadd_rn(__dmul_rn(l0, p0[c]), __dmul_rn(l1, p1[c])), __dmul_rn(l2, p2[c]));
-  w[j] = __dmul_rn(R.om[i], area);
+  __syncthreads();
+  const int64_t n = 3 * min((int64_t)256, J - j0);
+  for (int t = threadIdx.x; t < n; t += 256) x[3 * j0 + t] = sx[t];
 }
 
 }  // namespace

@@ -6,6 +6,8 @@
 // HBM-bound, 48 B per target, one pass.  The sum is carried as a (sum, compensation) fp64 pair (TwoSum) from the
 // per-thread accumulators through warp shuffles, the block tree and a fixed-order final pass over the per-CTA
 // partials: deterministic for a given K.
+#include <cmath>
+
 #include "internal.cuh"
 
 namespace sfd {
@@ -66,21 +68,50 @@ __device__ __forceinline__ double sigma_hat(double r) {
   return four_pi * sin(r) / r;
 }
 
+// (1+r^2)^-s: s = 1, 2 directly; other integer s <= 64 by binary powering (the paper's s = 5, 10; the generic pow costs
+// more FP64 instructions than the rest of the node put together and made the pass ALU-bound); pow otherwise.
 __device__ __forceinline__ double sobolev_weight(double q, double s, int s_kind) {
   if (s_kind == 1) return 1.0 / q;
   if (s_kind == 2) return 1.0 / (q * q);
+  if (s_kind > 2) {
+    double r = 1.0, b = q;
+    for (int e = s_kind; e > 0; e >>= 1) {   // uniform across the grid
+      if (e & 1) r *= b;
+      b *= b;
+    }
+    return 1.0 / r;
+  }
   return pow(q, -s);
 }
 
-// nuhat2 == nullptr: difference against the unit sphere's closed form; else against a second transform (mesh vs mesh)
+// nuhat2 == nullptr: difference against the unit sphere's closed form; else against a second transform (mesh vs mesh).
+// LATTICE: the nodes are the paper's lattice in the order of nodes.cu lattice_kernel and are recomputed
+// from the index with the same roundings (xi = 2 pi (m h), W = h^3 / 2^{faces}) instead of being read: 16 B per node.
+template <bool LATTICE>
 __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* __restrict__ nuhat,
                                                                const double2* __restrict__ nuhat2, const double* __restrict__ xi,
                                                                const double* __restrict__ W, int64_t K, double s, int s_kind,
-                                                               double scale2, Comp* __restrict__ partial) {
+                                                               double scale2, int M, double h, Comp* __restrict__ partial) {
   Comp acc{0.0, 0.0};
   const int64_t stride = (int64_t)gridDim.x * kThreads;
   for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < K; k += stride) {
-    const double a = xi[3 * k], b = xi[3 * k + 1], c = xi[3 * k + 2];
+    double a, b, c, wk;
+    if (LATTICE) {
+      const unsigned n = (unsigned)M + 1u, ku = (unsigned)k;
+      const unsigned ab = ku / n;
+      const int ic = (int)(ku - ab * n) - M / 2, ib = (int)(ab % n) - M / 2, ia = (int)(ab / n) - M / 2;
+      const double two_pi = 6.283185307179586476925286766559;
+      a = __dmul_rn(two_pi, __dmul_rn((double)ia, h));
+      b = __dmul_rn(two_pi, __dmul_rn((double)ib, h));
+      c = __dmul_rn(two_pi, __dmul_rn((double)ic, h));
+      wk = __dmul_rn(__dmul_rn(h, h), h);
+      if (ia == -M / 2 || ia == M / 2) wk = __dmul_rn(wk, 0.5);
+      if (ib == -M / 2 || ib == M / 2) wk = __dmul_rn(wk, 0.5);
+      if (ic == -M / 2 || ic == M / 2) wk = __dmul_rn(wk, 0.5);
+    } else {
+      a = xi[3 * k], b = xi[3 * k + 1], c = xi[3 * k + 2];
+      wk = W[k];
+    }
     const double2 nu = nuhat[k];
     const double r2 = a * a + b * b + c * c;
     const double r = sqrt(r2);
@@ -93,7 +124,7 @@ __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* _
       dre = nu.x - sigma_hat(r);
       dim = nu.y;
     }
-    const double term = W[k] * (dre * dre + dim * dim) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
+    const double term = wk * (dre * dre + dim * dim) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
     two_sum_add(acc, term);
   }
   const Comp tot = block_reduce(acc);
@@ -122,15 +153,16 @@ size_t reduce_workspace(int64_t K) {
   return 256 + align_up(sizeof(Comp) * kMaxBlocks);
 }
 
-int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
-                   size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref,
-                   const double* d_nuhat2) {
+namespace {
+int reduce_any(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
+               size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref, const double* d_nuhat2,
+               int M, double h) {
   if (pref < 0.0) pref = 1.0 / (6.283185307179586 * 6.283185307179586 * 6.283185307179586);   // (2 pi)^-3
   SFD_REQUIRE(K >= 0, SFD_ERR_INVALID_ARG, "K must be >= 0");
   SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
   SFD_REQUIRE(d_work && work_bytes >= reduce_workspace(K), SFD_ERR_WORKSPACE_TOO_SMALL,
               "reduction needs %zu workspace bytes, got %zu", reduce_workspace(K), work_bytes);
-  SFD_REQUIRE(K == 0 || (d_nuhat && d_xi && d_W), SFD_ERR_NULL, "sfd_reduce: NULL input buffer");
+  SFD_REQUIRE(K == 0 || (d_nuhat && (M > 0 || (d_xi && d_W))), SFD_ERR_NULL, "sfd_reduce: NULL input buffer");
   double* result = static_cast<double*>(d_work);
   Comp* partial = reinterpret_cast<Comp*>(static_cast<char*>(d_work) + 256);
   *d_result = result;
@@ -139,13 +171,31 @@ int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W,
     return SFD_OK;
   }
   const int blocks = reduce_blocks(K);
-  const int s_kind = s == 1.0 ? 1 : (s == 2.0 ? 2 : 0);
-  reduce_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(d_nuhat),
-                                                   reinterpret_cast<const double2*>(d_nuhat2), d_xi, d_W, K, s, s_kind,
-                                                   scale * scale, partial);
+  const int s_kind = (s == std::floor(s) && s >= 1.0 && s <= 64.0) ? (int)s : 0;   // integer exponent, else 0
+  const double2* nu = reinterpret_cast<const double2*>(d_nuhat);
+  const double2* nu2 = reinterpret_cast<const double2*>(d_nuhat2);
+  if (M > 0)
+    reduce_terms_kernel<true><<<blocks, kThreads, 0, st>>>(nu, nu2, nullptr, nullptr, K, s, s_kind, scale * scale, M, h, partial);
+  else
+    reduce_terms_kernel<false><<<blocks, kThreads, 0, st>>>(nu, nu2, d_xi, d_W, K, s, s_kind, scale * scale, 0, 0.0, partial);
   SFD_TRY(launch_check("reduce_terms_kernel"));
   reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);
   return launch_check("reduce_final_kernel");
+}
+}  // namespace
+
+int reduce_enqueue(const double* d_nuhat, const double* d_xi, const double* d_W, int64_t K, double s, void* d_work,
+                   size_t work_bytes, cudaStream_t st, double** d_result, double scale, double pref,
+                   const double* d_nuhat2) {
+  return reduce_any(d_nuhat, d_xi, d_W, K, s, d_work, work_bytes, st, d_result, scale, pref, d_nuhat2, 0, 0.0);
+}
+
+int reduce_lattice_enqueue(const double* d_nuhat, int M, double xi_max, double s, void* d_work, size_t work_bytes,
+                           cudaStream_t st, double** d_result, double scale, double pref) {
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 1624, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..1624 (got %d)", M);
+  const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
+  return reduce_any(d_nuhat, nullptr, nullptr, K, s, d_work, work_bytes, st, d_result, scale, pref, nullptr, M,
+                    2.0 * xi_max / M);
 }
 
 }  // namespace sfd

@@ -58,6 +58,22 @@ def test_reduce_ex(sfd, orc, torch):
         assert abs(got - ref) <= 1e-12 * ref
 
 
+def test_reduce_lattice(sfd, orc, torch):
+    """sfd_reduce_lattice = sfd_reduce_ex on the expanded lattice, bit for bit; and the oracle within 1e-12."""
+    rng = np.random.default_rng(3)
+    for M, xm, s in ((8, 5.0, 10.0), (30, 2.5, 5.0), (22, 3.0, 1.5)):
+        K = (M + 1) ** 3
+        nu = rng.normal(size=K) + 1j * rng.normal(size=K)
+        nud = dev(torch, nu.view(np.float64).reshape(-1, 2))
+        xi, W = sfd.sfd_lattice_nodes_device(M, xm)
+        a = sfd.sfd_reduce_ex(nud, xi, W, s, 1 / (2 * np.pi), 1.0)
+        b = sfd.sfd_reduce_lattice(nud, M, xm, s, 1 / (2 * np.pi), 1.0)
+        assert a == b
+        xo, Wo = orc.lattice_nodes(M, xm)
+        ref = orc.reduce_ex(nu, xo, Wo, s, 1 / (2 * np.pi), 1.0)
+        assert abs(b - ref) <= 1e-12 * ref
+
+
 def _cloud(rng, J, centre, half):
     x = (rng.random((J, 3)) * 2 - 1) * np.asarray(half) + np.asarray(centre)
     w = rng.normal(size=J)
