@@ -7,13 +7,14 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "sfd_oracle.cpp")
+SRCS = [os.path.join(HERE, "sfd_oracle.cpp"), os.path.join(HERE, "sfd_oracle_exact.cpp")]
 LIB = os.path.join(HERE, "libsfd_oracle.so")
-CMD = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", SRC, "-o", LIB]
+# -lquadmath: sfd_oracle_exact.cpp evaluates the exact triangle transform (eq. 2.19) in binary128
+CMD = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", *SRCS, "-o", LIB, "-lquadmath"]
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < os.path.getmtime(SRC):
+    if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(s) for s in SRCS):
         subprocess.run(CMD, check=True)
     return LIB
 

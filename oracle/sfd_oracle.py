@@ -1,4 +1,4 @@
-"""numpy/ctypes face of the CPU oracle (oracle/sfd_oracle.cpp).  TEST INFRASTRUCTURE.
+"""numpy/ctypes face of the CPU oracle (oracle/sfd_oracle.cpp, sfd_oracle_exact.cpp).  TEST INFRASTRUCTURE.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import
 this module.  It never imports paper_2304_06340_b200 and the CUDA path never imports it.
@@ -28,6 +28,7 @@ _lib.orc_nodes.argtypes = [_dp, _i64, _ip, _i64, C.c_int, _dp, _dp]
 _lib.orc_gauss_legendre.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
 _lib.orc_freq_nodes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _dp, _dp]
 _lib.orc_direct_sum.argtypes = [_dp, _dp, _i64, _dp, _i64, _dp]
+_lib.orc_exact_ft.argtypes = [_dp, _i64, _ip, _i64, _dp, _i64, _dp]
 _lib.orc_sigma_hat.argtypes = [C.c_double]
 _lib.orc_sigma_hat.restype = C.c_double
 _lib.orc_reduce.argtypes = [_dp, _dp, _dp, _i64, C.c_double]
@@ -111,6 +112,17 @@ def direct_sum(x, w, xi):
     xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
     out = np.empty((len(xi), 2), np.float64)
     _chk(_lib.orc_direct_sum(x, w, len(w), xi, len(xi), out), "direct_sum")
+    return out.view(np.complex128).reshape(-1)
+
+
+def exact_ft(V, F, xi):
+    """Exact transform of the flat mesh's surface measure, sum over faces of P:128 eq. 2.19 (e^{-i xi.x} convention),
+    evaluated in binary128 and rounded: complex128[K]."""
+    V = np.ascontiguousarray(V, np.float64).reshape(-1, 3)
+    F = np.ascontiguousarray(F, np.int32).reshape(-1, 3)
+    xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
+    out = np.empty((len(xi), 2), np.float64)
+    _chk(_lib.orc_exact_ft(V, len(V), F, len(F), xi, len(xi), out), "exact_ft")
     return out.view(np.complex128).reshape(-1)
 
 
