@@ -175,6 +175,21 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
                               double s_paper, double xi_max, int32_t M, double eps, void* d_work, size_t work_bytes,
                               sfd_stream stream, double* h_norm, double* h_I);
 
+/* ---- exact transform of the flat mesh -------------------------------------------------------
+ * out_k = sum_f int_{Q_f} e^{-i xi_k.x} dS(x): the sum over the mesh's triangles of P:128 eq. 2.19 (e^{-i xi.x}
+ * convention, gamma = 2 area), the O(N_S N_F) direct summation of the prior art, evaluated as a second
+ * divided difference of exp so that no configuration -- xi orthogonal to an edge, xi along the normal, xi = 0, tiny
+ * faces -- loses accuracy (P:140 names the cancellation of the literal formula): ~1e-15 sum_f area_f absolute, plus the
+ * fp64 rounding of the phases xi.p.  No quadrature rule is involved; against sfd_nodes + sfd_surface_ft it isolates
+ * the triangle rule's error.  Device pointers; d_out complex128 [K]; a face with a vertex index outside [0, nV)
+ * poisons every output with NaN (as sfd_nodes does).  d_work: sfd_exact_ft_workspace(nF) bytes (80 B per face).
+ * With few frequencies the faces are split over CTAs and the partial sums meet in fp64 reductions whose order is not
+ * fixed (reproducible to rounding only).  Enqueues on `stream`. */
+int sfd_exact_ft_workspace(int64_t nF, size_t* bytes);
+int sfd_exact_ft(const double* d_vertices /*[nV][3]*/, int64_t nV, const int32_t* d_faces /*[nF][3]*/, int64_t nF,
+                 const double* d_xi /*[K][3]*/, int64_t K, double* d_out /*[K][2]*/, void* d_work, size_t work_bytes,
+                 sfd_stream stream);
+
 /* ---- two meshes against each other ------------------------------------------------------------------
  * I = (2 pi)^-3 sum_k W_k |nuhat_a,k - nuhat_b,k|^2 (1+|xi_k|^2)^-s: the squared H^{-s} distance between two atomic
  * measures whose transforms on the same nodes are given (two calls of sfd_surface_ft).  Same workspace, determinism

@@ -64,6 +64,8 @@ _SIGS = {
     "sfd_weak_distance_lattice_workspace": (C.c_int, [_i64, C.c_int, C.c_int32, _dbl, _dbl, _dbl, _P(_sz)]),
     "sfd_weak_distance_lattice": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, C.c_int32, _dbl, _vp, _sz, _vp,
                                             _P(_dbl), _P(_dbl)]),
+    "sfd_exact_ft_workspace": (C.c_int, [_i64, _P(_sz)]),
+    "sfd_exact_ft": (C.c_int, [_vp, _i64, _vp, _i64, _vp, _i64, _vp, _vp, _sz, _vp]),
     "sfd_reduce_pair": (C.c_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
     "sfd_surface_ft_host": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp]),
     "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
@@ -395,6 +397,20 @@ def sfd_weak_distance_lattice(V, F, rule, s_paper, xi_max, M, eps=0.0, work=None
                                         float(xi_max), int(M), float(eps), _ptr(work), work.numel(), _stream(),
                                         C.byref(d), C.byref(I)))
     return d.value, I.value
+
+
+def sfd_exact_ft(V, F, xi):
+    """Exact transform of the flat mesh, sum over faces of P:128 eq. 2.19 (e^{-i xi.x} convention): complex128[K]."""
+    _dev_f64(V, 3), _dev_f64(xi, 3)
+    assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous()
+    K = xi.shape[0]
+    wb = _sz()
+    _chk(_lib.sfd_exact_ft_workspace(F.shape[0], C.byref(wb)))
+    work = _work(wb.value, V.device)
+    out = torch.empty((K, 2), dtype=torch.float64, device=V.device)
+    _chk(_lib.sfd_exact_ft(_ptr(V), V.shape[0], _ptr(F), F.shape[0], _ptr(xi), K, _ptr(out), _ptr(work), work.numel(),
+                           _stream()))
+    return torch.view_as_complex(out) if K > 0 else torch.empty(0, dtype=torch.complex128, device=V.device)
 
 
 # ---- two meshes against each other (P:137, P:254) ----------------------------------------------------------------

@@ -245,6 +245,29 @@ int sfd_surface_ft(const double* d_x, const double* d_w, int64_t J, const double
   return rc;
 }
 
+// ---- exact triangle transform (S:8(f) NEXT-3) -------------------------------------------------------
+int sfd_exact_ft_workspace(int64_t nF, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_exact_ft_workspace: bytes is NULL");
+  SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
+  *bytes = exact_ft_workspace(nF);
+  return SFD_OK;
+}
+
+int sfd_exact_ft(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, const double* d_xi, int64_t K,
+                 double* d_out, void* d_work, size_t work_bytes, sfd_stream stream) {
+  SFD_REQUIRE(nF >= 0 && K >= 0 && nV >= 0, SFD_ERR_INVALID_ARG, "nV, nF and K must be >= 0");
+  if (K == 0) return SFD_OK;
+  SFD_REQUIRE(d_xi && d_out, SFD_ERR_NULL, "sfd_exact_ft: NULL frequency or output buffer");
+  SFD_REQUIRE(nF == 0 || (d_vertices && d_faces), SFD_ERR_NULL, "sfd_exact_ft: NULL mesh buffer");
+  cudaStream_t st = as_stream(stream);
+  const bool own_prof = !g_prof.active;
+  if (own_prof) prof_begin(st);
+  const int rc = exact_ft(d_vertices, nV, d_faces, nF, d_xi, K, d_out, d_work, work_bytes, st);
+  prof_mark("exact_ft", st);
+  if (own_prof) prof_end(st);
+  return rc;
+}
+
 // ---- A6 -------------------------------------------------------------------------------------------
 int sfd_reduce_workspace(int64_t K, size_t* bytes) {
   SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_reduce_workspace: bytes is NULL");

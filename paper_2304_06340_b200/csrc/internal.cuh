@@ -50,6 +50,11 @@ int reduce_lattice_enqueue(const double* d_nuhat, int M, double xi_max, double s
 // nodes.cu: the paper's cube lattice: xi' = 2 pi xi_ijk, W = w_ijk h^3
 int lattice_expand(int M, double xi_max, double* d_xi, double* d_W, cudaStream_t st);
 
+// ---- exact.cu: direct summation of the exact triangle transform (eq. 2.19; S:8(f) NEXT-3) ---------
+size_t exact_ft_workspace(int64_t nF);
+int exact_ft(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, const double* d_xi, int64_t K, double* d_out,
+             void* d_work, size_t work_bytes, cudaStream_t st);
+
 // ---- probe.cu: measured FP64 FMA peak of the device (the direct sum's roofline denominator) ----------
 int probe_fp64(int iters, cudaStream_t st, double* h_tflops, double* h_ms);
 
