@@ -45,9 +45,11 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (2 = the headline)")
     ap.add_argument("--impl", default="sfd", choices=["sfd", "reference"])
-    ap.add_argument("--workload", default="config", choices=["config", "fig4a", "fig4b"],
+    ap.add_argument("--workload", default="config", choices=["config", "fig4a", "fig4b", "exact_a", "exact_b"],
                     help="config: BASELINE.json config (default); fig4a / fig4b: the paper's own timing experiments "
-                         "(P:244: N = 7, M = 128 / N = 5, M = 416; xi_max = 5, 64-pt rule, eps 1e-7)")
+                         "(P:244: N = 7, M = 128 / N = 5, M = 416; xi_max = 5, 64-pt rule, eps 1e-7); exact_a / exact_b: "
+                         "the exact-formula direct summation the paper quotes from [38] (P:244: ~100,000 triangles, "
+                         "M = 100 / 80 triangles, M = 400)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -303,12 +305,47 @@ def run_paper(args):
     return 0
 
 
+def run_exact(args):
+    """Direct summation of the exact triangle transform (eq. 2.19) on the workloads the paper quotes from the prior
+    art [38]: "10 sec on NVIDIA Tesla V100 for 100 000 triangles (N ~ 6) and M = 100" and "roughly 0.1 sec for 80
+    triangles (N = 1) and M = 400".  Frequencies: the paper's lattice at xi_max = 5, resident in HBM."""
+    import torch
+    import paper_2304_06340_b200 as P
+    torch.cuda.set_device(0)
+    N, M, paper_s = (6, 100, 10.0) if args.workload == "exact_a" else (1, 400, 0.1)
+    V, F = P.sfd_mesh_icosphere(N)
+    xi, _ = P.sfd_lattice_nodes_device(M, 5.0)
+    nF, K = F.shape[0], xi.shape[0]
+    for _ in range(max(args.warmup, 3)):
+        out = P.sfd_exact_ft(V, F, xi)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches0 = P.sfd_launch_count()
+    for a, b in ev:
+        a.record()
+        out = P.sfd_exact_ft(V, F, xi)
+        b.record()
+    torch.cuda.synchronize()
+    launches = (P.sfd_launch_count() - launches0) // args.steps
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    pairs = float(nF) * float(K)
+    line = {"metric": "triangle x frequency pairs per second, exact-formula direct summation (P:128 eq. 2.19, P:244)",
+            "value": pairs / (ms * 1e-3), "unit": "pairs/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"icosphere N={N} ({nF} triangles) x lattice M={M}, xi_max=5 ({K} frequencies), "
+                                   f"{pairs:.3g} pairs", "paper_quote": {"seconds": paper_s, "gpu": "Tesla V100, code of [38]",
+                                                                         "note": "another machine and code: context only"}},
+            "seconds": ms * 1e-3, "checksum": float(out.abs().sum().item()), "gpu_launches": int(launches)}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.workload != "config":
-        return run_paper(args)
+        return run_exact(args) if args.workload.startswith("exact") else run_paper(args)
     r = run_sfd(args)
     P, torch, dist = r["P"], r["torch"], r["dist"]
     c, J, K, q = r["c"], r["J"], r["K"], r["q"]
