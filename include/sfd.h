@@ -127,6 +127,11 @@ int sfd_reduce(const double* d_nuhat /*[K][2]*/, const double* d_xi /*[K][3]*/, 
  * Distance in H^{-s} between the mesh's surface measure and the unit sphere's.  Runs A3,
  * the frequency quadrature, A4 (eps == 0) or A5 (eps > 0) and A6 on `stream`; synchronises; writes
  * sqrt(I) to *h_distance and I to *h_I (either may be NULL).  R > 0, s > 0.5.
+ * The ball rule is symmetric under xi -> -xi when n_phi is even (Gauss-Legendre nodes in cos(theta) are symmetric and
+ * phi + pi is a node), the surface measure is real, so nuhat(-xi) = conj nuhat(xi), and sigmahat is real and radial:
+ * mirror nodes contribute equal terms to I.  The call therefore generates, transforms and reduces only the
+ * sfd_weak_distance_targets(q) nodes with xi_3 >= 0, with doubled weights (a ring at cos(theta) = 0 keeps its own) --
+ * the same I up to rounding, half the work.  An odd n_phi uses every node.
  * The workspace is sized for meshes whose bounding box has half-width <= x_extent on every axis (1.0 for an
  * icosphere; only used when eps > 0); a wider mesh fails with SFD_ERR_WORKSPACE_TOO_SMALL. */
 int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps,
@@ -134,6 +139,9 @@ int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature*
 int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
                       double s, double R, const sfd_freq_quadrature* q, double eps, void* d_work,
                       size_t work_bytes, sfd_stream stream, double* h_distance, double* h_I);
+/* Number of frequency nodes sfd_weak_distance evaluates for the rule q (host-only): n_r ceil(n_theta/2) n_phi when
+ * n_phi is even, n_r n_theta n_phi otherwise. */
+int sfd_weak_distance_targets(const sfd_freq_quadrature* q, int64_t* K_eval);
 
 /* ---- the paper's own variant: cube lattice, trapezoidal rule, its norm convention ----
  * Lattice of P:156-166 eqs. 3.3-3.4: xi_ijk = (i,j,k) h, h = 2 xi_max / M, i,j,k = -M/2..M/2 (M even, 2..2046), with

@@ -53,6 +53,7 @@ _SIGS = {
     "sfd_reduce_workspace": (C.c_int, [_i64, _P(_sz)]),
     "sfd_reduce": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
     "sfd_weak_distance_workspace": (C.c_int, [_i64, C.c_int, _P(sfd_freq_quadrature), _dbl, _dbl, _dbl, _P(_sz)]),
+    "sfd_weak_distance_targets": (C.c_int, [_P(sfd_freq_quadrature), _P(_i64)]),
     "sfd_weak_distance": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl, _vp,
                                     _sz, _vp, _P(_dbl), _P(_dbl)]),
     "sfd_lattice_nodes": (C.c_int, [C.c_int32, _dbl, _vp, _vp]),
@@ -245,6 +246,13 @@ def sfd_weak_distance_workspace(nF, rule, q, R, eps, x_extent=1.0):
     _chk(_lib.sfd_weak_distance_workspace(int(nF), int(rule), C.byref(q), float(R), float(eps), float(x_extent),
                                           C.byref(wb)))
     return wb.value
+
+
+def sfd_weak_distance_targets(q):
+    """Number of frequency nodes sfd_weak_distance evaluates (the xi_3 >= 0 half of a rule with even n_phi)."""
+    k = _i64()
+    _chk(_lib.sfd_weak_distance_targets(C.byref(_quad(q)), C.byref(k)))
+    return k.value
 
 
 def sfd_weak_distance(V, F, rule, s, R, q, eps=0.0, work=None, x_extent=None):

@@ -224,8 +224,9 @@ int sfd_surface_ft_plan(int64_t J, int64_t K, const double X[3], const double S[
   return SFD_OK;
 }
 
-int sfd_surface_ft(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
-                   double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+namespace {
+int surface_ft_impl(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
+                    double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream, bool origin_centred) {
   SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
   SFD_TRY(check_eps(eps));
   if (K == 0) return SFD_OK;
@@ -239,10 +240,16 @@ int sfd_surface_ft(const double* d_x, const double* d_w, int64_t J, const double
     rc = direct_sum(d_x, d_w, J, d_xi, K, d_nuhat, d_work, work_bytes, st);
     prof_mark("direct_sum", st);
   } else {
-    rc = nufft3(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, st);
+    rc = nufft3(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, st, origin_centred);
   }
   if (own_prof) prof_end(st);
   return rc;
+}
+}  // namespace
+
+int sfd_surface_ft(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
+                   double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+  return surface_ft_impl(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, stream, false);
 }
 
 // ---- exact triangle transform (S:8(f) NEXT-3) -------------------------------------------------------
@@ -335,6 +342,13 @@ int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature*
   return SFD_OK;
 }
 
+int sfd_weak_distance_targets(const sfd_freq_quadrature* q, int64_t* K_eval) {
+  SFD_REQUIRE(K_eval, SFD_ERR_NULL, "sfd_weak_distance_targets: K_eval is NULL");
+  SFD_TRY(check_quadrature(q, 1.0));
+  *K_eval = (q->n_phi & 1) == 0 ? freq_half_count(q, 0, q->n_r) : (int64_t)q->n_r * q->n_theta * q->n_phi;
+  return SFD_OK;
+}
+
 int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
                       double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes,
                       sfd_stream stream, double* h_distance, double* h_I) {
@@ -358,11 +372,15 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
   prof_mark("nodes", st);
   FreqTables t;
   if (rc == SFD_OK) rc = freq_tables(q, R, t);
-  if (rc == SFD_OK) rc = freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st);
+  // The ball rule is symmetric under xi -> -xi (even n_phi) and the measure is real: the nodes with xi_3 >= 0 carry
+  // the whole sum with doubled weights (nodes.cu freq_expand), so only they are generated, transformed and reduced.
+  const bool half = (q->n_phi & 1) == 0;
+  const int64_t K = half ? freq_half_count(q, 0, q->n_r) : L.K;
+  if (rc == SFD_OK) rc = freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st, 0, -1, half);
   prof_mark("freq_nodes", st);
-  if (rc == SFD_OK) rc = sfd_surface_ft(x, w, L.J, xi, L.K, eps, nu, base + L.ft, work_bytes - L.ft, stream);
+  if (rc == SFD_OK) rc = surface_ft_impl(x, w, L.J, xi, K, eps, nu, base + L.ft, work_bytes - L.ft, stream, half);
   double* d_res = nullptr;
-  if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, L.K, s, base + L.red, L.red_bytes, st, &d_res);
+  if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, &d_res);
   prof_mark("reduce", st);
   double I = 0.0;
   if (rc == SFD_OK) {

@@ -24,8 +24,10 @@ int freq_tables(const sfd_freq_quadrature* q, double R, FreqTables& t);
 void gauss_legendre_host(int n, std::vector<long double>& t, std::vector<long double>& wt);
 size_t freq_tables_bytes(const sfd_freq_quadrature* q);
 // radial shells [a0, a1) only (a1 < 0: all of them)
+// half: only the nodes with xi_3 >= 0, weights doubled (nodes.cu freq_expand: exact for real measures, even n_phi)
 int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
-                size_t work_bytes, cudaStream_t st, int a0 = 0, int a1 = -1);
+                size_t work_bytes, cudaStream_t st, int a0 = 0, int a1 = -1, bool half = false);
+int64_t freq_half_count(const sfd_freq_quadrature* q, int a0, int a1);
 int rule_table_host(int rule, double* lam, double* om);
 int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rule, double* d_x, double* d_w,
           cudaStream_t st);
@@ -68,8 +70,10 @@ struct Nufft3Sizes {
   size_t work_bytes;   // total workspace
 };
 int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out);
+// origin_centred: take the targets' box as symmetric about the origin whatever their extents say (the half rule of
+// nodes.cu freq_expand: the strengths then stay real and the Hermitian half band is used)
 int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
-           double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st);
+           double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred = false);
 int nufft3_release_cache();
 // Type-1 NUFFT onto the lattice xi = 2 pi h m, m in [-M/2, M/2]^3 (eq. 3.6, eq. 3.7), lattice order of
 // lattice_expand.  *applicable = false (and nothing enqueued): the lattice is too coarse for the sources' extent or

@@ -162,16 +162,19 @@ void legendre_rule(int n, std::vector<long double>& t, std::vector<long double>&
 }
 
 // Nodes of the radial shells [a0, a1) (a0 = 0, a1 = n_r: the whole rule); output index k - a0 n_th n_ph.
+// half != 0: only the rings b >= n_th/2 (mu >= 0, the half-space xi_3 >= 0), weights doubled except on a ring that is
+// its own mirror image (mu = 0, odd n_th) -- see freq_expand().  Output index ((a - a0) nb + (b - b0)) n_ph + c.
 __global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restrict__ tab, int n_r, int n_th, int n_ph,
-                                                          int a0, int a1, double wph, double* __restrict__ xi,
+                                                          int a0, int a1, int half, double wph, double* __restrict__ xi,
                                                           double* __restrict__ W) {
-  const int64_t K = (int64_t)(a1 - a0) * n_th * n_ph;
+  const int b0 = half ? n_th / 2 : 0, nb = n_th - b0;
+  const int64_t K = (int64_t)(a1 - a0) * nb * n_ph;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= K) return;
   const int c = (int)(k % n_ph);
   const int64_t ab = k / n_ph;
-  const int b = (int)(ab % n_th);
-  const int a = a0 + (int)(ab / n_th);
+  const int b = b0 + (int)(ab % nb);
+  const int a = a0 + (int)(ab / nb);
   const double* r = tab;
   const double* wr = r + n_r;
   const double* mu = wr + n_r;
@@ -183,7 +186,10 @@ __global__ void __launch_bounds__(256) freq_expand_kernel(const double* __restri
   xi[3 * k + 0] = __dmul_rn(ra, __dmul_rn(st[b], cph[c]));
   xi[3 * k + 1] = __dmul_rn(ra, __dmul_rn(st[b], sph[c]));
   xi[3 * k + 2] = __dmul_rn(ra, mu[b]);
-  if (W) W[k] = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(wr[a], ra), ra), wmu[b]), wph);
+  if (W) {
+    const double wk = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(wr[a], ra), ra), wmu[b]), wph);
+    W[k] = (half && b != n_th - 1 - b) ? __dmul_rn(2.0, wk) : wk;
+  }
 }
 
 }  // namespace
@@ -279,11 +285,20 @@ size_t freq_tables_bytes(const sfd_freq_quadrature* q) {
   return align_up(sizeof(double) * (2 * (size_t)q->n_r + 3 * (size_t)q->n_theta + 2 * (size_t)q->n_phi));
 }
 
+// half: the rule is symmetric under xi -> -xi when n_phi is even (Gauss-Legendre in mu is symmetric, phi + pi is a
+// node), and for a real measure nuhat(-xi) = conj nuhat(xi), sigmahat is real and radial, so the terms
+// W_k |nuhat_k - sigmahat_k|^2 (1+|xi_k|^2)^-s of mirror nodes are equal: the sum over the half-space xi_3 >= 0 with
+// doubled weights is the sum over the ball.  K_half = (a1 - a0) ceil(n_th / 2) n_ph nodes are written.
+int64_t freq_half_count(const sfd_freq_quadrature* q, int a0, int a1) {
+  return (int64_t)(a1 - a0) * (q->n_theta - q->n_theta / 2) * q->n_phi;
+}
+
 int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi, double* d_W, void* d_work,
-                size_t work_bytes, cudaStream_t st, int a0, int a1) {
+                size_t work_bytes, cudaStream_t st, int a0, int a1, bool half) {
   if (a1 < 0) a1 = q->n_r;
   SFD_REQUIRE(0 <= a0 && a0 <= a1 && a1 <= q->n_r, SFD_ERR_INVALID_ARG, "radial range [%d,%d) outside [0,%d)", a0, a1,
               q->n_r);
+  SFD_REQUIRE(!half || (q->n_phi & 1) == 0, SFD_ERR_INVALID_ARG, "the half rule needs an even n_phi (got %d)", q->n_phi);
   SFD_REQUIRE(work_bytes >= freq_tables_bytes(q) && d_work, SFD_ERR_WORKSPACE_TOO_SMALL,
               "frequency quadrature needs %zu workspace bytes, got %zu", freq_tables_bytes(q), work_bytes);
   std::vector<double> h;
@@ -291,10 +306,10 @@ int freq_expand(const sfd_freq_quadrature* q, const FreqTables& t, double* d_xi,
   for (const auto* v : {&t.r, &t.wr, &t.mu, &t.st, &t.wmu, &t.cph, &t.sph}) h.insert(h.end(), v->begin(), v->end());
   // pageable source: the runtime stages the copy before returning, so `h` may die at scope exit
   SFD_CUDA_TRY(cudaMemcpyAsync(d_work, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-  const int64_t K = (int64_t)(a1 - a0) * q->n_theta * q->n_phi;
+  const int64_t K = half ? freq_half_count(q, a0, a1) : (int64_t)(a1 - a0) * q->n_theta * q->n_phi;
   if (K == 0) return SFD_OK;
   freq_expand_kernel<<<(unsigned)((K + 255) / 256), 256, 0, st>>>(static_cast<const double*>(d_work), q->n_r,
-                                                                   q->n_theta, q->n_phi, a0, a1, t.wph, d_xi, d_W);
+                                                                   q->n_theta, q->n_phi, a0, a1, half ? 1 : 0, t.wph, d_xi, d_W);
   return launch_check("freq_expand_kernel");
 }
 

@@ -321,7 +321,7 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
 namespace sfd {
 
 int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps, double* d_nuhat,
-           void* d_work, size_t work_bytes, cudaStream_t st) {
+           void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred) {
   if (K == 0) return SFD_OK;
   SFD_REQUIRE(J > 0, SFD_ERR_INVALID_ARG, "nufft3: J must be > 0 (the caller handles J == 0)");
   SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
@@ -351,7 +351,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     S[d] = (0.5 * (hb[9 + d] - hb[6 + d])) * (1.0 + 1e-12) + 1e-300;
     // targets centred at the origin up to rounding (the ball quadrature): snap D to 0 so that c'_j = w_j is real
     const double reach = std::fmax(std::fabs(hb[6 + d]), std::fabs(hb[9 + d]));
-    if (std::fabs(p.D[d]) <= 1e-9 * reach) {
+    if (origin_centred || std::fabs(p.D[d]) <= 1e-9 * reach) {
       p.D[d] = 0.0;
       S[d] = reach * (1.0 + 1e-12) + 1e-300;
     } else {

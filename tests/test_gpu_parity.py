@@ -262,3 +262,22 @@ def test_nufft_every_kernel_width(sfd, orc, torch, eps):
     _nufft_case(sfd, orc, torch, x, w, xi, eps)
     x, w, xi = workloads.random_cloud(400, 300)
     _nufft_case(sfd, orc, torch, x, w, xi, eps)
+
+
+@pytest.mark.parametrize("q", [(6, 8, 10), (5, 7, 12), (4, 6, 9)])
+@pytest.mark.parametrize("eps", [0.0, 1e-10])
+def test_weak_distance_half_rule_equals_full_rule(sfd, torch, q, eps):
+    """sfd_weak_distance evaluates only the nodes with xi_3 >= 0 (doubled weights) when n_phi is even; the composition
+    of the public stages over every node gives the same I: even n_theta, odd n_theta (a ring at mu = 0 that is its own
+    mirror image) and odd n_phi (no symmetry: every node)."""
+    V, F = sfd.sfd_mesh_icosphere(2)
+    R, s = 9.0, 2.0
+    x, w = sfd.sfd_nodes(V, F, 12)
+    xi, W = sfd.sfd_freq_nodes_device(q, R)
+    I_full = sfd.sfd_reduce(sfd.sfd_surface_ft(x, w, xi, eps), xi, W, s)
+    d, I = sfd.sfd_weak_distance(V, F, 12, s, R, q, eps)
+    K_eval = sfd.sfd_weak_distance_targets(q)
+    assert K_eval == (q[0] * (q[1] - q[1] // 2) * q[2] if q[2] % 2 == 0 else q[0] * q[1] * q[2])
+    tol = 1e-12 if eps == 0.0 else 1e-7
+    assert abs(I - I_full) <= tol * I_full, (I, I_full)
+

@@ -365,3 +365,26 @@ def test_quadratic_rate_and_survey_crosscheck(orc):
         assert abs(d[(level, 2.0)] - gold[level][1]) < 1e-9 * gold[level][1]
     slopes = [math.log2(d[(l - 1, 2.0)] / d[(l, 2.0)]) for l in range(2, 5)]
     assert all(1.9 <= s <= 2.1 for s in slopes), slopes
+
+
+def test_mirror_nodes_contribute_equal_terms(orc):
+    """What the CUDA path's half rule rests on, in the oracle's own terms: for even n_phi the ball rule is invariant under
+    xi -> -xi, node (a, b, c) <-> (a, n_th-1-b, c + n_phi/2), with equal weights, and for real weights w_j
+    nuhat(-xi) = conj nuhat(xi); so the sum over the nodes with mu >= 0 with doubled weights (single weights on a ring
+    at mu = 0) is the sum over all nodes."""
+    V, F = orc.mesh_icosphere(1)
+    x, w = orc.nodes(V, F, 6)
+    for n_r, n_th, n_ph in ((3, 4, 6), (2, 5, 8)):
+        xi, W = orc.freq_nodes(n_r, n_th, n_ph, 7.0)
+        k = np.arange(n_r * n_th * n_ph)
+        a, b, c = k // (n_th * n_ph), (k // n_ph) % n_th, k % n_ph
+        mirror = (a * n_th + (n_th - 1 - b)) * n_ph + (c + n_ph // 2) % n_ph
+        assert np.abs(xi[mirror] + xi).max() <= 1e-15 * 7.0 and np.abs(W[mirror] - W).max() <= 1e-15 * W.max()
+        nu = orc.direct_sum(x, w, xi)
+        assert np.abs(nu[mirror] - np.conj(nu)).max() <= 1e-13 * w.sum()
+        I_full = orc.reduce(nu, xi, W, 2.0)
+        keep = b >= n_th // 2
+        W2 = np.where(b == n_th - 1 - b, W, 2 * W)[keep]
+        I_half = orc.reduce(nu[keep], xi[keep], W2, 2.0)
+        assert abs(I_half - I_full) <= 1e-12 * I_full
+
