@@ -169,8 +169,8 @@ __device__ __forceinline__ void fused_stages(double2* __restrict__ a, const doub
 }
 
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
-// 1024 with one (long transforms): 32 warps per SM either way -- the stages are latency-bound (shared-memory and
-// twiddle loads feeding short FP64 chains), so occupancy is what buys throughput (profiles/r1c_nufft.md).
+// 1024 with one (long transforms): 32 warps per SM either way -- the stages are bound by dependent FP64 chains and
+// the shared-memory pipe, so occupancy is what buys throughput (profiles/r1c_after_rewrites.md, r1j_fft_phases.md).
 template <bool REAL_IN, bool CONTIG, int THREADS, int CG, bool FUSED>
 __global__ void __launch_bounds__(THREADS, (FUSED ? 512 : 1024) / THREADS)
 fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
