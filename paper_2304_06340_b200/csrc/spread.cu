@@ -300,19 +300,39 @@ spread_runs_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __
         footprint(r.u[d], W, i0, sv[d]);
       }
       __syncwarp();   // the previous chunk's sweep has finished reading kv
+      // phi is even, so interval W-1-a is interval a mirrored: P_{W-1-a}(s) = P_a(-s).  With P_a(s) = E(s^2) + s O(s^2)
+      // one pair of intervals costs two half-degree Horner chains per dimension instead of two full ones.
+      {
+        constexpr int QE = DEG & ~1, QO = (DEG - 1) | 1;   // highest even / odd power
+        const double z0 = sv[0] * sv[0], z1 = sv[1] * sv[1], z2 = sv[2] * sv[2];
+        const double cw = lane < nch ? r.re : 0.0;
 #pragma unroll
-      for (int a = 0; a < W; ++a) {
-        double k0 = s_pc[DEG * W + a], k1 = k0, k2 = k0;
+        for (int a = 0; a < (W + 1) / 2; ++a) {
+          double e0 = s_pc[QE * W + a], e1 = e0, e2 = e0;
 #pragma unroll
-        for (int q = DEG - 1; q >= 0; --q) {
-          const double cq = s_pc[q * W + a];
-          k0 = __fma_rn(k0, sv[0], cq);
-          k1 = __fma_rn(k1, sv[1], cq);
-          k2 = __fma_rn(k2, sv[2], cq);
+          for (int q = QE - 2; q >= 0; q -= 2) {
+            const double cq = s_pc[q * W + a];
+            e0 = __fma_rn(e0, z0, cq);
+            e1 = __fma_rn(e1, z1, cq);
+            e2 = __fma_rn(e2, z2, cq);
+          }
+          double o0 = s_pc[QO * W + a], o1 = o0, o2 = o0;
+#pragma unroll
+          for (int q = QO - 2; q >= 1; q -= 2) {
+            const double cq = s_pc[q * W + a];
+            o0 = __fma_rn(o0, z0, cq);
+            o1 = __fma_rn(o1, z1, cq);
+            o2 = __fma_rn(o2, z2, cq);
+          }
+          kv[(0 * W + a) * PITCH + lane] = __fma_rn(sv[0], o0, e0) * cw;
+          kv[(1 * W + a) * PITCH + lane] = __fma_rn(sv[1], o1, e1);
+          kv[(2 * W + a) * PITCH + lane] = __fma_rn(sv[2], o2, e2);
+          if (a != W - 1 - a) {
+            kv[(0 * W + (W - 1 - a)) * PITCH + lane] = __fma_rn(-sv[0], o0, e0) * cw;
+            kv[(1 * W + (W - 1 - a)) * PITCH + lane] = __fma_rn(-sv[1], o1, e1);
+            kv[(2 * W + (W - 1 - a)) * PITCH + lane] = __fma_rn(-sv[2], o2, e2);
+          }
         }
-        kv[(0 * W + a) * PITCH + lane] = lane < nch ? k0 * r.re : 0.0;
-        kv[(1 * W + a) * PITCH + lane] = k1;
-        kv[(2 * W + a) * PITCH + lane] = k2;
       }
       __syncwarp();
 #pragma unroll 2
