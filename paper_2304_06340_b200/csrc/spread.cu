@@ -4,9 +4,9 @@
 //
 // The paper's GPU library spreads bin-sorted subproblems in shared memory with atomics and had to fall back to
 // single precision because fp64 subgrids did not fit.  Here:
-//   * one persistent CTA per SM pulls work items (an occupied bin, or a slice of <= kSrcCap sources of a heavy bin)
-//     from a device-side queue; the bin's padded subgrid lives in up to ~200 KB of shared memory in fp64 (real when
-//     the strengths are real, i.e. ball-centred targets; complex otherwise);
+//   * persistent CTAs (two per SM up to w = 11, one beyond) pull work items (an occupied bin, or a slice of <= kSrcCap
+//     sources of a heavy bin) from a device-side queue; the bin's padded subgrid lives in up to ~100 / ~200 KB of shared
+//     memory in fp64 (real when the strengths are real, i.e. ball-centred targets; complex otherwise);
 //   * no atomics in shared memory: x-plane ix of the subgrid is owned by warp ix mod W -- an absolute assignment, the
 //     same for every source -- so the W planes of a footprint go to the W warps of the CTA and no two warps ever
 //     touch the same cell; inside a warp the 32 lanes cover the W x W cells of the plane;
@@ -31,7 +31,13 @@ namespace sfd {
 namespace {
 
 constexpr int kChunk = 32;               // sources whose 3W kernel values are tabulated at a time (one per lane)
-constexpr int kSmemBytes = 200 * 1024;   // subgrid budget
+constexpr int kSmemBytes = 200 * 1024;   // subgrid budget of a CTA that has the SM to itself
+// Kernels up to w = 11 run two CTAs per SM on half the budget each: the sweep is latency-bound and every warp walks
+// every source of its CTA's item, so a second, independent CTA doubles the sources in flight.  Measured: spread
+// 0.93 -> 0.76 ms at w = 7 (config 3), 3.45 -> 3.06 ms at w = 10 (config 4), 17.1 -> 16.5 ms at w = 11 (config 5);
+// at w = 13 the 78-register budget spills and the gain is within the noise, so wider kernels keep one CTA.
+constexpr int kTwoCtaMaxW = 11;
+constexpr int ctas_per_sm(int w) { return w <= kTwoCtaMaxW ? 2 : 1; }
 
 struct ChunkTables {
   double k[3][kChunk][16];   // kernel values per dimension
@@ -40,7 +46,7 @@ struct ChunkTables {
 };
 
 template <int W, bool REAL, bool RUNS>
-__global__ void __launch_bounds__(32 * W, 1)
+__global__ void __launch_bounds__(32 * W, ctas_per_sm(W))
 spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restrict__ src,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
               const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
@@ -227,10 +233,11 @@ int launch(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const i
            double* d_grid, size_t smem, cudaStream_t st) {
   static bool attr = false;
   if (!attr) {
-    SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL, RUNS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 2048));
+    SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL, RUNS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (227 * 1024 - 2048) / ctas_per_sm(W) - 1024));
     attr = true;
   }
-  spread_kernel<W, REAL, RUNS><<<num_sms(), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
+  spread_kernel<W, REAL, RUNS><<<num_sms() * ctas_per_sm(W), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
                                                                 d_n_items, d_counter, d_grid);
   return launch_check("spread_kernel");
 }
@@ -401,7 +408,7 @@ int spread_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, co
 // shared-memory budget allows (at most 24: the sources lie on a shell, and smaller bins balance better).
 void spread_bins(int w, bool real_c, int bs[3]) {
   const int cell = real_c ? 8 : 16;
-  const int cap = (kSmemBytes - (int)sizeof(ChunkTables)) / cell;
+  const int cap = (kSmemBytes / ctas_per_sm(w) - (int)sizeof(ChunkTables)) / cell;
   double best = -1.0;
   for (int bz = real_c ? 16 : 8; bz <= 16; bz += 8) {
     const int pz = bz + w;
@@ -426,7 +433,7 @@ int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const i
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_grid, cudaStream_t st) {
   const size_t smem = spread_smem_bytes(p);
-  SFD_REQUIRE(smem <= 227 * 1024 - 2048 && p.bs[2] + p.w <= 32, SFD_ERR_INVALID_ARG,
+  SFD_REQUIRE(smem <= (size_t)((227 * 1024 - 2048) / ctas_per_sm(p.w) - 1024) && p.bs[2] + p.w <= 32, SFD_ERR_INVALID_ARG,
               "spread subgrid does not fit shared memory (%zu B)", smem);
   SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
 #define SFD_SPREAD_ARGS p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_grid, smem, st
