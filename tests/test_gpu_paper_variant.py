@@ -143,6 +143,27 @@ def test_clustered_sources_type3(sfd, orc, torch, centre, eps):
     assert np.abs(got - ref).max() <= 10 * eps * np.abs(w).sum()
 
 
+def test_surface_ft_lattice_edge_cases(sfd, orc, torch):
+    """No sources, one source, all sources at one point, the smallest lattice, a loose tolerance."""
+    xi, _ = orc.lattice_nodes(8, 1.5)
+    empty = torch.empty((0, 3), dtype=torch.float64, device="cuda")
+    nu = sfd.sfd_surface_ft_lattice(empty, torch.empty(0, dtype=torch.float64, device="cuda"), 8, 1.5, 1e-9)
+    assert nu.shape[0] == 729 and nu.abs().max().item() == 0.0
+    x1 = np.array([[0.3, -0.2, 0.5]])
+    got = sfd.sfd_surface_ft_lattice(dev(torch, x1), dev(torch, np.array([2.0])), 8, 1.5, 1e-9).cpu().numpy()
+    assert np.abs(got - 2.0 * np.exp(-1j * xi @ x1[0])).max() <= 40 * 1e-9 * 2.0      # single source: R10
+    xs = np.repeat(x1, 500, axis=0)
+    ws = np.linspace(0.5, 1.5, 500)
+    got = sfd.sfd_surface_ft_lattice(dev(torch, xs), dev(torch, ws), 8, 1.5, 1e-9).cpu().numpy()
+    assert np.abs(got - ws.sum() * np.exp(-1j * xi @ x1[0])).max() <= 40 * 1e-9 * ws.sum()
+    rng = np.random.default_rng(4)
+    x, w = _cloud(rng, 800, (0, 0, 0), (1, 1, 1))
+    for M, xm, eps in ((2, 0.4, 1e-9), (8, 1.5, 1e-1)):
+        xi, _ = orc.lattice_nodes(M, xm)
+        got = sfd.sfd_surface_ft_lattice(dev(torch, x), dev(torch, w), M, xm, eps).cpu().numpy()
+        assert np.abs(got - orc.direct_sum(x, w, xi)).max() <= 10 * eps * np.abs(w).sum()
+
+
 def test_surface_ft_lattice_is_the_type1_path(sfd, torch):
     """The stage list of the last call shows which transform ran: no interpolation stage on the type-1 path."""
     rng = np.random.default_rng(5)
