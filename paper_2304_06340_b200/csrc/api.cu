@@ -226,7 +226,8 @@ int sfd_surface_ft_plan(int64_t J, int64_t K, const double X[3], const double S[
 
 namespace {
 int surface_ft_impl(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
-                    double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream, bool origin_centred) {
+                    double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream, bool origin_centred,
+                    const ExtentHint* hint = nullptr) {
   SFD_REQUIRE(J >= 0 && K >= 0, SFD_ERR_INVALID_ARG, "J and K must be >= 0");
   SFD_TRY(check_eps(eps));
   if (K == 0) return SFD_OK;
@@ -240,7 +241,7 @@ int surface_ft_impl(const double* d_x, const double* d_w, int64_t J, const doubl
     rc = direct_sum(d_x, d_w, J, d_xi, K, d_nuhat, d_work, work_bytes, st);
     prof_mark("direct_sum", st);
   } else {
-    rc = nufft3(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, st, origin_centred);
+    rc = nufft3(d_x, d_w, J, d_xi, K, eps, d_nuhat, d_work, work_bytes, st, origin_centred, hint);
   }
   if (own_prof) prof_end(st);
   return rc;
@@ -378,7 +379,12 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
   const int64_t K = half ? freq_half_count(q, 0, q->n_r) : L.K;
   if (rc == SFD_OK) rc = freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st, 0, -1, half);
   prof_mark("freq_nodes", st);
-  if (rc == SFD_OK) rc = surface_ft_impl(x, w, L.J, xi, K, eps, nu, base + L.ft, work_bytes - L.ft, stream, half);
+  // extents without a pass over the atoms and the nodes: the atoms lie in the hull of the vertices, the nodes in [-R, R]^3
+  ExtentHint hint;
+  hint.d_hull = d_vertices;
+  hint.n_hull = nV;
+  hint.target_reach = R;
+  if (rc == SFD_OK) rc = surface_ft_impl(x, w, L.J, xi, K, eps, nu, base + L.ft, work_bytes - L.ft, stream, true, &hint);
   double* d_res = nullptr;
   if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, &d_res);
   prof_mark("reduce", st);
@@ -466,14 +472,14 @@ int lattice_ft_bytes(int64_t J, int M, double xi_max, const double X[3], double 
 // nuhat on the lattice; d_xi_buf = room for the expanded nodes (24 K bytes), filled and used only by the type-3 /
 // direct path.
 int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi_max, double eps, double* d_xi_buf,
-               double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream) {
+               double* d_nuhat, void* d_work, size_t work_bytes, sfd_stream stream, const ExtentHint* hint = nullptr) {
   const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
   cudaStream_t st = as_stream(stream);
   if (eps > 0.0 && J > 0) {
     const bool own_prof = !g_prof.active;
     if (own_prof) prof_begin(st);
     bool ok = false;
-    const int rc = nufft1_lattice(d_x, d_w, J, M, 2.0 * xi_max / M, eps, d_nuhat, d_work, work_bytes, st, &ok);
+    const int rc = nufft1_lattice(d_x, d_w, J, M, 2.0 * xi_max / M, eps, d_nuhat, d_work, work_bytes, st, &ok, hint);
     if (own_prof) prof_end(st);
     if (rc != SFD_OK || ok) return rc;
   }
@@ -588,7 +594,10 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   prof_mark("nodes", st);
   // the lattice nodes are expanded only if the transform falls back to type-3 / direct (lattice_ft); the reduction
   // recomputes them from the index
-  if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream);
+  ExtentHint hint;   // the atoms lie in the hull of the vertices
+  hint.d_hull = d_vertices;
+  hint.n_hull = nV;
+  if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream, &hint);
   double* d_res = nullptr;
   // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
   if (rc == SFD_OK)

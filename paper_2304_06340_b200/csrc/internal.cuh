@@ -70,16 +70,25 @@ struct Nufft3Sizes {
   size_t work_bytes;   // total workspace
 };
 int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out);
+// What a caller may know about the extents, which replaces the reductions over all sources / all targets:
+//   d_hull / n_hull: device points whose bounding box contains every source (the vertices of the mesh the atoms are
+//     convex combinations of);  target_reach > 0: every target lies in [-target_reach, target_reach]^3.
+struct ExtentHint {
+  const double* d_hull = nullptr;
+  int64_t n_hull = 0;
+  double target_reach = 0.0;
+};
 // origin_centred: take the targets' box as symmetric about the origin whatever their extents say (the half rule of
 // nodes.cu freq_expand: the strengths then stay real and the Hermitian half band is used)
 int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps,
-           double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred = false);
+           double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred = false,
+           const ExtentHint* hint = nullptr);
 int nufft3_release_cache();
 // Type-1 NUFFT onto the lattice xi = 2 pi h m, m in [-M/2, M/2]^3 (eq. 3.6, eq. 3.7), lattice order of
 // lattice_expand.  *applicable = false (and nothing enqueued): the lattice is too coarse for the sources' extent or
 // too long for the in-shared-memory FFT; the caller then runs the type-3 transform on the lattice nodes.
 int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double eps, bool* applicable, size_t* bytes);
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
-                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable);
+                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint = nullptr);
 
 }  // namespace sfd

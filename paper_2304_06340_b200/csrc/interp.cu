@@ -94,7 +94,6 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
     const int start = item_start[item], count = item_count[item];
     const int bz = bin % p.nbt[2], by = (bin / p.nbt[2]) % p.nbt[1], bx = bin / (p.nbt[2] * p.nbt[1]);
     const int ox = p.t0[0] + bx * p.bt[0] - W / 2, oy = p.t0[1] + by * p.bt[1] - W / 2, oz = p.t0[2] + bz * p.bt[2] - W / 2;
-    const int bx0 = ox - p.lo[0], by0 = oy - p.lo[1], bz0 = oz - p.lo[2];   // subgrid origin in band coordinates
 
     // stage the subgrid with 16-byte asynchronous copies (LDGSTS; zero-filled outside the band): every warp issues
     // all of its rows back to back and waits once, so the staging runs at L2 bandwidth instead of one round trip per

@@ -171,26 +171,29 @@ namespace {
 // exp(beta (cos(theta) - 1)) cos(kappa sin(theta)) cos(theta) is analytic on [0, pi/2] and 64 Gauss-Legendre nodes
 // in long double give it to ~1e-18.  Sampled at the Chebyshev nodes of y = 2 (kappa/kmax)^2 - 1 and turned into the
 // Chebyshev coefficients that the device evaluates (nufft3.cuh ChebTable).
+long double half_w_phihat_host(const N3Params& p, const std::vector<long double>& gt, const std::vector<long double>& gw,
+                               long double kappa) {
+  const long double pi = 3.14159265358979323846264338327950288L;
+  long double acc = 0.0L;
+  for (size_t i = 0; i < gt.size(); ++i) {
+    const long double th = (gt[i] + 1.0L) * pi / 4.0L;
+    const long double om = gw[i] * pi / 4.0L;
+    acc += (long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)) * cosl(kappa * sinl(th));
+  }
+  return acc;
+}
+
 void make_cheb(const N3Params& p, ChebTable* t) {
   const int nq = 64;
   std::vector<long double> gt, gw;
   gauss_legendre_host(nq, gt, gw);
   const long double pi = 3.14159265358979323846264338327950288L;
   const long double kmax = (long double)p.w * pi / 4.0L * (1.0L + 1e-9L);
-  auto F = [&](long double kappa) {
-    long double acc = 0.0L;
-    for (int i = 0; i < nq; ++i) {
-      const long double th = (gt[i] + 1.0L) * pi / 4.0L;
-      const long double om = gw[i] * pi / 4.0L;
-      acc += (long double)p.w * om * cosl(th) * expl((long double)p.beta * (cosl(th) - 1.0L)) * cosl(kappa * sinl(th));
-    }
-    return acc;
-  };
   const int n = kChebN;
   std::vector<long double> fv(n);
   for (int k = 0; k < n; ++k) {
     const long double y = cosl(pi * (2 * k + 1) / (2.0L * n));
-    fv[k] = F(kmax * sqrtl((y + 1.0L) / 2.0L));
+    fv[k] = half_w_phihat_host(p, gt, gw, kmax * sqrtl((y + 1.0L) / 2.0L));
   }
   for (int j = 0; j < n; ++j) {
     long double acc = 0.0L;
@@ -321,7 +324,7 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
 namespace sfd {
 
 int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps, double* d_nuhat,
-           void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred) {
+           void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred, const ExtentHint* hint) {
   if (K == 0) return SFD_OK;
   SFD_REQUIRE(J > 0, SFD_ERR_INVALID_ARG, "nufft3: J must be > 0 (the caller handles J == 0)");
   SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
@@ -331,12 +334,20 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   int32_t* d_ctl = reinterpret_cast<int32_t*>(base + 128);
   double* d_scratch = reinterpret_cast<double*>(base + 1024);
 
-  // A5-1: extents of sources and targets (the one host synchronisation of the transform)
-  SFD_TRY(bounds_minmax(d_x, J, d_bounds, d_scratch, st));
-  SFD_TRY(bounds_minmax(d_xi, K, d_bounds + 6, d_scratch, st));
+  // A5-1: extents of sources and targets (the one host synchronisation of the transform); a caller that knows a
+  // hull of the sources or the reach of the targets saves the pass over all of them
+  const bool hull = hint && hint->d_hull && hint->n_hull > 0;
+  const bool reach_known = hint && hint->target_reach > 0.0;
+  SFD_TRY(bounds_minmax(hull ? hint->d_hull : d_x, hull ? hint->n_hull : J, d_bounds, d_scratch, st));
+  if (!reach_known) SFD_TRY(bounds_minmax(d_xi, K, d_bounds + 6, d_scratch, st));
   double hb[12];
-  SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, sizeof(hb), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, (reach_known ? 6 : 12) * sizeof(double), cudaMemcpyDeviceToHost, st));
   SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  if (reach_known)
+    for (int d = 0; d < 3; ++d) {
+      hb[6 + d] = -hint->target_reach;
+      hb[9 + d] = hint->target_reach;
+    }
   prof_mark("bounds", st);
 
   N3Params p{};
@@ -523,7 +534,7 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
 }
 
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
-                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable) {
+                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint) {
   SFD_REQUIRE(J > 0 && applicable, SFD_ERR_INVALID_ARG, "nufft1_lattice: J must be > 0");
   SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
               "type-1 NUFFT needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
@@ -532,7 +543,8 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   int32_t* d_ctl = reinterpret_cast<int32_t*>(base + 128);
   double* d_scratch = reinterpret_cast<double*>(base + 1024);
 
-  SFD_TRY(bounds_minmax(d_x, J, d_bounds, d_scratch, st));
+  const bool hull = hint && hint->d_hull && hint->n_hull > 0;
+  SFD_TRY(bounds_minmax(hull ? hint->d_hull : d_x, hull ? hint->n_hull : J, d_bounds, d_scratch, st));
   double hb[6];
   SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, sizeof(hb), cudaMemcpyDeviceToHost, st));
   SFD_CUDA_TRY(cudaStreamSynchronize(st));
