@@ -68,6 +68,16 @@ struct Arena {
 
 int num_sms();
 
+// Kernel attributes (the opt-in to > 48 KB of dynamic shared memory) are per device: true when the calling thread has
+// not yet seen the current device with this slot (`last` is a static thread_local int initialised to -1).
+inline bool first_use_on_device(int& last) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return true;
+  if (last == dev) return false;
+  last = dev;
+  return true;
+}
+
 // stage timing (sfd_set_profiling)
 void prof_begin(cudaStream_t st);
 void prof_mark(const char* name, cudaStream_t st);

@@ -231,10 +231,9 @@ template <int W>
 int launch(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_G, size_t smem, cudaStream_t st) {
-  static bool attr = false;
-  if (!attr) {
+  static thread_local int attr_dev = -1;
+  if (first_use_on_device(attr_dev)) {
     SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
-    attr = true;
   }
   interp_kernel<W><<<num_sms(), 32 * kWarps, smem, st>>>(p, d_ptab, reinterpret_cast<const double2*>(d_v), d_tgt,
                                                         d_item_bin, d_item_start, d_item_count, d_n_items, d_counter,

@@ -231,11 +231,10 @@ template <int W, bool REAL, bool RUNS>
 int launch(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_grid, size_t smem, cudaStream_t st) {
-  static bool attr = false;
-  if (!attr) {
+  static thread_local int attr_dev = -1;
+  if (first_use_on_device(attr_dev)) {
     SFD_CUDA_TRY(cudaFuncSetAttribute(spread_kernel<W, REAL, RUNS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (227 * 1024 - 2048) / ctas_per_sm(W) - 1024));
-    attr = true;
   }
   spread_kernel<W, REAL, RUNS><<<num_sms() * ctas_per_sm(W), 32 * W, smem, st>>>(p, d_ptab, d_src, d_item_bin, d_item_start, d_item_count,
                                                                 d_n_items, d_counter, d_grid);
@@ -374,10 +373,9 @@ int launch_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, co
                 const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
                 double* d_grid, cudaStream_t st) {
   constexpr size_t smem = ((size_t)(W + 4) * W + (size_t)kRunWarps * 3 * W * 33) * sizeof(double);
-  static bool attr = false;
-  if (!attr) {
+  static thread_local int attr_dev = -1;
+  if (first_use_on_device(attr_dev)) {
     SFD_CUDA_TRY(cudaFuncSetAttribute(spread_runs_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
   }
   spread_runs_kernel<W><<<num_sms(), 32 * kRunWarps, smem, st>>>(p, d_ptab, d_src, d_item_key, d_item_start, d_item_count,
                                                               d_n_items, d_counter, d_grid);
