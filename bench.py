@@ -420,7 +420,7 @@ def main():
                     "frac": ach / fp64_tf,
                     # DRAM bytes per launch from the ncu --set full capture of this kernel on this workload
                     # (profiles/r1e_direct_sum_table.md: 26.2 MB read + 0.54 MB written; config 2 only)
-                    "traffic": 26743808 if args.config == 2 else None,
+                    "traffic": 13807360 if args.config == 2 else None,   # dram read + write of one launch, profiles/r1i (ncu --set full)
                     "peak_source": "measured live by sfd_probe_fp64 (dependency-free DFMA loop on all SMs)",
                     "peak_derived": 2 * FP64_LANES_PER_SM * 148 * sm_mhz * 1e6 * 1e-12,
                     "pipe_frac": (DFMA_PER_PAIR + DMUL_DADD_PER_PAIR) * J * K / (dms * 1e-3) /
