@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstring>
 
+#include "atoms.cuh"
 #include "internal.cuh"
 
 namespace sfd {
@@ -590,14 +591,24 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   double* xi = reinterpret_cast<double*>(base + L.xi);
   double* nu = reinterpret_cast<double*>(base + L.nu);
   prof_begin(st);
-  int rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
-  prof_mark("nodes", st);
-  // the lattice nodes are expanded only if the transform falls back to type-3 / direct (lattice_ft); the reduction
-  // recomputes them from the index
   ExtentHint hint;   // the atoms lie in the hull of the vertices
   hint.d_hull = d_vertices;
   hint.n_hull = nV;
-  if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream, &hint);
+  int rc = SFD_OK;
+  bool done = false;
+  if (eps > 0.0 && L.J > 0) {
+    // the paper's transform, with the atoms generated inside its sort kernels: (x, w) are never materialised
+    const MeshAtoms mesh{d_vertices, nV, d_faces, nF, rule};
+    rc = nufft1_lattice(nullptr, nullptr, L.J, M, 2.0 * xi_max / M, eps, nu, base + L.ft, work_bytes - L.ft, st, &done,
+                        &hint, &mesh);
+  }
+  if (rc == SFD_OK && !done) {
+    // direct sum, or a lattice too coarse for the type-1 transform: materialise the atoms; the lattice nodes are
+    // expanded inside lattice_ft only if the transform needs them (the reduction recomputes them from the index)
+    rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
+    prof_mark("nodes", st);
+    if (rc == SFD_OK) rc = lattice_ft(x, w, L.J, M, xi_max, eps, xi, nu, base + L.ft, work_bytes - L.ft, stream, &hint);
+  }
   double* d_res = nullptr;
   // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
   if (rc == SFD_OK)

@@ -88,7 +88,13 @@ int nufft3_release_cache();
 // lattice_expand.  *applicable = false (and nothing enqueued): the lattice is too coarse for the sources' extent or
 // too long for the in-shared-memory FFT; the caller then runs the type-3 transform on the lattice nodes.
 int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double eps, bool* applicable, size_t* bytes);
+// mesh != nullptr: the sources are the atoms of that mesh (J = nF * rule), generated inside the sort kernels; d_x and
+// d_w are not read.
+struct MeshAtoms;
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
-                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint = nullptr);
+                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint = nullptr,
+                   const MeshAtoms* mesh = nullptr);
+// nodes.cu: the rule as four columns lam0[Q], lam1[Q], lam2[Q], om[Q] (4 * rule doubles) in device memory
+int rule_table_device(int rule, double* d_tab, cudaStream_t st);
 
 }  // namespace sfd

@@ -6,6 +6,7 @@
 #include <tuple>
 #include <vector>
 
+#include "atoms.cuh"
 #include "internal.cuh"
 
 namespace sfd {
@@ -75,44 +76,19 @@ __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V
                                                     double* __restrict__ w) {
   __shared__ double sx[3 * 256];
   // the rule, one array per column: a warp's 32 atoms read 32 different rows, which the constant cache would serialise
-  __shared__ double s_rule[4][Q];
+  __shared__ double s_rule[4 * Q];
   {
     const RuleTable& R = c_rule[Q == 6 ? 0 : (Q == 12 ? 1 : 2)];
-    for (int t = threadIdx.x; t < 4 * Q; t += 256) s_rule[t / Q][t % Q] = t / Q < 3 ? R.lam[t % Q][t / Q] : R.om[t % Q];
+    for (int t = threadIdx.x; t < 4 * Q; t += 256) s_rule[t] = t / Q < 3 ? R.lam[t % Q][t / Q] : R.om[t % Q];
   }
   __syncthreads();
   const int64_t j0 = (int64_t)blockIdx.x * 256;
   const int64_t j = j0 + threadIdx.x;
   const int64_t J = nF * Q;
   if (j < J) {
-    const int64_t f = j / Q;
-    const int i = (int)(j - f * Q);
-    const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
-    const double nan = __longlong_as_double(0x7ff8000000000000LL);
-    if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
-      sx[3 * threadIdx.x] = sx[3 * threadIdx.x + 1] = sx[3 * threadIdx.x + 2] = nan;
-      w[j] = nan;
-    } else {
-      double p0[3], p1[3], p2[3], e1[3], e2[3];
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        p0[c] = V[3 * (int64_t)i0 + c];
-        p1[c] = V[3 * (int64_t)i1 + c];
-        p2[c] = V[3 * (int64_t)i2 + c];
-        e1[c] = __dsub_rn(p1[c], p0[c]);
-        e2[c] = __dsub_rn(p2[c], p0[c]);
-      }
-      const double cx = __dsub_rn(__dmul_rn(e1[1], e2[2]), __dmul_rn(e1[2], e2[1]));
-      const double cy = __dsub_rn(__dmul_rn(e1[2], e2[0]), __dmul_rn(e1[0], e2[2]));
-      const double cz = __dsub_rn(__dmul_rn(e1[0], e2[1]), __dmul_rn(e1[1], e2[0]));
-      const double n2 = __dadd_rn(__dadd_rn(__dmul_rn(cx, cx), __dmul_rn(cy, cy)), __dmul_rn(cz, cz));
-      const double area = __dmul_rn(0.5, __dsqrt_rn(n2));
-      const double l0 = s_rule[0][i], l1 = s_rule[1][i], l2 = s_rule[2][i];
-#pragma unroll
-      for (int c = 0; c < 3; ++c)
-        sx[3 * threadIdx.x + c] = __dadd_rn(__dadd_rn(__dmul_rn(l0, p0[c]), __dmul_rn(l1, p1[c])), __dmul_rn(l2, p2[c]));
-      w[j] = __dmul_rn(s_rule[3][i], area);
-    }
+    double wj;
+    atom_eval(V, nV, F, j, Q, s_rule, sx[3 * threadIdx.x], sx[3 * threadIdx.x + 1], sx[3 * threadIdx.x + 2], wj);
+    w[j] = wj;
   }
   __syncthreads();
   const int64_t n = 3 * min((int64_t)256, J - j0);
@@ -321,6 +297,21 @@ int rule_table_host(int rule, double* lam, double* om) {
     for (int c = 0; c < 3; ++c) lam[3 * i + c] = t.lam[i][c];
     om[i] = t.om[i];
   }
+  return SFD_OK;
+}
+
+// The rule as four columns lam0[Q], lam1[Q], lam2[Q], om[Q] in device memory (atoms.cuh atom_eval).
+int rule_table_device(int rule, double* d_tab, cudaStream_t st) {
+  SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
+  RuleTable t;
+  fill_rule(rule, t);
+  double h[4 * 64];
+  for (int i = 0; i < rule; ++i) {
+    for (int c = 0; c < 3; ++c) h[c * rule + i] = t.lam[i][c];
+    h[3 * rule + i] = t.om[i];
+  }
+  // pageable source: staged by the runtime before the call returns
+  SFD_CUDA_TRY(cudaMemcpyAsync(d_tab, h, sizeof(double) * 4 * rule, cudaMemcpyHostToDevice, st));
   return SFD_OK;
 }
 

@@ -20,6 +20,7 @@
 #include <tuple>
 #include <vector>
 
+#include "atoms.cuh"
 #include "fft.cuh"
 #include "internal.cuh"
 #include "nufft3.cuh"
@@ -31,8 +32,9 @@ constexpr double kPi = 3.14159265358979323846;
 constexpr int kSrcCap = 1024;   // sources per spread work item
 constexpr int kTgtCap = 512;    // targets per interp work item
 // fixed head of the workspace: [0,96) bounds of x and xi; [128,144) n_items_s, n_items_t, queue counters;
-// [1024, ...) scratch of the bounds reduction
+// [1024, ...) scratch of the bounds reduction; [kRuleOff, +2048) the triangle rule when the sources are a mesh's atoms
 constexpr size_t kMiscBytes = 32768;
+constexpr size_t kRuleOff = 24576;
 
 // smallest even n' >= n of the form 2^a 3^b 5^c (the radices of fft.cu: 4, 2, 3, 5)
 int64_t next_smooth_even(int64_t n) {
@@ -534,7 +536,8 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
 }
 
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
-                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint) {
+                   void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint,
+                   const MeshAtoms* mesh) {
   SFD_REQUIRE(J > 0 && applicable, SFD_ERR_INVALID_ARG, "nufft1_lattice: J must be > 0");
   SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
               "type-1 NUFFT needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
@@ -543,8 +546,11 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   int32_t* d_ctl = reinterpret_cast<int32_t*>(base + 128);
   double* d_scratch = reinterpret_cast<double*>(base + 1024);
 
+  // extents: a hull the caller knows, else the mesh's vertices (the atoms are convex combinations), else the sources
   const bool hull = hint && hint->d_hull && hint->n_hull > 0;
-  SFD_TRY(bounds_minmax(hull ? hint->d_hull : d_x, hull ? hint->n_hull : J, d_bounds, d_scratch, st));
+  const double* bsrc = hull ? hint->d_hull : (mesh ? mesh->d_V : d_x);
+  const int64_t nb = hull ? hint->n_hull : (mesh ? mesh->nV : J);
+  SFD_TRY(bounds_minmax(bsrc, nb, d_bounds, d_scratch, st));
   double hb[6];
   SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_bounds, sizeof(hb), cudaMemcpyDeviceToHost, st));
   SFD_CUDA_TRY(cudaStreamSynchronize(st));
@@ -592,9 +598,14 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   // rescale (eq. 3.7) and bin-sort the sources, as in the type-3 transform
   SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_keys + 1) * 4, st));
   SFD_CUDA_TRY(cudaMemsetAsync(scur, 0, (size_t)(L.ns_keys + 1) * 4, st));
-  SFD_TRY(source_keys(p, d_x, J, skey, shist, st));
+  double* d_rule = reinterpret_cast<double*>(base + kRuleOff);
+  if (mesh) {
+    SFD_REQUIRE(mesh->nF * mesh->rule == J, SFD_ERR_INVALID_ARG, "nufft1_lattice: J does not match the mesh");
+    SFD_TRY(rule_table_device(mesh->rule, d_rule, st));
+  }
+  SFD_TRY(source_keys(p, d_x, J, skey, shist, st, mesh, d_rule));
   SFD_TRY(exclusive_scan_i32(shist, soff, L.ns_keys, nullptr, scan_w, scan_b, st));
-  SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st));
+  SFD_TRY(source_scatter(p, d_x, d_w, J, skey, soff, scur, src, st, mesh, d_rule));
   if (p.fine == 1) {   // per-bin ranges out of the per-footprint ones
     int32_t* bh = reinterpret_cast<int32_t*>(base + L.sbhist);
     int32_t* bo = reinterpret_cast<int32_t*>(base + L.sboff);

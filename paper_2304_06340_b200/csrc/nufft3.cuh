@@ -111,14 +111,19 @@ constexpr int kBoundsBlocks = 296;
 // (min[3], max[3]) of n points into d_out6; d_scratch holds kBoundsBlocks*6 doubles.
 int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scratch, cudaStream_t st);
 // A5-2/A5-3: bin key of every source + histogram; then scatter into bin order with grid coordinates and c'_j.
-int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st);
+// mesh != nullptr: the sources are the atoms of the mesh, generated on the fly (atoms.cuh; d_x / d_w unused, d_rule = the
+// rule's columns from rule_table_device).
+struct MeshAtoms;
+int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st,
+                const MeshAtoms* mesh = nullptr, const double* d_rule = nullptr);
 // p.fine: keys are bin * cpb + sub-key, cpb = (bs0+1)(bs1+1)(bs2+1); after the scan of the fine histogram this
 // extracts the per-bin offsets and counts that make_items wants: d_boff[b] = d_off[b cpb], d_bhist[b] = their differences.
 inline int64_t source_subkeys(const N3Params& p) { return (int64_t)(p.bs[0] + 1) * (p.bs[1] + 1) * (p.bs[2] + 1); }
 int source_bin_ranges(const N3Params& p, const int32_t* d_off, int64_t nbins, int64_t J, int32_t* d_bhist,
                       int32_t* d_boff, cudaStream_t st);
 int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
-                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st);
+                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st,
+                   const MeshAtoms* mesh = nullptr, const double* d_rule = nullptr);
 // A5-7: same for the targets.
 int target_keys(const N3Params& p, const double* d_xi, int64_t K, int32_t* d_key, int32_t* d_hist, cudaStream_t st);
 int target_scatter(const N3Params& p, const double* d_xi, int64_t K, const int32_t* d_key, const int32_t* d_off,

@@ -5,6 +5,7 @@
 #include <algorithm>
 
 #include "internal.cuh"
+#include "atoms.cuh"
 #include "nufft3.cuh"
 
 namespace sfd {
@@ -94,16 +95,49 @@ __device__ __forceinline__ double tgt_coord(const N3Params& p, double xi, int d)
   return fmin(fmax(u, (double)p.t0[d]), (double)(p.t0[d] + p.n2[d] / 2));
 }
 
-__global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, const double* __restrict__ x, int64_t J,
-                                                        int32_t* __restrict__ key, int32_t* __restrict__ hist) {
+// Where the sources come from: the arrays x[J][3], w[J], or (V != nullptr) the atoms of a mesh generated on the fly
+// (atoms.cuh) -- the lattice variant's 2e7 atoms are then never written to or read from memory as (x, w).
+struct SrcView {
+  const double* x;
+  const double* w;
+  const double* V;
+  const int32_t* F;
+  int64_t nV;
+  const double* rule;   // 4 x Q columns (device)
+  int Q;
+};
+__device__ __forceinline__ void stage_rule(const SrcView& v, double* s_rule) {
+  if (v.V) {
+    for (int t = threadIdx.x; t < 4 * v.Q; t += kT) s_rule[t] = v.rule[t];
+    __syncthreads();
+  }
+}
+__device__ __forceinline__ void load_source(const SrcView& v, const double* s_rule, int64_t j, double& x0, double& x1,
+                                            double& x2, double& w) {
+  if (v.V) {
+    atom_eval(v.V, v.nV, v.F, j, v.Q, s_rule, x0, x1, x2, w);
+  } else {
+    x0 = v.x[3 * j];
+    x1 = v.x[3 * j + 1];
+    x2 = v.x[3 * j + 2];
+    w = v.w[j];
+  }
+}
+
+__global__ void __launch_bounds__(kT) source_keys_kernel(N3Params p, SrcView v, int64_t J, int32_t* __restrict__ key,
+                                                        int32_t* __restrict__ hist) {
+  __shared__ double s_rule[4 * 64];
+  stage_rule(v, s_rule);
   const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
   const bool active = j < J;
   int k = 0;
   if (active) {
+    double xs[3], wj;
+    load_source(v, s_rule, j, xs[0], xs[1], xs[2], wj);
     int b[3], c[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      const double u = src_coord(p, x[3 * j + d], d);
+      const double u = src_coord(p, xs[d], d);
       b[d] = clampi((int)floor(u / p.bs[d]), 0, p.nbs[d] - 1);
       // first cell of the footprint relative to the bin's padded subgrid: in [0, bs] (the footprint fits the subgrid)
       int i0;
@@ -127,10 +161,11 @@ __global__ void __launch_bounds__(kT) bin_ranges_kernel(const int32_t* __restric
   if (b < nbins) bhist[b] = (b + 1 < nbins ? off[(b + 1) * cpb] : (int32_t)J) - lo;
 }
 
-__global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const double* __restrict__ x, const double* __restrict__ w,
-                                                           int64_t J, const int32_t* __restrict__ key,
+__global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, SrcView v, int64_t J, const int32_t* __restrict__ key,
                                                            const int32_t* __restrict__ off, int32_t* __restrict__ cursor,
                                                            SrcRec* __restrict__ out) {
+  __shared__ double s_rule[4 * 64];
+  stage_rule(v, s_rule);
   const int64_t j = (int64_t)blockIdx.x * kT + threadIdx.x;
   const bool active = j < J;
   const int k = active ? key[j] : 0;
@@ -138,11 +173,11 @@ __global__ void __launch_bounds__(kT) source_scatter_kernel(N3Params p, const do
   if (!active) return;
   const int pos = off[k] + slot;
   SrcRec r;
-  const double x0 = x[3 * j], x1 = x[3 * j + 1], x2 = x[3 * j + 2];
+  double x0, x1, x2, wj;
+  load_source(v, s_rule, j, x0, x1, x2, wj);
   r.u[0] = src_coord(p, x0, 0);
   r.u[1] = src_coord(p, x1, 1);
   r.u[2] = src_coord(p, x2, 2);
-  const double wj = w[j];
   if (p.real_c) {
     r.re = wj;
     r.im = 0.0;
@@ -290,8 +325,23 @@ int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scra
   return launch_check("bounds_final_kernel");
 }
 
-int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st) {
-  source_keys_kernel<<<blocks_for(J), kT, 0, st>>>(p, d_x, J, d_key, d_hist);
+static SrcView src_view(const double* d_x, const double* d_w, const MeshAtoms* mesh, const double* d_rule) {
+  SrcView v{};
+  v.x = d_x;
+  v.w = d_w;
+  if (mesh) {
+    v.V = mesh->d_V;
+    v.F = mesh->d_F;
+    v.nV = mesh->nV;
+    v.rule = d_rule;
+    v.Q = mesh->rule;
+  }
+  return v;
+}
+
+int source_keys(const N3Params& p, const double* d_x, int64_t J, int32_t* d_key, int32_t* d_hist, cudaStream_t st,
+                const MeshAtoms* mesh, const double* d_rule) {
+  source_keys_kernel<<<blocks_for(J), kT, 0, st>>>(p, src_view(d_x, nullptr, mesh, d_rule), J, d_key, d_hist);
   return launch_check("source_keys_kernel");
 }
 int source_bin_ranges(const N3Params& p, const int32_t* d_off, int64_t nbins, int64_t J, int32_t* d_bhist,
@@ -300,8 +350,9 @@ int source_bin_ranges(const N3Params& p, const int32_t* d_off, int64_t nbins, in
   return launch_check("bin_ranges_kernel");
 }
 int source_scatter(const N3Params& p, const double* d_x, const double* d_w, int64_t J, const int32_t* d_key,
-                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st) {
-  source_scatter_kernel<<<blocks_for(J), kT, 0, st>>>(p, d_x, d_w, J, d_key, d_off, d_cursor, d_out);
+                   const int32_t* d_off, int32_t* d_cursor, SrcRec* d_out, cudaStream_t st, const MeshAtoms* mesh,
+                   const double* d_rule) {
+  source_scatter_kernel<<<blocks_for(J), kT, 0, st>>>(p, src_view(d_x, d_w, mesh, d_rule), J, d_key, d_off, d_cursor, d_out);
   return launch_check("source_scatter_kernel");
 }
 int target_keys(const N3Params& p, const double* d_xi, int64_t K, int32_t* d_key, int32_t* d_hist, cudaStream_t st) {
