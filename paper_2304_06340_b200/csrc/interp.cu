@@ -71,7 +71,7 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
   for (int q = 0; q <= DEG; ++q) pc[q] = li < W ? ptab[q * kPolyStride + li] : 0.0;
 
   // the lane's cells of a W x W plane: c = lane + 32 i -> (cy, cz); offset inside the plane cy Pz + cz
-  // (lanes beyond the last cell of the last round read cell 0 and get weight 0: no predicate in the plane loop)
+  // (lanes beyond the last cell of the last round load nothing in the plane loop and get weight 0)
   int off[NCL], cy[NCL], cz[NCL];
   bool on[NCL];
 #pragma unroll
@@ -183,7 +183,10 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
           const double kx = ktab[wq][u][0][a];
 #pragma unroll
           for (int i = 0; i < NCL; ++i) {
-            const double2 c = cell[u][i][a * plane];
+            // the last round of a plane covers only W*W - 32 (NCL-1) cells: lanes beyond them issue no load (a load
+            // of a dummy cell would still cost its shared-memory wavefronts: 2 of 9 per plane at W = 7)
+            double2 c = make_double2(0.0, 0.0);
+            if (i + 1 < NCL || on[i]) c = cell[u][i][a * plane];
             are[u][i] = __fma_rn(c.x, kx, are[u][i]);
             aim[u][i] = __fma_rn(c.y, kx, aim[u][i]);
           }
