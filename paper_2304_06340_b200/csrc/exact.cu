@@ -69,6 +69,21 @@ __global__ void __launch_bounds__(256) face_prep_kernel(const double* __restrict
   out[f] = r;
 }
 
+// g(u, v) = sum_{n < NT} (-i)^n H_n(u, v) / (n+2)!,  H_n = u H_{n-1} + v^n
+template <int NT>
+__device__ __forceinline__ void series(double u, double v, double& sr, double& si) {
+  double H = 1.0, P = 1.0;
+  sr = c_series[0];
+  si = 0.0;
+#pragma unroll
+  for (int n = 1; n < NT; ++n) {
+    P *= v;
+    H = __fma_rn(u, H, P);
+    if (n & 1) si = __fma_rn(c_series[n], H, si);
+    else sr = __fma_rn(c_series[n], H, sr);
+  }
+}
+
 // sin(h)/h
 __device__ __forceinline__ double sinc_fp64(double h) {
   double s, c;
@@ -108,14 +123,13 @@ __global__ void __launch_bounds__(kThreads) exact_sum_kernel(const FaceRec* __re
         // terms 0..nterm-1; remainder (n+1) d^n / (n+2)! below 1e-17
         int nterm = dmax <= 0.03 ? 8 : (dmax <= 0.1 ? 10 : (dmax <= 0.25 ? 12 : (dmax <= 0.5 ? 15 : 18)));
         nterm = __reduce_max_sync(__activemask(), nterm);
-        double H = 1.0, P = 1.0, sr = c_series[0], si = 0.0;
-#pragma unroll
-        for (int n = 1; n < 18; ++n) {
-          if (n >= nterm) break;   // uniform in the warp
-          P *= v;
-          H = __fma_rn(u, H, P);
-          if (n & 1) si = __fma_rn(c_series[n], H, si);
-          else sr = __fma_rn(c_series[n], H, sr);
+        double sr, si;
+        switch (nterm) {   // uniform in the warp: one fully unrolled series per length, no per-term test
+          case 8: series<8>(u, v, sr, si); break;
+          case 10: series<10>(u, v, sr, si); break;
+          case 12: series<12>(u, v, sr, si); break;
+          case 15: series<15>(u, v, sr, si); break;
+          default: series<18>(u, v, sr, si); break;
         }
         double s, c;
         sincos_fp64(a0, s, c);
