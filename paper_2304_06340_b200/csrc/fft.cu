@@ -81,6 +81,29 @@ __device__ __forceinline__ void bfly<5>(double2 (&x)[5]) {
   x[4] = cadd(a1, mul_pi(b1));
 }
 
+template <>
+__device__ __forceinline__ void bfly<7>(double2 (&x)[7]) {
+  // X_k = x0 + sum_j t_j cos(2 pi j k / 7) - i sum_j d_j sin(2 pi j k / 7),  t_j = x_j + x_{7-j}, d_j = x_j - x_{7-j}
+  const double c1 = 0.62348980185873353053, c2 = -0.22252093395631440429, c3 = -0.90096886790241912624;
+  const double s1 = 0.78183148246802980871, s2 = 0.97492791218182360702, s3 = 0.43388373911755812048;
+  const double2 x0 = x[0];
+  const double2 t1 = cadd(x[1], x[6]), t2 = cadd(x[2], x[5]), t3 = cadd(x[3], x[4]);
+  const double2 d1 = csub(x[1], x[6]), d2 = csub(x[2], x[5]), d3 = csub(x[3], x[4]);
+  const double2 a1 = make_double2(x0.x + c1 * t1.x + c2 * t2.x + c3 * t3.x, x0.y + c1 * t1.y + c2 * t2.y + c3 * t3.y);
+  const double2 a2 = make_double2(x0.x + c2 * t1.x + c3 * t2.x + c1 * t3.x, x0.y + c2 * t1.y + c3 * t2.y + c1 * t3.y);
+  const double2 a3 = make_double2(x0.x + c3 * t1.x + c1 * t2.x + c2 * t3.x, x0.y + c3 * t1.y + c1 * t2.y + c2 * t3.y);
+  const double2 b1 = make_double2(s1 * d1.x + s2 * d2.x + s3 * d3.x, s1 * d1.y + s2 * d2.y + s3 * d3.y);
+  const double2 b2 = make_double2(s2 * d1.x - s3 * d2.x - s1 * d3.x, s2 * d1.y - s3 * d2.y - s1 * d3.y);
+  const double2 b3 = make_double2(s3 * d1.x - s1 * d2.x + s2 * d3.x, s3 * d1.y - s1 * d2.y + s2 * d3.y);
+  x[0] = make_double2(x0.x + t1.x + t2.x + t3.x, x0.y + t1.y + t2.y + t3.y);
+  x[1] = cadd(a1, mul_mi(b1));
+  x[2] = cadd(a2, mul_mi(b2));
+  x[3] = cadd(a3, mul_mi(b3));
+  x[4] = cadd(a3, mul_pi(b3));
+  x[5] = cadd(a2, mul_pi(b2));
+  x[6] = cadd(a1, mul_pi(b1));
+}
+
 // One decimation-in-frequency stage of radix R.  A thread owns butterfly bf of CG consecutive rows of the tile: the
 // index arithmetic and the R-1 twiddle loads are paid once per thread and amortised over CG butterflies, whose
 // chains are independent (instruction-level parallelism on top of the warps).  Lanes run over (bf, column group) with
@@ -171,7 +194,9 @@ __device__ __forceinline__ void fused_stages(double2* __restrict__ a, const doub
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
 // 1024 with one (long transforms): 32 warps per SM either way -- the stages are bound by dependent FP64 chains and
 // the shared-memory pipe, so occupancy is what buys throughput (profiles/r1c_after_rewrites.md, r1j_fft_phases.md).
-template <bool REAL_IN, bool CONTIG, int THREADS, int CG, bool FUSED>
+// R7: the length has a factor 7 (a separate instantiation: the radix-7 butterfly's register pressure costs the other
+// lengths ~5 % when it shares their kernel).
+template <bool REAL_IN, bool CONTIG, int THREADS, int CG, bool FUSED, bool R7>
 __global__ void __launch_bounds__(THREADS, (FUSED ? 512 : 1024) / THREADS)
 fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict__ out) {
   constexpr int kFftThreads = THREADS;
@@ -307,9 +332,15 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         SFD_FFT_PAIR(4, 4) SFD_FFT_PAIR(4, 2) SFD_FFT_PAIR(4, 3) SFD_FFT_PAIR(2, 3) SFD_FFT_PAIR(2, 5) SFD_FFT_PAIR(3, 3)
         SFD_FFT_PAIR(3, 5) SFD_FFT_PAIR(2, 2) SFD_FFT_PAIR(4, 1) SFD_FFT_PAIR(2, 1) SFD_FFT_PAIR(3, 1) SFD_FFT_PAIR(5, 1)
       }
+      if (R7) {
+        switch (code) { SFD_FFT_PAIR(2, 7) SFD_FFT_PAIR(7, 1) }
+      }
     } else {
       switch (code) {
         SFD_FFT_STAGE(4) SFD_FFT_STAGE(2) SFD_FFT_STAGE(3) SFD_FFT_STAGE(5)
+      }
+      if (R7) {
+        switch (code) { SFD_FFT_STAGE(7) }
       }
     }
 #undef SFD_FFT_PAIR
@@ -377,7 +408,7 @@ const HostTables& tables_for(int N) {
   auto it = g_tables.find(N);
   if (it != g_tables.end()) return it->second;
   HostTables t;
-  // radices 4s, 2, 3s, 5s, then ordered so that consecutive stages pair up into register-resident radix-(R1 R2)
+  // radices 4s, 2, 3s, 5s, 7s, then ordered so that consecutive stages pair up into register-resident radix-(R1 R2)
   // butterflies with R1 R2 <= 16: take the first remaining factor and the largest other one that fits
   // (2700 -> (4,3)(3,5)(3,5); 1440 -> (4,4)(2,5)(3,3); 720 -> (4,4)(3,5)(3); 360 -> (4,3)(2,5)(3))
   std::vector<int> rest;
@@ -386,6 +417,7 @@ const HostTables& tables_for(int N) {
   while (n % 2 == 0) { rest.push_back(2); n /= 2; }
   while (n % 3 == 0) { rest.push_back(3); n /= 3; }
   while (n % 5 == 0) { rest.push_back(5); n /= 5; }
+  while (n % 7 == 0) { rest.push_back(7); n /= 7; }
   t.nfac = 0;
   t.npair = 0;
   while (!rest.empty()) {
@@ -431,6 +463,7 @@ bool fft_length_ok(int N) {
   while (n % 2 == 0) n /= 2;
   while (n % 3 == 0) n /= 3;
   while (n % 5 == 0) n /= 5;
+  while (n % 7 == 0) n /= 7;
   return n == 1 && N >= 2;
 }
 
@@ -528,14 +561,16 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   };
   // kernel variants: (real, contiguous) = pass A with real strengths; (complex, contiguous) = pass A otherwise;
   // (complex, strided) = passes B and C
-#define SFD_FFT_T(REAL_, CONTIG_)                                                                               \
-  (fused ? (threads == 256 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, true>)                                   \
-                           : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, true>))                                  \
-         : (threads == 256 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 2, false>)                       \
-                                      : go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, false>))                      \
-            : threads == 512 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 512, 2, false>)                     \
-                                        : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, false>))                    \
-                             : go(fft_pass_kernel<REAL_, CONTIG_, 1024, 1, false>)))
+  const bool r7 = P.N % 7 == 0;
+#define SFD_FFT_T7(REAL_, CONTIG_, R7_)                                                                          \
+  (fused ? (threads == 256 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, true, R7_>)                              \
+                           : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, true, R7_>))                             \
+         : (threads == 256 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 256, 2, false, R7_>)                  \
+                                      : go(fft_pass_kernel<REAL_, CONTIG_, 256, 1, false, R7_>))                 \
+            : threads == 512 ? (cg == 2 ? go(fft_pass_kernel<REAL_, CONTIG_, 512, 2, false, R7_>)                \
+                                        : go(fft_pass_kernel<REAL_, CONTIG_, 512, 1, false, R7_>))               \
+                             : go(fft_pass_kernel<REAL_, CONTIG_, 1024, 1, false, R7_>)))
+#define SFD_FFT_T(REAL_, CONTIG_) (r7 ? SFD_FFT_T7(REAL_, CONTIG_, true) : SFD_FFT_T7(REAL_, CONTIG_, false))
   SFD_REQUIRE(P.contig || (!P.real_in && !P.dec_axis && P.in_lo == 1 && P.out_lo == 1), SFD_ERR_INVALID_ARG,
               "strided FFT passes take complex input with unit row stride and no deconvolution factors");
   SFD_REQUIRE(!P.contig || (P.in_el == 1 && P.out_el == 1), SFD_ERR_INVALID_ARG,
@@ -547,6 +582,7 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   else
     SFD_TRY(SFD_FFT_T(false, false));
 #undef SFD_FFT_T
+#undef SFD_FFT_T7
   return launch_check("fft_pass_kernel");
 }
 

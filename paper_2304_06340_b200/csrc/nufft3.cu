@@ -36,8 +36,10 @@ constexpr int kTgtCap = 512;    // targets per interp work item
 constexpr size_t kMiscBytes = 32768;
 constexpr size_t kRuleOff = 24576;
 
-// smallest even n' >= n of the form 2^a 3^b 5^c (the radices of fft.cu: 4, 2, 3, 5)
-int64_t next_smooth_even(int64_t n) {
+// Grid size: the smallest even n' >= n of the form 2^a 3^b 5^c (the radices 4, 2, 3, 5 of fft.cu), or of the form
+// 2^a 3^b 5^c 7^d when that is at least 3 % smaller (a radix-7 stage costs more per point, and an extra stage when it
+// does not pair up: 1344 is not worth it against 1350, 336 against 360 and 672 against 720 are).
+int64_t next_smooth_even_of(int64_t n, bool with7) {
   if (n < 2) n = 2;
   if (n & 1) ++n;
   for (;; n += 2) {
@@ -45,8 +47,14 @@ int64_t next_smooth_even(int64_t n) {
     while (m % 2 == 0) m /= 2;
     while (m % 3 == 0) m /= 3;
     while (m % 5 == 0) m /= 5;
+    if (with7)
+      while (m % 7 == 0) m /= 7;
     if (m == 1) return n;
   }
+}
+int64_t next_smooth_even(int64_t n) {
+  const int64_t n5 = next_smooth_even_of(n, false), n7 = next_smooth_even_of(n, true);
+  return (double)n7 <= 0.97 * (double)n5 ? n7 : n5;
 }
 
 // Kernel width and shape for tolerance eps at upsampling 2 (parameter choice of the ES-kernel papers, refs [2,3]
