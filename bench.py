@@ -262,8 +262,9 @@ FP64_LANES_PER_SM = 64          # DFMA / clk / SM on B200 (nominal 37-40 TFLOP/s
 
 def run_paper(args):
     """The paper's Fig. 4 workloads on its own variant: icosphere level N, 64-point rule, lattice M at
-    xi_max = 5, transform tolerance 1e-7; timed region as in the paper = atoms + transform, without the pointwise
-    operations and the reduction (reported separately)."""
+    xi_max = 5, transform tolerance 1e-7; timed region as in the paper = atoms + transform (the paper leaves the
+    pointwise operations and the reduction out; here the deconvolution is folded into the reduction, so the reduction
+    is inside the timed region too)."""
     import torch
     import paper_2304_06340_b200 as P
     torch.cuda.set_device(0)
@@ -284,7 +285,10 @@ def run_paper(args):
         st = dict(P.sfd_last_stage_times())
         for k, v in st.items():
             stages.setdefault(k, []).append(v)
-        reg.append(sum(v for k, v in st.items() if k not in ("freq_nodes", "reduce")))
+        # the paper's timed region: atoms + transform.  When the library folds the transform's last step (deconvolution)
+        # into the reduction there is no separate "post" stage and the whole reduction is counted as well.
+        skip = ("freq_nodes", "reduce") if "post" in st else ("freq_nodes",)
+        reg.append(sum(v for k, v in st.items() if k not in skip))
     torch.cuda.synchronize()
     P.sfd_set_profiling(False)
     tot = [a.elapsed_time(b) for a, b in ev]
@@ -293,7 +297,8 @@ def run_paper(args):
     launches = (P.sfd_launch_count() - launches0) // args.steps
     # which transform the library ran: the paper's type-1 (no interpolation stage) or the type-3 fallback
     transform = "type-3" if "interp" in stages else "type-1"
-    line = {"metric": "seconds per evaluation: atoms + Fourier transform on the lattice (paper Fig. 4, P:244)",
+    line = {"metric": "seconds per evaluation: atoms + Fourier transform on the lattice (paper Fig. 4, P:244); includes the "
+                      "norm's reduction, into which the deconvolution is folded",
             "value": sec, "unit": "s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": float(np.mean(tot)), "higher_is_better": False, "scaling": "weak",
             "vs_baseline": sec / paper_gpu_s, "dtype": "f64", "data": "synthetic",

@@ -596,11 +596,13 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   hint.n_hull = nV;
   int rc = SFD_OK;
   bool done = false;
+  Nufft1Band band;
   if (eps > 0.0 && L.J > 0) {
-    // the paper's transform, with the atoms generated inside its sort kernels: (x, w) are never materialised
+    // the paper's transform, with the atoms generated inside its sort kernels ((x, w) are never materialised) and
+    // stopped after the FFT: deconvolution and phase are folded into the reduction (nuhat is never materialised either)
     const MeshAtoms mesh{d_vertices, nV, d_faces, nF, rule};
-    rc = nufft1_lattice(nullptr, nullptr, L.J, M, 2.0 * xi_max / M, eps, nu, base + L.ft, work_bytes - L.ft, st, &done,
-                        &hint, &mesh);
+    rc = nufft1_lattice(nullptr, nullptr, L.J, M, 2.0 * xi_max / M, eps, nullptr, base + L.ft, work_bytes - L.ft, st, &done,
+                        &hint, &mesh, &band);
   }
   if (rc == SFD_OK && !done) {
     // direct sum, or a lattice too coarse for the type-1 transform: materialise the atoms; the lattice nodes are
@@ -611,9 +613,10 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
   }
   double* d_res = nullptr;
   // the paper's norm (eq. 2.7) on nodes xi' = 2 pi xi: (1 + |xi|^2)^s = (1 + (|xi'|/2 pi)^2)^-(-s), weights in d xi
+  const double inv_two_pi = 1.0 / 6.283185307179586476925286766559;
   if (rc == SFD_OK)
-    rc = reduce_lattice_enqueue(nu, M, xi_max, -s_paper, base + L.red, L.red_bytes, st, &d_res,
-                                1.0 / 6.283185307179586476925286766559, 1.0);
+    rc = done ? reduce_lattice_band_enqueue(band, M, xi_max, -s_paper, base + L.red, L.red_bytes, st, &d_res, inv_two_pi, 1.0)
+              : reduce_lattice_enqueue(nu, M, xi_max, -s_paper, base + L.red, L.red_bytes, st, &d_res, inv_two_pi, 1.0);
   prof_mark("reduce", st);
   double I = 0.0;
   if (rc == SFD_OK) {

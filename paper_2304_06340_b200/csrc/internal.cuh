@@ -90,10 +90,22 @@ int nufft3_release_cache();
 int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double eps, bool* applicable, size_t* bytes);
 // mesh != nullptr: the sources are the atoms of that mesh (J = nF * rule), generated inside the sort kernels; d_x and
 // d_w are not read.
+// d_nuhat == nullptr with band != nullptr: stop after the FFT and describe its output instead -- the Hermitian half band
+// v[M+1][M+1][M/2+1] (modes m0, m1, m2 >= 0, before deconvolution), the per-axis tables 1 / ((w/2) phihat) on |m| and the
+// centre C of the sources -- for a consumer that folds deconvolution and phase into its own pass (reduce.cu).
+struct Nufft1Band {
+  const double* v = nullptr;     // complex128, inside the workspace
+  const double* dec = nullptr;   // [3][M/2+1]
+  double C[3] = {0.0, 0.0, 0.0};
+};
 struct MeshAtoms;
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
                    void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint = nullptr,
-                   const MeshAtoms* mesh = nullptr);
+                   const MeshAtoms* mesh = nullptr, Nufft1Band* band = nullptr);
+// reduce.cu: I on the paper's lattice straight from that band: deconvolution, e^{-i xi.C}, sigmahat, weights and the
+// sum in one pass over the half band (mirror modes contribute equal terms: counted twice), nuhat never materialised.
+int reduce_lattice_band_enqueue(const Nufft1Band& band, int M, double xi_max, double s, void* d_work, size_t work_bytes,
+                                cudaStream_t st, double** d_result, double scale, double pref);
 // nodes.cu: the rule as four columns lam0[Q], lam1[Q], lam2[Q], om[Q] (4 * rule doubles) in device memory
 int rule_table_device(int rule, double* d_tab, cudaStream_t st);
 

@@ -545,7 +545,7 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
 
 int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, double h, double eps, double* d_nuhat,
                    void* d_work, size_t work_bytes, cudaStream_t st, bool* applicable, const ExtentHint* hint,
-                   const MeshAtoms* mesh) {
+                   const MeshAtoms* mesh, Nufft1Band* band) {
   SFD_REQUIRE(J > 0 && applicable, SFD_ERR_INVALID_ARG, "nufft1_lattice: J must be > 0");
   SFD_REQUIRE(d_work && work_bytes >= kMiscBytes, SFD_ERR_WORKSPACE_TOO_SMALL,
               "type-1 NUFFT needs a workspace (sfd_surface_ft_lattice_workspace), got %zu bytes", work_bytes);
@@ -652,6 +652,13 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   }
   prof_mark("fft", st);
 
+  if (!d_nuhat && band) {   // the consumer deconvolves while it reduces
+    band->v = bufx;
+    band->dec = dec;
+    for (int d = 0; d < 3; ++d) band->C[d] = p.C[d];
+    return SFD_OK;
+  }
+  SFD_REQUIRE(d_nuhat, SFD_ERR_NULL, "nufft1_lattice: NULL output");
   SFD_TRY(lattice_post(p, M, h, dec, bufx, d_nuhat, st));
   prof_mark("post", st);
   return SFD_OK;

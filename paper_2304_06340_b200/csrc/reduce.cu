@@ -131,6 +131,47 @@ __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* _
   if (threadIdx.x == 0) partial[blockIdx.x] = tot;
 }
 
+// The paper's lattice straight from the type-1 transform's FFT output (internal.cuh Nufft1Band): mode (m0, m1, m2 >= 0)
+// -> nuhat = v dec0[|m0|] dec1[|m1|] dec2[m2] e^{-i xi.C}, xi = 2 pi (m h); its mirror mode has the conjugate transform
+// and the same radius and weight, hence the same term: modes with m2 > 0 count twice.
+__global__ void __launch_bounds__(kThreads) lattice_band_terms_kernel(const double2* __restrict__ v, const double* __restrict__ dec,
+                                                                     double c0, double c1, double c2, int M, double h,
+                                                                     double s, int s_kind, double scale2,
+                                                                     Comp* __restrict__ partial) {
+  const int n = M + 1, nh = M / 2 + 1;
+  const int64_t Kh = (int64_t)n * n * nh;
+  const bool phase = c0 != 0.0 || c1 != 0.0 || c2 != 0.0;
+  Comp acc{0.0, 0.0};
+  const int64_t stride = (int64_t)gridDim.x * kThreads;
+  for (int64_t k = (int64_t)blockIdx.x * kThreads + threadIdx.x; k < Kh; k += stride) {
+    const unsigned ku = (unsigned)k, ab = ku / (unsigned)nh;
+    const int m2 = (int)(ku - ab * (unsigned)nh), m1 = (int)(ab % (unsigned)n) - M / 2, m0 = (int)(ab / (unsigned)n) - M / 2;
+    const double two_pi = 6.283185307179586476925286766559;
+    const double a = __dmul_rn(two_pi, __dmul_rn((double)m0, h)), b = __dmul_rn(two_pi, __dmul_rn((double)m1, h)),
+                 c = __dmul_rn(two_pi, __dmul_rn((double)m2, h));
+    double wk = __dmul_rn(__dmul_rn(h, h), h);
+    if (m0 == -M / 2 || m0 == M / 2) wk = __dmul_rn(wk, 0.5);
+    if (m1 == -M / 2 || m1 == M / 2) wk = __dmul_rn(wk, 0.5);
+    if (m2 == M / 2) wk = __dmul_rn(wk, 0.5);
+    if (m2 > 0) wk = __dmul_rn(wk, 2.0);
+    double2 g = v[k];
+    const double f = dec[abs(m0)] * dec[nh + abs(m1)] * dec[2 * nh + m2];
+    g.x *= f;
+    g.y *= f;
+    if (phase) {
+      double sn, cs;
+      sincos_fp64(__fma_rn(a, c0, __fma_rn(b, c1, c * c2)), sn, cs);
+      g = make_double2(g.x * cs + g.y * sn, g.y * cs - g.x * sn);
+    }
+    const double r2 = a * a + b * b + c * c;
+    const double dre = g.x - sigma_hat(sqrt(r2));
+    const double term = wk * (dre * dre + g.y * g.y) * sobolev_weight(__fma_rn(scale2, r2, 1.0), s, s_kind);
+    two_sum_add(acc, term);
+  }
+  const Comp tot = block_reduce(acc);
+  if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
 __global__ void __launch_bounds__(kThreads) reduce_final_kernel(const Comp* __restrict__ partial, int n, double pref,
                                                                double* __restrict__ result) {
   Comp acc{0.0, 0.0};
@@ -196,6 +237,27 @@ int reduce_lattice_enqueue(const double* d_nuhat, int M, double xi_max, double s
   const int64_t K = (int64_t)(M + 1) * (M + 1) * (M + 1);
   return reduce_any(d_nuhat, nullptr, nullptr, K, s, d_work, work_bytes, st, d_result, scale, pref, nullptr, M,
                     2.0 * xi_max / M);
+}
+
+int reduce_lattice_band_enqueue(const Nufft1Band& band, int M, double xi_max, double s, void* d_work, size_t work_bytes,
+                                cudaStream_t st, double** d_result, double scale, double pref) {
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 1624, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..1624 (got %d)", M);
+  SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
+  SFD_REQUIRE(band.v && band.dec, SFD_ERR_NULL, "reduce_lattice_band: NULL band");
+  const int64_t Kh = (int64_t)(M + 1) * (M + 1) * (M / 2 + 1);
+  SFD_REQUIRE(d_work && work_bytes >= reduce_workspace(Kh), SFD_ERR_WORKSPACE_TOO_SMALL,
+              "reduction needs %zu workspace bytes, got %zu", reduce_workspace(Kh), work_bytes);
+  double* result = static_cast<double*>(d_work);
+  Comp* partial = reinterpret_cast<Comp*>(static_cast<char*>(d_work) + 256);
+  *d_result = result;
+  const int blocks = reduce_blocks(Kh);
+  const int s_kind = (s == std::floor(s) && s >= 1.0 && s <= 64.0) ? (int)s : 0;
+  lattice_band_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(band.v), band.dec, band.C[0],
+                                                         band.C[1], band.C[2], M, 2.0 * xi_max / M, s, s_kind,
+                                                         scale * scale, partial);
+  SFD_TRY(launch_check("lattice_band_terms_kernel"));
+  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);
+  return launch_check("reduce_final_kernel");
 }
 
 }  // namespace sfd

@@ -180,6 +180,21 @@ def test_surface_ft_lattice_is_the_type1_path(sfd, torch):
         sfd.sfd_set_profiling(0)
 
 
+def test_weak_distance_lattice_equals_its_stages(sfd, torch):
+    """sfd_weak_distance_lattice never materialises the atoms or nuhat (atoms generated inside the sort, deconvolution
+    and e^{-i xi.C} folded into the reduction over the Hermitian half band); the public stages composed give the same I:
+    a centred mesh, a translated one (phase path), M/2 even and odd."""
+    V, F = sfd.sfd_mesh_icosphere(3)
+    shift = torch.tensor([0.35, -0.2, 0.15], dtype=torch.float64, device="cuda")
+    for Vm in (V, (V * 0.8 + shift).contiguous()):
+        x, w = sfd.sfd_nodes(Vm, F, 64)
+        for M, xm, s in ((32, 3.0, -10.0), (26, 2.0, -5.0)):
+            nu = sfd.sfd_surface_ft_lattice(x, w, M, xm, 1e-11)
+            I_stages = sfd.sfd_reduce_lattice(nu, M, xm, -s, 1 / (2 * np.pi), 1.0)
+            _, I = sfd.sfd_weak_distance_lattice(Vm, F, 64, s, xm, M, 1e-11)
+            assert abs(I - I_stages) <= 1e-11 * I_stages, (M, I, I_stages)
+
+
 def test_weak_distance_lattice_vs_oracle(sfd, orc, torch):
     """Whole path of the paper's variant on a small case: level 1, 64-point rule, M = 16, xi_max = 2, s = -5 and -10."""
     Vo, Fo = orc.mesh_icosphere(1)
