@@ -246,9 +246,10 @@ def run_sfd(args):
     clocks = sampler.stop(t0, t1)
     launches = (P.sfd_launch_count() - l0) // args.steps
     P.sfd_set_profiling(False)
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
     return dict(P=P, torch=torch, dist=dist, world=world, rank=rank, dev=dev, c=c, level=level, J=J, K=K, q=q,
-                eps_list=eps_list, n_eval=n_eval, total_ms=total_ms, results=results, stage_ms=stage_ms,
+                eps_list=eps_list, n_eval=n_eval, total_ms=total_ms, step_ms=step_ms, results=results, stage_ms=stage_ms,
                 clocks=clocks, launches=launches, V=V, F=F, Vj=Vj, nV=nV, nF=nF, ext=ext)
 
 
@@ -477,6 +478,7 @@ def main():
             "config": dict(config_dict(args.config, world), K_evaluated=K,
                            symmetry="targets with xi_3 >= 0 only, doubled weights (mirror nodes give equal terms)"),
             "clocks": r["clocks"],
+            "ms_per_step_best": float(min(r["step_ms"])), "ms_per_step_median": float(np.median(r["step_ms"])),
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
                     "h2d_bytes_per_step": n_dist * (Vn.nbytes + Fn.nbytes), "d2h_bytes_per_step": n_dist * 16,
                     "api": "sfd_weak_distance_host"},

@@ -55,12 +55,14 @@ __global__ void __launch_bounds__(kT) bounds_partial_kernel(const double* __rest
     part[blockIdx.x * 6 + threadIdx.x] = v;
   }
 }
-__global__ void bounds_final_kernel(const double* __restrict__ part, int nblocks, double* __restrict__ out6) {
-  const int c = threadIdx.x;
-  if (c >= 6) return;
-  double v = part[c];
-  for (int i = 1; i < nblocks; ++i) v = c < 3 ? fmin(v, part[i * 6 + c]) : fmax(v, part[i * 6 + c]);
-  out6[c] = v;
+// one warp per component: the lanes stride over the per-block partials, then a shuffle reduction
+__global__ void __launch_bounds__(192) bounds_final_kernel(const double* __restrict__ part, int nblocks, double* __restrict__ out6) {
+  const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double v = c < 3 ? inf : -inf;
+  for (int i = lane; i < nblocks; i += 32) v = c < 3 ? fmin(v, part[i * 6 + c]) : fmax(v, part[i * 6 + c]);
+  v = c < 3 ? warp_min(v) : warp_max(v);
+  if (lane == 0) out6[c] = v;
 }
 
 // Warp-aggregated counter update: lanes of a warp that hold the same key share one atomicAdd (consecutive points
@@ -321,7 +323,7 @@ int bounds_minmax(const double* d_pts, int64_t n, double* d_out6, double* d_scra
   const int nb = (int)std::min<int64_t>(kBoundsBlocks, std::max<int64_t>(1, (n + kT - 1) / kT));
   bounds_partial_kernel<<<nb, kT, 0, st>>>(d_pts, n, d_scratch);
   SFD_TRY(launch_check("bounds_partial_kernel"));
-  bounds_final_kernel<<<1, 32, 0, st>>>(d_scratch, nb, d_out6);
+  bounds_final_kernel<<<1, 192, 0, st>>>(d_scratch, nb, d_out6);
   return launch_check("bounds_final_kernel");
 }
 
