@@ -6,7 +6,7 @@
 // 128 B/clk/SM of shared-memory bandwidth against 64 DFMA/clk/SM the gather is shared-memory-bandwidth bound by 4x
 // (w = 10: 125 clk per target and SM), far above its HBM traffic (the band of the inner grid, read once per bin).
 // The kernel is built to sit on that bound:
-//   * one persistent CTA per SM pulls work items (a target bin, or a slice of <= kTgtCap targets of one) from a
+//   * one persistent CTA per SM pulls work items (a target bin, or a slice of one: 512 to 4096 targets, nufft3.cu) from a
 //     device-side queue and stages the bin's padded subgrid (bt+w cells per axis) in shared memory as complex128;
 //   * the z extent of a bin is 8 or 16 cells, so the row pitch Pz = bt_z + w is congruent to w modulo 8 and the
 //     flattened (y,z) cell index c = y w + z lands in bank group c mod 8: any 8 consecutive lanes of an LDS.128 hit 8
