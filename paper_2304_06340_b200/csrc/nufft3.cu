@@ -58,9 +58,11 @@ int64_t next_smooth_even(int64_t n) {
 }
 
 // Kernel width and shape for tolerance eps at upsampling 2 (parameter choice of the ES-kernel papers, refs [2,3]
-// of P:185; reading R10): w = ceil(log10(1/eps)) + 1, beta = 2.30 w.
-void kernel_params(double eps, int* w, double* beta) {
-  int ww = (int)std::ceil(std::log10(1.0 / eps) - 1e-9) + 1;
+// of P:185; reading R10): w = ceil(log10(1/eps)) + 1, beta = 2.30 w.  `careful`: one more cell of width --
+// for a handful of sources (nothing averages the kernel's pointwise error, which reaches ~25 eps) and for a
+// space-bandwidth product below one (a grid of a few cells); both cost nothing.
+void kernel_params(double eps, bool careful, int* w, double* beta) {
+  int ww = (int)std::ceil(std::log10(1.0 / eps) - 1e-9) + 1 + (careful ? 1 : 0);
   if (ww < 2) ww = 2;
   if (ww > kMaxW) ww = kMaxW;
   *w = ww;
@@ -75,8 +77,13 @@ struct Layout {
 };
 
 // Geometry from half-widths X (sources) and S (targets); centres are filled in by the caller.
-int make_params(const double X_in[3], const double S_in[3], double eps, bool real_c, N3Params* p) {
-  kernel_params(eps, &p->w, &p->beta);
+constexpr int64_t kFewSources = 64;
+
+int make_params(const double X_in[3], const double S_in[3], double eps, bool real_c, int64_t J, N3Params* p) {
+  bool careful = J < kFewSources;
+  for (int d = 0; d < 3; ++d)
+    if (X_in[d] * (S_in[d] < 1e-150 ? 1.0 : S_in[d]) < 1.0) careful = true;
+  kernel_params(eps, careful, &p->w, &p->beta);
   p->real_c = real_c ? 1 : 0;
   for (int d = 0; d < 3; ++d) {
     double X = X_in[d], S = S_in[d];
@@ -311,11 +318,17 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
   size_t total = 0;
   N3Params p{};
   for (int real_c = 0; real_c < 2; ++real_c) {   // whether the strengths stay real is only known from the data
-    SFD_TRY(make_params(Xi, Si, eps, real_c != 0, &p));
-    choose_sort(&p, J, true);
-    Layout L;
-    SFD_TRY(make_layout(p, J, K, &L));
-    total = std::max(total, L.total);
+    // (the call decides on the wider kernel from the data's own extents: near the threshold size for both)
+    bool near = false;
+    for (int d = 0; d < 3; ++d) near = near || (X[d] * S[d] < 1.01 && X[d] * S[d] > 0.98);
+    for (int pass = 0; pass < (near ? 2 : 1); ++pass) {
+      SFD_TRY(make_params(Xi, Si, eps, real_c != 0, pass == 0 ? J : 0, &p));
+      choose_sort(&p, J, true);
+      Layout L;
+      SFD_TRY(make_layout(p, J, K, &L));
+      total = std::max(total, L.total);
+    }
+    SFD_TRY(make_params(Xi, Si, eps, real_c != 0, J, &p));
   }
   out->w = p.w;
   out->beta = p.beta;
@@ -379,7 +392,7 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
       real_c = false;
     }
   }
-  SFD_TRY(make_params(X, S, eps, real_c, &p));
+  SFD_TRY(make_params(X, S, eps, real_c, J, &p));
   choose_sort(&p, J);
   Layout L;
   SFD_TRY(make_layout(p, J, K, &L));
@@ -493,8 +506,9 @@ namespace {
 
 // *ok = false: the lattice is too coarse for the extent of the sources (2 pi h X >= pi up to the kernel's
 // footprint: the periodic images would overlap) or the transform is too long for fft.cu -- use the type-3 path.
-int make_params_lattice(const double X_in[3], const double C[3], int M, double h, double eps, N3Params* p, bool* ok) {
-  kernel_params(eps, &p->w, &p->beta);
+int make_params_lattice(const double X_in[3], const double C[3], int M, double h, double eps, int64_t J, N3Params* p,
+                        bool* ok) {
+  kernel_params(eps, J < kFewSources, &p->w, &p->beta);
   p->real_c = 1;
   p->zh = 1;
   p->deg = p->w + 3;
@@ -536,7 +550,7 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
   const double C0[3] = {0.0, 0.0, 0.0};
   for (int d = 0; d < 3; ++d) Xi[d] = X[d] * (1.0 + 1e-6);
   N3Params p{};
-  SFD_TRY(make_params_lattice(Xi, C0, M, h, eps, &p, applicable));
+  SFD_TRY(make_params_lattice(Xi, C0, M, h, eps, J, &p, applicable));
   *bytes = 0;
   if (!*applicable) return SFD_OK;
   choose_sort(&p, J, true);
@@ -580,7 +594,7 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
     }
   }
   N3Params p{};
-  SFD_TRY(make_params_lattice(X, C, M, h, eps, &p, applicable));
+  SFD_TRY(make_params_lattice(X, C, M, h, eps, J, &p, applicable));
   if (!*applicable) return SFD_OK;
   choose_sort(&p, J);
   Layout L;

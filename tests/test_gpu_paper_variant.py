@@ -151,11 +151,11 @@ def test_surface_ft_lattice_edge_cases(sfd, orc, torch):
     assert nu.shape[0] == 729 and nu.abs().max().item() == 0.0
     x1 = np.array([[0.3, -0.2, 0.5]])
     got = sfd.sfd_surface_ft_lattice(dev(torch, x1), dev(torch, np.array([2.0])), 8, 1.5, 1e-9).cpu().numpy()
-    assert np.abs(got - 2.0 * np.exp(-1j * xi @ x1[0])).max() <= 40 * 1e-9 * 2.0      # single source: R10
+    assert np.abs(got - 2.0 * np.exp(-1j * xi @ x1[0])).max() <= 10 * 1e-9 * 2.0      # single source: R10
     xs = np.repeat(x1, 500, axis=0)
     ws = np.linspace(0.5, 1.5, 500)
     got = sfd.sfd_surface_ft_lattice(dev(torch, xs), dev(torch, ws), 8, 1.5, 1e-9).cpu().numpy()
-    assert np.abs(got - ws.sum() * np.exp(-1j * xi @ x1[0])).max() <= 40 * 1e-9 * ws.sum()
+    assert np.abs(got - ws.sum() * np.exp(-1j * xi @ x1[0])).max() <= 25 * 1e-9 * ws.sum()   # 500 coincident sources: no averaging either
     rng = np.random.default_rng(4)
     x, w = _cloud(rng, 800, (0, 0, 0), (1, 1, 1))
     for M, xm, eps in ((2, 0.4, 1e-9), (8, 1.5, 1e-1)):
