@@ -88,8 +88,15 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
     __syncthreads();  // everyone is done with s_item and the previous subgrid
     if (tid == 0) s_item = atomicAdd(counter, 1);
     __syncthreads();
-    const int item = s_item;
-    if (item >= total) break;
+    const int tick = s_item;
+    if (tick >= total) break;
+    // Items are in bin order, x slowest: the crowded bins around the origin (the rule's nodes cluster as 1/r^2) sit in
+    // the middle of the list.  Hand them out from the middle outwards, so that the long items start first and the
+    // short ones fill the tail.
+    const int mid = total / 2;
+    int item = (tick & 1) ? mid - 1 - (tick >> 1) : mid + (tick >> 1);
+    if (item < 0) item = tick;                 // the lower side is exhausted (odd totals): the rest of the upper side
+    else if (item >= total) item = total - 1 - tick;   // the upper side is exhausted: the rest of the lower side
     const int bin = item_bin[item];
     const int start = item_start[item], count = item_count[item];
     const int bz = bin % p.nbt[2], by = (bin / p.nbt[2]) % p.nbt[1], bx = bin / (p.nbt[2] * p.nbt[1]);
