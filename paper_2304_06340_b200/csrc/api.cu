@@ -385,6 +385,7 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
   hint.d_hull = d_vertices;
   hint.n_hull = nV;
   hint.target_reach = R;
+  hint.target_ball = true;   // the ball rule's nodes satisfy |xi| <= R
   if (rc == SFD_OK) rc = surface_ft_impl(x, w, L.J, xi, K, eps, nu, base + L.ft, work_bytes - L.ft, stream, true, &hint);
   double* d_res = nullptr;
   if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, &d_res);

@@ -191,6 +191,14 @@ __device__ __forceinline__ void fused_stages(double2* __restrict__ a, const doub
   }
 }
 
+// FftPass::ball: normalised squared distance of column `lo` from the axis of the ellipsoid the consumer reads.
+__device__ __forceinline__ double ball_q(const FftPass& P, int64_t lo) {
+  const int64_t ia = P.ball == 1 ? lo / P.ball_nb : 0;
+  const double da = ((double)ia - P.ball_ca) * P.ball_ira;
+  const double db = ((double)(lo - ia * (P.ball == 1 ? P.ball_nb : 0)) - P.ball_cb) * P.ball_irb;
+  return da * da + db * db;
+}
+
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
 // 1024 with one (long transforms): 32 warps per SM either way -- the stages are bound by dependent FP64 chains and
 // the shared-memory pipe, so occupancy is what buys throughput (profiles/r1c_after_rewrites.md, r1j_fft_phases.md).
@@ -212,6 +220,11 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * rows_per_tile;
   const int nrow = (int)min(rows_per_tile, P.n_lo - lo0);   // rows of this tile
   const int ncol = (nrow + PACK - 1) / PACK;
+  if (!CONTIG && P.ball) {   // uniform in the block: every thread tests the tile's few columns
+    bool needed = false;
+    for (int c = 0; c < ncol; ++c) needed = needed || ball_q(P, lo0 + c) <= 1.0;
+    if (!needed) return;
+  }
   const int tsh = P.tb_shift;
   const double2* __restrict__ tw = P.tw;
 
@@ -379,9 +392,21 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
   } else {
     const int col = tid & (tb - 1), ty = tid >> tsh, nty = kFftThreads >> tsh;
     if (col < ncol) {
-      double2* o = out + hi * P.out_hi + lo0 + col + (int64_t)ty * P.out_el;
+      int mm0 = 0, mm1 = P.nout;   // the outputs this column has to store
+      if (P.ball) {
+        const double q = ball_q(P, lo0 + col);
+        if (q > 1.0) {
+          mm1 = 0;
+        } else {
+          const double rad = P.ball_rt * sqrt(1.0 - q) + 1.0;
+          mm0 = max(0, (int)floor(P.ball_ct - rad));
+          mm1 = min(P.nout, (int)ceil(P.ball_ct + rad) + 1);
+        }
+      }
+      const int first = mm0 + ((ty - mm0) % nty + nty) % nty;   // smallest mm >= mm0 congruent to ty modulo nty
+      double2* o = out + hi * P.out_hi + lo0 + col + (int64_t)first * P.out_el;
       const int64_t step = (int64_t)nty * P.out_el;
-      for (int mm = ty; mm < P.nout; mm += nty) {
+      for (int mm = first; mm < mm1; mm += nty) {
         int m = P.lo + mm;
         m = m < 0 ? m + N : (m >= N ? m - N : m);
         *o = a[P.rev[m] * tbp + col];

@@ -27,6 +27,13 @@ struct FftPass {
   int64_t in_hi, in_lo, in_el, out_hi, out_lo, out_el;
   int contig, real_in;
   const double *dec_axis, *dec_hi, *dec_lo;
+  // ball != 0 (strided passes): the consumer reads the output only inside an ellipsoid (the targets of the ball rule).
+  // With q = ((a - ball_ca) ball_ira)^2 + ((b - ball_cb) ball_irb)^2 of a column -- ball == 1: lo = a * ball_nb + b (both
+  // other axes are frequencies: the last pass); ball == 2: b = lo only (ball_ira = 0: the third axis is still spatial) --
+  // a column stores only the outputs |mm - ball_ct| <= ball_rt sqrt(1 - q) (+1), none when q > 1, and a tile none of
+  // whose columns has q <= 1 is skipped.  The rest of the output is left untouched.
+  int ball, ball_nb;
+  double ball_ca, ball_cb, ball_ira, ball_irb, ball_ct, ball_rt;
   // filled in by fft_pass():
   int tb, tbp, tb_shift, cg_shift, nfac, fac[16];   // cg_shift: log2(column groups per tile)
   int npair, pair[16];  // fused stage pairs: code = R1 * 8 + R2 (R2 = 1: single stage)

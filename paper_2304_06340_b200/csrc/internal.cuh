@@ -72,11 +72,13 @@ struct Nufft3Sizes {
 int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out);
 // What a caller may know about the extents, which replaces the reductions over all sources / all targets:
 //   d_hull / n_hull: device points whose bounding box contains every source (the vertices of the mesh the atoms are
-//     convex combinations of);  target_reach > 0: every target lies in [-target_reach, target_reach]^3.
+//     convex combinations of);  target_reach > 0: every target lies in [-target_reach, target_reach]^3 (target_ball: in
+//     the ball of that radius -- the last FFT pass then skips the columns of the band outside the ball's projection).
 struct ExtentHint {
   const double* d_hull = nullptr;
   int64_t n_hull = 0;
   double target_reach = 0.0;
+  bool target_ball = false;   // with target_reach: the targets lie in the ball |xi| <= target_reach, not just the cube
 };
 // origin_centred: take the targets' box as symmetric about the origin whatever their extents say (the half rule of
 // nodes.cu freq_expand: the strengths then stay real and the Hermitian half band is used)

@@ -461,12 +461,38 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     B.n_hi = nf0; B.n_lo = no2;
     B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
     B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    // Targets inside the ball |u2 - n2/2| <= n2/4 (the ball rule): only the part of the band within it, grown by the
+    // footprint's reach (w/2 + 1 cells per axis: sqrt 3 times that along the space diagonal) and a cell of slack, is
+    // ever read.  Pass B stops
+    // storing the m1 outside the ball's section at its m2; pass C skips the (m1, m2) columns outside the projection
+    // and stores only the m0 inside the ball.
+    const bool ball = hint && hint->target_ball && hint->target_reach > 0.0;
+    const double reach = (0.5 * p.w + 1.0) * 1.7321 + 1.0;
+    if (ball) {
+      B.ball = 2;
+      B.ball_nb = 0;
+      B.ball_ca = 0.0; B.ball_ira = 0.0;
+      B.ball_cb = 0.5 * p.n2[2] - p.lo[2];
+      B.ball_irb = 1.0 / (0.25 * p.n2[2] + reach);
+      B.ball_ct = 0.5 * p.n2[1] - p.lo[1];
+      B.ball_rt = 0.25 * p.n2[1] + reach;
+    }
     SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
     FftPass C{};   // axis 0: columns (m1, m2) of Y -> X[m0][m1][m2]
     C.N = p.n2[0]; C.n_in = p.nf[0]; C.lo = p.lo[0]; C.nout = p.nout[0];
     C.n_hi = 1; C.n_lo = no1 * no2;
     C.in_hi = 0; C.in_lo = 1; C.in_el = no1 * no2;
     C.out_hi = 0; C.out_lo = 1; C.out_el = no1 * no2;
+    if (ball) {
+      C.ball = 1;
+      C.ball_nb = (int)no2;
+      C.ball_ca = 0.5 * p.n2[1] - p.lo[1];
+      C.ball_cb = 0.5 * p.n2[2] - p.lo[2];
+      C.ball_ira = 1.0 / (0.25 * p.n2[1] + reach);
+      C.ball_irb = 1.0 / (0.25 * p.n2[2] + reach);
+      C.ball_ct = 0.5 * p.n2[0] - p.lo[0];
+      C.ball_rt = 0.25 * p.n2[0] + reach;
+    }
     SFD_TRY(fft_pass(C, ft, 0, bufy, bufx, st));
   }
   prof_mark("fft", st);
