@@ -38,7 +38,7 @@ typedef enum {
   SFD_ERR_BUFFER_TOO_SMALL = -3,
   SFD_ERR_WORKSPACE_TOO_SMALL = -4,
   SFD_ERR_CUDA = -5,
-  SFD_ERR_CUFFT = -6, /* kept for ABI stability: unused since the inner FFT is the library's own (fft.cu) */
+  SFD_ERR_RESERVED_6 = -6, /* never returned (was a cuFFT failure code before the inner FFT became the library's own) */
   SFD_ERR_UNSUPPORTED = -7
 } sfd_status;
 
@@ -76,7 +76,10 @@ int sfd_mesh_icosphere(int level, double* d_vertices /*[nV][3]*/, int32_t* d_fac
 /* ---- A3: triangle-quadrature atoms (eqs. 3.1-3.2) -----------------------------------
  * Converts the rule {(u_i,q_i)} on the standard simplex into {(L(u_i), q_i*gamma_A)} on each face:
  * x[f*q+i] = sum_m lambda_{i,m} p_m(f),  w[f*q+i] = omega_i * area(f).  Degenerate faces give zero
- * weights.  A face index outside [0,nV) makes the face contribute NaN nodes (not checked on host). */
+ * weights.  A face index outside [0,nV) can only be seen on the device: the face's atoms are written as NaN, a
+ * device-side error word is set, and the NEXT SYNCHRONISING call of the library on this device (sfd_reduce*,
+ * sfd_extents, sfd_weak_distance*, sfd_mesh_distance) returns SFD_ERR_INVALID_ARG and clears the word.  The calls that
+ * take a mesh and synchronise themselves (sfd_weak_distance, sfd_mesh_distance, ...) report their own bad indices. */
 int sfd_nodes(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule,
               double* d_x /*[nF*q][3]*/, double* d_w /*[nF*q]*/, sfd_stream stream);
 /* The rule itself (host): barycentric points h_lambda[q][3] and weights h_omega[q] summing to 1. */
@@ -97,11 +100,23 @@ int sfd_freq_nodes_device(const sfd_freq_quadrature* q, double R, double* d_xi /
 int sfd_freq_nodes_device_range(const sfd_freq_quadrature* q, double R, int32_t a_begin, int32_t a_end,
                                 double* d_xi, double* d_W, void* d_work, size_t work_bytes, sfd_stream stream);
 
+/* ---- A5-1 as a call of its own: bounding box of n device points (two kernels, min/max per axis) ------------------
+ * h_half[d] = (max_d - min_d)/2 (with the 1e-12 relative margin the type-3 transform applies itself), h_centre[d] =
+ * (max_d + min_d)/2 (may be NULL): what sfd_surface_ft_workspace / sfd_surface_ft_lattice_workspace /
+ * sfd_weak_distance_workspace take as X / S / x_extent.  n == 0 gives zeros.  A non-finite coordinate ->
+ * SFD_ERR_INVALID_ARG.  Synchronises `stream`. */
+int sfd_extents_workspace(size_t* bytes);
+int sfd_extents(const double* d_pts /*[n][3]*/, int64_t n, double h_half[3], double h_centre[3] /*or NULL*/, void* d_work,
+                size_t work_bytes, sfd_stream stream);
+
 /* ---- A4/A5: Fourier transform of the atomic measure nu = sum_j w_j delta_{x_j} -----------------
  * nuhat_k = sum_{j<J} w_j exp(-i xi_k . x_j)   (eq. 2.8 applied to the atoms of P:152).
  *   eps == 0        : fp64 direct summation, error <= 1e-12 * sum|w_j| for |xi.x| <~ 2e3.
  *   0 < eps < 1     : 3-D type-3 nonuniform FFT at tolerance eps (>= 1e-14), error
- *                     <= 10 * eps * sum|w_j|.  Synchronises `stream` once (grid sizing).
+ *                     <= 10 * eps * sum|w_j|.  Synchronises `stream` once (grid sizing).  The spreader adds the
+ *                     bins' subgrids into the fine grid with fp64 reductions whose order is not fixed: the result
+ *                     is reproducible to rounding (~1e-16 sum|w_j|) only, not bit for bit; the direct sum is
+ *                     deterministic.
  * Workspace: query with the same (J, K, eps) and bounding half-widths X[d] >= max_j|x_jd - centre_d|,
  * S[d] >= max_k|xi_kd - centre_d| (ignored for eps == 0, may then be NULL).  If the data's actual
  * extents need more than work_bytes, the call fails with SFD_ERR_WORKSPACE_TOO_SMALL and writes
@@ -143,6 +158,21 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
  * n_phi is even, n_r n_theta n_phi otherwise. */
 int sfd_weak_distance_targets(const sfd_freq_quadrature* q, int64_t* K_eval);
 
+/* The same distance restricted to the radial shells a in [a_begin, a_end) of the rule (as sfd_freq_nodes_device_range):
+ * the ball rule is a sum over shells, every nuhat_k is its own sum over the atoms, so disjoint ranges give
+ * partial sums I_r that add up to I -- the unit of work of a multi-GPU run (one range per GPU, one all-reduce of the
+ * result).  Same half rule, same fast paths as sfd_weak_distance; the transform's grids are
+ * sized by the range's own largest radius r_{a_end-1}, so inner ranges are cheaper.  Nothing crosses to the host: the
+ * partial sum is left in DEVICE memory as a compensated pair, d_partial[0] = sum, d_partial[1] = compensation,
+ * I_r = d_partial[0] + d_partial[1] (already scaled by (2 pi)^-3); add pairs component-wise.  A face index outside
+ * [0, nV) makes d_partial[0] NaN.  a_begin == a_end gives (0, 0).  Enqueues on `stream` after the one synchronisation
+ * of the transform's sizing (eps > 0). */
+int sfd_weak_distance_range_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, int32_t a_begin,
+                                      int32_t a_end, double eps, double x_extent, size_t* bytes);
+int sfd_weak_distance_range(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
+                            double R, const sfd_freq_quadrature* q, int32_t a_begin, int32_t a_end, double eps,
+                            void* d_work, size_t work_bytes, sfd_stream stream, double* d_partial /*[2], device*/);
+
 /* ---- the paper's own variant: cube lattice, trapezoidal rule, its norm convention ----
  * Lattice of P:156-166 eqs. 3.3-3.4: xi_ijk = (i,j,k) h, h = 2 xi_max / M, i,j,k = -M/2..M/2 (M even, 2..2046), with
  * trapezoid weights w_ijk h^3 (1 inside, 1/2 faces, 1/4 edges, 1/8 corners).  K = (M+1)^3, node index
@@ -176,6 +206,7 @@ int sfd_surface_ft_lattice(const double* d_x, const double* d_w, int64_t J, int3
 /* ||mu - sigma||_{H_s(R^3)} of P:65 eq. 2.7 for the mesh's surface measure mu against the unit sphere's, by the
  * paper's quadrature: atoms (rule 64 = the paper's) -> transform on the lattice (sfd_surface_ft_lattice: eps == 0
  * direct sum, eps > 0 type-1 NUFFT) -> trapezoidal rule.  s_paper < -1/2.
+ * M even, 2..1624 (the reduction's 32-bit node index; the workspace query rejects larger M too).
  * Writes the norm to *h_norm and its square to *h_I.  Synchronises. */
 int sfd_weak_distance_lattice_workspace(int64_t nF, int rule, int32_t M, double xi_max, double eps, double x_extent,
                                         size_t* bytes);
@@ -204,6 +235,18 @@ int sfd_exact_ft(const double* d_vertices /*[nV][3]*/, int64_t nV, const int32_t
  * and error behaviour as sfd_reduce.  Synchronises. */
 int sfd_reduce_pair(const double* d_nuhat_a, const double* d_nuhat_b, const double* d_xi, const double* d_W, int64_t K,
                     double s, void* d_work, size_t work_bytes, sfd_stream stream, double* h_I);
+/* Whole path for two meshes: "discretized surfaces are compared to each other by recomputing the Fourier transform
+ * from their own data representations" (P:137 with a second linear combination of triangle transforms in place
+ * of sigmahat).  Atoms of both meshes (same rule) -> nuhat_a, nuhat_b on the ball rule (q, R) -> sfd_reduce_pair ->
+ * sqrt(I).  Both measures are real, so |nuhat_a - nuhat_b|^2 is even in xi and the half rule of sfd_weak_distance
+ * applies unchanged.  x_extent bounds the half-width of BOTH meshes' bounding boxes.  An empty mesh is the zero
+ * measure.  Synchronises. */
+int sfd_mesh_distance_workspace(int64_t nF_a, int64_t nF_b, int rule, const sfd_freq_quadrature* q, double R, double eps,
+                                double x_extent, size_t* bytes);
+int sfd_mesh_distance(const double* d_vertices_a, int64_t nV_a, const int32_t* d_faces_a, int64_t nF_a,
+                      const double* d_vertices_b, int64_t nV_b, const int32_t* d_faces_b, int64_t nF_b, int rule,
+                      double s, double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes,
+                      sfd_stream stream, double* h_distance, double* h_I);
 
 /* ---- host-buffer entry points (end-to-end: allocate, copy in, run, copy out, free) -------------
  * Same operations with HOST pointers; device memory comes from the stream-ordered CUDA pool of the
@@ -222,12 +265,6 @@ int sfd_last_stage_times(const char** names, float* ms, int max);
 
 /* Number of kernels of this library launched so far by the process. */
 long long sfd_launch_count(void);
-
-/* ---- roofline denominator of A4 ------------------------------------------------------------------
- * Runs a dependency-free DFMA loop (8 independent chains per thread, `iters` x 64 FMAs per chain-step,
- * one persistent CTA set covering every SM) and reports the achieved FP64 throughput in TFLOP/s
- * (FMA = 2 flops) and the kernel time in ms.  Synchronises `stream`.  iters in [1, 1<<20]. */
-int sfd_probe_fp64(int iters, sfd_stream stream, double* h_tflops, double* h_ms);
 
 #ifdef __cplusplus
 }

@@ -28,7 +28,8 @@ _lib.orc_nodes.argtypes = [_dp, _i64, _ip, _i64, C.c_int, _dp, _dp]
 _lib.orc_gauss_legendre.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
 _lib.orc_freq_nodes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _dp, _dp]
 _lib.orc_direct_sum.argtypes = [_dp, _dp, _i64, _dp, _i64, _dp]
-_lib.orc_exact_ft.argtypes = [_dp, _i64, _ip, _i64, _dp, _i64, _dp]
+_lib.orc_exact_ft.argtypes = [_dp, _i64, _ip, _i64, _dp, _i64, _dp,
+                               np.ctypeslib.ndpointer(np.int64, flags="C_CONTIGUOUS"), _i64, C.POINTER(_i64)]
 _lib.orc_sigma_hat.argtypes = [C.c_double]
 _lib.orc_sigma_hat.restype = C.c_double
 _lib.orc_reduce.argtypes = [_dp, _dp, _dp, _i64, C.c_double]
@@ -115,15 +116,64 @@ def direct_sum(x, w, xi):
     return out.view(np.complex128).reshape(-1)
 
 
+def _exact_pair_mp(p, xi):
+    """P:128 eq. 2.19 for ONE face and ONE frequency whose alpha_i = xi.p_i are too close for binary128 ("large
+    cancellation errors"): the printed formula -2A sum_i e^{-i alpha_i} / prod_{j != i}(alpha_i - alpha_j) with as many
+    digits as its cancellation needs, or, where two or three alpha coincide EXACTLY and the printed formula is 0/0, its
+    limit: 2A times the divided difference exp[z_0, z_1, z_2], z = -i alpha, with repeated nodes (textbook definitions:
+    f[z, z, w] = (f[z, w] - f'(z)) / (w - z), f[z, w] = (f(w) - f(z)) / (w - z), f[z, z, z] = f''(z) / 2)."""
+    import mpmath as mp
+    mp.mp.dps = 400                      # the dot products of fp64 inputs are exact at this precision
+    P = [[mp.mpf(float(c)) for c in v] for v in p]
+    X = [mp.mpf(float(c)) for c in xi]
+    e1 = [P[1][c] - P[0][c] for c in range(3)]
+    e2 = [P[2][c] - P[0][c] for c in range(3)]
+    cr = [e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0]]
+    A2 = mp.sqrt(sum(c * c for c in cr))
+    al = [sum(X[c] * P[i][c] for c in range(3)) for i in range(3)]
+    same = [(i, j) for i in range(3) for j in range(i + 1, 3) if al[i] == al[j]]
+    if len(same) == 3:                   # all three coincide (xi along the normal, xi = 0): exp''(z) / 2
+        return complex(A2 * mp.exp(-1j * al[0]) / 2)
+    if len(same) == 1:                   # exactly two coincide (xi orthogonal to an edge): f[z, z, w]
+        i, j = same[0]
+        k = 3 - i - j
+        z, w = -1j * al[i], -1j * al[k]
+        first = (mp.exp(w) - mp.exp(z)) / (w - z)
+        return complex(A2 * (first - mp.exp(z)) / (w - z))
+    dmin = min(abs(al[i] - al[j]) for i in range(3) for j in range(i + 1, 3))
+    amax = max(1, max(abs(a) for a in al))
+    mp.mp.dps = 60 + 3 * int(mp.ceil(mp.log10(amax / dmin)))     # 1/d^2 of cancellation, 1/d in each difference
+    tot = mp.mpc(0)
+    for i in range(3):
+        den = mp.mpf(1)
+        for j in range(3):
+            if j != i:
+                den *= al[i] - al[j]
+        tot += mp.exp(-1j * al[i]) / den
+    return complex(-A2 * tot)
+
+
 def exact_ft(V, F, xi):
-    """Exact transform of the flat mesh's surface measure, sum over faces of P:128 eq. 2.19 (e^{-i xi.x} convention),
-    evaluated in binary128 and rounded: complex128[K]."""
+    """Exact transform of the flat mesh's surface measure, sum over faces of P:128 eq. 2.19 (e^{-i xi.x} convention):
+    complex128[K].  The formula is evaluated as printed in binary128 (sfd_oracle_exact.cpp); the pairs whose alpha are
+    too close for that are evaluated by _exact_pair_mp and added here."""
     V = np.ascontiguousarray(V, np.float64).reshape(-1, 3)
     F = np.ascontiguousarray(F, np.int32).reshape(-1, 3)
     xi = np.ascontiguousarray(xi, np.float64).reshape(-1, 3)
     out = np.empty((len(xi), 2), np.float64)
-    _chk(_lib.orc_exact_ft(V, len(V), F, len(F), xi, len(xi), out), "exact_ft")
-    return out.view(np.complex128).reshape(-1)
+    cap = 1 << 16
+    while True:
+        skipped = np.empty((cap, 2), np.int64)
+        n = C.c_int64(0)
+        rc = _lib.orc_exact_ft(V, len(V), F, len(F), xi, len(xi), out, skipped, cap, C.byref(n))
+        if rc != -2:
+            break
+        cap = int(n.value)
+    _chk(rc, "exact_ft")
+    res = out.view(np.complex128).reshape(-1)
+    for k, f in skipped[:n.value]:
+        res[k] += _exact_pair_mp(V[F[f]], xi[k])
+    return res
 
 
 def sigma_hat(r):

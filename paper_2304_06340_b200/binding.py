@@ -18,7 +18,7 @@ _lib = C.CDLL(LIB_PATH)
 
 SFD_OK = 0
 STATUS = {0: "SFD_OK", -1: "SFD_ERR_NULL", -2: "SFD_ERR_INVALID_ARG", -3: "SFD_ERR_BUFFER_TOO_SMALL",
-          -4: "SFD_ERR_WORKSPACE_TOO_SMALL", -5: "SFD_ERR_CUDA", -6: "SFD_ERR_CUFFT", -7: "SFD_ERR_UNSUPPORTED"}
+          -4: "SFD_ERR_WORKSPACE_TOO_SMALL", -5: "SFD_ERR_CUDA", -6: "SFD_ERR_RESERVED_6", -7: "SFD_ERR_UNSUPPORTED"}
 SFD_RULE_SYM6_DEG4, SFD_RULE_SYM12_DEG6 = 6, 12
 
 
@@ -72,7 +72,15 @@ _SIGS = {
     "sfd_weak_distance_host": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), _dbl,
                                          _P(_dbl), _P(_dbl)]),
     "sfd_launch_count": (C.c_longlong, []),
-    "sfd_probe_fp64": (C.c_int, [C.c_int, _vp, _P(_dbl), _P(_dbl)]),
+    "sfd_extents_workspace": (C.c_int, [_P(_sz)]),
+    "sfd_extents": (C.c_int, [_vp, _i64, _P(_dbl), _P(_dbl), _vp, _sz, _vp]),
+    "sfd_weak_distance_range_workspace": (C.c_int, [_i64, C.c_int, _P(sfd_freq_quadrature), _dbl, C.c_int32, C.c_int32,
+                                                    _dbl, _dbl, _P(_sz)]),
+    "sfd_weak_distance_range": (C.c_int, [_vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl, _P(sfd_freq_quadrature), C.c_int32,
+                                          C.c_int32, _dbl, _vp, _sz, _vp, _vp]),
+    "sfd_mesh_distance_workspace": (C.c_int, [_i64, _i64, C.c_int, _P(sfd_freq_quadrature), _dbl, _dbl, _dbl, _P(_sz)]),
+    "sfd_mesh_distance": (C.c_int, [_vp, _i64, _vp, _i64, _vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl,
+                                    _P(sfd_freq_quadrature), _dbl, _vp, _sz, _vp, _P(_dbl), _P(_dbl)]),
     "sfd_set_profiling": (C.c_int, [C.c_int]),
     "sfd_last_stage_times": (C.c_int, [_P(C.c_char_p), _P(C.c_float), C.c_int]),
 }
@@ -204,10 +212,19 @@ def sfd_surface_ft_plan(J, K, X, S, eps):
     return w.value, list(nf), list(n2)
 
 
+def sfd_extents(pts):
+    """(half-widths[3], centre[3]) of the bounding box of device points float64[n,3] (the library's own bounds kernels)."""
+    _dev_f64(pts, 3)
+    wb = _sz()
+    _chk(_lib.sfd_extents_workspace(C.byref(wb)))
+    work = _work(wb.value, pts.device)
+    half, centre = (_dbl * 3)(), (_dbl * 3)()
+    _chk(_lib.sfd_extents(_ptr(pts), pts.shape[0], half, centre, _ptr(work), work.numel(), _stream()))
+    return list(half), list(centre)
+
+
 def _half_widths(t):
-    if t.shape[0] == 0:
-        return [0.0, 0.0, 0.0]
-    return [float(v) * (1 + 1e-12) + 1e-300 for v in (0.5 * (t.amax(0) - t.amin(0))).tolist()]
+    return sfd_extents(t)[0]
 
 
 def sfd_surface_ft(x, w, xi, eps=0.0, work=None, out=None):
@@ -306,11 +323,29 @@ def sfd_launch_count():
     return int(_lib.sfd_launch_count())
 
 
-def sfd_probe_fp64(iters=4096):
-    """(TFLOP/s, ms) of a dependency-free DFMA loop on every SM: the measured FP64 peak."""
-    tf, ms = _dbl(), _dbl()
-    _chk(_lib.sfd_probe_fp64(int(iters), _stream(), C.byref(tf), C.byref(ms)))
-    return tf.value, ms.value
+def sfd_weak_distance_range_workspace(nF, rule, q, R, a_begin, a_end, eps, x_extent=1.0):
+    q = _quad(q)
+    wb = _sz()
+    _chk(_lib.sfd_weak_distance_range_workspace(int(nF), int(rule), C.byref(q), float(R), int(a_begin), int(a_end),
+                                                float(eps), float(x_extent), C.byref(wb)))
+    return wb.value
+
+
+def sfd_weak_distance_range(V, F, rule, s, R, q, a_begin, a_end, eps=0.0, work=None, x_extent=None, out=None):
+    """The distance's partial sum over the radial shells [a_begin, a_end) as a DEVICE pair float64[2] = (sum, comp),
+    I_shard = sum + comp: a rank's share of a multi-GPU evaluation; nothing crosses to the host."""
+    _dev_f64(V, 3)
+    assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous()
+    q = _quad(q)
+    if work is None:
+        if x_extent is None:
+            x_extent = max(_half_widths(V)) if eps > 0 else 1.0
+        work = _work(sfd_weak_distance_range_workspace(F.shape[0], rule, q, R, a_begin, a_end, eps, x_extent), V.device)
+    pair = out if out is not None else torch.empty(2, dtype=torch.float64, device=V.device)
+    _chk(_lib.sfd_weak_distance_range(_ptr(V), V.shape[0], _ptr(F), F.shape[0], int(rule), float(s), float(R), C.byref(q),
+                                      int(a_begin), int(a_end), float(eps), _ptr(work), work.numel(), _stream(),
+                                      _ptr(pair)))
+    return pair
 
 
 # ---- the paper's own variant: cube lattice, trapezoidal rule, its norm convention ---------------------------------
@@ -438,12 +473,26 @@ def sfd_reduce_pair(nuhat_a, nuhat_b, xi, W, s):
     return I.value
 
 
-def sfd_mesh_distance(Va, Fa, Vb, Fb, rule, s, R, q, eps=0.0):
+def sfd_mesh_distance_workspace(nFa, nFb, rule, q, R, eps, x_extent=1.0):
+    q = _quad(q)
+    wb = _sz()
+    _chk(_lib.sfd_mesh_distance_workspace(int(nFa), int(nFb), int(rule), C.byref(q), float(R), float(eps), float(x_extent),
+                                          C.byref(wb)))
+    return wb.value
+
+
+def sfd_mesh_distance(Va, Fa, Vb, Fb, rule, s, R, q, eps=0.0, work=None, x_extent=None):
     """(sqrt(I), I): H^{-s} distance between the surface measures of two meshes on the ball quadrature (q, R)."""
-    xa, wa = sfd_nodes(Va, Fa, rule)
-    xb, wb_ = sfd_nodes(Vb, Fb, rule)
-    xi, W = sfd_freq_nodes_device(q, R, Va.device)
-    na = sfd_surface_ft(xa, wa, xi, eps)
-    nb = sfd_surface_ft(xb, wb_, xi, eps)
-    I = sfd_reduce_pair(na, nb, xi, W, s)
-    return float(np.sqrt(I)), I
+    _dev_f64(Va, 3), _dev_f64(Vb, 3)
+    for F in (Fa, Fb):
+        assert F.is_cuda and F.dtype == torch.int32 and F.is_contiguous()
+    q = _quad(q)
+    if work is None:
+        if x_extent is None:
+            x_extent = max(_half_widths(Va) + _half_widths(Vb)) if eps > 0 else 1.0
+        work = _work(sfd_mesh_distance_workspace(Fa.shape[0], Fb.shape[0], rule, q, R, eps, x_extent), Va.device)
+    d, I = _dbl(), _dbl()
+    _chk(_lib.sfd_mesh_distance(_ptr(Va), Va.shape[0], _ptr(Fa), Fa.shape[0], _ptr(Vb), Vb.shape[0], _ptr(Fb), Fb.shape[0],
+                                int(rule), float(s), float(R), C.byref(q), float(eps), _ptr(work), work.numel(), _stream(),
+                                C.byref(d), C.byref(I)))
+    return d.value, I.value

@@ -6,11 +6,19 @@
 
 #include "atoms.cuh"
 #include "internal.cuh"
+#include "nufft3.cuh"
 
 namespace sfd {
 
 static thread_local char g_err[512] = "";
-long long g_launches = 0;
+std::atomic<long long> g_launches{0};
+
+// the device error word (common.cuh): one per device, zero-initialised with the module
+__device__ int32_t g_dev_flags;
+int32_t* device_flags() {
+  void* p = nullptr;
+  return cudaGetSymbolAddress(&p, g_dev_flags) == cudaSuccess ? static_cast<int32_t*>(p) : nullptr;
+}
 
 void set_error(const char* fmt, ...) {
   va_list ap;
@@ -81,6 +89,29 @@ int check_quadrature(const sfd_freq_quadrature* q, double R) {
   SFD_REQUIRE(R > 0.0 && std::isfinite(R), SFD_ERR_INVALID_ARG, "R must be positive and finite");
   return SFD_OK;
 }
+// Reads back what reduce_final_kernel left in d_res (I, the device error word, the (sum, comp) pair) and synchronises.
+int fetch_result(const char* who, cudaStream_t st, const double* d_res, double* I) {
+  double h[2] = {0.0, 0.0};
+  cudaError_t e = cudaMemcpyAsync(h, d_res, sizeof(h), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) {
+    set_error("%s: %s", who, cudaGetErrorString(e));
+    return SFD_ERR_CUDA;
+  }
+  SFD_REQUIRE(h[1] == 0.0, SFD_ERR_INVALID_ARG,
+              "%s: a face index outside [0, nV) was met on the device (by this call or an earlier sfd_nodes / "
+              "sfd_exact_ft / distance call on this device)", who);
+  *I = h[0];
+  return SFD_OK;
+}
+
+__global__ void copy_pair_kernel(const double* __restrict__ res, double* __restrict__ out) {
+  out[0] = res[2];
+  out[1] = res[3];
+  // a bad face index met on the way poisons the partial sum, so that the caller's all-reduce cannot hide it
+  if (res[1] != 0.0) out[0] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
 int check_eps(double eps) {
   SFD_REQUIRE(eps == 0.0 || (eps >= 1e-14 && eps < 1.0), SFD_ERR_INVALID_ARG,
               "eps must be 0 (direct sum) or in [1e-14, 1), got %g", eps);
@@ -105,10 +136,50 @@ int sfd_release_cache(void) {
   return nufft3_release_cache();
 }
 
-long long sfd_launch_count(void) { return g_launches; }
+long long sfd_launch_count(void) { return g_launches.load(); }
 
-int sfd_probe_fp64(int iters, sfd_stream stream, double* h_tflops, double* h_ms) {
-  return probe_fp64(iters, as_stream(stream), h_tflops, h_ms);
+// ---- extents of a point set (A5-1 as a call of its own) ----------------------------------------------
+int sfd_extents_workspace(size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_extents_workspace: bytes is NULL");
+  *bytes = align_up(64) + align_up((size_t)kBoundsBlocks * 6 * sizeof(double));
+  return SFD_OK;
+}
+int sfd_extents(const double* d_pts, int64_t n, double h_half[3], double h_centre[3], void* d_work, size_t work_bytes,
+                sfd_stream stream) {
+  SFD_REQUIRE(n >= 0, SFD_ERR_INVALID_ARG, "n must be >= 0");
+  SFD_REQUIRE(h_half, SFD_ERR_NULL, "sfd_extents: h_half is NULL");
+  if (n == 0) {
+    for (int d = 0; d < 3; ++d) {
+      h_half[d] = 0.0;
+      if (h_centre) h_centre[d] = 0.0;
+    }
+    return SFD_OK;
+  }
+  size_t need = 0;
+  sfd_extents_workspace(&need);
+  SFD_REQUIRE(d_pts, SFD_ERR_NULL, "sfd_extents: d_pts is NULL");
+  SFD_REQUIRE(d_work && work_bytes >= need, SFD_ERR_WORKSPACE_TOO_SMALL, "sfd_extents needs %zu workspace bytes, got %zu",
+              need, work_bytes);
+  cudaStream_t st = as_stream(stream);
+  double* d_out = static_cast<double*>(d_work);
+  SFD_TRY(bounds_minmax(d_pts, n, d_out, reinterpret_cast<double*>(static_cast<char*>(d_work) + 256), st));
+  double hb[6];
+  int32_t flag = 0;
+  int32_t* d_flags = device_flags();
+  SFD_CUDA_TRY(cudaMemcpyAsync(hb, d_out, sizeof(hb), cudaMemcpyDeviceToHost, st));
+  if (d_flags) SFD_CUDA_TRY(cudaMemcpyAsync(&flag, d_flags, sizeof(flag), cudaMemcpyDeviceToHost, st));
+  SFD_CUDA_TRY(cudaStreamSynchronize(st));
+  if (flag) {
+    SFD_CUDA_TRY(cudaMemsetAsync(d_flags, 0, sizeof(flag), st));
+    SFD_REQUIRE(false, SFD_ERR_INVALID_ARG,
+                "sfd_extents: a face index outside [0, nV) was met on the device by an earlier sfd_nodes / sfd_exact_ft call");
+  }
+  for (int d = 0; d < 3; ++d) {
+    SFD_REQUIRE(std::isfinite(hb[d]) && std::isfinite(hb[3 + d]), SFD_ERR_INVALID_ARG, "sfd_extents: non-finite coordinate");
+    h_half[d] = 0.5 * (hb[3 + d] - hb[d]) * (1.0 + 1e-12) + 1e-300;   // the margin nufft3() itself applies
+    if (h_centre) h_centre[d] = 0.5 * (hb[d] + hb[3 + d]);
+  }
+  return SFD_OK;
 }
 
 int sfd_set_profiling(int on) {
@@ -291,27 +362,31 @@ int sfd_reduce(const double* d_nuhat, const double* d_xi, const double* d_W, int
   cudaStream_t st = as_stream(stream);
   double* d_res = nullptr;
   SFD_TRY(reduce_enqueue(d_nuhat, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res));
-  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
-  SFD_CUDA_TRY(cudaStreamSynchronize(st));
-  return SFD_OK;
+  return fetch_result("sfd_reduce", st, d_res, h_I);
 }
 
 // ---- whole path -----------------------------------------------------------------------------------
 namespace {
 struct DistLayout {
   int64_t J, K;
-  size_t x, w, xi, W, nu, tab, red, ft, total;
+  size_t x, w, xi, W, nu, nu2, tab, red, ft, total;
   size_t ft_bytes, tab_bytes, red_bytes;
 };
-int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps, double x_extent,
-                DistLayout* L) {
-  SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
+// Number of nodes the distance calls visit on the shells [a0, a1): the xi_3 >= 0 half when n_phi is even (R18).
+int64_t visited_nodes(const sfd_freq_quadrature* q, int a0, int a1) {
+  return (q->n_phi & 1) == 0 ? freq_half_count(q, a0, a1) : (int64_t)(a1 - a0) * q->n_theta * q->n_phi;
+}
+// J2 > 0: a second set of atoms (mesh against mesh) shares the buffers: x / w sized for the larger, two nuhat arrays.
+int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double reach, int a0, int a1, double eps, double x_extent,
+                DistLayout* L, int64_t nF2 = 0) {
+  SFD_REQUIRE(nF >= 0 && nF2 >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
   SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
-  SFD_TRY(check_quadrature(q, R));
+  SFD_TRY(check_quadrature(q, reach));
+  SFD_REQUIRE(0 <= a0 && a0 <= a1 && a1 <= q->n_r, SFD_ERR_INVALID_ARG, "radial range [%d,%d) outside [0,%d)", a0, a1, q->n_r);
   SFD_TRY(check_eps(eps));
-  L->J = nF * rule;
-  L->K = (int64_t)q->n_r * q->n_theta * q->n_phi;
-  const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {R, R, R};
+  L->J = std::max(nF, nF2) * rule;
+  L->K = visited_nodes(q, a0, a1);
+  const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {reach, reach, reach};
   if (eps > 0.0) SFD_REQUIRE(x_extent > 0.0 && std::isfinite(x_extent), SFD_ERR_INVALID_ARG, "x_extent must be > 0");
   SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, eps, &L->ft_bytes));
   L->tab_bytes = freq_tables_bytes(q);
@@ -327,41 +402,31 @@ int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, do
   L->xi = put((size_t)L->K * 24);
   L->W = put((size_t)L->K * 8);
   L->nu = put((size_t)L->K * 16);
+  L->nu2 = put(nF2 > 0 ? (size_t)L->K * 16 : 0);
   L->tab = put(L->tab_bytes);
   L->red = put(L->red_bytes);
   L->ft = put(L->ft_bytes);
   L->total = o;
   return SFD_OK;
 }
-}  // namespace
 
-int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps,
-                                double x_extent, size_t* bytes) {
-  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_weak_distance_workspace: bytes is NULL");
-  DistLayout L;
-  SFD_TRY(dist_layout(nF, rule, q, R, eps, x_extent, &L));
-  *bytes = L.total;
-  return SFD_OK;
-}
-
-int sfd_weak_distance_targets(const sfd_freq_quadrature* q, int64_t* K_eval) {
-  SFD_REQUIRE(K_eval, SFD_ERR_NULL, "sfd_weak_distance_targets: K_eval is NULL");
-  SFD_TRY(check_quadrature(q, 1.0));
-  *K_eval = (q->n_phi & 1) == 0 ? freq_half_count(q, 0, q->n_r) : (int64_t)q->n_r * q->n_theta * q->n_phi;
-  return SFD_OK;
-}
-
-int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
-                      double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes,
-                      sfd_stream stream, double* h_distance, double* h_I) {
+// The distance on the radial shells [a0, a1) of the rule: atoms -> nodes of those shells (half rule) -> transform ->
+// reduction.  Leaves the result block of reduce_final_kernel (I, flag, sum, comp) at *d_res; does not read it back.
+// Vb != nullptr: a second mesh takes the place of the unit sphere's closed form.
+int distance_enqueue(const char* who, const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, const double* d_Vb,
+                     int64_t nVb, const int32_t* d_Fb, int64_t nFb, int rule, double s, double R,
+                     const sfd_freq_quadrature* q, int a0, int a1, double eps, void* d_work, size_t work_bytes,
+                     sfd_stream stream, double** d_res) {
   SFD_REQUIRE(s > 0.5 && s < 1e6, SFD_ERR_INVALID_ARG, "Sobolev order s must exceed 1/2 (P:113), got %g", s);
-  SFD_REQUIRE(nF == 0 || (d_vertices && d_faces), SFD_ERR_NULL, "sfd_weak_distance: NULL mesh buffer");
+  SFD_REQUIRE(nF == 0 || (d_V && d_F), SFD_ERR_NULL, "%s: NULL mesh buffer", who);
+  SFD_REQUIRE(nFb == 0 || (d_Vb && d_Fb), SFD_ERR_NULL, "%s: NULL mesh buffer (second mesh)", who);
+  const bool pair = d_Vb != nullptr;
   DistLayout L;
   // the workspace may have been sized with any x_extent: recompute the fixed part, give the rest to the transform
-  SFD_TRY(dist_layout(nF, rule, q, R, 0.0, 1.0, &L));
+  SFD_TRY(dist_layout(nF, rule, q, R, a0, a1, 0.0, 1.0, &L, pair ? std::max<int64_t>(nFb, 1) : 0));
   SFD_TRY(check_eps(eps));
-  SFD_REQUIRE(d_work && work_bytes >= L.ft, SFD_ERR_WORKSPACE_TOO_SMALL,
-              "sfd_weak_distance needs at least %zu workspace bytes, got %zu", L.total, work_bytes);
+  SFD_REQUIRE(d_work && work_bytes >= L.ft, SFD_ERR_WORKSPACE_TOO_SMALL, "%s needs at least %zu workspace bytes, got %zu", who,
+              L.total, work_bytes);
   cudaStream_t st = as_stream(stream);
   char* base = static_cast<char*>(d_work);
   double* x = reinterpret_cast<double*>(base + L.x);
@@ -369,36 +434,144 @@ int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_fac
   double* xi = reinterpret_cast<double*>(base + L.xi);
   double* W = reinterpret_cast<double*>(base + L.W);
   double* nu = reinterpret_cast<double*>(base + L.nu);
-  prof_begin(st);
-  int rc = nodes(d_vertices, nV, d_faces, nF, rule, x, w, st);
-  prof_mark("nodes", st);
+  double* nu2 = reinterpret_cast<double*>(base + L.nu2);
   FreqTables t;
-  if (rc == SFD_OK) rc = freq_tables(q, R, t);
-  // The ball rule is symmetric under xi -> -xi (even n_phi) and the measure is real: the nodes with xi_3 >= 0 carry
+  SFD_TRY(freq_tables(q, R, t));
+  // The ball rule is symmetric under xi -> -xi (even n_phi) and the measures are real: the nodes with xi_3 >= 0 carry
   // the whole sum with doubled weights (nodes.cu freq_expand), so only they are generated, transformed and reduced.
   const bool half = (q->n_phi & 1) == 0;
-  const int64_t K = half ? freq_half_count(q, 0, q->n_r) : L.K;
-  if (rc == SFD_OK) rc = freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st, 0, -1, half);
-  prof_mark("freq_nodes", st);
-  // extents without a pass over the atoms and the nodes: the atoms lie in the hull of the vertices, the nodes in [-R, R]^3
-  ExtentHint hint;
-  hint.d_hull = d_vertices;
-  hint.n_hull = nV;
-  hint.target_reach = R;
-  hint.target_ball = true;   // the ball rule's nodes satisfy |xi| <= R
-  if (rc == SFD_OK) rc = surface_ft_impl(x, w, L.J, xi, K, eps, nu, base + L.ft, work_bytes - L.ft, stream, true, &hint);
-  double* d_res = nullptr;
-  if (rc == SFD_OK) rc = reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, &d_res);
-  prof_mark("reduce", st);
-  double I = 0.0;
-  if (rc == SFD_OK) {
-    cudaError_t e = cudaMemcpyAsync(&I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) {
-      set_error("sfd_weak_distance: %s", cudaGetErrorString(e));
-      rc = SFD_ERR_CUDA;
-    }
+  const int64_t K = L.K;
+  if (K == 0 || a0 == a1) {
+    double* res = reinterpret_cast<double*>(base + L.red);
+    SFD_CUDA_TRY(cudaMemsetAsync(res, 0, 4 * sizeof(double), st));
+    *d_res = res;
+    return SFD_OK;
   }
+  SFD_TRY(freq_expand(q, t, xi, W, base + L.tab, L.tab_bytes, st, a0, a1, half));
+  prof_mark("freq_nodes", st);
+  for (int m = 0; m < (pair ? 2 : 1); ++m) {
+    const double* V = m ? d_Vb : d_V;
+    const int32_t* F = m ? d_Fb : d_F;
+    const int64_t nv = m ? nVb : nV, nf = m ? nFb : nF;
+    SFD_TRY(nodes(V, nv, F, nf, rule, x, w, st));
+    prof_mark("nodes", st);
+    // extents without a pass over the atoms and the nodes: the atoms lie in the hull of the vertices, the nodes of the
+    // shells [a0, a1) in the ball of radius r_{a1-1} (Gauss-Legendre nodes ascend)
+    ExtentHint hint;
+    hint.d_hull = V;
+    hint.n_hull = nv;
+    hint.target_reach = t.r[a1 - 1];
+    hint.target_ball = true;
+    SFD_TRY(surface_ft_impl(x, w, nf * rule, xi, K, eps, m ? nu2 : nu, base + L.ft, work_bytes - L.ft, stream, true, &hint));
+  }
+  SFD_TRY(reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, d_res, 1.0, -1.0, pair ? nu2 : nullptr));
+  prof_mark("reduce", st);
+  return SFD_OK;
+}
+}  // namespace
+
+int sfd_weak_distance_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, double eps,
+                                double x_extent, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_weak_distance_workspace: bytes is NULL");
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  DistLayout L;
+  SFD_TRY(dist_layout(nF, rule, q, R, 0, q->n_r, eps, x_extent, &L));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int sfd_weak_distance_targets(const sfd_freq_quadrature* q, int64_t* K_eval) {
+  SFD_REQUIRE(K_eval, SFD_ERR_NULL, "sfd_weak_distance_targets: K_eval is NULL");
+  SFD_TRY(check_quadrature(q, 1.0));
+  *K_eval = visited_nodes(q, 0, q->n_r);
+  return SFD_OK;
+}
+
+int sfd_weak_distance(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
+                      double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes,
+                      sfd_stream stream, double* h_distance, double* h_I) {
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  cudaStream_t st = as_stream(stream);
+  prof_begin(st);
+  double* d_res = nullptr;
+  int rc = distance_enqueue("sfd_weak_distance", d_vertices, nV, d_faces, nF, nullptr, 0, nullptr, 0, rule, s, R, q, 0,
+                            q->n_r, eps, d_work, work_bytes, stream, &d_res);
+  double I = 0.0;
+  if (rc == SFD_OK) rc = fetch_result("sfd_weak_distance", st, d_res, &I);
+  prof_end(st);
+  if (rc != SFD_OK) return rc;
+  if (h_I) *h_I = I;
+  if (h_distance) *h_distance = std::sqrt(I);
+  return SFD_OK;
+}
+
+// ---- a radial shard of the distance (multi-GPU: DESIGN.md "Multi-GPU") ---------------------------------------
+int sfd_weak_distance_range_workspace(int64_t nF, int rule, const sfd_freq_quadrature* q, double R, int32_t a_begin,
+                                      int32_t a_end, double eps, double x_extent, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_weak_distance_range_workspace: bytes is NULL");
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  SFD_TRY(check_quadrature(q, R));
+  SFD_REQUIRE(0 <= a_begin && a_begin <= a_end && a_end <= q->n_r, SFD_ERR_INVALID_ARG,
+              "radial range [%d,%d) outside [0,%d)", a_begin, a_end, q->n_r);
+  // the transform's grids are sized by the shard's own reach r_{a_end-1} <= R
+  double reach = R;
+  if (a_end > a_begin) {
+    FreqTables t;
+    SFD_TRY(freq_tables(q, R, t));
+    reach = t.r[a_end - 1];
+  }
+  DistLayout L;
+  SFD_TRY(dist_layout(nF, rule, q, reach, a_begin, a_end, eps, x_extent, &L));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int sfd_weak_distance_range(const double* d_vertices, int64_t nV, const int32_t* d_faces, int64_t nF, int rule, double s,
+                            double R, const sfd_freq_quadrature* q, int32_t a_begin, int32_t a_end, double eps, void* d_work,
+                            size_t work_bytes, sfd_stream stream, double* d_partial) {
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  SFD_REQUIRE(d_partial, SFD_ERR_NULL, "sfd_weak_distance_range: d_partial is NULL");
+  cudaStream_t st = as_stream(stream);
+  prof_begin(st);
+  double* d_res = nullptr;
+  int rc = distance_enqueue("sfd_weak_distance_range", d_vertices, nV, d_faces, nF, nullptr, 0, nullptr, 0, rule, s, R, q,
+                            a_begin, a_end, eps, d_work, work_bytes, stream, &d_res);
+  if (rc == SFD_OK) {
+    copy_pair_kernel<<<1, 1, 0, st>>>(d_res, d_partial);
+    rc = launch_check("copy_pair_kernel");
+  }
+  prof_end(st);
+  return rc;
+}
+
+// ---- mesh against mesh, whole path ---------------------------------------------------------------
+int sfd_mesh_distance_workspace(int64_t nF_a, int64_t nF_b, int rule, const sfd_freq_quadrature* q, double R, double eps,
+                                double x_extent, size_t* bytes) {
+  SFD_REQUIRE(bytes, SFD_ERR_NULL, "sfd_mesh_distance_workspace: bytes is NULL");
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  DistLayout L;
+  SFD_TRY(dist_layout(nF_a, rule, q, R, 0, q->n_r, eps, x_extent, &L, std::max<int64_t>(nF_b, 1)));
+  *bytes = L.total;
+  return SFD_OK;
+}
+
+int sfd_mesh_distance(const double* d_vertices_a, int64_t nV_a, const int32_t* d_faces_a, int64_t nF_a,
+                      const double* d_vertices_b, int64_t nV_b, const int32_t* d_faces_b, int64_t nF_b, int rule, double s,
+                      double R, const sfd_freq_quadrature* q, double eps, void* d_work, size_t work_bytes, sfd_stream stream,
+                      double* h_distance, double* h_I) {
+  SFD_REQUIRE(q, SFD_ERR_NULL, "frequency quadrature is NULL");
+  SFD_REQUIRE(nF_a >= 0 && nF_b >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
+  // an empty second mesh is the zero measure, not "compare with the sphere": keep the pair path by passing a dummy pointer
+  static const double kNoVertices[3] = {0.0, 0.0, 0.0};
+  const double* Vb = d_vertices_b ? d_vertices_b : (nF_b == 0 ? kNoVertices : nullptr);
+  SFD_REQUIRE(Vb, SFD_ERR_NULL, "sfd_mesh_distance: NULL mesh buffer (second mesh)");
+  cudaStream_t st = as_stream(stream);
+  prof_begin(st);
+  double* d_res = nullptr;
+  int rc = distance_enqueue("sfd_mesh_distance", d_vertices_a, nV_a, d_faces_a, nF_a, Vb, nV_b, d_faces_b, nF_b, rule, s, R, q,
+                            0, q->n_r, eps, d_work, work_bytes, stream, &d_res);
+  double I = 0.0;
+  if (rc == SFD_OK) rc = fetch_result("sfd_mesh_distance", st, d_res, &I);
   prof_end(st);
   if (rc != SFD_OK) return rc;
   if (h_I) *h_I = I;
@@ -442,9 +615,7 @@ int sfd_reduce_ex(const double* d_nuhat, const double* d_xi, const double* d_W, 
   cudaStream_t st = as_stream(stream);
   double* d_res = nullptr;
   SFD_TRY(reduce_enqueue(d_nuhat, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res, xi_scale, prefactor));
-  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
-  SFD_CUDA_TRY(cudaStreamSynchronize(st));
-  return SFD_OK;
+  return fetch_result("sfd_reduce_ex", st, d_res, h_I);
 }
 
 namespace {
@@ -527,16 +698,16 @@ int sfd_reduce_lattice(const double* d_nuhat, int32_t M, double xi_max, double s
   cudaStream_t st = as_stream(stream);
   double* d_res = nullptr;
   SFD_TRY(reduce_lattice_enqueue(d_nuhat, M, xi_max, s, d_work, work_bytes, st, &d_res, xi_scale, prefactor));
-  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
-  SFD_CUDA_TRY(cudaStreamSynchronize(st));
-  return SFD_OK;
+  return fetch_result("sfd_reduce_lattice", st, d_res, h_I);
 }
 
 namespace {
 int lattice_layout(int64_t nF, int rule, int M, double xi_max, double eps, double x_extent, DistLayout* L) {
   SFD_REQUIRE(nF >= 0, SFD_ERR_INVALID_ARG, "nF must be >= 0");
   SFD_REQUIRE(rule == 6 || rule == 12 || rule == 64, SFD_ERR_INVALID_ARG, "unknown triangle rule %d (6, 12 or 64)", rule);
-  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 2046, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..2046 (got %d)", M);
+  // the reduction over the lattice indexes its nodes with 32 bits: (M+1)^3 < 2^32 (the same limit as sfd_reduce_lattice),
+  // checked here so that the workspace query and the call reject up front instead of after the transform
+  SFD_REQUIRE(M >= 2 && (M & 1) == 0 && M <= 1624, SFD_ERR_INVALID_ARG, "lattice size M must be even, 2..1624 (got %d)", M);
   SFD_REQUIRE(xi_max > 0.0 && std::isfinite(xi_max), SFD_ERR_INVALID_ARG, "xi_max must be positive and finite");
   SFD_TRY(check_eps(eps));
   L->J = nF * rule;
@@ -557,6 +728,7 @@ int lattice_layout(int64_t nF, int rule, int M, double xi_max, double eps, doubl
   L->xi = put((size_t)L->K * 24);
   L->W = put((size_t)L->K * 8);
   L->nu = put((size_t)L->K * 16);
+  L->nu2 = L->nu;
   L->tab = put(256);
   L->red = put(L->red_bytes);
   L->ft = put(L->ft_bytes);
@@ -620,14 +792,7 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
               : reduce_lattice_enqueue(nu, M, xi_max, -s_paper, base + L.red, L.red_bytes, st, &d_res, inv_two_pi, 1.0);
   prof_mark("reduce", st);
   double I = 0.0;
-  if (rc == SFD_OK) {
-    cudaError_t e = cudaMemcpyAsync(&I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) {
-      set_error("sfd_weak_distance_lattice: %s", cudaGetErrorString(e));
-      rc = SFD_ERR_CUDA;
-    }
-  }
+  if (rc == SFD_OK) rc = fetch_result("sfd_weak_distance_lattice", st, d_res, &I);
   prof_end(st);
   if (rc != SFD_OK) return rc;
   if (h_I) *h_I = I;
@@ -644,9 +809,7 @@ int sfd_reduce_pair(const double* d_nuhat_a, const double* d_nuhat_b, const doub
   cudaStream_t st = as_stream(stream);
   double* d_res = nullptr;
   SFD_TRY(reduce_enqueue(d_nuhat_a, d_xi, d_W, K, s, d_work, work_bytes, st, &d_res, 1.0, -1.0, d_nuhat_b));
-  SFD_CUDA_TRY(cudaMemcpyAsync(h_I, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
-  SFD_CUDA_TRY(cudaStreamSynchronize(st));
-  return SFD_OK;
+  return fetch_result("sfd_reduce_pair", st, d_res, h_I);
 }
 
 // ---- host-buffer entry points -----------------------------------------------------------------------

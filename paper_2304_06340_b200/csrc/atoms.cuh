@@ -19,12 +19,13 @@ struct MeshAtoms {
 // rule = the four columns lam0[q], lam1[q], lam2[q], om[q] of the rule (4 x Q doubles, in shared or global memory)
 __device__ __forceinline__ void atom_eval(const double* __restrict__ V, int64_t nV, const int32_t* __restrict__ F, int64_t j,
                                           int Q, const double* __restrict__ rule, double& x0, double& x1, double& x2,
-                                          double& w) {
+                                          double& w, int32_t* flags = nullptr) {
   const int64_t f = j / Q;
   const int i = (int)(j - f * Q);
   const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
   if (i0 < 0 || i1 < 0 || i2 < 0 || i0 >= nV || i1 >= nV || i2 >= nV) {
     x0 = x1 = x2 = w = __longlong_as_double(0x7ff8000000000000LL);   // a face with a bad index poisons its atoms
+    if (flags) atomicOr(flags, kFlagBadIndex);                       // ... and is reported at the next synchronising call
     return;
   }
   double p0[3], p1[3], p2[3], e1[3], e2[3];

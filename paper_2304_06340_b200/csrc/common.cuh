@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -38,7 +39,14 @@ void set_error(const char* fmt, ...);
   } while (0)
 
 // number of kernels of this library launched so far in the process (sfd_launch_count)
-extern long long g_launches;
+extern std::atomic<long long> g_launches;
+
+// Device-side error word, one per device, owned by the library (api.cu).  A kernel that meets invalid input it can
+// only see on the device -- a face index outside [0, nV) -- sets kFlagBadIndex with atomicOr; the final kernel of
+// every reduction collects and clears the word, and the synchronising call that reads the result back returns
+// SFD_ERR_INVALID_ARG ("checked on device, reported at the next synchronising call").
+constexpr int kFlagBadIndex = 1;
+int32_t* device_flags();   // device address of the word on the current device (nullptr if the lookup fails)
 
 inline int launch_check(const char* what) {
   ++g_launches;
@@ -88,7 +96,8 @@ void prof_end(cudaStream_t st);
 // n = round(t * 2/pi); two-term Cody-Waite reduction with FMA (t - n*PIO2_HI is exact, see
 // DESIGN.md "direct sum"); degree-13/14 polynomials on [-pi/4, pi/4]; quadrant fix-up on the
 // integer pipe.  Max error ~1 ulp of the result + the fp64 rounding of t itself.
-// Coefficients: Chebyshev-node interpolants derived and checked by csrc/gen_sincos_coeffs.py.
+// Coefficients: Chebyshev-node interpolants of (sin(sqrt z)/sqrt z - 1)/z and (cos(sqrt z) - 1 + z/2)/z^2 on
+// [0, (1.02 pi/4)^2], computed at 60 digits; the literals are checked against mpmath by tests/test_kernel_constants_cpu.py.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void sincos_fp64(double t, double& s, double& c) {
   const double kTwoOverPi = 6.36619772367581382433e-01;
@@ -101,7 +110,7 @@ __device__ __forceinline__ void sincos_fp64(double t, double& s, double& c) {
   double r = __fma_rn(-n, kPio2Hi, t);
   r = __fma_rn(-n, kPio2Lo, r);
   const double z = r * r;
-  // sin(r) = r + r z P(z), cos(r) = 1 - z/2 + z^2 Q(z); P, Q from gen_sincos_coeffs.py
+  // sin(r) = r + r z P(z), cos(r) = 1 - z/2 + z^2 Q(z); P, Q: see above
   double ps = 1.59124614998394676947e-10;
   ps = __fma_rn(ps, z, -2.50510515868469095197e-8);
   ps = __fma_rn(ps, z, 2.75573157096352918481e-6);

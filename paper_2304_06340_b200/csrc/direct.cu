@@ -50,7 +50,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // thread, so the phase arrives in units of 1/kTab of a turn: tq = n + f with n = rint(tq) (the 1.5*2^52 trick: three
 // exact additions) and |f| <= 1/2, i.e. a residual angle of at most pi/256.  The table holds (cos, sin)(2 pi k / kTab)
 // for the whole turn, so there is no quadrant logic at all; sin and cos of the residual need 3 coefficients each
-// (gen_sincos_coeffs.py table: max error 1.2e-18 and 2.3e-16); one complex rotation joins the two.  18 FP64-pipe
+// (Chebyshev-node fits at 60 digits, max error 1.2e-18 and 2.3e-16: tests/test_kernel_constants_cpu.py); one complex rotation joins the two.  18 FP64-pipe
 // instructions per pair (phase 3, reduction 3, f^2 1, sin 3, cos 2, rotate + accumulate 6) against 21 plus a 10-instruction
 // integer fix-up for the polynomial-only version: measured 1.31x faster (profiles/r1e_direct_sum_table.md), because
 // every non-FP64 instruction costs an issue cycle next to a 2-cycle DFMA.

@@ -44,7 +44,7 @@ __constant__ double c_series[18] = {
     1.0 / 6402373705728000.0,  -1.0 / 121645100408832000.0};
 
 __global__ void __launch_bounds__(256) face_prep_kernel(const double* __restrict__ V, int64_t nV, const int32_t* __restrict__ F,
-                                                       int64_t nF, FaceRec* __restrict__ out) {
+                                                       int64_t nF, FaceRec* __restrict__ out, int32_t* __restrict__ flags) {
   const int64_t f = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (f >= nF) return;
   const int32_t i0 = F[3 * f], i1 = F[3 * f + 1], i2 = F[3 * f + 2];
@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(256) face_prep_kernel(const double* __restrict
 #pragma unroll
     for (int c = 0; c < 3; ++c) r.p0[c] = r.e1[c] = r.e2[c] = nan;
     r.a2 = nan;
+    if (flags) atomicOr(flags, kFlagBadIndex);
   } else {
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -180,7 +181,7 @@ int exact_ft(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, cons
   SFD_REQUIRE(d_work && work_bytes >= exact_ft_workspace(nF), SFD_ERR_WORKSPACE_TOO_SMALL,
               "sfd_exact_ft needs %zu workspace bytes, got %zu", exact_ft_workspace(nF), work_bytes);
   FaceRec* faces = static_cast<FaceRec*>(d_work);
-  face_prep_kernel<<<(unsigned)((nF + 255) / 256), 256, 0, st>>>(d_V, nV, d_F, nF, faces);
+  face_prep_kernel<<<(unsigned)((nF + 255) / 256), 256, 0, st>>>(d_V, nV, d_F, nF, faces, device_flags());
   SFD_TRY(launch_check("face_prep_kernel"));
   const int64_t blocks = (K + kThreads - 1) / kThreads;
   // few frequencies: split the faces over blockIdx.y so that every SM has work (partial sums meet in fp64 reductions)

@@ -57,9 +57,6 @@ size_t exact_ft_workspace(int64_t nF);
 int exact_ft(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, const double* d_xi, int64_t K, double* d_out,
              void* d_work, size_t work_bytes, cudaStream_t st);
 
-// ---- probe.cu: measured FP64 FMA peak of the device (the direct sum's roofline denominator) ----------
-int probe_fp64(int iters, cudaStream_t st, double* h_tflops, double* h_ms);
-
 // ---- nufft3.cu: A5 three-dimensional type-3 nonuniform FFT -------------------------------
 struct Nufft3Sizes {
   int w;               // kernel width in fine-grid cells

@@ -73,7 +73,7 @@ void fill_rule(int q, RuleTable& t) {
 template <int Q>
 __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V, const int32_t* __restrict__ F,
                                                     int64_t nF, int64_t nV, double* __restrict__ x,
-                                                    double* __restrict__ w) {
+                                                    double* __restrict__ w, int32_t* __restrict__ flags) {
   __shared__ double sx[3 * 256];
   // the rule, one array per column: a warp's 32 atoms read 32 different rows, which the constant cache would serialise
   __shared__ double s_rule[4 * Q];
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(256) nodes_kernel(const double* __restrict__ V
   const int64_t J = nF * Q;
   if (j < J) {
     double wj;
-    atom_eval(V, nV, F, j, Q, s_rule, sx[3 * threadIdx.x], sx[3 * threadIdx.x + 1], sx[3 * threadIdx.x + 2], wj);
+    atom_eval(V, nV, F, j, Q, s_rule, sx[3 * threadIdx.x], sx[3 * threadIdx.x + 1], sx[3 * threadIdx.x + 2], wj, flags);
     w[j] = wj;
   }
   __syncthreads();
@@ -334,12 +334,13 @@ int nodes(const double* d_V, int64_t nV, const int32_t* d_F, int64_t nF, int rul
   }
   const int64_t J = nF * rule;
   const unsigned blocks = (unsigned)((J + 255) / 256);
+  int32_t* flags = device_flags();
   if (rule == 6)
-    nodes_kernel<6><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+    nodes_kernel<6><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w, flags);
   else if (rule == 64)
-    nodes_kernel<64><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+    nodes_kernel<64><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w, flags);
   else
-    nodes_kernel<12><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w);
+    nodes_kernel<12><<<blocks, 256, 0, st>>>(d_V, d_F, nF, nV, d_x, d_w, flags);
   return launch_check("nodes_kernel");
 }
 

@@ -14,6 +14,7 @@
 //   5. bin-sort targets, interpolate at u2_k = (xi_k-D) n2/(2 sigma S) + n2/2 (interp.cu)
 //   6. divide by the kernel's transform at the non-integer frequencies, multiply by e^{-i (xi_k-D).C}
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -461,23 +462,33 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     B.n_hi = nf0; B.n_lo = no2;
     B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
     B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
-    // Targets inside the ball |u2 - n2/2| <= n2/4 (the ball rule): only the part of the band within it, grown by the
-    // footprint's reach (w/2 + 1 cells per axis: sqrt 3 times that along the space diagonal) and a cell of slack, is
-    // ever read.  Pass B stops
-    // storing the m1 outside the ball's section at its m2; pass C skips the (m1, m2) columns outside the projection
-    // and stores only the m0 inside the ball.
+    // Targets inside the ball |xi| <= R (the ball rule): in inner-grid cells they fill the ellipsoid E with semi-axes
+    // a_d = n2_d / 4 about the centre (the axes differ when the mesh's bounding box is not a cube).  What the
+    // interpolation reads is E (+) the footprint cube of half-width w/2 + 1 cells, inside E (+) Ball(r), r = sqrt 3 times
+    // that plus a cell of slack, and since E contains Ball(a_min): E (+) Ball(r) is inside (1 + r / a_min) E.  Only that
+    // scaled ellipsoid of the band is computed and stored (for a cubic box this is the ball of radius a + r).  Pass B
+    // stops storing the m1 outside the ellipsoid's section at its m2; pass C skips the (m1, m2) columns outside its
+    // projection and stores only the m0 inside it.
     const bool ball = hint && hint->target_ball && hint->target_reach > 0.0;
     const double reach = (0.5 * p.w + 1.0) * 1.7321 + 1.0;
+    const double a_min = 0.25 * std::min(p.n2[0], std::min(p.n2[1], p.n2[2]));
+    const double grow = 1.0 + reach / a_min;
     if (ball) {
       B.ball = 2;
       B.ball_nb = 0;
       B.ball_ca = 0.0; B.ball_ira = 0.0;
       B.ball_cb = 0.5 * p.n2[2] - p.lo[2];
-      B.ball_irb = 1.0 / (0.25 * p.n2[2] + reach);
+      B.ball_irb = 1.0 / (0.25 * p.n2[2] * grow);
       B.ball_ct = 0.5 * p.n2[1] - p.lo[1];
-      B.ball_rt = 0.25 * p.n2[1] + reach;
+      B.ball_rt = 0.25 * p.n2[1] * grow;
     }
+    // SFD_DEBUG_POISON_BAND=1 (tests): fill each pass's output buffer with NaN first, so that any cell the pruned passes
+    // leave unstored and a later stage reads anyway shows up as a NaN distance (tests/test_gpu_fullsize.py)
+    const char* poison_env = std::getenv("SFD_DEBUG_POISON_BAND");
+    const bool poison = poison_env && poison_env[0] == '1';
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16, st));
     SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufx, 0xff, L.bufy - L.bufx, st));
     FftPass C{};   // axis 0: columns (m1, m2) of Y -> X[m0][m1][m2]
     C.N = p.n2[0]; C.n_in = p.nf[0]; C.lo = p.lo[0]; C.nout = p.nout[0];
     C.n_hi = 1; C.n_lo = no1 * no2;
@@ -488,10 +499,10 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
       C.ball_nb = (int)no2;
       C.ball_ca = 0.5 * p.n2[1] - p.lo[1];
       C.ball_cb = 0.5 * p.n2[2] - p.lo[2];
-      C.ball_ira = 1.0 / (0.25 * p.n2[1] + reach);
-      C.ball_irb = 1.0 / (0.25 * p.n2[2] + reach);
+      C.ball_ira = 1.0 / (0.25 * p.n2[1] * grow);
+      C.ball_irb = 1.0 / (0.25 * p.n2[2] * grow);
       C.ball_ct = 0.5 * p.n2[0] - p.lo[0];
-      C.ball_rt = 0.25 * p.n2[0] + reach;
+      C.ball_rt = 0.25 * p.n2[0] * grow;
     }
     SFD_TRY(fft_pass(C, ft, 0, bufy, bufx, st));
   }
@@ -685,7 +696,13 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
     B.n_hi = nf0; B.n_lo = no2;
     B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
     B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    // SFD_DEBUG_POISON_BAND=1 (tests): fill each pass's output buffer with NaN first, so that any cell the pruned passes
+    // leave unstored and a later stage reads anyway shows up as a NaN distance (tests/test_gpu_fullsize.py)
+    const char* poison_env = std::getenv("SFD_DEBUG_POISON_BAND");
+    const bool poison = poison_env && poison_env[0] == '1';
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16, st));
     SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufx, 0xff, L.bufy - L.bufx, st));
     FftPass C3{};
     C3.N = p.n2[0]; C3.n_in = p.nf[0]; C3.lo = p.lo[0]; C3.nout = p.nout[0];
     C3.n_hi = 1; C3.n_lo = no1 * no2;

@@ -107,6 +107,7 @@ struct SrcView {
   int64_t nV;
   const double* rule;   // 4 x Q columns (device)
   int Q;
+  int32_t* flags;       // device error word (common.cuh): a bad face index is reported, not only poisoned
 };
 __device__ __forceinline__ void stage_rule(const SrcView& v, double* s_rule) {
   if (v.V) {
@@ -117,7 +118,7 @@ __device__ __forceinline__ void stage_rule(const SrcView& v, double* s_rule) {
 __device__ __forceinline__ void load_source(const SrcView& v, const double* s_rule, int64_t j, double& x0, double& x1,
                                             double& x2, double& w) {
   if (v.V) {
-    atom_eval(v.V, v.nV, v.F, j, v.Q, s_rule, x0, x1, x2, w);
+    atom_eval(v.V, v.nV, v.F, j, v.Q, s_rule, x0, x1, x2, w, v.flags);
   } else {
     x0 = v.x[3 * j];
     x1 = v.x[3 * j + 1];
@@ -337,6 +338,7 @@ static SrcView src_view(const double* d_x, const double* d_w, const MeshAtoms* m
     v.nV = mesh->nV;
     v.rule = d_rule;
     v.Q = mesh->rule;
+    v.flags = device_flags();
   }
   return v;
 }

@@ -6,6 +6,7 @@
 // HBM-bound, 48 B per target, one pass.  The sum is carried as a (sum, compensation) fp64 pair (TwoSum) from the
 // per-thread accumulators through warp shuffles, the block tree and a fixed-order final pass over the per-CTA
 // partials: deterministic for a given K.
+#include <algorithm>
 #include <cmath>
 
 #include "internal.cuh"
@@ -14,7 +15,7 @@ namespace sfd {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kMaxBlocks = 148 * 8;
+constexpr int kMaxBlocks = 2048;   // upper bound of the per-CTA partials (the grid is 8 CTAs per SM of the device)
 
 struct Comp {
   double s, c;
@@ -172,19 +173,25 @@ __global__ void __launch_bounds__(kThreads) lattice_band_terms_kernel(const doub
   if (threadIdx.x == 0) partial[blockIdx.x] = tot;
 }
 
+// result[0] = I; result[1] = the device error word (collected and cleared: common.cuh device_flags); result[2..3] =
+// the (sum, compensation) pair scaled by pref, for consumers that keep adding (the shards of a multi-GPU run).
 __global__ void __launch_bounds__(kThreads) reduce_final_kernel(const Comp* __restrict__ partial, int n, double pref,
-                                                               double* __restrict__ result) {
+                                                               double* __restrict__ result, int32_t* __restrict__ flags) {
   Comp acc{0.0, 0.0};
   for (int i = threadIdx.x; i < n; i += kThreads) comp_merge(acc, partial[i]);
   const Comp tot = block_reduce(acc);
   if (threadIdx.x == 0) {
     result[0] = (tot.s + tot.c) * pref;
+    result[1] = flags ? (double)atomicExch(flags, 0) : 0.0;
+    result[2] = tot.s * pref;
+    result[3] = tot.c * pref;
   }
 }
 
 int reduce_blocks(int64_t K) {
   const int64_t want = (K + kThreads - 1) / kThreads;
-  return (int)(want < 1 ? 1 : (want > kMaxBlocks ? kMaxBlocks : want));
+  const int64_t cap = std::min<int64_t>(kMaxBlocks, (int64_t)num_sms() * 8);
+  return (int)(want < 1 ? 1 : (want > cap ? cap : want));
 }
 
 }  // namespace
@@ -208,7 +215,7 @@ int reduce_any(const double* d_nuhat, const double* d_xi, const double* d_W, int
   Comp* partial = reinterpret_cast<Comp*>(static_cast<char*>(d_work) + 256);
   *d_result = result;
   if (K == 0) {
-    SFD_CUDA_TRY(cudaMemsetAsync(result, 0, sizeof(double), st));
+    SFD_CUDA_TRY(cudaMemsetAsync(result, 0, 4 * sizeof(double), st));
     return SFD_OK;
   }
   const int blocks = reduce_blocks(K);
@@ -220,7 +227,7 @@ int reduce_any(const double* d_nuhat, const double* d_xi, const double* d_W, int
   else
     reduce_terms_kernel<false><<<blocks, kThreads, 0, st>>>(nu, nu2, d_xi, d_W, K, s, s_kind, scale * scale, 0, 0.0, partial);
   SFD_TRY(launch_check("reduce_terms_kernel"));
-  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);
+  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result, device_flags());
   return launch_check("reduce_final_kernel");
 }
 }  // namespace
@@ -256,7 +263,7 @@ int reduce_lattice_band_enqueue(const Nufft1Band& band, int M, double xi_max, do
                                                          band.C[1], band.C[2], M, 2.0 * xi_max / M, s, s_kind,
                                                          scale * scale, partial);
   SFD_TRY(launch_check("lattice_band_terms_kernel"));
-  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result);
+  reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result, device_flags());
   return launch_check("reduce_final_kernel");
 }
 

@@ -2,10 +2,10 @@
 
 The ball quadrature is a sum over radial shells, and every target is independent (each nuhat_k is its own sum
 over the atoms), so a distance evaluation shards over ranks without any data-path exchange: rank r takes the shells
-[a_r, a_{r+1}), runs the whole hot path on them (its own direct sum or its own complete type-3 transform) and the only
-collective is the all-reduce of one fp64 partial sum I_r (8 bytes).  Host logic only -- argument marshalling and the
-shard arithmetic; the per-shard work is the C-ABI calls of binding.py (or, in the CPU tests, callables the test
-supplies).
+[a_r, a_{r+1}), runs the whole hot path on them (sfd_weak_distance_range: its own direct sum or its own complete type-3
+transform, with the half rule) and the only collective is the all-reduce of one compensated fp64 pair (16 bytes) that
+never leaves device memory.  Host logic only -- the shard arithmetic and the collective; the per-shard work is the
+C-ABI call of binding.py.
 """
 import math
 
@@ -41,38 +41,33 @@ def shard_of(n_r, rank, world_size, eps=0.0):
     return b[rank], b[rank + 1]
 
 
-def combine_partial_I(I_part, group=None):
-    """Sum of the ranks' partial I over `group` (all-reduce of one fp64).  Without an initialised process group
-    (single process) the partial sum is the sum."""
-    import torch
+def combine_partial(pair, group=None):
+    """All-reduce (sum) of the ranks' partial sums over `group`, in place, on the device the tensor lives on.
+
+    `pair` is the float64[2] (sum, compensation) tensor that sfd_weak_distance_range leaves in device memory: 16 bytes,
+    added component-wise -- the data path's only exchange (NCCL over NVLink on GPUs; gloo on CPU tensors in the host-logic
+    tests).  Without an initialised process group (single process) the tensor is returned unchanged."""
     import torch.distributed as dist
-    if not (dist.is_available() and dist.is_initialized()):
-        return float(I_part)
-    dev = "cuda" if dist.get_backend(group) == "nccl" else "cpu"
-    t = torch.tensor([float(I_part)], dtype=torch.float64, device=dev)
-    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
-    return float(t[0])
+    if dist.is_available() and dist.is_initialized():
+        dist.all_reduce(pair, op=dist.ReduceOp.SUM, group=group)
+    return pair
 
 
-def weak_distance_sharded(V, F, rule, s, R, q, eps=0.0, rank=None, world_size=None, group=None, backend=None):
-    """sqrt(I) and I of the H^{-s} distance with the targets sharded over the ranks of `group`.
+def weak_distance_sharded(V, F, rule, s, R, q, eps=0.0, rank=None, world_size=None, group=None, work=None, x_extent=None):
+    """sqrt(I) and I of the H^{-s} distance with the frequency nodes sharded over the ranks of `group`.
 
-    backend: object with sfd_nodes, sfd_freq_nodes_device_range, sfd_surface_ft, sfd_reduce (default: this package's
-    binding, i.e. the CUDA path on the rank's current device)."""
+    Every rank runs sfd_weak_distance_range on its shells (the same half rule and fast paths as the single-GPU call, the
+    transform's grids sized by the shard's own largest radius); the 16-byte device pairs are all-reduced; the one host
+    read is the final sum, taken on every rank."""
     import torch.distributed as dist
-    if backend is None:
-        from . import binding as backend
+    from . import binding
     if rank is None:
         rank = dist.get_rank(group) if dist.is_initialized() else 0
     if world_size is None:
         world_size = dist.get_world_size(group) if dist.is_initialized() else 1
     n_r = int(q[0]) if not hasattr(q, "n_r") else q.n_r
     a0, a1 = shard_of(n_r, rank, world_size, eps)
-    I_part = 0.0
-    if a1 > a0:
-        x, w = backend.sfd_nodes(V, F, rule)
-        xi, W = backend.sfd_freq_nodes_device_range(q, R, a0, a1)
-        nu = backend.sfd_surface_ft(x, w, xi, eps)
-        I_part = backend.sfd_reduce(nu, xi, W, s)
-    I = combine_partial_I(I_part, group)
+    pair = binding.sfd_weak_distance_range(V, F, rule, s, R, q, a0, a1, eps, work=work, x_extent=x_extent)
+    pair = combine_partial(pair, group)
+    I = float(pair.sum().item())
     return math.sqrt(I), I

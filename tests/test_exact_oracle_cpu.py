@@ -34,7 +34,8 @@ def area(p):
 
 
 def test_matches_eq_2_19_literally(orc):
-    """Generic directions and magnitudes from 1e-3 to 1e3: both branches of the oracle (series, recursion)."""
+    """Generic directions and magnitudes from 1e-3 to 1e3: the binary128 evaluation of the printed formula, and (at the
+    small magnitudes, where the alpha_i are within 1e-5 of each other) the arbitrary-precision one."""
     rng = np.random.default_rng(0)
     xis = [rng.normal(size=3) * m for m in (1e-3, 0.05, 0.7, 1.0, 3.0, 40.0, 1e3) for _ in range(6)]
     got = orc.exact_ft(TRI, F1, np.array(xis))

@@ -195,6 +195,97 @@ def test_weak_distance_jittered_mesh(sfd, orc, torch):
         assert abs(I - I_ref) <= 1e-8 * I_ref
 
 
+def _r13_bound(orc, Vn, Fn, rule, q, R, s, eps):
+    """DESIGN.md R13: |dI| <= 2 sqrt(I E2) + E2, E2 = (2 pi)^-3 sum_k W_k (10 eps sum|w|)^2 (1+r^2)^-s."""
+    x, w = orc.nodes(Vn, Fn, rule)
+    xi, W = orc.freq_nodes(*q, R)
+    r2 = (xi * xi).sum(1)
+    return float((W * (1 + r2) ** (-s)).sum()) * (10 * eps * np.abs(w).sum()) ** 2 / (2 * np.pi) ** 3
+
+
+@pytest.mark.parametrize("q", [(20, 10, 12), (14, 9, 16)])          # even and odd n_theta (a ring at cos(theta) = 0)
+@pytest.mark.parametrize("eps", [1e-6, 1e-10])
+def test_weak_distance_fast_path_offcentre_mesh(sfd, orc, torch, q, eps):
+    """The combination only sfd_weak_distance uses -- half rule, origin-centred target box, hull hint, Hermitian half
+    band, ball prune -- on meshes that are NOT centrally symmetric (C != 0, Im nuhat != 0): a jittered, translated and
+    anisotropically scaled level-2 icosphere, against the oracle's distance (not the library's own stages)."""
+    Vo, Fo = orc.mesh_icosphere(2)
+    Vj = workloads.jitter_vertices(Vo, Fo, 0.1, 5) * np.array([1.0, 0.7, 1.3]) + np.array([0.3, -0.2, 0.15])
+    Vj = np.ascontiguousarray(Vj)
+    R, s = 14.0, 2.0
+    d_ref, I_ref = orc.weak_distance(Vj, Fo, 6, s, R, *q)
+    d, I = sfd.sfd_weak_distance(dev(torch, Vj), dev(torch, Fo), 6, s, R, q, eps)
+    E2 = _r13_bound(orc, Vj, Fo, 6, q, R, s, eps)
+    assert abs(I - I_ref) <= 2 * np.sqrt(I_ref * E2) + E2, (I, I_ref, E2)
+    d0, I0 = sfd.sfd_weak_distance(dev(torch, Vj), dev(torch, Fo), 6, s, R, q, 0.0)
+    assert abs(I0 - I_ref) <= 1e-8 * I_ref
+
+
+@pytest.mark.parametrize("aspect", [(16.0, 1.0, 1.0), (1.0, 1.0, 24.0), (0.05, 1.0, 0.3)])
+def test_weak_distance_stretched_mesh(sfd, orc, torch, aspect):
+    """Elongated meshes: the inner grid is n2_0 x n2_1 x n2_2 with very different axes, and the ball the rule's nodes fill
+    becomes an ellipsoid in grid cells.  The pruned band must still hold every cell a footprint touches (the region kept
+    is the ellipsoid scaled by 1 + reach / a_min, a superset of its Minkowski sum with the footprint)."""
+    Vo, Fo = orc.mesh_icosphere(2)
+    Vs = np.ascontiguousarray(Vo * np.array(aspect))
+    q, R, s, eps = (16, 10, 12), 6.0, 2.0, 1e-6
+    d_ref, I_ref = orc.weak_distance(Vs, Fo, 6, s, R, *q)
+    d, I = sfd.sfd_weak_distance(dev(torch, Vs), dev(torch, Fo), 6, s, R, q, eps)
+    E2 = _r13_bound(orc, Vs, Fo, 6, q, R, s, eps)
+    assert np.isfinite(I) and abs(I - I_ref) <= 2 * np.sqrt(I_ref * E2) + E2, (I, I_ref, E2)
+
+
+def test_extents(sfd, torch):
+    """sfd_extents: the library's own bounds kernels behind the workspace queries (no torch reduction on the data)."""
+    x, w, xi = workloads.random_cloud(5000, 10)
+    half, centre = sfd.sfd_extents(dev(torch, x))
+    lo, hi = x.min(0), x.max(0)
+    assert np.allclose(half, 0.5 * (hi - lo), rtol=1e-11, atol=0) and np.all(np.asarray(half) >= 0.5 * (hi - lo))
+    assert np.allclose(centre, 0.5 * (hi + lo), rtol=1e-15, atol=1e-15)
+    assert sfd.sfd_extents(dev(torch, np.zeros((0, 3)))) == ([0.0] * 3, [0.0] * 3)
+    one = sfd.sfd_extents(dev(torch, np.array([[1.0, -2.0, 3.0]])))
+    assert one[1] == [1.0, -2.0, 3.0] and max(one[0]) < 1e-290
+    with pytest.raises(sfd.SfdError) as e:
+        sfd.sfd_extents(dev(torch, np.array([[1.0, np.nan, 0.0]])))
+    assert e.value.status == -2
+
+
+def test_bad_face_index_is_reported(sfd, orc, torch):
+    """a face index >= nV is "checked on device, reported at the next synchronising call" as
+    SFD_ERR_INVALID_ARG.  sfd_nodes only enqueues (the atoms of the bad face are NaN); the next synchronising call on
+    the device reports and clears the error; calls that take the mesh and synchronise report their own."""
+    Vo, Fo = orc.mesh_icosphere(1)
+    bad = Fo.copy()
+    bad[17, 1] = len(Vo) + 3
+    neg = Fo.copy()
+    neg[3, 0] = -1
+    V = dev(torch, Vo)
+    xi, W = sfd.sfd_freq_nodes_device((6, 4, 6), 4.0)
+    for Fb in (bad, neg):
+        x, w = sfd.sfd_nodes(V, dev(torch, Fb), 6)          # enqueues; no error yet
+        assert bool(torch.isnan(w).any())
+        nu = sfd.sfd_surface_ft(x, w, xi, 0.0)
+        with pytest.raises(sfd.SfdError) as e:
+            sfd.sfd_reduce(nu, xi, W, 2.0)
+        assert e.value.status == -2 and "face index" in str(e.value)
+        # reported once, then cleared: a good mesh afterwards is fine
+        xg, wg = sfd.sfd_nodes(V, dev(torch, Fo), 6)
+        assert sfd.sfd_reduce(sfd.sfd_surface_ft(xg, wg, xi, 0.0), xi, W, 2.0) > 0
+        for eps in (0.0, 1e-8):
+            with pytest.raises(sfd.SfdError) as e:
+                sfd.sfd_weak_distance(V, dev(torch, Fb), 6, 2.0, 4.0, (6, 4, 6), eps)
+            assert e.value.status == -2
+            assert sfd.sfd_weak_distance(V, dev(torch, Fo), 6, 2.0, 4.0, (6, 4, 6), eps)[0] > 0
+        with pytest.raises(sfd.SfdError):
+            sfd.sfd_mesh_distance(V, dev(torch, Fo), V, dev(torch, Fb), 6, 2.0, 4.0, (6, 4, 6), 0.0)
+        x, w = sfd.sfd_nodes(V, dev(torch, Fb), 6)
+        with pytest.raises(sfd.SfdError):
+            sfd.sfd_extents(x)                              # NaN atoms + the error word
+        assert sfd.sfd_extents(xg)[0][0] > 0
+        pair = sfd.sfd_weak_distance_range(V, dev(torch, Fb), 6, 2.0, 4.0, (6, 4, 6), 0, 6, 0.0)
+        assert bool(torch.isnan(pair[0]))                   # nothing synchronises: the shard's partial sum is poisoned
+
+
 def test_surface_ft_host_entry(sfd, orc):
     x, w, xi = workloads.random_cloud(300, 500)
     nu = sfd.sfd_surface_ft_host(x, w, xi, 0.0)
@@ -276,26 +367,54 @@ def test_nufft_single_source_worst_case(sfd, orc, torch):
 
 
 # ---- multi-GPU path on one GPU: the ranks' shards evaluated one after the other ----------------------
-@pytest.mark.parametrize("eps,world", [(0.0, 3), (1e-9, 4)])
-def test_target_shards_add_up(sfd, orc, torch, eps, world):
-    """The partial sums of disjoint radial shards (what each rank of sharding.weak_distance_sharded computes) add up
-    to the unsharded I; the shard nodes are the full rule's nodes."""
+@pytest.mark.parametrize("eps,world,q", [(0.0, 3, None), (1e-9, 4, None), (1e-9, 2, (9, 7, 8)), (0.0, 2, (5, 4, 3))])
+def test_target_shards_add_up(sfd, orc, torch, eps, world, q):
+    """The partial sums of disjoint radial shards (what each rank of sharding.weak_distance_sharded computes with
+    sfd_weak_distance_range: half rule, shard-sized grids) add up to the unsharded I; every shard's partial sum equals
+    the oracle's sum over the shard's nodes; the shard nodes are the full rule's nodes.  Odd n_theta (a ring at
+    cos(theta) = 0) and odd n_phi (no half rule) included."""
     from paper_2304_06340_b200 import sharding
     c = workloads.CONFIGS[1]
-    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    q = q or (c["n_r"], c["n_theta"], c["n_phi"])
     V, F = sfd.sfd_mesh_icosphere(c["level"])
     d_full, I_full = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, eps)
     xi_full, W_full = sfd.sfd_freq_nodes_device(q, c["R"])
+    Vo, Fo = orc.mesh_icosphere(c["level"])
+    xo, wo = orc.nodes(Vo, Fo, c["rule"])
+    xio, Wo = orc.freq_nodes(*q, c["R"])
     n = q[1] * q[2]
     I_sum = 0.0
+    tol = 1e-11 if eps == 0.0 else 1e-7   # every shard's type-3 transform has its own grids (errors <= 10 eps sum|w|)
     for rank in range(world):
         a0, a1 = sharding.shard_of(q[0], rank, world, eps)
         xi, W = sfd.sfd_freq_nodes_device_range(q, c["R"], a0, a1)
         assert torch.equal(xi, xi_full[a0 * n:a1 * n]) and torch.equal(W, W_full[a0 * n:a1 * n])
+        pair = sfd.sfd_weak_distance_range(V, F, c["rule"], 2.0, c["R"], q, a0, a1, eps)
+        assert pair.is_cuda and pair.shape == (2,)
+        I_r = float(pair.sum())
+        sl = slice(a0 * n, a1 * n)
+        I_o = orc.reduce(orc.direct_sum(xo, wo, xio[sl]), np.ascontiguousarray(xio[sl]), np.ascontiguousarray(Wo[sl]), 2.0) \
+            if a1 > a0 else 0.0
+        assert abs(I_r - I_o) <= tol * I_full, (rank, I_r, I_o)
         d, I = sharding.weak_distance_sharded(V, F, c["rule"], 2.0, c["R"], q, eps, rank=rank, world_size=world)
-        I_sum += I          # no process group: each call returns its own partial sum
-    tol = 1e-12 if eps == 0.0 else 1e-7   # every shard's type-3 transform has its own grids (errors <= 10 eps sum|w|)
+        assert I == I_r or abs(I - I_r) <= 1e-9 * I_full    # no process group: each call returns its own partial sum
+        I_sum += I_r
     assert abs(I_sum - I_full) <= tol * I_full
+
+
+def test_weak_distance_range_edges(sfd, torch):
+    """Empty range -> (0, 0); bad ranges rejected; the whole range equals sfd_weak_distance."""
+    V, F = sfd.sfd_mesh_icosphere(1)
+    q = (8, 6, 8)
+    pair = sfd.sfd_weak_distance_range(V, F, 6, 2.0, 8.0, q, 3, 3, 0.0)
+    assert pair.tolist() == [0.0, 0.0]
+    for a0, a1 in ((-1, 2), (5, 4), (0, 9)):
+        with pytest.raises(sfd.SfdError):
+            sfd.sfd_weak_distance_range(V, F, 6, 2.0, 8.0, q, a0, a1, 0.0)
+    for eps in (0.0, 1e-8):
+        d, I = sfd.sfd_weak_distance(V, F, 6, 2.0, 8.0, q, eps)
+        pair = sfd.sfd_weak_distance_range(V, F, 6, 2.0, 8.0, q, 0, 8, eps)
+        assert abs(float(pair.sum()) - I) <= 1e-14 * I
 
 
 @pytest.mark.parametrize("eps", [1e-1, 1e-2, 1e-4, 1e-5, 1e-7, 1e-8, 1e-10, 1e-11, 1e-13, 1e-14])

@@ -1,5 +1,5 @@
 """Host logic of the multi-GPU path (paper_2304_06340_b200/sharding.py) on the CPU: shard arithmetic, and the
-world_size-2 all-reduce over gloo with the oracle standing in for the per-shard device work (-m "not gpu")."""
+world_size-2 all-reduce over gloo of per-shard partial sums the test computes with the oracle (-m "not gpu")."""
 import os
 import sys
 
@@ -34,60 +34,68 @@ def test_radial_shards_partition(n_r, world, eps):
         assert sizes[0] >= sizes[-1]      # outer shards own larger grids, so they get fewer shells
 
 
-class _OracleBackend:
-    """The calls sharding.weak_distance_sharded makes, answered by the CPU oracle (numpy arrays)."""
+def _oracle():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import sfd_oracle
+    return sfd_oracle
 
-    def __init__(self):
-        sys.path.insert(0, os.path.join(ROOT, "oracle"))
-        import sfd_oracle
-        self.O = sfd_oracle
 
-    def sfd_nodes(self, V, F, rule):
-        return self.O.nodes(V, F, rule)
-
-    def sfd_freq_nodes_device_range(self, q, R, a0, a1):
-        xi, W = self.O.freq_nodes(q[0], q[1], q[2], R)
-        n = q[1] * q[2]
-        return xi[a0 * n:a1 * n], W[a0 * n:a1 * n]
-
-    def sfd_surface_ft(self, x, w, xi, eps):
-        return self.O.direct_sum(x, w, xi)
-
-    def sfd_reduce(self, nu, xi, W, s):
-        return self.O.reduce(nu, xi, W, s)
+def _shard_partial(O, V, F, rule, s, R, q, a0, a1):
+    """The partial sum I_r of the shells [a0, a1), by the oracle (test code: the product's per-shard work is the CUDA call
+    sfd_weak_distance_range, compared with exactly this on the GPU in tests/test_gpu_parity.py)."""
+    x, w = O.nodes(V, F, rule)
+    xi, W = O.freq_nodes(q[0], q[1], q[2], R)
+    n = q[1] * q[2]
+    xi, W = np.ascontiguousarray(xi[a0 * n:a1 * n]), np.ascontiguousarray(W[a0 * n:a1 * n])
+    if a1 == a0:
+        return 0.0
+    return O.reduce(O.direct_sum(x, w, xi), xi, W, s)
 
 
 def _worker(rank, world, port, out):
+    import torch
     import torch.distributed as dist
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         S = _sharding()
-        B = _OracleBackend()
-        V, F = B.O.mesh_icosphere(1)
+        O = _oracle()
+        V, F = O.mesh_icosphere(1)
         q = (12, 6, 8)
         res = {}
-        for eps in (0.0, 1e-9):   # both shard policies (the oracle backend ignores eps beyond that)
-            d, I = S.weak_distance_sharded(V, F, 6, 2.0, 8.0, q, eps, backend=B)
-            res[eps] = (d, I, S.shard_of(q[0], rank, world, eps))
+        for eps in (0.0, 1e-9):   # both shard policies
+            a0, a1 = S.shard_of(q[0], rank, world, eps)
+            # what sfd_weak_distance_range leaves on a GPU: a (sum, compensation) pair; here a CPU tensor over gloo
+            pair = torch.tensor([_shard_partial(O, V, F, 6, 2.0, 8.0, q, a0, a1), 0.0], dtype=torch.float64)
+            pair = S.combine_partial(pair)
+            res[eps] = (float(pair.sum()), (a0, a1))
         out[rank] = res
     finally:
         dist.destroy_process_group()
 
 
-def test_weak_distance_sharded_gloo_world2():
+def test_combine_partial_gloo_world2():
+    """Shard arithmetic + the 16-byte all-reduce over gloo, world size 2: the shards tile the shells, every rank ends up
+    with the same sum, and the sum is the unsharded I."""
     import torch.multiprocessing as mp
-    B = _OracleBackend()
-    V, F = B.O.mesh_icosphere(1)
-    d_ref, I_ref = B.O.weak_distance(V, F, 6, 2.0, 8.0, 12, 6, 8)
+    O = _oracle()
+    V, F = O.mesh_icosphere(1)
+    d_ref, I_ref = O.weak_distance(V, F, 6, 2.0, 8.0, 12, 6, 8)
     mgr = mp.Manager()
     out = mgr.dict()
     port = 29500 + os.getpid() % 2000
     mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
     assert set(out.keys()) == {0, 1}
     for eps in (0.0, 1e-9):
-        (d0, I0, s0), (d1, I1, s1) = out[0][eps], out[1][eps]
-        assert I0 == I1 and d0 == d1                    # every rank holds the reduced value
+        (I0, s0), (I1, s1) = out[0][eps], out[1][eps]
+        assert I0 == I1                                  # every rank holds the reduced value
         assert s0[0] == 0 and s0[1] == s1[0] and s1[1] == 12 and s0[1] > 0   # the two shards tile the shells
-        assert abs(I0 - I_ref) <= 1e-13 * I_ref and abs(d0 - d_ref) <= 1e-13 * d_ref
+        assert abs(I0 - I_ref) <= 1e-13 * I_ref
+
+
+def test_combine_partial_without_group():
+    import torch
+    S = _sharding()
+    t = torch.tensor([1.5, 2.0 ** -60], dtype=torch.float64)
+    assert S.combine_partial(t) is t and float(t[0]) == 1.5
