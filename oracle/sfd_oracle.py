@@ -121,7 +121,8 @@ def _exact_pair_mp(p, xi):
     cancellation errors"): the printed formula -2A sum_i e^{-i alpha_i} / prod_{j != i}(alpha_i - alpha_j) with as many
     digits as its cancellation needs, or, where two or three alpha coincide EXACTLY and the printed formula is 0/0, its
     limit: 2A times the divided difference exp[z_0, z_1, z_2], z = -i alpha, with repeated nodes (textbook definitions:
-    f[z, z, w] = (f[z, w] - f'(z)) / (w - z), f[z, w] = (f(w) - f(z)) / (w - z), f[z, z, z] = f''(z) / 2)."""
+    f[z, z, w] = (f[z, w] - f'(z)) / (w - z), f[z, w] = (f(w) - f(z)) / (w - z), f[z, z, z] = f''(z) / 2).  Returns an mpmath
+    complex (the caller sums a frequency's pairs before rounding)."""
     import mpmath as mp
     mp.mp.dps = 400                      # the dot products of fp64 inputs are exact at this precision
     P = [[mp.mpf(float(c)) for c in v] for v in p]
@@ -133,13 +134,13 @@ def _exact_pair_mp(p, xi):
     al = [sum(X[c] * P[i][c] for c in range(3)) for i in range(3)]
     same = [(i, j) for i in range(3) for j in range(i + 1, 3) if al[i] == al[j]]
     if len(same) == 3:                   # all three coincide (xi along the normal, xi = 0): exp''(z) / 2
-        return complex(A2 * mp.exp(-1j * al[0]) / 2)
+        return A2 * mp.exp(-1j * al[0]) / 2
     if len(same) == 1:                   # exactly two coincide (xi orthogonal to an edge): f[z, z, w]
         i, j = same[0]
         k = 3 - i - j
         z, w = -1j * al[i], -1j * al[k]
         first = (mp.exp(w) - mp.exp(z)) / (w - z)
-        return complex(A2 * (first - mp.exp(z)) / (w - z))
+        return A2 * (first - mp.exp(z)) / (w - z)
     dmin = min(abs(al[i] - al[j]) for i in range(3) for j in range(i + 1, 3))
     amax = max(1, max(abs(a) for a in al))
     mp.mp.dps = 60 + 3 * int(mp.ceil(mp.log10(amax / dmin)))     # 1/d^2 of cancellation, 1/d in each difference
@@ -150,7 +151,7 @@ def _exact_pair_mp(p, xi):
             if j != i:
                 den *= al[i] - al[j]
         tot += mp.exp(-1j * al[i]) / den
-    return complex(-A2 * tot)
+    return -A2 * tot
 
 
 def exact_ft(V, F, xi):
@@ -171,8 +172,11 @@ def exact_ft(V, F, xi):
         cap = int(n.value)
     _chk(rc, "exact_ft")
     res = out.view(np.complex128).reshape(-1)
+    extra = {}                           # the skipped pairs of a frequency are summed at full precision, rounded once
     for k, f in skipped[:n.value]:
-        res[k] += _exact_pair_mp(V[F[f]], xi[k])
+        extra[int(k)] = extra.get(int(k), 0) + _exact_pair_mp(V[F[f]], xi[k])
+    for k, v in extra.items():
+        res[k] += complex(v)
     return res
 
 

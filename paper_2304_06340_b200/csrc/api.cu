@@ -388,7 +388,14 @@ int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double reach
   L->K = visited_nodes(q, a0, a1);
   const double X[3] = {x_extent, x_extent, x_extent}, S[3] = {reach, reach, reach};
   if (eps > 0.0) SFD_REQUIRE(x_extent > 0.0 && std::isfinite(x_extent), SFD_ERR_INVALID_ARG, "x_extent must be > 0");
-  SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, eps, &L->ft_bytes));
+  // the distance calls centre the targets' box at the origin: the strengths stay real (half the transform's grids)
+  if (eps == 0.0 || L->J == 0 || L->K == 0) {
+    SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, 0.0, &L->ft_bytes));
+  } else {
+    Nufft3Sizes sz;
+    SFD_TRY(nufft3_sizes(L->J, L->K, X, S, eps, &sz, true));
+    L->ft_bytes = sz.work_bytes;
+  }
   L->tab_bytes = freq_tables_bytes(q);
   L->red_bytes = reduce_workspace(L->K);
   size_t o = 0;

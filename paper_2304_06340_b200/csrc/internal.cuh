@@ -66,7 +66,9 @@ struct Nufft3Sizes {
   int64_t nout[3];     // kept part of the inner grid per axis (pruned FFT output)
   size_t work_bytes;   // total workspace
 };
-int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out);
+// real_only: size for real strengths only (targets known to be centred at the origin: about half the grids)
+int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out,
+                 bool real_only = false);
 // What a caller may know about the extents, which replaces the reductions over all sources / all targets:
 //   d_hull / n_hull: device points whose bounding box contains every source (the vertices of the mesh the atoms are
 //     convex combinations of);  target_reach > 0: every target lies in [-target_reach, target_reach]^3 (target_ball: in

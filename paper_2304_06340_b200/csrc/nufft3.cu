@@ -308,7 +308,7 @@ int items_and_spread(const N3Params& p, int64_t J, int64_t ns_bins, int64_t ns_k
 
 int nufft3_release_cache() { return SFD_OK; }   // nothing is cached on the device any more
 
-int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out) {
+int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], double eps, Nufft3Sizes* out, bool real_only) {
   SFD_REQUIRE(X && S && out, SFD_ERR_NULL, "nufft3_sizes: NULL argument");
   // the call recomputes the extents from the data; the query leaves room for their rounding
   double Xi[3], Si[3];
@@ -318,7 +318,9 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
   }
   size_t total = 0;
   N3Params p{};
-  for (int real_c = 0; real_c < 2; ++real_c) {   // whether the strengths stay real is only known from the data
+  // whether the strengths stay real is only known from the data, unless the caller knows the targets to be centred at
+  // the origin (the distance calls: real_only)
+  for (int real_c = real_only ? 1 : 0; real_c < 2; ++real_c) {
     // (the call decides on the wider kernel from the data's own extents: near the threshold size for both)
     bool near = false;
     for (int d = 0; d < 3; ++d) near = near || (X[d] * S[d] < 1.01 && X[d] * S[d] > 0.98);
