@@ -16,6 +16,7 @@
 // A is conflict-free too) -- and the band is written out through the digit-reversal table.  HBM traffic per pass is
 // one read of the input rows and one write of the band: ~16x less than padded library transforms at config 3.
 #include <algorithm>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <vector>
@@ -197,6 +198,310 @@ __device__ __forceinline__ double ball_q(const FftPass& P, int64_t lo) {
   const double da = ((double)ia - P.ball_ca) * P.ball_ira;
   const double db = ((double)(lo - ia * (P.ball == 1 ? P.ball_nb : 0)) - P.ball_cb) * P.ball_irb;
   return da * da + db * db;
+}
+
+// =====================================================================================================================
+// Fixed-geometry pruned passes.  For the transform lengths the type-3 planner emits on BASELINE.json's configurations
+// (n2 = 360, 672, 720, 1344, 1440, 2700) with exactly the central half of the inputs non-zero (n_in = N/2: sigma = 2), the
+// pass is compiled for the length: N = G1 G2 G3 with three register-resident groups G = A B <= 16 (radix A then radix B
+// fused, as in fused_stages), every stride, twiddle step and loop bound a compile-time constant.  Against the generic
+// kernel above this removes the zero-padding and the separate load phase (group 1 reads its inputs straight from global
+// memory -- with A1 = 4 the elements q1 = 1, 2 of every radix-4 butterfly lie in the zero half, so only q1 = 0, 3 are
+// loaded and the butterfly costs 4 complex additions), the separate store phase of the strided passes (group 3 writes the
+// band straight from registers: in those passes every output element is its own 16 TB-byte segment whatever the order),
+// the trivial twiddles of the last stage, and the run-time index arithmetic (~58 of 124 instructions per point in the
+// generic kernel, profiles/r1j_fft_phases.md).  Shared-memory round trips per point: 2 (4 accesses) instead of 4-5.
+template <int N_, int A1_, int B1_, int A2_, int B2_, int A3_, int B3_, int TB_, int T_, int CTAS_>
+struct FixedPlan {
+  static constexpr int N = N_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_, A3 = A3_, B3 = B3_, TB = TB_, T = T_, CTAS = CTAS_;
+  static constexpr int G1 = A1 * B1, G2 = A2 * B2, G3 = A3 * B3;
+  static_assert(G1 * G2 * G3 == N && A1 == 4 && N % 4 == 0, "plan must factor N with a leading radix 4");
+  static_assert((TB & (TB - 1)) == 0, "tile height must be a power of two");
+};
+
+// One fused group in registers: radix A over q1, twiddle, radix B over q2, twiddle.  v[q1][q2] -> v[p1][p2].
+// The twiddles come from per-stage tables laid out [row][jp] (FixedTw below), so that the lanes of a warp -- consecutive
+// jp -- read consecutive 16-byte entries: ta[((p1-1) B + q2) stride] = w^{p1 (jp + q2 Lq) tstep}, tb[(p2-1) stride] =
+// w^{p2 jp tstep A}; both pointers already point at column jp.  (Indexing the one table exp(-2 pi i k / N) by the products
+// made every lane of a load touch its own cache line: the L1 was the busiest unit of the pass, profiles/r2b_fft.md.)
+// LAST: the last group (jp = 0) has only the inner constants w_G^{p1 q2}, q2 >= 1: ta[(p1-1)(B-1) + (q2-1)].
+template <int A, int B, bool LAST>
+__device__ __forceinline__ void group_dft(double2 (&v)[A][B], const double2* __restrict__ ta, const double2* __restrict__ tb,
+                                          int stride) {
+#pragma unroll
+  for (int q2 = 0; q2 < B; ++q2) {
+    double2 x[A];
+#pragma unroll
+    for (int q1 = 0; q1 < A; ++q1) x[q1] = v[q1][q2];
+    bfly<A>(x);
+    v[0][q2] = x[0];
+#pragma unroll
+    for (int p1 = 1; p1 < A; ++p1) {
+      if (LAST)
+        v[p1][q2] = (B == 1 || q2 == 0) ? x[p1] : cmul(x[p1], __ldg(&ta[(p1 - 1) * (B - 1) + (q2 - 1)]));
+      else
+        v[p1][q2] = cmul(x[p1], __ldg(&ta[((p1 - 1) * B + q2) * stride]));
+    }
+  }
+  if (B > 1) {
+#pragma unroll
+    for (int p1 = 0; p1 < A; ++p1) {
+      double2 x[B];
+#pragma unroll
+      for (int q2 = 0; q2 < B; ++q2) x[q2] = v[p1][q2];
+      bfly<B>(x);
+      v[p1][0] = x[0];
+#pragma unroll
+      for (int p2 = 1; p2 < B; ++p2) v[p1][p2] = LAST ? x[p2] : cmul(x[p2], __ldg(&tb[(p2 - 1) * stride]));
+    }
+  }
+}
+
+// Layout of the per-stage twiddle tables of a fixed plan (complex128 entries, one array per axis).
+template <class PL>
+struct FixedTw {
+  static constexpr int Lq1 = PL::N / PL::G1, Lq2 = PL::G3;
+  static constexpr int off1a = 0;                                         // [3 B1][Lq1]: w^{p1 (jp + q2 Lq1)}
+  static constexpr int off1b = off1a + 3 * PL::B1 * Lq1;                   // [B1-1][Lq1]: w^{4 p2 jp}
+  static constexpr int off2a = off1b + (PL::B1 - 1) * Lq1;                 // [(A2-1) B2][Lq2]: w^{p1 (jp + q2 Lq2) G1}
+  static constexpr int off2b = off2a + (PL::A2 - 1) * PL::B2 * Lq2;        // [B2-1][Lq2]: w^{p2 jp G1 A2}
+  static constexpr int off3 = off2b + (PL::B2 - 1) * Lq2;                  // [(A3-1)(B3-1)]: w^{p1 q2 N / G3}
+  static constexpr int total = off3 + (PL::A3 - 1) * (PL::B3 - 1);
+};
+
+// MODE 0: contiguous axis, real input, two rows packed per column (pass A, real strengths); 1: contiguous axis, complex
+// input (pass A, complex strengths); 2: strided complex (passes B, C).  Shared memory: N * TB complex128, element
+// (pos, col) at pos * TB + col in the strided passes (lanes run over the tile's columns first, like the global accesses)
+// and at col * N + pos in the contiguous ones (lanes run along the axis).
+template <class PL, int MODE>
+__global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(FftPass P, const void* __restrict__ in_raw,
+                                                                    double2* __restrict__ out) {
+  constexpr int N = PL::N, TB = PL::TB, T = PL::T;
+  constexpr int A1 = PL::A1, B1 = PL::B1, A2 = PL::A2, B2 = PL::B2, A3 = PL::A3, B3 = PL::B3;
+  constexpr int G1 = PL::G1, G2 = PL::G2, G3 = PL::G3;
+  constexpr bool STRIDED = MODE == 2;
+  constexpr int PACK = MODE == 0 ? 2 : 1;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double2* a = reinterpret_cast<double2*>(smem_raw);
+  __shared__ int s_mm[2 * TB];   // strided passes: the range of outputs [mm0, mm1) every column of the tile has to store
+  const int tid = threadIdx.x;
+  using FT = FixedTw<PL>;
+  const double2* __restrict__ ftw = P.ftw;
+  auto at = [](int pos, int col) { return STRIDED ? pos * TB + col : col * N + pos; };
+
+  constexpr int64_t rows_per_tile = (int64_t)TB * PACK;
+  const int64_t tiles_per_hi = (P.n_lo + rows_per_tile - 1) / rows_per_tile;
+  const int64_t hi = blockIdx.x / tiles_per_hi;
+  const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * rows_per_tile;
+  const int nrow = (int)min(rows_per_tile, P.n_lo - lo0);
+  const int ncol = (nrow + PACK - 1) / PACK;
+  if (STRIDED) {
+    if (P.ball) {   // uniform in the block
+      bool needed = false;
+      for (int c = 0; c < ncol; ++c) needed = needed || ball_q(P, lo0 + c) <= 1.0;
+      if (!needed) return;
+    }
+    if (tid < TB) {
+      int mm0 = 0, mm1 = tid < ncol ? P.nout : 0;
+      if (P.ball && tid < ncol) {
+        const double q = ball_q(P, lo0 + tid);
+        if (q > 1.0) {
+          mm1 = 0;
+        } else {
+          const double rad = P.ball_rt * sqrt(1.0 - q) + 1.0;
+          mm0 = max(0, (int)floor(P.ball_ct - rad));
+          mm1 = min(P.nout, (int)ceil(P.ball_ct + rad) + 1);
+        }
+      }
+      s_mm[2 * tid] = mm0;
+      s_mm[2 * tid + 1] = mm1;
+    }
+  }
+
+  // ---- group 1: inputs from global memory.  Input i <-> mode l = i - N/4 <-> position l mod N: positions [0, N/4) hold
+  // i = pos + N/4, positions [3N/4, N) hold i = pos - 3N/4, the rest is zero: of the radix-4 butterfly (elements r + q1 N/4,
+  // r < N/4) only q1 = 0 (hi = in[r + N/4]) and q1 = 3 (lo = in[r]) exist:  X_p = hi + i^p lo.
+  constexpr int Lq1 = N / G1;
+  bool nz = STRIDED;
+  const double fhi = (MODE != 2 && P.dec_hi) ? P.dec_hi[hi] : 1.0;
+  for (int idx = tid; idx < Lq1 * TB; idx += T) {
+    const int col = STRIDED ? idx % TB : idx / Lq1;
+    const int jp = STRIDED ? idx / TB : idx % Lq1;
+    double2 xl[B1], xh[B1];
+    if (MODE == 2) {
+      const bool live = col < ncol;
+      const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0);
+#pragma unroll
+      for (int q2 = 0; q2 < B1; ++q2) {
+        const int r = jp + q2 * Lq1;
+        xl[q2] = live ? __ldcs(src + (int64_t)r * P.in_el) : make_double2(0.0, 0.0);
+        xh[q2] = live ? __ldcs(src + (int64_t)(r + N / 4) * P.in_el) : make_double2(0.0, 0.0);
+      }
+    } else if (MODE == 1) {
+      const bool live = col < ncol;
+      const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + (live ? col : 0)) * P.in_lo;
+      const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + (live ? col : 0)] : 1.0;
+#pragma unroll
+      for (int q2 = 0; q2 < B1; ++q2) {
+        const int r = jp + q2 * Lq1;
+        const double fl = P.dec_axis ? f0 * P.dec_axis[r] : 1.0, fh = P.dec_axis ? f0 * P.dec_axis[r + N / 4] : 1.0;
+        const double2 l = live ? __ldcs(src + r) : make_double2(0.0, 0.0);
+        const double2 h = live ? __ldcs(src + r + N / 4) : make_double2(0.0, 0.0);
+        xl[q2] = make_double2(l.x * fl, l.y * fl);
+        xh[q2] = make_double2(h.x * fh, h.y * fh);
+        nz |= (l.x != 0.0) | (l.y != 0.0) | (h.x != 0.0) | (h.y != 0.0);
+      }
+    } else {
+      const bool live = col < ncol, two = 2 * col + 1 < nrow;
+      const int64_t r0 = lo0 + 2 * (live ? col : 0);
+      const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
+      const double* src1 = src0 + (two ? P.in_lo : 0);
+      const double f0 = live ? (P.dec_axis ? fhi * P.dec_lo[r0] : 1.0) : 0.0;
+      const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
+      double la[B1], lb[B1], ha[B1], hb[B1], fl[B1], fh[B1];
+#pragma unroll
+      for (int q2 = 0; q2 < B1; ++q2) {
+        const int r = jp + q2 * Lq1;
+        la[q2] = __ldcs(src0 + r);
+        lb[q2] = __ldcs(src1 + r);
+        ha[q2] = __ldcs(src0 + r + N / 4);
+        hb[q2] = __ldcs(src1 + r + N / 4);
+        fl[q2] = P.dec_axis ? P.dec_axis[r] : 1.0;
+        fh[q2] = P.dec_axis ? P.dec_axis[r + N / 4] : 1.0;
+      }
+#pragma unroll
+      for (int q2 = 0; q2 < B1; ++q2) {
+        nz |= live & ((la[q2] != 0.0) | (lb[q2] != 0.0) | (ha[q2] != 0.0) | (hb[q2] != 0.0));
+        xl[q2] = make_double2(la[q2] * (fl[q2] * f0), lb[q2] * (fl[q2] * f1));
+        xh[q2] = make_double2(ha[q2] * (fh[q2] * f0), hb[q2] * (fh[q2] * f1));
+      }
+    }
+    double2 v[A1][B1];
+#pragma unroll
+    for (int q2 = 0; q2 < B1; ++q2) {
+      const int r = jp + q2 * Lq1;
+      const double2 h = xh[q2], l = xl[q2];
+      (void)r;
+      const double2* t1 = ftw + FT::off1a + q2 * Lq1 + jp;
+      v[0][q2] = cadd(h, l);
+      v[1][q2] = cmul(make_double2(h.x - l.y, h.y + l.x), __ldg(t1));                     // (h + i l) w^r
+      v[2][q2] = cmul(csub(h, l), __ldg(t1 + B1 * Lq1));                                  // (h - l) w^2r
+      v[3][q2] = cmul(make_double2(h.x + l.y, h.y - l.x), __ldg(t1 + 2 * B1 * Lq1));      // (h - i l) w^3r
+    }
+    if (B1 > 1) {
+#pragma unroll
+      for (int p1 = 0; p1 < A1; ++p1) {
+        double2 x[B1];
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) x[q2] = v[p1][q2];
+        bfly<B1>(x);
+        v[p1][0] = x[0];
+#pragma unroll
+        for (int p2 = 1; p2 < B1; ++p2) v[p1][p2] = cmul(x[p2], __ldg(ftw + FT::off1b + (p2 - 1) * Lq1 + jp));
+      }
+    }
+#pragma unroll
+    for (int p1 = 0; p1 < A1; ++p1)
+#pragma unroll
+      for (int p2 = 0; p2 < B1; ++p2) a[at(jp + p1 * (N / A1) + p2 * Lq1, col)] = v[p1][p2];
+  }
+  // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) are
+  // entirely zero, and so is their transform: store zeros, skip the other two groups.
+  const bool all_zero = __syncthreads_or(nz) == 0;
+  if (!STRIDED && all_zero) {
+    for (int row = 0; row < nrow; ++row) {
+      double2* o = out + hi * P.out_hi + (lo0 + row) * P.out_lo;
+      for (int mm = tid; mm < P.nout; mm += T) o[mm] = make_double2(0.0, 0.0);
+    }
+    return;
+  }
+
+  // ---- group 2: blocks of L2 = N / G1 points, twiddle step G1
+  {
+    constexpr int L2 = N / G1, Lq2 = L2 / G2;
+    for (int idx = tid; idx < (N / G2) * TB; idx += T) {
+      const int col = STRIDED ? idx % TB : idx / (N / G2);
+      const int g = STRIDED ? idx / TB : idx % (N / G2);
+      const int b = g / Lq2, jp = g - b * Lq2;
+      const int base = b * L2 + jp;
+      double2 v[A2][B2];
+#pragma unroll
+      for (int q1 = 0; q1 < A2; ++q1)
+#pragma unroll
+        for (int q2 = 0; q2 < B2; ++q2) v[q1][q2] = a[at(base + q1 * (L2 / A2) + q2 * Lq2, col)];
+      group_dft<A2, B2, false>(v, ftw + FT::off2a + jp, ftw + FT::off2b + jp, Lq2);
+#pragma unroll
+      for (int p1 = 0; p1 < A2; ++p1)
+#pragma unroll
+        for (int p2 = 0; p2 < B2; ++p2) a[at(base + p1 * (L2 / A2) + p2 * Lq2, col)] = v[p1][p2];
+    }
+  }
+  __syncthreads();
+
+  // ---- group 3: blocks of G3 points (no twiddles after the last radix); output (p1, p2) of block b is frequency
+  // klow[b] + (N / G3)(p1 + A3 p2)
+  for (int idx = tid; idx < (N / G3) * TB; idx += T) {
+    const int col = STRIDED ? idx % TB : idx / (N / G3);
+    const int b = STRIDED ? idx / TB : idx % (N / G3);
+    double2 v[A3][B3];
+#pragma unroll
+    for (int q1 = 0; q1 < A3; ++q1)
+#pragma unroll
+      for (int q2 = 0; q2 < B3; ++q2) v[q1][q2] = a[at(b * G3 + q1 * B3 + q2, col)];
+    group_dft<A3, B3, true>(v, ftw + FT::off3, nullptr, 0);
+    if (STRIDED) {
+      const int mm0 = s_mm[2 * col], mm1 = s_mm[2 * col + 1];
+      if (mm1 > mm0) {
+        double2* o = out + hi * P.out_hi + lo0 + col;
+        int mm = __ldg(&P.klow[b]) - P.lo;   // output index of frequency klow[b]; the band may wrap around N
+#pragma unroll
+        for (int p2 = 0; p2 < B3; ++p2)
+#pragma unroll
+          for (int p1 = 0; p1 < A3; ++p1) {
+            int m = mm + (N / G3) * (p1 + A3 * p2);
+            m = m < 0 ? m + N : (m >= N ? m - N : m);
+            if (m >= mm0 && m < mm1) o[(int64_t)m * P.out_el] = v[p1][p2];
+          }
+      }
+    } else {
+#pragma unroll
+      for (int p1 = 0; p1 < A3; ++p1)
+#pragma unroll
+        for (int p2 = 0; p2 < B3; ++p2) a[at(b * G3 + p1 * B3 + p2, col)] = v[p1][p2];
+    }
+  }
+  if (STRIDED) return;
+  __syncthreads();
+
+  // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table
+  for (int col = 0; col < ncol; ++col) {
+    double2* o0 = out + hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
+    const bool two = 2 * col + 1 < nrow;
+    for (int mm = tid; mm < P.nout; mm += T) {
+      int m = P.lo + mm;
+      m = m < 0 ? m + N : (m >= N ? m - N : m);
+      const double2 z = a[at(__ldg(&P.rev[m]), col)];
+      if (MODE == 0) {
+        const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
+        o0[mm] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
+        if (two) o0[P.out_lo + mm] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
+      } else {
+        o0[mm] = z;
+      }
+    }
+  }
+}
+
+// The lengths with a fixed plan and their factor sequence (A1, B1, A2, B2, A3, B3).
+bool fixed_plan_factors(int N, int f[6]) {
+  static const int plans[][7] = {{360, 4, 2, 3, 3, 5, 1},  {672, 4, 2, 4, 3, 7, 1},  {720, 4, 4, 3, 3, 5, 1},
+                                 {1344, 4, 4, 4, 3, 7, 1}, {1440, 4, 4, 2, 5, 3, 3}, {2700, 4, 3, 3, 5, 3, 5}};
+  for (const auto& pl : plans)
+    if (pl[0] == N) {
+      for (int i = 0; i < 6; ++i) f[i] = pl[1 + i];
+      return true;
+    }
+  return false;
 }
 
 // One pass; see FftPass (fft.cuh).  Shared memory: a[N][tbp] complex128.  THREADS = 512 with two CTAs per SM, or
@@ -420,6 +725,8 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
 struct HostTables {
   std::vector<double> tw;     // N complex: exp(-2 pi i t / N)
   std::vector<int32_t> rev;   // position of output frequency k after the DIF stages
+  std::vector<int32_t> klow;  // fixed-geometry plans: klow[b] = frequency stored at position b * G3 (G3 = last group)
+  std::vector<double> ftw;    // fixed-geometry plans: per-stage twiddle tables (FixedTw), complex
   int nfac;
   int fac[16];      // single radices in execution order
   int npair;
@@ -445,6 +752,16 @@ const HostTables& tables_for(int N) {
   while (n % 7 == 0) { rest.push_back(7); n /= 7; }
   t.nfac = 0;
   t.npair = 0;
+  int fx[6];
+  const bool fixed = fixed_plan_factors(N, fx);
+  if (fixed) {   // the fixed-geometry kernels and the generic one share the factor order (and so the reversal table)
+    rest.clear();
+    for (int g = 0; g < 3; ++g) {
+      t.fac[t.nfac++] = fx[2 * g];
+      if (fx[2 * g + 1] > 1) t.fac[t.nfac++] = fx[2 * g + 1];
+      t.pair[t.npair++] = fx[2 * g] * 8 + fx[2 * g + 1];
+    }
+  }
   while (!rest.empty()) {
     const int r1 = rest.front();
     rest.erase(rest.begin());
@@ -478,6 +795,29 @@ const HostTables& tables_for(int N) {
     }
     t.rev[k] = pos;
   }
+  t.klow.assign(N, 0);
+  if (fixed) {
+    const int A1 = fx[0], B1 = fx[1], A2 = fx[2], B2 = fx[3], A3 = fx[4], B3 = fx[5];
+    const int G1 = A1 * B1, G3 = A3 * B3, Lq1 = N / G1, Lq2 = G3;
+    for (int k = 0; k < N / G3; ++k) t.klow[t.rev[k] / G3] = k;
+    auto put = [&](long long idx) {   // exp(-2 pi i idx / N), the index reduced first so that every entry is exact to an ulp
+      idx %= N;
+      t.ftw.push_back(t.tw[2 * idx]);
+      t.ftw.push_back(t.tw[2 * idx + 1]);
+    };
+    for (int p1 = 1; p1 < A1; ++p1)
+      for (int q2 = 0; q2 < B1; ++q2)
+        for (int jp = 0; jp < Lq1; ++jp) put((long long)p1 * (jp + q2 * Lq1));
+    for (int p2 = 1; p2 < B1; ++p2)
+      for (int jp = 0; jp < Lq1; ++jp) put((long long)p2 * jp * A1);
+    for (int p1 = 1; p1 < A2; ++p1)
+      for (int q2 = 0; q2 < B2; ++q2)
+        for (int jp = 0; jp < Lq2; ++jp) put((long long)p1 * (jp + q2 * Lq2) * G1);
+    for (int p2 = 1; p2 < B2; ++p2)
+      for (int jp = 0; jp < Lq2; ++jp) put((long long)p2 * jp * G1 * A2);
+    for (int p1 = 1; p1 < A3; ++p1)
+      for (int q2 = 1; q2 < B3; ++q2) put((long long)p1 * q2 * (N / G3));
+  }
   return g_tables.emplace(N, std::move(t)).first->second;
 }
 
@@ -494,7 +834,9 @@ bool fft_length_ok(int N) {
 
 size_t fft_tables_bytes(const int n2[3]) {
   size_t b = 0;
-  for (int d = 0; d < 3; ++d) b += align_up((size_t)n2[d] * 16) + align_up((size_t)n2[d] * 4);
+  // twiddles, reversal table, klow, and the per-stage tables of a fixed plan (< 1.25 N entries)
+  for (int d = 0; d < 3; ++d)
+    b += align_up((size_t)n2[d] * 16) + 2 * align_up((size_t)n2[d] * 4) + align_up((size_t)n2[d] * 20 + 4096);
   return b;
 }
 
@@ -530,6 +872,13 @@ int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStrea
     out->rev[d] = reinterpret_cast<int32_t*>(base + o);
     SFD_CUDA_TRY(cudaMemcpyAsync(base + o, t.rev.data(), (size_t)n2[d] * 4, cudaMemcpyHostToDevice, st));
     o += align_up((size_t)n2[d] * 4);
+    out->klow[d] = reinterpret_cast<int32_t*>(base + o);
+    SFD_CUDA_TRY(cudaMemcpyAsync(base + o, t.klow.data(), (size_t)n2[d] * 4, cudaMemcpyHostToDevice, st));
+    o += align_up((size_t)n2[d] * 4);
+    out->ftw[d] = reinterpret_cast<double2*>(base + o);
+    SFD_REQUIRE(t.ftw.size() * 8 <= (size_t)n2[d] * 20 + 4096, SFD_ERR_UNSUPPORTED, "fixed-plan twiddle tables do not fit");
+    if (!t.ftw.empty()) SFD_CUDA_TRY(cudaMemcpyAsync(base + o, t.ftw.data(), t.ftw.size() * 8, cudaMemcpyHostToDevice, st));
+    o += align_up((size_t)n2[d] * 20 + 4096);
     out->nfac[d] = t.nfac;
     for (int s = 0; s < t.nfac; ++s) out->fac[d][s] = t.fac[s];
     out->npair[d] = t.npair;
@@ -538,9 +887,52 @@ int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStrea
   return SFD_OK;
 }
 
+namespace {
+// Launch of a fixed-geometry pass (above) when the length has a plan and exactly the central half of the inputs is
+// non-zero; returns false when the generic kernel has to run.
+template <class PL>
+int launch_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t st) {
+  const int mode = P.contig ? (P.real_in ? 0 : 1) : 2;
+  const int64_t rows_per_tile = (int64_t)PL::TB * (mode == 0 ? 2 : 1);
+  const int64_t tiles = P.n_hi * ((P.n_lo + rows_per_tile - 1) / rows_per_tile);
+  if (tiles == 0) return SFD_OK;
+  SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
+  const size_t smem = (size_t)PL::N * PL::TB * 16;
+  auto go = [&](auto kern) -> int {
+    SFD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)tiles, PL::T, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
+    return SFD_OK;
+  };
+  if (mode == 0) SFD_TRY(go(fft_fixed_kernel<PL, 0>));
+  else if (mode == 1) SFD_TRY(go(fft_fixed_kernel<PL, 1>));
+  else SFD_TRY(go(fft_fixed_kernel<PL, 2>));
+  return launch_check("fft_fixed_kernel");
+}
+bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t st, int* rc) {
+  if (P.n_in * 2 != P.N) return false;
+  if (P.contig ? (P.in_el != 1 || P.out_el != 1) : (P.real_in || P.dec_axis || P.in_lo != 1 || P.out_lo != 1)) return false;
+  switch (P.N) {   //                       N    A1 B1 A2 B2 A3 B3  TB   T  CTAs/SM
+    case 360:  *rc = launch_fixed<FixedPlan<360,  4, 2, 3, 3, 5, 1, 8, 128, 4>>(P, d_in, d_out, st); return true;
+    case 672:  *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 8, 256, 2>>(P, d_in, d_out, st); return true;
+    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 4, 3, 3, 5, 1, 8, 256, 2>>(P, d_in, d_out, st); return true;
+    case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
+    case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
+    case 2700: *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 2, 256, 2>>(P, d_in, d_out, st); return true;
+  }
+  return false;
+}
+}  // namespace
+
 int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* d_out, cudaStream_t st) {
   P.tw = T.tw[axis];
   P.rev = T.rev[axis];
+  P.klow = T.klow[axis];
+  P.ftw = T.ftw[axis];
+  {
+    int rc = SFD_OK;
+    const char* generic = std::getenv("SFD_FFT_GENERIC");   // debugging / A-B measurements: force the generic kernel
+    if (!(generic && generic[0] == '1') && try_fixed(P, d_in, d_out, st, &rc)) return rc;
+  }
   P.nfac = T.nfac[axis];
   for (int s = 0; s < P.nfac; ++s) P.fac[s] = T.fac[axis][s];
   P.tb = fft_tile(P.N, P.contig, &P.tbp);

@@ -8,6 +8,8 @@ namespace sfd {
 struct FftTables {
   const double2* tw[3];
   const int32_t* rev[3];
+  const int32_t* klow[3];   // fixed-geometry kernels: frequency of the first output of the last group's block b
+  const double2* ftw[3];    // fixed-geometry kernels: per-stage twiddle tables
   int nfac[3];
   int fac[3][16];
   int npair[3];
@@ -40,6 +42,8 @@ struct FftPass {
   unsigned magic[16];   // floor(2^32 / Lq) + 1 per pair: g / Lq = umulhi(g, magic)
   const double2* tw;
   const int32_t* rev;
+  const int32_t* klow;
+  const double2* ftw;
 };
 
 bool fft_length_ok(int N);
