@@ -221,7 +221,7 @@ int sfd_weak_distance_lattice(const double* d_vertices, int64_t nV, const int32_
  * faces -- loses accuracy (P:140 names the cancellation of the literal formula): ~1e-15 sum_f area_f absolute, plus the
  * fp64 rounding of the phases xi.p.  No quadrature rule is involved; against sfd_nodes + sfd_surface_ft it isolates
  * the triangle rule's error.  Device pointers; d_out complex128 [K]; a face with a vertex index outside [0, nV)
- * poisons every output with NaN (as sfd_nodes does).  d_work: sfd_exact_ft_workspace(nF) bytes (80 B per face).
+ * poisons every output with NaN and is reported by the next synchronising call (as for sfd_nodes).  d_work: sfd_exact_ft_workspace(nF) bytes (80 B per face).
  * With few frequencies the faces are split over CTAs and the partial sums meet in fp64 reductions whose order is not
  * fixed (reproducible to rounding only).  Enqueues on `stream`. */
 int sfd_exact_ft_workspace(int64_t nF, size_t* bytes);

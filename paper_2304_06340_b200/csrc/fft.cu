@@ -219,30 +219,25 @@ struct FixedPlan {
   static_assert((TB & (TB - 1)) == 0, "tile height must be a power of two");
 };
 
-// One fused group in registers: radix A over q1, twiddle, radix B over q2, twiddle.  v[q1][q2] -> v[p1][p2].
-// The twiddles come from per-stage tables laid out [row][jp] (FixedTw below), so that the lanes of a warp -- consecutive
-// jp -- read consecutive 16-byte entries: ta[((p1-1) B + q2) stride] = w^{p1 (jp + q2 Lq) tstep}, tb[(p2-1) stride] =
-// w^{p2 jp tstep A}; both pointers already point at column jp.  (Indexing the one table exp(-2 pi i k / N) by the products
-// made every lane of a load touch its own cache line: the L1 was the busiest unit of the pass, profiles/r2b_fft.md.)
-// LAST: the last group (jp = 0) has only the inner constants w_G^{p1 q2}, q2 >= 1: ta[(p1-1)(B-1) + (q2-1)].
+// One fused group = a radix-G DFT (G = A B) in registers followed by its outer twiddles, v[q1][q2] -> v[p1][p2]:
+//   radix A over q1;  inner constants c[p1][q2] = e^{-2 pi i p1 q2 / G} (p1, q2 >= 1; FftPass::cst, i.e. the kernel's
+//   parameter bank: compile-time indices make them immediate operands of the DFMA / DMUL);  radix B over q2;
+//   outer twiddles w^{p1 jp tstep} (row p1-1 of ta) and w^{p2 jp tstep A} (row p2-1 of tb), both in SHARED memory, laid out
+//   [row][jp] so that the lanes of a warp -- consecutive jp -- read consecutive 16-byte entries (pointers already point at
+//   column jp; `stride` = row length).  The product form w^{p1 (jp + q2 Lq)} = w^{p1 jp} c[p1][q2] keeps the tables at
+//   (A + B - 2) Lq entries per group (22 KB for N = 2700) instead of N: small enough to sit beside two resident CTAs' data.
+//   History: indexing the one table exp(-2 pi i k / N) by the products made every lane of a load touch its own cache line
+//   and the L1 the busiest unit of the pass (79 %); per-stage tables read through the L1 missed 80 % of the time
+//   (profiles/r2b_fft.md).
+// LAST: the last group (jp = 0) has no outer twiddles.
 template <int A, int B, bool LAST>
-__device__ __forceinline__ void group_dft(double2 (&v)[A][B], const double2* __restrict__ ta, const double2* __restrict__ tb,
-                                          int stride) {
+__device__ __forceinline__ void group_twiddle_b(double2 (&v)[A][B], const double2* __restrict__ cst,
+                                                const double2* __restrict__ ta, const double2* __restrict__ tb, int stride) {
+  // on entry v[p1][q2] holds the radix-A outputs (before any twiddle)
 #pragma unroll
-  for (int q2 = 0; q2 < B; ++q2) {
-    double2 x[A];
+  for (int p1 = 1; p1 < A; ++p1)
 #pragma unroll
-    for (int q1 = 0; q1 < A; ++q1) x[q1] = v[q1][q2];
-    bfly<A>(x);
-    v[0][q2] = x[0];
-#pragma unroll
-    for (int p1 = 1; p1 < A; ++p1) {
-      if (LAST)
-        v[p1][q2] = (B == 1 || q2 == 0) ? x[p1] : cmul(x[p1], __ldg(&ta[(p1 - 1) * (B - 1) + (q2 - 1)]));
-      else
-        v[p1][q2] = cmul(x[p1], __ldg(&ta[((p1 - 1) * B + q2) * stride]));
-    }
-  }
+    for (int q2 = 1; q2 < B; ++q2) v[p1][q2] = cmul(v[p1][q2], cst[(p1 - 1) * (B - 1) + (q2 - 1)]);
   if (B > 1) {
 #pragma unroll
     for (int p1 = 0; p1 < A; ++p1) {
@@ -250,245 +245,280 @@ __device__ __forceinline__ void group_dft(double2 (&v)[A][B], const double2* __r
 #pragma unroll
       for (int q2 = 0; q2 < B; ++q2) x[q2] = v[p1][q2];
       bfly<B>(x);
-      v[p1][0] = x[0];
 #pragma unroll
-      for (int p2 = 1; p2 < B; ++p2) v[p1][p2] = LAST ? x[p2] : cmul(x[p2], __ldg(&tb[(p2 - 1) * stride]));
+      for (int p2 = 0; p2 < B; ++p2) v[p1][p2] = x[p2];
+    }
+  }
+  if (!LAST) {
+#pragma unroll
+    for (int p1 = 1; p1 < A; ++p1) {
+      const double2 t = ta[(p1 - 1) * stride];
+#pragma unroll
+      for (int p2 = 0; p2 < B; ++p2) v[p1][p2] = cmul(v[p1][p2], t);
+    }
+#pragma unroll
+    for (int p2 = 1; p2 < B; ++p2) {
+      const double2 t = tb[(p2 - 1) * stride];
+#pragma unroll
+      for (int p1 = 0; p1 < A; ++p1) v[p1][p2] = cmul(v[p1][p2], t);
     }
   }
 }
+template <int A, int B, bool LAST>
+__device__ __forceinline__ void group_dft(double2 (&v)[A][B], const double2* __restrict__ cst, const double2* __restrict__ ta,
+                                          const double2* __restrict__ tb, int stride) {
+#pragma unroll
+  for (int q2 = 0; q2 < B; ++q2) {
+    double2 x[A];
+#pragma unroll
+    for (int q1 = 0; q1 < A; ++q1) x[q1] = v[q1][q2];
+    bfly<A>(x);
+#pragma unroll
+    for (int p1 = 0; p1 < A; ++p1) v[p1][q2] = x[p1];
+  }
+  group_twiddle_b<A, B, LAST>(v, cst, ta, tb, stride);
+}
 
-// Layout of the per-stage twiddle tables of a fixed plan (complex128 entries, one array per axis).
+// Layout of the outer-twiddle tables of a fixed plan (complex128 entries; one array per axis in global memory, copied
+// to shared memory once per CTA).
 template <class PL>
 struct FixedTw {
   static constexpr int Lq1 = PL::N / PL::G1, Lq2 = PL::G3;
-  static constexpr int off1a = 0;                                         // [3 B1][Lq1]: w^{p1 (jp + q2 Lq1)}
-  static constexpr int off1b = off1a + 3 * PL::B1 * Lq1;                   // [B1-1][Lq1]: w^{4 p2 jp}
-  static constexpr int off2a = off1b + (PL::B1 - 1) * Lq1;                 // [(A2-1) B2][Lq2]: w^{p1 (jp + q2 Lq2) G1}
-  static constexpr int off2b = off2a + (PL::A2 - 1) * PL::B2 * Lq2;        // [B2-1][Lq2]: w^{p2 jp G1 A2}
-  static constexpr int off3 = off2b + (PL::B2 - 1) * Lq2;                  // [(A3-1)(B3-1)]: w^{p1 q2 N / G3}
-  static constexpr int total = off3 + (PL::A3 - 1) * (PL::B3 - 1);
+  static constexpr int off1a = 0;                                   // [A1-1][Lq1]: w^{p1 jp}
+  static constexpr int off1b = off1a + (PL::A1 - 1) * Lq1;          // [B1-1][Lq1]: w^{A1 p2 jp}
+  static constexpr int off2a = off1b + (PL::B1 - 1) * Lq1;          // [A2-1][Lq2]: w^{p1 jp G1}
+  static constexpr int off2b = off2a + (PL::A2 - 1) * Lq2;          // [B2-1][Lq2]: w^{p2 jp G1 A2}
+  static constexpr int total = off2b + (PL::B2 - 1) * Lq2;
 };
 
 // MODE 0: contiguous axis, real input, two rows packed per column (pass A, real strengths); 1: contiguous axis, complex
-// input (pass A, complex strengths); 2: strided complex (passes B, C).  Shared memory: N * TB complex128, element
-// (pos, col) at pos * TB + col in the strided passes (lanes run over the tile's columns first, like the global accesses)
-// and at col * N + pos in the contiguous ones (lanes run along the axis).
+// input (pass A, complex strengths); 2: strided complex (passes B, C).  Persistent CTAs (PL::CTAS per SM) walk the tiles
+// of TB columns.  Shared memory: the twiddle tables, then N * TB complex128 of data, element (pos, col) at pos * TB + col
+// in the strided passes (lanes run over the tile's columns first, like the global accesses) and at col * N + pos in the
+// contiguous ones (lanes run along the axis).
 template <class PL, int MODE>
-__global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(FftPass P, const void* __restrict__ in_raw,
-                                                                    double2* __restrict__ out) {
+__global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid_constant__ FftPass P, const void* __restrict__ in_raw,
+                                                                    double2* __restrict__ out, int64_t n_tiles, int RUN) {
   constexpr int N = PL::N, TB = PL::TB, T = PL::T;
   constexpr int A1 = PL::A1, B1 = PL::B1, A2 = PL::A2, B2 = PL::B2, A3 = PL::A3, B3 = PL::B3;
   constexpr int G1 = PL::G1, G2 = PL::G2, G3 = PL::G3;
   constexpr bool STRIDED = MODE == 2;
   constexpr int PACK = MODE == 0 ? 2 : 1;
+  using FT = FixedTw<PL>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double2* a = reinterpret_cast<double2*>(smem_raw);
+  double2* stw = reinterpret_cast<double2*>(smem_raw);
+  double2* a = stw + FT::total;
   __shared__ int s_mm[2 * TB];   // strided passes: the range of outputs [mm0, mm1) every column of the tile has to store
   const int tid = threadIdx.x;
-  using FT = FixedTw<PL>;
-  const double2* __restrict__ ftw = P.ftw;
   auto at = [](int pos, int col) { return STRIDED ? pos * TB + col : col * N + pos; };
+  for (int i = tid; i < FT::total; i += T) stw[i] = P.ftw[i];
+  (void)G1;
+  __syncthreads();   // the twiddle tables are in place
 
   constexpr int64_t rows_per_tile = (int64_t)TB * PACK;
   const int64_t tiles_per_hi = (P.n_lo + rows_per_tile - 1) / rows_per_tile;
-  const int64_t hi = blockIdx.x / tiles_per_hi;
-  const int64_t lo0 = (blockIdx.x - hi * tiles_per_hi) * rows_per_tile;
-  const int nrow = (int)min(rows_per_tile, P.n_lo - lo0);
-  const int ncol = (nrow + PACK - 1) / PACK;
-  if (STRIDED) {
-    if (P.ball) {   // uniform in the block
-      bool needed = false;
-      for (int c = 0; c < ncol; ++c) needed = needed || ball_q(P, lo0 + c) <= 1.0;
-      if (!needed) return;
+  // Tiles are handed out in RUNS of consecutive tiles from a device counter (zeroed with the tables), so that the tiles in
+  // flight stay a contiguous window like the hardware's own block order: a tile touches TB * 16 bytes of every 128-byte
+  // line of the strided arrays, and the rest of the line is wanted by its neighbours while it is still in the L2 (with a
+  // fixed stride per CTA, or with streaming loads, the strided passes read 3.8x their input from DRAM:
+  // profiles/r2b_fft.md).
+  __shared__ int s_run;
+  for (;;) {
+    if (tid == 0) s_run = atomicAdd(P.counter, 1);
+    __syncthreads();
+    const int64_t run = s_run;
+    __syncthreads();   // (a run whose tiles are all skipped has no other barrier before s_run is written again)
+    if (run * RUN >= n_tiles) break;
+   for (int64_t tile = run * RUN; tile < min(n_tiles, (run + 1) * RUN); ++tile) {
+    const int64_t hi = tile / tiles_per_hi;
+    const int64_t lo0 = (tile - hi * tiles_per_hi) * rows_per_tile;
+    const int nrow = (int)min(rows_per_tile, P.n_lo - lo0);
+    const int ncol = (nrow + PACK - 1) / PACK;
+    if (STRIDED) {
+      if (P.ball) {   // uniform in the block
+        bool needed = false;
+        for (int c = 0; c < ncol; ++c) needed = needed || ball_q(P, lo0 + c) <= 1.0;
+        if (!needed) continue;
+      }
+      if (tid < TB) {
+        int mm0 = 0, mm1 = tid < ncol ? P.nout : 0;
+        if (P.ball && tid < ncol) {
+          const double q = ball_q(P, lo0 + tid);
+          if (q > 1.0) {
+            mm1 = 0;
+          } else {
+            const double rad = P.ball_rt * sqrt(1.0 - q) + 1.0;
+            mm0 = max(0, (int)floor(P.ball_ct - rad));
+            mm1 = min(P.nout, (int)ceil(P.ball_ct + rad) + 1);
+          }
+        }
+        s_mm[2 * tid] = mm0;
+        s_mm[2 * tid + 1] = mm1;
+      }
     }
-    if (tid < TB) {
-      int mm0 = 0, mm1 = tid < ncol ? P.nout : 0;
-      if (P.ball && tid < ncol) {
-        const double q = ball_q(P, lo0 + tid);
-        if (q > 1.0) {
-          mm1 = 0;
-        } else {
-          const double rad = P.ball_rt * sqrt(1.0 - q) + 1.0;
-          mm0 = max(0, (int)floor(P.ball_ct - rad));
-          mm1 = min(P.nout, (int)ceil(P.ball_ct + rad) + 1);
+
+    // ---- group 1: inputs from global memory.  Input i <-> mode l = i - N/4 <-> position l mod N: positions [0, N/4)
+    // hold i = pos + N/4, positions [3N/4, N) hold i = pos - 3N/4, the rest is zero: of the radix-4 butterfly (elements
+    // r + q1 N/4, r < N/4) only q1 = 0 (h = in[r + N/4]) and q1 = 3 (l = in[r]) exist:  X_p = h + i^p l.
+    constexpr int Lq1 = N / G1;
+    bool nz = STRIDED;
+    const double fhi = (MODE != 2 && P.dec_hi) ? P.dec_hi[hi] : 1.0;
+    for (int idx = tid; idx < Lq1 * TB; idx += T) {
+      const int col = STRIDED ? idx % TB : idx / Lq1;
+      const int jp = STRIDED ? idx / TB : idx % Lq1;
+      double2 xl[B1], xh[B1];
+      if (MODE == 2) {
+        const bool live = col < ncol;
+        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0);
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          const int r = jp + q2 * Lq1;
+          // L2-only loads with the normal retention: a tile uses TB * 16 bytes of every 128-byte line and the rest of
+          // the line is wanted by the next tiles of the run (streaming loads mark the line evict-first: 3.8x re-reads)
+          xl[q2] = live ? __ldcg(src + (int64_t)r * P.in_el) : make_double2(0.0, 0.0);
+          xh[q2] = live ? __ldcg(src + (int64_t)(r + N / 4) * P.in_el) : make_double2(0.0, 0.0);
+        }
+      } else if (MODE == 1) {
+        const bool live = col < ncol;
+        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + (live ? col : 0)) * P.in_lo;
+        const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + (live ? col : 0)] : 1.0;
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          const int r = jp + q2 * Lq1;
+          const double fl = P.dec_axis ? f0 * P.dec_axis[r] : 1.0, fh = P.dec_axis ? f0 * P.dec_axis[r + N / 4] : 1.0;
+          const double2 l = live ? __ldcs(src + r) : make_double2(0.0, 0.0);
+          const double2 h = live ? __ldcs(src + r + N / 4) : make_double2(0.0, 0.0);
+          xl[q2] = make_double2(l.x * fl, l.y * fl);
+          xh[q2] = make_double2(h.x * fh, h.y * fh);
+          nz |= (l.x != 0.0) | (l.y != 0.0) | (h.x != 0.0) | (h.y != 0.0);
+        }
+      } else {
+        const bool live = col < ncol, two = 2 * col + 1 < nrow;
+        const int64_t r0 = lo0 + 2 * (live ? col : 0);
+        const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
+        const double* src1 = src0 + (two ? P.in_lo : 0);
+        const double f0 = live ? (P.dec_axis ? fhi * P.dec_lo[r0] : 1.0) : 0.0;
+        const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
+        double la[B1], lb[B1], ha[B1], hb[B1], fl[B1], fh[B1];
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          const int r = jp + q2 * Lq1;
+          la[q2] = __ldcs(src0 + r);
+          lb[q2] = __ldcs(src1 + r);
+          ha[q2] = __ldcs(src0 + r + N / 4);
+          hb[q2] = __ldcs(src1 + r + N / 4);
+          fl[q2] = P.dec_axis ? P.dec_axis[r] : 1.0;
+          fh[q2] = P.dec_axis ? P.dec_axis[r + N / 4] : 1.0;
+        }
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          nz |= live & ((la[q2] != 0.0) | (lb[q2] != 0.0) | (ha[q2] != 0.0) | (hb[q2] != 0.0));
+          xl[q2] = make_double2(la[q2] * (fl[q2] * f0), lb[q2] * (fl[q2] * f1));
+          xh[q2] = make_double2(ha[q2] * (fh[q2] * f0), hb[q2] * (fh[q2] * f1));
         }
       }
-      s_mm[2 * tid] = mm0;
-      s_mm[2 * tid + 1] = mm1;
-    }
-  }
-
-  // ---- group 1: inputs from global memory.  Input i <-> mode l = i - N/4 <-> position l mod N: positions [0, N/4) hold
-  // i = pos + N/4, positions [3N/4, N) hold i = pos - 3N/4, the rest is zero: of the radix-4 butterfly (elements r + q1 N/4,
-  // r < N/4) only q1 = 0 (hi = in[r + N/4]) and q1 = 3 (lo = in[r]) exist:  X_p = hi + i^p lo.
-  constexpr int Lq1 = N / G1;
-  bool nz = STRIDED;
-  const double fhi = (MODE != 2 && P.dec_hi) ? P.dec_hi[hi] : 1.0;
-  for (int idx = tid; idx < Lq1 * TB; idx += T) {
-    const int col = STRIDED ? idx % TB : idx / Lq1;
-    const int jp = STRIDED ? idx / TB : idx % Lq1;
-    double2 xl[B1], xh[B1];
-    if (MODE == 2) {
-      const bool live = col < ncol;
-      const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0);
+      double2 v[A1][B1];
 #pragma unroll
       for (int q2 = 0; q2 < B1; ++q2) {
-        const int r = jp + q2 * Lq1;
-        xl[q2] = live ? __ldcs(src + (int64_t)r * P.in_el) : make_double2(0.0, 0.0);
-        xh[q2] = live ? __ldcs(src + (int64_t)(r + N / 4) * P.in_el) : make_double2(0.0, 0.0);
+        const double2 h = xh[q2], l = xl[q2];
+        v[0][q2] = cadd(h, l);
+        v[1][q2] = make_double2(h.x - l.y, h.y + l.x);   // h + i l
+        v[2][q2] = csub(h, l);
+        v[3][q2] = make_double2(h.x + l.y, h.y - l.x);   // h - i l
       }
-    } else if (MODE == 1) {
-      const bool live = col < ncol;
-      const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + (live ? col : 0)) * P.in_lo;
-      const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + (live ? col : 0)] : 1.0;
+      group_twiddle_b<A1, B1, false>(v, P.cst[0], stw + FT::off1a + jp, stw + FT::off1b + jp, Lq1);
 #pragma unroll
-      for (int q2 = 0; q2 < B1; ++q2) {
-        const int r = jp + q2 * Lq1;
-        const double fl = P.dec_axis ? f0 * P.dec_axis[r] : 1.0, fh = P.dec_axis ? f0 * P.dec_axis[r + N / 4] : 1.0;
-        const double2 l = live ? __ldcs(src + r) : make_double2(0.0, 0.0);
-        const double2 h = live ? __ldcs(src + r + N / 4) : make_double2(0.0, 0.0);
-        xl[q2] = make_double2(l.x * fl, l.y * fl);
-        xh[q2] = make_double2(h.x * fh, h.y * fh);
-        nz |= (l.x != 0.0) | (l.y != 0.0) | (h.x != 0.0) | (h.y != 0.0);
-      }
-    } else {
-      const bool live = col < ncol, two = 2 * col + 1 < nrow;
-      const int64_t r0 = lo0 + 2 * (live ? col : 0);
-      const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
-      const double* src1 = src0 + (two ? P.in_lo : 0);
-      const double f0 = live ? (P.dec_axis ? fhi * P.dec_lo[r0] : 1.0) : 0.0;
-      const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
-      double la[B1], lb[B1], ha[B1], hb[B1], fl[B1], fh[B1];
+      for (int p1 = 0; p1 < A1; ++p1)
 #pragma unroll
-      for (int q2 = 0; q2 < B1; ++q2) {
-        const int r = jp + q2 * Lq1;
-        la[q2] = __ldcs(src0 + r);
-        lb[q2] = __ldcs(src1 + r);
-        ha[q2] = __ldcs(src0 + r + N / 4);
-        hb[q2] = __ldcs(src1 + r + N / 4);
-        fl[q2] = P.dec_axis ? P.dec_axis[r] : 1.0;
-        fh[q2] = P.dec_axis ? P.dec_axis[r + N / 4] : 1.0;
-      }
-#pragma unroll
-      for (int q2 = 0; q2 < B1; ++q2) {
-        nz |= live & ((la[q2] != 0.0) | (lb[q2] != 0.0) | (ha[q2] != 0.0) | (hb[q2] != 0.0));
-        xl[q2] = make_double2(la[q2] * (fl[q2] * f0), lb[q2] * (fl[q2] * f1));
-        xh[q2] = make_double2(ha[q2] * (fh[q2] * f0), hb[q2] * (fh[q2] * f1));
-      }
+        for (int p2 = 0; p2 < B1; ++p2) a[at(jp + p1 * (N / A1) + p2 * Lq1, col)] = v[p1][p2];
     }
-    double2 v[A1][B1];
-#pragma unroll
-    for (int q2 = 0; q2 < B1; ++q2) {
-      const int r = jp + q2 * Lq1;
-      const double2 h = xh[q2], l = xl[q2];
-      (void)r;
-      const double2* t1 = ftw + FT::off1a + q2 * Lq1 + jp;
-      v[0][q2] = cadd(h, l);
-      v[1][q2] = cmul(make_double2(h.x - l.y, h.y + l.x), __ldg(t1));                     // (h + i l) w^r
-      v[2][q2] = cmul(csub(h, l), __ldg(t1 + B1 * Lq1));                                  // (h - l) w^2r
-      v[3][q2] = cmul(make_double2(h.x + l.y, h.y - l.x), __ldg(t1 + 2 * B1 * Lq1));      // (h - i l) w^3r
-    }
-    if (B1 > 1) {
-#pragma unroll
-      for (int p1 = 0; p1 < A1; ++p1) {
-        double2 x[B1];
-#pragma unroll
-        for (int q2 = 0; q2 < B1; ++q2) x[q2] = v[p1][q2];
-        bfly<B1>(x);
-        v[p1][0] = x[0];
-#pragma unroll
-        for (int p2 = 1; p2 < B1; ++p2) v[p1][p2] = cmul(x[p2], __ldg(ftw + FT::off1b + (p2 - 1) * Lq1 + jp));
+    // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) are
+    // entirely zero, and so is their transform: store zeros, skip the other two groups.
+    const bool all_zero = __syncthreads_or(nz) == 0;
+    if (!STRIDED && all_zero) {
+      for (int row = 0; row < nrow; ++row) {
+        double2* o = out + hi * P.out_hi + (lo0 + row) * P.out_lo;
+        for (int mm = tid; mm < P.nout; mm += T) o[mm] = make_double2(0.0, 0.0);
       }
+      continue;   // (the next tile's group 1 writes shared memory nobody reads any more: every thread is past the barrier)
     }
-#pragma unroll
-    for (int p1 = 0; p1 < A1; ++p1)
-#pragma unroll
-      for (int p2 = 0; p2 < B1; ++p2) a[at(jp + p1 * (N / A1) + p2 * Lq1, col)] = v[p1][p2];
-  }
-  // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) are
-  // entirely zero, and so is their transform: store zeros, skip the other two groups.
-  const bool all_zero = __syncthreads_or(nz) == 0;
-  if (!STRIDED && all_zero) {
-    for (int row = 0; row < nrow; ++row) {
-      double2* o = out + hi * P.out_hi + (lo0 + row) * P.out_lo;
-      for (int mm = tid; mm < P.nout; mm += T) o[mm] = make_double2(0.0, 0.0);
-    }
-    return;
-  }
 
-  // ---- group 2: blocks of L2 = N / G1 points, twiddle step G1
-  {
-    constexpr int L2 = N / G1, Lq2 = L2 / G2;
-    for (int idx = tid; idx < (N / G2) * TB; idx += T) {
-      const int col = STRIDED ? idx % TB : idx / (N / G2);
-      const int g = STRIDED ? idx / TB : idx % (N / G2);
-      const int b = g / Lq2, jp = g - b * Lq2;
-      const int base = b * L2 + jp;
-      double2 v[A2][B2];
+    // ---- group 2: blocks of L2 = N / G1 points, twiddle step G1
+    {
+      constexpr int L2 = N / G1, Lq2 = L2 / G2;
+      for (int idx = tid; idx < (N / G2) * TB; idx += T) {
+        const int col = STRIDED ? idx % TB : idx / (N / G2);
+        const int g = STRIDED ? idx / TB : idx % (N / G2);
+        const int b = g / Lq2, jp = g - b * Lq2;
+        const int base = b * L2 + jp;
+        double2 v[A2][B2];
 #pragma unroll
-      for (int q1 = 0; q1 < A2; ++q1)
+        for (int q1 = 0; q1 < A2; ++q1)
 #pragma unroll
-        for (int q2 = 0; q2 < B2; ++q2) v[q1][q2] = a[at(base + q1 * (L2 / A2) + q2 * Lq2, col)];
-      group_dft<A2, B2, false>(v, ftw + FT::off2a + jp, ftw + FT::off2b + jp, Lq2);
+          for (int q2 = 0; q2 < B2; ++q2) v[q1][q2] = a[at(base + q1 * (L2 / A2) + q2 * Lq2, col)];
+        group_dft<A2, B2, false>(v, P.cst[1], stw + FT::off2a + jp, stw + FT::off2b + jp, Lq2);
 #pragma unroll
-      for (int p1 = 0; p1 < A2; ++p1)
+        for (int p1 = 0; p1 < A2; ++p1)
 #pragma unroll
-        for (int p2 = 0; p2 < B2; ++p2) a[at(base + p1 * (L2 / A2) + p2 * Lq2, col)] = v[p1][p2];
-    }
-  }
-  __syncthreads();
-
-  // ---- group 3: blocks of G3 points (no twiddles after the last radix); output (p1, p2) of block b is frequency
-  // klow[b] + (N / G3)(p1 + A3 p2)
-  for (int idx = tid; idx < (N / G3) * TB; idx += T) {
-    const int col = STRIDED ? idx % TB : idx / (N / G3);
-    const int b = STRIDED ? idx / TB : idx % (N / G3);
-    double2 v[A3][B3];
-#pragma unroll
-    for (int q1 = 0; q1 < A3; ++q1)
-#pragma unroll
-      for (int q2 = 0; q2 < B3; ++q2) v[q1][q2] = a[at(b * G3 + q1 * B3 + q2, col)];
-    group_dft<A3, B3, true>(v, ftw + FT::off3, nullptr, 0);
-    if (STRIDED) {
-      const int mm0 = s_mm[2 * col], mm1 = s_mm[2 * col + 1];
-      if (mm1 > mm0) {
-        double2* o = out + hi * P.out_hi + lo0 + col;
-        int mm = __ldg(&P.klow[b]) - P.lo;   // output index of frequency klow[b]; the band may wrap around N
-#pragma unroll
-        for (int p2 = 0; p2 < B3; ++p2)
-#pragma unroll
-          for (int p1 = 0; p1 < A3; ++p1) {
-            int m = mm + (N / G3) * (p1 + A3 * p2);
-            m = m < 0 ? m + N : (m >= N ? m - N : m);
-            if (m >= mm0 && m < mm1) o[(int64_t)m * P.out_el] = v[p1][p2];
-          }
+          for (int p2 = 0; p2 < B2; ++p2) a[at(base + p1 * (L2 / A2) + p2 * Lq2, col)] = v[p1][p2];
       }
-    } else {
-#pragma unroll
-      for (int p1 = 0; p1 < A3; ++p1)
-#pragma unroll
-        for (int p2 = 0; p2 < B3; ++p2) a[at(b * G3 + p1 * B3 + p2, col)] = v[p1][p2];
     }
-  }
-  if (STRIDED) return;
-  __syncthreads();
+    __syncthreads();
 
-  // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table
-  for (int col = 0; col < ncol; ++col) {
-    double2* o0 = out + hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
-    const bool two = 2 * col + 1 < nrow;
-    for (int mm = tid; mm < P.nout; mm += T) {
-      int m = P.lo + mm;
-      m = m < 0 ? m + N : (m >= N ? m - N : m);
-      const double2 z = a[at(__ldg(&P.rev[m]), col)];
-      if (MODE == 0) {
-        const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
-        o0[mm] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
-        if (two) o0[P.out_lo + mm] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
+    // ---- group 3: blocks of G3 points (no outer twiddles); output (p1, p2) of block b is frequency
+    // klow[b] + (N / G3)(p1 + A3 p2)
+    for (int idx = tid; idx < (N / G3) * TB; idx += T) {
+      const int col = STRIDED ? idx % TB : idx / (N / G3);
+      const int b = STRIDED ? idx / TB : idx % (N / G3);
+      double2 v[A3][B3];
+#pragma unroll
+      for (int q1 = 0; q1 < A3; ++q1)
+#pragma unroll
+        for (int q2 = 0; q2 < B3; ++q2) v[q1][q2] = a[at(b * G3 + q1 * B3 + q2, col)];
+      group_dft<A3, B3, true>(v, P.cst[2], nullptr, nullptr, 0);
+      if (STRIDED) {
+        const int mm0 = s_mm[2 * col], mm1 = s_mm[2 * col + 1];
+        if (mm1 > mm0) {
+          double2* o = out + hi * P.out_hi + lo0 + col;
+          const int mm = __ldg(&P.klow[b]) - P.lo;   // output index of frequency klow[b]; the band may wrap around N
+#pragma unroll
+          for (int p2 = 0; p2 < B3; ++p2)
+#pragma unroll
+            for (int p1 = 0; p1 < A3; ++p1) {
+              int m = mm + (N / G3) * (p1 + A3 * p2);
+              m = m < 0 ? m + N : (m >= N ? m - N : m);
+              if (m >= mm0 && m < mm1) o[(int64_t)m * P.out_el] = v[p1][p2];   // (partial lines: they meet in the L2)
+            }
+        }
       } else {
-        o0[mm] = z;
+#pragma unroll
+        for (int p1 = 0; p1 < A3; ++p1)
+#pragma unroll
+          for (int p2 = 0; p2 < B3; ++p2) a[at(b * G3 + p1 * B3 + p2, col)] = v[p1][p2];
       }
     }
+    __syncthreads();
+    if (STRIDED) continue;
+
+    // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table
+    for (int col = 0; col < ncol; ++col) {
+      double2* o0 = out + hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
+      const bool two = 2 * col + 1 < nrow;
+      for (int mm = tid; mm < P.nout; mm += T) {
+        int m = P.lo + mm;
+        m = m < 0 ? m + N : (m >= N ? m - N : m);
+        const double2 z = a[at(__ldg(&P.rev[m]), col)];
+        if (MODE == 0) {
+          const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
+          __stcs(&o0[mm], make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)));
+          if (two) __stcs(&o0[P.out_lo + mm], make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)));
+        } else {
+          __stcs(&o0[mm], z);
+        }
+      }
+    }
+    __syncthreads();
+   }
   }
 }
 
@@ -726,7 +756,8 @@ struct HostTables {
   std::vector<double> tw;     // N complex: exp(-2 pi i t / N)
   std::vector<int32_t> rev;   // position of output frequency k after the DIF stages
   std::vector<int32_t> klow;  // fixed-geometry plans: klow[b] = frequency stored at position b * G3 (G3 = last group)
-  std::vector<double> ftw;    // fixed-geometry plans: per-stage twiddle tables (FixedTw), complex
+  std::vector<double> ftw;    // fixed-geometry plans: outer-twiddle tables (FixedTw), complex
+  double cst[3][9][2] = {};   // fixed-geometry plans: inner constants of the three groups
   int nfac;
   int fac[16];      // single radices in execution order
   int npair;
@@ -806,17 +837,25 @@ const HostTables& tables_for(int N) {
       t.ftw.push_back(t.tw[2 * idx + 1]);
     };
     for (int p1 = 1; p1 < A1; ++p1)
-      for (int q2 = 0; q2 < B1; ++q2)
-        for (int jp = 0; jp < Lq1; ++jp) put((long long)p1 * (jp + q2 * Lq1));
+      for (int jp = 0; jp < Lq1; ++jp) put((long long)p1 * jp);
     for (int p2 = 1; p2 < B1; ++p2)
       for (int jp = 0; jp < Lq1; ++jp) put((long long)p2 * jp * A1);
     for (int p1 = 1; p1 < A2; ++p1)
-      for (int q2 = 0; q2 < B2; ++q2)
-        for (int jp = 0; jp < Lq2; ++jp) put((long long)p1 * (jp + q2 * Lq2) * G1);
+      for (int jp = 0; jp < Lq2; ++jp) put((long long)p1 * jp * G1);
     for (int p2 = 1; p2 < B2; ++p2)
       for (int jp = 0; jp < Lq2; ++jp) put((long long)p2 * jp * G1 * A2);
-    for (int p1 = 1; p1 < A3; ++p1)
-      for (int q2 = 1; q2 < B3; ++q2) put((long long)p1 * q2 * (N / G3));
+    // inner constants of the three groups: e^{-2 pi i p1 q2 / (A B)} = entry p1 q2 N / (A B) of the twiddle table
+    for (int g = 0; g < 3; ++g) {
+      const int A = fx[2 * g], B = fx[2 * g + 1];
+      for (int p1 = 1; p1 < A; ++p1)
+        for (int q2 = 1; q2 < B; ++q2) {
+          const long long idx = ((long long)p1 * q2 * (N / (A * B))) % N;
+          t.cst[g][(p1 - 1) * (B - 1) + (q2 - 1)][0] = t.tw[2 * idx];
+          t.cst[g][(p1 - 1) * (B - 1) + (q2 - 1)][1] = t.tw[2 * idx + 1];
+        }
+    }
+    (void)A3;
+    (void)B3;
   }
   return g_tables.emplace(N, std::move(t)).first->second;
 }
@@ -837,7 +876,7 @@ size_t fft_tables_bytes(const int n2[3]) {
   // twiddles, reversal table, klow, and the per-stage tables of a fixed plan (< 1.25 N entries)
   for (int d = 0; d < 3; ++d)
     b += align_up((size_t)n2[d] * 16) + 2 * align_up((size_t)n2[d] * 4) + align_up((size_t)n2[d] * 20 + 4096);
-  return b;
+  return b + 256;   // + the passes' tile counters
 }
 
 // Rows per tile (a power of two) and row pitch.  Prefer tiles that let two CTAs share an SM (one CTA's loads and
@@ -862,7 +901,9 @@ int fft_tile(int N, int contig, int* tbp) {
 
 int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStream_t st) {
   char* base = static_cast<char*>(d_tables);
-  size_t o = 0;
+  size_t o = 256;
+  out->counters = reinterpret_cast<int32_t*>(base);   // one tile counter per pass, zero until its pass runs
+  SFD_CUDA_TRY(cudaMemsetAsync(base, 0, 256, st));
   for (int d = 0; d < 3; ++d) {
     SFD_REQUIRE(fft_length_ok(n2[d]) && fft_tile(n2[d], 1, nullptr) > 0, SFD_ERR_UNSUPPORTED, "FFT length %d is not supported", n2[d]);
     const HostTables& t = tables_for(n2[d]);
@@ -879,6 +920,8 @@ int fft_upload_tables(const int n2[3], void* d_tables, FftTables* out, cudaStrea
     SFD_REQUIRE(t.ftw.size() * 8 <= (size_t)n2[d] * 20 + 4096, SFD_ERR_UNSUPPORTED, "fixed-plan twiddle tables do not fit");
     if (!t.ftw.empty()) SFD_CUDA_TRY(cudaMemcpyAsync(base + o, t.ftw.data(), t.ftw.size() * 8, cudaMemcpyHostToDevice, st));
     o += align_up((size_t)n2[d] * 20 + 4096);
+    for (int g = 0; g < 3; ++g)
+      for (int i = 0; i < 9; ++i) out->cst[d][g][i] = make_double2(t.cst[g][i][0], t.cst[g][i][1]);
     out->nfac[d] = t.nfac;
     for (int s = 0; s < t.nfac; ++s) out->fac[d][s] = t.fac[s];
     out->npair[d] = t.npair;
@@ -896,11 +939,14 @@ int launch_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t
   const int64_t rows_per_tile = (int64_t)PL::TB * (mode == 0 ? 2 : 1);
   const int64_t tiles = P.n_hi * ((P.n_lo + rows_per_tile - 1) / rows_per_tile);
   if (tiles == 0) return SFD_OK;
-  SFD_REQUIRE(tiles < 0x7fffffffLL, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
-  const size_t smem = (size_t)PL::N * PL::TB * 16;
+  const size_t smem = ((size_t)PL::N * PL::TB + FixedTw<PL>::total) * 16;
+  SFD_REQUIRE(tiles < 0x7fffffffLL && P.counter, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
+  unsigned grid = (unsigned)std::min<int64_t>(tiles, (int64_t)PL::CTAS * num_sms());   // persistent CTAs
+  // tiles per run: two 64-byte tiles share a 128-byte line (measured at config 5: run 1 / 2 / 4 -> 49.6 / 47.1 / 50.1 ms)
+  const int run = (mode == 2 && PL::TB <= 4) ? 2 : 1;
   auto go = [&](auto kern) -> int {
     SFD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<(unsigned)tiles, PL::T, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out));
+    kern<<<grid, PL::T, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out), tiles, run);
     return SFD_OK;
   };
   if (mode == 0) SFD_TRY(go(fft_fixed_kernel<PL, 0>));
@@ -917,7 +963,9 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
     case 720:  *rc = launch_fixed<FixedPlan<720,  4, 4, 3, 3, 5, 1, 8, 256, 2>>(P, d_in, d_out, st); return true;
     case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
     case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
-    case 2700: *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 2, 256, 2>>(P, d_in, d_out, st); return true;
+    // 2700: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each (54.6 -> 47.1 ms
+    // at config 5: the strided passes' DRAM over-fetch halves); at 1344 the same trade loses (5.0 -> 5.6 ms)
+    case 2700: *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 4, 512, 1>>(P, d_in, d_out, st); return true;
   }
   return false;
 }
@@ -928,6 +976,9 @@ int fft_pass(FftPass P, const FftTables& T, int axis, const void* d_in, double* 
   P.rev = T.rev[axis];
   P.klow = T.klow[axis];
   P.ftw = T.ftw[axis];
+  P.counter = T.counters + axis;
+  for (int g = 0; g < 3; ++g)
+    for (int i = 0; i < 9; ++i) P.cst[g][i] = T.cst[axis][g][i];
   {
     int rc = SFD_OK;
     const char* generic = std::getenv("SFD_FFT_GENERIC");   // debugging / A-B measurements: force the generic kernel

@@ -9,7 +9,9 @@ struct FftTables {
   const double2* tw[3];
   const int32_t* rev[3];
   const int32_t* klow[3];   // fixed-geometry kernels: frequency of the first output of the last group's block b
-  const double2* ftw[3];    // fixed-geometry kernels: per-stage twiddle tables
+  const double2* ftw[3];    // fixed-geometry kernels: outer-twiddle tables
+  int32_t* counters;        // fixed-geometry kernels: one zeroed tile counter per axis (each pass runs once per upload)
+  double2 cst[3][3][9];     // fixed-geometry kernels: inner constants e^{-2 pi i p1 q2 / G} of the three groups, per axis
   int nfac[3];
   int fac[3][16];
   int npair[3];
@@ -44,6 +46,8 @@ struct FftPass {
   const int32_t* rev;
   const int32_t* klow;
   const double2* ftw;
+  int32_t* counter;
+  double2 cst[3][9];
 };
 
 bool fft_length_ok(int N);

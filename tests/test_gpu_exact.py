@@ -120,3 +120,8 @@ def test_exact_ft_edge_cases(sfd, torch):
     bad = F.clone()
     bad[5, 1] = V.shape[0]                                   # out-of-range vertex index poisons the output
     assert torch.isnan(torch.view_as_real(sfd.sfd_exact_ft(V, bad, xi))).all()
+    # ... and is reported (SFD_ERR_INVALID_ARG) by the next synchronising call on the device, once
+    with pytest.raises(sfd.SfdError) as e:
+        sfd.sfd_extents(V)
+    assert e.value.status == -2
+    assert sfd.sfd_extents(V)[0][0] > 0
