@@ -257,6 +257,20 @@ int sfd_weak_distance_host(const double* h_vertices, int64_t nV, const int32_t* 
                            double s, double R, const sfd_freq_quadrature* q, double eps,
                            double* h_distance, double* h_I);
 
+/* ---- single-precision grids -----------------------------------------------------------------
+ * The paper ran its GPU NUFFT "in single precision" at eps_rel = 1e-7 because "shared memory is too small for practical
+ * computations in the double-precision" (Fig. 4 caption P:242).  sfd_set_grid_precision(32) makes every
+ * later transform of the CALLING THREAD keep its grids in single precision: the fine (spreading) grid, the
+ * intermediates and the output band of the FFT passes in global memory, and the interpolation's shared-memory subgrid
+ * (8-byte cells, twice the cells per bin; the gather accumulates its w planes in fp32).  Everything else -- atoms,
+ * kernel evaluation, the spreader's shared-memory accumulation, the butterflies, phases, deconvolution factors, the
+ * reduction -- stays fp64, so the error is the rounding of the stored grids (~6e-8 of their largest entries) on top of
+ * the kernel's eps.  Accepted tolerances: eps >= 1e-6 for the type-3 transform, eps >= 1e-7 (the paper's) on the
+ * lattice (type-1: no interpolation); a smaller eps > 0 returns SFD_ERR_INVALID_ARG while the switch is on.  eps == 0
+ * (direct sum) is unaffected.  Error bar: 10 * max(eps, 1e-6) * sum|w_j|.  Workspace queries are precision-independent
+ * (sized for fp64).  bits = 64 (the default) restores double precision.  Host-only; thread-local. */
+int sfd_set_grid_precision(int bits);
+
 /* ---- per-stage device timings of the last sfd_surface_ft / sfd_weak_distance call on this thread
  * (only recorded after sfd_set_profiling(1); adds event records and a sync).  Names are static
  * strings; returns the number of stages written (<= max). */

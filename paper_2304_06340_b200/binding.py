@@ -82,6 +82,7 @@ _SIGS = {
     "sfd_mesh_distance": (C.c_int, [_vp, _i64, _vp, _i64, _vp, _i64, _vp, _i64, C.c_int, _dbl, _dbl,
                                     _P(sfd_freq_quadrature), _dbl, _vp, _sz, _vp, _P(_dbl), _P(_dbl)]),
     "sfd_set_profiling": (C.c_int, [C.c_int]),
+    "sfd_set_grid_precision": (C.c_int, [C.c_int]),
     "sfd_last_stage_times": (C.c_int, [_P(C.c_char_p), _P(C.c_float), C.c_int]),
 }
 for _name, (_res, _args) in _SIGS.items():
@@ -310,6 +311,11 @@ def sfd_weak_distance_host(V, F, rule, s, R, q, eps=0.0):
 
 def sfd_set_profiling(on):
     _chk(_lib.sfd_set_profiling(1 if on else 0))
+
+
+def sfd_set_grid_precision(bits):
+    """32: later transforms of this thread keep their grids in single precision (eps >= 1e-6); 64: fp64."""
+    _chk(_lib.sfd_set_grid_precision(int(bits)))
 
 
 def sfd_last_stage_times():

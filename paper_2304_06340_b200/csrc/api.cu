@@ -40,6 +40,10 @@ int num_sms() {
   return sms;
 }
 
+// ---- grid precision of the calling thread's transforms (sfd_set_grid_precision) ----------------------------------
+static thread_local bool g_grid_f32 = false;
+bool grid_f32() { return g_grid_f32; }
+
 // ---- stage timing ---------------------------------------------------------------------------------
 namespace {
 constexpr int kMaxStages = 32;
@@ -137,6 +141,12 @@ int sfd_release_cache(void) {
 }
 
 long long sfd_launch_count(void) { return g_launches.load(); }
+
+int sfd_set_grid_precision(int bits) {
+  SFD_REQUIRE(bits == 32 || bits == 64, SFD_ERR_INVALID_ARG, "grid precision must be 32 or 64 bits, got %d", bits);
+  g_grid_f32 = bits == 32;
+  return SFD_OK;
+}
 
 // ---- extents of a point set (A5-1 as a call of its own) ----------------------------------------------
 int sfd_extents_workspace(size_t* bytes) {
@@ -664,7 +674,13 @@ int lattice_ft(const double* d_x, const double* d_w, int64_t J, int M, double xi
     if (rc != SFD_OK || ok) return rc;
   }
   SFD_TRY(lattice_expand(M, xi_max, d_xi_buf, nullptr, st));
-  return sfd_surface_ft(d_x, d_w, J, d_xi_buf, K, eps, d_nuhat, d_work, work_bytes, stream);
+  // the fallback is the type-3 transform, whose single-precision grids carry eps >= 1e-6 only: a tighter tolerance (the
+  // lattice accepts 1e-7, the paper's) runs it with fp64 grids
+  const bool f32 = g_grid_f32;
+  if (eps < 1e-6) g_grid_f32 = false;
+  const int rc = sfd_surface_ft(d_x, d_w, J, d_xi_buf, K, eps, d_nuhat, d_work, work_bytes, stream);
+  g_grid_f32 = f32;
+  return rc;
 }
 }  // namespace
 

@@ -35,6 +35,30 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
 __device__ __forceinline__ double2 mul_mi(double2 a) { return make_double2(a.y, -a.x); }   // a * (-i)
 __device__ __forceinline__ double2 mul_pi(double2 a) { return make_double2(-a.y, a.x); }   // a * (+i)
 
+// Global-memory elements of a pass: fp64, or single precision when FftPass::f32 (the arithmetic and the shared-memory
+// rows stay fp64 either way).  `i` counts elements of the array's own type.
+__device__ __forceinline__ double ld_real(const void* base, int64_t i, int f32) {
+  return f32 ? (double)__ldcs(static_cast<const float*>(base) + i) : __ldcs(static_cast<const double*>(base) + i);
+}
+__device__ __forceinline__ double2 ld_cplx_cs(const void* base, int64_t i, int f32) {
+  if (f32) {
+    const float2 v = __ldcs(static_cast<const float2*>(base) + i);
+    return make_double2((double)v.x, (double)v.y);
+  }
+  return __ldcs(static_cast<const double2*>(base) + i);
+}
+__device__ __forceinline__ double2 ld_cplx_cg(const void* base, int64_t i, int f32) {
+  if (f32) {
+    const float2 v = __ldcg(static_cast<const float2*>(base) + i);
+    return make_double2((double)v.x, (double)v.y);
+  }
+  return __ldcg(static_cast<const double2*>(base) + i);
+}
+__device__ __forceinline__ void st_cplx(double2* base, int64_t i, double2 v, int f32) {
+  if (f32) reinterpret_cast<float2*>(base)[i] = make_float2((float)v.x, (float)v.y);
+  else base[i] = v;
+}
+
 // ---- radix-R butterflies on register arrays: x <- DFT_R(x), forward sign, natural output order -------------------
 template <int R>
 __device__ __forceinline__ void bfly(double2 (&x)[R]);
@@ -369,25 +393,25 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
       double2 xl[B1], xh[B1];
       if (MODE == 2) {
         const bool live = col < ncol;
-        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0);
+        const int64_t src = hi * P.in_hi + lo0 + (live ? col : 0);
 #pragma unroll
         for (int q2 = 0; q2 < B1; ++q2) {
           const int r = jp + q2 * Lq1;
           // L2-only loads with the normal retention: a tile uses TB * 16 bytes of every 128-byte line and the rest of
           // the line is wanted by the next tiles of the run (streaming loads mark the line evict-first: 3.8x re-reads)
-          xl[q2] = live ? __ldcg(src + (int64_t)r * P.in_el) : make_double2(0.0, 0.0);
-          xh[q2] = live ? __ldcg(src + (int64_t)(r + N / 4) * P.in_el) : make_double2(0.0, 0.0);
+          xl[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)r * P.in_el, P.f32) : make_double2(0.0, 0.0);
+          xh[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)(r + N / 4) * P.in_el, P.f32) : make_double2(0.0, 0.0);
         }
       } else if (MODE == 1) {
         const bool live = col < ncol;
-        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + (live ? col : 0)) * P.in_lo;
+        const int64_t src = hi * P.in_hi + (lo0 + (live ? col : 0)) * P.in_lo;
         const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + (live ? col : 0)] : 1.0;
 #pragma unroll
         for (int q2 = 0; q2 < B1; ++q2) {
           const int r = jp + q2 * Lq1;
           const double fl = P.dec_axis ? f0 * P.dec_axis[r] : 1.0, fh = P.dec_axis ? f0 * P.dec_axis[r + N / 4] : 1.0;
-          const double2 l = live ? __ldcs(src + r) : make_double2(0.0, 0.0);
-          const double2 h = live ? __ldcs(src + r + N / 4) : make_double2(0.0, 0.0);
+          const double2 l = live ? ld_cplx_cs(in_raw, src + r, P.f32) : make_double2(0.0, 0.0);
+          const double2 h = live ? ld_cplx_cs(in_raw, src + r + N / 4, P.f32) : make_double2(0.0, 0.0);
           xl[q2] = make_double2(l.x * fl, l.y * fl);
           xh[q2] = make_double2(h.x * fh, h.y * fh);
           nz |= (l.x != 0.0) | (l.y != 0.0) | (h.x != 0.0) | (h.y != 0.0);
@@ -395,18 +419,18 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
       } else {
         const bool live = col < ncol, two = 2 * col + 1 < nrow;
         const int64_t r0 = lo0 + 2 * (live ? col : 0);
-        const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
-        const double* src1 = src0 + (two ? P.in_lo : 0);
+        const int64_t src0 = hi * P.in_hi + r0 * P.in_lo;
+        const int64_t src1 = src0 + (two ? P.in_lo : 0);
         const double f0 = live ? (P.dec_axis ? fhi * P.dec_lo[r0] : 1.0) : 0.0;
         const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
         double la[B1], lb[B1], ha[B1], hb[B1], fl[B1], fh[B1];
 #pragma unroll
         for (int q2 = 0; q2 < B1; ++q2) {
           const int r = jp + q2 * Lq1;
-          la[q2] = __ldcs(src0 + r);
-          lb[q2] = __ldcs(src1 + r);
-          ha[q2] = __ldcs(src0 + r + N / 4);
-          hb[q2] = __ldcs(src1 + r + N / 4);
+          la[q2] = ld_real(in_raw, src0 + r, P.f32);
+          lb[q2] = ld_real(in_raw, src1 + r, P.f32);
+          ha[q2] = ld_real(in_raw, src0 + r + N / 4, P.f32);
+          hb[q2] = ld_real(in_raw, src1 + r + N / 4, P.f32);
           fl[q2] = P.dec_axis ? P.dec_axis[r] : 1.0;
           fh[q2] = P.dec_axis ? P.dec_axis[r + N / 4] : 1.0;
         }
@@ -437,8 +461,8 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
     const bool all_zero = __syncthreads_or(nz) == 0;
     if (!STRIDED && all_zero) {
       for (int row = 0; row < nrow; ++row) {
-        double2* o = out + hi * P.out_hi + (lo0 + row) * P.out_lo;
-        for (int mm = tid; mm < P.nout; mm += T) o[mm] = make_double2(0.0, 0.0);
+        const int64_t o = hi * P.out_hi + (lo0 + row) * P.out_lo;
+        for (int mm = tid; mm < P.nout; mm += T) st_cplx(out, o + mm, make_double2(0.0, 0.0), P.f32);
       }
       continue;   // (the next tile's group 1 writes shared memory nobody reads any more: every thread is past the barrier)
     }
@@ -479,7 +503,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
       if (STRIDED) {
         const int mm0 = s_mm[2 * col], mm1 = s_mm[2 * col + 1];
         if (mm1 > mm0) {
-          double2* o = out + hi * P.out_hi + lo0 + col;
+          const int64_t o = hi * P.out_hi + lo0 + col;
           const int mm = __ldg(&P.klow[b]) - P.lo;   // output index of frequency klow[b]; the band may wrap around N
 #pragma unroll
           for (int p2 = 0; p2 < B3; ++p2)
@@ -487,7 +511,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
             for (int p1 = 0; p1 < A3; ++p1) {
               int m = mm + (N / G3) * (p1 + A3 * p2);
               m = m < 0 ? m + N : (m >= N ? m - N : m);
-              if (m >= mm0 && m < mm1) o[(int64_t)m * P.out_el] = v[p1][p2];   // (partial lines: they meet in the L2)
+              if (m >= mm0 && m < mm1) st_cplx(out, o + (int64_t)m * P.out_el, v[p1][p2], P.f32);   // (partial lines meet in the L2)
             }
         }
       } else {
@@ -502,7 +526,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 
     // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table
     for (int col = 0; col < ncol; ++col) {
-      double2* o0 = out + hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
+      const int64_t o0 = hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
       const bool two = 2 * col + 1 < nrow;
       for (int mm = tid; mm < P.nout; mm += T) {
         int m = P.lo + mm;
@@ -510,10 +534,10 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
         const double2 z = a[at(__ldg(&P.rev[m]), col)];
         if (MODE == 0) {
           const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
-          __stcs(&o0[mm], make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)));
-          if (two) __stcs(&o0[P.out_lo + mm], make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)));
+          st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), P.f32);
+          if (two) st_cplx(out, o0 + P.out_lo + mm, make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)), P.f32);
         } else {
-          __stcs(&o0[mm], z);
+          st_cplx(out, o0 + mm, z, P.f32);
         }
       }
     }
@@ -593,8 +617,8 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
       if (REAL_IN) {
         const int64_t r0 = lo0 + 2 * col;
         const bool two = 2 * col + 1 < nrow;
-        const double* src0 = static_cast<const double*>(in_raw) + hi * P.in_hi + r0 * P.in_lo;
-        const double* src1 = src0 + (two ? P.in_lo : 0);
+        const int64_t src0 = hi * P.in_hi + r0 * P.in_lo;
+        const int64_t src1 = src0 + (two ? P.in_lo : 0);
         const double f0 = P.dec_axis ? fhi * P.dec_lo[r0] : 1.0;
         const double f1 = two ? (P.dec_axis ? fhi * P.dec_lo[r0 + 1] : 1.0) : 0.0;
         for (int i0 = lane + 32 * seg; i0 < P.n_in; i0 += 4 * lstep) {
@@ -603,8 +627,8 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
           for (int u = 0; u < 4; ++u) {
             const int i = i0 + lstep * u;
             const bool ok = i < P.n_in;
-            va[u] = ok ? src0[i] : 0.0;
-            vb[u] = ok ? src1[i] : 0.0;
+            va[u] = ok ? ld_real(in_raw, src0 + i, P.f32) : 0.0;
+            vb[u] = ok ? ld_real(in_raw, src1 + i, P.f32) : 0.0;
             fa[u] = (ok && P.dec_axis) ? P.dec_axis[i] : 1.0;
           }
 #pragma unroll
@@ -618,7 +642,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
           }
         }
       } else {
-        const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + (lo0 + col) * P.in_lo;
+        const int64_t src = hi * P.in_hi + (lo0 + col) * P.in_lo;
         const double f0 = P.dec_axis ? fhi * P.dec_lo[lo0 + col] : 1.0;
         for (int i0 = lane + 32 * seg; i0 < P.n_in; i0 += 4 * lstep) {
           double2 v[4];
@@ -627,7 +651,7 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
           for (int u = 0; u < 4; ++u) {
             const int i = i0 + lstep * u;
             const bool ok = i < P.n_in;
-            v[u] = ok ? src[i] : make_double2(0.0, 0.0);
+            v[u] = ok ? ld_cplx_cs(in_raw, src + i, P.f32) : make_double2(0.0, 0.0);
             fa[u] = (ok && P.dec_axis) ? P.dec_axis[i] * f0 : 1.0;
           }
 #pragma unroll
@@ -649,9 +673,16 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
     // 16-byte asynchronous copies (LDGSTS) straight into the padded rows: every thread issues all of its elements
     // back to back and waits once -- the pass is bound by memory latency, so what counts is bytes in flight
     const bool live = col < ncol;
+    if (P.f32) {   // single-precision input: converted on the way in (no asynchronous copy can do that)
+      const int64_t src32 = hi * P.in_hi + lo0 + (live ? col : 0);
+      for (int i = ty; i < P.n_in; i += nty) {
+        const int l = i - half_in;
+        a[(l < 0 ? l + N : l) * tbp + col] = live ? ld_cplx_cg(in_raw, src32 + (int64_t)i * P.in_el, 1) : make_double2(0.0, 0.0);
+      }
+    }
     const double2* src = static_cast<const double2*>(in_raw) + hi * P.in_hi + lo0 + (live ? col : 0) + (int64_t)ty * P.in_el;
     const int64_t step = (int64_t)nty * P.in_el;
-    for (int i = ty; i < P.n_in; i += nty) {
+    for (int i = ty; i < (P.f32 ? 0 : P.n_in); i += nty) {
       const int l = i - half_in;
       const unsigned dst = (unsigned)__cvta_generic_to_shared(a + (l < 0 ? l + N : l) * tbp + col);
       const int nbytes = live ? 16 : 0;   // src-size 0: zero-fill (columns beyond the edge of the array)
@@ -706,21 +737,21 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
     for (int col = nw >= tb ? wrp % tb : wrp; col < ncol && seg < nseg; col += cstep) {
       if (REAL_IN) {
         const bool two = 2 * col + 1 < nrow;
-        double2* o0 = out + hi * P.out_hi + (lo0 + 2 * col) * P.out_lo;
-        double2* o1 = o0 + P.out_lo;
+        const int64_t o0 = hi * P.out_hi + (lo0 + 2 * col) * P.out_lo;
+        const int64_t o1 = o0 + P.out_lo;
         for (int mm = lane + 32 * seg; mm < P.nout; mm += lstep) {
           int m = P.lo + mm;
           m = m < 0 ? m + N : (m >= N ? m - N : m);
           const double2 z = a[P.rev[m] * tbp + col], zc = a[P.rev[m == 0 ? 0 : N - m] * tbp + col];
-          o0[mm] = make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y));
-          if (two) o1[mm] = make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x));
+          st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), P.f32);
+          if (two) st_cplx(out, o1 + mm, make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)), P.f32);
         }
       } else {
-        double2* o0 = out + hi * P.out_hi + (lo0 + col) * P.out_lo;
+        const int64_t o0 = hi * P.out_hi + (lo0 + col) * P.out_lo;
         for (int mm = lane + 32 * seg; mm < P.nout; mm += lstep) {
           int m = P.lo + mm;
           m = m < 0 ? m + N : (m >= N ? m - N : m);
-          o0[mm] = a[P.rev[m] * tbp + col];
+          st_cplx(out, o0 + mm, a[P.rev[m] * tbp + col], P.f32);
         }
       }
     }
@@ -739,12 +770,12 @@ fft_pass_kernel(FftPass P, const void* __restrict__ in_raw, double2* __restrict_
         }
       }
       const int first = mm0 + ((ty - mm0) % nty + nty) % nty;   // smallest mm >= mm0 congruent to ty modulo nty
-      double2* o = out + hi * P.out_hi + lo0 + col + (int64_t)first * P.out_el;
+      int64_t o = hi * P.out_hi + lo0 + col + (int64_t)first * P.out_el;
       const int64_t step = (int64_t)nty * P.out_el;
       for (int mm = first; mm < mm1; mm += nty) {
         int m = P.lo + mm;
         m = m < 0 ? m + N : (m >= N ? m - N : m);
-        *o = a[P.rev[m] * tbp + col];
+        st_cplx(out, o, a[P.rev[m] * tbp + col], P.f32);
         o += step;
       }
     }

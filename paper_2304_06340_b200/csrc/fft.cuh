@@ -30,6 +30,7 @@ struct FftPass {
   int64_t n_hi, n_lo;
   int64_t in_hi, in_lo, in_el, out_hi, out_lo, out_el;
   int contig, real_in;
+  int f32;   // 1: input and output arrays are single precision (float / float2); arithmetic and shared memory stay fp64
   const double *dec_axis, *dec_hi, *dec_lo;
   // ball != 0 (strided passes): the consumer reads the output only inside an ellipsoid (the targets of the ball rule).
   // With q = ((a - ball_ca) ball_ira)^2 + ((b - ball_cb) ball_irb)^2 of a column -- ball == 1: lo = a * ball_nb + b (both

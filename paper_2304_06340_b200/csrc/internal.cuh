@@ -85,6 +85,8 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
            double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred = false,
            const ExtentHint* hint = nullptr);
 int nufft3_release_cache();
+// api.cu: the calling thread's grid precision (sfd_set_grid_precision): true = single-precision grids
+bool grid_f32();
 // Type-1 NUFFT onto the lattice xi = 2 pi h m, m in [-M/2, M/2]^3 (eq. 3.6, eq. 3.7), lattice order of
 // lattice_expand.  *applicable = false (and nothing enqueued): the lattice is too coarse for the sources' extent or
 // too long for the in-shared-memory FFT; the caller then runs the type-3 transform on the lattice nodes.
@@ -95,7 +97,8 @@ int nufft1_lattice_sizes(int64_t J, int M, double h, const double X[3], double e
 // v[M+1][M+1][M/2+1] (modes m0, m1, m2 >= 0, before deconvolution), the per-axis tables 1 / ((w/2) phihat) on |m| and the
 // centre C of the sources -- for a consumer that folds deconvolution and phase into its own pass (reduce.cu).
 struct Nufft1Band {
-  const double* v = nullptr;     // complex128, inside the workspace
+  const double* v = nullptr;     // complex128 (complex64 when f32), inside the workspace
+  int f32 = 0;
   const double* dec = nullptr;   // [3][M/2+1]
   double C[3] = {0.0, 0.0, 0.0};
 };

@@ -17,6 +17,8 @@
 //   * the 3w kernel values of a target are piecewise polynomials (nufft3.cuh footprint()) whose coefficients live
 //     in registers: lane i (mod 16) owns interval i, lanes 0-15 evaluate x then z, lanes 16-31 evaluate y;
 //   * w is a template parameter: plane loop, cell map and polynomial degree are compile-time.
+#include <type_traits>
+
 #include "nufft3.cuh"
 
 namespace sfd {
@@ -46,9 +48,20 @@ constexpr int bin_z(int w) {
   return l16 > l8 ? 16 : 8;
 }
 
-template <int W>
+// Single-precision subgrid (N3Params::f32): 8-byte cells, so the same shared memory holds a bin of twice the cells;
+// z extent 16, i.e. the row pitch is congruent to w modulo 16 and the 16 lanes of an LDS.64 phase hit 16 distinct 8-byte
+// bank groups.  The plane loop accumulates in fp32 (w terms per accumulator), everything after it is fp64.
+constexpr int kSmemCells32 = 2 * kSmemCells;
+constexpr int bin_xy32(int w) {
+  int m = 1;
+  while ((m + 1) * (m + 1) * (16 + w) <= kSmemCells32) ++m;
+  return m - w;
+}
+constexpr int kMaxW32 = 8;   // eps >= 1e-6 (w <= 7, one more for a handful of sources)
+
+template <int W, bool F32>
 __global__ void __launch_bounds__(32 * kWarps, 1)
-interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __restrict__ v, const TgtRec* __restrict__ tgt,
+interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restrict__ v_raw, const TgtRec* __restrict__ tgt,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
               const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
               int32_t* __restrict__ counter, double2* __restrict__ G) {
@@ -56,12 +69,15 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
   constexpr int NCL = (W * W + 31) / 32;
   constexpr int TPW = tpw_for(W);
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  using CT = std::conditional_t<F32, float2, double2>;   // a cell of the subgrid (and of the band in global memory)
+  using AT = std::conditional_t<F32, float, double>;     // the plane loop's accumulators
+  const CT* __restrict__ v = static_cast<const CT*>(v_raw);
   double (*ktab)[kMaxTpw][3][16] = reinterpret_cast<double (*)[kMaxTpw][3][16]>(smem_raw);
-  double2* sub = reinterpret_cast<double2*>(smem_raw + kTabBytes);
+  CT* sub = reinterpret_cast<CT*>(smem_raw + kTabBytes);
   __shared__ int s_item;
 
   const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, li = lane & 15;
-  constexpr int BZ = bin_z(W), BXY = bin_xy(W, BZ);
+  constexpr int BZ = F32 ? 16 : bin_z(W), BXY = F32 ? bin_xy32(W) : bin_xy(W, BZ);
   constexpr int Px = BXY + W, Py = BXY + W, Pz = BZ + W;
   constexpr int plane = Py * Pz;
 
@@ -117,10 +133,13 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
         }
         const int gx = mx - p.lo[0], gy = my - p.lo[1], gz = mz - p.lo[2];
         const bool inside = gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nout[0] && gy < p.nout[1] && gz < p.nout[2];
-        const double2* srcp = inside ? v + (((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz) : v;
+        const CT* srcp = inside ? v + (((size_t)gx * p.nout[1] + gy) * p.nout[2] + gz) : v;
         const unsigned dst = (unsigned)__cvta_generic_to_shared(sub + row * Pz + lane);
-        const int nbytes = inside ? 16 : 0;   // src-size 0: the 16 destination bytes are zero-filled
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(srcp), "r"(nbytes) : "memory");
+        const int nbytes = inside ? (int)sizeof(CT) : 0;   // src-size 0: the destination bytes are zero-filled
+        if (F32)
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(srcp), "r"(nbytes) : "memory");
+        else
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(srcp), "r"(nbytes) : "memory");
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -172,14 +191,14 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
       }
       __syncwarp();
 
-      double are[TPW][NCL], aim[TPW][NCL];
-      const double2* cell[TPW][NCL];   // the lane's cells in plane 0 of the footprint; plane a is an immediate offset
+      AT are[TPW][NCL], aim[TPW][NCL];
+      const CT* cell[TPW][NCL];   // the lane's cells in plane 0 of the footprint; plane a is an immediate offset
 #pragma unroll
       for (int u = 0; u < TPW; ++u) {
-        const double2* base = sub + ((i0x[u] - ox) * Py + (i0y[u] - oy)) * Pz + (i0z[u] - oz);
+        const CT* base = sub + ((i0x[u] - ox) * Py + (i0y[u] - oy)) * Pz + (i0z[u] - oz);
 #pragma unroll
         for (int i = 0; i < NCL; ++i) {
-          are[u][i] = aim[u][i] = 0.0;
+          are[u][i] = aim[u][i] = (AT)0;
           cell[u][i] = base + off[i];
         }
       }
@@ -187,15 +206,15 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
       for (int a = 0; a < W; ++a) {
 #pragma unroll
         for (int u = 0; u < TPW; ++u) {
-          const double kx = ktab[wq][u][0][a];
+          const AT kx = (AT)ktab[wq][u][0][a];
 #pragma unroll
           for (int i = 0; i < NCL; ++i) {
             // the last round of a plane covers only W*W - 32 (NCL-1) cells: lanes beyond them issue no load (a load
             // of a dummy cell would still cost its shared-memory wavefronts: 2 of 9 per plane at W = 7)
-            double2 c = make_double2(0.0, 0.0);
+            CT c{};
             if (i + 1 < NCL || on[i]) c = cell[u][i][a * plane];
-            are[u][i] = __fma_rn(c.x, kx, are[u][i]);
-            aim[u][i] = __fma_rn(c.y, kx, aim[u][i]);
+            are[u][i] = fma(c.x, kx, are[u][i]);
+            aim[u][i] = fma(c.y, kx, aim[u][i]);
           }
         }
       }
@@ -206,9 +225,9 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
 #pragma unroll
         for (int i = 0; i < NCL; ++i) {
           const double kyz = on[i] ? ktab[wq][u][1][cy[i]] * ktab[wq][u][2][cz[i]] : 0.0;
-          re[u] = __fma_rn(are[u][i], kyz, re[u]);
+          re[u] = __fma_rn((double)are[u][i], kyz, re[u]);
           // cells below the centre plane hold the mirror cell un-conjugated: flip the sign of their imaginary part
-          im[u] = __fma_rn(aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
+          im[u] = __fma_rn((double)aim[u][i], (p.zh && i0z[u] + cz[i] < czc) ? -kyz : kyz, im[u]);
         }
       }
       if (TPW == 2) {
@@ -237,15 +256,15 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const double2* __rest
   }
 }
 
-template <int W>
+template <int W, bool F32>
 int launch(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_G, size_t smem, cudaStream_t st) {
   static thread_local int attr_dev = -1;
   if (first_use_on_device(attr_dev)) {
-    SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
+    SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel<W, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
   }
-  interp_kernel<W><<<num_sms(), 32 * kWarps, smem, st>>>(p, d_ptab, reinterpret_cast<const double2*>(d_v), d_tgt,
+  interp_kernel<W, F32><<<num_sms(), 32 * kWarps, smem, st>>>(p, d_ptab, d_v, d_tgt,
                                                         d_item_bin, d_item_start, d_item_count, d_n_items, d_counter,
                                                         reinterpret_cast<double2*>(d_G));
   return launch_check("interp_kernel");
@@ -253,13 +272,18 @@ int launch(const N3Params& p, const double* d_ptab, const double* d_v, const Tgt
 
 }  // namespace
 
-void interp_bins(int w, int bt[3]) {
+void interp_bins(int w, bool f32, int bt[3]) {
+  if (f32 && w <= kMaxW32) {
+    bt[2] = 16;
+    bt[0] = bt[1] = bin_xy32(w);
+    return;
+  }
   bt[2] = bin_z(w);
   bt[0] = bt[1] = bin_xy(w, bt[2]);
 }
 
 size_t interp_smem_bytes(const N3Params& p) {
-  return kTabBytes + (size_t)(p.bt[0] + p.w) * (p.bt[1] + p.w) * (p.bt[2] + p.w) * 16;
+  return kTabBytes + (size_t)(p.bt[0] + p.w) * (p.bt[1] + p.w) * (p.bt[2] + p.w) * (p.f32 ? 8 : 16);
 }
 
 int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
@@ -269,8 +293,19 @@ int interp(const N3Params& p, const double* d_ptab, const double* d_v, const Tgt
   SFD_REQUIRE(smem <= 227 * 1024 - 1024 && p.bt[2] + p.w <= 32, SFD_ERR_INVALID_ARG,
               "interp subgrid does not fit shared memory (%zu B)", smem);
   SFD_CUDA_TRY(cudaMemsetAsync(d_counter, 0, sizeof(int32_t), st));
+  if (p.f32) {
+#define SFD_INTERP_CASE32(W_) \
+  case W_: return launch<W_, true>(p, d_ptab, d_v, d_tgt, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_G, smem, st);
+    switch (p.w) {
+      SFD_INTERP_CASE32(2) SFD_INTERP_CASE32(3) SFD_INTERP_CASE32(4) SFD_INTERP_CASE32(5) SFD_INTERP_CASE32(6)
+      SFD_INTERP_CASE32(7) SFD_INTERP_CASE32(8)
+    }
+#undef SFD_INTERP_CASE32
+    set_error("interp: single-precision grids support kernel widths up to %d (eps >= 1e-6), got %d", kMaxW32, p.w);
+    return SFD_ERR_UNSUPPORTED;
+  }
 #define SFD_INTERP_CASE(W_) \
-  case W_: return launch<W_>(p, d_ptab, d_v, d_tgt, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_G, smem, st);
+  case W_: return launch<W_, false>(p, d_ptab, d_v, d_tgt, d_item_bin, d_item_start, d_item_count, d_n_items, d_counter, d_G, smem, st);
   switch (p.w) {
     SFD_INTERP_CASE(2) SFD_INTERP_CASE(3) SFD_INTERP_CASE(4) SFD_INTERP_CASE(5) SFD_INTERP_CASE(6)
     SFD_INTERP_CASE(7) SFD_INTERP_CASE(8) SFD_INTERP_CASE(9) SFD_INTERP_CASE(10) SFD_INTERP_CASE(11)

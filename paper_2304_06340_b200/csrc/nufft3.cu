@@ -80,12 +80,14 @@ struct Layout {
 // Geometry from half-widths X (sources) and S (targets); centres are filled in by the caller.
 constexpr int64_t kFewSources = 64;
 
-int make_params(const double X_in[3], const double S_in[3], double eps, bool real_c, int64_t J, N3Params* p) {
+int make_params(const double X_in[3], const double S_in[3], double eps, bool real_c, int64_t J, N3Params* p,
+                bool f32 = false) {
   bool careful = J < kFewSources;
   for (int d = 0; d < 3; ++d)
     if (X_in[d] * (S_in[d] < 1e-150 ? 1.0 : S_in[d]) < 1.0) careful = true;
   kernel_params(eps, careful, &p->w, &p->beta);
   p->real_c = real_c ? 1 : 0;
+  p->f32 = f32 ? 1 : 0;
   for (int d = 0; d < 3; ++d) {
     double X = X_in[d], S = S_in[d];
     SFD_REQUIRE(std::isfinite(X) && std::isfinite(S) && X >= 0 && S >= 0, SFD_ERR_INVALID_ARG,
@@ -103,7 +105,7 @@ int make_params(const double X_in[3], const double S_in[3], double eps, bool rea
   }
   p->deg = p->w + 3;
   spread_bins(p->w, real_c, p->bs);
-  interp_bins(p->w, p->bt);
+  interp_bins(p->w, f32, p->bt);
   for (int d = 0; d < 3; ++d) {
     p->nbs[d] = (p->nf[d] + p->bs[d] - 1) / p->bs[d];
     p->t0[d] = p->n2[d] / 4;                      // targets occupy u2 in [n2/4, 3 n2/4]
@@ -168,12 +170,13 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2] + p.nout[0] + p.nout[1] + p.nout[2]) * 8);
   L->scan = put(scan_workspace(std::max(L->ns_keys, L->nt_bins) + 1));
   L->ffttab = put(fft_tables_bytes(p.n2));
-  L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? 8 : 16);
+  const size_t cb = p.f32 ? 8 : 16;   // bytes of a complex cell of the grids
+  L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? cb / 2 : cb);
   L->fine = put(L->fine_bytes);
   // FFT passes: fine -> X [nf0][nf1][nout2] -> Y [nf0][nout1][nout2] -> X [nout0][nout1][nout2]
   const size_t xa = (size_t)p.nf[0] * p.nf[1] * p.nout[2], xc = (size_t)p.nout[0] * p.nout[1] * p.nout[2];
-  L->bufx = put(std::max(xa, xc) * 16);
-  L->bufy = put((size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16);
+  L->bufx = put(std::max(xa, xc) * cb);
+  L->bufy = put((size_t)p.nf[0] * p.nout[1] * p.nout[2] * cb);
   L->total = o;
   return SFD_OK;
 }
@@ -395,7 +398,10 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
       real_c = false;
     }
   }
-  SFD_TRY(make_params(X, S, eps, real_c, J, &p));
+  const bool f32 = grid_f32();
+  SFD_REQUIRE(!f32 || eps >= 1e-6, SFD_ERR_INVALID_ARG,
+              "single-precision grids (sfd_set_grid_precision(32)) carry tolerances eps >= 1e-6 only, got %g", eps);
+  SFD_TRY(make_params(X, S, eps, real_c, J, &p, f32));
   choose_sort(&p, J);
   Layout L;
   SFD_TRY(make_layout(p, J, K, &L));
@@ -456,14 +462,14 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     A.n_hi = nf0; A.n_lo = nf1;
     A.in_hi = nf1 * nf2; A.in_lo = nf2; A.in_el = 1;
     A.out_hi = nf1 * no2; A.out_lo = no2; A.out_el = 1;
-    A.contig = 1; A.real_in = p.real_c;
+    A.contig = 1; A.real_in = p.real_c; A.f32 = p.f32;
     A.dec_axis = dec + p.nf[0] + p.nf[1]; A.dec_hi = dec; A.dec_lo = dec + p.nf[0];
     SFD_TRY(fft_pass(A, ft, 2, fine, bufx, st));
     FftPass B{};   // axis 1: columns (i0, m2) of X -> Y[i0][m1][m2]
     B.N = p.n2[1]; B.n_in = p.nf[1]; B.lo = p.lo[1]; B.nout = p.nout[1];
     B.n_hi = nf0; B.n_lo = no2;
     B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
-    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2; B.f32 = p.f32;
     // Targets inside the ball |xi| <= R (the ball rule): in inner-grid cells they fill the ellipsoid E with semi-axes
     // a_d = n2_d / 4 about the centre (the axes differ when the mesh's bounding box is not a cube).  What the
     // interpolation reads is E (+) the footprint cube of half-width w/2 + 1 cells, inside E (+) Ball(r), r = sqrt 3 times
@@ -488,14 +494,14 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     // leave unstored and a later stage reads anyway shows up as a NaN distance (tests/test_gpu_fullsize.py)
     const char* poison_env = std::getenv("SFD_DEBUG_POISON_BAND");
     const bool poison = poison_env && poison_env[0] == '1';
-    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16, st));
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * (p.f32 ? 8 : 16), st));
     SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
     if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufx, 0xff, L.bufy - L.bufx, st));
     FftPass C{};   // axis 0: columns (m1, m2) of Y -> X[m0][m1][m2]
     C.N = p.n2[0]; C.n_in = p.nf[0]; C.lo = p.lo[0]; C.nout = p.nout[0];
     C.n_hi = 1; C.n_lo = no1 * no2;
     C.in_hi = 0; C.in_lo = 1; C.in_el = no1 * no2;
-    C.out_hi = 0; C.out_lo = 1; C.out_el = no1 * no2;
+    C.out_hi = 0; C.out_lo = 1; C.out_el = no1 * no2; C.f32 = p.f32;
     if (ball) {
       C.ball = 1;
       C.ball_nb = (int)no2;
@@ -546,9 +552,10 @@ namespace {
 // *ok = false: the lattice is too coarse for the extent of the sources (2 pi h X >= pi up to the kernel's
 // footprint: the periodic images would overlap) or the transform is too long for fft.cu -- use the type-3 path.
 int make_params_lattice(const double X_in[3], const double C[3], int M, double h, double eps, int64_t J, N3Params* p,
-                        bool* ok) {
+                        bool* ok, bool f32 = false) {
   kernel_params(eps, J < kFewSources, &p->w, &p->beta);
   p->real_c = 1;
+  p->f32 = f32 ? 1 : 0;
   p->zh = 1;
   p->deg = p->w + 3;
   *ok = false;
@@ -633,7 +640,11 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
     }
   }
   N3Params p{};
-  SFD_TRY(make_params_lattice(X, C, M, h, eps, J, &p, applicable));
+  const bool f32 = grid_f32();
+  SFD_REQUIRE(!f32 || eps >= 1e-7, SFD_ERR_INVALID_ARG,
+              "single-precision grids (sfd_set_grid_precision(32)) carry tolerances eps >= 1e-7 on the lattice (the paper's "
+              "setting, P:238) and >= 1e-6 otherwise, got %g", eps);
+  SFD_TRY(make_params_lattice(X, C, M, h, eps, J, &p, applicable, f32));
   if (!*applicable) return SFD_OK;
   choose_sort(&p, J);
   Layout L;
@@ -691,31 +702,32 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
     A.n_hi = nf0; A.n_lo = nf1;
     A.in_hi = nf1 * nf2; A.in_lo = nf2; A.in_el = 1;
     A.out_hi = nf1 * no2; A.out_lo = no2; A.out_el = 1;
-    A.contig = 1; A.real_in = 1;
+    A.contig = 1; A.real_in = 1; A.f32 = p.f32;
     SFD_TRY(fft_pass(A, ft, 2, fine, bufx, st));
     FftPass B{};
     B.N = p.n2[1]; B.n_in = p.nf[1]; B.lo = p.lo[1]; B.nout = p.nout[1];
     B.n_hi = nf0; B.n_lo = no2;
     B.in_hi = nf1 * no2; B.in_lo = 1; B.in_el = no2;
-    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2;
+    B.out_hi = no1 * no2; B.out_lo = 1; B.out_el = no2; B.f32 = p.f32;
     // SFD_DEBUG_POISON_BAND=1 (tests): fill each pass's output buffer with NaN first, so that any cell the pruned passes
     // leave unstored and a later stage reads anyway shows up as a NaN distance (tests/test_gpu_fullsize.py)
     const char* poison_env = std::getenv("SFD_DEBUG_POISON_BAND");
     const bool poison = poison_env && poison_env[0] == '1';
-    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * 16, st));
+    if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufy, 0xff, (size_t)p.nf[0] * p.nout[1] * p.nout[2] * (p.f32 ? 8 : 16), st));
     SFD_TRY(fft_pass(B, ft, 1, bufx, bufy, st));
     if (poison) SFD_CUDA_TRY(cudaMemsetAsync(bufx, 0xff, L.bufy - L.bufx, st));
     FftPass C3{};
     C3.N = p.n2[0]; C3.n_in = p.nf[0]; C3.lo = p.lo[0]; C3.nout = p.nout[0];
     C3.n_hi = 1; C3.n_lo = no1 * no2;
     C3.in_hi = 0; C3.in_lo = 1; C3.in_el = no1 * no2;
-    C3.out_hi = 0; C3.out_lo = 1; C3.out_el = no1 * no2;
+    C3.out_hi = 0; C3.out_lo = 1; C3.out_el = no1 * no2; C3.f32 = p.f32;
     SFD_TRY(fft_pass(C3, ft, 0, bufy, bufx, st));
   }
   prof_mark("fft", st);
 
   if (!d_nuhat && band) {   // the consumer deconvolves while it reduces
     band->v = bufx;
+    band->f32 = p.f32;
     band->dec = dec;
     for (int d = 0; d < 3; ++d) band->C[d] = p.C[d];
     return SFD_OK;

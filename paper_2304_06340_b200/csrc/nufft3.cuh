@@ -29,6 +29,8 @@ struct N3Params {
                              // and the spreader accumulates them in registers (many sources per cell: P:236)
                              // 2: so many per cell that one warp spreads a whole run (spread.cu spread_runs_kernel)
   int lo[3], nout[3];        // band of the inner grid that is computed and stored: v[m - lo], m in [lo, lo + nout)
+  int f32;                   // 1: the grids in global memory (fine grid, FFT intermediates, band) and the interpolation's
+                             // subgrid are single precision (S:8(f) NEXT-4); everything else stays fp64
   int zh;                    // 1: real strengths => v is Hermitian about the centre m = n2/2 (v[c+k] = conj v[c-k]) and
                              // only the half m_2 >= n2_2/2 of the band is computed and stored (lo[2] = n2_2/2); the
                              // interpolation reads the other half by reflection (all three indices) and conjugation
@@ -83,7 +85,8 @@ __device__ __forceinline__ void footprint(double u, int w, int& i0, double& s) {
 
 // ---- spread.cu (A5-4) ------------------------------------------------------------------------------------
 // Work item i: sources [item_start[i], item_start[i]+item_count[i]) of bin item_bin[i].  *n_items on the device.
-// grid is real double[nf0][nf1][nf2] (real_c) or complex double[nf0][nf1][nf2][2]; must be zero on entry.
+// grid is real double[nf0][nf1][nf2] (real_c) or complex double[nf0][nf1][nf2][2] -- float instead of double when
+// p.f32 --; must be zero on entry.
 void spread_bins(int w, bool real_c, int bs[3]);   // source-bin shape for kernel width w
 size_t spread_smem_bytes(const N3Params& p);
 int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin, const int32_t* d_item_start,
@@ -101,7 +104,7 @@ int spread_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, co
 // v = complex double[nout_0][nout_1][nout_2][2], the band [lo, lo+nout) of the inner grid; writes G[k] (complex) for
 // every sorted target.
 size_t interp_smem_bytes(const N3Params& p);
-void interp_bins(int w, int bt[3]);   // target-bin shape for kernel width w
+void interp_bins(int w, bool f32, int bt[3]);   // target-bin shape for kernel width w (fp32 subgrids hold twice the cells)
 int interp(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
            double* d_G, cudaStream_t st);

@@ -300,7 +300,14 @@ __global__ void __launch_bounds__(kT) lattice_post_kernel(N3Params p, int M, dou
   const int m0 = a - M / 2, m1 = b - M / 2, m2 = c - M / 2;
   const bool refl = m2 < 0;
   const int ia = refl ? M - a : a, ib = refl ? M - b : b, ic = refl ? -m2 : m2;
-  double2 g = v[((int64_t)ia * n + ib) * nh + ic];
+  const int64_t cell = ((int64_t)ia * n + ib) * nh + ic;
+  double2 g;
+  if (p.f32) {   // single-precision band
+    const float2 gf = reinterpret_cast<const float2*>(v)[cell];
+    g = make_double2((double)gf.x, (double)gf.y);
+  } else {
+    g = v[cell];
+  }
   if (refl) g.y = -g.y;
   const double f = dec[abs(m0)] * dec[nh + abs(m1)] * dec[2 * nh + ic];
   g.x *= f;

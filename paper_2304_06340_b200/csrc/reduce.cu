@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(kThreads) reduce_terms_kernel(const double2* _
 // and the same radius and weight, hence the same term: modes with m2 > 0 count twice.
 __global__ void __launch_bounds__(kThreads) lattice_band_terms_kernel(const double2* __restrict__ v, const double* __restrict__ dec,
                                                                      double c0, double c1, double c2, int M, double h,
-                                                                     double s, int s_kind, double scale2,
+                                                                     double s, int s_kind, double scale2, int f32,
                                                                      Comp* __restrict__ partial) {
   const int n = M + 1, nh = M / 2 + 1;
   const int64_t Kh = (int64_t)n * n * nh;
@@ -155,7 +155,13 @@ __global__ void __launch_bounds__(kThreads) lattice_band_terms_kernel(const doub
     if (m1 == -M / 2 || m1 == M / 2) wk = __dmul_rn(wk, 0.5);
     if (m2 == M / 2) wk = __dmul_rn(wk, 0.5);
     if (m2 > 0) wk = __dmul_rn(wk, 2.0);
-    double2 g = v[k];
+    double2 g;
+    if (f32) {   // single-precision band (N3Params::f32)
+      const float2 gf = reinterpret_cast<const float2*>(v)[k];
+      g = make_double2((double)gf.x, (double)gf.y);
+    } else {
+      g = v[k];
+    }
     const double f = dec[abs(m0)] * dec[nh + abs(m1)] * dec[2 * nh + m2];
     g.x *= f;
     g.y *= f;
@@ -261,7 +267,7 @@ int reduce_lattice_band_enqueue(const Nufft1Band& band, int M, double xi_max, do
   const int s_kind = (s == std::floor(s) && s >= 1.0 && s <= 64.0) ? (int)s : 0;
   lattice_band_terms_kernel<<<blocks, kThreads, 0, st>>>(reinterpret_cast<const double2*>(band.v), band.dec, band.C[0],
                                                          band.C[1], band.C[2], M, 2.0 * xi_max / M, s, s_kind,
-                                                         scale * scale, partial);
+                                                         scale * scale, band.f32, partial);
   SFD_TRY(launch_check("lattice_band_terms_kernel"));
   reduce_final_kernel<<<1, kThreads, 0, st>>>(partial, blocks, pref, result, device_flags());
   return launch_check("reduce_final_kernel");

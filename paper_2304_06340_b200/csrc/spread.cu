@@ -214,13 +214,23 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
       const int gx = ox + ix, gy = oy + iy, gz = oz + lane;
       if (lane < Pz && gx >= 0 && gy >= 0 && gz >= 0 && gx < p.nf[0] && gy < p.nf[1] && gz < p.nf[2]) {
         const size_t g = ((size_t)gx * p.nf[1] + gy) * p.nf[2] + gz;
+        // (p.f32: the global grid is single precision -- the subgrid sum, accumulated in fp64, is rounded once per bin)
+        float* gridf = reinterpret_cast<float*>(grid);
         if (REAL) {
           const double v = sub[row * Pz + lane];
-          if (v != 0.0) atomicAdd(&grid[g], v);
+          if (v != 0.0) {
+            if (p.f32) atomicAdd(&gridf[g], (float)v);
+            else atomicAdd(&grid[g], v);
+          }
         } else {
           const double2 v = reinterpret_cast<double2*>(sub)[row * Pz + lane];
-          if (v.x != 0.0) atomicAdd(&grid[2 * g], v.x);
-          if (v.y != 0.0) atomicAdd(&grid[2 * g + 1], v.y);
+          if (p.f32) {
+            if (v.x != 0.0) atomicAdd(&gridf[2 * g], (float)v.x);
+            if (v.y != 0.0) atomicAdd(&gridf[2 * g + 1], (float)v.y);
+          } else {
+            if (v.x != 0.0) atomicAdd(&grid[2 * g], v.x);
+            if (v.y != 0.0) atomicAdd(&grid[2 * g + 1], v.y);
+          }
         }
       }
     }
@@ -361,7 +371,8 @@ spread_runs_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __
       for (int i = 0; i < NCL; ++i) {
         if (on[i] && acc[a][i] != 0.0) {
           const size_t g = ((size_t)(i0x + a) * p.nf[1] + (i0y + cy[i])) * p.nf[2] + (i0z + cz[i]);
-          atomicAdd(&grid[g], acc[a][i]);
+          if (p.f32) atomicAdd(reinterpret_cast<float*>(grid) + g, (float)acc[a][i]);
+          else atomicAdd(&grid[g], acc[a][i]);
         }
       }
     }
