@@ -320,7 +320,7 @@ struct FixedTw {
 // of TB columns.  Shared memory: the twiddle tables, then N * TB complex128 of data, element (pos, col) at pos * TB + col
 // in the strided passes (lanes run over the tile's columns first, like the global accesses) and at col * N + pos in the
 // contiguous ones (lanes run along the axis).
-template <class PL, int MODE>
+template <class PL, int MODE, bool F32>
 __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid_constant__ FftPass P, const void* __restrict__ in_raw,
                                                                     double2* __restrict__ out, int64_t n_tiles, int RUN) {
   constexpr int N = PL::N, TB = PL::TB, T = PL::T;
@@ -399,8 +399,8 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
           const int r = jp + q2 * Lq1;
           // L2-only loads with the normal retention: a tile uses TB * 16 bytes of every 128-byte line and the rest of
           // the line is wanted by the next tiles of the run (streaming loads mark the line evict-first: 3.8x re-reads)
-          xl[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)r * P.in_el, P.f32) : make_double2(0.0, 0.0);
-          xh[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)(r + N / 4) * P.in_el, P.f32) : make_double2(0.0, 0.0);
+          xl[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)r * P.in_el, F32) : make_double2(0.0, 0.0);
+          xh[q2] = live ? ld_cplx_cg(in_raw, src + (int64_t)(r + N / 4) * P.in_el, F32) : make_double2(0.0, 0.0);
         }
       } else if (MODE == 1) {
         const bool live = col < ncol;
@@ -410,8 +410,8 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
         for (int q2 = 0; q2 < B1; ++q2) {
           const int r = jp + q2 * Lq1;
           const double fl = P.dec_axis ? f0 * P.dec_axis[r] : 1.0, fh = P.dec_axis ? f0 * P.dec_axis[r + N / 4] : 1.0;
-          const double2 l = live ? ld_cplx_cs(in_raw, src + r, P.f32) : make_double2(0.0, 0.0);
-          const double2 h = live ? ld_cplx_cs(in_raw, src + r + N / 4, P.f32) : make_double2(0.0, 0.0);
+          const double2 l = live ? ld_cplx_cs(in_raw, src + r, F32) : make_double2(0.0, 0.0);
+          const double2 h = live ? ld_cplx_cs(in_raw, src + r + N / 4, F32) : make_double2(0.0, 0.0);
           xl[q2] = make_double2(l.x * fl, l.y * fl);
           xh[q2] = make_double2(h.x * fh, h.y * fh);
           nz |= (l.x != 0.0) | (l.y != 0.0) | (h.x != 0.0) | (h.y != 0.0);
@@ -427,10 +427,10 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 #pragma unroll
         for (int q2 = 0; q2 < B1; ++q2) {
           const int r = jp + q2 * Lq1;
-          la[q2] = ld_real(in_raw, src0 + r, P.f32);
-          lb[q2] = ld_real(in_raw, src1 + r, P.f32);
-          ha[q2] = ld_real(in_raw, src0 + r + N / 4, P.f32);
-          hb[q2] = ld_real(in_raw, src1 + r + N / 4, P.f32);
+          la[q2] = ld_real(in_raw, src0 + r, F32);
+          lb[q2] = ld_real(in_raw, src1 + r, F32);
+          ha[q2] = ld_real(in_raw, src0 + r + N / 4, F32);
+          hb[q2] = ld_real(in_raw, src1 + r + N / 4, F32);
           fl[q2] = P.dec_axis ? P.dec_axis[r] : 1.0;
           fh[q2] = P.dec_axis ? P.dec_axis[r + N / 4] : 1.0;
         }
@@ -462,7 +462,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
     if (!STRIDED && all_zero) {
       for (int row = 0; row < nrow; ++row) {
         const int64_t o = hi * P.out_hi + (lo0 + row) * P.out_lo;
-        for (int mm = tid; mm < P.nout; mm += T) st_cplx(out, o + mm, make_double2(0.0, 0.0), P.f32);
+        for (int mm = tid; mm < P.nout; mm += T) st_cplx(out, o + mm, make_double2(0.0, 0.0), F32);
       }
       continue;   // (the next tile's group 1 writes shared memory nobody reads any more: every thread is past the barrier)
     }
@@ -511,7 +511,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
             for (int p1 = 0; p1 < A3; ++p1) {
               int m = mm + (N / G3) * (p1 + A3 * p2);
               m = m < 0 ? m + N : (m >= N ? m - N : m);
-              if (m >= mm0 && m < mm1) st_cplx(out, o + (int64_t)m * P.out_el, v[p1][p2], P.f32);   // (partial lines meet in the L2)
+              if (m >= mm0 && m < mm1) st_cplx(out, o + (int64_t)m * P.out_el, v[p1][p2], F32);   // (partial lines meet in the L2)
             }
         }
       } else {
@@ -534,10 +534,10 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
         const double2 z = a[at(__ldg(&P.rev[m]), col)];
         if (MODE == 0) {
           const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
-          st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), P.f32);
-          if (two) st_cplx(out, o0 + P.out_lo + mm, make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)), P.f32);
+          st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), F32);
+          if (two) st_cplx(out, o0 + P.out_lo + mm, make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)), F32);
         } else {
-          st_cplx(out, o0 + mm, z, P.f32);
+          st_cplx(out, o0 + mm, z, F32);
         }
       }
     }
@@ -980,9 +980,15 @@ int launch_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t
     kern<<<grid, PL::T, smem, st>>>(P, d_in, reinterpret_cast<double2*>(d_out), tiles, run);
     return SFD_OK;
   };
-  if (mode == 0) SFD_TRY(go(fft_fixed_kernel<PL, 0>));
-  else if (mode == 1) SFD_TRY(go(fft_fixed_kernel<PL, 1>));
-  else SFD_TRY(go(fft_fixed_kernel<PL, 2>));
+  if (P.f32) {   // single-precision arrays: instantiations of their own, so that the fp64 ones carry no branch
+    if (mode == 0) SFD_TRY(go(fft_fixed_kernel<PL, 0, true>));
+    else if (mode == 1) SFD_TRY(go(fft_fixed_kernel<PL, 1, true>));
+    else SFD_TRY(go(fft_fixed_kernel<PL, 2, true>));
+  } else {
+    if (mode == 0) SFD_TRY(go(fft_fixed_kernel<PL, 0, false>));
+    else if (mode == 1) SFD_TRY(go(fft_fixed_kernel<PL, 1, false>));
+    else SFD_TRY(go(fft_fixed_kernel<PL, 2, false>));
+  }
   return launch_check("fft_fixed_kernel");
 }
 bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t st, int* rc) {
