@@ -40,7 +40,8 @@ constexpr int kTwoCtaMaxW = 11;
 constexpr int ctas_per_sm(int w) { return w <= kTwoCtaMaxW ? 2 : 1; }
 
 struct ChunkTables {
-  double k[3][kChunk][16];   // kernel values per dimension
+  double k[3][kChunk][17];   // kernel values per dimension (pitch 17: the lanes of a warp, one source each, write and
+                             // read column a of 32 rows -- with a pitch of 16 doubles all 32 land in one bank pair)
   double c[kChunk][2];       // strengths
   int i0[kChunk][3];         // first cell of the footprint, relative to the subgrid origin
 };
