@@ -39,6 +39,13 @@ constexpr int kSmemBytes = 200 * 1024;   // subgrid budget of a CTA that has the
 constexpr int kTwoCtaMaxW = 11;
 constexpr int ctas_per_sm(int w) { return w <= kTwoCtaMaxW ? 2 : 1; }
 
+// Sources of a chunk whose W x W products ky[cy] kz[cz] are tabulated at a time (kyz table, ~16 KB whatever W): every
+// one of the W warps that visit a source needs the same W^2 products -- computed once and read as ceil(W^2/32)
+// contiguous LDS.64, instead of twice as many gathers from the ky and kz columns plus a DMUL per cell and visit.
+constexpr int kyz_sub(int W) { return W <= 8 ? 32 : (W <= 11 ? 16 : 8); }
+constexpr int kyz_pitch(int W) { return ((W * W + 31) / 32) * 32 + 1; }   // odd: lanes = consecutive sources write a column
+constexpr int kyz_bytes(int W) { return kyz_sub(W) * kyz_pitch(W) * 8; }
+
 struct ChunkTables {
   double k[3][kChunk][17];   // kernel values per dimension (pitch 17: the lanes of a warp, one source each, write and
                              // read column a of 32 rows -- with a pitch of 16 doubles all 32 land in one bank pair)
@@ -56,7 +63,9 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
   constexpr int DEG = W + 3;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ChunkTables& tab = *reinterpret_cast<ChunkTables*>(smem_raw);
-  double* sub = reinterpret_cast<double*>(smem_raw + sizeof(ChunkTables));
+  constexpr int KS = kyz_sub(W), KP = kyz_pitch(W);
+  double* kyzt = reinterpret_cast<double*>(smem_raw + sizeof(ChunkTables));          // [KS][KP]
+  double* sub = reinterpret_cast<double*>(smem_raw + sizeof(ChunkTables) + ((kyz_bytes(W) + 15) & ~15));
   __shared__ int s_item;
 
   const int tid = threadIdx.x, lane = tid & 31, a_own = tid >> 5;   // warp a_own owns the x-planes ix = a_own mod W
@@ -157,26 +166,38 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
       const double kx = lane < nch ? tab.k[0][lane][a] : 0.0;
       const double cre_l = r.re * kx;
       const double cim_l = REAL ? 0.0 : r.im * kx;
-      // sweep over the chunk's sources, software-pipelined: the broadcasts and the ky kz products of source s+1 are
-      // fetched while source s is accumulated
-      int base_n = __shfl_sync(0xffffffffu, base_l, 0);
-      double cre_n = __shfl_sync(0xffffffffu, cre_l, 0);
-      double cim_n = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, 0);
+      // sweep over the chunk's sources in sub-chunks of KS: first every thread of the CTA fills its share of the
+      // sub-chunk's ky kz products (index p = source + KS * cell: consecutive lanes are consecutive sources, so the
+      // pitch-17 columns and the odd-pitch product rows are read and written without bank conflicts), then every warp
+      // sweeps the KS sources, software-pipelined: the broadcasts and the products of source s+1 are fetched while
+      // source s is accumulated
+      for (int sc0 = 0; sc0 < nch; sc0 += KS) {
+      const int nsc = min(KS, nch - sc0);
+      if (sc0 > 0) __syncthreads();   // the previous sub-chunk's products are no longer read
+      for (int pidx = tid; pidx < KS * W * W; pidx += 32 * W) {
+        const int sl = pidx % KS, c = pidx / KS;
+        const int ccy = c / W, ccz = c - ccy * W;
+        if (sl < nsc) kyzt[sl * KP + c] = tab.k[1][sc0 + sl][ccy] * tab.k[2][sc0 + sl][ccz];
+      }
+      __syncthreads();
+      int base_n = __shfl_sync(0xffffffffu, base_l, sc0);
+      double cre_n = __shfl_sync(0xffffffffu, cre_l, sc0);
+      double cim_n = REAL ? 0.0 : __shfl_sync(0xffffffffu, cim_l, sc0);
       double kyz_n[NCL];
 #pragma unroll
-      for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? tab.k[1][0][cy[i]] * tab.k[2][0][cz[i]] : 0.0;
-      for (int s = 0; s < nch; ++s) {
+      for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? kyzt[lane + 32 * i] : 0.0;
+      for (int s = 0; s < nsc; ++s) {
         const int base = base_n;
         const double cre = cre_n, cim = cim_n;
         double kyz[NCL];
 #pragma unroll
         for (int i = 0; i < NCL; ++i) kyz[i] = kyz_n[i];
-        const int sn = min(s + 1, nch - 1);
-        base_n = __shfl_sync(0xffffffffu, base_l, sn);
-        cre_n = __shfl_sync(0xffffffffu, cre_l, sn);
-        if (!REAL) cim_n = __shfl_sync(0xffffffffu, cim_l, sn);
+        const int sn = min(s + 1, nsc - 1);
+        base_n = __shfl_sync(0xffffffffu, base_l, sc0 + sn);
+        cre_n = __shfl_sync(0xffffffffu, cre_l, sc0 + sn);
+        if (!REAL) cim_n = __shfl_sync(0xffffffffu, cim_l, sc0 + sn);
 #pragma unroll
-        for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? tab.k[1][sn][cy[i]] * tab.k[2][sn][cz[i]] : 0.0;
+        for (int i = 0; i < NCL; ++i) kyz_n[i] = on[i] ? kyzt[sn * KP + lane + 32 * i] : 0.0;
         if (RUNS) {
           if (base != run_base) {   // warp-uniform
             flush();
@@ -205,6 +226,7 @@ spread_kernel(N3Params p, const double* __restrict__ ptab, const SrcRec* __restr
           __syncwarp();
         }
       }
+      }   // sub-chunks
     }
     if (RUNS) flush();
     __syncthreads();
@@ -418,7 +440,7 @@ int spread_runs(const N3Params& p, const double* d_ptab, const SrcRec* d_src, co
 // shared-memory budget allows (at most 24: the sources lie on a shell, and smaller bins balance better).
 void spread_bins(int w, bool real_c, int bs[3]) {
   const int cell = real_c ? 8 : 16;
-  const int cap = (kSmemBytes / ctas_per_sm(w) - (int)sizeof(ChunkTables)) / cell;
+  const int cap = (kSmemBytes / ctas_per_sm(w) - (int)sizeof(ChunkTables) - ((kyz_bytes(w) + 15) & ~15)) / cell;
   double best = -1.0;
   for (int bz = real_c ? 16 : 8; bz <= 16; bz += 8) {
     const int pz = bz + w;
@@ -436,7 +458,8 @@ void spread_bins(int w, bool real_c, int bs[3]) {
 }
 
 size_t spread_smem_bytes(const N3Params& p) {
-  return sizeof(ChunkTables) + (size_t)(p.bs[0] + p.w) * (p.bs[1] + p.w) * (p.bs[2] + p.w) * (p.real_c ? 8 : 16);
+  return sizeof(ChunkTables) + ((kyz_bytes(p.w) + 15) & ~15) +
+         (size_t)(p.bs[0] + p.w) * (p.bs[1] + p.w) * (p.bs[2] + p.w) * (p.real_c ? 8 : 16);
 }
 
 int spread(const N3Params& p, const double* d_ptab, const SrcRec* d_src, const int32_t* d_item_bin,
