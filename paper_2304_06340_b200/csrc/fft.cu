@@ -548,7 +548,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 
 // The lengths with a fixed plan and their factor sequence (A1, B1, A2, B2, A3, B3).
 bool fixed_plan_factors(int N, int f[6]) {
-  static const int plans[][7] = {{360, 4, 2, 3, 3, 5, 1},  {672, 4, 2, 4, 3, 7, 1},  {720, 4, 4, 3, 3, 5, 1},
+  static const int plans[][7] = {{360, 4, 2, 3, 3, 5, 1},  {672, 4, 2, 4, 3, 7, 1},  {720, 4, 2, 2, 5, 3, 3},
                                  {1344, 4, 4, 4, 3, 7, 1}, {1440, 4, 4, 2, 5, 3, 3}, {2700, 4, 3, 3, 5, 3, 5}};
   for (const auto& pl : plans)
     if (pl[0] == N) {
@@ -996,8 +996,10 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
   if (P.contig ? (P.in_el != 1 || P.out_el != 1) : (P.real_in || P.dec_axis || P.in_lo != 1 || P.out_lo != 1)) return false;
   switch (P.N) {   //                       N    A1 B1 A2 B2 A3 B3  TB   T  CTAs/SM
     case 360:  *rc = launch_fixed<FixedPlan<360,  4, 2, 3, 3, 5, 1, 8, 128, 4>>(P, d_in, d_out, st); return true;
-    case 672:  *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 8, 256, 2>>(P, d_in, d_out, st); return true;
-    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 4, 3, 3, 5, 1, 8, 256, 2>>(P, d_in, d_out, st); return true;
+    // 672 / 720: groups of at most 12 / 10 points fit 80 registers, i.e. two CTAs of 384 threads = 24 warps per SM
+    // (0.676 -> 0.661 ms and 0.803 -> 0.768 ms at config 3 against 256 threads with groups of up to 16)
+    case 672:  *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 8, 384, 2>>(P, d_in, d_out, st); return true;
+    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2>>(P, d_in, d_out, st); return true;
     case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
     case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
     // 2700: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each (54.6 -> 47.1 ms
