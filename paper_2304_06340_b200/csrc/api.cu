@@ -401,6 +401,7 @@ int dist_layout(int64_t nF, int rule, const sfd_freq_quadrature* q, double reach
   // the distance calls centre the targets' box at the origin: the strengths stay real (half the transform's grids)
   if (eps == 0.0 || L->J == 0 || L->K == 0) {
     SFD_TRY(sfd_surface_ft_workspace(L->J, L->K, X, S, 0.0, &L->ft_bytes));
+    if (L->J > 0 && L->K > 0) L->ft_bytes = std::max(L->ft_bytes, direct_ball_work_bytes(L->J, L->K));
   } else {
     Nufft3Sizes sz;
     SFD_TRY(nufft3_sizes(L->J, L->K, X, S, eps, &sz, true));
@@ -479,7 +480,16 @@ int distance_enqueue(const char* who, const double* d_V, int64_t nV, const int32
     hint.n_hull = nv;
     hint.target_reach = t.r[a1 - 1];
     hint.target_ball = true;
-    SFD_TRY(surface_ft_impl(x, w, nf * rule, xi, K, eps, m ? nu2 : nu, base + L.ft, work_bytes - L.ft, stream, true, &hint));
+    bool ball_done = false;
+    if (eps == 0.0) {
+      // the nodes are the ball rule's: the direct sum takes them from the rule's tables (one direction and four radii
+      // per thread share the dot product dhat . x: direct.cu BALL); too small a rule falls through to the general kernel
+      SFD_TRY(direct_sum_ball(x, w, nf * rule, reinterpret_cast<const double*>(base + L.tab), q->n_r, q->n_theta, q->n_phi,
+                              a0, a1, half ? q->n_theta / 2 : 0, m ? nu2 : nu, base + L.ft, work_bytes - L.ft, st, &ball_done));
+      if (ball_done) prof_mark("direct_sum", st);
+    }
+    if (!ball_done)
+      SFD_TRY(surface_ft_impl(x, w, nf * rule, xi, K, eps, m ? nu2 : nu, base + L.ft, work_bytes - L.ft, stream, true, &hint));
   }
   SFD_TRY(reduce_enqueue(nu, xi, W, K, s, base + L.red, L.red_bytes, st, d_res, 1.0, -1.0, pair ? nu2 : nullptr));
   prof_mark("reduce", st);

@@ -69,10 +69,26 @@ struct __align__(16) Stage {
   double w[kTile];
 };
 
-template <int T>
+// BALL: the targets are nodes of the ball rule, xi_k = r_a dhat_m with k = (a - a0) n_dir + m (nodes.cu
+// freq_expand_kernel; `xi` then points at the rule's 1-D tables).  A thread holds ONE direction and T radii: the dot
+// product g = dhat . x_j is shared by its T pairs and the phase of a pair is one multiplication r_a g -- 16 + 3/T FP64
+// instructions per pair instead of 18 (8 + 2/T DFMA, 5 + 1/T DMUL, 3 DADD), and two of the six three-register DFMAs
+// (which issue every 3 clocks instead of 2, profiles/r1b) gone.  blockIdx.y then runs over groups of T radii and blockIdx.z over the source splits.
+// radii per thread of the ball-rule variant.  Measured at config 2 (direct_sum stage): general kernel 20.54 ms; ball
+// variant with 4 / 8 / 12 / 16 radii per thread 19.05 / 17.76 / 18.09 / 16.86 ms (63 / 94 / 126 / 168 registers, 4 / 4 / 3 / 3
+// CTAs per SM): the shared dot product and the per-source loads are amortised over more pairs
+constexpr int kBallT = 16;
+struct BallRule {
+  int n_r, n_th, n_ph;   // sizes of the rule's tables: r[n_r] wr[n_r] mu[n_th] st[n_th] wmu[n_th] cph[n_ph] sph[n_ph]
+  int a0, na;            // radial shells [a0, a0 + na)
+  int b0, nb;            // rings [b0, b0 + nb) (the half rule: b0 = n_th / 2)
+};
+
+template <int T, bool BALL>
 __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __restrict__ x, const double* __restrict__ w,
                                                              int64_t J, const double* __restrict__ xi, int64_t K,
-                                                             double* __restrict__ out, int64_t j_per_split, int use_tma) {
+                                                             double* __restrict__ out, int64_t j_per_split, int use_tma,
+                                                             BallRule ball) {
   extern __shared__ __align__(16) unsigned char smem_raw[];   // 48.1 KB: beyond the static limit
   Stage* stage = reinterpret_cast<Stage*>(smem_raw);
   double2* tab = reinterpret_cast<double2*>(smem_raw + 2 * sizeof(Stage));
@@ -86,17 +102,36 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
   }
   const double2* tl = tab + (tid & (kRep - 1));
   const int64_t k0 = (int64_t)blockIdx.x * (kThreads * T);
-  const int64_t jb = (int64_t)blockIdx.y * j_per_split;
+  const int64_t jb = (int64_t)(BALL ? blockIdx.z : blockIdx.y) * j_per_split;
   const int64_t je = min(J, jb + j_per_split);
   const int ntiles = (int)((je - jb + kTile - 1) / kTile);
 
   double a0[T], a1[T], a2[T], re[T], im[T];
+  const int n_dir = BALL ? ball.nb * ball.n_ph : 0;
+  const int m_dir = BALL ? min((int)(blockIdx.x * kThreads + tid), n_dir - 1) : 0;   // this thread's direction
 #pragma unroll
   for (int t = 0; t < T; ++t) {
-    const int64_t k = min(k0 + t * kThreads + tid, K - 1);
-    a0[t] = xi[3 * k] * c_sc[7];   // phases in units of 1/kTab of a turn
-    a1[t] = xi[3 * k + 1] * c_sc[7];
-    a2[t] = xi[3 * k + 2] * c_sc[7];
+    if (BALL) {
+      const double* tr = xi;                       // r
+      const double* tmu = xi + 2 * ball.n_r;       // mu, st, wmu, cph, sph
+      const double* tst = tmu + ball.n_th;
+      const double* tcp = tst + 2 * ball.n_th;
+      const double* tsp = tcp + ball.n_ph;
+      const int b = ball.b0 + m_dir / ball.n_ph, c = m_dir % ball.n_ph;
+      // a0[0..2] = dhat in units of 1/kTab of a turn per unit radius (t == 0 only); a1[t] = the t-th radius
+      if (t == 0) {
+        a0[0] = __dmul_rn(tst[b], tcp[c]) * c_sc[7];
+        a0[T > 1 ? 1 : 0] = __dmul_rn(tst[b], tsp[c]) * c_sc[7];
+        a0[T > 2 ? 2 : 0] = tmu[b] * c_sc[7];
+      }
+      a1[t] = tr[ball.a0 + min((int)blockIdx.y * T + t, ball.na - 1)];
+      a2[t] = 0.0;
+    } else {
+      const int64_t k = min(k0 + t * kThreads + tid, K - 1);
+      a0[t] = xi[3 * k] * c_sc[7];   // phases in units of 1/kTab of a turn
+      a1[t] = xi[3 * k + 1] * c_sc[7];
+      a2[t] = xi[3 * k + 2] * c_sc[7];
+    }
     re[t] = 0.0;
     im[t] = 0.0;
   }
@@ -136,9 +171,10 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
       const double x0 = s.x[3 * j], x1 = s.x[3 * j + 1], x2 = s.x[3 * j + 2], wj = s.w[j];
+      const double g = BALL ? __fma_rn(a0[0], x0, __fma_rn(a0[T > 1 ? 1 : 0], x1, a0[T > 2 ? 2 : 0] * x2)) : 0.0;
 #pragma unroll
       for (int u = 0; u < T; ++u) {
-        const double tq = __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
+        const double tq = BALL ? a1[u] * g : __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
         const double nm = __dadd_rn(tq, c_sc[6]);
         const int q = __double2loint(nm);
         const double nn = __dsub_rn(nm, c_sc[6]);
@@ -158,11 +194,17 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
     __syncthreads();  // everyone is done with this stage before it is refilled
   }
 
-  double* o = out + (size_t)blockIdx.y * (size_t)K * 2;
+  double* o = out + (size_t)(BALL ? blockIdx.z : blockIdx.y) * (size_t)K * 2;
 #pragma unroll
   for (int t = 0; t < T; ++t) {
-    const int64_t k = k0 + t * kThreads + tid;
-    if (k < K) reinterpret_cast<double2*>(o)[k] = make_double2(re[t], -im[t]);
+    if (BALL) {
+      const int ia = (int)blockIdx.y * T + t;
+      const int m = (int)(blockIdx.x * kThreads + tid);
+      if (ia < ball.na && m < n_dir) reinterpret_cast<double2*>(o)[(int64_t)ia * n_dir + m] = make_double2(re[t], -im[t]);
+    } else {
+      const int64_t k = k0 + t * kThreads + tid;
+      if (k < K) reinterpret_cast<double2*>(o)[k] = make_double2(re[t], -im[t]);
+    }
   }
 }
 
@@ -179,16 +221,29 @@ constexpr size_t kSmemBytes = 2 * sizeof(Stage) + sizeof(double2) * kTab * kRep 
 // Resident CTAs per SM of direct_sum_kernel<T> (shared memory binds: 4 with the current build); queried from the
 // runtime once, with that number as the fallback when there is no device (workspace queries on a CPU box).
 int ctas_per_sm(int T) {
-  static int cache[5] = {0, 0, 0, 0, 0};
+  static int cache[kBallT + 1] = {};
+  if (T == kBallT) {   // the ball-rule variant: 168 registers, 3 CTAs per SM
+    if (cache[T] == 0) {
+      int n = 0;
+      cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<kBallT, true>, kThreads, kSmemBytes) != cudaSuccess ||
+          n <= 0) {
+        cudaGetLastError();
+        return 3;
+      }
+      cache[T] = n;
+    }
+    return cache[T];
+  }
   if (cache[T] == 0) {
     int n = 0;
     cudaError_t e = cudaErrorUnknown;
-    cudaFuncSetAttribute(direct_sum_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    cudaFuncSetAttribute(direct_sum_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    cudaFuncSetAttribute(direct_sum_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (T == 4) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<4>, kThreads, kSmemBytes);
-    if (T == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<2>, kThreads, kSmemBytes);
-    if (T == 1) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<1>, kThreads, kSmemBytes);
+    cudaFuncSetAttribute(direct_sum_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    cudaFuncSetAttribute(direct_sum_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    cudaFuncSetAttribute(direct_sum_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (T == 4) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<4, false>, kThreads, kSmemBytes);
+    if (T == 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<2, false>, kThreads, kSmemBytes);
+    if (T == 1) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<1, false>, kThreads, kSmemBytes);
     if (e != cudaSuccess || n <= 0) {
       cudaGetLastError();
       return 4;
@@ -200,10 +255,11 @@ int ctas_per_sm(int T) {
 
 }  // namespace
 
-DirectPlan direct_plan(int64_t J, int64_t K) {
+DirectPlan direct_plan(int64_t J, int64_t K, int T_force) {
   DirectPlan p;
   const int64_t sms = num_sms();
   p.T = K >= sms * kThreads * 4 * 2 ? 4 : (K >= sms * kThreads * 2 * 2 ? 2 : 1);
+  if (T_force > 0) p.T = T_force;
   p.blocks_k = (K + (int64_t)kThreads * p.T - 1) / ((int64_t)kThreads * p.T);
   // The CTAs are equal pieces of work and the SMs hold `slots` of them at a time: blocks_k * nsplit CTAs run in
   // ceil(blocks_k * nsplit / slots) waves, the last one partly empty.  Split the sources over gridDim.y so that
@@ -247,9 +303,9 @@ int direct_sum(const double* d_x, const double* d_w, int64_t J, const double* d_
     int dev = 0;
     SFD_CUDA_TRY(cudaGetDevice(&dev));
     if (attr_dev != dev) {
-      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
       attr_dev = dev;
     }
   }
@@ -260,9 +316,9 @@ int direct_sum(const double* d_x, const double* d_w, int64_t J, const double* d_
   double* out = p.nsplit > 1 ? static_cast<double*>(d_work) : d_nuhat;
   dim3 grid((unsigned)p.blocks_k, (unsigned)p.nsplit);
   switch (p.T) {
-    case 4: direct_sum_kernel<4><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
-    case 2: direct_sum_kernel<2><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
-    default: direct_sum_kernel<1><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma); break;
+    case 4: direct_sum_kernel<4, false><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma, BallRule{}); break;
+    case 2: direct_sum_kernel<2, false><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma, BallRule{}); break;
+    default: direct_sum_kernel<1, false><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_xi, K, out, p.j_per_split, use_tma, BallRule{}); break;
   }
   SFD_TRY(launch_check("direct_sum_kernel"));
   if (p.nsplit > 1) {
@@ -270,6 +326,47 @@ int direct_sum(const double* d_x, const double* d_w, int64_t J, const double* d_
     combine_splits_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(out, p.nsplit, n2, d_nuhat);
     SFD_TRY(launch_check("combine_splits_kernel"));
   }
+  return SFD_OK;
+}
+
+size_t direct_ball_work_bytes(int64_t J, int64_t K) { return direct_plan(J, K, kBallT).work_bytes; }
+
+// The same sum on the nodes of the ball rule (shells [a0, a1), rings [b0, n_theta) -- b0 = n_theta / 2 is the half rule),
+// taken from the rule's 1-D tables in device memory (layout of nodes.cu freq_expand) instead of from the expanded nodes:
+// one direction and four radii per thread (BALL above).  *used = false (nothing enqueued) when the rule is too small
+// for that shape; the caller then runs direct_sum() on the expanded nodes.  Same workspace as direct_sum(J, K).
+int direct_sum_ball(const double* d_x, const double* d_w, int64_t J, const double* d_tables, int n_r, int n_th, int n_ph,
+                    int a0, int a1, int b0, double* d_nuhat, void* d_work, size_t work_bytes, cudaStream_t st, bool* used) {
+  *used = false;
+  const int na = a1 - a0, nb = n_th - b0;
+  const int64_t n_dir = (int64_t)nb * n_ph, K = (int64_t)na * n_dir;
+  if (J == 0 || K == 0 || na < kBallT || n_dir < kThreads) return SFD_OK;
+  if (n_dir > 0x7fffffffLL / 4) return SFD_OK;
+  const DirectPlan p = direct_plan(J, K, kBallT);
+  {
+    static thread_local int attr_dev = -1;
+    int dev = 0;
+    SFD_CUDA_TRY(cudaGetDevice(&dev));
+    if (attr_dev != dev) {
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      attr_dev = dev;
+    }
+  }
+  SFD_REQUIRE(work_bytes >= p.work_bytes && (p.work_bytes == 0 || d_work), SFD_ERR_WORKSPACE_TOO_SMALL,
+              "direct sum needs %zu workspace bytes, got %zu", p.work_bytes, work_bytes);
+  const int use_tma = ((reinterpret_cast<uintptr_t>(d_x) | reinterpret_cast<uintptr_t>(d_w)) & 15) == 0;
+  double* out = p.nsplit > 1 ? static_cast<double*>(d_work) : d_nuhat;
+  const BallRule ball{n_r, n_th, n_ph, a0, na, b0, nb};
+  dim3 grid((unsigned)((n_dir + kThreads - 1) / kThreads), (unsigned)((na + kBallT - 1) / kBallT), (unsigned)p.nsplit);
+  SFD_REQUIRE(grid.y <= 65535 && grid.z <= 65535, SFD_ERR_UNSUPPORTED, "direct_sum_ball: rule too large");
+  direct_sum_kernel<kBallT, true><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_tables, K, out, p.j_per_split, use_tma, ball);
+  SFD_TRY(launch_check("direct_sum_kernel"));
+  if (p.nsplit > 1) {
+    const int64_t n2 = 2 * K;
+    combine_splits_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, st>>>(out, p.nsplit, n2, d_nuhat);
+    SFD_TRY(launch_check("combine_splits_kernel"));
+  }
+  *used = true;
   return SFD_OK;
 }
 

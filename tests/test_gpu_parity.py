@@ -443,6 +443,6 @@ def test_weak_distance_half_rule_equals_full_rule(sfd, torch, q, eps):
     d, I = sfd.sfd_weak_distance(V, F, 12, s, R, q, eps)
     K_eval = sfd.sfd_weak_distance_targets(q)
     assert K_eval == (q[0] * (q[1] - q[1] // 2) * q[2] if q[2] % 2 == 0 else q[0] * q[1] * q[2])
-    tol = 1e-12 if eps == 0.0 else 1e-7
+    tol = 1e-11 if eps == 0.0 else 1e-7   # (eps = 0: two direct-sum kernels with independent roundings)
     assert abs(I - I_full) <= tol * I_full, (I, I_full)
 
