@@ -70,6 +70,8 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     ap.add_argument("--replicas", action="store_true",
                     help="multi-GPU: N independent evaluations (weak scaling, no collective) instead of the sharded path")
+    ap.add_argument("--force-sharded", action="store_true",
+                    help="run the sharded code path (sfd_weak_distance_range + combine) even with one rank: a self-test")
     ap.add_argument("--simulate-ranks", type=int, default=0,
                     help="one GPU: evaluate the shards of an N-rank run one after the other and report their device times")
     return ap.parse_args()
@@ -350,7 +352,7 @@ def run_sfd(args):
     eps_list = [e for e in c["eps"]]
     if args.config == 2:
         eps_list = [0.0, 1e-9]
-    sharded = world > 1 and not args.replicas
+    sharded = (world > 1 and not args.replicas) or args.force_sharded
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream()
 
@@ -722,7 +724,8 @@ def main():
     if e2e_ms is not None:
         e2e_value = pairs_per_step / (e2e_ms / args.steps * 1e-3) if n_direct else e2e_ms / args.steps / n_dist
         line["e2e"] = {"value": e2e_value, "unit": unit, "ms_per_step": e2e_ms / args.steps,
-                       "h2d_bytes_per_step": n_dist * (Vn.nbytes + Fn.nbytes), "d2h_bytes_per_step": n_dist * 16,
+                       "h2d_bytes_per_step": (1 if r["sharded"] else n_dist) * (Vn.nbytes + Fn.nbytes),
+                       "d2h_bytes_per_step": n_dist * (8 if r["sharded"] else 16),
                        "api": "sfd_weak_distance_host" if not r["sharded"] else
                               "pinned host mesh -> device, sharding.weak_distance_sharded (sfd_weak_distance_range + all-reduce)"}
 
