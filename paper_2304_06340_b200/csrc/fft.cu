@@ -235,10 +235,20 @@ __device__ __forceinline__ double ball_q(const FftPass& P, int64_t lo) {
 // band straight from registers: in those passes every output element is its own 16 TB-byte segment whatever the order),
 // the trivial twiddles of the last stage, and the run-time index arithmetic (~58 of 124 instructions per point in the
 // generic kernel, profiles/r1j_fft_phases.md).  Shared-memory round trips per point: 2 (4 accesses) instead of 4-5.
-template <int N_, int A1_, int B1_, int A2_, int B2_, int A3_, int B3_, int TB_, int T_, int CTAS_>
+template <int N_, int A1_, int B1_, int A2_, int B2_, int A3_, int B3_, int TB_, int T_, int CTAS_, bool PADDED_ = true>
 struct FixedPlan {
   static constexpr int N = N_, A1 = A1_, B1 = B1_, A2 = A2_, B2 = B2_, A3 = A3_, B3 = B3_, TB = TB_, T = T_, CTAS = CTAS_;
   static constexpr int G1 = A1 * B1, G2 = A2 * B2, G3 = A3 * B3;
+  // Contiguous passes (lanes run along the axis, a column is N consecutive cells): every block of L2 = N / G1 positions
+  // is followed by PAD cells with L2 + PAD = G3 (mod 8), so that (i) the lanes of group 2 -- G3 consecutive positions,
+  // then the next block -- and (ii) eight consecutive frequencies of the digit-reversed store -- positions N/4 and
+  // N/(4 B1) apart -- fall into different 16-byte bank groups (unpadded: 2-way and 4-way conflicts, 35 % of pass A's
+  // shared-memory wavefronts at N = 672, profiles/r2b_fft.md).
+  static constexpr int L2 = N / G1;
+  // (PADDED_ = false where the padding would push two CTAs' shared memory from the 196 KB to the 228 KB carve-out and
+  // the L1 from 60 to 28 KB: N = 720 measured 0.768 ms without, 0.793 ms with)
+  static constexpr int PAD = PADDED_ ? ((G3 - L2) % 8 + 8) % 8 : 0;
+  static constexpr int NP = N + G1 * PAD;   // cells of a padded column
   static_assert(G1 * G2 * G3 == N && A1 == 4 && N % 4 == 0, "plan must factor N with a leading radix 4");
   static_assert((TB & (TB - 1)) == 0, "tile height must be a power of two");
 };
@@ -334,7 +344,8 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
   double2* a = stw + FT::total;
   __shared__ int s_mm[2 * TB];   // strided passes: the range of outputs [mm0, mm1) every column of the tile has to store
   const int tid = threadIdx.x;
-  auto at = [](int pos, int col) { return STRIDED ? pos * TB + col : col * N + pos; };
+  // element `pos` (in block blk = pos / L2) of column col
+  auto at = [](int pos, int blk, int col) { return STRIDED ? pos * TB + col : col * PL::NP + pos + blk * PL::PAD; };
   for (int i = tid; i < FT::total; i += T) stw[i] = P.ftw[i];
   (void)G1;
   __syncthreads();   // the twiddle tables are in place
@@ -454,7 +465,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 #pragma unroll
       for (int p1 = 0; p1 < A1; ++p1)
 #pragma unroll
-        for (int p2 = 0; p2 < B1; ++p2) a[at(jp + p1 * (N / A1) + p2 * Lq1, col)] = v[p1][p2];
+        for (int p2 = 0; p2 < B1; ++p2) a[at(jp + p1 * (N / A1) + p2 * Lq1, p1 * B1 + p2, col)] = v[p1][p2];
     }
     // The sources lie on a shell: a third of the rows of the first pass (those outside the shell's projection) are
     // entirely zero, and so is their transform: store zeros, skip the other two groups.
@@ -479,12 +490,12 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 #pragma unroll
         for (int q1 = 0; q1 < A2; ++q1)
 #pragma unroll
-          for (int q2 = 0; q2 < B2; ++q2) v[q1][q2] = a[at(base + q1 * (L2 / A2) + q2 * Lq2, col)];
+          for (int q2 = 0; q2 < B2; ++q2) v[q1][q2] = a[at(base + q1 * (L2 / A2) + q2 * Lq2, b, col)];
         group_dft<A2, B2, false>(v, P.cst[1], stw + FT::off2a + jp, stw + FT::off2b + jp, Lq2);
 #pragma unroll
         for (int p1 = 0; p1 < A2; ++p1)
 #pragma unroll
-          for (int p2 = 0; p2 < B2; ++p2) a[at(base + p1 * (L2 / A2) + p2 * Lq2, col)] = v[p1][p2];
+          for (int p2 = 0; p2 < B2; ++p2) a[at(base + p1 * (L2 / A2) + p2 * Lq2, b, col)] = v[p1][p2];
       }
     }
     __syncthreads();
@@ -498,7 +509,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 #pragma unroll
       for (int q1 = 0; q1 < A3; ++q1)
 #pragma unroll
-        for (int q2 = 0; q2 < B3; ++q2) v[q1][q2] = a[at(b * G3 + q1 * B3 + q2, col)];
+        for (int q2 = 0; q2 < B3; ++q2) v[q1][q2] = a[at(b * G3 + q1 * B3 + q2, b / G2, col)];
       group_dft<A3, B3, true>(v, P.cst[2], nullptr, nullptr, 0);
       if (STRIDED) {
         const int mm0 = s_mm[2 * col], mm1 = s_mm[2 * col + 1];
@@ -518,7 +529,7 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
 #pragma unroll
         for (int p1 = 0; p1 < A3; ++p1)
 #pragma unroll
-          for (int p2 = 0; p2 < B3; ++p2) a[at(b * G3 + p1 * B3 + p2, col)] = v[p1][p2];
+          for (int p2 = 0; p2 < B3; ++p2) a[at(b * G3 + p1 * B3 + p2, b / G2, col)] = v[p1][p2];
       }
     }
     __syncthreads();
@@ -531,9 +542,11 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
       for (int mm = tid; mm < P.nout; mm += T) {
         int m = P.lo + mm;
         m = m < 0 ? m + N : (m >= N ? m - N : m);
-        const double2 z = a[at(__ldg(&P.rev[m]), col)];
+        const int pz = __ldg(&P.rev[m]);
+        const double2 z = a[at(pz, pz / PL::L2, col)];
         if (MODE == 0) {
-          const double2 zc = a[at(__ldg(&P.rev[m == 0 ? 0 : N - m]), col)];
+          const int pc = __ldg(&P.rev[m == 0 ? 0 : N - m]);
+          const double2 zc = a[at(pc, pc / PL::L2, col)];
           st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), F32);
           if (two) st_cplx(out, o0 + P.out_lo + mm, make_double2(0.5 * (z.y + zc.y), 0.5 * (zc.x - z.x)), F32);
         } else {
@@ -970,7 +983,7 @@ int launch_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t
   const int64_t rows_per_tile = (int64_t)PL::TB * (mode == 0 ? 2 : 1);
   const int64_t tiles = P.n_hi * ((P.n_lo + rows_per_tile - 1) / rows_per_tile);
   if (tiles == 0) return SFD_OK;
-  const size_t smem = ((size_t)PL::N * PL::TB + FixedTw<PL>::total) * 16;
+  const size_t smem = ((size_t)(mode == 2 ? PL::N : PL::NP) * PL::TB + FixedTw<PL>::total) * 16;
   SFD_REQUIRE(tiles < 0x7fffffffLL && P.counter, SFD_ERR_UNSUPPORTED, "FFT pass has too many tiles");
   unsigned grid = (unsigned)std::min<int64_t>(tiles, (int64_t)PL::CTAS * num_sms());   // persistent CTAs
   // tiles per run: two 64-byte tiles share a 128-byte line (measured at config 5: run 1 / 2 / 4 -> 49.6 / 47.1 / 50.1 ms)
@@ -999,7 +1012,7 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
     // 672 / 720: groups of at most 12 / 10 points fit 80 registers, i.e. two CTAs of 384 threads = 24 warps per SM
     // (0.676 -> 0.661 ms and 0.803 -> 0.768 ms at config 3 against 256 threads with groups of up to 16)
     case 672:  *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 8, 384, 2>>(P, d_in, d_out, st); return true;
-    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2>>(P, d_in, d_out, st); return true;
+    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2, false>>(P, d_in, d_out, st); return true;
     case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
     case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
     // 2700: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each (54.6 -> 47.1 ms
