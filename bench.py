@@ -244,13 +244,14 @@ class ClockSampler:
 
 
 # FP64-pipe instructions per source.target pair of direct_sum_kernel (checked against the SASS of
-# the inner loop): phase 1 DMUL + 2 DFMA; reduction to 1/256 turn 3 DADD; f^2 1 DMUL; sin 2 DFMA + 1 DMUL; cos 2 DFMA;
-# rotation by the table entry and accumulation 2 DMUL + 4 DFMA  ->  10 DFMA + 5 DMUL + 3 DADD = 18.
-# sfd_weak_distance runs the ball-rule variant of that kernel (one direction and BALL_T = 16 radii per thread share the dot
-# product dhat . x: direct.cu BALL): phase 1/16 (1 DMUL + 2 DFMA) + 1 DMUL per pair -> (8 + 2/16) DFMA + (5 + 1/16) DMUL +
-# 3 DADD = 16.19 FP64 instructions, 24.31 flops per pair.  The counts below are what the timed kernel executes.
+# the inner loop).  sfd_weak_distance runs the ball-rule variant of that kernel (one direction and BALL_T = 16 radii per
+# thread share the dot product dhat . x: direct.cu BALL).  Per pair: rounding addition and residual with the product r g
+# inside them 2 DFMA + 1 DADD; f^2 1 DMUL; monic sin / cos polynomials 2 DADD + 2 DFMA + 1 DMUL; leading coefficients and
+# weight 2 DMUL; rotation by the table entry and accumulation 4 DFMA.  Per source (/16): dot product 1 DMUL + 2 DFMA,
+# weight x leading coefficients 2 DMUL  ->  (8 + 2/16) DFMA + (4 + 3/16) DMUL + 3 DADD = 15.31 FP64 instructions, 23.44 flops
+# per pair.  The counts below are what the timed kernel executes.
 BALL_T = 16
-DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 8 + 2 / BALL_T, 8 + 1 / BALL_T
+DFMA_PER_PAIR, DMUL_DADD_PER_PAIR = 8 + 2 / BALL_T, 7 + 3 / BALL_T
 FLOPS_PER_PAIR = 2 * DFMA_PER_PAIR + DMUL_DADD_PER_PAIR
 FP64_LANES_PER_SM = 64          # DFMA / clk / SM on B200 (nominal 37-40 TFLOP/s at 1.965 GHz x 148 SMs)
 

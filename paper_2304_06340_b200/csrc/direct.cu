@@ -1,6 +1,6 @@
 // direct.cu -- A4: fp64 direct summation nuhat_k = sum_j w_j exp(-i xi_k . x_j)  (eq. 2.8
-// applied to the atoms of P:152).  FP64-pipe bound: 18 FP64 instructions per pair (phase 3, reduction 3, table +
-// short polynomials 6, rotate and accumulate 6).
+// applied to the atoms of P:152).  FP64-pipe bound: 17 FP64 instructions per pair (phase 3, reduction 3, table +
+// short monic polynomials 5, rotate and accumulate 6); 15.3 in the ball-rule variant (BALL below).
 //
 // Layout: one CTA = 128 threads x T targets held in registers (xi and the two accumulators); the sources
 // stream through shared memory in tiles of kTile atoms, double-buffered with 1-D bulk TMA copies
@@ -8,6 +8,7 @@
 // time (shared-memory broadcast, no bank conflicts).  For small K the source range is split over
 // gridDim.y and the partial sums are combined in a fixed order by a second kernel (deterministic).
 #include <algorithm>
+#include <type_traits>
 
 #include "common.cuh"
 #include "direct.cuh"
@@ -50,17 +51,21 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // thread, so the phase arrives in units of 1/kTab of a turn: tq = n + f with n = rint(tq) (the 1.5*2^52 trick: three
 // exact additions) and |f| <= 1/2, i.e. a residual angle of at most pi/256.  The table holds (cos, sin)(2 pi k / kTab)
 // for the whole turn, so there is no quadrant logic at all; sin and cos of the residual need 3 coefficients each
-// (Chebyshev-node fits at 60 digits, max error 1.2e-18 and 2.3e-16: tests/test_kernel_constants_cpu.py); one complex rotation joins the two.  18 FP64-pipe
-// instructions per pair (phase 3, reduction 3, f^2 1, sin 3, cos 2, rotate + accumulate 6) against 21 plus a 10-instruction
+// (Chebyshev-node fits at 60 digits, max error 1.2e-18 and 2.3e-16: tests/test_kernel_constants_cpu.py); one complex rotation joins the two.  17 FP64-pipe
+// instructions per pair (phase 3, reduction 3, f^2 1, sin 3, cos 2, rotate + accumulate 6 -- 2 per source fold the polynomials' leading coefficients into the weight) against 21 plus a 10-instruction
 // integer fix-up for the polynomial-only version: measured 1.31x faster (profiles/r1e_direct_sum_table.md), because
 // every non-FP64 instruction costs an issue cycle next to a 2-cycle DFMA.
 // The table is replicated kRep = 8 times in shared memory, entry (k, lane & 7) at index k*8 + (lane & 7): the 8 lanes
 // of each LDS.128 phase then read 8 different 16-byte bank groups whatever their k -- conflict-free by construction.
 constexpr int kTab = 256;
 constexpr int kRep = 8;
+static_assert(kRep * sizeof(double2) == 128, "the inner loop addresses table entry q at byte 128 q");
+// The two polynomials are kept monic, S(z) = S2 ((z + As) z + Bs) and C(z) = C2 ((z + Ac) z + Bc), with the leading
+// coefficients folded into the source's weight once per source: every step then reads at most two registers and one
+// constant (a DFMA on three registers issues every 3 clocks instead of 2, profiles/r1b_direct_sum.md).
 __constant__ double c_sc[8] = {
-    7.4219134520576935249e-11, -2.4641574764100320108e-6, 0.024543692606170259123,   // S2..S0: sin(a f) = f S(f^2)
-    1.5119764735229900432e-8, -0.00030119642336197489329, 0.9999999999999998425,      // C2..C0: cos(a f) = C(f^2)
+    -33201.10767024445654340395, 330692250.2493696703277053, 7.4219134520576935249e-11,   // As, Bs, S2: sin(a f) = f S(f^2)
+    -19920.70833352124336730809, 66138595.24347913412699348, 1.5119764735229900432e-8,    // Ac, Bc, C2: cos(a f) = C(f^2)
     6755399441055744.0,                                                               // 1.5 * 2^52
     40.743665431525205956834243423364};                                               // kTab / (2 pi)
 
@@ -71,9 +76,12 @@ struct __align__(16) Stage {
 
 // BALL: the targets are nodes of the ball rule, xi_k = r_a dhat_m with k = (a - a0) n_dir + m (nodes.cu
 // freq_expand_kernel; `xi` then points at the rule's 1-D tables).  A thread holds ONE direction and T radii: the dot
-// product g = dhat . x_j is shared by its T pairs and the phase of a pair is one multiplication r_a g -- 16 + 3/T FP64
-// instructions per pair instead of 18 (8 + 2/T DFMA, 5 + 1/T DMUL, 3 DADD), and two of the six three-register DFMAs
-// (which issue every 3 clocks instead of 2, profiles/r1b) gone.  blockIdx.y then runs over groups of T radii and blockIdx.z over the source splits.
+// product g = dhat . x_j is shared by its T pairs and the phase of a pair, r_a g, is never formed on its own: it enters
+// the rounding addition and the residual f as the product of a DFMA -- 15 + 5/T FP64 instructions per pair instead of 17
+// (8 + 2/T DFMA, 4 + 3/T DMUL, 3 DADD); five of them read three registers (the four accumulations and f) and issue every
+// 3 clocks instead of 2 (profiles/r1b), the polynomial steps read two and a constant.  Measured at config 2: 37.0 clocks
+// per warp and pair = 2 x 15.3 + 5.1 + 1.3 (four non-FP64 instructions: shift, mask, add, LDS.128).
+// blockIdx.y runs over groups of T radii and blockIdx.z over the source splits.
 // radii per thread of the ball-rule variant.  Measured at config 2 (direct_sum stage): general kernel 20.54 ms; ball
 // variant with 4 / 8 / 12 / 16 radii per thread 19.05 / 17.76 / 18.09 / 16.86 ms (63 / 94 / 126 / 168 registers, 4 / 4 / 3 / 3
 // CTAs per SM): the shared dot product and the per-source loads are amortised over more pairs
@@ -91,8 +99,19 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
                                                              BallRule ball) {
   extern __shared__ __align__(16) unsigned char smem_raw[];   // 48.1 KB: beyond the static limit
   Stage* stage = reinterpret_cast<Stage*>(smem_raw);
-  double2* tab = reinterpret_cast<double2*>(smem_raw + 2 * sizeof(Stage));
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * sizeof(Stage) + sizeof(double2) * kTab * kRep);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 2 * sizeof(Stage));
+  // The table sits right after the stages and the barriers -- or, when the launch left room for it (kSmemAligned), at
+  // the next shared-memory address that is a multiple of its 32 KB: the address of entry q is then a single LOP3,
+  // ((q << 7) & 0x7f80) | (table + 16 (lane & 7)), instead of a mask and an addition (every non-FP64 instruction costs
+  // the inner loop about a clock per pair: 16.03 -> 15.57 ms at config 2).  Decided here, uniformly for the CTA.
+  const uint32_t smem_base = smem_u32(smem_raw), tab_lo = smem_base + 2 * (uint32_t)sizeof(Stage) + 16;
+  uint32_t dyn_bytes;
+  asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn_bytes));
+  constexpr uint32_t kTabBytes = sizeof(double2) * kTab * kRep;
+  const uint32_t tab_hi = (tab_lo + kTabBytes - 1) & ~(kTabBytes - 1);
+  const bool aligned = BALL && tab_hi + kTabBytes <= smem_base + dyn_bytes;
+  const uint32_t tab_sa = aligned ? tab_hi : tab_lo;
+  double2* tab = reinterpret_cast<double2*>(smem_raw + (tab_sa - smem_base));
   const int tid = threadIdx.x;
   // (cos, sin)(2 pi k / kTab), replicated: entry (k, r) at k*kRep + r
   for (int i = tid; i < kTab * kRep; i += kThreads) {
@@ -100,7 +119,7 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
     sincospi((double)(i / kRep) * (2.0 / kTab), &sv, &cv);
     tab[i] = make_double2(cv, sv);
   }
-  const double2* tl = tab + (tid & (kRep - 1));
+  const uint32_t lane_sa = tab_sa + (uint32_t)(tid & (kRep - 1)) * 16;   // this lane's copy of entry 0
   const int64_t k0 = (int64_t)blockIdx.x * (kThreads * T);
   const int64_t jb = (int64_t)(BALL ? blockIdx.z : blockIdx.y) * j_per_split;
   const int64_t je = min(J, jb + j_per_split);
@@ -155,6 +174,8 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
 
   if (tid == 0 && ntiles > 0 && use_tma && tile_n(0) == kTile) issue(0);
 
+  auto run = [&](auto aligned_tag) {
+  constexpr bool ALIGNED = decltype(aligned_tag)::value;
   for (int t = 0; t < ntiles; ++t) {
     const int n = tile_n(t);
     Stage& s = stage[t & 1];
@@ -171,28 +192,37 @@ __global__ void __launch_bounds__(kThreads) direct_sum_kernel(const double* __re
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
       const double x0 = s.x[3 * j], x1 = s.x[3 * j + 1], x2 = s.x[3 * j + 2], wj = s.w[j];
+      const double wcj = wj * c_sc[5], wsj = wj * c_sc[2];   // w_j C2, w_j S2
       const double g = BALL ? __fma_rn(a0[0], x0, __fma_rn(a0[T > 1 ? 1 : 0], x1, a0[T > 2 ? 2 : 0] * x2)) : 0.0;
 #pragma unroll
       for (int u = 0; u < T; ++u) {
-        const double tq = BALL ? a1[u] * g : __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
-        const double nm = __dadd_rn(tq, c_sc[6]);
+        // BALL: the product r_a g goes into both additions unrounded (one instruction fewer, f exact)
+        const double tq = BALL ? 0.0 : __fma_rn(a0[u], x0, __fma_rn(a1[u], x1, a2[u] * x2));
+        const double nm = BALL ? __fma_rn(a1[u], g, c_sc[6]) : __dadd_rn(tq, c_sc[6]);
         const int q = __double2loint(nm);
         const double nn = __dsub_rn(nm, c_sc[6]);
-        const double f = __dsub_rn(tq, nn);
+        const double f = BALL ? __fma_rn(a1[u], g, -nn) : __dsub_rn(tq, nn);
         const double z = f * f;
-        const double sr = f * __fma_rn(__fma_rn(c_sc[0], z, c_sc[1]), z, c_sc[2]);
-        const double cr = __fma_rn(__fma_rn(c_sc[3], z, c_sc[4]), z, c_sc[5]);
-        const double2 e = tl[(q & (kTab - 1)) * kRep];
+        const double qs = __fma_rn(__dadd_rn(z, c_sc[0]), z, c_sc[1]);
+        const double qc = __fma_rn(__dadd_rn(z, c_sc[3]), z, c_sc[4]);
+        // table entry (q mod kTab, lane & 7) by its byte offset: 128 q + 16 (lane & 7)
+        const uint32_t qoff = (uint32_t)(q << 7) & (uint32_t)((kTab - 1) << 7);
+        const uint32_t ea = ALIGNED ? (qoff | lane_sa) : qoff + lane_sa;
+        double2 e;   // read-only after the barrier above: no memory clobber needed
+        asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(e.x), "=d"(e.y) : "r"(ea));
         // w e^{+i theta} = w (e.x + i e.y)(cr + i sr); the sign of the imaginary part is flipped at the store
-        const double wc = wj * cr, ws = wj * sr;
+        const double wc = wcj * qc, ws = wsj * (f * qs);
         re[u] = __fma_rn(e.x, wc, re[u]);
-        re[u] = __fma_rn(-e.y, ws, re[u]);
         im[u] = __fma_rn(e.y, wc, im[u]);
+        re[u] = __fma_rn(-e.y, ws, re[u]);
         im[u] = __fma_rn(e.x, ws, im[u]);
       }
     }
     __syncthreads();  // everyone is done with this stage before it is refilled
   }
+  };
+  if (BALL && aligned) run(std::true_type{});
+  else run(std::false_type{});
 
   double* o = out + (size_t)(BALL ? blockIdx.z : blockIdx.y) * (size_t)K * 2;
 #pragma unroll
@@ -217,6 +247,10 @@ __global__ void combine_splits_kernel(const double* __restrict__ part, int nspli
 }
 
 constexpr size_t kSmemBytes = 2 * sizeof(Stage) + sizeof(double2) * kTab * kRep + 16;   // stages, table, 2 mbarriers
+// The ball-rule variant (3 CTAs per SM by its registers) asks for enough to hold the table at a multiple of 32 KB: the
+// dynamic segment starts 1 KB into the CTA's window (the system-reserved part), so the table can sit at 32 KB ... 64 KB.
+// The kernel checks what it got and falls back to the packed layout otherwise.
+constexpr size_t kSmemAligned = 64 * 1024 - 1024;
 
 // Resident CTAs per SM of direct_sum_kernel<T> (shared memory binds: 4 with the current build); queried from the
 // runtime once, with that number as the fallback when there is no device (workspace queries on a CPU box).
@@ -225,8 +259,8 @@ int ctas_per_sm(int T) {
   if (T == kBallT) {   // the ball-rule variant: 168 registers, 3 CTAs per SM
     if (cache[T] == 0) {
       int n = 0;
-      cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<kBallT, true>, kThreads, kSmemBytes) != cudaSuccess ||
+      cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemAligned);
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, direct_sum_kernel<kBallT, true>, kThreads, kSmemAligned) != cudaSuccess ||
           n <= 0) {
         cudaGetLastError();
         return 3;
@@ -348,7 +382,7 @@ int direct_sum_ball(const double* d_x, const double* d_w, int64_t J, const doubl
     int dev = 0;
     SFD_CUDA_TRY(cudaGetDevice(&dev));
     if (attr_dev != dev) {
-      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+      SFD_CUDA_TRY(cudaFuncSetAttribute(direct_sum_kernel<kBallT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemAligned));
       attr_dev = dev;
     }
   }
@@ -359,7 +393,7 @@ int direct_sum_ball(const double* d_x, const double* d_w, int64_t J, const doubl
   const BallRule ball{n_r, n_th, n_ph, a0, na, b0, nb};
   dim3 grid((unsigned)((n_dir + kThreads - 1) / kThreads), (unsigned)((na + kBallT - 1) / kBallT), (unsigned)p.nsplit);
   SFD_REQUIRE(grid.y <= 65535 && grid.z <= 65535, SFD_ERR_UNSUPPORTED, "direct_sum_ball: rule too large");
-  direct_sum_kernel<kBallT, true><<<grid, kThreads, kSmemBytes, st>>>(d_x, d_w, J, d_tables, K, out, p.j_per_split, use_tma, ball);
+  direct_sum_kernel<kBallT, true><<<grid, kThreads, kSmemAligned, st>>>(d_x, d_w, J, d_tables, K, out, p.j_per_split, use_tma, ball);
   SFD_TRY(launch_check("direct_sum_kernel"));
   if (p.nsplit > 1) {
     const int64_t n2 = 2 * K;

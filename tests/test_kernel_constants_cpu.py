@@ -48,19 +48,22 @@ def test_sincos_fp64_literals():
 
 def test_direct_sum_table_literals():
     """direct.cu c_sc: with a = 2 pi / 256 and |f| <= 1/2, sin(a f) = f S(f^2) and cos(a f) = C(f^2), three coefficients
-    each; the last two entries are 1.5 * 2^52 and 256 / (2 pi).  DESIGN.md 5.2 quotes 1.8e-18 and 2.6e-16."""
+    each, stored monic: S(z) = S2 ((z + As) z + Bs), C(z) = C2 ((z + Ac) z + Bc) -- evaluated here in the kernel's order
+    (the leading coefficient multiplies the weight first); the last two entries are 1.5 * 2^52 and 256 / (2 pi).
+    DESIGN.md 5.2 quotes 1.8e-18 and 2.6e-16."""
     src = open(os.path.join(CSRC, "direct.cu")).read()
     m = re.search(r"c_sc\[8\] = \{(.*?)\};", src, flags=re.S)
     vals = [float(v) for v in re.findall(NUM, re.sub(r"//.*", "", m.group(1)))]
     assert len(vals) == 8, vals
-    S, Cc, magic, scale = vals[0:3], vals[3:6], vals[6], vals[7]
+    (As, Bs, S2), (Ac, Bc, C2), magic, scale = vals[0:3], vals[3:6], vals[6], vals[7]
     assert magic == 1.5 * 2.0 ** 52
     mp.mp.dps = 40
     assert scale == float(256 / (2 * mp.pi))
     a = 2 * mp.pi / 256
     f = np.linspace(-0.5, 0.5, 20001)
-    f2 = f * f
-    s = f * ((S[0] * f2 + S[1]) * f2 + S[2])
-    c = (Cc[0] * f2 + Cc[1]) * f2 + Cc[2]
-    assert np.abs(s - _exact(lambda t: mp.sin(a * t), f)).max() <= 4e-18
-    assert np.abs(c - _exact(lambda t: mp.cos(a * t), f)).max() <= 3e-16
+    z = f * f
+    for w in (1.0, 0.731, 3.1e-4):
+        s = (w * S2) * (f * ((z + As) * z + Bs))
+        c = (w * C2) * ((z + Ac) * z + Bc)
+        assert np.abs(s - w * _exact(lambda t: mp.sin(a * t), f)).max() <= 8e-18 * w
+        assert np.abs(c - w * _exact(lambda t: mp.cos(a * t), f)).max() <= 7e-16 * w   # the fit as evaluated (2.3e-16) + w C2 + the product + this reference
