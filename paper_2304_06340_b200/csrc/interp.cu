@@ -7,7 +7,10 @@
 // (w = 10: 125 clk per target and SM), far above its HBM traffic (the band of the inner grid, read once per bin).
 // The kernel is built to sit on that bound:
 //   * one persistent CTA per SM pulls work items (a target bin, or a slice of one: 512 to 4096 targets, nufft3.cu) from a
-//     device-side queue and stages the bin's padded subgrid (bt+w cells per axis) in shared memory as complex128;
+//     device-side queue and stages the bin's padded subgrid (bt+w cells per axis) in shared memory as complex128 -- one 3-D
+//     TMA box copy (cp.async.bulk.tensor, zero fill outside the band) issued by one thread, so that the staging costs the
+//     LSU pipe (the kernel's bottleneck) nothing; the bins at the centre plane of the Hermitian half band, whose lower
+//     cells are reflections, and the single-precision grids are staged with 16-byte LDGSTS copies instead;
 //   * the z extent of a bin is 8 or 16 cells, so the row pitch Pz = bt_z + w is congruent to w modulo 8 and the
 //     flattened (y,z) cell index c = y w + z lands in bank group c mod 8: any 8 consecutive lanes of an LDS.128 hit 8
 //     distinct 16-byte bank groups -- no bank conflicts for any w;
@@ -17,6 +20,10 @@
 //   * the 3w kernel values of a target are piecewise polynomials (nufft3.cuh footprint()) whose coefficients live
 //     in registers: lane i (mod 16) owns interval i, lanes 0-15 evaluate x then z, lanes 16-31 evaluate y;
 //   * w is a template parameter: plane loop, cell map and polynomial degree are compile-time.
+#include <cuda.h>   // CUtensorMap (the encoder is looked up through the runtime: no link against libcuda)
+
+#include <cstdlib>
+#include <cstring>
 #include <type_traits>
 
 #include "nufft3.cuh"
@@ -61,22 +68,29 @@ constexpr int kMaxW32 = 8;   // eps >= 1e-6 (w <= 7, one more for a handful of s
 
 template <int W, bool F32>
 __global__ void __launch_bounds__(32 * kWarps, 1)
-interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restrict__ v_raw, const TgtRec* __restrict__ tgt,
+interp_kernel(N3Params p, const __grid_constant__ CUtensorMap tmap, int use_tma, const double* __restrict__ ptab,
+              const void* __restrict__ v_raw, const TgtRec* __restrict__ tgt,
               const int32_t* __restrict__ item_bin, const int32_t* __restrict__ item_start,
               const int32_t* __restrict__ item_count, const int32_t* __restrict__ n_items,
               int32_t* __restrict__ counter, double2* __restrict__ G) {
   constexpr int DEG = W + 3;
   constexpr int NCL = (W * W + 31) / 32;
   constexpr int TPW = tpw_for(W);
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];   // (the TMA destination wants 128-byte alignment)
   using CT = std::conditional_t<F32, float2, double2>;   // a cell of the subgrid (and of the band in global memory)
   using AT = std::conditional_t<F32, float, double>;     // the plane loop's accumulators
   const CT* __restrict__ v = static_cast<const CT*>(v_raw);
   double (*ktab)[kMaxTpw][3][16] = reinterpret_cast<double (*)[kMaxTpw][3][16]>(smem_raw);
   CT* sub = reinterpret_cast<CT*>(smem_raw + kTabBytes);
   __shared__ int s_item;
+  __shared__ __align__(8) uint64_t s_bar;   // completion of the TMA box copy
+  uint32_t bar_phase = 0;
 
   const int tid = threadIdx.x, lane = tid & 31, wq = tid >> 5, li = lane & 15;
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&s_bar)));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   constexpr int BZ = F32 ? 16 : bin_z(W), BXY = F32 ? bin_xy32(W) : bin_xy(W, BZ);
   constexpr int Px = BXY + W, Py = BXY + W, Pz = BZ + W;
   constexpr int plane = Py * Pz;
@@ -101,6 +115,9 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restric
 
   const int total = *n_items;
   for (;;) {
+    // (the subgrid is read, and on the LDGSTS path written, through the generic proxy; the next box copy writes it
+    // through the async proxy)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();  // everyone is done with s_item and the previous subgrid
     if (tid == 0) s_item = atomicAdd(counter, 1);
     __syncthreads();
@@ -118,10 +135,24 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restric
     const int bz = bin % p.nbt[2], by = (bin / p.nbt[2]) % p.nbt[1], bx = bin / (p.nbt[2] * p.nbt[1]);
     const int ox = p.t0[0] + bx * p.bt[0] - W / 2, oy = p.t0[1] + by * p.bt[1] - W / 2, oz = p.t0[2] + bz * p.bt[2] - W / 2;
 
+    const int cx2 = p.n2[0], cy2 = p.n2[1], czc = p.n2[2] / 2;   // reflection m -> n2 - m about the centre n2/2
+    // The subgrid as one TMA box [Px][Py][2 Pz] of doubles at (ox, oy, oz) - lo, zero-filled outside the band: possible
+    // unless the box reaches below the centre plane of a half band (those cells are reflections of stored ones).
+    const bool box = !F32 && use_tma && !(p.zh && oz < czc);
+    if (box) {
+      if (tid == 0) {
+        constexpr uint32_t bytes = (uint32_t)Px * Py * Pz * sizeof(double2);
+        const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar), dst = (uint32_t)__cvta_generic_to_shared(sub);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+        asm volatile(
+            "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+            "l"(reinterpret_cast<uint64_t>(&tmap)), "r"(2 * (oz - p.lo[2])), "r"(oy - p.lo[1]), "r"(ox - p.lo[0]), "r"(bar)
+            : "memory");
+      }
+    } else {
     // stage the subgrid with 16-byte asynchronous copies (LDGSTS; zero-filled outside the band): every warp issues
     // all of its rows back to back and waits once, so the staging runs at L2 bandwidth instead of one round trip per
     // row.  One (x,y) row of Pz <= 32 cells per warp pass, coalesced along z.
-    const int cx2 = p.n2[0], cy2 = p.n2[1], czc = p.n2[2] / 2;   // reflection m -> n2 - m about the centre n2/2
     for (int row = wq; row < Px * Py; row += kWarps) {
       const int ix = row / Py, iy = row - ix * Py;
       if (lane < Pz) {
@@ -142,11 +173,27 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restric
           asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(srcp), "r"(nbytes) : "memory");
       }
     }
+    }
     asm volatile("cp.async.commit_group;" ::: "memory");
     TgtRec r[TPW];
 #pragma unroll
     for (int u = 0; u < TPW; ++u) r[u] = tgt[start + min(wq + u * kWarps, count - 1)];
     asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (box) {
+      const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
+      asm volatile(
+          "{\n"
+          ".reg .pred p;\n"
+          "WAIT_%=:\n"
+          "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+          "@p bra DONE_%=;\n"
+          "bra WAIT_%=;\n"
+          "DONE_%=:\n"
+          "}\n" ::"r"(bar),
+          "r"(bar_phase)
+          : "memory");
+      bar_phase ^= 1;
+    }
     __syncthreads();
 
     for (int t = wq; t < count; t += kWarps * TPW) {
@@ -256,6 +303,34 @@ interp_kernel(N3Params p, const double* __restrict__ ptab, const void* __restric
   }
 }
 
+// Tensor map of the band [nout0][nout1][nout2] of complex128 cells, seen as doubles [nout0][nout1][2 nout2], with the box
+// of one staged subgrid.  *ok = false when the driver offers no encoder or rejects the shape: LDGSTS staging then.
+void band_tensor_map(const N3Params& p, const double* d_v, CUtensorMap* tm, bool* ok) {
+  using Encode = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Encode encode = [] {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess ||
+        qr != cudaDriverEntryPointSuccess)
+      fn = nullptr;
+    cudaGetLastError();
+    return reinterpret_cast<Encode>(fn);
+  }();
+  *ok = false;
+  std::memset(tm, 0, sizeof(*tm));
+  if (!encode || p.f32) return;
+  const cuuint64_t dim[3] = {2ull * p.nout[2], (cuuint64_t)p.nout[1], (cuuint64_t)p.nout[0]};
+  const cuuint64_t stride[2] = {16ull * p.nout[2], 16ull * p.nout[2] * p.nout[1]};   // bytes, dimensions 1 and 2
+  const cuuint32_t boxd[3] = {2u * (p.bt[2] + p.w), (cuuint32_t)(p.bt[1] + p.w), (cuuint32_t)(p.bt[0] + p.w)};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  if (boxd[0] > 256 || boxd[1] > 256 || boxd[2] > 256 || (reinterpret_cast<uintptr_t>(d_v) & 15) != 0) return;
+  *ok = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(d_v), dim, stride, boxd, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int W, bool F32>
 int launch(const N3Params& p, const double* d_ptab, const double* d_v, const TgtRec* d_tgt, const int32_t* d_item_bin,
            const int32_t* d_item_start, const int32_t* d_item_count, const int32_t* d_n_items, int32_t* d_counter,
@@ -264,7 +339,12 @@ int launch(const N3Params& p, const double* d_ptab, const double* d_v, const Tgt
   if (first_use_on_device(attr_dev)) {
     SFD_CUDA_TRY(cudaFuncSetAttribute(interp_kernel<W, F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024));
   }
-  interp_kernel<W, F32><<<num_sms(), 32 * kWarps, smem, st>>>(p, d_ptab, d_v, d_tgt,
+  CUtensorMap tm;
+  bool tma = false;
+  band_tensor_map(p, d_v, &tm, &tma);
+  const char* no_tma = std::getenv("SFD_INTERP_NO_TMA");   // A-B measurements
+  if (no_tma && no_tma[0] == '1') tma = false;
+  interp_kernel<W, F32><<<num_sms(), 32 * kWarps, smem, st>>>(p, tm, tma ? 1 : 0, d_ptab, d_v, d_tgt,
                                                         d_item_bin, d_item_start, d_item_count, d_n_items, d_counter,
                                                         reinterpret_cast<double2*>(d_G));
   return launch_check("interp_kernel");
