@@ -17,6 +17,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <functional>
 #include <mutex>
 #include <tuple>
 #include <vector>
@@ -72,7 +73,7 @@ void kernel_params(double eps, bool careful, int* w, double* beta) {
 
 struct Layout {
   size_t src, skey, shist, soff, scur, sbhist, sboff, sitems, tgt, tkey, thist, toff, tcur, titems, fine, bufx, bufy, ffttab, dec,
-      scan, misc, ptab, total;
+      scan, scan_t, misc, ptab, total;
   int64_t ns_bins, ns_keys, nt_bins, ns_items, nt_items;
   size_t fine_bytes;
 };
@@ -169,6 +170,7 @@ int make_layout(const N3Params& p, int64_t J, int64_t K, Layout* L) {
   L->titems = put((size_t)L->nt_items * 4 * 3);
   L->dec = put((size_t)(p.nf[0] + p.nf[1] + p.nf[2] + p.nout[0] + p.nout[1] + p.nout[2]) * 8);
   L->scan = put(scan_workspace(std::max(L->ns_keys, L->nt_bins) + 1));
+  L->scan_t = put(scan_workspace(L->nt_bins + 1));   // the target sort runs beside the source side, on a stream of its own
   L->ffttab = put(fft_tables_bytes(p.n2));
   const size_t cb = p.f32 ? 8 : 16;   // bytes of a complex cell of the grids
   L->fine_bytes = (size_t)p.nf[0] * p.nf[1] * p.nf[2] * (p.real_c ? cb / 2 : cb);
@@ -285,12 +287,14 @@ void width_tables(const N3Params& p, ChebTable* quad, double* h_ptab) {
 // Work items of the spreader and the spread itself (shared by the type-3 and the type-1 transform).
 int items_and_spread(const N3Params& p, int64_t J, int64_t ns_bins, int64_t ns_keys, int64_t ns_items, int32_t* hist,
                      int32_t* off, int32_t* tmp, int32_t* sitems, int32_t* d_ctl, void* scan_w, size_t scan_b,
-                     const double* ptab, const SrcRec* src, double* fine, size_t fine_bytes, cudaStream_t st) {
+                     const double* ptab, const SrcRec* src, double* fine, size_t fine_bytes, cudaStream_t st,
+                     const std::function<int()>& before_spread = nullptr) {
   if (p.fine == 2) {
     // one item per run of equal footprints (hist / off are the per-footprint tables), cut at spread_runs_cap()
     SFD_TRY(make_items(hist, off, ns_keys, spread_runs_cap(), tmp, sitems, ns_items, d_ctl + 0, scan_w, scan_b, st));
     prof_mark("src_sort", st);
     SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
+    if (before_spread) SFD_TRY(before_spread());
     SFD_TRY(spread_runs(p, ptab, src, sitems, sitems + ns_items, sitems + 2 * ns_items, d_ctl + 0, d_ctl + 2, fine, st));
     prof_mark("spread", st);
     return SFD_OK;
@@ -302,6 +306,7 @@ int items_and_spread(const N3Params& p, int64_t J, int64_t ns_bins, int64_t ns_k
   SFD_TRY(make_items(hist, off, ns_bins, src_cap, tmp, sitems, ns_items, d_ctl + 0, scan_w, scan_b, st));
   prof_mark("src_sort", st);
   SFD_CUDA_TRY(cudaMemsetAsync(fine, 0, fine_bytes, st));
+  if (before_spread) SFD_TRY(before_spread());
   SFD_TRY(spread(p, ptab, src, sitems, sitems + ns_items, sitems + 2 * ns_items, d_ctl + 0, d_ctl + 2, fine, st));
   prof_mark("spread", st);
   return SFD_OK;
@@ -351,6 +356,43 @@ int nufft3_sizes(int64_t J, int64_t K, const double X[3], const double S[3], dou
 
 // ================================================================================================================
 namespace sfd {
+
+namespace {
+// The target sort (A5-7) depends on the geometry only, not on the source side, and is bandwidth-light work that fits beside
+// the spreader (LSU-bound) and the FFT passes: it runs on a second stream, forked from the caller's stream once the geometry
+// is known and joined before the interpolation.  One stream and two events per host thread and device, created on first use.
+struct SideStream {
+  cudaStream_t s = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+  int dev = -1;
+};
+int side_stream(SideStream** out) {
+  static thread_local SideStream side;
+  int dev = 0;
+  SFD_CUDA_TRY(cudaGetDevice(&dev));
+  if (side.dev != dev) {
+    // (a stream of another device is left alone: the thread may come back to it)
+    side = SideStream{};
+    SFD_CUDA_TRY(cudaStreamCreateWithFlags(&side.s, cudaStreamNonBlocking));
+    SFD_CUDA_TRY(cudaEventCreateWithFlags(&side.fork, cudaEventDisableTiming));
+    SFD_CUDA_TRY(cudaEventCreateWithFlags(&side.join, cudaEventDisableTiming));
+    side.dev = dev;
+  }
+  *out = &side;
+  return SFD_OK;
+}
+// Leaves no work of the second stream unordered with the caller's stream, whichever way the function returns (an error
+// between fork and join included: the caller may free the workspace as soon as its own stream has drained).
+struct SideJoin {
+  SideStream* side = nullptr;
+  cudaStream_t st = nullptr;
+  bool forked = false;
+  ~SideJoin() {
+    if (!forked) return;
+    if (cudaEventRecord(side->join, side->s) == cudaSuccess) cudaStreamWaitEvent(st, side->join, 0);
+  }
+};
+}  // namespace
 
 int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, int64_t K, double eps, double* d_nuhat,
            void* d_work, size_t work_bytes, cudaStream_t st, bool origin_centred, const ExtentHint* hint) {
@@ -430,8 +472,25 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   double* bufx = reinterpret_cast<double*>(base + L.bufx);
   double* bufy = reinterpret_cast<double*>(base + L.bufy);
   void* scan_w = base + L.scan;
-  const size_t scan_b = L.ffttab - L.scan;
+  const size_t scan_b = L.scan_t - L.scan;
   const size_t fine_bytes = L.fine_bytes;
+
+  // A5-7: rescale and bin-sort the targets
+  auto target_sort = [&](cudaStream_t ts, void* sw, size_t sb) -> int {
+    SFD_CUDA_TRY(cudaMemsetAsync(thist, 0, (size_t)(L.nt_bins + 1) * 4, ts));
+    SFD_CUDA_TRY(cudaMemsetAsync(tcur, 0, (size_t)(L.nt_bins + 1) * 4, ts));
+    SFD_TRY(target_keys(p, d_xi, K, tkey, thist, ts));
+    SFD_TRY(exclusive_scan_i32(thist, toff, L.nt_bins, nullptr, sw, sb, ts));
+    SFD_TRY(target_scatter(p, d_xi, K, tkey, toff, tcur, tgt, ts));
+    // slices of a crowded bin each stage the bin's subgrid again: larger slices when there are enough targets to keep
+    // every SM busy (measured: interp -15 % at config 3 with 4096, +25 % at config 2 where 4096 leaves SMs idle)
+    const int tgt_cap = (int)std::min<int64_t>(4096, std::max<int64_t>(kTgtCap, K / ((int64_t)num_sms() * 4)));
+    return make_items(thist, toff, L.nt_bins, tgt_cap, tcur, titems, L.nt_items, d_ctl + 1, sw, sb, ts);
+  };
+  const char* no_overlap = std::getenv("SFD_NO_OVERLAP");   // A-B measurements: everything on the caller's stream
+  const bool overlap = !(no_overlap && no_overlap[0] == '1');
+  SideStream* side = nullptr;
+  SideJoin side_join;
 
   // A5-2/A5-3: rescale, pre-phase and bin-sort the sources
   SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_keys + 1) * 4, st));
@@ -446,9 +505,25 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
     shist = bh;
     soff = bo;
   }
-  // A5-4: work items and spread
+  // A5-4: work items and spread.  The fork sits between the zero-fill and the spreader's launch: the target sort's kernels
+  // fill the machine on their own, so made eligible any earlier they only run ahead of the source side; from here on they
+  // share the SMs with the spreader's persistent CTAs (no shared memory, few registers) and with the FFT passes.
+  auto fork = [&]() -> int {
+    if (!overlap) return SFD_OK;
+    SFD_TRY(side_stream(&side));
+    SFD_CUDA_TRY(cudaEventRecord(side->fork, st));
+    SFD_CUDA_TRY(cudaStreamWaitEvent(side->s, side->fork, 0));
+    side_join.side = side;
+    side_join.st = st;
+    side_join.forked = true;
+    return SFD_OK;
+  };
   SFD_TRY(items_and_spread(p, J, L.ns_bins, L.ns_keys, L.ns_items, shist, soff, scur, sitems, d_ctl, scan_w, scan_b, ptab,
-                           src, fine, fine_bytes, st));
+                           src, fine, fine_bytes, st, fork));
+  if (overlap) {   // (submitted behind the spreader)
+    SFD_TRY(target_sort(side->s, base + L.scan_t, L.ffttab - L.scan_t));
+    SFD_CUDA_TRY(cudaEventRecord(side->join, side->s));
+  }
 
   // A5-5 + A5-6: deconvolution folded into the first of three pruned 1-D FFT passes (timed on its own)
   SFD_TRY(deconv_tables(p, quad, dec, st));
@@ -516,16 +591,13 @@ int nufft3(const double* d_x, const double* d_w, int64_t J, const double* d_xi, 
   }
   prof_mark("fft", st);
 
-  // A5-7: rescale and bin-sort the targets
-  SFD_CUDA_TRY(cudaMemsetAsync(thist, 0, (size_t)(L.nt_bins + 1) * 4, st));
-  SFD_CUDA_TRY(cudaMemsetAsync(tcur, 0, (size_t)(L.nt_bins + 1) * 4, st));
-  SFD_TRY(target_keys(p, d_xi, K, tkey, thist, st));
-  SFD_TRY(exclusive_scan_i32(thist, toff, L.nt_bins, nullptr, scan_w, scan_b, st));
-  SFD_TRY(target_scatter(p, d_xi, K, tkey, toff, tcur, tgt, st));
-  // slices of a crowded bin each stage the bin's subgrid again: larger slices when there are enough targets to keep
-  // every SM busy (measured: interp -15 % at config 3 with 4096, +25 % at config 2 where 4096 leaves SMs idle)
-  const int tgt_cap = (int)std::min<int64_t>(4096, std::max<int64_t>(kTgtCap, K / ((int64_t)num_sms() * 4)));
-  SFD_TRY(make_items(thist, toff, L.nt_bins, tgt_cap, tcur, titems, L.nt_items, d_ctl + 1, scan_w, scan_b, st));
+  // A5-7 (enqueued above on the second stream): the interpolation waits for it
+  if (overlap) {
+    SFD_CUDA_TRY(cudaStreamWaitEvent(st, side->join, 0));
+    side_join.forked = false;
+  } else {
+    SFD_TRY(target_sort(st, scan_w, scan_b));
+  }
   prof_mark("tgt_sort", st);
 
   // A5-8: interpolate;  A5-9: post-deconvolve + post-phase
@@ -668,7 +740,7 @@ int nufft1_lattice(const double* d_x, const double* d_w, int64_t J, int M, doubl
   double* bufx = reinterpret_cast<double*>(base + L.bufx);
   double* bufy = reinterpret_cast<double*>(base + L.bufy);
   void* scan_w = base + L.scan;
-  const size_t scan_b = L.ffttab - L.scan;
+  const size_t scan_b = L.scan_t - L.scan;
 
   // rescale (eq. 3.7) and bin-sort the sources, as in the type-3 transform
   SFD_CUDA_TRY(cudaMemsetAsync(shist, 0, (size_t)(L.ns_keys + 1) * 4, st));
