@@ -11,7 +11,10 @@
  *     the caller; the library keeps no pointer after the call returns except for work already
  *     enqueued on `stream`.  Outputs are fully overwritten, never accumulated into.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
- *     calls only enqueue work unless the description says "synchronises".
+ *     calls only enqueue work unless the description says "synchronises".  The type-3 transform (eps > 0) runs part of its
+ *     work (the target sort) on a second, non-blocking stream that the library creates once per host thread and device;
+ *     that work is ordered after everything enqueued on `stream` before the call and before everything after it (event
+ *     fork / join), so to the caller the call behaves as if all of it ran on `stream`.
  *   - Every call that needs scratch memory has a *_workspace query; d_work must be 256-byte aligned.
  *   - Arrays are C-contiguous fp64 / int32: points double[n][3], complex values double[n][2] = (re,im).
  *   - NULL pointer where one is required -> SFD_ERR_NULL; out-of-range scalar -> SFD_ERR_INVALID_ARG;
