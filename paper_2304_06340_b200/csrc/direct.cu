@@ -8,6 +8,7 @@
 // time (shared-memory broadcast, no bank conflicts).  For small K the source range is split over
 // gridDim.y and the partial sums are combined in a fixed order by a second kernel (deterministic).
 #include <algorithm>
+#include <cstdlib>
 #include <type_traits>
 
 #include "common.cuh"
@@ -393,7 +394,10 @@ int direct_sum_ball(const double* d_x, const double* d_w, int64_t J, const doubl
   const BallRule ball{n_r, n_th, n_ph, a0, na, b0, nb};
   dim3 grid((unsigned)((n_dir + kThreads - 1) / kThreads), (unsigned)((na + kBallT - 1) / kBallT), (unsigned)p.nsplit);
   SFD_REQUIRE(grid.y <= 65535 && grid.z <= 65535, SFD_ERR_UNSUPPORTED, "direct_sum_ball: rule too large");
-  direct_sum_kernel<kBallT, true><<<grid, kThreads, kSmemAligned, st>>>(d_x, d_w, J, d_tables, K, out, p.j_per_split, use_tma, ball);
+  // SFD_DIRECT_PACKED=1 (tests): launch without the room for the aligned table, i.e. run the kernel's packed-layout loop
+  const char* packed = std::getenv("SFD_DIRECT_PACKED");
+  const size_t smem = packed && packed[0] == '1' ? kSmemBytes : kSmemAligned;
+  direct_sum_kernel<kBallT, true><<<grid, kThreads, smem, st>>>(d_x, d_w, J, d_tables, K, out, p.j_per_split, use_tma, ball);
   SFD_TRY(launch_check("direct_sum_kernel"));
   if (p.nsplit > 1) {
     const int64_t n2 = 2 * K;

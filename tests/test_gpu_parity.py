@@ -195,6 +195,32 @@ def test_weak_distance_jittered_mesh(sfd, orc, torch):
         assert abs(I - I_ref) <= 1e-8 * I_ref
 
 
+def test_code_paths_behind_switches_agree(sfd, orc, torch, monkeypatch):
+    """The alternatives the library chooses between at run time compute the same thing: the ball-rule direct sum with its
+    table packed behind the stages instead of 32 KB-aligned (bit-identical: same arithmetic, other addresses), the type-3
+    transform with the subgrids staged by LDGSTS instead of TMA box copies and with the target sort on the caller's stream
+    instead of the second one (identical up to the order of the spreader's additions).  Config 1, against the oracle too."""
+    c = workloads.CONFIGS[1]
+    q = (c["n_r"], c["n_theta"], c["n_phi"])
+    V, F = sfd.sfd_mesh_icosphere(c["level"])
+    Vo, Fo = orc.mesh_icosphere(c["level"])
+    _, I_ref = orc.weak_distance(Vo, Fo, c["rule"], 2.0, c["R"], *q)
+    _, I0 = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 0.0)
+    monkeypatch.setenv("SFD_DIRECT_PACKED", "1")
+    _, I1 = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, 0.0)
+    monkeypatch.delenv("SFD_DIRECT_PACKED")
+    assert I1 == I0 and abs(I0 - I_ref) <= 1e-8 * I_ref
+    for eps in (1e-6, 1e-10):
+        _, Ia = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, eps)
+        monkeypatch.setenv("SFD_INTERP_NO_TMA", "1")
+        monkeypatch.setenv("SFD_NO_OVERLAP", "1")
+        _, Ib = sfd.sfd_weak_distance(V, F, c["rule"], 2.0, c["R"], q, eps)
+        monkeypatch.delenv("SFD_INTERP_NO_TMA")
+        monkeypatch.delenv("SFD_NO_OVERLAP")
+        assert abs(Ia - Ib) <= 1e-12 * Ia, (eps, Ia, Ib)
+        assert abs(Ia - I_ref) <= 2 * np.sqrt(I_ref * _r13_bound(orc, Vo, Fo, c["rule"], q, c["R"], 2.0, eps)) + _r13_bound(orc, Vo, Fo, c["rule"], q, c["R"], 2.0, eps)
+
+
 def _r13_bound(orc, Vn, Fn, rule, q, R, s, eps):
     """DESIGN.md R13: |dI| <= 2 sqrt(I E2) + E2, E2 = (2 pi)^-3 sum_k W_k (10 eps sum|w|)^2 (1+r^2)^-s."""
     x, w = orc.nodes(Vn, Fn, rule)
