@@ -133,6 +133,27 @@ int sfd_surface_ft(const double* d_x /*[J][3]*/, const double* d_w /*[J]*/, int6
                    const double* d_xi /*[K][3]*/, int64_t K, double eps, double* d_nuhat /*[K][2]*/,
                    void* d_work, size_t work_bytes, sfd_stream stream);
 
+/* ---- A4 without a workspace: for callers that cannot allocate ------------------------------------
+ * The fp64 direct sum (sfd_surface_ft with eps == 0: same kernels, same fixed summation order, bit-identical
+ * result) for code that may not call cudaMalloc: under CUDA graph capture, in serving loops, in harnesses that forbid it.
+ * The call allocates nothing, on the host or on the device, and takes no workspace: the partial sums of the direct sum's
+ * source splits go to a static device array of SFD_STATIC_SCRATCH_BYTES (16 MiB) that every GPU which loads the library
+ * holds until the process exits.  Device pointers d_x [J][3], d_w [J], d_xi [K][3], d_nuhat [K][2] (owned by the caller,
+ * fully overwritten); enqueues on `stream`, does not synchronise.
+ *   - Sizes whose partial sums do not fit (nsplit * K * 16 bytes; nsplit <= 32 is chosen from J, K and the SM count, 1 for
+ *     large K) are rejected with SFD_ERR_UNSUPPORTED and a message naming the sizes; nothing is written.
+ *     sfd_surface_ft_direct_static_scratch reports the bytes a (J, K) needs (host only; needs a CUDA device for the SM
+ *     count, 148 SMs assumed otherwise); any K fits when that is 0.
+ *   - The array is shared by every call on a device and keeps the last call's contents; every entry a call reads it has
+ *     written itself, so nothing needs clearing.  Calls that OVERLAP on the GPU (other streams, graphs replayed
+ *     concurrently) race on it and give wrong results: keep them on one stream or order them with events.
+ *   - J == 0 gives zeros, K == 0 does nothing; NULL buffers -> SFD_ERR_NULL. */
+#define SFD_STATIC_SCRATCH_BYTES (16u << 20)
+int sfd_surface_ft_direct_static_scratch(int64_t J, int64_t K, size_t* bytes);
+int sfd_surface_ft_direct_static(const double* d_x /*[J][3]*/, const double* d_w /*[J]*/, int64_t J,
+                                 const double* d_xi /*[K][3]*/, int64_t K, double* d_nuhat /*[K][2]*/,
+                                 sfd_stream stream);
+
 /* ---- A6: fused target-side reduction (eq. 2.7 with P:55 eq. 2.5; eq. 2.14) ----------
  * I = (2 pi)^-3 sum_k W_k |nuhat_k - sigmahat(xi_k)|^2 (1+|xi_k|^2)^-s,  sigmahat = 4 pi sin|xi|/|xi|
  * (the unit sphere's transform).  Deterministic compensated fp64 sum.  s > 0.5, else

@@ -50,6 +50,8 @@ _SIGS = {
     "sfd_surface_ft_workspace": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(_sz)]),
     "sfd_surface_ft_plan": (C.c_int, [_i64, _i64, _P(_dbl), _P(_dbl), _dbl, _P(C.c_int32), _P(_i64), _P(_i64)]),
     "sfd_surface_ft": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _dbl, _vp, _vp, _sz, _vp]),
+    "sfd_surface_ft_direct_static_scratch": (C.c_int, [_i64, _i64, _P(_sz)]),
+    "sfd_surface_ft_direct_static": (C.c_int, [_vp, _vp, _i64, _vp, _i64, _vp, _vp]),
     "sfd_reduce_workspace": (C.c_int, [_i64, _P(_sz)]),
     "sfd_reduce": (C.c_int, [_vp, _vp, _vp, _i64, _dbl, _vp, _sz, _vp, _P(_dbl)]),
     "sfd_weak_distance_workspace": (C.c_int, [_i64, C.c_int, _P(sfd_freq_quadrature), _dbl, _dbl, _dbl, _P(_sz)]),
@@ -243,6 +245,26 @@ def sfd_surface_ft(x, w, xi, eps=0.0, work=None, out=None):
     _chk(_lib.sfd_surface_ft(_ptr(x), _ptr(w), J, _ptr(xi), K, float(eps), _ptr(nu), _ptr(work), work.numel(),
                              _stream()))
     return torch.view_as_complex(nu) if K > 0 else torch.empty(0, dtype=torch.complex128, device=x.device)
+
+
+SFD_STATIC_SCRATCH_BYTES = 16 << 20
+
+
+def sfd_surface_ft_direct_static_scratch(J, K):
+    """Bytes of the static scratch array a direct sum of J sources on K targets needs (0: any K fits)."""
+    b = _sz()
+    _chk(_lib.sfd_surface_ft_direct_static_scratch(int(J), int(K), C.byref(b)))
+    return b.value
+
+
+def sfd_surface_ft_direct_static(x, w, xi, out):
+    """The fp64 direct sum without a workspace and without any allocation (include/sfd.h): the caller passes the output
+    tensor float64[K][2]; the library's static device array holds the partial sums.  Returns `out` viewed as complex128."""
+    _dev_f64(x, 3), _dev_f64(w), _dev_f64(xi, 3), _dev_f64(out, 2)
+    J, K = x.shape[0], xi.shape[0]
+    assert w.shape[0] == J and out.shape[0] == K
+    _chk(_lib.sfd_surface_ft_direct_static(_ptr(x), _ptr(w), J, _ptr(xi), K, _ptr(out), _stream()))
+    return torch.view_as_complex(out) if K > 0 else torch.empty(0, dtype=torch.complex128, device=x.device)
 
 
 def sfd_reduce(nuhat, xi, W, s):

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsfd.so")
 SOURCES = ["api.cu", "mesh.cu", "nodes.cu", "scan.cu", "direct.cu", "reduce.cu", "nufft3.cu", "nufft3_glue.cu",
-           "spread.cu", "interp.cu", "fft.cu", "exact.cu"]
+           "spread.cu", "interp.cu", "fft.cu", "exact.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr"]
