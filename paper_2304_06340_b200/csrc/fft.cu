@@ -535,16 +535,23 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
     __syncthreads();
     if (STRIDED) continue;
 
-    // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table
-    for (int col = 0; col < ncol; ++col) {
-      const int64_t o0 = hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
-      const bool two = 2 * col + 1 < nrow;
-      for (int mm = tid; mm < P.nout; mm += T) {
+    // ---- contiguous passes: the band goes out along the axis, through the digit-reversal table.  One loop over all
+    // (column, output) pairs of the tile: with a loop per column only nout of the T threads had work (47 % at n2 = 672).
+    {
+      const int nout = P.nout, total = ncol * nout;
+      const float inv_nout = 1.0f / (float)nout;
+      for (int idx = tid; idx < total; idx += T) {
+        // idx / nout: the half-cell offset keeps the rounded quotient on the right side of every multiple of nout
+        // (idx < 2^15, nout < 2^12: the float error is far below 0.5 / nout)
+        const int col = (int)(((float)idx + 0.5f) * inv_nout);
+        const int mm = idx - col * nout;
+        const int64_t o0 = hi * P.out_hi + (lo0 + PACK * col) * P.out_lo;
         int m = P.lo + mm;
         m = m < 0 ? m + N : (m >= N ? m - N : m);
         const int pz = __ldg(&P.rev[m]);
         const double2 z = a[at(pz, pz / PL::L2, col)];
         if (MODE == 0) {
+          const bool two = 2 * col + 1 < nrow;
           const int pc = __ldg(&P.rev[m == 0 ? 0 : N - m]);
           const double2 zc = a[at(pc, pc / PL::L2, col)];
           st_cplx(out, o0 + mm, make_double2(0.5 * (z.x + zc.x), 0.5 * (z.y - zc.y)), F32);
@@ -1011,8 +1018,17 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
     case 360:  *rc = launch_fixed<FixedPlan<360,  4, 2, 3, 3, 5, 1, 8, 128, 4>>(P, d_in, d_out, st); return true;
     // 672 / 720: groups of at most 12 / 10 points fit 80 registers, i.e. two CTAs of 384 threads = 24 warps per SM
     // (0.676 -> 0.661 ms and 0.803 -> 0.768 ms at config 3 against 256 threads with groups of up to 16)
-    case 672:  *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 8, 384, 2>>(P, d_in, d_out, st); return true;
-    case 720:  *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2, false>>(P, d_in, d_out, st); return true;
+    // 672 / 720: groups of at most 12 / 10 points fit 80 registers; tiles of 4 columns in 3 or 4 CTAs per SM interleave the
+    // phases of more tiles than tiles of 8 columns in 2 CTAs do (stage `fft` at config 3, all passes with <8, 384, 2>:
+    // 0.649 / 0.768 ms; measured per pass: profiles/r2b_fft.md)
+    case 672:
+      if (P.contig) *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 256, 3>>(P, d_in, d_out, st);
+      else *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 192, 4>>(P, d_in, d_out, st);
+      return true;
+    case 720:
+      if (P.contig) *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 4, 192, 4, false>>(P, d_in, d_out, st);
+      else *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2, false>>(P, d_in, d_out, st);
+      return true;
     case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
     case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
     // 2700: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each (54.6 -> 47.1 ms
