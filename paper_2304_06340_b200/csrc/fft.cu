@@ -1016,24 +1016,34 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
   if (P.contig ? (P.in_el != 1 || P.out_el != 1) : (P.real_in || P.dec_axis || P.in_lo != 1 || P.out_lo != 1)) return false;
   switch (P.N) {   //                       N    A1 B1 A2 B2 A3 B3  TB   T  CTAs/SM
     case 360:  *rc = launch_fixed<FixedPlan<360,  4, 2, 3, 3, 5, 1, 8, 128, 4>>(P, d_in, d_out, st); return true;
-    // 672 / 720: groups of at most 12 / 10 points fit 80 registers, i.e. two CTAs of 384 threads = 24 warps per SM
-    // (0.676 -> 0.661 ms and 0.803 -> 0.768 ms at config 3 against 256 threads with groups of up to 16)
-    // 672 / 720: groups of at most 12 / 10 points fit 80 registers; tiles of 4 columns in 3 or 4 CTAs per SM interleave the
-    // phases of more tiles than tiles of 8 columns in 2 CTAs do (stage `fft` at config 3, all passes with <8, 384, 2>:
-    // 0.649 / 0.768 ms; measured per pass: profiles/r2b_fft.md)
+    // How many columns a tile has and how many CTAs share an SM is measured per length and per kind of pass
+    // (profiles/r2b_fft.md).  The warps of a CTA go through a tile's phases together -- all load, all compute, all store,
+    // a barrier between -- so what keeps the SM's pipes busy is the number of CTAs in different phases, not the number of
+    // warps: the contiguous pass, whose global accesses run along the axis whatever the tile, takes ONE column (two
+    // packed real rows) per tile in as many CTAs as fit; the strided passes need TB * 16-byte segments of the other axis.
+    // 672 / 720: groups of at most 12 / 10 points fit 80 registers.
     case 672:
       if (P.contig) *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 256, 3>>(P, d_in, d_out, st);
       else *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 192, 4>>(P, d_in, d_out, st);
       return true;
     case 720:
-      if (P.contig) *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 4, 192, 4, false>>(P, d_in, d_out, st);
+      if (P.contig) *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 1, 96, 8>>(P, d_in, d_out, st);
       else *rc = launch_fixed<FixedPlan<720,  4, 2, 2, 5, 3, 3, 8, 384, 2, false>>(P, d_in, d_out, st);
       return true;
-    case 1344: *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st); return true;
-    case 1440: *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st); return true;
-    // 2700: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each (54.6 -> 47.1 ms
-    // at config 5: the strided passes' DRAM over-fetch halves); at 1344 the same trade loses (5.0 -> 5.6 ms)
-    case 2700: *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 4, 512, 1>>(P, d_in, d_out, st); return true;
+    case 1344:
+      if (P.contig) *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 1, 96, 6>>(P, d_in, d_out, st);
+      else *rc = launch_fixed<FixedPlan<1344, 4, 4, 4, 3, 7, 1, 4, 256, 2>>(P, d_in, d_out, st);
+      return true;
+    case 1440:
+      if (P.contig) *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 1, 96, 6>>(P, d_in, d_out, st);
+      else *rc = launch_fixed<FixedPlan<1440, 4, 4, 2, 5, 3, 3, 4, 256, 2>>(P, d_in, d_out, st);
+      return true;
+    // 2700, strided: one 512-thread CTA per SM with 4 columns (64-byte segments) beats two CTAs with 2 columns each
+    // (54.6 -> 47.1 ms at config 5: the strided passes' DRAM over-fetch halves); at 1344 the same trade loses (5.0 -> 5.6 ms)
+    case 2700:
+      if (P.contig) *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 1, 192, 3>>(P, d_in, d_out, st);
+      else *rc = launch_fixed<FixedPlan<2700, 4, 3, 3, 5, 3, 5, 4, 512, 1>>(P, d_in, d_out, st);
+      return true;
   }
   return false;
 }
