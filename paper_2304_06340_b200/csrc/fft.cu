@@ -1023,7 +1023,7 @@ bool try_fixed(const FftPass& P, const void* d_in, double* d_out, cudaStream_t s
     // packed real rows) per tile in as many CTAs as fit; the strided passes need TB * 16-byte segments of the other axis.
     // 672 / 720: groups of at most 12 / 10 points fit 80 registers.
     case 672:
-      if (P.contig) *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 256, 3>>(P, d_in, d_out, st);
+      if (P.contig) *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 1, 96, 8>>(P, d_in, d_out, st);
       else *rc = launch_fixed<FixedPlan<672,  4, 2, 4, 3, 7, 1, 4, 192, 4>>(P, d_in, d_out, st);
       return true;
     case 720:
