@@ -36,8 +36,12 @@ constexpr int kSmemBytes = 200 * 1024;   // subgrid budget of a CTA that has the
 // every source of its CTA's item, so a second, independent CTA doubles the sources in flight.  Measured: spread
 // 0.93 -> 0.76 ms at w = 7 (config 3), 3.45 -> 3.06 ms at w = 10 (config 4), 17.1 -> 16.5 ms at w = 11 (config 5);
 // at w = 13 the 78-register budget spills and the gain is within the noise, so wider kernels keep one CTA.
+// Three CTAs (80 registers, bins of a third of the shared memory) at w <= 8: 0.416 -> 0.343 ms at w = 5, 0.505 -> 0.466 at
+// w = 6, 0.626 -> 0.596 at w = 7, 0.670 -> 0.641 at w = 8 (config 3's sources); four at w <= 6 lose again (0.373 / 0.483:
+// the bins shrink to 5 cells a side).  As in the FFT passes, CTAs in different phases fill the pipes, not warps.
 constexpr int kTwoCtaMaxW = 11;
-constexpr int ctas_per_sm(int w) { return w <= kTwoCtaMaxW ? 2 : 1; }
+constexpr int kThreeCtaMaxW = 8;
+constexpr int ctas_per_sm(int w) { return w <= kThreeCtaMaxW ? 3 : (w <= kTwoCtaMaxW ? 2 : 1); }
 
 // Sources of a chunk whose W x W products ky[cy] kz[cz] are tabulated at a time (kyz table, ~16 KB whatever W): every
 // one of the W warps that visit a source needs the same W^2 products -- computed once and read as ceil(W^2/32)
