@@ -398,11 +398,43 @@ __global__ void __launch_bounds__(PL::T, PL::CTAS) fft_fixed_kernel(const __grid
     constexpr int Lq1 = N / G1;
     bool nz = STRIDED;
     const double fhi = (MODE != 2 && P.dec_hi) ? P.dec_hi[hi] : 1.0;
+    // Strided passes, fp64 arrays: every thread first issues the loads of ALL its group-1 tasks as 16-byte asynchronous
+    // copies straight into the tile, each input at the position it has in the column (h at r, l at r + 3N/4) -- the task
+    // that reads them is the only one that writes positions congruent to jp modulo Lq1, so the tile is its own staging
+    // buffer and no barrier is needed, only the thread's own wait.  All loads of the tile are then in flight at once
+    // instead of one round of 2 B1 register loads per task with a DRAM round trip each.
+    constexpr bool ASYNC_IN = MODE == 2 && !F32;
+    if (ASYNC_IN) {
+      for (int idx = tid; idx < Lq1 * TB; idx += T) {
+        const int col = idx % TB, jp = idx / TB;
+        const bool live = col < ncol;
+        const int64_t src = hi * P.in_hi + lo0 + (live ? col : 0);
+        const double2* inb = static_cast<const double2*>(in_raw);
+        const int nbytes = live ? 16 : 0;   // src-size 0: zero fill
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          const int r = jp + q2 * Lq1;
+          const unsigned dh = (unsigned)__cvta_generic_to_shared(&a[at(r, 0, col)]);
+          const unsigned dl = (unsigned)__cvta_generic_to_shared(&a[at(r + 3 * (N / 4), 0, col)]);
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dh), "l"(inb + src + (int64_t)(r + N / 4) * P.in_el), "r"(nbytes) : "memory");
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dl), "l"(inb + src + (int64_t)r * P.in_el), "r"(nbytes) : "memory");
+        }
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
     for (int idx = tid; idx < Lq1 * TB; idx += T) {
       const int col = STRIDED ? idx % TB : idx / Lq1;
       const int jp = STRIDED ? idx / TB : idx % Lq1;
       double2 xl[B1], xh[B1];
-      if (MODE == 2) {
+      if (ASYNC_IN) {
+#pragma unroll
+        for (int q2 = 0; q2 < B1; ++q2) {
+          const int r = jp + q2 * Lq1;
+          xh[q2] = a[at(r, 0, col)];
+          xl[q2] = a[at(r + 3 * (N / 4), 0, col)];
+        }
+      } else if (MODE == 2) {
         const bool live = col < ncol;
         const int64_t src = hi * P.in_hi + lo0 + (live ? col : 0);
 #pragma unroll
