@@ -304,6 +304,14 @@ int sfd_last_stage_times(const char** names, float* ms, int max);
 /* Number of kernels of this library launched so far by the process. */
 long long sfd_launch_count(void);
 
+/* ---- environment switches (read at each call; for tests and A-B measurements, none changes a result beyond rounding) ----
+ *   SFD_NO_OVERLAP=1         type-3 transform: the target sort stays on the caller's stream (no second stream)
+ *   SFD_INTERP_NO_TMA=1      interpolation: subgrids staged by 16-byte asynchronous copies instead of TMA box copies
+ *   SFD_DIRECT_PACKED=1      direct sum on the ball rule: rotation table packed behind the stages instead of 32 KB-aligned
+ *   SFD_FFT_GENERIC=1        FFT passes: the generic kernel instead of the fixed-geometry ones
+ *   SFD_DEBUG_POISON_BAND=1  FFT passes' output buffers filled with NaN first (a cell that is read without having been
+ *                            stored then shows up as a NaN result) */
+
 #ifdef __cplusplus
 }
 #endif
