@@ -43,10 +43,14 @@ constexpr int kTwoCtaMaxW = 11;
 constexpr int kThreeCtaMaxW = 8;
 constexpr int ctas_per_sm(int w) { return w <= kThreeCtaMaxW ? 3 : (w <= kTwoCtaMaxW ? 2 : 1); }
 
-// Sources of a chunk whose W x W products ky[cy] kz[cz] are tabulated at a time (kyz table, ~16 KB whatever W): every
-// one of the W warps that visit a source needs the same W^2 products -- computed once and read as ceil(W^2/32)
-// contiguous LDS.64, instead of twice as many gathers from the ky and kz columns plus a DMUL per cell and visit.
-constexpr int kyz_sub(int W) { return W <= 8 ? 32 : (W <= 11 ? 16 : 8); }
+// Sources of a chunk whose W x W products ky[cy] kz[cz] are tabulated at a time: every one of the W warps that visit a
+// source needs the same W^2 products -- computed once and read as ceil(W^2/32) contiguous LDS.64, instead of twice as
+// many gathers from the ky and kz columns plus a DMUL per cell and visit.  The whole chunk of 32 where the shared memory
+// allows it (one CTA per SM above w = 11: 49 KB at w = 13; ~17 KB at w <= 8), half a chunk at w = 9 ... 11 (two CTAs per
+// SM: a whole chunk would shrink the bins too far).  Measured at config 3's sources, sub-chunks of 8 / 16 / 32 sources:
+// w = 12 2.00 / 1.87 / 1.80 ms, w = 13 2.56 / 2.41 / 2.31 ms, w = 14 3.01 / 2.87 / 2.77 ms (every sub-chunk costs two
+// barriers); w = 10 (config 4) 2.88 / 2.80 / 2.86 ms, w = 11 (config 5) 15.0 / 14.7 / 15.3 ms; w = 7 16 / 32: 0.613 / 0.594 ms.
+constexpr int kyz_sub(int W) { return (W <= 8 || W > 11) ? 32 : 16; }
 constexpr int kyz_pitch(int W) { return ((W * W + 31) / 32) * 32 + 1; }   // odd: lanes = consecutive sources write a column
 constexpr int kyz_bytes(int W) { return kyz_sub(W) * kyz_pitch(W) * 8; }
 
